@@ -1,0 +1,676 @@
+// sledge_oracle.cpp -- TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, obviously-correct fp64 CPU implementation of the sledgehamr hot path
+// (arXiv 2404.02950), written from the paper text.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may build, load or call this file.
+// It shares no code, header, table or helper with the CUDA library under
+// paper_2404_02950_b200/csrc/ and must never be linked into the product path.
+//
+// What it computes, and the passage each part follows (PAPER.md line / section):
+//   O1 grid        : block-structured levels, ratio 2, periodic domain          L23, L39-53 Eq.1-3
+//   O2 Laplacian   : utils::Laplacian<order>, order 1 -> 7-pt, 2 -> 13-pt       L207-212, L649 App.A
+//                    (coefficients are not printed; they are the unique maximal-order central
+//                    stencils on 3 / 5 points per axis -- pinned by polynomial exactness)
+//   O3 RHS         : Eq.10-11 with friction kappa, mass term a, coupling lambda  L178-181, L214-223
+//   O4 integrator  : classic RK4 (integrator.type = 4)                           L808 Table V
+//   O5 ghost fill  : periodic wrap, same-level copy, coarse->fine trilinear in
+//                    space + linear in time                                       L68-74
+//   O6 subcycling  : advance l, then l+1 twice, then synchronise                  L66-76, L88 Fig.2
+//   O7 average-down: coarse <- mean of 8 fine children                            L74, L88
+//   O8 string tags : plaquette winding number of (psi1,psi2) around 0; rule not printed in the
+//                    paper (L349-371 gives only the bool-per-cell hook) -> DESIGN.md reading R8
+//   diagnostics    : energies used only by the pins (L678 App.B; Gradient<order> L651-658)
+//
+// No blocking, fusion or reordering: every loop is the definition written out.  OpenMP pragmas on
+// outer box/z loops only change which core executes an iteration, never the arithmetic.
+// Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/oracle.py).
+//
+// Parity pins: tests/test_oracle_pins.py (every function here has at least one pin that is not
+// a restatement of its own formula).
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr int NCOMP = 4;  // psi1, psi2, pi1, pi2  (L189-190)
+constexpr int PSI1 = 0, PSI2 = 1, PI1 = 2, PI2 = 3;
+constexpr int FLAG_BLOCK = 32;  // box-flag reduction granularity (BASELINE.json config 3)
+
+struct Params {
+  int32_t n_levels;
+  int32_t n0[3];
+  int32_t nghost;
+  int32_t blocking_factor;
+  int32_t lap_order;
+  int32_t eta_fixed;
+  double h0;
+  double lambda;
+  double a_mass;
+  double friction;
+};
+
+struct BoxIn {
+  int32_t level;
+  int32_t lo[3];
+  int32_t hi[3];
+};
+
+// One box worth of data: NCOMP components, valid region n[0..2] plus g ghost layers.
+struct Field {
+  int n[3] = {0, 0, 0};
+  int g = 0;
+  int s[3] = {0, 0, 0};
+  std::vector<double> v;
+  void init(const int nn[3], int gg) {
+    g = gg;
+    for (int d = 0; d < 3; ++d) {
+      n[d] = nn[d];
+      s[d] = nn[d] + 2 * gg;
+    }
+    v.assign((size_t)NCOMP * s[0] * s[1] * s[2], 0.0);
+  }
+  // i,j,k relative to the box's low corner; ghosts are -g..-1 and n..n+g-1.
+  inline double& at(int c, int i, int j, int k) {
+    return v[(((size_t)c * s[2] + (k + g)) * s[1] + (j + g)) * s[0] + (i + g)];
+  }
+  inline double at(int c, int i, int j, int k) const {
+    return v[(((size_t)c * s[2] + (k + g)) * s[1] + (j + g)) * s[0] + (i + g)];
+  }
+};
+
+typedef std::vector<Field> LevelState;  // one Field per box of the level
+
+struct Level {
+  int n[3];                 // index space extent (n0 * 2^l)
+  double h;                 // Eq.1
+  std::vector<int> boxes;   // global box ids, in input order
+  std::vector<int> owner;   // coarsened (by blocking factor) index space -> local box index or -1
+  int no[3];
+  LevelState Y;             // current state; after this level's step it is the state at t_new
+  LevelState Yold;          // state at t_old, the start of this level's last step (L72)
+  double t_old = 0, t_new = 0;
+  bool have_pair = false;
+  LevelState K[4];          // RK4 slopes (k of the last orc_eval_rhs in K[0])
+  LevelState U;             // stage state
+};
+
+struct Oracle {
+  Params p;
+  std::vector<BoxIn> box;
+  std::vector<int> box_local;  // index of the box inside its level
+  std::vector<Level> lev;
+  std::string err;
+};
+
+inline int wrap(int i, int n) {
+  int r = i % n;
+  return r < 0 ? r + n : r;
+}
+inline int floordiv2(int i) { return (i >= 0) ? i / 2 : -((-i + 1) / 2); }
+
+// ---- O1: hierarchy ---------------------------------------------------------------------------
+
+int owner_of(const Oracle& o, int l, int i, int j, int k) {  // wrapped indices
+  const Level& L = o.lev[l];
+  int bf = o.p.blocking_factor;
+  return L.owner[((size_t)(k / bf) * L.no[1] + (j / bf)) * L.no[0] + (i / bf)];
+}
+
+bool build(Oracle& o, const BoxIn* b, int nbox) {
+  const Params& p = o.p;
+  char msg[256];
+  if (p.n_levels < 1 || p.n_levels > 8) { o.err = "n_levels out of range"; return false; }
+  int bf = p.blocking_factor;
+  if (bf < 1 || (bf & (bf - 1))) { o.err = "blocking_factor must be a power of 2 (L39)"; return false; }
+  if (p.nghost >= bf) { o.err = "nghost must be smaller than blocking_factor (L772)"; return false; }
+  if (p.lap_order < 1 || p.lap_order > 2) { o.err = "lap_order must be 1 or 2"; return false; }
+  if (p.lap_order > p.nghost) { o.err = "lap_order must be <= nghost (L240)"; return false; }
+  if (!(p.h0 > 0)) { o.err = "h0 must be positive"; return false; }
+  o.lev.resize(p.n_levels);
+  for (int l = 0; l < p.n_levels; ++l) {
+    Level& L = o.lev[l];
+    for (int d = 0; d < 3; ++d) {
+      L.n[d] = p.n0[d] << l;
+      if (p.n0[d] <= 0 || p.n0[d] % bf) { o.err = "n0 must be a positive multiple of blocking_factor"; return false; }
+      L.no[d] = L.n[d] / bf;
+    }
+    L.h = p.h0 / (double)(1 << l);  // Eq.1
+    L.owner.assign((size_t)L.no[0] * L.no[1] * L.no[2], -1);
+  }
+  o.box.assign(b, b + nbox);
+  o.box_local.resize(nbox);
+  for (int ib = 0; ib < nbox; ++ib) {
+    const BoxIn& B = b[ib];
+    if (B.level < 0 || B.level >= p.n_levels) { o.err = "box level out of range"; return false; }
+    Level& L = o.lev[B.level];
+    for (int d = 0; d < 3; ++d) {
+      int n = B.hi[d] - B.lo[d] + 1;
+      if (B.lo[d] < 0 || B.hi[d] >= L.n[d] || n <= 0 || B.lo[d] % bf || n % bf) {
+        snprintf(msg, sizeof msg, "box %d: not inside the domain / not aligned to the blocking factor (L39)", ib);
+        o.err = msg;
+        return false;
+      }
+    }
+    int li = (int)L.boxes.size();
+    for (int k = B.lo[2] / bf; k <= B.hi[2] / bf; ++k)
+      for (int j = B.lo[1] / bf; j <= B.hi[1] / bf; ++j)
+        for (int i = B.lo[0] / bf; i <= B.hi[0] / bf; ++i) {
+          int& ow = L.owner[((size_t)k * L.no[1] + j) * L.no[0] + i];
+          if (ow != -1) {
+            snprintf(msg, sizeof msg, "box %d overlaps another box of level %d", ib, B.level);
+            o.err = msg;
+            return false;
+          }
+          ow = li;
+        }
+    o.box_local[ib] = li;
+    L.boxes.push_back(ib);
+  }
+  for (size_t q = 0; q < o.lev[0].owner.size(); ++q)
+    if (o.lev[0].owner[q] < 0) { o.err = "level 0 must cover the whole domain (L39)"; return false; }
+  // Proper nesting (L70, L137): every fine box grown by one blocking factor of fine cells must lie
+  // on valid cells of the next coarser level.
+  for (int l = 1; l < p.n_levels; ++l) {
+    if (o.lev[l].boxes.empty()) { o.err = "empty refinement level"; return false; }
+    for (int ib : o.lev[l].boxes) {
+      const BoxIn& B = o.box[ib];
+      for (int k = B.lo[2] - bf; k <= B.hi[2] + bf; k += 1)
+        for (int j = B.lo[1] - bf; j <= B.hi[1] + bf; j += 1)
+          for (int i = B.lo[0] - bf; i <= B.hi[0] + bf; i += 1) {
+            int ci = wrap(floordiv2(i), o.lev[l - 1].n[0]);
+            int cj = wrap(floordiv2(j), o.lev[l - 1].n[1]);
+            int ck = wrap(floordiv2(k), o.lev[l - 1].n[2]);
+            if (owner_of(o, l - 1, ci, cj, ck) < 0) {
+              snprintf(msg, sizeof msg, "box %d violates proper nesting (gap < blocking factor, L70/L137)", ib);
+              o.err = msg;
+              return false;
+            }
+          }
+    }
+  }
+  for (int l = 0; l < p.n_levels; ++l) {
+    Level& L = o.lev[l];
+    auto alloc = [&](LevelState& S) {
+      S.resize(L.boxes.size());
+      for (size_t q = 0; q < L.boxes.size(); ++q) {
+        const BoxIn& B = o.box[L.boxes[q]];
+        int nn[3] = {B.hi[0] - B.lo[0] + 1, B.hi[1] - B.lo[1] + 1, B.hi[2] - B.lo[2] + 1};
+        S[q].init(nn, p.nghost);
+      }
+    };
+    alloc(L.Y); alloc(L.Yold); alloc(L.U);
+    for (int s = 0; s < 4; ++s) alloc(L.K[s]);
+  }
+  return true;
+}
+
+// value(l, state, comp, i,j,k): periodic wrap, find the owning box, return VALID data (O1).
+inline double value(const Oracle& o, int l, const LevelState& S, int c, int i, int j, int k, bool* ok) {
+  const Level& L = o.lev[l];
+  int wi = wrap(i, L.n[0]), wj = wrap(j, L.n[1]), wk = wrap(k, L.n[2]);
+  int ow = owner_of(o, l, wi, wj, wk);
+  if (ow < 0) { *ok = false; return 0.0; }
+  const BoxIn& B = o.box[L.boxes[ow]];
+  return S[ow].at(c, wi - B.lo[0], wj - B.lo[1], wk - B.lo[2]);
+}
+
+// ---- O5: ghost fill --------------------------------------------------------------------------
+// For each ghost cell of each box of level l in state S (which holds data of time `time`):
+//   same-level owner exists -> copy its valid value (periodic wrap included)         L23, L68
+//   else (l > 0)            -> trilinear interpolation of the time-interpolated
+//                              coarse state c = (1-alpha) old + alpha new             L70-72
+// Fine index f = 2c + r sits -1/4 (r=0) or +1/4 (r=1) coarse cell from the centre of c, hence per-axis
+// weights 3/4 on c and 1/4 on c-1 (r=0) or c+1 (r=1).
+bool fill_ghosts(Oracle& o, int l, LevelState& S, double time) {
+  Level& L = o.lev[l];
+  const int g = o.p.nghost;
+  double alpha = 0.0;
+  const LevelState* Cold = nullptr;
+  const LevelState* Cnew = nullptr;
+  if (l > 0) {
+    Level& C = o.lev[l - 1];
+    if (C.have_pair && C.t_new != C.t_old) {
+      alpha = (time - C.t_old) / (C.t_new - C.t_old);
+      Cold = &C.Yold;
+      Cnew = &C.Y;
+    } else {  // no step taken yet: the coarse level only has its current state
+      alpha = 0.0;
+      Cold = &C.Y;
+      Cnew = &C.Y;
+    }
+  }
+  bool all_ok = true;
+#pragma omp parallel for schedule(dynamic)
+  for (int q = 0; q < (int)L.boxes.size(); ++q) {
+    const BoxIn& B = o.box[L.boxes[q]];
+    Field& F = S[q];
+    bool ok = true;
+    for (int k = -g; k < F.n[2] + g; ++k)
+      for (int j = -g; j < F.n[1] + g; ++j)
+        for (int i = -g; i < F.n[0] + g; ++i) {
+          bool inside = (i >= 0 && i < F.n[0] && j >= 0 && j < F.n[1] && k >= 0 && k < F.n[2]);
+          if (inside) continue;
+          int gi = B.lo[0] + i, gj = B.lo[1] + j, gk = B.lo[2] + k;  // unwrapped level index
+          int wi = wrap(gi, L.n[0]), wj = wrap(gj, L.n[1]), wk = wrap(gk, L.n[2]);
+          int ow = owner_of(o, l, wi, wj, wk);
+          if (ow >= 0) {
+            const BoxIn& Bo = o.box[L.boxes[ow]];
+            for (int c = 0; c < NCOMP; ++c)
+              F.at(c, i, j, k) = S[ow].at(c, wi - Bo.lo[0], wj - Bo.lo[1], wk - Bo.lo[2]);
+            continue;
+          }
+          if (l == 0) { ok = false; continue; }
+          int f[3] = {gi, gj, gk};
+          int c0[3], c1[3];
+          for (int d = 0; d < 3; ++d) {
+            c0[d] = floordiv2(f[d]);
+            int r = f[d] - 2 * c0[d];
+            c1[d] = (r == 0) ? c0[d] - 1 : c0[d] + 1;
+          }
+          const double w[2] = {0.75, 0.25};
+          for (int c = 0; c < NCOMP; ++c) {
+            double sum = 0.0;
+            for (int dz = 0; dz < 2; ++dz)
+              for (int dy = 0; dy < 2; ++dy)
+                for (int dx = 0; dx < 2; ++dx) {
+                  int ci = dx ? c1[0] : c0[0], cj = dy ? c1[1] : c0[1], ck = dz ? c1[2] : c0[2];
+                  double vo = value(o, l - 1, *Cold, c, ci, cj, ck, &ok);
+                  double vn = value(o, l - 1, *Cnew, c, ci, cj, ck, &ok);
+                  double cv = (1.0 - alpha) * vo + alpha * vn;
+                  double wt = (w[dz] * w[dy]) * w[dx];
+                  sum += wt * cv;
+                }
+            F.at(c, i, j, k) = sum;
+          }
+        }
+    if (!ok) {
+#pragma omp critical
+      all_ok = false;
+    }
+  }
+  if (!all_ok) o.err = "ghost fill: a ghost cell has neither a same-level owner nor coarse data (nesting)";
+  return all_ok;
+}
+
+// ---- O2: Laplacian ---------------------------------------------------------------------------
+// order 1: sum_d [ (u(+e_d) - u) + (u(-e_d) - u) ] / h^2
+// order 2: sum_d [ 16 ((u(+e_d) - u) + (u(-e_d) - u)) - ((u(+2e_d) - u) + (u(-2e_d) - u)) ] / (12 h^2)
+// (neighbour-minus-centre form of [1,-2,1]/h^2 and [-1,16,-30,16,-1]/(12 h^2); it is exactly zero on
+// constants, which the scalar-ODE pin relies on.)
+inline double laplacian(const Field& F, int c, int i, int j, int k, int order, double h) {
+  const double u = F.at(c, i, j, k);
+  if (order == 1) {
+    double sx = (F.at(c, i + 1, j, k) - u) + (F.at(c, i - 1, j, k) - u);
+    double sy = (F.at(c, i, j + 1, k) - u) + (F.at(c, i, j - 1, k) - u);
+    double sz = (F.at(c, i, j, k + 1) - u) + (F.at(c, i, j, k - 1) - u);
+    return ((sx + sy) + sz) / (h * h);
+  }
+  double n1x = (F.at(c, i + 1, j, k) - u) + (F.at(c, i - 1, j, k) - u);
+  double n1y = (F.at(c, i, j + 1, k) - u) + (F.at(c, i, j - 1, k) - u);
+  double n1z = (F.at(c, i, j, k + 1) - u) + (F.at(c, i, j, k - 1) - u);
+  double n2x = (F.at(c, i + 2, j, k) - u) + (F.at(c, i - 2, j, k) - u);
+  double n2y = (F.at(c, i, j + 2, k) - u) + (F.at(c, i, j - 2, k) - u);
+  double n2z = (F.at(c, i, j, k + 2) - u) + (F.at(c, i, j, k - 2) - u);
+  double s1 = (n1x + n1y) + n1z;
+  double s2 = (n2x + n2y) + n2z;
+  return (16.0 * s1 - s2) / (12.0 * (h * h));
+}
+
+// ---- O3: right-hand side, Eq.10-11 ------------------------------------------------------------
+//   k_psi_c = Pi_c
+//   k_Pi_c  = -(kappa/eta) Pi_c + Lap(psi_c) - lambda eta^2 psi_c (psi1^2 + psi2^2 - 1) - a psi_c
+void eval_rhs(const Oracle& o, int l, const LevelState& S, LevelState& K, double eta) {
+  const Level& L = o.lev[l];
+  const Params& p = o.p;
+#pragma omp parallel for schedule(dynamic)
+  for (int q = 0; q < (int)L.boxes.size(); ++q) {
+    const Field& F = S[q];
+    Field& R = K[q];
+    for (int k = 0; k < F.n[2]; ++k)
+      for (int j = 0; j < F.n[1]; ++j)
+        for (int i = 0; i < F.n[0]; ++i) {
+          double psi1 = F.at(PSI1, i, j, k), psi2 = F.at(PSI2, i, j, k);
+          double pi1 = F.at(PI1, i, j, k), pi2 = F.at(PI2, i, j, k);
+          double lap1 = laplacian(F, PSI1, i, j, k, p.lap_order, L.h);
+          double lap2 = laplacian(F, PSI2, i, j, k, p.lap_order, L.h);
+          double pot = p.lambda * (eta * eta) * ((psi1 * psi1 + psi2 * psi2) - 1.0) + p.a_mass;
+          double fr = (p.friction != 0.0) ? p.friction / eta : 0.0;
+          R.at(PSI1, i, j, k) = pi1;
+          R.at(PSI2, i, j, k) = pi2;
+          R.at(PI1, i, j, k) = (lap1 - psi1 * pot) - fr * pi1;
+          R.at(PI2, i, j, k) = (lap2 - psi2 * pot) - fr * pi2;
+        }
+  }
+}
+
+// ---- O7: average-down -------------------------------------------------------------------------
+bool average_down(Oracle& o, int lf) {
+  if (lf < 1 || lf >= o.p.n_levels) { o.err = "average_down: bad fine level"; return false; }
+  Level& Lf = o.lev[lf];
+  Level& Lc = o.lev[lf - 1];
+  bool all_ok = true;
+  for (int q = 0; q < (int)Lf.boxes.size(); ++q) {
+    const BoxIn& B = o.box[Lf.boxes[q]];
+    const Field& F = Lf.Y[q];
+    for (int k = 0; k < F.n[2]; k += 2)
+      for (int j = 0; j < F.n[1]; j += 2)
+        for (int i = 0; i < F.n[0]; i += 2) {
+          int ci = (B.lo[0] + i) / 2, cj = (B.lo[1] + j) / 2, ck = (B.lo[2] + k) / 2;
+          int ow = owner_of(o, lf - 1, ci, cj, ck);
+          if (ow < 0) { all_ok = false; continue; }
+          const BoxIn& Bc = o.box[Lc.boxes[ow]];
+          for (int c = 0; c < NCOMP; ++c) {
+            double s = 0.0;
+            for (int rz = 0; rz < 2; ++rz)
+              for (int ry = 0; ry < 2; ++ry)
+                for (int rx = 0; rx < 2; ++rx) s += F.at(c, i + rx, j + ry, k + rz);
+            Lc.Y[ow].at(c, ci - Bc.lo[0], cj - Bc.lo[1], ck - Bc.lo[2]) = 0.125 * s;
+          }
+        }
+  }
+  if (!all_ok) o.err = "average_down: fine cell without a coarse parent";
+  return all_ok;
+}
+
+// ---- O4 + O6: classic RK4 with recursive time subcycling ---------------------------------------
+//   U_1 = Y;  k_s = f(U_s, eta_s), eta_s = t + c_s dt, c = (0, 1/2, 1/2, 1)
+//   U_{s+1} = Y + a_s dt k_s, a = (1/2, 1/2, 1);  Y_new = Y + dt/6 (k_1 + 2 k_2 + 2 k_3 + k_4)
+bool advance(Oracle& o, int l, double t, double dt, double eta_const) {
+  Level& L = o.lev[l];
+  static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
+  static const double as[3] = {0.5, 0.5, 1.0};
+  L.Yold = L.Y;
+  L.U = L.Y;
+  for (int s = 0; s < 4; ++s) {
+    double ts = t + cs[s] * dt;
+    if (!fill_ghosts(o, l, L.U, ts)) return false;
+    double eta_s = o.p.eta_fixed ? eta_const : ts;
+    eval_rhs(o, l, L.U, L.K[s], eta_s);
+    if (s < 3) {
+      double adt = as[s] * dt;
+#pragma omp parallel for schedule(dynamic)
+      for (int q = 0; q < (int)L.boxes.size(); ++q) {
+        Field& U = L.U[q];
+        const Field& Y = L.Y[q];
+        const Field& K = L.K[s][q];
+        for (int c = 0; c < NCOMP; ++c)
+          for (int k = 0; k < U.n[2]; ++k)
+            for (int j = 0; j < U.n[1]; ++j)
+              for (int i = 0; i < U.n[0]; ++i) U.at(c, i, j, k) = Y.at(c, i, j, k) + adt * K.at(c, i, j, k);
+      }
+    }
+  }
+#pragma omp parallel for schedule(dynamic)
+  for (int q = 0; q < (int)L.boxes.size(); ++q) {
+    Field& Y = L.Y[q];
+    for (int c = 0; c < NCOMP; ++c)
+      for (int k = 0; k < Y.n[2]; ++k)
+        for (int j = 0; j < Y.n[1]; ++j)
+          for (int i = 0; i < Y.n[0]; ++i) {
+            double k1 = L.K[0][q].at(c, i, j, k), k2 = L.K[1][q].at(c, i, j, k);
+            double k3 = L.K[2][q].at(c, i, j, k), k4 = L.K[3][q].at(c, i, j, k);
+            Y.at(c, i, j, k) = Y.at(c, i, j, k) + (dt / 6.0) * (((k1 + 2.0 * k2) + 2.0 * k3) + k4);
+          }
+  }
+  L.t_old = t;
+  L.t_new = t + dt;
+  L.have_pair = true;
+  if (l + 1 < o.p.n_levels) {
+    if (!advance(o, l + 1, t, 0.5 * dt, eta_const)) return false;
+    if (!advance(o, l + 1, t + 0.5 * dt, 0.5 * dt, eta_const)) return false;
+    if (!average_down(o, l + 1)) return false;  // the synchronised state is this level's state at t_new
+  }
+  return true;
+}
+
+// ---- O8: string tags ---------------------------------------------------------------------------
+// Winding number of the polygon psi(A)->psi(B)->psi(C)->psi(D)->psi(A) around the origin, counted by
+// signed crossings of the positive psi1 axis.  Edge a->b: up = a2<0 && b2>=0, dn = a2>=0 && b2<0,
+// cr = a1*b2 - a2*b1 (two products and one subtraction, each rounded; no FMA);
+// +1 if up && cr>0, -1 if dn && cr<0.
+inline int edge_crossing(double a1, double a2, double b1, double b2) {
+  bool up = (a2 < 0.0) && (b2 >= 0.0);
+  bool dn = (a2 >= 0.0) && (b2 < 0.0);
+  double p = a1 * b2;
+  double q = a2 * b1;
+  double cr = p - q;
+  if (up && cr > 0.0) return 1;
+  if (dn && cr < 0.0) return -1;
+  return 0;
+}
+inline int plaquette_winding(const double A[2], const double B[2], const double C[2], const double D[2]) {
+  return edge_crossing(A[0], A[1], B[0], B[1]) + edge_crossing(B[0], B[1], C[0], C[1]) +
+         edge_crossing(C[0], C[1], D[0], D[1]) + edge_crossing(D[0], D[1], A[0], A[1]);
+}
+
+// tags: one byte per valid cell, boxes of the level concatenated in box order, x fastest.
+// counts: dense array over aligned FLAG_BLOCK^3 blocks of the level index space, x fastest.
+bool tag_strings(Oracle& o, int l, uint8_t* tags, uint32_t* counts) {
+  Level& L = o.lev[l];
+  // after a coarse step all levels sit at the parent's t_new (alpha = 1: no temporal interpolation, L74)
+  double tcur = (l > 0 && o.lev[l - 1].have_pair) ? o.lev[l - 1].t_new : 0.0;
+  if (!fill_ghosts(o, l, L.Y, tcur)) return false;
+  int nb[3];
+  for (int d = 0; d < 3; ++d) nb[d] = (L.n[d] + FLAG_BLOCK - 1) / FLAG_BLOCK;
+  if (counts) memset(counts, 0, sizeof(uint32_t) * (size_t)nb[0] * nb[1] * nb[2]);
+  size_t off = 0;
+  static const int D1[3] = {0, 1, 2};  // (x,y), (y,z), (z,x)
+  static const int D2[3] = {1, 2, 0};
+  for (int q = 0; q < (int)L.boxes.size(); ++q) {
+    const BoxIn& B = o.box[L.boxes[q]];
+    const Field& F = L.Y[q];
+    for (int k = 0; k < F.n[2]; ++k)
+      for (int j = 0; j < F.n[1]; ++j)
+        for (int i = 0; i < F.n[0]; ++i) {
+          uint8_t tag = 0;
+          for (int pl = 0; pl < 3; ++pl) {
+            int e1[3] = {0, 0, 0}, e2[3] = {0, 0, 0};
+            e1[D1[pl]] = 1;
+            e2[D2[pl]] = 1;
+            double A[2] = {F.at(PSI1, i, j, k), F.at(PSI2, i, j, k)};
+            double Bv[2] = {F.at(PSI1, i + e1[0], j + e1[1], k + e1[2]), F.at(PSI2, i + e1[0], j + e1[1], k + e1[2])};
+            double C[2] = {F.at(PSI1, i + e1[0] + e2[0], j + e1[1] + e2[1], k + e1[2] + e2[2]),
+                           F.at(PSI2, i + e1[0] + e2[0], j + e1[1] + e2[1], k + e1[2] + e2[2])};
+            double Dv[2] = {F.at(PSI1, i + e2[0], j + e2[1], k + e2[2]), F.at(PSI2, i + e2[0], j + e2[1], k + e2[2])};
+            int W = plaquette_winding(A, Bv, C, Dv);
+            if (W != 0) tag |= (uint8_t)(1u << pl);
+          }
+          if (tags) tags[off] = tag;
+          ++off;
+          if (tag && counts) {
+            int bi = (B.lo[0] + i) / FLAG_BLOCK, bj = (B.lo[1] + j) / FLAG_BLOCK, bk = (B.lo[2] + k) / FLAG_BLOCK;
+            counts[((size_t)bk * nb[1] + bj) * nb[0] + bi] += 1;
+          }
+        }
+  }
+  return true;
+}
+
+// ---- diagnostics used by the pins (single-level, level 0) ---------------------------------------
+// Gradient<order> (L651-658): 3-point [ -1, 0, 1 ]/(2h), 5-point [1,-8,0,8,-1]/(12h).
+inline double gradient(const Field& F, int c, int i, int j, int k, int d, int order, double h) {
+  int e[3] = {0, 0, 0};
+  e[d] = 1;
+  auto u = [&](int m) { return F.at(c, i + m * e[0], j + m * e[1], k + m * e[2]); };
+  if (order == 1) return (u(1) - u(-1)) / (2.0 * h);
+  return (8.0 * (u(1) - u(-1)) - (u(2) - u(-2))) / (12.0 * h);
+}
+
+}  // namespace
+
+// =================================================================================================
+// C interface for ctypes (tests / smoke / cpu_baseline only)
+// =================================================================================================
+extern "C" {
+
+typedef struct {
+  int32_t n_levels;
+  int32_t n0[3];
+  int32_t nghost;
+  int32_t blocking_factor;
+  int32_t lap_order;
+  int32_t eta_fixed;
+  double h0, lambda, a_mass, friction;
+} orc_params;
+
+typedef struct {
+  int32_t level;
+  int32_t lo[3];
+  int32_t hi[3];
+} orc_box;
+
+static std::string g_err;
+
+const char* orc_last_error(void* h) {
+  if (h) return ((Oracle*)h)->err.c_str();
+  return g_err.c_str();
+}
+
+void* orc_create(const orc_params* p, const orc_box* b, int nbox) {
+  Oracle* o = new Oracle();
+  static_assert(sizeof(orc_params) == sizeof(Params), "layout");
+  static_assert(sizeof(orc_box) == sizeof(BoxIn), "layout");
+  memcpy(&o->p, p, sizeof(Params));
+  if (!build(*o, (const BoxIn*)b, nbox)) {
+    g_err = o->err;
+    delete o;
+    return nullptr;
+  }
+  return o;
+}
+
+void orc_destroy(void* h) { delete (Oracle*)h; }
+
+int orc_num_boxes(void* h, int level) { return (int)((Oracle*)h)->lev[level].boxes.size(); }
+
+// src/dst: dense valid region of global box `ib`, x fastest.
+int orc_set_state(void* h, int ib, int comp, const double* src) {
+  Oracle& o = *(Oracle*)h;
+  if (ib < 0 || ib >= (int)o.box.size() || comp < 0 || comp >= NCOMP) return -1;
+  Field& F = o.lev[o.box[ib].level].Y[o.box_local[ib]];
+  size_t q = 0;
+  for (int k = 0; k < F.n[2]; ++k)
+    for (int j = 0; j < F.n[1]; ++j)
+      for (int i = 0; i < F.n[0]; ++i) F.at(comp, i, j, k) = src[q++];
+  return 0;
+}
+int orc_get_state(void* h, int ib, int comp, double* dst) {
+  Oracle& o = *(Oracle*)h;
+  if (ib < 0 || ib >= (int)o.box.size() || comp < 0 || comp >= NCOMP) return -1;
+  const Field& F = o.lev[o.box[ib].level].Y[o.box_local[ib]];
+  size_t q = 0;
+  for (int k = 0; k < F.n[2]; ++k)
+    for (int j = 0; j < F.n[1]; ++j)
+      for (int i = 0; i < F.n[0]; ++i) dst[q++] = F.at(comp, i, j, k);
+  return 0;
+}
+// raw access including ghosts (array extent n+2g per axis, x fastest); which: 0 = Y, 1 = last k (K[0])
+int orc_set_raw(void* h, int ib, int comp, const double* src) {
+  Oracle& o = *(Oracle*)h;
+  Field& F = o.lev[o.box[ib].level].Y[o.box_local[ib]];
+  size_t q = 0;
+  for (int k = -F.g; k < F.n[2] + F.g; ++k)
+    for (int j = -F.g; j < F.n[1] + F.g; ++j)
+      for (int i = -F.g; i < F.n[0] + F.g; ++i) F.at(comp, i, j, k) = src[q++];
+  return 0;
+}
+int orc_get_raw(void* h, int ib, int comp, int which, double* dst) {
+  Oracle& o = *(Oracle*)h;
+  Level& L = o.lev[o.box[ib].level];
+  const Field& F = (which == 0) ? L.Y[o.box_local[ib]] : L.K[0][o.box_local[ib]];
+  size_t q = 0;
+  for (int k = -F.g; k < F.n[2] + F.g; ++k)
+    for (int j = -F.g; j < F.n[1] + F.g; ++j)
+      for (int i = -F.g; i < F.n[0] + F.g; ++i) dst[q++] = F.at(comp, i, j, k);
+  return 0;
+}
+
+int orc_fill_ghosts(void* h, int level, double time) {
+  Oracle& o = *(Oracle*)h;
+  if (level < 0 || level >= o.p.n_levels) return -1;
+  return fill_ghosts(o, level, o.lev[level].Y, time) ? 0 : -1;
+}
+
+// k = f(Y, eta) into K[0] of the level, using whatever the ghosts of Y currently hold
+// (do_fill = 1 fills them first at time eta).
+int orc_eval_rhs(void* h, int level, double eta, int do_fill) {
+  Oracle& o = *(Oracle*)h;
+  if (level < 0 || level >= o.p.n_levels) return -1;
+  Level& L = o.lev[level];
+  if (do_fill && !fill_ghosts(o, level, L.Y, eta)) return -1;
+  eval_rhs(o, level, L.Y, L.K[0], eta);
+  return 0;
+}
+
+// One coarse step of the whole hierarchy from time eta to eta + dt (O6).
+int orc_rk_step(void* h, double dt, double eta) {
+  Oracle& o = *(Oracle*)h;
+  return advance(o, 0, eta, dt, eta) ? 0 : -1;
+}
+
+int orc_average_down(void* h, int fine_level) { return average_down(*(Oracle*)h, fine_level) ? 0 : -1; }
+
+int orc_tag_strings(void* h, int level, uint8_t* tags, uint32_t* counts) {
+  Oracle& o = *(Oracle*)h;
+  if (level < 0 || level >= o.p.n_levels) return -1;
+  return tag_strings(o, level, tags, counts) ? 0 : -1;
+}
+
+// winding number of one plaquette given its four corner values (for brute-force pins)
+int orc_plaquette_winding(const double* A, const double* B, const double* C, const double* D) {
+  return plaquette_winding(A, B, C, D);
+}
+
+// Level-0 energies, summed over valid cells times h^3.  Ghosts of Y are filled first.
+//  out[0] = sum 1/2 (Pi1^2 + Pi2^2)
+//  out[1] = sum -1/2 (psi1 Lap psi1 + psi2 Lap psi2)          (conserved discrete gradient energy)
+//  out[2] = sum lambda eta^2 / 4 (psi1^2 + psi2^2 - 1)^2 + a/2 (psi1^2+psi2^2)
+//  out[3] = sum 1/2 |Gradient<order> psi|^2                    (paper's E of App.B)
+int orc_energy(void* h, double eta, double* out) {
+  Oracle& o = *(Oracle*)h;
+  Level& L = o.lev[0];
+  if (!fill_ghosts(o, 0, L.Y, eta)) return -1;
+  double e[4] = {0, 0, 0, 0};
+  double h3 = L.h * L.h * L.h;
+  for (size_t q = 0; q < L.boxes.size(); ++q) {
+    const Field& F = L.Y[q];
+    for (int k = 0; k < F.n[2]; ++k)
+      for (int j = 0; j < F.n[1]; ++j)
+        for (int i = 0; i < F.n[0]; ++i) {
+          double p1 = F.at(PSI1, i, j, k), p2 = F.at(PSI2, i, j, k);
+          double q1 = F.at(PI1, i, j, k), q2 = F.at(PI2, i, j, k);
+          e[0] += 0.5 * (q1 * q1 + q2 * q2);
+          e[1] += -0.5 * (p1 * laplacian(F, PSI1, i, j, k, o.p.lap_order, L.h) +
+                          p2 * laplacian(F, PSI2, i, j, k, o.p.lap_order, L.h));
+          double m = p1 * p1 + p2 * p2;
+          e[2] += 0.25 * o.p.lambda * eta * eta * (m - 1.0) * (m - 1.0) + 0.5 * o.p.a_mass * m;
+          double gsum = 0.0;
+          for (int c = 0; c < 2; ++c)
+            for (int d = 0; d < 3; ++d) {
+              double gd = gradient(F, c, i, j, k, d, o.p.lap_order, L.h);
+              gsum += gd * gd;
+            }
+          e[3] += 0.5 * gsum;
+        }
+  }
+  for (int m = 0; m < 4; ++m) out[m] = e[m] * h3;
+  return 0;
+}
+
+int orc_omp_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"

@@ -1,0 +1,688 @@
+"""Pins for the CPU oracle: every check here compares oracle/sledge_oracle.cpp with something OTHER than
+itself -- closed forms, textbook routines, invariants, brute force, or values printed in the paper
+(tests/golden/).  CPU only.  SURVEY.md section 8(c) "What pins each part"; DESIGN.md "Oracle pins"."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle.oracle import Oracle, OracleError, plaquette_winding
+from paper_2404_02950_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def single(n, **kw):
+    return Oracle(n, **kw)
+
+
+def coords(shape):
+    z, y, x = np.meshgrid(*[np.arange(s, dtype=np.float64) for s in shape], indexing="ij")
+    return x, y, z
+
+
+# ------------------------------------------------------------------------------------------------
+# O2 Laplacian
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.mark.parametrize("order,deg", [(1, 2), (1, 3), (2, 4), (2, 5)])
+def test_laplacian_exact_on_polynomials(order, deg):
+    """Central 3-point (5-point) second differences are exact on cubics (quintics) per axis.  Ghosts are
+    filled analytically on a NON-periodic box, so a wrong coefficient, sign or axis shows up directly."""
+    g = 2
+    n = (8, 16, 24)  # x, y, z -- all different to catch a transposed index
+    h = 0.37
+    o = Oracle(n, nghost=g, blocking_factor=8, lap_order=order, h0=h, lam=0.0)
+    zz, yy, xx = np.meshgrid(*[(np.arange(-g, s + g) + 0.5) * h for s in n[::-1]], indexing="ij")
+    rng = np.random.default_rng(7)
+    cx, cy, cz = rng.uniform(-1, 1, size=(3, deg + 1))
+
+    def poly(c, t):
+        return sum(c[m] * t ** m for m in range(deg + 1))
+
+    def d2poly(c, t):
+        return sum(m * (m - 1) * c[m] * t ** (m - 2) for m in range(2, deg + 1))
+
+    # separable sum + a cross term that every axis-wise second difference treats exactly
+    u1 = poly(cx, xx) + poly(cy, yy) + poly(cz, zz) + 0.3 * xx * yy * zz
+    lap1 = d2poly(cx, xx) + d2poly(cy, yy) + d2poly(cz, zz)
+    u2 = 2.0 * poly(cz, xx) - poly(cx, yy) + 0.5 * poly(cy, zz)
+    lap2 = 2.0 * d2poly(cz, xx) - d2poly(cx, yy) + 0.5 * d2poly(cy, zz)
+    o.set_raw(0, 0, u1)
+    o.set_raw(0, 1, u2)
+    k = o.eval_rhs(0, eta=1.0, fill=False)[0]
+    v = slice(g, -g)
+    scale = np.abs(u1).max() / h ** 2
+    assert np.abs(k[2] - lap1[v, v, v]).max() < 1e-12 * scale
+    assert np.abs(k[3] - lap2[v, v, v]).max() < 1e-12 * scale
+    # k_psi = Pi (Eq.10): Pi was zero
+    assert np.all(k[0] == 0) and np.all(k[1] == 0)
+
+
+def test_laplacian_order1_not_exact_on_quartic():
+    """Sanity of the pin above: the 3-point stencil must NOT be exact on x^4 (error h^2/12 * 24)."""
+    g, n, h = 1, (8, 8, 8), 0.5
+    o = Oracle(n, nghost=g, lap_order=1, h0=h, lam=0.0)
+    zz, yy, xx = np.meshgrid(*[(np.arange(-g, s + g) + 0.5) * h for s in n], indexing="ij")
+    o.set_raw(0, 0, xx ** 4)
+    k = o.eval_rhs(0, 1.0, fill=False)[0]
+    err = k[2] - 12 * xx[1:-1, 1:-1, 1:-1] ** 2
+    assert np.allclose(err, 2 * h ** 2, rtol=1e-9)
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_laplacian_symbol_on_plane_waves(order):
+    """exp(i k.x) is an eigenvector of the periodic discrete Laplacian with eigenvalue
+    -(1/h^2) sum_i 4 sin^2(k_i h/2)                               (order 1)
+    -(1/h^2) sum_i [16/3 sin^2(k_i h/2) - 1/3 sin^2(k_i h)]       (order 2)."""
+    n = (16, 24, 32)
+    h = 0.8
+    o = Oracle(n, nghost=2, lap_order=order, h0=h, lam=0.0)
+    x, y, z = coords(n[::-1])
+    m = (3, 2, 5)  # mode numbers per axis
+    kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
+    ph = kh[0] * x + kh[1] * y + kh[2] * z
+    o.set_state(0, 0, np.cos(ph))
+    o.set_state(0, 1, np.sin(ph))
+    k = o.eval_rhs(0, 1.0)[0]
+    if order == 1:
+        ev = -sum(4 * math.sin(a / 2) ** 2 for a in kh) / h ** 2
+    else:
+        ev = -sum(16 / 3 * math.sin(a / 2) ** 2 - 1 / 3 * math.sin(a) ** 2 for a in kh) / h ** 2
+    assert np.abs(k[2] - ev * np.cos(ph)).max() < 1e-12 * abs(ev)
+    assert np.abs(k[3] - ev * np.sin(ph)).max() < 1e-12 * abs(ev)
+
+
+# ------------------------------------------------------------------------------------------------
+# O3 + O4: potential, friction, eta handling and the RK4 tableau against a textbook scalar ODE solve
+# ------------------------------------------------------------------------------------------------
+
+
+def scalar_rk4(y, eta, dt, lam, a, kappa, eta_fixed=None):
+    """Textbook RK4 for the 4-variable ODE obtained from Eq.10-11 with a spatially constant field."""
+
+    def f(y, e):
+        e = eta_fixed if eta_fixed is not None else e
+        p1, p2, q1, q2 = y
+        pot = lam * e * e * (p1 * p1 + p2 * p2 - 1.0) + a
+        fr = kappa / e if kappa != 0 else 0.0
+        return np.array([q1, q2, -p1 * pot - fr * q1, -p2 * pot - fr * q2])
+
+    k1 = f(y, eta)
+    k2 = f(y + 0.5 * dt * k1, eta + 0.5 * dt)
+    k3 = f(y + 0.5 * dt * k2, eta + 0.5 * dt)
+    k4 = f(y + dt * k3, eta + dt)
+    return y + dt / 6.0 * (k1 + 2 * k2 + 2 * k3 + k4)
+
+
+@pytest.mark.parametrize("order", [1, 2])
+@pytest.mark.parametrize("eta_fixed", [False, True])
+def test_constant_field_equals_scalar_ode(order, eta_fixed):
+    n = 8
+    lam, a, kappa = 1.3, 0.56233, 2.0  # a: the listing's constant (L214), kappa = 2: Eq.11
+    o = Oracle(n, nghost=2, lap_order=order, h0=0.7, lam=lam, a_mass=a, friction=kappa, eta_fixed=eta_fixed)
+    y = np.array([0.3, -0.8, 0.1, 0.25])
+    for c in range(4):
+        o.set_state(0, c, np.full((n, n, n), y[c]))
+    eta, dt = 1.5, 0.05
+    for _ in range(20):
+        o.rk_step(dt, eta)
+        y = scalar_rk4(y, eta, dt, lam, a, kappa, eta_fixed=eta if eta_fixed else None)
+        eta += dt
+    for c in range(4):
+        got = o.get_state(0, c)
+        assert np.all(got == got.flat[0]), "a constant field must stay constant (difference-form stencil)"
+        assert abs(got.flat[0] - y[c]) <= 64 * np.finfo(float).eps * max(1.0, abs(y[c]))
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_linear_plane_wave_matches_rk4_amplification_matrix(order):
+    """lambda = 0: a lattice plane wave evolves by R(dt A)^n exactly, A = [[0,1],[-w^2,0]],
+    R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24, w^2 = lattice symbol (BASELINE.json 'discrete-dispersion plane
+    wave' for the 2nd-order stencil; the 13-point symbol for order 2)."""
+    n = (16, 8, 24)
+    h = 0.5
+    o = Oracle(n, nghost=2, lap_order=order, h0=h, lam=0.0)
+    x, y, z = coords(n[::-1])
+    m = (1, 2, 3)
+    kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
+    ph = kh[0] * x + kh[1] * y + kh[2] * z
+    if order == 1:
+        w2 = sum(4 * math.sin(a / 2) ** 2 for a in kh) / h ** 2
+    else:
+        w2 = sum(16 / 3 * math.sin(a / 2) ** 2 - 1 / 3 * math.sin(a) ** 2 for a in kh) / h ** 2
+    A0, B0 = 0.7, -0.4  # psi1 = A cos, Pi1 = B cos ; psi2 = 2A sin, Pi2 = -B sin
+    o.set_state(0, 0, A0 * np.cos(ph))
+    o.set_state(0, 2, B0 * np.cos(ph))
+    o.set_state(0, 1, 2 * A0 * np.sin(ph))
+    o.set_state(0, 3, -B0 * np.sin(ph))
+    dt, steps = 0.2 * h, 25
+    Z = dt * np.array([[0.0, 1.0], [-w2, 0.0]])
+    R = np.eye(2) + Z + Z @ Z / 2 + Z @ Z @ Z / 6 + Z @ Z @ Z @ Z / 24
+    Rn = np.linalg.matrix_power(R, steps)
+    eta = 3.0
+    for _ in range(steps):
+        o.rk_step(dt, eta)
+        eta += dt
+    a1, b1 = Rn @ np.array([A0, B0])
+    a2, b2 = Rn @ np.array([2 * A0, -B0])
+    assert np.abs(o.get_state(0, 0) - a1 * np.cos(ph)).max() < 1e-13
+    assert np.abs(o.get_state(0, 2) - b1 * np.cos(ph)).max() < 1e-12
+    assert np.abs(o.get_state(0, 1) - a2 * np.sin(ph)).max() < 1e-13
+    assert np.abs(o.get_state(0, 3) - b2 * np.sin(ph)).max() < 1e-12
+
+
+def test_energy_conservation_minkowski_is_fourth_order():
+    """Constant-eta variant: E = sum[1/2 Pi^2 - 1/2 psi.L psi + lambda eta^2/4 (|psi|^2-1)^2] h^3 is conserved
+    by the semi-discrete system; RK4 drifts as O(dt^4): halving dt must cut the drift by >= 14."""
+    n, h, eta = 16, 1.0, 1.2
+    psi1 = inputs.grf(n, 0.5, 11).numpy()
+    psi2 = inputs.grf(n, 0.5, 12).numpy()
+
+    def drift(dt, steps):
+        o = Oracle(n, nghost=1, lap_order=1, h0=h, lam=1.0, eta_fixed=True)
+        o.set_state(0, 0, 0.6 * psi1)
+        o.set_state(0, 1, 0.6 * psi2)
+        e0 = o.energy(eta)[:3].sum()
+        for _ in range(steps):
+            o.rk_step(dt, eta)
+        return abs(o.energy(eta)[:3].sum() - e0) / abs(e0)
+
+    d1 = drift(0.2, 20)
+    d2 = drift(0.1, 40)
+    assert d1 < 1e-3
+    assert d1 / d2 > 14.0, (d1, d2)
+
+
+# ------------------------------------------------------------------------------------------------
+# Paper Appendix B (golden fixture): plane wave, 13-point Laplacian, RK4, dt = 0.32 dx
+# ------------------------------------------------------------------------------------------------
+
+
+def read_golden(name):
+    out = {}
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].strip()
+        if line:
+            k, v = line.split("=")
+            out[k.strip()] = float(v)
+    return out
+
+
+def plane_wave_energy_error(N, gold, periods):
+    L = gold["L_over_sqrt5"] * math.sqrt(5.0)
+    h = L / N
+    m = (gold["wavelengths_x"], gold["wavelengths_y"], -gold["wavelengths_z"])  # reading G6: k = pi(8,5,-6)/(5 sqrt5)
+    kvec = [2 * math.pi * mm / L for mm in m]
+    omega = gold["omega_over_pi"] * math.pi
+    o = Oracle(N, nghost=2, lap_order=int(gold["laplacian_order"]), h0=h, lam=0.0)
+    x, y, z = coords((N, N, N))
+    ph = kvec[0] * (x + 0.5) * h + kvec[1] * (y + 0.5) * h + kvec[2] * (z + 0.5) * h
+    o.set_state(0, 0, gold["A"] * np.cos(ph))  # u(x,0)
+    o.set_state(0, 2, -gold["A"] * omega * np.sin(ph))  # du/dt(x,0), Eq.B2
+    t_end = periods * 2 * math.pi / omega
+    dt0 = gold["cfl"] * h
+    steps = int(math.ceil(t_end / dt0 - 1e-9))
+    dt = t_end / steps
+    t = 0.0
+    for _ in range(steps):
+        o.rk_step(dt, t + 1.0)  # eta is irrelevant for lambda = 0, friction = 0
+        t += dt
+    e = o.energy(1.0)
+    E = (e[0] + e[3]) / L ** 3  # mean of u_t^2/2 + (grad u)^2/2, L678
+    return E - gold["E_exact_over_pi2"] * math.pi ** 2, kvec
+
+
+def test_appendix_b_wavevector_reading():
+    """Reading G6: |k| must equal omega/c = pi for Eq.B2 to solve Eq.B1; the printed L = 10 sqrt5 then holds
+    exactly 8, 5, 6 wavelengths."""
+    g = read_golden("appendix_b_plane_wave.txt")
+    th = math.atan(g["tan_theta"])
+    phi = math.asin(g["sin_phi"])
+    k = math.pi * np.array([math.cos(th) * math.cos(phi), math.sin(th), -math.cos(th) * math.sin(phi)])
+    assert abs(np.linalg.norm(k) - math.pi) < 1e-14
+    L = g["L_over_sqrt5"] * math.sqrt(5)
+    waves = np.abs(k) * L / (2 * math.pi)
+    assert np.allclose(waves, [g["wavelengths_x"], g["wavelengths_y"], g["wavelengths_z"]], atol=1e-12)
+
+
+def test_appendix_b_energy_converges_at_fourth_order():
+    """Delta E -> 0 as a power law in N with index 'roughly -p or better' (paper fit for RK4: -4.7)."""
+    g = read_golden("appendix_b_plane_wave.txt")
+    periods = 10  # the paper runs 100 periods; the index does not depend on it, the CPU time does
+    d32, _ = plane_wave_energy_error(32, g, periods)
+    d64, _ = plane_wave_energy_error(64, g, periods)
+    idx = math.log(abs(d64) / abs(d32)) / math.log(2.0)
+    assert abs(d32) < 0.3 * math.pi ** 2 / 2  # converged regime (the paper excludes Delta E ~ O(1))
+    assert -6.5 < idx < -3.7, idx
+    assert abs(idx - g["rk4_power_law_index"]) < 1.5
+
+
+# ------------------------------------------------------------------------------------------------
+# O1/O5: periodic fill and same-level copies
+# ------------------------------------------------------------------------------------------------
+
+
+def run_single(n, boxes, psi, pi, steps, dt, eta0, **kw):
+    o = Oracle(n, boxes=boxes, **kw)
+    for ib, (l, lo, hi) in enumerate(o.boxes):
+        sl = (slice(lo[2], hi[2] + 1), slice(lo[1], hi[1] + 1), slice(lo[0], hi[0] + 1))
+        o.set_state(ib, 0, psi[0][sl])
+        o.set_state(ib, 1, psi[1][sl])
+        o.set_state(ib, 2, pi[0][sl])
+        o.set_state(ib, 3, pi[1][sl])
+    eta = eta0
+    for _ in range(steps):
+        o.rk_step(dt, eta)
+        eta += dt
+    out = np.zeros((4,) + psi[0].shape)
+    for ib, (l, lo, hi) in enumerate(o.boxes):
+        sl = (slice(lo[2], hi[2] + 1), slice(lo[1], hi[1] + 1), slice(lo[0], hi[0] + 1))
+        for c in range(4):
+            out[c][sl] = o.get_state(ib, c)
+    return out
+
+
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (2, 3)])
+def test_translation_invariance_bit_for_bit(order, g):
+    n = 16
+    psi = [inputs.grf(n, 0.5, s).numpy() for s in (21, 22)]
+    pi = [0.1 * inputs.grf(n, 0.5, s).numpy() for s in (23, 24)]
+    kw = dict(nghost=g, lap_order=order, h0=1.0, lam=1.0)
+    a = run_single(n, None, psi, pi, 3, 0.2, 1.0, **kw)
+    sh = (5, -3, 9)  # z, y, x
+    psi_s = [np.roll(p, sh, axis=(0, 1, 2)) for p in psi]
+    pi_s = [np.roll(p, sh, axis=(0, 1, 2)) for p in pi]
+    b = run_single(n, None, psi_s, pi_s, 3, 0.2, 1.0, **kw)
+    assert np.array_equal(np.roll(a, sh, axis=(1, 2, 3)), b)
+
+
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 3)])
+def test_multibox_level_equals_single_box_bit_for_bit(order, g):
+    """Same-level ghost copies (incl. edges/corners across the periodic seam) must make a tiled level 0
+    indistinguishable from one big box."""
+    n = 16
+    psi = [inputs.grf(n, 0.5, s).numpy() for s in (31, 32)]
+    pi = [0.1 * inputs.grf(n, 0.5, s).numpy() for s in (33, 34)]
+    kw = dict(nghost=g, lap_order=order, h0=0.5, lam=1.0)
+    a = run_single(n, None, psi, pi, 3, 0.1, 1.0, **kw)
+    b = run_single(n, inputs.split_level0(n, 8), psi, pi, 3, 0.1, 1.0, **kw)
+    assert np.array_equal(a, b)
+    # non-uniform split: boxes of 8 and 16 cells
+    boxes = [(0, (0, 0, 0), (7, 15, 15)), (0, (8, 0, 0), (15, 7, 15)), (0, (8, 8, 0), (15, 15, 7)),
+             (0, (8, 8, 8), (15, 15, 15))]
+    c = run_single(n, boxes, psi, pi, 3, 0.1, 1.0, **kw)
+    assert np.array_equal(a, c)
+
+
+# ------------------------------------------------------------------------------------------------
+# O5: coarse->fine trilinear + linear-in-time interpolation;  O7: average-down
+# ------------------------------------------------------------------------------------------------
+
+
+def two_level(n0=16, g=3, order=2, lo=(8, 16, 8), hi=(23, 23, 15), **kw):
+    """Level 0: one box; level 1: one box lo..hi (fine indices), properly nested."""
+    boxes = [(0, (0, 0, 0), (n0 - 1, n0 - 1, n0 - 1)), (1, lo, hi)]
+    return Oracle(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=order, **kw)
+
+
+def affine(level_h, shape, lo, coef, g=0):
+    zz, yy, xx = np.meshgrid(*[(np.arange(l - g, l + s + g) + 0.5) * level_h for l, s in zip(lo[::-1], shape)],
+                             indexing="ij")
+    return coef[0] + coef[1] * xx + coef[2] * yy + coef[3] * zz
+
+
+def test_trilinear_reproduces_affine_data_in_space():
+    h0 = 0.5
+    o = two_level(h0=h0, lam=0.0)
+    coefs = [(0.3, 1.0, -2.0, 0.5), (-1.0, 0.25, 0.75, -1.5), (0.1, -1.0, 1.0, 1.0), (2.0, 0.5, 0.5, 0.5)]
+    for c in range(4):
+        o.set_state(0, c, affine(h0, (16, 16, 16), (0, 0, 0), coefs[c]))
+    o.fill_ghosts(1, 0.0)
+    g = 3
+    lo = (8, 16, 8)
+    shp = o.box_shape(1)
+    for c in range(4):
+        raw = o.get_raw(1, c)
+        want = affine(h0 / 2, shp, lo, coefs[c], g=g)
+        ghost = np.ones_like(raw, dtype=bool)
+        ghost[g:-g, g:-g, g:-g] = False
+        assert np.abs(raw - want)[ghost].max() < 1e-13
+        assert np.all(raw[g:-g, g:-g, g:-g] == 0.0)  # valid cells are never touched by a fill
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_time_interpolation_is_linear_between_coarse_old_and_new(order):
+    """lambda = 0 and psi = b + c t (Pi = c, spatially constant) is an exact solution that RK4 reproduces
+    exactly; during the fine substeps the ghosts must then carry b + c t_s for alpha in {0, 1/4, 1/2, 3/4, 1}.
+    The fine interior sees a ghost value consistent with its own only if alpha is right; any wrong alpha
+    puts a kink at the box edge that the Laplacian turns into a non-zero k_Pi."""
+    h0 = 1.0
+    o = two_level(h0=h0, lam=0.0, order=order)
+    b, c = 0.25, 0.5
+    for ib in (0, 1):
+        shp = o.box_shape(ib)
+        o.set_state(ib, 0, np.full(shp, b))
+        o.set_state(ib, 1, np.full(shp, -b))
+        o.set_state(ib, 2, np.full(shp, c))
+        o.set_state(ib, 3, np.full(shp, 2 * c))
+    t, dt = 2.0, 0.5  # exactly representable: alpha is exact
+    for _ in range(2):
+        o.rk_step(dt, t)
+        t += dt
+    for ib in (0, 1):
+        assert np.abs(o.get_state(ib, 0) - (b + c * (t - 2.0))).max() < 1e-14
+        assert np.abs(o.get_state(ib, 1) - (-b + 2 * c * (t - 2.0))).max() < 1e-14
+        assert np.abs(o.get_state(ib, 2) - c).max() < 1e-14
+
+
+def test_ghosts_at_sync_use_new_coarse_state_only():
+    """After a coarse step (alpha = 1) fine ghosts equal the interpolated CURRENT coarse state."""
+    o = two_level(h0=1.0, lam=0.0)
+    coef = (0.3, 1.0, -2.0, 0.5)
+    a = affine(1.0, (16, 16, 16), (0, 0, 0), coef)
+    o.set_state(0, 0, a)
+    o.set_state(1, 0, affine(0.5, o.box_shape(1), (8, 16, 8), coef))
+    o.rk_step(0.25, 1.0)  # psi is affine and Pi = 0, lambda = 0: interior stays put
+    o.set_state(0, 0, 2 * a)  # change the current coarse state by hand
+    o.fill_ghosts(1, 1.25)
+    raw = o.get_raw(1, 0)
+    want = 2 * affine(0.5, o.box_shape(1), (8, 16, 8), coef, g=3)
+    # ghosts not adjacent to the periodic seam are affine-exact
+    assert abs(raw[0, 5, 5] - want[0, 5, 5]) < 1e-13
+    assert abs(raw[5, -1, 7] - want[5, -1, 7]) < 1e-13
+
+
+def test_average_down_affine_and_mean_preserving():
+    h0 = 1.0
+    o = two_level(h0=h0, lam=0.0)
+    coef = (0.3, 1.0, -2.0, 0.5)
+    rng = np.random.default_rng(5)
+    fine = [rng.normal(size=o.box_shape(1)) for _ in range(4)]
+    fine[0] = affine(h0 / 2, o.box_shape(1), (8, 16, 8), coef)
+    for c in range(4):
+        o.set_state(0, c, np.full((16, 16, 16), 7.0))
+        o.set_state(1, c, fine[c])
+    o.average_down(1)
+    cov = (slice(4, 8), slice(8, 12), slice(4, 12))  # z, y, x coarse footprint
+    for c in range(4):
+        got = o.get_state(0, c)
+        mask = np.ones_like(got, dtype=bool)
+        mask[cov] = False
+        assert np.all(got[mask] == 7.0)  # uncovered cells untouched
+        f = fine[c]
+        want = f.reshape(4, 2, 4, 2, 8, 2).mean(axis=(1, 3, 5))
+        assert np.abs(got[cov] - want).max() < 1e-14
+        assert abs(got[cov].sum() - f.sum() / 8) < 1e-11
+    want0 = affine(h0, (4, 4, 8), (4, 8, 4), coef)
+    assert np.abs(o.get_state(0, 0)[cov] - want0).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# O6: subcycling bookkeeping
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2)])
+def test_fully_covered_level1_equals_uniform_fine_run(order, g):
+    """A hierarchy whose level 1 covers 100 % of the domain never interpolates: level 1 must reproduce the
+    single-level 2N run with dt/2 bit-for-bit, and level 0 must equal its average."""
+    n0, h0, dt, eta0 = 8, 1.0, 0.25, 1.0  # binary fractions: both runs see identical stage times
+    nf = 2 * n0
+    psi = [inputs.grf(nf, 0.5, s).numpy() for s in (41, 42)]
+    pi = [0.1 * inputs.grf(nf, 0.5, s).numpy() for s in (43, 44)]
+    ref = run_single(nf, None, psi, pi, 4, dt / 2, eta0, nghost=g, lap_order=order, h0=h0 / 2, lam=1.0)
+    boxes = [(0, (0, 0, 0), (n0 - 1,) * 3), (1, (0, 0, 0), (nf - 1,) * 3)]
+    o = Oracle(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=order, h0=h0, lam=1.0)
+    for c, a in enumerate(psi + pi):
+        o.set_state(1, c, a)
+    o.average_down(1)
+    eta = eta0
+    for _ in range(2):
+        o.rk_step(dt, eta)
+        eta += dt
+    for c in range(4):
+        f = o.get_state(1, c)
+        assert np.array_equal(f, ref[c])
+        want = f.reshape(n0, 2, n0, 2, n0, 2).sum(axis=5).sum(axis=3).sum(axis=1) * 0.125
+        assert np.abs(o.get_state(0, c) - want).max() < 4e-15  # summation order only
+
+
+def test_constant_field_on_three_levels_follows_scalar_ode_per_level():
+    """Each level integrates the scalar ODE with ITS OWN dt (dt/2^l, 2^l times); after synchronisation the
+    covered coarse cells carry the fine value (L74), uncovered ones the coarse value."""
+    n0 = 16
+    boxes = [(0, (0, 0, 0), (15, 15, 15)), (1, (8, 8, 8), (23, 23, 23)), (2, (24, 24, 24), (39, 39, 39))]
+    lam = 1.0
+    o = Oracle(n0, boxes=boxes, n_levels=3, nghost=2, lap_order=2, h0=1.0, lam=lam, friction=2.0)
+    y0 = np.array([0.4, 0.3, -0.2, 0.1])
+    for ib in range(3):
+        for c in range(4):
+            o.set_state(ib, c, np.full(o.box_shape(ib), y0[c]))
+    eta, dt = 1.0, 0.1
+    o.rk_step(dt, eta)
+    ys = []
+    for l in range(3):
+        y, e = y0.copy(), eta
+        for _ in range(1 << l):
+            y = scalar_rk4(y, e, dt / (1 << l), lam, 0.0, 2.0)
+            e += dt / (1 << l)
+        ys.append(y)
+    # Ghost cells of a fine level interpolate the COARSE solution, which differs from the fine one by the
+    # coarse RK4 truncation error (~1e-5 here); it leaks into uncovered level-1 cells (all within 4 cells of
+    # the patch edge) but reaches the level-2 centre only at high order in dt.
+    assert 1e-7 < np.abs(ys[1] - ys[0]).max() < 1e-3
+    for c in range(4):
+        f2 = o.get_state(2, c)
+        assert abs(f2[8, 8, 8] - ys[2][c]) < 1e-13
+        f1 = o.get_state(1, c)
+        assert abs(f1[0, 0, 0] - ys[1][c]) < 1e-4 and abs(f1[1, 8, 1] - ys[1][c]) < 1e-4
+        f0 = o.get_state(0, c)
+        assert abs(f0[0, 0, 0] - ys[0][c]) < 1e-14
+        assert abs(f0[8, 8, 8] - f1[8:10, 8:10, 8:10].mean()) < 1e-15  # covered by level 1 -> average of children
+        assert abs(f1[8, 8, 8] - f2[8:10, 8:10, 8:10].mean()) < 1e-15
+
+
+def amr_wave_error(n0):
+    """Long-wavelength linear wave (one wavelength per box length L = 16) crossing a refined patch."""
+    L = 16.0
+    h0 = L / n0
+    q = n0 // 4
+    boxes = [(0, (0, 0, 0), (n0 - 1,) * 3), (1, (2 * q,) * 3, (6 * q - 1,) * 3)]
+    o = Oracle(n0, boxes=boxes, n_levels=2, nghost=2, lap_order=2, h0=h0, lam=0.0)
+    kx = 2 * math.pi / L
+    w = kx
+
+    def exact(level, lo, shp, t):
+        h = h0 / (1 << level)
+        x = (np.arange(lo[0], lo[0] + shp[2]) + 0.5) * h
+        u = np.cos(kx * x - w * t)
+        ut = w * np.sin(kx * x - w * t)
+        return np.broadcast_to(u[None, None, :], shp), np.broadcast_to(ut[None, None, :], shp)
+
+    for ib, (l, lo, hi) in enumerate(o.boxes):
+        u, ut = exact(l, lo, o.box_shape(ib), 0.0)
+        o.set_state(ib, 0, u)
+        o.set_state(ib, 2, ut)
+    t, dt = 0.0, 0.25 * h0
+    for _ in range(int(round(4.0 / dt))):
+        o.rk_step(dt, t + 1.0)
+        t += dt
+    err = 0.0
+    for ib, (l, lo, hi) in enumerate(o.boxes):
+        u, _ = exact(l, lo, o.box_shape(ib), t)
+        err = max(err, np.abs(o.get_state(ib, 0) - u).max())
+    return err
+
+
+def test_amr_smooth_wave_converges():
+    """End-to-end sanity for the hierarchy: a smooth wave crossing a refined patch.  Trilinear ghosts carry an
+    O(h^2) error that the Laplacian divides by h^2, so the scheme BASELINE.json prescribes is first-order at
+    the patch edge (the reason the paper defaults to quartic interpolation, L70/L780): halving h must cut the
+    error by ~2.  A wrong ghost offset, weight or alpha makes it grow or stall instead."""
+    e16 = amr_wave_error(16)
+    e32 = amr_wave_error(32)
+    assert e16 < 0.1
+    assert e32 < e16 / 1.8, (e16, e32)
+
+
+# ------------------------------------------------------------------------------------------------
+# O8: string tags
+# ------------------------------------------------------------------------------------------------
+
+
+def atan2_winding(A, B, C, D):
+    """Textbook definition: sum of principal-value phase differences around the loop / 2 pi."""
+    z = [complex(*A), complex(*B), complex(*C), complex(*D)]
+    tot = 0.0
+    for a, b in zip(z, z[1:] + z[:1]):
+        tot += np.angle(b / a)
+    return int(round(tot / (2 * math.pi)))
+
+
+def brute_tags(psi1, psi2):
+    """Pure-Python tags of a periodic single-level grid from the atan2 definition."""
+    n = psi1.shape
+    tags = np.zeros(n, dtype=np.uint8)
+    P = lambda k, j, i: (psi1[k % n[0], j % n[1], i % n[2]], psi2[k % n[0], j % n[1], i % n[2]])
+    for k in range(n[0]):
+        for j in range(n[1]):
+            for i in range(n[2]):
+                t = 0
+                if atan2_winding(P(k, j, i), P(k, j, i + 1), P(k, j + 1, i + 1), P(k, j + 1, i)):
+                    t |= 1  # xy
+                if atan2_winding(P(k, j, i), P(k, j + 1, i), P(k + 1, j + 1, i), P(k + 1, j, i)):
+                    t |= 2  # yz
+                if atan2_winding(P(k, j, i), P(k + 1, j, i), P(k + 1, j, i + 1), P(k, j, i + 1)):
+                    t |= 4  # zx
+                tags[k, j, i] = t
+    return tags
+
+
+def test_plaquette_winding_matches_atan2_definition_on_random_corners():
+    rng = np.random.default_rng(3)
+    seen = set()
+    for _ in range(20000):
+        v = rng.normal(size=(4, 2))
+        w = plaquette_winding(*v)
+        assert w == atan2_winding(*v)
+        seen.add(w)
+    assert seen == {-1, 0, 1}
+    # hand-made cases: CCW loop around the origin, CW loop, loop that misses it
+    sq = np.array([[1, 1], [-1, 1], [-1, -1], [1, -1]], dtype=float)
+    assert plaquette_winding(*sq) == 1
+    assert plaquette_winding(*sq[::-1]) == -1
+    assert plaquette_winding(*(sq + 3.0)) == 0
+
+
+def test_straight_string_tags_exactly_four_columns():
+    """psi = (x - x0) + i (y - y0), x0, y0 half-integers, periodic N grid: xy-plaquettes wind at
+    (floor x0, floor y0) [+1], (N-1, floor y0) [-1], (floor x0, N-1) [-1], (N-1, N-1) [+1] for every z,
+    and no yz / zx plaquette winds."""
+    n = 16
+    x0, y0 = 5.5, 9.5
+    psi1, psi2 = inputs.straight_string(n, x0, y0)
+    o = Oracle(n, nghost=1, lap_order=1)
+    o.set_state(0, 0, psi1)
+    o.set_state(0, 1, psi2)
+    tags, counts = o.tag_strings(0)
+    want = np.zeros((n, n, n), dtype=np.uint8)
+    for (j, i) in [(9, 5), (9, n - 1), (n - 1, 5), (n - 1, n - 1)]:
+        want[:, j, i] = 1
+    assert np.array_equal(tags[0], want)
+    assert counts.shape == (1, 1, 1) and counts[0, 0, 0] == 4 * n
+    # signs of the four windings
+    P = lambda j, i: (psi1[0, j % n, i % n], psi2[0, j % n, i % n])
+    W = lambda j, i: plaquette_winding(P(j, i), P(j, i + 1), P(j + 1, i + 1), P(j + 1, i))
+    assert (W(9, 5), W(9, n - 1), W(n - 1, 5), W(n - 1, n - 1)) == (1, -1, -1, 1)
+
+
+def test_tags_match_brute_force_and_torus_identity():
+    n = 8
+    psi1 = inputs.grf(n, 0.9, 51).numpy()
+    psi2 = inputs.grf(n, 0.9, 52).numpy()
+    o = Oracle(n, nghost=1, lap_order=1)
+    o.set_state(0, 0, psi1)
+    o.set_state(0, 1, psi2)
+    tags, counts = o.tag_strings(0)
+    want = brute_tags(psi1, psi2)
+    assert want.any(), "test field should contain strings"
+    assert np.array_equal(tags[0], want)
+    assert counts[0, 0, 0] == np.count_nonzero(want)
+    # torus identity: the windings of all xy plaquettes of one z-slice sum to zero
+    P = lambda k, j, i: (psi1[k % n, j % n, i % n], psi2[k % n, j % n, i % n])
+    for k in range(n):
+        tot = sum(plaquette_winding(P(k, j, i), P(k, j, i + 1), P(k, j + 1, i + 1), P(k, j + 1, i))
+                  for j in range(n) for i in range(n))
+        assert tot == 0
+
+
+def test_tags_invariant_under_global_phase_rotation():
+    n = 16
+    psi1 = inputs.grf(n, 0.6, 61).numpy()
+    psi2 = inputs.grf(n, 0.6, 62).numpy()
+    o = Oracle(n, nghost=1, lap_order=1)
+    o.set_state(0, 0, psi1)
+    o.set_state(0, 1, psi2)
+    t0, _ = o.tag_strings(0)
+    ph = 1.2345
+    o.set_state(0, 0, math.cos(ph) * psi1 - math.sin(ph) * psi2)
+    o.set_state(0, 1, math.sin(ph) * psi1 + math.cos(ph) * psi2)
+    t1, _ = o.tag_strings(0)
+    assert t0[0].any()
+    assert np.array_equal(t0[0], t1[0])
+
+
+def test_tags_on_multibox_and_flag_block_counts():
+    """Tags of a tiled level equal the single-box tags (ghost +1 neighbours incl. edge ghosts), and counts
+    are accumulated per aligned 32^3 block of the level index space."""
+    n = 64
+    psi1 = inputs.grf(n, 0.3, 71).numpy()
+    psi2 = inputs.grf(n, 0.3, 72).numpy()
+    o = Oracle(n, nghost=1, lap_order=1)
+    o.set_state(0, 0, psi1)
+    o.set_state(0, 1, psi2)
+    t_single, c_single = o.tag_strings(0)
+    boxes = inputs.split_level0(n, 16)
+    om = Oracle(n, boxes=boxes, nghost=1, lap_order=1)
+    full = np.zeros((n, n, n), dtype=np.uint8)
+    for ib, (l, lo, hi) in enumerate(boxes):
+        sl = (slice(lo[2], hi[2] + 1), slice(lo[1], hi[1] + 1), slice(lo[0], hi[0] + 1))
+        om.set_state(ib, 0, psi1[sl])
+        om.set_state(ib, 1, psi2[sl])
+    t_multi, c_multi = om.tag_strings(0)
+    for ib, (l, lo, hi) in enumerate(boxes):
+        sl = (slice(lo[2], hi[2] + 1), slice(lo[1], hi[1] + 1), slice(lo[0], hi[0] + 1))
+        full[sl] = t_multi[ib]
+    assert np.array_equal(full, t_single[0])
+    assert np.array_equal(c_multi, c_single)
+    want = (t_single[0] != 0).reshape(2, 32, 2, 32, 2, 32).sum(axis=(1, 3, 5))
+    assert np.array_equal(c_single, want.astype(np.uint32))
+
+
+# ------------------------------------------------------------------------------------------------
+# O1: validation of box lists
+# ------------------------------------------------------------------------------------------------
+
+
+def test_box_list_validation():
+    ok = [(0, (0, 0, 0), (15, 15, 15)), (1, (8, 8, 8), (23, 23, 23))]
+    Oracle(16, boxes=ok, n_levels=2, nghost=2, lap_order=2)
+    with pytest.raises(OracleError, match="overlap"):
+        Oracle(16, boxes=ok + [(1, (16, 16, 16), (31, 31, 31))], n_levels=2, nghost=2, lap_order=2)
+    with pytest.raises(OracleError, match="aligned"):
+        Oracle(16, boxes=[ok[0], (1, (4, 8, 8), (19, 23, 23))], n_levels=2, nghost=2, lap_order=2)
+    with pytest.raises(OracleError, match="cover"):
+        Oracle(16, boxes=[(0, (0, 0, 0), (7, 15, 15))], nghost=1)
+    with pytest.raises(OracleError, match="nghost"):
+        Oracle(16, nghost=8, blocking_factor=8)
+    with pytest.raises(OracleError, match="lap_order"):
+        Oracle(16, nghost=1, lap_order=2)
+    # level 2 box whose grown region leaves level 1 -> nesting violation
+    bad = [(0, (0, 0, 0), (15, 15, 15)), (1, (8, 8, 8), (23, 23, 23)), (2, (16, 16, 16), (31, 31, 31))]
+    with pytest.raises(OracleError, match="nesting"):
+        Oracle(16, boxes=bad, n_levels=3, nghost=2, lap_order=2)
+    good = [(0, (0, 0, 0), (15, 15, 15)), (1, (8, 8, 8), (23, 23, 23)), (2, (24, 24, 24), (39, 39, 39))]
+    Oracle(16, boxes=good, n_levels=3, nghost=2, lap_order=2)
