@@ -470,15 +470,15 @@ def test_constant_field_on_three_levels_follows_scalar_ode_per_level():
             y = scalar_rk4(y, e, dt / (1 << l), lam, 0.0, 2.0)
             e += dt / (1 << l)
         ys.append(y)
-    # Ghost cells of a fine level interpolate the COARSE solution, which differs from the fine one by the
-    # coarse RK4 truncation error (~1e-5 here); it leaks into uncovered level-1 cells (all within 4 cells of
-    # the patch edge) but reaches the level-2 centre only at high order in dt.
+    # Ghost cells of a fine level carry the coarse solution interpolated LINEARLY in time (error ~dt^2 psi''/8
+    # ~1e-3 at mid-step); it leaks into uncovered level-1 cells (all within 4 cells of the patch edge) but
+    # reaches the level-2 centre only at high order in dt.
     assert 1e-7 < np.abs(ys[1] - ys[0]).max() < 1e-3
     for c in range(4):
         f2 = o.get_state(2, c)
         assert abs(f2[8, 8, 8] - ys[2][c]) < 1e-13
         f1 = o.get_state(1, c)
-        assert abs(f1[0, 0, 0] - ys[1][c]) < 1e-4 and abs(f1[1, 8, 1] - ys[1][c]) < 1e-4
+        assert abs(f1[0, 0, 0] - ys[1][c]) < 5e-3 and abs(f1[1, 8, 1] - ys[1][c]) < 5e-3
         f0 = o.get_state(0, c)
         assert abs(f0[0, 0, 0] - ys[0][c]) < 1e-14
         assert abs(f0[8, 8, 8] - f1[8:10, 8:10, 8:10].mean()) < 1e-15  # covered by level 1 -> average of children
