@@ -1,0 +1,394 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the sledge hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl sledge|reference]
+
+A "step" is one pass of the whole hot path over the workload: sledge_rk_step (per RK stage: ghost fill +
+fused Laplacian/potential/RK-stage kernel; with AMR: subcycling + average-down) followed by
+sledge_tag_strings (winding tags + per-32^3 block counts).  Metric: cell-updates per second per RK stage,
+`value` = valid cell-stage updates of all levels per step / step time.  Inputs are seeded synthetic
+fields (paper_2404_02950_b200.inputs); every state buffer is far larger than L2, so no flush is needed.
+Multi-GPU: the path does not shard in this build ("replicas only"): every rank runs an independent replica.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Gcell-updates/s per RK stage"
+UNIT = "Gcell-updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="sledge", choices=["sledge", "reference"])
+    ap.add_argument("--flow", default="lean", choices=["lean", "classic"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------
+# workload construction (shared recipe; no arithmetic of the method here)
+# ---------------------------------------------------------------------------------------------------
+
+def hierarchy(cfg):
+    from paper_2404_02950_b200 import inputs
+    if cfg.n_levels == 1:
+        return None, [(0, (0, 0, 0), (cfg.n0 - 1,) * 3)], [1.0]
+    ex = cfg.extra
+    rings = inputs.make_rings(cfg.n0, ex["n_rings"], ex["rmin"], ex["rmax"], ex["core_w"], cfg.seeds[0])
+    boxes, cover = inputs.amr_boxes_for_rings(rings, n_levels=cfg.n_levels, box=ex["box"], r1=ex["r1"], r2=ex["r2"],
+                                              blocking_factor=cfg.blocking_factor)
+    return rings, boxes, cover
+
+
+def cells_per_step(cfg, boxes):
+    """valid cell-steps per coarse step: level l takes 2^l steps (Eq.3)."""
+    tot = 0
+    per_level = [0] * cfg.n_levels
+    for l, lo, hi in boxes:
+        n = (hi[0] - lo[0] + 1) * (hi[1] - lo[1] + 1) * (hi[2] - lo[2] + 1)
+        per_level[l] += n
+        tot += n * (1 << l)
+    return tot, per_level
+
+
+def initial_fields(cfg, rings, boxes, device, tdtype):
+    """yield (box index, comp, tensor on `device`) for psi1, psi2; Pi = 0 is the zero-filled arena."""
+    import torch
+    from paper_2404_02950_b200 import inputs
+    if cfg.n_levels == 1:
+        for c, seed in enumerate(cfg.seeds):
+            yield 0, c, inputs.grf(cfg.n0, cfg.grf_f, seed, device=device, dtype=tdtype).contiguous()
+    else:
+        for ib, (l, lo, hi) in enumerate(boxes):
+            re, im = inputs.ring_field(rings, l, lo, hi, device=device)
+            yield ib, 0, re.to(tdtype).contiguous()
+            yield ib, 1, im.to(tdtype).contiguous()
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------------------
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.samples, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference): the oracle as it stands, on a bounded sample
+# ---------------------------------------------------------------------------------------------------
+
+def oracle_sample(cfg):
+    """A bounded sample of the workload for the CPU oracle: same stencil, dtype-independent fp64 arithmetic,
+    same parameters, a periodic 128^3 (64^3 for C1: 32^3) sub-volume cut into 32^3 boxes so that the oracle's
+    OpenMP loops over boxes use the host cores; AMR: the same recipe at base 64^3 with 16^3 boxes."""
+    from oracle.oracle import Oracle
+    from paper_2404_02950_b200 import inputs
+    import numpy as np
+    if cfg.n_levels == 1:
+        n = min(cfg.n0, 128)
+        boxes = inputs.split_level0(n, 32)
+        o = Oracle(n, boxes=boxes, nghost=cfg.nghost, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam)
+        f = [inputs.grf(n, cfg.grf_f, s).numpy() for s in cfg.seeds]
+        for ib, (_, lo, hi) in enumerate(boxes):
+            for c in range(2):
+                o.set_state(ib, c, np.ascontiguousarray(f[c][lo[2]:hi[2] + 1, lo[1]:hi[1] + 1, lo[0]:hi[0] + 1]))
+        desc = f"periodic {n}^3 sub-volume of the workload in 32^3 boxes, same stencil and parameters"
+        cells = n ** 3
+        levels = 1
+    else:
+        n = 64
+        ex = cfg.extra
+        rings = inputs.make_rings(n, 3, 8.0, 16.0, ex["core_w"], cfg.seeds[0])
+        boxes, _ = inputs.amr_boxes_for_rings(rings, n_levels=3, box=16, r1=4.0, r2=1.0, blocking_factor=8)
+        o = Oracle(n, boxes=boxes, n_levels=3, nghost=cfg.nghost, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam)
+        for ib, (l, lo, hi) in enumerate(boxes):
+            re, im = inputs.ring_field(rings, l, lo, hi)
+            o.set_state(ib, 0, re.numpy())
+            o.set_state(ib, 1, im.numpy())
+        cells, _ = cells_per_step(cfg, boxes)
+        desc = f"3-level ring hierarchy at base {n}^3 with 16^3 boxes ({len(boxes)} boxes), same stencil and parameters"
+        levels = 3
+    return o, cells, desc, levels
+
+
+def oracle_step(o, cfg, eta, levels):
+    o.rk_step(cfg.dt, eta)
+    for l in range(levels):
+        o.tag_strings(l)
+
+
+def time_oracle(cfg, budget_s=12.0, steps=None, warmup=1):
+    from oracle import oracle as orc
+    o, cells, desc, levels = oracle_sample(cfg)
+    eta = cfg.eta0
+    for _ in range(warmup):
+        oracle_step(o, cfg, eta, levels)
+        eta += cfg.dt
+    t0 = time.perf_counter()
+    oracle_step(o, cfg, eta, levels)
+    eta += cfg.dt
+    one = time.perf_counter() - t0
+    n = steps if steps is not None else max(1, min(50, int(budget_s / max(one, 1e-6)) - 1))
+    t0 = time.perf_counter()
+    for _ in range(n):
+        oracle_step(o, cfg, eta, levels)
+        eta += cfg.dt
+    dt = (time.perf_counter() - t0) / n
+    return {"value": cells * 4 / dt / 1e9, "unit": UNIT, "cores": orc.omp_threads(), "kind": "oracle",
+            "sample": f"{desc}; {n} steps of rk_step + tag_strings, {dt * 1e3:.1f} ms/step"}, dt, n
+
+
+# ---------------------------------------------------------------------------------------------------
+# reference arm: the oracle on the host cores
+# ---------------------------------------------------------------------------------------------------
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cpu, dt, n = time_oracle(cfg, steps=args.steps, warmup=max(1, min(args.warmup, 2)))
+    line = {"impl": "reference", "metric": METRIC, "value": cpu["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": n, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name} (bounded sample for the CPU oracle)", "sample": cpu["sample"]},
+            "cpu_baseline": cpu,
+            "e2e": {"value": cpu["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------------
+
+def run_sledge(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2404_02950_b200 import build as sbuild
+    from paper_2404_02950_b200 import sledge as S
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the sledge path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    if not os.path.exists(S.LIB_PATH):
+        sbuild.build()
+
+    rings, boxes, cover = hierarchy(cfg)
+    cell_steps, per_level = cells_per_step(cfg, boxes)
+    s = S.Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=cfg.nghost, blocking_factor=cfg.blocking_factor,
+                 dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=args.flow, device=dev)
+    for ib, c, t in initial_fields(cfg, rings, boxes, dev, s.tdtype):
+        s.set_state(ib, c, t)
+        del t
+    torch.cuda.empty_cache()
+    tags = [torch.empty(s.level_cells(l)[0], dtype=torch.uint8, device=dev) for l in range(cfg.n_levels)]
+    counts = [torch.empty(s.count_shape(l), dtype=torch.int32, device=dev) for l in range(cfg.n_levels)]
+
+    eta = [cfg.eta0]
+
+    def step():
+        s.rk_step(cfg.dt, eta[0])
+        eta[0] += cfg.dt
+        for l in range(cfg.n_levels):
+            s.tag_strings(l, tags[l], counts[l])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    s.synchronize()
+    # ---- timed region: K steps, CUDA events on the launching stream, clocks sampled meanwhile ----
+    clk = ClockSampler(local)
+    if rank == 0:
+        clk.start()
+    s.profile_enable(True)
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1) / args.steps
+    launches = s.launch_count() - l0
+    prof = {k: s.profile_read(kind) for k, kind in
+            (("stage", S.KIND_STAGE), ("ghost", S.KIND_GHOST), ("tag", S.KIND_TAG), ("avg", S.KIND_AVG))}
+    s.profile_enable(False)
+    clocks = clk.stop() if rank == 0 else None
+    s.synchronize()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- roofline of the dominant kernel (K1) -----------------------------------------------------
+    esz = 8 if cfg.dtype == "f64" else 4
+    words_per_cell_step = 52 if args.flow == "lean" else 64
+    n_stage, ms_stage = prof["stage"]
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    # profile counters cover the timed K steps: n_stage launches moved cell_steps * words * esz bytes per step
+    stage_bytes_total = cell_steps * words_per_cell_step * esz * args.steps
+    achieved = stage_bytes_total / (ms_stage * 1e-3) / 1e9 if ms_stage > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "k_rk_stage (K1, mean over the 4 stage launches)", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
+                "peak_source": peak_src, "traffic": None,
+                "bytes_per_cell_step": words_per_cell_step * esz,
+                "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage}
+    shares = {k: (v[1] / args.steps) for k, v in prof.items()}
+
+    value = world * cell_steps * 4 / (ms * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {cfg.n0}^3 base, {cfg.n_levels} level(s), {cfg.dtype}, "
+                                   f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, RK4 ({args.flow} data-flow), "
+                                   f"dt={cfg.dt}, h0={cfg.h0}, tags + 32^3 counts every step",
+                       "cells_per_level": per_level, "coverage": cover, "cell_steps_per_step": cell_steps,
+                       "l2": "state buffers >> 126 MB L2 (no flush needed)" if cell_steps * esz * 4 > 4e8 else
+                             "state fits in L2 (small case; not a roofline workload)",
+                       "multi_gpu": "replicas only"},
+            "gcell_steps_per_s": value / 4,
+            "kernel_ms_per_step": shares, "roofline": roofline, "gpu_launches": launches, "clocks": clocks}
+
+    # ---- e2e: same step through the C ABI with HOST buffers -----------------------------------------
+    if not args.no_e2e:
+        line["e2e"] = e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags=(tags, counts))
+    del s
+    torch.cuda.empty_cache()
+    if rank == 0 and not args.no_cpu:
+        line["cpu_baseline"], _, _ = time_oracle(cfg)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags):
+    """Per step: host->device copy of the whole state (4 components of every box, pinned host memory) through
+    sledge_set_state_host, rk_step + tag_strings, device->host copy of the new state and the block counts."""
+    import torch
+    tags, counts = step_tags
+    host_in = [[torch.empty(s.box_shape(ib), dtype=s.tdtype).pin_memory() for _ in range(4)] for ib in range(len(boxes))]
+    host_out = [[torch.empty(s.box_shape(ib), dtype=s.tdtype).pin_memory() for _ in range(4)] for ib in range(len(boxes))]
+    host_counts = [torch.empty(c.shape, dtype=torch.int32).pin_memory() for c in counts]
+    for ib in range(len(boxes)):
+        for c in range(4):
+            s.get_state_host(ib, c, host_in[ib][c])
+    s.synchronize()
+    bi = sum(t.numel() * t.element_size() for b in host_in for t in b)
+    bo = bi + sum(t.numel() * t.element_size() for t in host_counts)
+    eta = cfg.eta0
+
+    def one():
+        for ib in range(len(boxes)):
+            for c in range(4):
+                s.set_state_host(ib, c, host_in[ib][c])
+        s.rk_step(cfg.dt, eta)
+        for l in range(cfg.n_levels):
+            s.tag_strings(l, tags[l], counts[l])
+            host_counts[l].copy_(counts[l], non_blocking=True)
+        for ib in range(len(boxes)):
+            for c in range(4):
+                s.get_state_host(ib, c, host_out[ib][c])
+
+    one()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.e2e_steps):
+        one()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.e2e_steps
+    return {"value": world * cell_steps * 4 / (ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms,
+            "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "steps": args.e2e_steps,
+            "what": "sledge_set_state_host x4/box + sledge_rk_step + sledge_tag_strings + sledge_get_state_host x4/box + counts"}
+
+
+def main():
+    args = parse()
+    from paper_2404_02950_b200 import inputs
+    cfg = inputs.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_sledge(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

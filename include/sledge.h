@@ -1,0 +1,147 @@
+/* sledge.h -- C ABI of the B200-native sledgehamr hot path (arXiv 2404.02950).
+ *
+ * One library, libsledge.so, hand-written CUDA for sm_100a.  No torch types, no exceptions, no CPU
+ * fallback: every compute entry point launches kernels on the CUDA stream given at create time and
+ * returns immediately (asynchronous), or fails with a negative code.
+ *
+ * Citations are PAPER.md line numbers (text of arXiv 2404.02950) and DESIGN.md readings (R#).
+ *
+ * Grid (Eq.1-3): level l has the periodic index space [0, n0*2^l)^3, spacing
+ * h_l = h0/2^l, and is covered by rectangular boxes whose low corner and size are multiples of
+ * blocking_factor; level 0 covers the domain; level l+1 is properly nested in level l (L70, L137).
+ * State per cell: u = (psi1, psi2, Pi1, Pi2) (L189-190), component index 0..3 in that order.
+ *
+ * Device layout: per level, 4 state buffers; a buffer is two
+ * planes, PSI = interleaved (psi1,psi2) pairs and PI = interleaved (Pi1,Pi2) pairs, boxes stored back
+ * to back, each box with nghost ghost layers and its x rows padded to 128-byte multiples.
+ *
+ * Ownership: the caller allocates ONE device arena (sledge_arena_bytes tells how large) and lends
+ * it for the lifetime of the context; the library never allocates device memory.  All `dev_`
+ * pointers are device pointers, all `host_` pointers are host pointers (pinned for async copies).
+ *
+ * Errors: 0 on success, a negative sledge_status otherwise; sledge_last_error() returns the text.
+ */
+#ifndef SLEDGE_H
+#define SLEDGE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sledge_ctx sledge_ctx; /* opaque; host-side metadata only */
+
+typedef enum {
+  SLEDGE_OK = 0,
+  SLEDGE_EINVAL = -1, /* bad parameter / overlapping, misaligned or non-nested boxes            */
+  SLEDGE_ENOMEM = -2, /* arena too small or misaligned                                           */
+  SLEDGE_ECUDA = -3,  /* CUDA runtime / launch error (no device, bad stream, kernel fault)       */
+  SLEDGE_ESTATE = -4  /* call not valid in the current state (e.g. rk_stage out of order)        */
+} sledge_status;
+
+enum { SLEDGE_F32 = 0, SLEDGE_F64 = 1 };
+enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1 };
+
+/* Inclusive cell range lo..hi of one box in the index space of `level`; axis order x, y, z. */
+typedef struct {
+  int32_t level;
+  int32_t lo[3];
+  int32_t hi[3];
+} sledge_box;
+
+typedef struct {
+  int32_t n_levels;        /* 1..8                                                                */
+  int32_t n0[3];           /* level-0 cells per axis, periodic (L23); multiples of blocking_factor */
+  int32_t nghost;          /* ghost layers per box (L68-70, L772): lap_order <= nghost < blocking_factor */
+  int32_t blocking_factor; /* power of 2 (L39, L771)                                              */
+  int32_t dtype;           /* SLEDGE_F32 / SLEDGE_F64: storage AND arithmetic type                */
+  int32_t lap_order;       /* paper's `order` (L649): 1 = 7-point, 2 = 13-point Laplacian         */
+  int32_t eta_fixed;       /* 1 = Minkowski test variant: eta_s = eta for every stage (R3)         */
+  int32_t rk_dataflow;     /* SLEDGE_RK_LEAN: 52 words/cell-step; SLEDGE_RK_CLASSIC: 64 (R5)       */
+  double h0;               /* level-0 spacing, Eq.1                                               */
+  double lambda;           /* Eq.11 generalised (R2): k_Pi = -(friction/eta) Pi + Lap psi          */
+  double a_mass;           /*        - lambda eta^2 psi (psi1^2+psi2^2-1) - a_mass psi             */
+  double friction;         /* paper: 2 (Eq.11); BASELINE.json configs: 0                          */
+} sledge_params;
+
+/* Size of the device arena needed for this hierarchy.  Host-only: validates params and boxes
+ * (same checks as sledge_create) and needs no GPU.  ctx-less errors: sledge_last_error(NULL). */
+int sledge_arena_bytes(const sledge_params* params, const sledge_box* boxes, int nbox, size_t* bytes);
+
+/* Build a context.  dev_arena: device memory, 256-byte aligned, >= sledge_arena_bytes, zero-filled
+ * by this call.  cuda_stream: a cudaStream_t (0 = legacy default stream); every later call enqueues
+ * on it.  Box indices used below are positions in `boxes`. */
+int sledge_create(sledge_ctx** ctx, const sledge_params* params, const sledge_box* boxes, int nbox,
+                  void* dev_arena, size_t arena_bytes, void* cuda_stream);
+int sledge_destroy(sledge_ctx* ctx);
+
+/* Copy one component of one box between a dense device array of its valid region (x fastest,
+ * nx*ny*nz reals of the context's dtype) and the current state.  Setting a state invalidates the
+ * level's (old,new) pair used for temporal ghost interpolation. */
+int sledge_set_state(sledge_ctx* ctx, int box, int comp, const void* dev_src);
+int sledge_get_state(sledge_ctx* ctx, int box, int comp, void* dev_dst);
+/* Same with HOST buffers: the library stages through a device scratch inside the arena
+ * (cudaMemcpyAsync on the context stream; truly asynchronous only for pinned memory). */
+int sledge_set_state_host(sledge_ctx* ctx, int box, int comp, const void* host_src);
+int sledge_get_state_host(sledge_ctx* ctx, int box, int comp, void* host_dst);
+/* One component of one box INCLUDING ghosts: (nx+2g)*(ny+2g)*(nz+2g) reals, x fastest.  Only psi1,
+ * psi2 ghosts are ever filled (Pi is never differenced, R10). */
+int sledge_get_ghosted(sledge_ctx* ctx, int box, int comp, void* dev_dst);
+
+/* Ghost fill of the CURRENT state of `level` (L68-74): every psi ghost cell <- the valid cell of the
+ * same level at the periodically wrapped index if one exists, else trilinear interpolation of the
+ * next coarser level, itself linearly interpolated in time between its states at the start and end
+ * of its last step (alpha = (time - t_old)/(t_new - t_old); the current coarse state alone if that
+ * level has not stepped since its state was set). */
+int sledge_fill_ghosts(sledge_ctx* ctx, int level, double time);
+
+/* One classic-RK4 stage (integrator.type 4, L808) of `level`: ghost fill of the stage input at
+ * eta + c_s dt, then the fused Laplacian + potential + stage-update kernel (Eq.10-11).  stage =
+ * 0,1,2,3 in order; `eta` is the time at the START of the step for all four calls.  Stage 3 makes
+ * the new state current.  Test / timing hook; sledge_rk_step is built from it. */
+int sledge_rk_stage(sledge_ctx* ctx, int level, int stage, double dt, double eta);
+
+/* ONE coarse step eta -> eta + dt of the whole hierarchy (L64-76, L88 Fig.2): level l takes 2^l steps
+ * of dt/2^l (Eq.3) with per-stage ghost fills, finest first to finish, average-down after each pair
+ * of fine steps.  Afterwards the valid cells of every level hold the state at eta + dt; ghost
+ * contents are unspecified until the next sledge_fill_ghosts. */
+int sledge_rk_step(sledge_ctx* ctx, double dt, double eta);
+
+/* String tagging (L349-371 hook; rule: DESIGN.md R8) of the current state of `level`, ghosts filled
+ * first.  dev_tags: one byte per valid cell, boxes of the level back to back in box order, x fastest;
+ * bit0/1/2 = the xy / yz / zx plaquette whose lowest corner is the cell has non-zero winding.
+ * dev_counts: uint32 per aligned 32^3 block of the level's index space (x fastest,
+ * ceil(n/32) per axis) = number of tagged cells in it; zeroed by the call.  Either may be NULL. */
+int sledge_tag_strings(sledge_ctx* ctx, int level, uint8_t* dev_tags, uint32_t* dev_counts);
+
+/* Level synchronisation (L74): every cell of level fine_level-1 covered by fine_level <- mean of its 8
+ * children, all four components, on the current states. */
+int sledge_average_down(sledge_ctx* ctx, int fine_level);
+
+/* Bookkeeping. */
+int sledge_level_cells(const sledge_ctx* ctx, int level, int64_t* valid_cells, int64_t* count_blocks);
+int64_t sledge_launch_count(const sledge_ctx* ctx); /* kernels launched by this context so far */
+
+/* Wait for everything enqueued so far and report deferred errors: SLEDGE_ECUDA for a kernel fault,
+ * SLEDGE_ESTATE if a kernel met a ghost or coarse cell that no box provides (cannot happen for box
+ * lists that passed sledge_create's nesting check).  The only blocking call besides
+ * sledge_profile_read and sledge_destroy. */
+int sledge_synchronize(sledge_ctx* ctx);
+
+/* Per-kernel device timing with CUDA events on the context stream (bench.py's roofline leg).
+ * kind: 0 = rk stage kernel, 1 = ghost fill, 2 = tagging, 3 = average-down.  While enabled every
+ * launch of that kind is bracketed by an event pair (at most 4096 pairs are kept).
+ * sledge_profile_read synchronises the stream and returns launches and their summed milliseconds
+ * since the last enable. */
+int sledge_profile_enable(sledge_ctx* ctx, int on);
+int sledge_profile_read(sledge_ctx* ctx, int kind, int64_t* launches, double* total_ms);
+
+/* Text of the last error of this context (or of the last failed ctx-less call if ctx == NULL). */
+const char* sledge_last_error(const sledge_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLEDGE_H */

@@ -1,0 +1,731 @@
+// sledge.cu -- host side of libsledge.so: hierarchy validation, arena layout, launch logic, C ABI.
+//
+// Everything the path computes runs in the kernels under csrc/k_*.cuh; this file only validates the box
+// list, lays the caller's arena out, builds the device descriptor
+// tables and enqueues launches on the caller's stream.  There is no CPU fallback of any step.
+#include "../../include/sledge.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "k_avgdown.cuh"
+#include "k_ghost.cuh"
+#include "k_rk_stage.cuh"
+#include "k_tag.cuh"
+
+using namespace sledge;
+
+namespace {
+
+constexpr int NBUF = 4;
+constexpr int COUNT_BLOCK = 32;  // box-flag reduction granularity (BASELINE.json config 3)
+constexpr int MAX_EVENT_PAIRS = 4096;
+constexpr size_t ALIGN = 256;
+
+// K1 tile shapes (threads); cells per tile in x = TX * cells-per-16-bytes
+constexpr int K1_TX = 32, K1_TY = 8, K1_NZ = 64;
+
+thread_local std::string g_err;
+
+struct LevelHost {
+  int n[3], no[3];
+  double h;
+  std::vector<int> boxes;  // global box ids in input order
+  std::vector<BoxDev> boxdev;
+  std::vector<int> owner;
+  std::vector<TileDev> tiles, tag_tiles;
+  std::vector<int> ghost_prefix, avg_prefix;
+  long long plane_cells = 0;  // pairs per plane (all boxes, ghosts and padding included)
+  long long valid_cells = 0;
+  long long count_blocks = 0;
+  int nb[3];
+  // arena offsets (bytes)
+  size_t off_buf[NBUF][2];
+  size_t off_boxes, off_tiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix;
+  // run state
+  int cur = 0, old = 0;
+  bool have_pair = false;
+  double t_old = 0, t_new = 0;
+};
+
+struct Plan {
+  sledge_params p;
+  std::vector<sledge_box> box;
+  std::vector<int> box_local;
+  std::vector<LevelHost> lev;
+  int esz = 8;       // bytes per real
+  int cpa = 8;       // cells (pairs) per 128 bytes
+  int ox = 8;        // x offset of the first valid cell inside a row
+  size_t off_scratch = 0, scratch_bytes = 0, off_err = 0, total = 0;
+};
+
+}  // namespace
+
+struct sledge_ctx {
+  Plan plan;
+  char* arena = nullptr;
+  cudaStream_t stream = nullptr;
+  std::string err;
+  int64_t launches = 0;
+  bool profiling = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
+  size_t ev_used[4] = {0, 0, 0, 0};
+};
+
+namespace {
+
+int fail(sledge_ctx* ctx, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf; else g_err = buf;
+  return code;
+}
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline int ilog2(int v) {
+  int s = 0;
+  while ((1 << s) < v) ++s;
+  return s;
+}
+inline int fdiv2(int i) { return i >> 1; }
+
+// ---- validation + layout (host only; shared by sledge_arena_bytes and sledge_create) --------------
+int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbox) {
+  if (!pp || !boxes || nbox <= 0) return fail(nullptr, SLEDGE_EINVAL, "null params / empty box list");
+  P.p = *pp;
+  const sledge_params& p = P.p;
+  if (p.n_levels < 1 || p.n_levels > 8) return fail(nullptr, SLEDGE_EINVAL, "n_levels must be 1..8");
+  const int bf = p.blocking_factor;
+  if (bf < 2 || (bf & (bf - 1))) return fail(nullptr, SLEDGE_EINVAL, "blocking_factor must be a power of 2 >= 2 (L39)");
+  if (p.nghost < 1 || p.nghost >= bf) return fail(nullptr, SLEDGE_EINVAL, "need 1 <= nghost < blocking_factor (L772)");
+  if (p.lap_order < 1 || p.lap_order > 2) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be 1 (7-point) or 2 (13-point)");
+  if (p.lap_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be <= nghost (L240)");
+  if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
+  if (p.rk_dataflow != SLEDGE_RK_LEAN && p.rk_dataflow != SLEDGE_RK_CLASSIC) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
+  if (!(p.h0 > 0)) return fail(nullptr, SLEDGE_EINVAL, "h0 must be positive");
+  for (int d = 0; d < 3; ++d) {
+    if (p.n0[d] <= 0 || p.n0[d] % bf) return fail(nullptr, SLEDGE_EINVAL, "n0 must be a positive multiple of blocking_factor (L39)");
+    if (((long long)p.n0[d] << (p.n_levels - 1)) > (1 << 24)) return fail(nullptr, SLEDGE_EINVAL, "finest level index space too large");
+  }
+  P.esz = p.dtype == SLEDGE_F64 ? 8 : 4;
+  P.cpa = 128 / (2 * P.esz);
+  P.ox = (p.nghost + P.cpa - 1) / P.cpa * P.cpa;
+  const int g = p.nghost, bfs = ilog2(bf);
+  P.lev.assign(p.n_levels, LevelHost());
+  for (int l = 0; l < p.n_levels; ++l) {
+    LevelHost& L = P.lev[l];
+    for (int d = 0; d < 3; ++d) {
+      L.n[d] = p.n0[d] << l;
+      L.no[d] = L.n[d] / bf;
+      L.nb[d] = (L.n[d] + COUNT_BLOCK - 1) / COUNT_BLOCK;
+    }
+    L.h = p.h0 / (double)(1 << l);  // Eq.1
+    L.owner.assign((size_t)L.no[0] * L.no[1] * L.no[2], -1);
+    L.count_blocks = (long long)L.nb[0] * L.nb[1] * L.nb[2];
+  }
+  P.box.assign(boxes, boxes + nbox);
+  P.box_local.assign(nbox, -1);
+  size_t max_box_cells = 0;
+  for (int ib = 0; ib < nbox; ++ib) {
+    const sledge_box& B = boxes[ib];
+    if (B.level < 0 || B.level >= p.n_levels) return fail(nullptr, SLEDGE_EINVAL, "box %d: level out of range", ib);
+    LevelHost& L = P.lev[B.level];
+    BoxDev bd;
+    for (int d = 0; d < 3; ++d) {
+      const int n = B.hi[d] - B.lo[d] + 1;
+      if (B.lo[d] < 0 || B.hi[d] >= L.n[d] || n <= 0 || B.lo[d] % bf || n % bf)
+        return fail(nullptr, SLEDGE_EINVAL, "box %d: outside the domain or not aligned to the blocking factor (L39)", ib);
+      bd.n[d] = n;
+      bd.lo[d] = B.lo[d];
+    }
+    const int li = (int)L.boxes.size();
+    for (int k = B.lo[2] >> bfs; k <= B.hi[2] >> bfs; ++k)
+      for (int j = B.lo[1] >> bfs; j <= B.hi[1] >> bfs; ++j)
+        for (int i = B.lo[0] >> bfs; i <= B.hi[0] >> bfs; ++i) {
+          int& ow = L.owner[((size_t)k * L.no[1] + j) * L.no[0] + i];
+          if (ow != -1) return fail(nullptr, SLEDGE_EINVAL, "box %d overlaps box %d of level %d", ib, L.boxes[ow], B.level);
+          ow = li;
+        }
+    // row: [0, ox) left pad + ghosts, [ox, ox+n) valid, then >= g ghosts, pitch a multiple of 128 bytes
+    bd.sx = (P.ox + bd.n[0] + g + P.cpa - 1) / P.cpa * P.cpa;
+    bd.sy = bd.n[1] + 2 * g;
+    bd.base = L.plane_cells;
+    bd.tag_base = L.valid_cells;
+    L.plane_cells += (long long)bd.sx * bd.sy * (bd.n[2] + 2 * g);
+    L.valid_cells += (long long)bd.n[0] * bd.n[1] * bd.n[2];
+    max_box_cells = std::max(max_box_cells, (size_t)(bd.n[0] + 2 * g) * (bd.n[1] + 2 * g) * (bd.n[2] + 2 * g));
+    P.box_local[ib] = li;
+    L.boxes.push_back(ib);
+    L.boxdev.push_back(bd);
+  }
+  for (size_t q = 0; q < P.lev[0].owner.size(); ++q)
+    if (P.lev[0].owner[q] < 0) return fail(nullptr, SLEDGE_EINVAL, "level 0 must cover the whole domain (L39)");
+  // proper nesting (L70, L137): a fine box grown by one blocking factor (fine cells) lies on valid coarse cells
+  for (int l = 1; l < p.n_levels; ++l) {
+    const LevelHost& L = P.lev[l];
+    const LevelHost& C = P.lev[l - 1];
+    if (L.boxes.empty()) return fail(nullptr, SLEDGE_EINVAL, "level %d has no boxes", l);
+    for (size_t q = 0; q < L.boxes.size(); ++q) {
+      const BoxDev& b = L.boxdev[q];
+      // coarse cells touched by the grown box; owner granularity is bf coarse cells
+      int clo[3], chi[3];
+      for (int d = 0; d < 3; ++d) {
+        clo[d] = fdiv2(b.lo[d] - bf);
+        chi[d] = fdiv2(b.lo[d] + b.n[d] - 1 + bf);
+      }
+      for (int k = clo[2] >> bfs; k <= chi[2] >> bfs; ++k)
+        for (int j = clo[1] >> bfs; j <= chi[1] >> bfs; ++j)
+          for (int i = clo[0] >> bfs; i <= chi[0] >> bfs; ++i) {
+            const int wi = ((i % C.no[0]) + C.no[0]) % C.no[0];
+            const int wj = ((j % C.no[1]) + C.no[1]) % C.no[1];
+            const int wk = ((k % C.no[2]) + C.no[2]) % C.no[2];
+            if (C.owner[((size_t)wk * C.no[1] + wj) * C.no[0] + wi] < 0)
+              return fail(nullptr, SLEDGE_EINVAL, "box %d violates proper nesting: gap to the level-%d boundary < blocking factor (L70, L137)",
+                          L.boxes[q], l - 1);
+          }
+    }
+  }
+  // work tables
+  const int cpt = p.dtype == SLEDGE_F64 ? 1 : 2;
+  for (int l = 0; l < p.n_levels; ++l) {
+    LevelHost& L = P.lev[l];
+    L.ghost_prefix.assign(1, 0);
+    L.avg_prefix.assign(1, 0);
+    for (size_t q = 0; q < L.boxdev.size(); ++q) {
+      const BoxDev& b = L.boxdev[q];
+      const int txc = K1_TX * cpt;
+      for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
+        for (int y0 = 0; y0 < b.n[1]; y0 += K1_TY)
+          for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
+      for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
+        for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
+          for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
+      const long long Gx = b.n[0] + 2 * g, Gy = b.n[1] + 2 * g;
+      const long long nghost = Gx * Gy * 2 * g + Gx * 2 * g * b.n[2] + 2LL * g * b.n[1] * b.n[2];
+      L.ghost_prefix.push_back(L.ghost_prefix.back() + (int)((nghost + GHOST_THREADS - 1) / GHOST_THREADS));
+      const long long ncoarse = (long long)(b.n[0] / 2) * (b.n[1] / 2) * (b.n[2] / 2);
+      L.avg_prefix.push_back(L.avg_prefix.back() + (int)((ncoarse + AVG_THREADS - 1) / AVG_THREADS));
+    }
+  }
+  // arena layout
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    const size_t o = off;
+    off = align_up(off + bytes, ALIGN);
+    return o;
+  };
+  for (int l = 0; l < p.n_levels; ++l) {
+    LevelHost& L = P.lev[l];
+    const size_t plane_bytes = (size_t)L.plane_cells * 2 * P.esz;
+    for (int b = 0; b < NBUF; ++b)
+      for (int c = 0; c < 2; ++c) L.off_buf[b][c] = take(plane_bytes);
+    L.off_boxes = take(L.boxdev.size() * sizeof(BoxDev));
+    L.off_tiles = take(L.tiles.size() * sizeof(TileDev));
+    L.off_tag_tiles = take(L.tag_tiles.size() * sizeof(TileDev));
+    L.off_owner = take(L.owner.size() * sizeof(int));
+    L.off_ghost_prefix = take(L.ghost_prefix.size() * sizeof(int));
+    L.off_avg_prefix = take(L.avg_prefix.size() * sizeof(int));
+  }
+  P.scratch_bytes = max_box_cells * P.esz;
+  P.off_scratch = take(P.scratch_bytes);
+  P.off_err = take(sizeof(int));
+  P.total = off;
+  return SLEDGE_OK;
+}
+
+}  // namespace
+
+// ---- launch plumbing ---------------------------------------------------------------------------
+namespace {
+
+enum Kind { KIND_STAGE = 0, KIND_GHOST = 1, KIND_TAG = 2, KIND_AVG = 3 };
+
+struct Timed {  // brackets a launch with an event pair while profiling is on
+  sledge_ctx* c;
+  int kind;
+  cudaEvent_t stop = nullptr;
+  Timed(sledge_ctx* ctx, int k) : c(ctx), kind(k) {
+    ++c->launches;
+    if (!c->profiling || c->ev_used[k] >= MAX_EVENT_PAIRS) return;
+    if (c->ev_used[k] == c->ev[k].size()) {
+      cudaEvent_t a, b;
+      cudaEventCreate(&a);
+      cudaEventCreate(&b);
+      c->ev[k].push_back({a, b});
+    }
+    cudaEventRecord(c->ev[k][c->ev_used[k]].first, c->stream);
+    stop = c->ev[k][c->ev_used[k]].second;
+    ++c->ev_used[k];
+  }
+  ~Timed() {
+    if (stop) cudaEventRecord(stop, c->stream);
+  }
+};
+
+int check_launch(sledge_ctx* c, const char* what) {
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+  return SLEDGE_OK;
+}
+
+template <typename T> typename PairOf<T>::type* plane_ptr(sledge_ctx* c, int l, int buf, int which) {
+  return reinterpret_cast<typename PairOf<T>::type*>(c->arena + c->plan.lev[l].off_buf[buf & 3][which]);
+}
+template <typename U> U* tab(sledge_ctx* c, size_t off) { return reinterpret_cast<U*>(c->arena + off); }
+
+LevelGeom geom_of(const Plan& P, int l) {
+  const LevelHost& L = P.lev[l];
+  LevelGeom gm;
+  for (int d = 0; d < 3; ++d) {
+    gm.n[d] = L.n[d];
+    gm.no[d] = L.no[d];
+  }
+  gm.bf_shift = ilog2(P.p.blocking_factor);
+  gm.g = P.p.nghost;
+  gm.ox = P.ox;
+  return gm;
+}
+
+// K2 on buffer `buf` of level l, whose data is at time `time`
+template <typename T>
+int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  GhostArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.boxes = tab<BoxDev>(c, L.off_boxes);
+  a.blk_prefix = tab<int>(c, L.off_ghost_prefix);
+  a.nbox = (int)L.boxdev.size();
+  a.psi = plane_ptr<T>(c, l, buf, 0);
+  a.pi = plane_ptr<T>(c, l, buf, 1);
+  a.owner = tab<int>(c, L.off_owner);
+  a.geom = geom_of(P, l);
+  a.err_flag = tab<int>(c, P.off_err);
+  a.has_coarse = l > 0;
+  a.alpha = T(0);
+  if (l > 0) {
+    LevelHost& C = P.lev[l - 1];
+    a.cboxes = tab<BoxDev>(c, C.off_boxes);
+    a.cowner = tab<int>(c, C.off_owner);
+    a.cgeom = geom_of(P, l - 1);
+    int bo = C.cur, bn = C.cur;
+    double alpha = 0.0;
+    if (C.have_pair && C.t_new != C.t_old) {  // linear in time between the coarse old and new states (L72)
+      alpha = (time - C.t_old) / (C.t_new - C.t_old);
+      bo = C.old;
+    }
+    a.alpha = (T)alpha;
+    a.c_old_psi = plane_ptr<T>(c, l - 1, bo, 0);
+    a.c_new_psi = plane_ptr<T>(c, l - 1, bn, 0);
+    a.c_old_pi = plane_ptr<T>(c, l - 1, bo, 1);
+    a.c_new_pi = plane_ptr<T>(c, l - 1, bn, 1);
+  }
+  const int grid = L.ghost_prefix.back();
+  if (grid == 0) return SLEDGE_OK;
+  {
+    Timed t(c, KIND_GHOST);
+    if (fill_pi) k_fill_ghosts<T, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+    else k_fill_ghosts<T, false><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+  }
+  return check_launch(c, "k_fill_ghosts");
+}
+
+template <typename T, int ORDER, int MODE>
+void launch_stage_kernel(sledge_ctx* c, const StageArgs<T>& a, int grid) {
+  k_rk_stage<T, ORDER, MODE, K1_TX, K1_TY><<<grid, K1_TX * K1_TY, 0, c->stream>>>(a);
+}
+template <typename T, int ORDER>
+void launch_stage_mode(sledge_ctx* c, const StageArgs<T>& a, int grid, int mode) {
+  switch (mode) {
+    case LEAN_S1: launch_stage_kernel<T, ORDER, LEAN_S1>(c, a, grid); break;
+    case LEAN_S23: launch_stage_kernel<T, ORDER, LEAN_S23>(c, a, grid); break;
+    case LEAN_S4: launch_stage_kernel<T, ORDER, LEAN_S4>(c, a, grid); break;
+    case CLASSIC_S1: launch_stage_kernel<T, ORDER, CLASSIC_S1>(c, a, grid); break;
+    case CLASSIC_S23: launch_stage_kernel<T, ORDER, CLASSIC_S23>(c, a, grid); break;
+    default: launch_stage_kernel<T, ORDER, CLASSIC_S4>(c, a, grid); break;
+  }
+}
+
+// One RK4 stage of level l: ghost fill of the stage input at its time, then K1.
+// t = time at the start of the level's step, eta_const = eta used when eta_fixed.
+template <typename T>
+int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
+  static const double as[4] = {0.5, 0.5, 1.0, 1.0 / 6.0};
+  const double ts = t + cs[s] * dt;
+  const double eta_s = P.p.eta_fixed ? eta_const : ts;
+  const int cur = L.cur;
+  const bool lean = P.p.rk_dataflow == SLEDGE_RK_LEAN;
+  int ubuf, mode, in[3] = {-1, -1, -1}, out[2] = {-1, -1};
+  double adt = (s < 3) ? as[s] * dt : dt / 6.0, bdt = 0.0;
+  if (lean) {  // buffers: cur = Y, cur+1 = U2 (then Ynew), cur+2 = U3, cur+3 = U4
+    if (s == 0) { ubuf = cur; mode = LEAN_S1; out[0] = cur + 1; }
+    else if (s == 1) { ubuf = cur + 1; mode = LEAN_S23; in[0] = cur; out[0] = cur + 2; }
+    else if (s == 2) { ubuf = cur + 2; mode = LEAN_S23; in[0] = cur; out[0] = cur + 3; }
+    else { ubuf = cur + 3; mode = LEAN_S4; in[0] = cur; in[1] = cur + 1; in[2] = cur + 2; out[0] = cur + 1; }
+  } else {  // buffers: cur = Y, cur+1 = ACC (then Ynew), cur+2 = Ua, cur+3 = Ub
+    if (s == 0) { ubuf = cur; mode = CLASSIC_S1; out[0] = cur + 2; out[1] = cur + 1; bdt = dt / 6.0; }
+    else if (s == 1) { ubuf = cur + 2; mode = CLASSIC_S23; in[0] = cur; in[1] = cur + 1; out[0] = cur + 3; out[1] = cur + 1; bdt = dt / 3.0; }
+    else if (s == 2) { ubuf = cur + 3; mode = CLASSIC_S23; in[0] = cur; in[1] = cur + 1; out[0] = cur + 2; out[1] = cur + 1; bdt = dt / 3.0; }
+    else { ubuf = cur + 2; mode = CLASSIC_S4; in[0] = cur + 1; out[0] = cur + 1; }
+  }
+  int rc = launch_ghosts<T>(c, l, ubuf, ts, false);
+  if (rc) return rc;
+  StageArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.boxes = tab<BoxDev>(c, L.off_boxes);
+  a.tiles = tab<TileDev>(c, L.off_tiles);
+  a.u_psi = plane_ptr<T>(c, l, ubuf, 0);
+  a.u_pi = plane_ptr<T>(c, l, ubuf, 1);
+  for (int q = 0; q < 3; ++q)
+    if (in[q] >= 0) {
+      a.in_psi[q] = plane_ptr<T>(c, l, in[q], 0);
+      a.in_pi[q] = plane_ptr<T>(c, l, in[q], 1);
+    }
+  for (int q = 0; q < 2; ++q)
+    if (out[q] >= 0) {
+      a.out_psi[q] = plane_ptr<T>(c, l, out[q], 0);
+      a.out_pi[q] = plane_ptr<T>(c, l, out[q], 1);
+    }
+  a.g = P.p.nghost;
+  a.ox = P.ox;
+  const double h2 = L.h * L.h;
+  a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : 1.0 / (12.0 * h2));
+  a.lam_eta2 = (T)(P.p.lambda * (eta_s * eta_s));
+  a.a_mass = (T)P.p.a_mass;
+  a.fric = (T)(P.p.friction != 0.0 ? P.p.friction / eta_s : 0.0);
+  a.adt = (T)adt;
+  a.bdt = (T)bdt;
+  const int grid = (int)L.tiles.size();
+  {
+    Timed tm(c, KIND_STAGE);
+    if (P.p.lap_order == 1) launch_stage_mode<T, 1>(c, a, grid, mode);
+    else launch_stage_mode<T, 2>(c, a, grid, mode);
+  }
+  rc = check_launch(c, "k_rk_stage");
+  if (rc) return rc;
+  if (s == 3) {  // the new state becomes current; the previous one is kept as `old` (L72)
+    L.old = cur & 3;
+    L.cur = (cur + 1) & 3;
+    L.t_old = t;
+    L.t_new = t + dt;
+    L.have_pair = true;
+  }
+  return SLEDGE_OK;
+}
+
+template <typename T>
+int do_average_down(sledge_ctx* c, int lf) {
+  Plan& P = c->plan;
+  LevelHost& F = P.lev[lf];
+  LevelHost& C = P.lev[lf - 1];
+  AvgArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.fboxes = tab<BoxDev>(c, F.off_boxes);
+  a.blk_prefix = tab<int>(c, F.off_avg_prefix);
+  a.nfbox = (int)F.boxdev.size();
+  a.f_psi = plane_ptr<T>(c, lf, F.cur, 0);
+  a.f_pi = plane_ptr<T>(c, lf, F.cur, 1);
+  a.fgeom = geom_of(P, lf);
+  a.cboxes = tab<BoxDev>(c, C.off_boxes);
+  a.cowner = tab<int>(c, C.off_owner);
+  a.cgeom = geom_of(P, lf - 1);
+  a.c_psi = plane_ptr<T>(c, lf - 1, C.cur, 0);
+  a.c_pi = plane_ptr<T>(c, lf - 1, C.cur, 1);
+  a.err_flag = tab<int>(c, P.off_err);
+  const int grid = F.avg_prefix.back();
+  {
+    Timed t(c, KIND_AVG);
+    k_average_down<T><<<grid, AVG_THREADS, 0, c->stream>>>(a);
+  }
+  return check_launch(c, "k_average_down");
+}
+
+// O6 / L66-76, Fig.2: level l one step, then level l+1 two half steps, then synchronise.
+template <typename T>
+int advance(sledge_ctx* c, int l, double t, double dt, double eta_const) {
+  for (int s = 0; s < 4; ++s) {
+    const int rc = do_stage<T>(c, l, s, t, dt, eta_const);
+    if (rc) return rc;
+  }
+  if (l + 1 < c->plan.p.n_levels) {
+    int rc = advance<T>(c, l + 1, t, 0.5 * dt, eta_const);
+    if (rc) return rc;
+    rc = advance<T>(c, l + 1, t + 0.5 * dt, 0.5 * dt, eta_const);
+    if (rc) return rc;
+    rc = do_average_down<T>(c, l + 1);
+    if (rc) return rc;
+  }
+  return SLEDGE_OK;
+}
+
+template <typename T>
+int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  // after a coarse step every level sits at its parent's t_new: alpha = 1, no temporal interpolation (L74)
+  const double tcur = (l > 0 && P.lev[l - 1].have_pair) ? P.lev[l - 1].t_new : 0.0;
+  int rc = launch_ghosts<T>(c, l, L.cur, tcur, false);
+  if (rc) return rc;
+  if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)L.count_blocks, c->stream);
+  TagArgs<T> a;
+  a.boxes = tab<BoxDev>(c, L.off_boxes);
+  a.tiles = tab<TileDev>(c, L.off_tag_tiles);
+  a.psi = plane_ptr<T>(c, l, L.cur, 0);
+  a.tags = tags;
+  a.counts = counts;
+  a.g = P.p.nghost;
+  a.ox = P.ox;
+  a.nb0 = L.nb[0];
+  a.nb1 = L.nb[1];
+  {
+    Timed t(c, KIND_TAG);
+    k_tag_strings<T><<<(int)L.tag_tiles.size(), TAG_TX * TAG_TY, 0, c->stream>>>(a);
+  }
+  return check_launch(c, "k_tag_strings");
+}
+
+template <typename T>
+int do_copy_comp(sledge_ctx* c, int ib, int comp, void* dense, bool to_state, bool with_ghosts) {
+  Plan& P = c->plan;
+  const int l = P.box[ib].level;
+  LevelHost& L = P.lev[l];
+  const BoxDev& b = L.boxdev[P.box_local[ib]];
+  const int e = with_ghosts ? P.p.nghost : 0;
+  const long long total = (long long)(b.n[0] + 2 * e) * (b.n[1] + 2 * e) * (b.n[2] + 2 * e);
+  const int grid = (int)std::min<long long>((total + 255) / 256, 148 * 32);
+  auto* pl = plane_ptr<T>(c, l, L.cur, comp >> 1);
+  ++c->launches;
+  if (to_state) k_copy_comp<T, true><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
+  else k_copy_comp<T, false><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
+  return check_launch(c, "k_copy_comp");
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI (include/sledge.h)
+// =================================================================================================
+#define DISPATCH(ctx, call_f32, call_f64) ((ctx)->plan.p.dtype == SLEDGE_F64 ? (call_f64) : (call_f32))
+
+extern "C" {
+
+int sledge_arena_bytes(const sledge_params* params, const sledge_box* boxes, int nbox, size_t* bytes) {
+  Plan P;
+  const int rc = make_plan(P, params, boxes, nbox);
+  if (rc) return rc;
+  if (bytes) *bytes = P.total;
+  return SLEDGE_OK;
+}
+
+int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_box* boxes, int nbox, void* dev_arena,
+                  size_t arena_bytes, void* cuda_stream) {
+  if (!out) return fail(nullptr, SLEDGE_EINVAL, "ctx output pointer is null");
+  *out = nullptr;
+  sledge_ctx* c = new sledge_ctx();
+  int rc = make_plan(c->plan, params, boxes, nbox);
+  if (rc) {
+    delete c;
+    return rc;
+  }
+  Plan& P = c->plan;
+  if (!dev_arena || ((uintptr_t)dev_arena % ALIGN) || arena_bytes < P.total) {
+    rc = fail(nullptr, SLEDGE_ENOMEM, "arena null, not 256-byte aligned or too small (%zu bytes needed, %zu given)", P.total,
+              arena_bytes);
+    delete c;
+    return rc;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    delete c;
+    return fail(nullptr, SLEDGE_ECUDA, "no CUDA device: libsledge has no CPU fallback");
+  }
+  c->arena = (char*)dev_arena;
+  c->stream = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaMemsetAsync(c->arena, 0, P.total, c->stream);
+  auto up = [&](size_t off, const void* src, size_t bytes) {
+    if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(c->arena + off, src, bytes, cudaMemcpyHostToDevice, c->stream);
+  };
+  for (LevelHost& L : P.lev) {
+    up(L.off_boxes, L.boxdev.data(), L.boxdev.size() * sizeof(BoxDev));
+    up(L.off_tiles, L.tiles.data(), L.tiles.size() * sizeof(TileDev));
+    up(L.off_tag_tiles, L.tag_tiles.data(), L.tag_tiles.size() * sizeof(TileDev));
+    up(L.off_owner, L.owner.data(), L.owner.size() * sizeof(int));
+    up(L.off_ghost_prefix, L.ghost_prefix.data(), L.ghost_prefix.size() * sizeof(int));
+    up(L.off_avg_prefix, L.avg_prefix.data(), L.avg_prefix.size() * sizeof(int));
+  }
+  // the tables above are pageable host memory: make sure the copies are done before they can go away
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) {
+    rc = fail(nullptr, SLEDGE_ECUDA, "sledge_create: %s", cudaGetErrorString(e));
+    delete c;
+    return rc;
+  }
+  *out = c;
+  return SLEDGE_OK;
+}
+
+int sledge_destroy(sledge_ctx* c) {
+  if (!c) return SLEDGE_OK;
+  cudaStreamSynchronize(c->stream);
+  for (auto& v : c->ev)
+    for (auto& pr : v) {
+      cudaEventDestroy(pr.first);
+      cudaEventDestroy(pr.second);
+    }
+  delete c;
+  return SLEDGE_OK;
+}
+
+static int check_box_comp(sledge_ctx* c, int box, int comp, const void* ptr) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  if (box < 0 || box >= (int)c->plan.box.size()) return fail(c, SLEDGE_EINVAL, "box index %d out of range", box);
+  if (comp < 0 || comp > 3) return fail(c, SLEDGE_EINVAL, "component %d out of range (0..3)", comp);
+  if (!ptr) return fail(c, SLEDGE_EINVAL, "null data pointer");
+  return SLEDGE_OK;
+}
+
+int sledge_set_state(sledge_ctx* c, int box, int comp, const void* dev_src) {
+  int rc = check_box_comp(c, box, comp, dev_src);
+  if (rc) return rc;
+  c->plan.lev[c->plan.box[box].level].have_pair = false;
+  return DISPATCH(c, do_copy_comp<float>(c, box, comp, (void*)dev_src, true, false),
+                  do_copy_comp<double>(c, box, comp, (void*)dev_src, true, false));
+}
+
+int sledge_get_state(sledge_ctx* c, int box, int comp, void* dev_dst) {
+  int rc = check_box_comp(c, box, comp, dev_dst);
+  if (rc) return rc;
+  return DISPATCH(c, do_copy_comp<float>(c, box, comp, dev_dst, false, false),
+                  do_copy_comp<double>(c, box, comp, dev_dst, false, false));
+}
+
+int sledge_get_ghosted(sledge_ctx* c, int box, int comp, void* dev_dst) {
+  int rc = check_box_comp(c, box, comp, dev_dst);
+  if (rc) return rc;
+  return DISPATCH(c, do_copy_comp<float>(c, box, comp, dev_dst, false, true),
+                  do_copy_comp<double>(c, box, comp, dev_dst, false, true));
+}
+
+static size_t box_valid_bytes(sledge_ctx* c, int box) {
+  const sledge_box& B = c->plan.box[box];
+  return (size_t)(B.hi[0] - B.lo[0] + 1) * (B.hi[1] - B.lo[1] + 1) * (B.hi[2] - B.lo[2] + 1) * c->plan.esz;
+}
+
+int sledge_set_state_host(sledge_ctx* c, int box, int comp, const void* host_src) {
+  int rc = check_box_comp(c, box, comp, host_src);
+  if (rc) return rc;
+  void* scratch = c->arena + c->plan.off_scratch;
+  const cudaError_t e = cudaMemcpyAsync(scratch, host_src, box_valid_bytes(c, box), cudaMemcpyHostToDevice, c->stream);
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "set_state_host: %s", cudaGetErrorString(e));
+  return sledge_set_state(c, box, comp, scratch);
+}
+
+int sledge_get_state_host(sledge_ctx* c, int box, int comp, void* host_dst) {
+  int rc = check_box_comp(c, box, comp, host_dst);
+  if (rc) return rc;
+  void* scratch = c->arena + c->plan.off_scratch;
+  rc = sledge_get_state(c, box, comp, scratch);
+  if (rc) return rc;
+  const cudaError_t e = cudaMemcpyAsync(host_dst, scratch, box_valid_bytes(c, box), cudaMemcpyDeviceToHost, c->stream);
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "get_state_host: %s", cudaGetErrorString(e));
+  return SLEDGE_OK;
+}
+
+static int check_level(sledge_ctx* c, int level) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  if (level < 0 || level >= c->plan.p.n_levels) return fail(c, SLEDGE_EINVAL, "level %d out of range", level);
+  return SLEDGE_OK;
+}
+
+int sledge_fill_ghosts(sledge_ctx* c, int level, double time) {
+  int rc = check_level(c, level);
+  if (rc) return rc;
+  const int cur = c->plan.lev[level].cur;
+  return DISPATCH(c, launch_ghosts<float>(c, level, cur, time, true), launch_ghosts<double>(c, level, cur, time, true));
+}
+
+int sledge_rk_stage(sledge_ctx* c, int level, int stage, double dt, double eta) {
+  int rc = check_level(c, level);
+  if (rc) return rc;
+  if (stage < 0 || stage > 3) return fail(c, SLEDGE_EINVAL, "stage must be 0..3");
+  return DISPATCH(c, do_stage<float>(c, level, stage, eta, dt, eta), do_stage<double>(c, level, stage, eta, dt, eta));
+}
+
+int sledge_rk_step(sledge_ctx* c, double dt, double eta) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  if (!(dt > 0)) return fail(c, SLEDGE_EINVAL, "dt must be positive");
+  return DISPATCH(c, advance<float>(c, 0, eta, dt, eta), advance<double>(c, 0, eta, dt, eta));
+}
+
+int sledge_tag_strings(sledge_ctx* c, int level, uint8_t* dev_tags, uint32_t* dev_counts) {
+  int rc = check_level(c, level);
+  if (rc) return rc;
+  return DISPATCH(c, do_tag<float>(c, level, dev_tags, dev_counts), do_tag<double>(c, level, dev_tags, dev_counts));
+}
+
+int sledge_average_down(sledge_ctx* c, int fine_level) {
+  int rc = check_level(c, fine_level);
+  if (rc) return rc;
+  if (fine_level < 1) return fail(c, SLEDGE_EINVAL, "average_down needs fine_level >= 1");
+  return DISPATCH(c, do_average_down<float>(c, fine_level), do_average_down<double>(c, fine_level));
+}
+
+int sledge_level_cells(const sledge_ctx* c, int level, int64_t* valid_cells, int64_t* count_blocks) {
+  if (!c || level < 0 || level >= c->plan.p.n_levels) return SLEDGE_EINVAL;
+  if (valid_cells) *valid_cells = c->plan.lev[level].valid_cells;
+  if (count_blocks) *count_blocks = c->plan.lev[level].count_blocks;
+  return SLEDGE_OK;
+}
+
+int64_t sledge_launch_count(const sledge_ctx* c) { return c ? c->launches : 0; }
+
+int sledge_synchronize(sledge_ctx* c) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  int flag = 0;
+  if (e == cudaSuccess) e = cudaMemcpy(&flag, c->arena + c->plan.off_err, sizeof(int), cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "synchronize: %s", cudaGetErrorString(e));
+  if (flag) return fail(c, SLEDGE_ESTATE, "a kernel found a cell with neither a same-level owner nor coarse data (nesting)");
+  return SLEDGE_OK;
+}
+
+int sledge_profile_enable(sledge_ctx* c, int on) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  c->profiling = on != 0;
+  for (int k = 0; k < 4; ++k) c->ev_used[k] = 0;
+  return SLEDGE_OK;
+}
+
+int sledge_profile_read(sledge_ctx* c, int kind, int64_t* launches, double* total_ms) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  if (kind < 0 || kind > 3) return fail(c, SLEDGE_EINVAL, "kind must be 0..3");
+  const cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "profile_read: %s", cudaGetErrorString(e));
+  double ms = 0;
+  for (size_t q = 0; q < c->ev_used[kind]; ++q) {
+    float t = 0;
+    cudaEventElapsedTime(&t, c->ev[kind][q].first, c->ev[kind][q].second);
+    ms += t;
+  }
+  if (launches) *launches = (int64_t)c->ev_used[kind];
+  if (total_ms) *total_ms = ms;
+  return SLEDGE_OK;
+}
+
+const char* sledge_last_error(const sledge_ctx* c) { return c ? c->err.c_str() : g_err.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,300 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): fp64 max abs field error <= 1e-11 after the configured number of steps;
+fp32 max relative error <= 2e-5; string tags and box counts bit-exact when both sides tag the same state.
+Sizes: small enough for the oracle to finish in seconds, large enough to span several K1 tiles
+(32 x 8 x 64 cells fp64, 64 x 8 x 64 fp32) and ragged tails."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2404_02950_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+F64_TOL = 1e-11
+F32_TOL = 2e-5
+
+
+def _pair():
+    import _pair as P  # tests/ is on sys.path (pytest rootdir conftest)
+    return P
+
+
+def _compare_tags(o, s, level):
+    P = _pair()
+    P.upload_oracle_state(o, s)
+    ot, oc = o.tag_strings(level)
+    gt, gc = s.tag_strings(level)
+    s.synchronize()
+    gts = s.split_tags(level, gt)
+    for a, b in zip(ot, gts):
+        assert np.array_equal(a, b.cpu().numpy())
+    assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
+    return sum(int((a != 0).sum()) for a in ot)
+
+
+# ---- C1: the small BASELINE.json config, full length -------------------------------------------------
+
+@pytest.mark.parametrize("flow", ["lean", "classic"])
+def test_c1_32cubed_10_steps_with_tags(flow):
+    P = _pair()
+    cfg = inputs.CONFIGS["C1"]
+    o, s = P.make_pair(cfg.n0, nghost=cfg.nghost, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=flow)
+    P.init_grf(o, s, cfg.n0, cfg.grf_f, cfg.seeds)
+    eta = cfg.eta0
+    n_tagged = 0
+    for step in range(cfg.steps):
+        o.rk_step(cfg.dt, eta)
+        s.rk_step(cfg.dt, eta)
+        eta += cfg.dt
+        assert P.max_err(o, s) <= F64_TOL, f"step {step}"
+        # free-running tags (information): both sides tag their own state
+        ot, oc = o.tag_strings(0)
+        gt, gc = s.tag_strings(0)
+        assert np.array_equal(ot[0], s.split_tags(0, gt)[0].cpu().numpy())
+        assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
+        n_tagged += int((ot[0] != 0).sum())
+    assert eta == pytest.approx(3.5)
+    assert n_tagged > 0  # the GRF does contain strings
+    s.synchronize()
+
+
+# ---- ragged single-level grids, several boxes, both stencils, friction and mass terms -----------------
+
+def _ragged_boxes():
+    # 40 x 24 x 72 domain cut into boxes of different sizes (bf = 8): exercises partial K1 tiles in x and y,
+    # same-level ghost copies across box faces/edges/corners and the periodic wrap, and two z chunks.
+    return [
+        (0, (0, 0, 0), (31, 15, 71)),
+        (0, (32, 0, 0), (39, 15, 71)),
+        (0, (0, 16, 0), (39, 23, 39)),
+        (0, (0, 16, 40), (15, 23, 71)),
+        (0, (16, 16, 40), (39, 23, 71)),
+    ]
+
+
+@pytest.mark.parametrize("order,g", [(1, 1), (1, 3), (2, 2), (2, 3)])
+@pytest.mark.parametrize("flow", ["lean", "classic"])
+def test_ragged_multibox_fp64(order, g, flow):
+    P = _pair()
+    n0 = (40, 24, 72)
+    o, s = P.make_pair(n0, boxes=_ragged_boxes(), nghost=g, lap_order=order, h0=0.5, lam=0.7, a_mass=0.3,
+                       friction=2.0, rk_dataflow=flow)
+    P.init_smooth(o, s, n0, seed=11)
+    eta, dt = 1.5, 0.1
+    for _ in range(4):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    _compare_tags(o, s, 0)
+
+
+def test_eta_fixed_minkowski_variant():
+    P = _pair()
+    o, s = P.make_pair(16, nghost=2, lap_order=2, h0=0.25, eta_fixed=True)
+    P.init_smooth(o, s, 16, seed=5)
+    for q in range(3):
+        o.rk_step(0.05, 2.0)
+        s.rk_step(0.05, 2.0)
+    assert P.max_err(o, s) <= F64_TOL
+
+
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2)])
+def test_fp32_relative_error(order, g):
+    P = _pair()
+    n = 64
+    o, s = P.make_pair(n, nghost=g, lap_order=order, h0=0.125, dtype="f32")
+    P.init_grf(o, s, n, 0.25, (71, 72))
+    eta, dt = 1.0, 0.03125
+    for _ in range(20):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, relative=True) <= F32_TOL
+    # tags on the same (fp32-representable) state are bit-exact
+    assert _compare_tags(o, s, 0) > 0
+
+
+# ---- ghost fill ------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("g", [1, 2, 3])
+def test_ghost_fill_two_levels_matches_oracle_bitwise(g):
+    """Periodic wrap, same-level copy and coarse->fine trilinear interpolation (no time interpolation yet:
+    the coarse level has not stepped).  Same arithmetic order on both sides -> identical bits."""
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=1, h0=1.0)
+    P.init_smooth(o, s, n0, seed=3)
+    for l in (0, 1):
+        o.fill_ghosts(l, 0.0)
+        s.fill_ghosts(l, 0.0)
+    s.synchronize()
+    for ib in range(len(boxes)):
+        for c in range(4):
+            a = o.get_raw(ib, c)
+            b = s.get_ghosted(ib, c).cpu().numpy()
+            assert np.array_equal(a, b), (ib, c)
+
+
+def test_ghost_fill_time_interpolation():
+    """After a coarse step the fine ghosts at an intermediate time are (1-alpha) old + alpha new (L72)."""
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=2, lap_order=2, h0=0.5)
+    P.init_smooth(o, s, n0, seed=4)
+    o.rk_step(0.1, 1.0)
+    s.rk_step(0.1, 1.0)
+    for time in (1.0, 1.025, 1.05, 1.1):
+        o.fill_ghosts(1, time)
+        s.fill_ghosts(1, time)
+        for ib in s.level_boxes(1):
+            for c in range(4):
+                a = o.get_raw(ib, c)
+                b = s.get_ghosted(ib, c).cpu().numpy()
+                assert np.abs(a - b).max() <= F64_TOL, (time, ib, c)
+    s.synchronize()
+
+
+# ---- average-down ------------------------------------------------------------------------------------
+
+def test_average_down_matches_oracle_bitwise():
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=1, h0=1.0)
+    P.init_smooth(o, s, n0, seed=8)
+    o.average_down(1)
+    s.average_down(1)
+    s.synchronize()
+    for c in range(4):
+        a = o.get_state(0, c)
+        b = s.get_state(0, c).cpu().numpy()
+        assert np.array_equal(a, b)
+    # something was actually overwritten
+    assert not np.array_equal(o.get_state(0, 0), P.smooth_field(((0, 0, 0), (31, 31, 31)), 0, (32,) * 3, 80))
+
+
+# ---- AMR with subcycling ---------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("flow", ["lean", "classic"])
+def test_two_level_subcycled_steps(flow):
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=3, lap_order=2, h0=0.5, rk_dataflow=flow)
+    P.init_smooth(o, s, n0, seed=9, comps=(0, 1))
+    eta, dt = 2.0, 0.1
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    for l in (0, 1):
+        _compare_tags(o, s, l)
+
+
+def _ring_hierarchy(n0=32, box=16, n_levels=3):
+    rings = inputs.make_rings(n0, 2, 5.0, 9.0, 1.5, seed=77)
+    boxes, cover = inputs.amr_boxes_for_rings(rings, n_levels=n_levels, box=box, r1=3.0, r2=1.0, blocking_factor=8)
+    return rings, boxes, cover
+
+
+def test_three_level_ring_hierarchy_like_c5():
+    """Small version of BASELINE.json config 5: vortex rings, 3 levels, boxes of one size placed around the
+    ring curves, 13-point stencil, 3 ghost cells, subcycling 1/2/4, average-down after every fine pair."""
+    P = _pair()
+    n0 = 32
+    rings, boxes, cover = _ring_hierarchy(n0)
+    assert 0 < cover[2] < cover[1] < 1
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.25)
+    for ib, (l, lo, hi) in enumerate(boxes):
+        re, im = inputs.ring_field(rings, l, lo, hi)
+        P.set_both(o, s, ib, 0, re.numpy())
+        P.set_both(o, s, ib, 1, im.numpy())
+    eta, dt = 2.0, 0.0625
+    for _ in range(2):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    s.synchronize()
+    assert P.max_err(o, s) <= F64_TOL
+    total = 0
+    for l in range(3):
+        total += _compare_tags(o, s, l)
+    assert total > 0
+
+
+def test_fully_covered_level1_equals_uniform_fine_run_on_gpu():
+    """Bookkeeping identity: a hierarchy whose level 1 covers the whole domain reproduces on
+    level 1 the single-level 2N run with dt/2, bit for bit -- GPU against GPU, no oracle involved."""
+    from paper_2404_02950_b200.sledge import Sledge
+    P = _pair()
+    n0, g = 16, 2
+    boxes = [(0, (0, 0, 0), (15, 15, 15)), (1, (0, 0, 0), (31, 31, 31))]
+    two = Sledge(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=2, h0=0.5)
+    one = Sledge(2 * n0, nghost=g, lap_order=2, h0=0.25)
+    for c in range(2):
+        fine = torch.from_numpy(P.smooth_field(((0, 0, 0), (31, 31, 31)), 1, (n0,) * 3, 40 + c)).cuda().contiguous()
+        coarse = torch.nn.functional.avg_pool3d(fine[None, None], 2)[0, 0].contiguous()
+        two.set_state(0, c, coarse)
+        two.set_state(1, c, fine)
+        one.set_state(0, c, fine)
+    eta, dt = 1.0, 0.1
+    two.rk_step(dt, eta)
+    one.rk_step(dt / 2, eta)
+    one.rk_step(dt / 2, eta + dt / 2)
+    for c in range(4):
+        assert torch.equal(two.get_state(1, c), one.get_state(0, c))
+    two.synchronize()
+    one.synchronize()
+
+
+# ---- hooks and error paths -----------------------------------------------------------------------------
+
+def test_rk_stage_hook_equals_rk_step():
+    from paper_2404_02950_b200.sledge import Sledge
+    P = _pair()
+    a = Sledge(16, nghost=1, lap_order=1, h0=0.5)
+    b = Sledge(16, nghost=1, lap_order=1, h0=0.5)
+    for c in range(4):
+        f = torch.from_numpy(P.smooth_field(((0, 0, 0), (15, 15, 15)), 0, (16,) * 3, 60 + c)).cuda().contiguous()
+        a.set_state(0, c, f)
+        b.set_state(0, c, f)
+    a.rk_step(0.05, 1.0)
+    for st in range(4):
+        b.rk_stage(0, st, 0.05, 1.0)
+    for c in range(4):
+        assert torch.equal(a.get_state(0, c), b.get_state(0, c))
+    assert a.launch_count() > 0
+
+
+def test_host_buffer_roundtrip_and_profile_counters():
+    from paper_2404_02950_b200.sledge import Sledge, KIND_STAGE, KIND_GHOST
+    s = Sledge(16, nghost=1)
+    src = torch.randn(16, 16, 16, dtype=torch.float64).pin_memory()
+    dst = torch.empty(16, 16, 16, dtype=torch.float64).pin_memory()
+    s.set_state_host(0, 1, src)
+    s.get_state_host(0, 1, dst)
+    s.synchronize()
+    assert torch.equal(src, dst)
+    s.profile_enable(True)
+    s.rk_step(0.01, 1.0)
+    n, ms = s.profile_read(KIND_STAGE)
+    assert n == 4 and ms > 0
+    n, ms = s.profile_read(KIND_GHOST)
+    assert n == 4
+    s.profile_enable(False)
+
+
+def test_create_rejects_bad_arena():
+    import ctypes as C
+    from paper_2404_02950_b200 import sledge as S
+    p, arr, boxes, _ = S._marshal(16, None, 1, 1, 8, "f64", 1, 1.0, 1.0, 0.0, 0.0, False, "lean")
+    h = C.c_void_p()
+    buf = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    rc = S.lib().sledge_create(C.byref(h), C.byref(p), arr, 1, buf.data_ptr(), 1024, None)
+    assert rc == -2 and b"arena" in S.lib().sledge_last_error(None)
