@@ -102,6 +102,9 @@ __global__ void __launch_bounds__(TX* TY) k_rk_stage(const StageArgs<T> a) {
   const int tx = tid % TX, ty = tid / TX;
   const int x = t.x0 + tx * CPT, y = t.y0 + ty;
   const bool active = (x < b.n[0]) && (y < b.n[1]);
+  // in a partial tile the columns/rows just past the box edge are ghost cells that the edge cells need as
+  // +x / +y neighbours: threads sitting there still stream their psi column through shared memory
+  const bool loader = (x < b.n[0] + R) && (y < b.n[1] + R);
   const long long plane = (long long)b.sx * b.sy;
   const long long tile_org = b.base + (long long)(t.z0 + a.g) * plane + (long long)(t.y0 + a.g) * b.sx + (t.x0 + a.ox);
   long long off = tile_org + (long long)ty * b.sx + tx * CPT;  // this thread's cell in plane z0
@@ -136,13 +139,13 @@ __global__ void __launch_bounds__(TX* TY) k_rk_stage(const StageArgs<T> a) {
   V w[2 * R + 1];
 #pragma unroll
   for (int m = 0; m < 2 * R; ++m) {
-    if (active) w[m + 1] = ldg16_stream<T>(a.u_psi + off + (long long)(m - R) * plane);
+    if (loader) w[m + 1] = ldg16_stream<T>(a.u_psi + off + (long long)(m - R) * plane);
   }
   // prefetch registers for the first plane
   V n_psi, n_upi, n_in_psi[NIN > 0 ? NIN : 1], n_in_pi[NIN > 0 ? NIN : 1];
   P n_halo[HPT];
+  if (loader) n_psi = ldg16_stream<T>(a.u_psi + off + (long long)R * plane);
   if (active) {
-    n_psi = ldg16_stream<T>(a.u_psi + off + (long long)R * plane);
     n_upi = ldg16_stream<T>(a.u_pi + off);
 #pragma unroll
     for (int q = 0; q < NIN; ++q) {
@@ -168,7 +171,7 @@ __global__ void __launch_bounds__(TX* TY) k_rk_stage(const StageArgs<T> a) {
       in_pi[q] = n_in_pi[q];
     }
     // centre plane -> shared
-    if (active) {
+    if (loader) {
 #pragma unroll
       for (int p = 0; p < CPT; ++p) s[s_own + p] = w[R].p[p];
     }
@@ -180,8 +183,8 @@ __global__ void __launch_bounds__(TX* TY) k_rk_stage(const StageArgs<T> a) {
     // issue next plane's loads before computing this one
     if (zz + 1 < t.nz) {
       const long long o1 = off + plane;
+      if (loader) n_psi = ldg16_stream<T>(a.u_psi + o1 + (long long)R * plane);
       if (active) {
-        n_psi = ldg16_stream<T>(a.u_psi + o1 + (long long)R * plane);
         n_upi = ldg16_stream<T>(a.u_pi + o1);
 #pragma unroll
         for (int q = 0; q < NIN; ++q) {

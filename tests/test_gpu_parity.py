@@ -35,29 +35,55 @@ def _compare_tags(o, s, level):
 
 
 # ---- C1: the small BASELINE.json config, full length -------------------------------------------------
+# DESIGN.md reading R12: with the literal C1 numbers (h = 1, dt = 0.25, unit-variance GRF, eta up to 3.5) classic
+# RK4 is unstable -- the local frequency sqrt(12/h^2 + lambda eta^2 (3|psi|^2 - 1)) dt passes the RK4 limit
+# 2.83 where |psi| > 1 -- and the fields reach 1e2 at step 8, 1e22 at step 9 and overflow at step 10 IN THE ORACLE
+# (tests/test_oracle_pins.py::test_c1_literal_parameters_blow_up).  The literal run is therefore compared
+# with 1e-11 * max(1, largest |oracle value|) while the oracle is finite (1e-11 absolute for the first steps,
+# relative once the instability has taken off); the stabilised variant C1s (same grid, fields, eta range;
+# dt = 0.0625, 40 steps) carries the 1e-11 absolute bar over the whole run.
 
-@pytest.mark.parametrize("flow", ["lean", "classic"])
-def test_c1_32cubed_10_steps_with_tags(flow):
+def _c1_run(flow, dt, steps, literal):
     P = _pair()
     cfg = inputs.CONFIGS["C1"]
     o, s = P.make_pair(cfg.n0, nghost=cfg.nghost, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=flow)
     P.init_grf(o, s, cfg.n0, cfg.grf_f, cfg.seeds)
     eta = cfg.eta0
     n_tagged = 0
-    for step in range(cfg.steps):
-        o.rk_step(cfg.dt, eta)
-        s.rk_step(cfg.dt, eta)
-        eta += cfg.dt
-        assert P.max_err(o, s) <= F64_TOL, f"step {step}"
-        # free-running tags (information): both sides tag their own state
+    for step in range(steps):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+        big = max(float(np.abs(o.get_state(0, c)).max()) for c in range(4))
+        if not np.isfinite(big):
+            assert literal
+            break
+        if not literal:
+            assert big < 20.0
+            assert P.max_err(o, s) <= F64_TOL, f"step {step}"
+        else:  # diverging run: bar relative to the largest oracle value once that exceeds 1
+            assert P.max_err(o, s) <= F64_TOL * max(1.0, big), f"step {step}"
+        # free-running tags: both sides tag their own state; identical while the states agree to the last bits
         ot, oc = o.tag_strings(0)
         gt, gc = s.tag_strings(0)
-        assert np.array_equal(ot[0], s.split_tags(0, gt)[0].cpu().numpy())
-        assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
+        if big < 1e3:
+            assert np.array_equal(ot[0], s.split_tags(0, gt)[0].cpu().numpy())
+            assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
         n_tagged += int((ot[0] != 0).sum())
-    assert eta == pytest.approx(3.5)
     assert n_tagged > 0  # the GRF does contain strings
     s.synchronize()
+    return eta
+
+
+@pytest.mark.parametrize("flow", ["lean", "classic"])
+def test_c1_literal_32cubed_10_steps_with_tags(flow):
+    _c1_run(flow, dt=inputs.CONFIGS["C1"].dt, steps=10, literal=True)
+
+
+@pytest.mark.parametrize("flow", ["lean", "classic"])
+def test_c1s_stabilised_32cubed_eta_1_to_3p5_with_tags(flow):
+    eta = _c1_run(flow, dt=0.0625, steps=40, literal=False)
+    assert eta == pytest.approx(3.5)
 
 
 # ---- ragged single-level grids, several boxes, both stencils, friction and mass terms -----------------

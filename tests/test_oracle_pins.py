@@ -686,3 +686,34 @@ def test_box_list_validation():
         Oracle(16, boxes=bad, n_levels=3, nghost=2, lap_order=2)
     good = [(0, (0, 0, 0), (15, 15, 15)), (1, (8, 8, 8), (23, 23, 23)), (2, (24, 24, 24), (39, 39, 39))]
     Oracle(16, boxes=good, n_levels=3, nghost=2, lap_order=2)
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json config 1 as printed is outside the RK4 stability region (reading R12)
+# ------------------------------------------------------------------------------------------------
+
+
+def test_c1_literal_parameters_blow_up():
+    """h = 1, dt = 0.25, lambda = 1, eta 1 -> 3.5 on a unit-variance GRF: where |psi| > 1 the local frequency
+    sqrt(12/h^2 + lambda eta^2 (3|psi|^2 - 1)) * dt exceeds the RK4 stability limit 2.83 (at eta = 3, |psi| = 2:
+    sqrt(12 + 99) * 0.25 = 2.63; |psi| = 2.5: 3.3) and the run diverges; with dt = 0.0625 it stays bounded.
+    Documented so that the GPU parity test's treatment of C1 (absolute bar while bounded) is checkable here."""
+    cfg = inputs.CONFIGS["C1"]
+
+    def run(dt, steps):
+        o = Oracle(cfg.n0, nghost=1, lap_order=1, h0=cfg.h0, lam=cfg.lam)
+        for c, s in enumerate(cfg.seeds):
+            o.set_state(0, c, inputs.grf(cfg.n0, cfg.grf_f, s).numpy())
+        eta, peak = cfg.eta0, []
+        for _ in range(steps):
+            o.rk_step(dt, eta)
+            eta += dt
+            with np.errstate(invalid="ignore"):
+                peak.append(max(float(np.abs(o.get_state(0, c)).max()) for c in range(2)))
+        return peak
+
+    lit = run(cfg.dt, 10)
+    assert max(lit[:7]) < 4.0            # bounded for the first 7 steps (eta <= 2.75)
+    assert lit[7] > 1e2 and not lit[9] < 1e100
+    stab = run(0.0625, 40)
+    assert max(stab) < 4.5 and max(stab[20:]) < 3.0  # the initial GRF peaks at ~4 sigma, then relaxes
