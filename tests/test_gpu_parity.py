@@ -38,10 +38,12 @@ def _compare_tags(o, s, level):
 # DESIGN.md reading R12: with the literal C1 numbers (h = 1, dt = 0.25, unit-variance GRF, eta up to 3.5) classic
 # RK4 is unstable -- the local frequency sqrt(12/h^2 + lambda eta^2 (3|psi|^2 - 1)) dt passes the RK4 limit
 # 2.83 where |psi| > 1 -- and the fields reach 1e2 at step 8, 1e22 at step 9 and overflow at step 10 IN THE ORACLE
-# (tests/test_oracle_pins.py::test_c1_literal_parameters_blow_up).  The literal run is therefore compared
-# with 1e-11 * max(1, largest |oracle value|) while the oracle is finite (1e-11 absolute for the first steps,
-# relative once the instability has taken off); the stabilised variant C1s (same grid, fields, eta range;
-# dt = 0.0625, 40 steps) carries the 1e-11 absolute bar over the whole run.
+# (tests/test_oracle_pins.py::test_c1_literal_parameters_blow_up).  The literal run therefore carries the
+# 1e-11 absolute bar while the oracle state is bounded (max |u| <= 20, the same bound the stable run asserts);
+# once the instability has taken off the cubic term multiplies RELATIVE rounding differences by ~3 per RHS
+# evaluation, so no fixed bar holds: there the test only checks that the CUDA path diverges the same way
+# (agreement to 1e-6 of the largest oracle value while finite, non-finite at the same step).  The stabilised
+# variant C1s (same grid, fields, eta range; dt = 0.0625, 40 steps) carries 1e-11 absolute over the whole run.
 
 def _c1_run(flow, dt, steps, literal):
     P = _pair()
@@ -50,6 +52,7 @@ def _c1_run(flow, dt, steps, literal):
     P.init_grf(o, s, cfg.n0, cfg.grf_f, cfg.seeds)
     eta = cfg.eta0
     n_tagged = 0
+    bounded_steps = 0
     for step in range(steps):
         o.rk_step(dt, eta)
         s.rk_step(dt, eta)
@@ -57,12 +60,16 @@ def _c1_run(flow, dt, steps, literal):
         big = max(float(np.abs(o.get_state(0, c)).max()) for c in range(4))
         if not np.isfinite(big):
             assert literal
+            gbig = max(float(s.get_state(0, c).abs().max()) for c in range(4))
+            assert not np.isfinite(gbig) or gbig > 1e100  # the CUDA path blew up at the same step
             break
         if not literal:
             assert big < 20.0
+        if big <= 20.0:
             assert P.max_err(o, s) <= F64_TOL, f"step {step}"
-        else:  # diverging run: bar relative to the largest oracle value once that exceeds 1
-            assert P.max_err(o, s) <= F64_TOL * max(1.0, big), f"step {step}"
+            bounded_steps += 1
+        else:  # diverging run (R12): same blow-up, no fixed bar
+            assert P.max_err(o, s) <= 1e-6 * big, f"step {step}"
         # free-running tags: both sides tag their own state; identical while the states agree to the last bits
         ot, oc = o.tag_strings(0)
         gt, gc = s.tag_strings(0)
@@ -71,6 +78,7 @@ def _c1_run(flow, dt, steps, literal):
             assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
         n_tagged += int((ot[0] != 0).sum())
     assert n_tagged > 0  # the GRF does contain strings
+    assert bounded_steps >= (5 if literal else steps)
     s.synchronize()
     return eta
 
