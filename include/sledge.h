@@ -42,7 +42,7 @@ typedef enum {
 } sledge_status;
 
 enum { SLEDGE_F32 = 0, SLEDGE_F64 = 1 };
-enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1 };
+enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1, SLEDGE_RK_FUSED = 2 };
 
 /* Inclusive cell range lo..hi of one box in the index space of `level`; axis order x, y, z. */
 typedef struct {
@@ -59,7 +59,8 @@ typedef struct {
   int32_t dtype;           /* SLEDGE_F32 / SLEDGE_F64: storage AND arithmetic type                */
   int32_t lap_order;       /* paper's `order` (L649): 1 = 7-point, 2 = 13-point Laplacian         */
   int32_t eta_fixed;       /* 1 = Minkowski test variant: eta_s = eta for every stage (R3)         */
-  int32_t rk_dataflow;     /* SLEDGE_RK_LEAN: 52 words/cell-step; SLEDGE_RK_CLASSIC: 64 (R5)       */
+  int32_t rk_dataflow;     /* words moved per cell-step (R5): SLEDGE_RK_FUSED 20 (two stages per sweep on
+                              level 0, LEAN on finer levels), SLEDGE_RK_LEAN 52, SLEDGE_RK_CLASSIC 64   */
   double h0;               /* level-0 spacing, Eq.1                                               */
   double lambda;           /* Eq.11 generalised (R2): k_Pi = -(friction/eta) Pi + Lap psi          */
   double a_mass;           /*        - lambda eta^2 psi (psi1^2+psi2^2-1) - a_mass psi             */

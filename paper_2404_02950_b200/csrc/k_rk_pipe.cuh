@@ -1,0 +1,380 @@
+// k_rk_pipe.cuh -- K1: fused Laplacian + Mexican-hat potential + RK4 stage update(s), cp.async-pipelined.
+//
+// What it computes (Eq.10-11; Laplacian<order> L649; RK4 = integrator.type 4, L808):
+//   k_psi_c = Pi_c(U)
+//   k_Pi_c  = Lap_h psi_c(U) - psi_c (lambda eta_s^2 (psi1^2 + psi2^2 - 1) + a) - (kappa/eta_s) Pi_c(U)
+// for every valid cell of every box of a level in ONE launch, combined into one of the data-flows below.
+//
+// Data-flows (words = reals moved per cell, R + W):
+//   LEAN    (52 words / cell-step)   S1: U2 = Y + dt/2 k                         4R + 4W
+//                                    S2: U3 = Y + dt/2 k                         8R + 4W
+//                                    S3: U4 = Y + dt k                           8R + 4W
+//                                    S4: Ynew = (U2 + 2U3 + U4 - Y)/3 + dt/6 k   16R + 4W
+//   CLASSIC (64 words / cell-step)   S1: U2 = Y + dt/2 k ; ACC = Y + dt/6 k      4R + 8W
+//                                    S2/S3: U = Y + a dt k ; ACC += dt/3 k       12R + 8W
+//                                    S4: Ynew = ACC + dt/6 k                     8R + 4W
+//   FUSED   (20 words / cell-step)   two stages per sweep.  Because k_psi = Pi is pointwise, the NEXT stage's psi
+//     is known at every neighbour from the current stage's (psi, Pi) there, and the Laplacian is linear:
+//       PASS A (stages 1+2):  Lap psi2 = Lap psi_Y + dt/2 Lap Pi_Y              4R + 4W   -> U3
+//       PASS B (stages 3+4):  Lap psi4 = Lap psi_Y + dt   Lap Pi3               8R + 4W   -> Ynew
+//     PASS B recomputes k1 from Y (same expression as PASS A, same bits) and recovers dt/2 k2 = Pi3 - Pi_Y.
+//     Pi is differenced here, so the ghost fill must fill Pi ghosts too (same-level / periodic copies).
+//
+// Mapping: a CTA owns a TXC x TY column tile of one box and marches along z.  Each thread keeps the 2R+1
+// z-window of its own column of every differenced field in registers; only the centre planes go through
+// shared memory (double buffered, one __syncthreads per plane) so that x/y neighbours come from on-chip
+// memory.  ALL global loads are 16-byte cp.async (LDGSTS) into a D-stage shared-memory ring issued D planes
+// ahead, so the bytes in flight do not occupy registers: own-column values of the differenced fields for
+// plane z+R, pointwise inputs for plane z, and the x/y halo of plane z.  Outputs go registers -> HBM with
+// 16-byte stores.
+#pragma once
+#include "layout.h"
+
+namespace sledge {
+
+enum StageMode {
+  LEAN_S1 = 0,
+  LEAN_S23 = 1,
+  LEAN_S4 = 2,
+  CLASSIC_S1 = 3,
+  CLASSIC_S23 = 4,
+  CLASSIC_S4 = 5,
+  FUSED_A = 6,
+  FUSED_B = 7
+};
+
+template <int MODE> struct ModeInfo;
+// NF: differenced (stencil) fields; NP: pointwise inputs (pairs); NOUT: output states (psi + pi each)
+template <> struct ModeInfo<LEAN_S1> { static constexpr int NF = 1, NP = 1, NOUT = 1; };
+template <> struct ModeInfo<LEAN_S23> { static constexpr int NF = 1, NP = 3, NOUT = 1; };
+template <> struct ModeInfo<LEAN_S4> { static constexpr int NF = 1, NP = 7, NOUT = 1; };
+template <> struct ModeInfo<CLASSIC_S1> { static constexpr int NF = 1, NP = 1, NOUT = 2; };
+template <> struct ModeInfo<CLASSIC_S23> { static constexpr int NF = 1, NP = 5, NOUT = 2; };
+template <> struct ModeInfo<CLASSIC_S4> { static constexpr int NF = 1, NP = 3, NOUT = 1; };
+template <> struct ModeInfo<FUSED_A> { static constexpr int NF = 2, NP = 0, NOUT = 1; };
+template <> struct ModeInfo<FUSED_B> { static constexpr int NF = 3, NP = 1, NOUT = 1; };
+
+// Field roles.  Unfused modes: sten[0] = psi(U); pnt[0] = Pi(U); pnt[1+2q], pnt[2+2q] = psi, Pi of input q
+// (LEAN: q0 = Y, q1 = U2, q2 = U3; CLASSIC: q0 = Y (S23) or ACC (S4), q1 = ACC).
+// FUSED_A: sten = {psi_Y, Pi_Y}.  FUSED_B: sten = {psi_3, Pi_3, psi_Y}, pnt[0] = Pi_Y.
+template <typename T>
+struct PipeArgs {
+  using P = typename PairOf<T>::type;
+  const BoxDev* boxes;
+  const TileDev* tiles;
+  const P* sten[3];
+  const P* pnt[7];
+  P* out_psi[2];
+  P* out_pi[2];
+  int g, ox;
+  T inv_h2;        // 1/h^2 (order 1) or 1/(12 h^2) (order 2)
+  T lam_eta2[3];   // lambda * eta^2 at t, t + dt/2, t + dt (unfused: [0] = the stage's value)
+  T fric[3];       // kappa / eta at the same times
+  T a_mass;
+  T adt;           // unfused: a_s * dt (S1-S3) or dt/6 (S4);  fused: dt
+  T bdt;           // classic: b_s * dt for the accumulator
+};
+
+__device__ __forceinline__ void cp_async_16(void* smem, const void* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+#ifdef SLEDGE_CPASYNC_CA
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+#else
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+#endif
+}
+__device__ __forceinline__ void cp_async_pair(double2* smem, const double2* gmem) { cp_async_16(smem, gmem); }
+__device__ __forceinline__ void cp_async_pair(float2* smem, const float2* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// Laplacian of one component from its 6 (12) neighbours; same association as the definition:
+// sum_d [(u+ - u) + (u- - u)], x then y then z; order 2: (16 s1 - s2) / (12 h^2).
+template <typename T, int ORDER>
+__device__ __forceinline__ T lap_from(T u, const T* xm, const T* xp, const T* ym, const T* yp, const T* zm,
+                                      const T* zp, T inv_h2) {
+  T n1x = (xp[0] - u) + (xm[0] - u);
+  T n1y = (yp[0] - u) + (ym[0] - u);
+  T n1z = (zp[0] - u) + (zm[0] - u);
+  T s1 = (n1x + n1y) + n1z;
+  if (ORDER == 1) return s1 * inv_h2;
+  T n2x = (xp[1] - u) + (xm[1] - u);
+  T n2y = (yp[1] - u) + (ym[1] - u);
+  T n2z = (zp[1] - u) + (zm[1] - u);
+  T s2 = (n2x + n2y) + n2z;
+  return (T(16) * s1 - s2) * inv_h2;
+}
+
+template <typename T, int ORDER, int MODE, int TX, int TY, int D>
+struct PipeCfg {
+  static constexpr int R = ORDER;
+  static constexpr int CPT = Vec16<T>::CPT;
+  static constexpr int TXC = TX * CPT;
+  static constexpr int SW = TXC + 2 * R;
+  static constexpr int SH = TY + 2 * R;
+  static constexpr int NT = TX * TY;
+  static constexpr int NH = 2 * R * (TXC + TY);  // halo pairs per plane (star stencil: no corners)
+  static constexpr int HPT = (NH + NT - 1) / NT;
+  static constexpr int NF = ModeInfo<MODE>::NF;
+  static constexpr int NP = ModeInfo<MODE>::NP;
+  static constexpr int NOUT = ModeInfo<MODE>::NOUT;
+  static constexpr size_t PAIR = 2 * sizeof(T);
+  static constexpr size_t OWN_BYTES = (size_t)D * (NF + NP) * NT * 16;
+  static constexpr size_t HALO_BYTES = (size_t)D * NF * NH * PAIR;  // ring slot = NH pairs per field
+  static constexpr size_t CTR_BYTES = (size_t)2 * NF * SH * SW * PAIR;
+  static constexpr size_t SMEM_BYTES = OWN_BYTES + HALO_BYTES + CTR_BYTES;
+};
+
+// Deepest ring (<= dmax stages, >= 2) whose shared memory fits `budget` bytes.
+template <typename T, int ORDER, int MODE, int TX, int TY>
+constexpr int pipe_depth(size_t budget, int dmax) {
+  int d = 2;
+  if (dmax >= 3 && PipeCfg<T, ORDER, MODE, TX, TY, 3>::SMEM_BYTES <= budget) d = 3;
+  if (dmax >= 4 && PipeCfg<T, ORDER, MODE, TX, TY, 4>::SMEM_BYTES <= budget) d = 4;
+  if (dmax >= 5 && PipeCfg<T, ORDER, MODE, TX, TY, 5>::SMEM_BYTES <= budget) d = 5;
+  if (dmax >= 6 && PipeCfg<T, ORDER, MODE, TX, TY, 6>::SMEM_BYTES <= budget) d = 6;
+  return d;
+}
+
+template <typename T, int ORDER, int MODE, int TX, int TY, int D>
+__global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
+  using P = typename PairOf<T>::type;
+  using V = Vec16<T>;
+  using C = PipeCfg<T, ORDER, MODE, TX, TY, D>;
+  constexpr int R = C::R, CPT = C::CPT, TXC = C::TXC, SW = C::SW, SH = C::SH, NT = C::NT, NH = C::NH, HPT = C::HPT;
+  constexpr int NF = C::NF, NP = C::NP, NOUT = C::NOUT;
+  constexpr int NPA = NP > 0 ? NP : 1;
+
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  V* const own = reinterpret_cast<V*>(smem_raw);                             // [D][NF + NP][NT]
+  P* const halo = reinterpret_cast<P*>(smem_raw + C::OWN_BYTES);             // [D][NF][NH]
+  P* const ctr = reinterpret_cast<P*>(smem_raw + C::OWN_BYTES + C::HALO_BYTES);  // [2][NF][SH * SW]
+
+  const TileDev t = a.tiles[blockIdx.x];
+  const BoxDev b = a.boxes[t.box];
+  const int tid = threadIdx.x;
+  const int tx = tid % TX, ty = tid / TX;
+  const int x = t.x0 + tx * CPT, y = t.y0 + ty;
+  const bool active = (x < b.n[0]) && (y < b.n[1]);
+  // in a partial tile the columns/rows just past the box edge are ghost cells that the edge cells need as
+  // +x / +y neighbours: threads sitting there still stream their own column through shared memory
+  const bool loader = (x < b.n[0] + R) && (y < b.n[1] + R);
+  const long long plane = (long long)b.sx * b.sy;
+  const long long tile_org =
+      b.base + (long long)(t.z0 + a.g) * plane + (long long)(t.y0 + a.g) * b.sx + (t.x0 + a.ox);
+  long long off = tile_org + (long long)ty * b.sx + tx * CPT;  // this thread's cell in plane z0
+
+  // halo assignment: pair index -> (hx, hy) relative to the tile origin
+  int h_goff[HPT];  // global offset relative to tile_org (within a plane)
+  int h_soff[HPT];  // offset inside a centre plane, -1 = none
+#pragma unroll
+  for (int q = 0; q < HPT; ++q) {
+    const int idx = tid + q * NT;
+    int hx = 0, hy = 0;
+    bool ok = idx < NH;
+    if (idx < 2 * R * TXC) {  // bottom / top strips, x fastest
+      const int row = idx / TXC;
+      hx = idx % TXC;
+      hy = (row < R) ? (row - R) : (TY + row - R);
+    } else {
+      const int j = idx - 2 * R * TXC;  // left / right strips
+      const int col = j % (2 * R);
+      hy = j / (2 * R);
+      hx = (col < R) ? (col - R) : (TXC + col - R);
+    }
+    // stay inside the box's ghosted extent (partial tiles at the high end of a box)
+    ok = ok && (t.x0 + hx < b.n[0] + R) && (t.y0 + hy < b.n[1] + R);
+    h_goff[q] = hy * b.sx + hx;
+    h_soff[q] = ok ? ((hy + R) * SW + (hx + R)) : -1;
+  }
+  const int s_own = (ty + R) * SW + (tx * CPT + R);
+
+  // one pipeline stage = everything iteration `st` consumes: own-column values of plane z0+st+R of the
+  // differenced fields, pointwise inputs of plane z0+st, x/y halo of plane z0+st
+  auto issue = [&](int st) {
+    const int slot = st % D;
+    V* const o = own + (size_t)slot * (NF + NP) * NT + tid;
+    const long long po = off + (long long)st * plane;  // `off` is never advanced (see below)
+    if (loader) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) cp_async_16(o + f * NT, a.sten[f] + po + (long long)R * plane);
+    }
+    if (active) {
+#pragma unroll
+      for (int q = 0; q < NP; ++q) cp_async_16(o + (NF + q) * NT, a.pnt[q] + po);
+    }
+    const long long ho = tile_org + (long long)st * plane;
+#pragma unroll
+    for (int q = 0; q < HPT; ++q)
+      if (h_soff[q] >= 0) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+          cp_async_pair(halo + ((size_t)slot * NF + f) * NH + tid + q * NT, a.sten[f] + ho + h_goff[q]);
+      }
+  };
+
+  // prologue: fill the ring, then the lower 2R planes of the z-windows straight into registers
+#pragma unroll
+  for (int st = 0; st < D; ++st) {
+    if (st < t.nz) issue(st);
+    cp_async_commit();
+  }
+  V w[NF][2 * R + 1];  // w[f][m] = field f at plane z + m - R
+#pragma unroll
+  for (int f = 0; f < NF; ++f)
+#pragma unroll
+    for (int m = 0; m < 2 * R; ++m)
+      if (loader) w[f][m + 1] = ldg16_keep<T>(a.sten[f] + off + (long long)(m - R) * plane);
+
+  for (int zz = 0; zz < t.nz; ++zz) {
+    const int slot = zz % D;
+    P* const cb = ctr + (size_t)(zz & 1) * NF * SH * SW;
+    cp_async_wait<D - 1>();  // this thread's copies of stage zz have landed (only this thread reads them)
+    const V* const o = own + (size_t)slot * (NF + NP) * NT + tid;
+    V pv[NPA];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+#pragma unroll
+      for (int m = 0; m < 2 * R; ++m) w[f][m] = w[f][m + 1];
+      if (loader) {
+        w[f][2 * R] = o[f * NT];
+#pragma unroll
+        for (int p = 0; p < CPT; ++p) cb[f * SH * SW + s_own + p] = w[f][R].p[p];
+      }
+    }
+    if (active) {
+#pragma unroll
+      for (int q = 0; q < NP; ++q) pv[q] = o[(NF + q) * NT];
+    }
+#pragma unroll
+    for (int q = 0; q < HPT; ++q)
+      if (h_soff[q] >= 0) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+          cb[f * SH * SW + h_soff[q]] = halo[((size_t)slot * NF + f) * NH + tid + q * NT];
+      }
+    // refill the slot just drained with stage zz + D
+    if (zz + D < t.nz) issue(zz + D);
+    cp_async_commit();
+    __syncthreads();
+
+    if (active) {
+      V o_psi[NOUT], o_pi[NOUT];
+#pragma unroll
+      for (int p = 0; p < CPT; ++p) {
+        const int sc = s_own + p;
+        T lap[NF][2];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          const P* const s = cb + f * SH * SW;
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            auto comp = [c](const P& v) -> T { return c == 0 ? v.x : v.y; };
+            T xm[2], xp[2], ym[2], yp[2], zm[2], zp[2];
+#pragma unroll
+            for (int r = 1; r <= R; ++r) {
+              xm[r - 1] = comp(s[sc - r]);
+              xp[r - 1] = comp(s[sc + r]);
+              ym[r - 1] = comp(s[sc - r * SW]);
+              yp[r - 1] = comp(s[sc + r * SW]);
+              zm[r - 1] = comp(w[f][R - r].p[p]);
+              zp[r - 1] = comp(w[f][R + r].p[p]);
+            }
+            lap[f][c] = lap_from<T, ORDER>(comp(w[f][R].p[p]), xm, xp, ym, yp, zm, zp, a.inv_h2);
+          }
+        }
+        if (MODE == FUSED_A) {
+          // stages 1 + 2 (O4): U3 = Y + dt/2 k(U2), U2 = Y + dt/2 k(Y); U2 is never stored
+          const T hdt = T(0.5) * a.adt;
+          const T y1 = w[0][R].p[p].x, y2 = w[0][R].p[p].y, q1 = w[1][R].p[p].x, q2 = w[1][R].p[p].y;
+          const T pot1 = a.lam_eta2[0] * ((y1 * y1 + y2 * y2) - T(1)) + a.a_mass;
+          const T k1a = (lap[0][0] - y1 * pot1) - a.fric[0] * q1;
+          const T k1b = (lap[0][1] - y2 * pot1) - a.fric[0] * q2;
+          const T p2a = q1 + hdt * k1a, p2b = q2 + hdt * k1b;  // Pi(U2)
+          const T u2a = y1 + hdt * q1, u2b = y2 + hdt * q2;    // psi(U2)
+          const T l2a = lap[0][0] + hdt * lap[1][0], l2b = lap[0][1] + hdt * lap[1][1];
+          const T pot2 = a.lam_eta2[1] * ((u2a * u2a + u2b * u2b) - T(1)) + a.a_mass;
+          const T k2a = (l2a - u2a * pot2) - a.fric[1] * p2a;
+          const T k2b = (l2b - u2b * pot2) - a.fric[1] * p2b;
+          o_psi[0].p[p] = mkpair(y1 + hdt * p2a, y2 + hdt * p2b);
+          o_pi[0].p[p] = mkpair(q1 + hdt * k2a, q2 + hdt * k2b);
+        } else if (MODE == FUSED_B) {
+          // stages 3 + 4 and the final combination; k1 recomputed from Y, dt/2 k2 = Pi3 - Pi_Y
+          const T dt = a.adt, hdt = T(0.5) * a.adt, sixth = a.adt / T(6);
+          const T u3a = w[0][R].p[p].x, u3b = w[0][R].p[p].y, p3a = w[1][R].p[p].x, p3b = w[1][R].p[p].y;
+          const T y1 = w[2][R].p[p].x, y2 = w[2][R].p[p].y, q1 = pv[0].p[p].x, q2 = pv[0].p[p].y;
+          const T pot3 = a.lam_eta2[1] * ((u3a * u3a + u3b * u3b) - T(1)) + a.a_mass;
+          const T k3a = (lap[0][0] - u3a * pot3) - a.fric[1] * p3a;
+          const T k3b = (lap[0][1] - u3b * pot3) - a.fric[1] * p3b;
+          const T u4a = y1 + dt * p3a, u4b = y2 + dt * p3b;  // psi(U4)
+          const T p4a = q1 + dt * k3a, p4b = q2 + dt * k3b;  // Pi(U4)
+          const T l4a = lap[2][0] + dt * lap[1][0], l4b = lap[2][1] + dt * lap[1][1];
+          const T pot4 = a.lam_eta2[2] * ((u4a * u4a + u4b * u4b) - T(1)) + a.a_mass;
+          const T k4a = (l4a - u4a * pot4) - a.fric[2] * p4a;
+          const T k4b = (l4b - u4b * pot4) - a.fric[2] * p4b;
+          const T pot1 = a.lam_eta2[0] * ((y1 * y1 + y2 * y2) - T(1)) + a.a_mass;
+          const T k1a = (lap[2][0] - y1 * pot1) - a.fric[0] * q1;
+          const T k1b = (lap[2][1] - y2 * pot1) - a.fric[0] * q2;
+          const T p2a = q1 + hdt * k1a, p2b = q2 + hdt * k1b;  // Pi(U2), same bits as in PASS A
+          const T twothirds = T(2) / T(3);
+          o_psi[0].p[p] = mkpair(y1 + sixth * ((q1 + p4a) + T(2) * (p2a + p3a)),
+                                 y2 + sixth * ((q2 + p4b) + T(2) * (p2b + p3b)));
+          o_pi[0].p[p] = mkpair((q1 + twothirds * (p3a - q1)) + sixth * ((k1a + k4a) + T(2) * k3a),
+                                (q2 + twothirds * (p3b - q2)) + sixth * ((k1b + k4b) + T(2) * k3b));
+        } else {
+          const T psi1 = w[0][R].p[p].x, psi2 = w[0][R].p[p].y;
+          const T pi1 = pv[0].p[p].x, pi2 = pv[0].p[p].y;
+          const T pot = a.lam_eta2[0] * ((psi1 * psi1 + psi2 * psi2) - T(1)) + a.a_mass;
+          const T kpsi1 = pi1, kpsi2 = pi2;
+          const T kpi1 = (lap[0][0] - psi1 * pot) - a.fric[0] * pi1;
+          const T kpi2 = (lap[0][1] - psi2 * pot) - a.fric[0] * pi2;
+          // pointwise inputs: in_psi(q) = pv[1 + 2q], in_pi(q) = pv[2 + 2q]
+          auto ipsi = [&](int q) -> const P& { return pv[(1 + 2 * q) < NPA ? (1 + 2 * q) : 0].p[p]; };
+          auto ipi = [&](int q) -> const P& { return pv[(2 + 2 * q) < NPA ? (2 + 2 * q) : 0].p[p]; };
+          if (MODE == LEAN_S1) {  // U2 = U + adt k   (U = Y)
+            o_psi[0].p[p] = mkpair(psi1 + a.adt * kpsi1, psi2 + a.adt * kpsi2);
+            o_pi[0].p[p] = mkpair(pi1 + a.adt * kpi1, pi2 + a.adt * kpi2);
+          } else if (MODE == LEAN_S23) {  // U' = Y + adt k   (in0 = Y)
+            o_psi[0].p[p] = mkpair(ipsi(0).x + a.adt * kpsi1, ipsi(0).y + a.adt * kpsi2);
+            o_pi[0].p[p] = mkpair(ipi(0).x + a.adt * kpi1, ipi(0).y + a.adt * kpi2);
+          } else if (MODE == LEAN_S4) {  // in0 = Y, in1 = U2, in2 = U3, U = U4, adt = dt/6
+            const T third = T(1) / T(3);
+            auto comb = [&](T yv, T u2, T u3, T u4, T kk) -> T {
+              return (((u2 + T(2) * u3) + u4) - yv) * third + a.adt * kk;
+            };
+            o_psi[0].p[p] = mkpair(comb(ipsi(0).x, ipsi(1).x, ipsi(2).x, psi1, kpsi1),
+                                   comb(ipsi(0).y, ipsi(1).y, ipsi(2).y, psi2, kpsi2));
+            o_pi[0].p[p] = mkpair(comb(ipi(0).x, ipi(1).x, ipi(2).x, pi1, kpi1),
+                                  comb(ipi(0).y, ipi(1).y, ipi(2).y, pi2, kpi2));
+          } else if (MODE == CLASSIC_S1) {  // out0 = U + adt k ; out1 (ACC) = U + bdt k
+            o_psi[0].p[p] = mkpair(psi1 + a.adt * kpsi1, psi2 + a.adt * kpsi2);
+            o_pi[0].p[p] = mkpair(pi1 + a.adt * kpi1, pi2 + a.adt * kpi2);
+            o_psi[NOUT - 1].p[p] = mkpair(psi1 + a.bdt * kpsi1, psi2 + a.bdt * kpsi2);
+            o_pi[NOUT - 1].p[p] = mkpair(pi1 + a.bdt * kpi1, pi2 + a.bdt * kpi2);
+          } else if (MODE == CLASSIC_S23) {  // in0 = Y, in1 = ACC ; out0 = Y + adt k ; out1 = ACC + bdt k
+            o_psi[0].p[p] = mkpair(ipsi(0).x + a.adt * kpsi1, ipsi(0).y + a.adt * kpsi2);
+            o_pi[0].p[p] = mkpair(ipi(0).x + a.adt * kpi1, ipi(0).y + a.adt * kpi2);
+            o_psi[NOUT - 1].p[p] = mkpair(ipsi(1).x + a.bdt * kpsi1, ipsi(1).y + a.bdt * kpsi2);
+            o_pi[NOUT - 1].p[p] = mkpair(ipi(1).x + a.bdt * kpi1, ipi(1).y + a.bdt * kpi2);
+          } else {  // CLASSIC_S4: in0 = ACC ; out0 = ACC + adt k
+            o_psi[0].p[p] = mkpair(ipsi(0).x + a.adt * kpsi1, ipsi(0).y + a.adt * kpsi2);
+            o_pi[0].p[p] = mkpair(ipi(0).x + a.adt * kpi1, ipi(0).y + a.adt * kpi2);
+          }
+        }
+      }
+      const long long oo = off + (long long)zz * plane;
+#pragma unroll
+      for (int q = 0; q < NOUT; ++q) {
+        stg16<T>(a.out_psi[q] + oo, o_psi[q]);
+        stg16<T>(a.out_pi[q] + oo, o_pi[q]);
+      }
+    }
+  }
+}
+
+}  // namespace sledge

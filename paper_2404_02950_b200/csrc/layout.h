@@ -57,23 +57,71 @@ __device__ __forceinline__ Vec16<T> ldg16(const typename PairOf<T>::type* ptr) {
   *reinterpret_cast<int4*>(&r) = raw;
   return r;
 }
+// L2 eviction-priority policies (createpolicy): stencil data that a neighbouring CTA re-reads as halo is
+// loaded evict_last, pure streams (pointwise inputs, all outputs) evict_first.
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+#ifndef SLEDGE_POL
+#define SLEDGE_POL 0
+#endif
 // streaming variant: the data is touched once per launch, keep it out of L1
 template <typename T>
 __device__ __forceinline__ Vec16<T> ldg16_stream(const typename PairOf<T>::type* ptr) {
   Vec16<T> r;
   int4 raw;
+#if SLEDGE_POL == 2
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=r"(raw.x), "=r"(raw.y), "=r"(raw.z), "=r"(raw.w)
+               : "l"(ptr), "l"(l2_policy_evict_first()));
+#else
   asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
                : "=r"(raw.x), "=r"(raw.y), "=r"(raw.z), "=r"(raw.w)
                : "l"(ptr));
+#endif
+  *reinterpret_cast<int4*>(&r) = raw;
+  return r;
+}
+// stencil variant: a neighbouring CTA reads the same line as halo shortly before / after
+template <typename T>
+__device__ __forceinline__ Vec16<T> ldg16_keep(const typename PairOf<T>::type* ptr) {
+  Vec16<T> r;
+  int4 raw;
+#if SLEDGE_POL == 2
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=r"(raw.x), "=r"(raw.y), "=r"(raw.z), "=r"(raw.w)
+               : "l"(ptr), "l"(l2_policy_evict_last()));
+#elif SLEDGE_POL == 1
+  asm volatile("ld.global.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(raw.x), "=r"(raw.y), "=r"(raw.z), "=r"(raw.w)
+               : "l"(ptr));
+#else
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(raw.x), "=r"(raw.y), "=r"(raw.z), "=r"(raw.w)
+               : "l"(ptr));
+#endif
   *reinterpret_cast<int4*>(&r) = raw;
   return r;
 }
 template <typename T>
 __device__ __forceinline__ void stg16(typename PairOf<T>::type* ptr, const Vec16<T>& v) {
   const int4 raw = *reinterpret_cast<const int4*>(&v);
+#if SLEDGE_POL == 2
+  asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.s32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(ptr), "r"(raw.x),
+               "r"(raw.y), "r"(raw.z), "r"(raw.w), "l"(l2_policy_evict_first())
+               : "memory");
+#else
   asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(raw.x), "r"(raw.y),
                "r"(raw.z), "r"(raw.w)
                : "memory");
+#endif
 }
 
 __host__ __device__ __forceinline__ int wrap_idx(int i, int n) {

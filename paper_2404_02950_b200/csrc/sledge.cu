@@ -17,7 +17,7 @@
 
 #include "k_avgdown.cuh"
 #include "k_ghost.cuh"
-#include "k_rk_stage.cuh"
+#include "k_rk_pipe.cuh"
 #include "k_tag.cuh"
 
 using namespace sledge;
@@ -29,8 +29,22 @@ constexpr int COUNT_BLOCK = 32;  // box-flag reduction granularity (BASELINE.jso
 constexpr int MAX_EVENT_PAIRS = 4096;
 constexpr size_t ALIGN = 256;
 
-// K1 tile shapes (threads); cells per tile in x = TX * cells-per-16-bytes
-constexpr int K1_TX = 32, K1_TY = 8, K1_NZ = 64;
+// K1 tile shape (threads; cells per tile in x = TX * cells-per-16-bytes), z-chunk length and cp.async ring depth
+#ifndef SLEDGE_K1_TY
+#define SLEDGE_K1_TY 16
+#endif
+#ifndef SLEDGE_K1_NZ
+#define SLEDGE_K1_NZ 64
+#endif
+#ifndef SLEDGE_K1_DMAX
+#define SLEDGE_K1_DMAX 4
+#endif
+#ifndef SLEDGE_K1_SMEM
+#define SLEDGE_K1_SMEM (227 * 1024)
+#endif
+constexpr int K1_TX = 32, K1_TY = SLEDGE_K1_TY, K1_NZ = SLEDGE_K1_NZ;
+constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
+constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
 
 thread_local std::string g_err;
 
@@ -111,7 +125,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   if (p.lap_order < 1 || p.lap_order > 2) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be 1 (7-point) or 2 (13-point)");
   if (p.lap_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be <= nghost (L240)");
   if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
-  if (p.rk_dataflow != SLEDGE_RK_LEAN && p.rk_dataflow != SLEDGE_RK_CLASSIC) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
+  if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
   if (!(p.h0 > 0)) return fail(nullptr, SLEDGE_EINVAL, "h0 must be positive");
   for (int d = 0; d < 3; ++d) {
     if (p.n0[d] <= 0 || p.n0[d] % bf) return fail(nullptr, SLEDGE_EINVAL, "n0 must be a positive multiple of blocking_factor (L39)");
@@ -341,20 +355,112 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
 }
 
 template <typename T, int ORDER, int MODE>
-void launch_stage_kernel(sledge_ctx* c, const StageArgs<T>& a, int grid) {
-  k_rk_stage<T, ORDER, MODE, K1_TX, K1_TY><<<grid, K1_TX * K1_TY, 0, c->stream>>>(a);
+cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
+  constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, K1_TY>(K1_SMEM, K1_DMAX);
+  static_assert(PipeCfg<T, ORDER, MODE, K1_TX, K1_TY, D>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
+  using C = PipeCfg<T, ORDER, MODE, K1_TX, K1_TY, D>;
+  auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, K1_TY, D>;
+  static bool configured = false;  // per instantiation
+  if (!configured) {
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  kern<<<grid, K1_TX * K1_TY, C::SMEM_BYTES, c->stream>>>(a);
+  return cudaSuccess;
 }
 template <typename T, int ORDER>
-void launch_stage_mode(sledge_ctx* c, const StageArgs<T>& a, int grid, int mode) {
+cudaError_t launch_pipe_mode(sledge_ctx* c, const PipeArgs<T>& a, int grid, int mode) {
   switch (mode) {
-    case LEAN_S1: launch_stage_kernel<T, ORDER, LEAN_S1>(c, a, grid); break;
-    case LEAN_S23: launch_stage_kernel<T, ORDER, LEAN_S23>(c, a, grid); break;
-    case LEAN_S4: launch_stage_kernel<T, ORDER, LEAN_S4>(c, a, grid); break;
-    case CLASSIC_S1: launch_stage_kernel<T, ORDER, CLASSIC_S1>(c, a, grid); break;
-    case CLASSIC_S23: launch_stage_kernel<T, ORDER, CLASSIC_S23>(c, a, grid); break;
-    default: launch_stage_kernel<T, ORDER, CLASSIC_S4>(c, a, grid); break;
+    case LEAN_S1: return launch_pipe_kernel<T, ORDER, LEAN_S1>(c, a, grid);
+    case LEAN_S23: return launch_pipe_kernel<T, ORDER, LEAN_S23>(c, a, grid);
+    case LEAN_S4: return launch_pipe_kernel<T, ORDER, LEAN_S4>(c, a, grid);
+    case CLASSIC_S1: return launch_pipe_kernel<T, ORDER, CLASSIC_S1>(c, a, grid);
+    case CLASSIC_S23: return launch_pipe_kernel<T, ORDER, CLASSIC_S23>(c, a, grid);
+    case CLASSIC_S4: return launch_pipe_kernel<T, ORDER, CLASSIC_S4>(c, a, grid);
+    case FUSED_A: return launch_pipe_kernel<T, ORDER, FUSED_A>(c, a, grid);
+    default: return launch_pipe_kernel<T, ORDER, FUSED_B>(c, a, grid);
   }
 }
+
+template <typename T>
+int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  a.boxes = tab<BoxDev>(c, L.off_boxes);
+  a.tiles = tab<TileDev>(c, L.off_tiles);
+  a.g = P.p.nghost;
+  a.ox = P.ox;
+  const double h2 = L.h * L.h;
+  a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : 1.0 / (12.0 * h2));
+  a.a_mass = (T)P.p.a_mass;
+  const int grid = (int)L.tiles.size();
+  cudaError_t e;
+  {
+    Timed tm(c, KIND_STAGE);
+    e = P.p.lap_order == 1 ? launch_pipe_mode<T, 1>(c, a, grid, mode) : launch_pipe_mode<T, 2>(c, a, grid, mode);
+  }
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "k_rk_pipe: %s", cudaGetErrorString(e));
+  return check_launch(c, "k_rk_pipe");
+}
+
+template <typename T>
+void set_eta(const Plan& P, PipeArgs<T>& a, int slot, double eta_s) {
+  a.lam_eta2[slot] = (T)(P.p.lambda * (eta_s * eta_s));
+  a.fric[slot] = (T)(P.p.friction != 0.0 ? P.p.friction / eta_s : 0.0);
+}
+
+// The level's new state `nbuf` becomes current; the previous one is kept as `old` (L72).
+void finish_step(LevelHost& L, int nbuf, double t, double dt) {
+  L.old = L.cur & 3;
+  L.cur = nbuf & 3;
+  L.t_old = t;
+  L.t_new = t + dt;
+  L.have_pair = true;
+}
+
+// FUSED data-flow (k_rk_pipe.cuh): pass 0 = RK4 stages 1+2 (Y -> U3), pass 1 = stages 3+4 (Y, U3 -> Ynew).
+// Buffers: cur = Y, cur+1 = U3, cur+2 = Ynew.  Pi is differenced, so its ghosts are filled too.
+template <typename T>
+int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double eta_const) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  const int cur = L.cur;
+  const bool fx = P.p.eta_fixed != 0;
+  PipeArgs<T> a;
+  memset(&a, 0, sizeof a);
+  set_eta(P, a, 0, fx ? eta_const : t);
+  set_eta(P, a, 1, fx ? eta_const : t + 0.5 * dt);
+  set_eta(P, a, 2, fx ? eta_const : t + dt);
+  a.adt = (T)dt;
+  int rc;
+  if (pass == 0) {
+    rc = launch_ghosts<T>(c, l, cur, t, true);
+    if (rc) return rc;
+    a.sten[0] = plane_ptr<T>(c, l, cur, 0);
+    a.sten[1] = plane_ptr<T>(c, l, cur, 1);
+    a.out_psi[0] = plane_ptr<T>(c, l, cur + 1, 0);
+    a.out_pi[0] = plane_ptr<T>(c, l, cur + 1, 1);
+    return launch_k1<T>(c, l, FUSED_A, a);
+  }
+  rc = launch_ghosts<T>(c, l, cur + 1, t + 0.5 * dt, true);  // Y's ghosts are still valid from pass 0
+  if (rc) return rc;
+  a.sten[0] = plane_ptr<T>(c, l, cur + 1, 0);
+  a.sten[1] = plane_ptr<T>(c, l, cur + 1, 1);
+  a.sten[2] = plane_ptr<T>(c, l, cur, 0);
+  a.pnt[0] = plane_ptr<T>(c, l, cur, 1);
+  a.out_psi[0] = plane_ptr<T>(c, l, cur + 2, 0);
+  a.out_pi[0] = plane_ptr<T>(c, l, cur + 2, 1);
+  rc = launch_k1<T>(c, l, FUSED_B, a);
+  if (rc) return rc;
+  finish_step(L, cur + 2, t, dt);
+  return SLEDGE_OK;
+}
+
+// Fused sweeps need every psi AND Pi ghost to be a copy of a valid cell of the same level, which holds on
+// level 0 (it covers the periodic domain, L39); finer levels take their ghosts from time-interpolated coarse
+// data at every stage time (L72) and run the LEAN stages.
+inline bool level_is_fused(const Plan& P, int l) { return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0; }
 
 // One RK4 stage of level l: ghost fill of the stage input at its time, then K1.
 // t = time at the start of the level's step, eta_const = eta used when eta_fixed.
@@ -362,12 +468,17 @@ template <typename T>
 int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
+  if (level_is_fused(P, l)) {  // stage calls 1 and 3 run the two sweeps, 0 and 2 are no-ops
+    if (s == 1) return do_fused_pass<T>(c, l, 0, t, dt, eta_const);
+    if (s == 3) return do_fused_pass<T>(c, l, 1, t, dt, eta_const);
+    return SLEDGE_OK;
+  }
   static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
   static const double as[4] = {0.5, 0.5, 1.0, 1.0 / 6.0};
   const double ts = t + cs[s] * dt;
   const double eta_s = P.p.eta_fixed ? eta_const : ts;
   const int cur = L.cur;
-  const bool lean = P.p.rk_dataflow == SLEDGE_RK_LEAN;
+  const bool lean = P.p.rk_dataflow != SLEDGE_RK_CLASSIC;
   int ubuf, mode, in[3] = {-1, -1, -1}, out[2] = {-1, -1};
   double adt = (s < 3) ? as[s] * dt : dt / 6.0, bdt = 0.0;
   if (lean) {  // buffers: cur = Y, cur+1 = U2 (then Ynew), cur+2 = U3, cur+3 = U4
@@ -383,46 +494,26 @@ int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const)
   }
   int rc = launch_ghosts<T>(c, l, ubuf, ts, false);
   if (rc) return rc;
-  StageArgs<T> a;
+  PipeArgs<T> a;
   memset(&a, 0, sizeof a);
-  a.boxes = tab<BoxDev>(c, L.off_boxes);
-  a.tiles = tab<TileDev>(c, L.off_tiles);
-  a.u_psi = plane_ptr<T>(c, l, ubuf, 0);
-  a.u_pi = plane_ptr<T>(c, l, ubuf, 1);
+  a.sten[0] = plane_ptr<T>(c, l, ubuf, 0);
+  a.pnt[0] = plane_ptr<T>(c, l, ubuf, 1);
   for (int q = 0; q < 3; ++q)
     if (in[q] >= 0) {
-      a.in_psi[q] = plane_ptr<T>(c, l, in[q], 0);
-      a.in_pi[q] = plane_ptr<T>(c, l, in[q], 1);
+      a.pnt[1 + 2 * q] = plane_ptr<T>(c, l, in[q], 0);
+      a.pnt[2 + 2 * q] = plane_ptr<T>(c, l, in[q], 1);
     }
   for (int q = 0; q < 2; ++q)
     if (out[q] >= 0) {
       a.out_psi[q] = plane_ptr<T>(c, l, out[q], 0);
       a.out_pi[q] = plane_ptr<T>(c, l, out[q], 1);
     }
-  a.g = P.p.nghost;
-  a.ox = P.ox;
-  const double h2 = L.h * L.h;
-  a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : 1.0 / (12.0 * h2));
-  a.lam_eta2 = (T)(P.p.lambda * (eta_s * eta_s));
-  a.a_mass = (T)P.p.a_mass;
-  a.fric = (T)(P.p.friction != 0.0 ? P.p.friction / eta_s : 0.0);
+  set_eta(P, a, 0, eta_s);
   a.adt = (T)adt;
   a.bdt = (T)bdt;
-  const int grid = (int)L.tiles.size();
-  {
-    Timed tm(c, KIND_STAGE);
-    if (P.p.lap_order == 1) launch_stage_mode<T, 1>(c, a, grid, mode);
-    else launch_stage_mode<T, 2>(c, a, grid, mode);
-  }
-  rc = check_launch(c, "k_rk_stage");
+  rc = launch_k1<T>(c, l, mode, a);
   if (rc) return rc;
-  if (s == 3) {  // the new state becomes current; the previous one is kept as `old` (L72)
-    L.old = cur & 3;
-    L.cur = (cur + 1) & 3;
-    L.t_old = t;
-    L.t_new = t + dt;
-    L.have_pair = true;
-  }
+  if (s == 3) finish_step(L, cur + 1, t, dt);
   return SLEDGE_OK;
 }
 

@@ -83,12 +83,12 @@ def _c1_run(flow, dt, steps, literal):
     return eta
 
 
-@pytest.mark.parametrize("flow", ["lean", "classic"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
 def test_c1_literal_32cubed_10_steps_with_tags(flow):
     _c1_run(flow, dt=inputs.CONFIGS["C1"].dt, steps=10, literal=True)
 
 
-@pytest.mark.parametrize("flow", ["lean", "classic"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
 def test_c1s_stabilised_32cubed_eta_1_to_3p5_with_tags(flow):
     eta = _c1_run(flow, dt=0.0625, steps=40, literal=False)
     assert eta == pytest.approx(3.5)
@@ -109,7 +109,7 @@ def _ragged_boxes():
 
 
 @pytest.mark.parametrize("order,g", [(1, 1), (1, 3), (2, 2), (2, 3)])
-@pytest.mark.parametrize("flow", ["lean", "classic"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
 def test_ragged_multibox_fp64(order, g, flow):
     P = _pair()
     n0 = (40, 24, 72)
@@ -214,7 +214,7 @@ def test_average_down_matches_oracle_bitwise():
 
 # ---- AMR with subcycling ---------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("flow", ["lean", "classic"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
 def test_two_level_subcycled_steps(flow):
     P = _pair()
     n0 = 32
