@@ -34,7 +34,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="sledge", choices=["sledge", "reference"])
-    ap.add_argument("--flow", default="lean", choices=["lean", "classic"])
+    ap.add_argument("--flow", default="fused", choices=["fused", "lean", "classic"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -292,7 +292,12 @@ def run_sledge(args, cfg):
 
     # ---- roofline of the dominant kernel (K1) -----------------------------------------------------
     esz = 8 if cfg.dtype == "f64" else 4
-    words_per_cell_step = 52 if args.flow == "lean" else 64
+    # algorithmic words (reals read + written) per cell-step of the data-flow that runs:
+    # FUSED 20 on level 0 (finer levels run LEAN), LEAN 52, CLASSIC 64
+    flow_words = {"fused": 20, "lean": 52, "classic": 64}
+    stage_words_per_step = sum(n * (1 << l) * (flow_words[args.flow] if (l == 0 or args.flow != "fused") else 52)
+                               for l, n in enumerate(per_level))
+    words_per_cell_step = stage_words_per_step / cell_steps
     n_stage, ms_stage = prof["stage"]
     peaks = {}
     try:
@@ -302,9 +307,9 @@ def run_sledge(args, cfg):
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     # profile counters cover the timed K steps: n_stage launches moved cell_steps * words * esz bytes per step
-    stage_bytes_total = cell_steps * words_per_cell_step * esz * args.steps
+    stage_bytes_total = stage_words_per_step * esz * args.steps
     achieved = stage_bytes_total / (ms_stage * 1e-3) / 1e9 if ms_stage > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_rk_stage (K1, mean over the 4 stage launches)", "achieved": achieved,
+    roofline = {"bound": "hbm", "kernel": "k_rk_pipe (K1, mean over the stage launches of a step: 2 sweeps per level-step FUSED, 4 otherwise)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "peak_source": peak_src, "traffic": None,
                 "bytes_per_cell_step": words_per_cell_step * esz,
