@@ -1,0 +1,82 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The oracle cannot step a 512^3 or 1024^3 grid in seconds, but the path is periodic and translation invariant
+(pinned for the oracle in test_oracle_pins.py::test_translation_invariance_bit_for_bit): a field
+that repeats with period P cells evolves into a field that repeats with period P, and every one of its periods
+equals the run on the P^3 periodic grid.  So the full-size GPU run started from a P^3 seeded GRF tiled N/P times
+per axis (inputs.tile_periodic) is compared, at EVERY cell, with the tiled result of the P^3 oracle run: same
+parameters, same step count as the config, all of the full-size grid's K1 tiles, z chunks and ghost wraps.
+Tags and per-32^3 block counts are compared bit for bit on the uploaded oracle state (R19).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2404_02950_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+F64_TOL = 1e-11
+F32_TOL = 2e-5
+
+
+def _run_tiled(name, period, flow, steps=None, check_tags=False):
+    from oracle.oracle import Oracle
+    from paper_2404_02950_b200.sledge import Sledge
+    cfg = inputs.CONFIGS[name]
+    steps = cfg.steps if steps is None else steps
+    reps = cfg.n0 // period
+    tdt = torch.float64 if cfg.dtype == "f64" else torch.float32
+    o = Oracle(period, nghost=cfg.nghost, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam)
+    s = Sledge(cfg.n0, nghost=cfg.nghost, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, dtype=cfg.dtype,
+               rk_dataflow=flow)
+    # the band limit is a fraction of k_Nyquist = pi/h, the same on the small and on the full grid
+    for c, seed in enumerate(cfg.seeds):
+        small = inputs.grf(period, cfg.grf_f, seed).to(tdt)
+        o.set_state(0, c, small.to(torch.float64).numpy())
+        s.set_state(0, c, inputs.tile_periodic(small.cuda(), reps).contiguous())
+    eta = cfg.eta0
+    for _ in range(steps):
+        o.rk_step(cfg.dt, eta)
+        s.rk_step(cfg.dt, eta)
+        eta += cfg.dt
+    s.synchronize()
+    worst = 0.0
+    for c in range(4):
+        ref = torch.from_numpy(o.get_state(0, c)).cuda()
+        got = s.get_state(0, c).to(torch.float64)
+        err = float((got.view(reps, period, reps, period, reps, period) - ref[None, :, None, :, None, :]).abs().max())
+        scale = float(ref.abs().max()) if cfg.dtype == "f32" else 1.0
+        worst = max(worst, err / scale if scale > 0 else err)
+        del got, ref
+    assert worst <= (F64_TOL if cfg.dtype == "f64" else F32_TOL), worst
+    if check_tags:
+        for c in range(4):
+            ref = torch.from_numpy(o.get_state(0, c)).to(tdt).cuda()
+            s.set_state(0, c, inputs.tile_periodic(ref, reps).contiguous())
+        ot, oc = o.tag_strings(0)
+        gt, gc = s.tag_strings(0)
+        s.synchronize()
+        want = inputs.tile_periodic(torch.from_numpy(ot[0]).cuda(), reps)
+        assert torch.equal(s.split_tags(0, gt)[0], want)
+        wantc = inputs.tile_periodic(torch.from_numpy(oc.astype(np.int32)).cuda(), reps)
+        assert torch.equal(gc, wantc)
+        assert int((ot[0] != 0).sum()) > 0
+    s.close()
+    return worst
+
+
+@pytest.mark.parametrize("flow", ["fused", "lean"])
+def test_c3_512cubed_fp64_13pt_50_steps_all_cells_and_tags(flow):
+    _run_tiled("C3", 64, flow, check_tags=True)
+
+
+def test_c2_256cubed_fp64_7pt_100_steps_all_cells():
+    _run_tiled("C2", 64, "fused")
+
+
+def test_c4_1024cubed_fp32_7pt_20_steps_all_cells_and_tags():
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs ~80 GB of free HBM")
+    _run_tiled("C4", 64, "fused", check_tags=True)
