@@ -93,21 +93,30 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// Laplacian of one component from its 6 (12) neighbours; same association as the definition:
-// sum_d [(u+ - u) + (u- - u)], x then y then z; order 2: (16 s1 - s2) / (12 h^2).
+// Laplacian of one component from its 6 (12) neighbours.  The library is compiled with --fmad=false (the tag
+// rule needs individually rounded products); K1 is where the fp64 pipe matters, so it contracts explicitly:
+// neighbour-sum form s_r = sum_d (u(+r e_d) + u(-r e_d)), then
+//   order 1: (s1 - 6u) / h^2            order 2: (16 s1 - s2 - 90u) / (12 h^2)
+// 13 fp64 instructions for the 13-point stencil instead of 25 in difference form.  The result differs from the
+// oracle's difference form by rounding only (|err| <~ 1e-15 / h^2 on O(1) fields).
 template <typename T, int ORDER>
 __device__ __forceinline__ T lap_from(T u, const T* xm, const T* xp, const T* ym, const T* yp, const T* zm,
                                       const T* zp, T inv_h2) {
-  T n1x = (xp[0] - u) + (xm[0] - u);
-  T n1y = (yp[0] - u) + (ym[0] - u);
-  T n1z = (zp[0] - u) + (zm[0] - u);
-  T s1 = (n1x + n1y) + n1z;
-  if (ORDER == 1) return s1 * inv_h2;
-  T n2x = (xp[1] - u) + (xm[1] - u);
-  T n2y = (yp[1] - u) + (ym[1] - u);
-  T n2z = (zp[1] - u) + (zm[1] - u);
-  T s2 = (n2x + n2y) + n2z;
-  return (T(16) * s1 - s2) * inv_h2;
+  const T s1 = ((xp[0] + xm[0]) + (yp[0] + ym[0])) + (zp[0] + zm[0]);
+  if (ORDER == 1) return fma(T(-6), u, s1) * inv_h2;
+  const T s2 = ((xp[1] + xm[1]) + (yp[1] + ym[1])) + (zp[1] + zm[1]);
+  return fma(T(16), s1, fma(T(-90), u, -s2)) * inv_h2;
+}
+
+// k_Pi of one component (Eq.11 generalised, R2): lap - psi * pot - fric * pi, contracted
+template <typename T>
+__device__ __forceinline__ T kpi_of(T lap, T psi, T pot, T fric, T pi) {
+  return fma(-fric, pi, fma(-psi, pot, lap));
+}
+// pot = lambda eta^2 (psi1^2 + psi2^2 - 1) + a
+template <typename T>
+__device__ __forceinline__ T pot_of(T lam_eta2, T a_mass, T p1, T p2) {
+  return fma(lam_eta2, fma(p1, p1, fma(p2, p2, T(-1))), a_mass);
 }
 
 template <typename T, int ORDER, int MODE, int TX, int TY, int D>
@@ -292,78 +301,80 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
           // stages 1 + 2 (O4): U3 = Y + dt/2 k(U2), U2 = Y + dt/2 k(Y); U2 is never stored
           const T hdt = T(0.5) * a.adt;
           const T y1 = w[0][R].p[p].x, y2 = w[0][R].p[p].y, q1 = w[1][R].p[p].x, q2 = w[1][R].p[p].y;
-          const T pot1 = a.lam_eta2[0] * ((y1 * y1 + y2 * y2) - T(1)) + a.a_mass;
-          const T k1a = (lap[0][0] - y1 * pot1) - a.fric[0] * q1;
-          const T k1b = (lap[0][1] - y2 * pot1) - a.fric[0] * q2;
-          const T p2a = q1 + hdt * k1a, p2b = q2 + hdt * k1b;  // Pi(U2)
-          const T u2a = y1 + hdt * q1, u2b = y2 + hdt * q2;    // psi(U2)
-          const T l2a = lap[0][0] + hdt * lap[1][0], l2b = lap[0][1] + hdt * lap[1][1];
-          const T pot2 = a.lam_eta2[1] * ((u2a * u2a + u2b * u2b) - T(1)) + a.a_mass;
-          const T k2a = (l2a - u2a * pot2) - a.fric[1] * p2a;
-          const T k2b = (l2b - u2b * pot2) - a.fric[1] * p2b;
-          o_psi[0].p[p] = mkpair(y1 + hdt * p2a, y2 + hdt * p2b);
-          o_pi[0].p[p] = mkpair(q1 + hdt * k2a, q2 + hdt * k2b);
+          const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
+          const T k1a = kpi_of(lap[0][0], y1, pot1, a.fric[0], q1);
+          const T k1b = kpi_of(lap[0][1], y2, pot1, a.fric[0], q2);
+          const T p2a = fma(hdt, k1a, q1), p2b = fma(hdt, k1b, q2);  // Pi(U2)
+          const T u2a = fma(hdt, q1, y1), u2b = fma(hdt, q2, y2);    // psi(U2)
+          const T l2a = fma(hdt, lap[1][0], lap[0][0]), l2b = fma(hdt, lap[1][1], lap[0][1]);
+          const T pot2 = pot_of(a.lam_eta2[1], a.a_mass, u2a, u2b);
+          const T k2a = kpi_of(l2a, u2a, pot2, a.fric[1], p2a);
+          const T k2b = kpi_of(l2b, u2b, pot2, a.fric[1], p2b);
+          o_psi[0].p[p] = mkpair(fma(hdt, p2a, y1), fma(hdt, p2b, y2));
+          o_pi[0].p[p] = mkpair(fma(hdt, k2a, q1), fma(hdt, k2b, q2));
         } else if (MODE == FUSED_B) {
-          // stages 3 + 4 and the final combination; k1 recomputed from Y, dt/2 k2 = Pi3 - Pi_Y
+          // stages 3 + 4 and the final combination; k1 recomputed from Y (same expression, same bits as in
+          // PASS A), dt/2 k2 = Pi3 - Pi_Y
           const T dt = a.adt, hdt = T(0.5) * a.adt, sixth = a.adt / T(6);
           const T u3a = w[0][R].p[p].x, u3b = w[0][R].p[p].y, p3a = w[1][R].p[p].x, p3b = w[1][R].p[p].y;
           const T y1 = w[2][R].p[p].x, y2 = w[2][R].p[p].y, q1 = pv[0].p[p].x, q2 = pv[0].p[p].y;
-          const T pot3 = a.lam_eta2[1] * ((u3a * u3a + u3b * u3b) - T(1)) + a.a_mass;
-          const T k3a = (lap[0][0] - u3a * pot3) - a.fric[1] * p3a;
-          const T k3b = (lap[0][1] - u3b * pot3) - a.fric[1] * p3b;
-          const T u4a = y1 + dt * p3a, u4b = y2 + dt * p3b;  // psi(U4)
-          const T p4a = q1 + dt * k3a, p4b = q2 + dt * k3b;  // Pi(U4)
-          const T l4a = lap[2][0] + dt * lap[1][0], l4b = lap[2][1] + dt * lap[1][1];
-          const T pot4 = a.lam_eta2[2] * ((u4a * u4a + u4b * u4b) - T(1)) + a.a_mass;
-          const T k4a = (l4a - u4a * pot4) - a.fric[2] * p4a;
-          const T k4b = (l4b - u4b * pot4) - a.fric[2] * p4b;
-          const T pot1 = a.lam_eta2[0] * ((y1 * y1 + y2 * y2) - T(1)) + a.a_mass;
-          const T k1a = (lap[2][0] - y1 * pot1) - a.fric[0] * q1;
-          const T k1b = (lap[2][1] - y2 * pot1) - a.fric[0] * q2;
-          const T p2a = q1 + hdt * k1a, p2b = q2 + hdt * k1b;  // Pi(U2), same bits as in PASS A
+          const T pot3 = pot_of(a.lam_eta2[1], a.a_mass, u3a, u3b);
+          const T k3a = kpi_of(lap[0][0], u3a, pot3, a.fric[1], p3a);
+          const T k3b = kpi_of(lap[0][1], u3b, pot3, a.fric[1], p3b);
+          const T u4a = fma(dt, p3a, y1), u4b = fma(dt, p3b, y2);  // psi(U4)
+          const T p4a = fma(dt, k3a, q1), p4b = fma(dt, k3b, q2);  // Pi(U4)
+          const T l4a = fma(dt, lap[1][0], lap[2][0]), l4b = fma(dt, lap[1][1], lap[2][1]);
+          const T pot4 = pot_of(a.lam_eta2[2], a.a_mass, u4a, u4b);
+          const T k4a = kpi_of(l4a, u4a, pot4, a.fric[2], p4a);
+          const T k4b = kpi_of(l4b, u4b, pot4, a.fric[2], p4b);
+          const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
+          const T k1a = kpi_of(lap[2][0], y1, pot1, a.fric[0], q1);
+          const T k1b = kpi_of(lap[2][1], y2, pot1, a.fric[0], q2);
+          const T p2a = fma(hdt, k1a, q1), p2b = fma(hdt, k1b, q2);  // Pi(U2), same bits as in PASS A
           const T twothirds = T(2) / T(3);
-          o_psi[0].p[p] = mkpair(y1 + sixth * ((q1 + p4a) + T(2) * (p2a + p3a)),
-                                 y2 + sixth * ((q2 + p4b) + T(2) * (p2b + p3b)));
-          o_pi[0].p[p] = mkpair((q1 + twothirds * (p3a - q1)) + sixth * ((k1a + k4a) + T(2) * k3a),
-                                (q2 + twothirds * (p3b - q2)) + sixth * ((k1b + k4b) + T(2) * k3b));
+          o_psi[0].p[p] = mkpair(fma(sixth, (q1 + p4a) + T(2) * (p2a + p3a), y1),
+                                 fma(sixth, (q2 + p4b) + T(2) * (p2b + p3b), y2));
+          o_pi[0].p[p] = mkpair(fma(sixth, fma(T(2), k3a, k1a + k4a), fma(twothirds, p3a - q1, q1)),
+                                fma(sixth, fma(T(2), k3b, k1b + k4b), fma(twothirds, p3b - q2, q2)));
         } else {
           const T psi1 = w[0][R].p[p].x, psi2 = w[0][R].p[p].y;
           const T pi1 = pv[0].p[p].x, pi2 = pv[0].p[p].y;
-          const T pot = a.lam_eta2[0] * ((psi1 * psi1 + psi2 * psi2) - T(1)) + a.a_mass;
+          const T pot = pot_of(a.lam_eta2[0], a.a_mass, psi1, psi2);
           const T kpsi1 = pi1, kpsi2 = pi2;
-          const T kpi1 = (lap[0][0] - psi1 * pot) - a.fric[0] * pi1;
-          const T kpi2 = (lap[0][1] - psi2 * pot) - a.fric[0] * pi2;
+          const T kpi1 = kpi_of(lap[0][0], psi1, pot, a.fric[0], pi1);
+          const T kpi2 = kpi_of(lap[0][1], psi2, pot, a.fric[0], pi2);
           // pointwise inputs: in_psi(q) = pv[1 + 2q], in_pi(q) = pv[2 + 2q]
           auto ipsi = [&](int q) -> const P& { return pv[(1 + 2 * q) < NPA ? (1 + 2 * q) : 0].p[p]; };
           auto ipi = [&](int q) -> const P& { return pv[(2 + 2 * q) < NPA ? (2 + 2 * q) : 0].p[p]; };
+          auto axpy = [](T c, T k, T y) -> T { return fma(c, k, y); };
           if (MODE == LEAN_S1) {  // U2 = U + adt k   (U = Y)
-            o_psi[0].p[p] = mkpair(psi1 + a.adt * kpsi1, psi2 + a.adt * kpsi2);
-            o_pi[0].p[p] = mkpair(pi1 + a.adt * kpi1, pi2 + a.adt * kpi2);
+            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, psi1), axpy(a.adt, kpsi2, psi2));
+            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, pi1), axpy(a.adt, kpi2, pi2));
           } else if (MODE == LEAN_S23) {  // U' = Y + adt k   (in0 = Y)
-            o_psi[0].p[p] = mkpair(ipsi(0).x + a.adt * kpsi1, ipsi(0).y + a.adt * kpsi2);
-            o_pi[0].p[p] = mkpair(ipi(0).x + a.adt * kpi1, ipi(0).y + a.adt * kpi2);
+            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
+            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
           } else if (MODE == LEAN_S4) {  // in0 = Y, in1 = U2, in2 = U3, U = U4, adt = dt/6
             const T third = T(1) / T(3);
             auto comb = [&](T yv, T u2, T u3, T u4, T kk) -> T {
-              return (((u2 + T(2) * u3) + u4) - yv) * third + a.adt * kk;
+              return fma(a.adt, kk, ((fma(T(2), u3, u2) + u4) - yv) * third);
             };
             o_psi[0].p[p] = mkpair(comb(ipsi(0).x, ipsi(1).x, ipsi(2).x, psi1, kpsi1),
                                    comb(ipsi(0).y, ipsi(1).y, ipsi(2).y, psi2, kpsi2));
             o_pi[0].p[p] = mkpair(comb(ipi(0).x, ipi(1).x, ipi(2).x, pi1, kpi1),
                                   comb(ipi(0).y, ipi(1).y, ipi(2).y, pi2, kpi2));
           } else if (MODE == CLASSIC_S1) {  // out0 = U + adt k ; out1 (ACC) = U + bdt k
-            o_psi[0].p[p] = mkpair(psi1 + a.adt * kpsi1, psi2 + a.adt * kpsi2);
-            o_pi[0].p[p] = mkpair(pi1 + a.adt * kpi1, pi2 + a.adt * kpi2);
-            o_psi[NOUT - 1].p[p] = mkpair(psi1 + a.bdt * kpsi1, psi2 + a.bdt * kpsi2);
-            o_pi[NOUT - 1].p[p] = mkpair(pi1 + a.bdt * kpi1, pi2 + a.bdt * kpi2);
+            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, psi1), axpy(a.adt, kpsi2, psi2));
+            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, pi1), axpy(a.adt, kpi2, pi2));
+            o_psi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpsi1, psi1), axpy(a.bdt, kpsi2, psi2));
+            o_pi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpi1, pi1), axpy(a.bdt, kpi2, pi2));
           } else if (MODE == CLASSIC_S23) {  // in0 = Y, in1 = ACC ; out0 = Y + adt k ; out1 = ACC + bdt k
-            o_psi[0].p[p] = mkpair(ipsi(0).x + a.adt * kpsi1, ipsi(0).y + a.adt * kpsi2);
-            o_pi[0].p[p] = mkpair(ipi(0).x + a.adt * kpi1, ipi(0).y + a.adt * kpi2);
-            o_psi[NOUT - 1].p[p] = mkpair(ipsi(1).x + a.bdt * kpsi1, ipsi(1).y + a.bdt * kpsi2);
-            o_pi[NOUT - 1].p[p] = mkpair(ipi(1).x + a.bdt * kpi1, ipi(1).y + a.bdt * kpi2);
+            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
+            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
+            o_psi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpsi1, ipsi(1).x), axpy(a.bdt, kpsi2, ipsi(1).y));
+            o_pi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpi1, ipi(1).x), axpy(a.bdt, kpi2, ipi(1).y));
           } else {  // CLASSIC_S4: in0 = ACC ; out0 = ACC + adt k
-            o_psi[0].p[p] = mkpair(ipsi(0).x + a.adt * kpsi1, ipsi(0).y + a.adt * kpsi2);
-            o_pi[0].p[p] = mkpair(ipi(0).x + a.adt * kpi1, ipi(0).y + a.adt * kpi2);
+            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
+            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
           }
         }
       }

@@ -42,9 +42,25 @@ constexpr size_t ALIGN = 256;
 #ifndef SLEDGE_K1_SMEM
 #define SLEDGE_K1_SMEM (227 * 1024)
 #endif
+// The FUSED sweeps are not HBM-bound (fp64 pipe, shared-memory bandwidth and HBM all within 2x of each other):
+// they want several small CTAs per SM so that one CTA's barrier / load phase overlaps another's arithmetic.
+// Measured on C3 (profiles/r01_k1_tile_sweep.md): 32x8 threads with a 56 KB budget (3-4 CTAs per SM).
+#ifndef SLEDGE_K1F_TY
+#define SLEDGE_K1F_TY 8
+#endif
+#ifndef SLEDGE_K1F_SMEM
+#define SLEDGE_K1F_SMEM (56 * 1024)
+#endif
 constexpr int K1_TX = 32, K1_TY = SLEDGE_K1_TY, K1_NZ = SLEDGE_K1_NZ;
 constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
+constexpr int K1F_TY = SLEDGE_K1F_TY;            // tile rows / budget of the FUSED sweeps
+constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
+template <int MODE> struct K1Shape {
+  static constexpr bool fused = (MODE == FUSED_A || MODE == FUSED_B);
+  static constexpr int TY = fused ? K1F_TY : K1_TY;
+  static constexpr size_t SMEM = fused ? K1F_SMEM : K1_SMEM;
+};
 
 thread_local std::string g_err;
 
@@ -54,7 +70,7 @@ struct LevelHost {
   std::vector<int> boxes;  // global box ids in input order
   std::vector<BoxDev> boxdev;
   std::vector<int> owner;
-  std::vector<TileDev> tiles, tag_tiles;
+  std::vector<TileDev> tiles, ftiles, tag_tiles;  // K1 staged / K1 fused / K3
   std::vector<int> ghost_prefix, avg_prefix;
   long long plane_cells = 0;  // pairs per plane (all boxes, ghosts and padding included)
   long long valid_cells = 0;
@@ -62,7 +78,7 @@ struct LevelHost {
   int nb[3];
   // arena offsets (bytes)
   size_t off_buf[NBUF][2];
-  size_t off_boxes, off_tiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix;
+  size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix;
   // run state
   int cur = 0, old = 0;
   bool have_pair = false;
@@ -222,6 +238,9 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
         for (int y0 = 0; y0 < b.n[1]; y0 += K1_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
       for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
+        for (int y0 = 0; y0 < b.n[1]; y0 += K1F_TY)
+          for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
+      for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
         for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
       const long long Gx = b.n[0] + 2 * g, Gy = b.n[1] + 2 * g;
@@ -245,6 +264,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       for (int c = 0; c < 2; ++c) L.off_buf[b][c] = take(plane_bytes);
     L.off_boxes = take(L.boxdev.size() * sizeof(BoxDev));
     L.off_tiles = take(L.tiles.size() * sizeof(TileDev));
+    L.off_ftiles = take(L.ftiles.size() * sizeof(TileDev));
     L.off_tag_tiles = take(L.tag_tiles.size() * sizeof(TileDev));
     L.off_owner = take(L.owner.size() * sizeof(int));
     L.off_ghost_prefix = take(L.ghost_prefix.size() * sizeof(int));
@@ -356,17 +376,18 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
 
 template <typename T, int ORDER, int MODE>
 cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
-  constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, K1_TY>(K1_SMEM, K1_DMAX);
-  static_assert(PipeCfg<T, ORDER, MODE, K1_TX, K1_TY, D>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
-  using C = PipeCfg<T, ORDER, MODE, K1_TX, K1_TY, D>;
-  auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, K1_TY, D>;
+  constexpr int TY = K1Shape<MODE>::TY;
+  constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, TY>(K1Shape<MODE>::SMEM, K1_DMAX);
+  static_assert(PipeCfg<T, ORDER, MODE, K1_TX, TY, D>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
+  using C = PipeCfg<T, ORDER, MODE, K1_TX, TY, D>;
+  auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, TY, D>;
   static bool configured = false;  // per instantiation
   if (!configured) {
     const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  kern<<<grid, K1_TX * K1_TY, C::SMEM_BYTES, c->stream>>>(a);
+  kern<<<grid, K1_TX * TY, C::SMEM_BYTES, c->stream>>>(a);
   return cudaSuccess;
 }
 template <typename T, int ORDER>
@@ -388,13 +409,14 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
   a.boxes = tab<BoxDev>(c, L.off_boxes);
-  a.tiles = tab<TileDev>(c, L.off_tiles);
+  const bool fused = (mode == FUSED_A || mode == FUSED_B);
+  a.tiles = tab<TileDev>(c, fused ? L.off_ftiles : L.off_tiles);
   a.g = P.p.nghost;
   a.ox = P.ox;
   const double h2 = L.h * L.h;
   a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : 1.0 / (12.0 * h2));
   a.a_mass = (T)P.p.a_mass;
-  const int grid = (int)L.tiles.size();
+  const int grid = (int)(fused ? L.ftiles.size() : L.tiles.size());
   cudaError_t e;
   {
     Timed tm(c, KIND_STAGE);
@@ -653,6 +675,7 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   for (LevelHost& L : P.lev) {
     up(L.off_boxes, L.boxdev.data(), L.boxdev.size() * sizeof(BoxDev));
     up(L.off_tiles, L.tiles.data(), L.tiles.size() * sizeof(TileDev));
+    up(L.off_ftiles, L.ftiles.data(), L.ftiles.size() * sizeof(TileDev));
     up(L.off_tag_tiles, L.tag_tiles.data(), L.tag_tiles.size() * sizeof(TileDev));
     up(L.off_owner, L.owner.data(), L.owner.size() * sizeof(int));
     up(L.off_ghost_prefix, L.ghost_prefix.data(), L.ghost_prefix.size() * sizeof(int));
