@@ -98,7 +98,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
 // neighbour-sum form s_r = sum_d (u(+r e_d) + u(-r e_d)), then
 //   order 1: (s1 - 6u) / h^2            order 2: (16 s1 - s2 - 90u) / (12 h^2)
 // 13 fp64 instructions for the 13-point stencil instead of 25 in difference form.  The result differs from the
-// oracle's difference form by rounding only (|err| <~ 1e-15 / h^2 on O(1) fields).
+// difference form sum_d [(u+ - u) + (u- - u)] by rounding only (|err| <~ 1e-15 / h^2 on O(1) fields; R11).
 template <typename T, int ORDER>
 __device__ __forceinline__ T lap_from(T u, const T* xm, const T* xp, const T* ym, const T* yp, const T* zm,
                                       const T* zp, T inv_h2) {
