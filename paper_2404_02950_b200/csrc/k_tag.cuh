@@ -8,18 +8,30 @@
 // tag bit0/1/2 = winding(xy / yz / zx) != 0.  Per aligned 32^3 block of the level index space: number of
 // cells with tag != 0 (tagging statistics, L776).
 //
-// Mapping: a warp owns 32 consecutive x cells of one row and marches along z; a CTA is TAG_TY such rows.
-// Every thread loads its own cell (x,y) and (x,y+1) of each new plane; the +x neighbours come from the
-// next lane by shuffle (lane 31 loads them).  The previous plane stays in registers, so each psi value is
-// fetched from L1/L2 at most twice and from HBM once.  Counts: ballot + popc per plane, accumulated per
-// warp across the march and flushed with one atomicAdd whenever the warp leaves a 32-block in z.
+// Mapping (edge form).  The contribution E(a->b) of an edge is antisymmetric bit for bit: the reversed edge
+// swaps up/dn and negates cr exactly (same two rounded products, x - y = -(y - x) in IEEE), so
+//   W_xy(P) = Ex(P) + Ey(P+x) - Ex(P+y) - Ey(P)      Ex/Ey/Ez(P) = E(P -> P+e_x / e_y / e_z)
+//   W_yz(P) = Ey(P) + Ez(P+y) - Ey(P+z) - Ez(P)
+//   W_zx(P) = Ez(P) + Ex(P+z) - Ez(P+x) - Ex(P)
+// and only the edges that START at a cell are ever evaluated (3 cross products per cell instead of 12).
+// A warp owns a 31 x TAG_RY patch of cells and marches along z without any block-level synchronisation: lane l
+// holds the column x0+l of TAG_RY+1 rows (the last row and lane 31 are halo: they only supply edges), the
+// plane below stays in registers, loads run one plane ahead, psi(P+x) and the packed edges of P+x come from
+// lane l+1 by shuffle.  Per plane and thread: Ex, Ez on TAG_RY+1 rows and Ey on TAG_RY rows (3.5 edges per cell
+// for TAG_RY = 4).  Warps step by 31 cells in x so that every lane's +x partner is in the warp.
+// Counts: per-thread counters, reduced over the warp (redux) and flushed with one atomicAdd per 32-block
+// whenever the warp leaves a 32-block in z.
 #pragma once
 #include "layout.h"
 
 namespace sledge {
 
-constexpr int TAG_TX = 32;
-constexpr int TAG_TY = 8;
+constexpr int TAG_TX = 31;                 // cells per warp row that produce tags (lane 31 is the +x halo)
+constexpr int TAG_RY = 4;                  // rows per warp
+constexpr int TAG_WARPS = 4;               // warps per CTA, stacked in y
+constexpr int TAG_TY = TAG_RY * TAG_WARPS; // rows per CTA tile
+constexpr int TAG_THREADS = TAG_WARPS * 32;
+static_assert(TAG_RY <= 32, "a warp's rows may straddle at most two 32-blocks");
 
 template <typename T>
 struct TagArgs {
@@ -33,27 +45,22 @@ struct TagArgs {
   int nb0, nb1;  // count blocks per axis (x, y)
 };
 
-template <typename T>
-__device__ __forceinline__ int edge_cross(T a1, T a2, T b1, T b2);
-template <>
-__device__ __forceinline__ int edge_cross<double>(double a1, double a2, double b1, double b2) {
-  const bool up = (a2 < 0.0) && (b2 >= 0.0);
-  const bool dn = (a2 >= 0.0) && (b2 < 0.0);
-  const double cr = __dsub_rn(__dmul_rn(a1, b2), __dmul_rn(a2, b1));
-  return (up && cr > 0.0) ? 1 : ((dn && cr < 0.0) ? -1 : 0);
+// individually rounded a1*b2 - a2*b1 (R8: no FMA)
+__device__ __forceinline__ double cross_rn(double a1, double a2, double b1, double b2) {
+  return __dsub_rn(__dmul_rn(a1, b2), __dmul_rn(a2, b1));
 }
-template <>
-__device__ __forceinline__ int edge_cross<float>(float a1, float a2, float b1, float b2) {
-  const bool up = (a2 < 0.f) && (b2 >= 0.f);
-  const bool dn = (a2 >= 0.f) && (b2 < 0.f);
-  const float cr = __fsub_rn(__fmul_rn(a1, b2), __fmul_rn(a2, b1));
-  return (up && cr > 0.f) ? 1 : ((dn && cr < 0.f) ? -1 : 0);
+__device__ __forceinline__ float cross_rn(float a1, float a2, float b1, float b2) {
+  return __fsub_rn(__fmul_rn(a1, b2), __fmul_rn(a2, b1));
 }
 
+// E(a -> b): +1 if up && cr > 0, -1 if dn && cr < 0, else 0, with up = a2<0 && b2>=0, dn = a2>=0 && b2<0
+// (the comparisons are written as in the definition so that NaN / -0 behave identically)
 template <typename T, typename P>
-__device__ __forceinline__ int winding(const P& A, const P& B, const P& C, const P& D) {
-  return edge_cross<T>(A.x, A.y, B.x, B.y) + edge_cross<T>(B.x, B.y, C.x, C.y) + edge_cross<T>(C.x, C.y, D.x, D.y) +
-         edge_cross<T>(D.x, D.y, A.x, A.y);
+__device__ __forceinline__ int edge_of(const P& a, const P& b) {
+  const T cr = cross_rn(a.x, a.y, b.x, b.y);
+  const bool up = (a.y < T(0)) && (b.y >= T(0));
+  const bool dn = (a.y >= T(0)) && (b.y < T(0));
+  return (up && cr > T(0)) ? 1 : ((dn && cr < T(0)) ? -1 : 0);
 }
 
 template <typename P>
@@ -67,75 +74,107 @@ __device__ __forceinline__ float2 shfl_down_pair<float2>(const float2& v, int de
   return make_float2(__shfl_down_sync(0xffffffffu, v.x, delta), __shfl_down_sync(0xffffffffu, v.y, delta));
 }
 
+
+
+// edges of P+x packed for the shuffle: (Ey+1) | (Ez+1)<<2
 template <typename T>
-__global__ void __launch_bounds__(TAG_TX* TAG_TY) k_tag_strings(const TagArgs<T> a) {
+__global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a) {
   using P = typename PairOf<T>::type;
+  constexpr int RY = TAG_RY;
   const TileDev t = a.tiles[blockIdx.x];
   const BoxDev b = a.boxes[t.box];
-  const int lane = threadIdx.x % TAG_TX, ty = threadIdx.x / TAG_TX;
-  const int x = t.x0 + lane, y = t.y0 + ty;
-  if (y >= b.n[1]) return;  // whole warp leaves together (a warp is one row)
-  // lanes past the box edge clamp to the last valid cell: they load valid memory and write nothing
-  const bool act = x < b.n[0];
-  const int xc = act ? x : b.n[0] - 1;
-  const bool edge = (lane == TAG_TX - 1) || (x == b.n[0] - 1);  // must load its own +x neighbour
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int x = t.x0 + lane, y0 = t.y0 + warp * RY;
+  if (y0 >= b.n[1]) return;  // whole warp leaves together; there is no block-level synchronisation
+  // cells past the box edge clamp to the first ghost layer (g >= 1): valid memory, results unused
+  const int xc = min(x, b.n[0]);
+  const bool actx = lane < TAG_TX && x < b.n[0];
   const long long plane = (long long)b.sx * b.sy;
-  long long off = b.base + ((long long)(t.z0 + a.g) * b.sy + (y + a.g)) * b.sx + (xc + a.ox);
+  const long long org = b.base + (long long)(t.z0 + a.g) * plane + (xc + a.ox);
+  long long orow[RY + 1];
+#pragma unroll
+  for (int r = 0; r <= RY; ++r) orow[r] = org + (long long)(min(y0 + r, b.n[1]) + a.g) * b.sx;
 
-  auto load_plane = [&](long long o, P& c00, P& c10, P& c01, P& c11) {
-    c00 = __ldg(a.psi + o);
-    c01 = __ldg(a.psi + o + b.sx);
-    P e0 = c00, e1 = c01;
-    if (edge) {
-      e0 = __ldg(a.psi + o + 1);
-      e1 = __ldg(a.psi + o + b.sx + 1);
-    }
-    c10 = shfl_down_pair<P>(c00, 1);
-    c11 = shfl_down_pair<P>(c01, 1);
-    if (edge) {
-      c10 = e0;
-      c11 = e1;
-    }
-  };
+  // plane index n is relative to t.z0; n = nz is the first plane above the tile (a ghost plane or the next tile)
+  auto ld = [&](int r, int n) -> P { return __ldg(a.psi + orow[r] + (long long)min(n, t.nz) * plane); };
+  P pre[RY + 1], cur[RY + 1];
+#pragma unroll
+  for (int r = 0; r <= RY; ++r) {
+    pre[r] = ld(r, 0);
+    cur[r] = pre[r];
+  }
+  int exc[RY], eyc[RY], wxyc[RY];  // in-plane edges and W_xy of the plane below
+#pragma unroll
+  for (int r = 0; r < RY; ++r) exc[r] = eyc[r] = wxyc[r] = 0;
 
-  P c00, c10, c01, c11;  // plane k:   (x,y) (x+1,y) (x,y+1) (x+1,y+1)
-  load_plane(off, c00, c10, c01, c11);
-
-  const int gx = b.lo[0] + xc, gy = b.lo[1] + y;
-  const int bi = gx >> 5, bj = gy >> 5;
+  // count blocks: lanes split over at most two x-blocks, rows over at most two y-blocks
+  const int bi = (b.lo[0] + min(x, b.n[0] - 1)) >> 5;
   const int bi0 = __shfl_sync(0xffffffffu, bi, 0);
-  int cnt0 = 0, cnt1 = 0;  // tagged cells in x-block bi0 / bi0+1 (a warp can straddle two when lo % 32 != 0)
+  const int bj0 = (b.lo[1] + y0) >> 5;
+  int cntA = 0, cntB = 0;  // this thread's tagged cells in y-block bj0 / bj0 + 1
   int cur_bk = (b.lo[2] + t.z0) >> 5;
   auto flush = [&](int bk) {
-    if (a.counts && lane == 0) {
-      if (cnt0) atomicAdd(a.counts + ((long long)bk * a.nb1 + bj) * a.nb0 + bi0, (uint32_t)cnt0);
-      if (cnt1) atomicAdd(a.counts + ((long long)bk * a.nb1 + bj) * a.nb0 + bi0 + 1, (uint32_t)cnt1);
+    if (a.counts) {
+      const unsigned m = 0xffffffffu;
+      const int v00 = __reduce_add_sync(m, bi == bi0 ? cntA : 0), v10 = __reduce_add_sync(m, bi == bi0 ? 0 : cntA);
+      const int v01 = __reduce_add_sync(m, bi == bi0 ? cntB : 0), v11 = __reduce_add_sync(m, bi == bi0 ? 0 : cntB);
+      if (lane == 0) {
+        uint32_t* const c0 = a.counts + ((long long)bk * a.nb1 + bj0) * a.nb0 + bi0;
+        if (v00) atomicAdd(c0, (uint32_t)v00);
+        if (v10) atomicAdd(c0 + 1, (uint32_t)v10);
+        if (v01) atomicAdd(c0 + a.nb0, (uint32_t)v01);
+        if (v11) atomicAdd(c0 + a.nb0 + 1, (uint32_t)v11);
+      }
     }
-    cnt0 = cnt1 = 0;
+    cntA = cntB = 0;
   };
 
-  for (int zz = 0; zz < t.nz; ++zz) {
-    const int z = t.z0 + zz;
-    P n00, n10, n01, n11;  // plane k+1
-    load_plane(off + plane, n00, n10, n01, n11);
-    const int wxy = winding<T, P>(c00, c10, c11, c01);  // A=P, B=P+x, C=P+x+y, D=P+y
-    const int wyz = winding<T, P>(c00, c01, n01, n00);  // A=P, B=P+y, C=P+y+z, D=P+z
-    const int wzx = winding<T, P>(c00, n00, n10, c10);  // A=P, B=P+z, C=P+z+x, D=P+x
-    const uint8_t tag = (uint8_t)((wxy != 0 ? 1 : 0) | (wyz != 0 ? 2 : 0) | (wzx != 0 ? 4 : 0));
-    if (a.tags && act) a.tags[b.tag_base + ((long long)z * b.n[1] + y) * b.n[0] + x] = tag;
+  for (int n = 0; n <= t.nz; ++n) {
+    P nO[RY + 1], nX[RY + 1];
+#pragma unroll
+    for (int r = 0; r <= RY; ++r) {
+      nO[r] = pre[r];
+      pre[r] = ld(r, n + 1);
+      nX[r] = shfl_down_pair<P>(nO[r], 1);  // lane 31 gets itself: its Ex is never used
+    }
+    int ex[RY + 1], ez[RY + 1], ey[RY];
+#pragma unroll
+    for (int r = 0; r <= RY; ++r) {
+      ex[r] = edge_of<T, P>(nO[r], nX[r]);   // plane n
+      ez[r] = edge_of<T, P>(cur[r], nO[r]);  // plane n-1 -> n (0 at n = 0: cur == nO)
+    }
+#pragma unroll
+    for (int r = 0; r < RY; ++r) ey[r] = edge_of<T, P>(nO[r], nO[r + 1]);
+    int pk = 0;  // (Ey+1) | (Ez+1)<<2 of every row, 4 bits per row, for the lane on the left
+#pragma unroll
+    for (int r = 0; r < RY; ++r) pk |= ((ey[r] + 1) | ((ez[r] + 1) << 2)) << (4 * r);
+    const int nb = __shfl_down_sync(0xffffffffu, pk, 1);
+    const int z = t.z0 + n - 1;
     const int bk = (b.lo[2] + z) >> 5;
-    if (bk != cur_bk) {
+    if (n > 0 && bk != cur_bk) {
       flush(cur_bk);
       cur_bk = bk;
     }
-    const bool hit = act && tag != 0;
-    cnt0 += __popc(__ballot_sync(0xffffffffu, hit && bi == bi0));
-    cnt1 += __popc(__ballot_sync(0xffffffffu, hit && bi != bi0));
-    c00 = n00;
-    c10 = n10;
-    c01 = n01;
-    c11 = n11;
-    off += plane;
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+      const int eyx = ((nb >> (4 * r)) & 3) - 1, ezx = ((nb >> (4 * r + 2)) & 3) - 1;  // Ey(P+x), Ez(P+x)
+      const int wxyn = ex[r] + eyx - ex[r + 1] - ey[r];
+      if (n > 0) {
+        const int wyz = eyc[r] + ez[r + 1] - ey[r] - ez[r];
+        const int wzx = ez[r] + ex[r] - ezx - exc[r];
+        const uint8_t tag = (uint8_t)((wxyc[r] != 0 ? 1 : 0) | (wyz != 0 ? 2 : 0) | (wzx != 0 ? 4 : 0));
+        const int y = y0 + r;
+        const bool act = actx && y < b.n[1];
+        if (a.tags && act) a.tags[b.tag_base + ((long long)z * b.n[1] + y) * b.n[0] + x] = tag;
+        const int hit = (act && tag != 0) ? 1 : 0;
+        if (((b.lo[1] + y) >> 5) == bj0) cntA += hit; else cntB += hit;
+      }
+      wxyc[r] = wxyn;
+      exc[r] = ex[r];
+      eyc[r] = ey[r];
+    }
+#pragma unroll
+    for (int r = 0; r <= RY; ++r) cur[r] = nO[r];
   }
   flush(cur_bk);
 }

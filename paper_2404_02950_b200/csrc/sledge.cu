@@ -605,7 +605,7 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   a.nb1 = L.nb[1];
   {
     Timed t(c, KIND_TAG);
-    k_tag_strings<T><<<(int)L.tag_tiles.size(), TAG_TX * TAG_TY, 0, c->stream>>>(a);
+    k_tag_strings<T><<<(int)L.tag_tiles.size(), TAG_THREADS, 0, c->stream>>>(a);
   }
   return check_launch(c, "k_tag_strings");
 }
