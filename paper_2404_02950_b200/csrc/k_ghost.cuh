@@ -47,42 +47,76 @@ __device__ __forceinline__ long long cell_offset(const BoxDev& b, int g, int ox,
   return b.base + ((long long)(k + g) * b.sy + (j + g)) * b.sx + (i + ox);
 }
 
+// periodic wrap of an index known to lie in [-n, 2n): ghost cells and their coarse parents are less than one
+// ghost width (< blocking factor <= n) outside the domain
+__device__ __forceinline__ int wrap1(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
+
 __device__ __forceinline__ int owner_lookup(const int* owner, const LevelGeom& gm, int wi, int wj, int wk) {
   return owner[((long long)(wk >> gm.bf_shift) * gm.no[1] + (wj >> gm.bf_shift)) * gm.no[0] + (wi >> gm.bf_shift)];
 }
 
+// Offsets of the 8 coarse cells (dz, dy, dx in {0: c0, 1: c1}) inside the coarse level's planes; false if one
+// of them is not a valid coarse cell.  Fast path: when c0 and c1 have the same owner box all 8 corners lie in
+// it (a box is convex), so one owner pair and one box descriptor serve all of them.
+__device__ __forceinline__ bool coarse_offsets(const BoxDev* cboxes, const int* cowner, const LevelGeom& cg,
+                                               const int c0[3], const int c1[3], long long o[8]) {
+  int w0[3], w1[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    w0[d] = wrap1(c0[d], cg.n[d]);
+    w1[d] = wrap1(c1[d], cg.n[d]);
+  }
+  const int ow0 = owner_lookup(cowner, cg, w0[0], w0[1], w0[2]);
+  const int ow1 = owner_lookup(cowner, cg, w1[0], w1[1], w1[2]);
+  if (ow0 >= 0 && ow0 == ow1) {
+    const BoxDev cb = cboxes[ow0];
+    const long long ox0 = w0[0] - cb.lo[0] + cg.ox, ox1 = w1[0] - cb.lo[0] + cg.ox;
+    const long long oy0 = (long long)(w0[1] - cb.lo[1] + cg.g) * cb.sx, oy1 = (long long)(w1[1] - cb.lo[1] + cg.g) * cb.sx;
+    const long long pl = (long long)cb.sx * cb.sy;
+    const long long oz0 = cb.base + (w0[2] - cb.lo[2] + cg.g) * pl, oz1 = cb.base + (w1[2] - cb.lo[2] + cg.g) * pl;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) o[q] = ((q & 4) ? oz1 : oz0) + ((q & 2) ? oy1 : oy0) + ((q & 1) ? ox1 : ox0);
+    return true;
+  }
+  bool ok = true;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const int ci = (q & 1) ? w1[0] : w0[0], cj = (q & 2) ? w1[1] : w0[1], ck = (q & 4) ? w1[2] : w0[2];
+    const int ow = owner_lookup(cowner, cg, ci, cj, ck);
+    o[q] = 0;
+    if (ow < 0) {
+      ok = false;
+      continue;
+    }
+    const BoxDev cb = cboxes[ow];
+    o[q] = cell_offset(cb, cg.g, cg.ox, ci - cb.lo[0], cj - cb.lo[1], ck - cb.lo[2]);
+  }
+  return ok;
+}
+
+// trilinear x linear-in-time combination (L70-72); q = dz*4 + dy*2 + dx, summed dx fastest from 0
 template <typename T>
-__device__ __forceinline__ typename PairOf<T>::type interp_coarse(
-    const typename PairOf<T>::type* c_old, const typename PairOf<T>::type* c_new, const BoxDev* cboxes,
-    const int* cowner, const LevelGeom& cg, T alpha, const int c0[3], const int c1[3], bool& ok) {
+__device__ __forceinline__ typename PairOf<T>::type interp_coarse(const typename PairOf<T>::type* c_old,
+                                                                  const typename PairOf<T>::type* c_new, T alpha,
+                                                                  const long long o[8]) {
   using P = typename PairOf<T>::type;
   const T w[2] = {T(0.75), T(0.25)};
   const T oma = T(1) - alpha;
   T s0 = T(0), s1 = T(0);
+  P vo[8], vn[8];
 #pragma unroll
-  for (int dz = 0; dz < 2; ++dz)
+  for (int q = 0; q < 8; ++q) {
+    vo[q] = c_old[o[q]];
+    vn[q] = c_new[o[q]];
+  }
 #pragma unroll
-    for (int dy = 0; dy < 2; ++dy)
-#pragma unroll
-      for (int dx = 0; dx < 2; ++dx) {
-        const int ci = wrap_idx(dx ? c1[0] : c0[0], cg.n[0]);
-        const int cj = wrap_idx(dy ? c1[1] : c0[1], cg.n[1]);
-        const int ck = wrap_idx(dz ? c1[2] : c0[2], cg.n[2]);
-        const int ow = owner_lookup(cowner, cg, ci, cj, ck);
-        if (ow < 0) {
-          ok = false;
-          continue;
-        }
-        const BoxDev cb = cboxes[ow];
-        const long long o = cell_offset(cb, cg.g, cg.ox, ci - cb.lo[0], cj - cb.lo[1], ck - cb.lo[2]);
-        const P vo = c_old[o];
-        const P vn = c_new[o];
-        const T cv0 = oma * vo.x + alpha * vn.x;
-        const T cv1 = oma * vo.y + alpha * vn.y;
-        const T wt = (w[dz] * w[dy]) * w[dx];
-        s0 += wt * cv0;
-        s1 += wt * cv1;
-      }
+  for (int q = 0; q < 8; ++q) {
+    const T cv0 = oma * vo[q].x + alpha * vn[q].x;
+    const T cv1 = oma * vo[q].y + alpha * vn[q].y;
+    const T wt = (w[(q >> 2) & 1] * w[(q >> 1) & 1]) * w[q & 1];
+    s0 += wt * cv0;
+    s1 += wt * cv1;
+  }
   return mkpair(s0, s1);
 }
 
@@ -100,37 +134,34 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
   const int g = a.geom.g;
   const int nx = b.n[0], ny = b.n[1], nz = b.n[2];
   const int Gx = nx + 2 * g, Gy = ny + 2 * g;
-  const long long nA = (long long)Gx * Gy * (2 * g);  // z slabs
-  const long long nB = (long long)Gx * (2 * g) * nz;  // y slabs
-  const long long nC = (long long)(2 * g) * ny * nz;  // x slabs
-  const long long q = (long long)(blk - a.blk_prefix[lo_b]) * GHOST_THREADS + threadIdx.x;
+  // 32-bit arithmetic throughout: a box's ghost shell has far fewer than 2^31 cells (checked at create)
+  const unsigned uGx = (unsigned)Gx, uGxy = (unsigned)(Gx * Gy), g2 = (unsigned)(2 * g);
+  const unsigned nA = uGxy * g2;                 // z slabs
+  const unsigned nB = uGx * g2 * (unsigned)nz;   // y slabs
+  const unsigned nC = g2 * (unsigned)ny * (unsigned)nz;  // x slabs
+  const unsigned q = (unsigned)(blk - a.blk_prefix[lo_b]) * GHOST_THREADS + threadIdx.x;
   if (q >= nA + nB + nC) return;
   int i, j, k;
   if (q < nA) {
-    const int zz = (int)(q / ((long long)Gx * Gy));
-    const int r = (int)(q - (long long)zz * Gx * Gy);
-    j = r / Gx - g;
-    i = r % Gx - g;
-    k = zz < g ? zz - g : nz + (zz - g);
+    const unsigned zz = q / uGxy, r = q - zz * uGxy, jj = r / uGx;
+    j = (int)jj - g;
+    i = (int)(r - jj * uGx) - g;
+    k = (int)zz < g ? (int)zz - g : nz + ((int)zz - g);
   } else if (q < nA + nB) {
-    const long long p = q - nA;
-    const int rowlen = Gx * 2 * g;
-    k = (int)(p / rowlen);
-    const int r = (int)(p - (long long)k * rowlen);
-    const int yy = r / Gx;
-    i = r % Gx - g;
-    j = yy < g ? yy - g : ny + (yy - g);
+    const unsigned p = q - nA, rowlen = uGx * g2;
+    const unsigned kk = p / rowlen, r = p - kk * rowlen, yy = r / uGx;
+    k = (int)kk;
+    i = (int)(r - yy * uGx) - g;
+    j = (int)yy < g ? (int)yy - g : ny + ((int)yy - g);
   } else {
-    const long long p = q - nA - nB;
-    const int rowlen = 2 * g * ny;
-    k = (int)(p / rowlen);
-    const int r = (int)(p - (long long)k * rowlen);
-    j = r / (2 * g);
-    const int xx = r % (2 * g);
-    i = xx < g ? xx - g : nx + (xx - g);
+    const unsigned p = q - nA - nB, rowlen = g2 * (unsigned)ny;
+    const unsigned kk = p / rowlen, r = p - kk * rowlen, jj = r / g2, xx = r - jj * g2;
+    k = (int)kk;
+    j = (int)jj;
+    i = (int)xx < g ? (int)xx - g : nx + ((int)xx - g);
   }
   const int f0 = b.lo[0] + i, f1 = b.lo[1] + j, f2 = b.lo[2] + k;  // unwrapped level index
-  const int wi = wrap_idx(f0, a.geom.n[0]), wj = wrap_idx(f1, a.geom.n[1]), wk = wrap_idx(f2, a.geom.n[2]);
+  const int wi = wrap1(f0, a.geom.n[0]), wj = wrap1(f1, a.geom.n[1]), wk = wrap1(f2, a.geom.n[2]);
   const long long dst = cell_offset(b, g, a.geom.ox, i, j, k);
   const int ow = owner_lookup(a.owner, a.geom, wi, wj, wk);
   if (ow >= 0) {
@@ -152,10 +183,12 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
     const int r = f[d] - 2 * c0[d];
     c1[d] = r == 0 ? c0[d] - 1 : c0[d] + 1;
   }
-  bool ok = true;
-  a.psi[dst] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.cboxes, a.cowner, a.cgeom, a.alpha, c0, c1, ok);
-  if (FILL_PI)
-    a.pi[dst] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.cboxes, a.cowner, a.cgeom, a.alpha, c0, c1, ok);
+  long long o[8];
+  const bool ok = coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o);
+  if (ok) {
+    a.psi[dst] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
+    if (FILL_PI) a.pi[dst] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
+  }
   if (!ok) *a.err_flag = 1;
 }
 
