@@ -10,15 +10,29 @@
 //     coarse owner table (their existence is what proper nesting guarantees, L70).
 // Only valid cells are read and only ghost cells are written, so one launch per level has no hazards.
 //
-// Work distribution: the ghost shell of a box is cut into three slab pairs (z-low/high: full ghosted
-// xy-planes; y-low/high: full ghosted x-rows; x-low/high), enumerated x-fastest so that the wide slabs are
-// written with coalesced rows.  A prefix table over boxes (in CTAs) maps blockIdx.x -> box by bisection.
+// The box list is static (regridding is outside the library), so WHERE every ghost cell takes its data from
+// never changes: k_plan_ghosts resolves it once at create time -- enumeration of the ghost shell, periodic
+// wrap, owner lookup, coarse parents -- into one 16-byte GhostEntry per ghost cell, and k_fill_ghosts, which
+// runs before every RK stage, only streams that list: one thread per entry, load the entry, move the data.
+//   copy   {dst, src}                                  same-level / periodic copy
+//   interp {dst, o0, sx | sy << 16, signs}             all 8 coarse parents in ONE coarse box: offset of the
+//                                                      (c0,c0,c0) corner, the box's pitches, and per axis
+//                                                      whether c1 = c0 + 1 or c0 - 1
+//   slow   {dst, (f0+g) | (f1+g) << 16, f2+g}          parents spread over several coarse boxes: the fine index
+//                                                      is kept and the parents are looked up on the fly
+// Enumeration: the ghost shell of a box is cut into three slab pairs (z-low/high: full ghosted xy-planes;
+// y-low/high: full ghosted x-rows; x-low/high), x fastest, so that the wide slabs are written with coalesced
+// rows.  A prefix table over boxes (in CTAs) maps the plan kernel's blockIdx.x -> box by bisection.
 #pragma once
 #include "layout.h"
 
 namespace sledge {
 
 constexpr int GHOST_THREADS = 256;
+
+enum GhostKind { GHOST_COPY = 0, GHOST_INTERP = 1, GHOST_SLOW = 2, GHOST_NONE = 3 };
+// x = dst, y / z = see above, w = kind | signs << 2 (bit d of signs: c1 = c0 + 1 along axis d)
+typedef uint4 GhostEntry;
 
 template <typename T>
 struct GhostArgs {
@@ -41,6 +55,8 @@ struct GhostArgs {
   T alpha;
   int has_coarse;
   int* err_flag;  // set to 1 if a ghost cell has neither a same-level owner nor coarse data
+  GhostEntry* list;  // GHOST_THREADS entries per CTA of the enumeration (written by the plan, read by the fill)
+  unsigned n_entries;
 };
 
 __device__ __forceinline__ long long cell_offset(const BoxDev& b, int g, int ox, int i, int j, int k) {
@@ -120,9 +136,17 @@ __device__ __forceinline__ typename PairOf<T>::type interp_coarse(const typename
   return mkpair(s0, s1);
 }
 
-template <typename T, bool FILL_PI>
-__global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T> a) {
-  using P = typename PairOf<T>::type;
+// parents of fine index f along one axis: f = 2 c0 + r sits -1/4 (r = 0) or +1/4 (r = 1) of a coarse cell from
+// the centre of c0; the second parent is c0 - 1 (r = 0) or c0 + 1 (r = 1)
+__device__ __forceinline__ void parents_of(int f, int& c0, int& c1) {
+  c0 = floordiv2(f);
+  c1 = (f - 2 * c0) == 0 ? c0 - 1 : c0 + 1;
+}
+
+// Create-time pass: one thread per slot of the enumeration, writes a.list[blockIdx.x * GHOST_THREADS + tid].
+template <typename T>
+__global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T> a) {
+  GhostEntry* const out = a.list + (size_t)blockIdx.x * GHOST_THREADS + threadIdx.x;
   // blockIdx.x -> box
   int lo_b = 0, hi_b = a.nbox;
   const int blk = blockIdx.x;
@@ -140,7 +164,10 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
   const unsigned nB = uGx * g2 * (unsigned)nz;   // y slabs
   const unsigned nC = g2 * (unsigned)ny * (unsigned)nz;  // x slabs
   const unsigned q = (unsigned)(blk - a.blk_prefix[lo_b]) * GHOST_THREADS + threadIdx.x;
-  if (q >= nA + nB + nC) return;
+  if (q >= nA + nB + nC) {
+    *out = make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
+    return;
+  }
   int i, j, k;
   if (q < nA) {
     const unsigned zz = q / uGxy, r = q - zz * uGxy, jj = r / uGx;
@@ -162,34 +189,73 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
   }
   const int f0 = b.lo[0] + i, f1 = b.lo[1] + j, f2 = b.lo[2] + k;  // unwrapped level index
   const int wi = wrap1(f0, a.geom.n[0]), wj = wrap1(f1, a.geom.n[1]), wk = wrap1(f2, a.geom.n[2]);
-  const long long dst = cell_offset(b, g, a.geom.ox, i, j, k);
+  const unsigned dst = (unsigned)cell_offset(b, g, a.geom.ox, i, j, k);
   const int ow = owner_lookup(a.owner, a.geom, wi, wj, wk);
-  if (ow >= 0) {
+  if (ow >= 0) {  // same-level copy wins (R9)
     const BoxDev sb = a.boxes[ow];
     const long long src = cell_offset(sb, g, a.geom.ox, wi - sb.lo[0], wj - sb.lo[1], wk - sb.lo[2]);
-    a.psi[dst] = a.psi[src];
-    if (FILL_PI) a.pi[dst] = a.pi[src];
+    *out = make_uint4(dst, (unsigned)src, 0u, (unsigned)GHOST_COPY);
     return;
   }
   if (!a.has_coarse) {
     *a.err_flag = 1;
+    *out = make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
     return;
   }
-  int c0[3], c1[3];
   const int f[3] = {f0, f1, f2};
+  int c0[3], c1[3], w0[3], w1[3];
+  bool unit = true;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    c0[d] = floordiv2(f[d]);
-    const int r = f[d] - 2 * c0[d];
-    c1[d] = r == 0 ? c0[d] - 1 : c0[d] + 1;
+    parents_of(f[d], c0[d], c1[d]);
+    w0[d] = wrap1(c0[d], a.cgeom.n[d]);
+    w1[d] = wrap1(c1[d], a.cgeom.n[d]);
+    unit = unit && (w1[d] - w0[d] == c1[d] - c0[d]);  // no periodic seam between the two parents
   }
+  const int ow0 = owner_lookup(a.cowner, a.cgeom, w0[0], w0[1], w0[2]);
+  const int ow1 = owner_lookup(a.cowner, a.cgeom, w1[0], w1[1], w1[2]);
+  if (unit && ow0 >= 0 && ow0 == ow1) {
+    const BoxDev cb = a.cboxes[ow0];
+    const long long o0 = cell_offset(cb, a.cgeom.g, a.cgeom.ox, w0[0] - cb.lo[0], w0[1] - cb.lo[1], w0[2] - cb.lo[2]);
+    const unsigned signs = (c1[0] > c0[0] ? 1u : 0u) | (c1[1] > c0[1] ? 2u : 0u) | (c1[2] > c0[2] ? 4u : 0u);
+    *out = make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (signs << 2));
+    return;
+  }
+  // parents in several coarse boxes (or across the periodic seam of a single one): resolved at fill time
   long long o[8];
-  const bool ok = coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o);
-  if (ok) {
-    a.psi[dst] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
-    if (FILL_PI) a.pi[dst] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
+  if (!coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o)) *a.err_flag = 1;
+  *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW);
+}
+
+// The fill itself: one thread per entry of the level's list.
+template <typename T, bool FILL_PI>
+__global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T> a) {
+  const unsigned e = blockIdx.x * GHOST_THREADS + threadIdx.x;
+  if (e >= a.n_entries) return;
+  const uint4 en = __ldg(reinterpret_cast<const uint4*>(a.list) + e);
+  const unsigned kind = en.w & 3u;
+  if (kind == GHOST_COPY) {
+    a.psi[en.x] = a.psi[en.y];
+    if (FILL_PI) a.pi[en.x] = a.pi[en.y];
+    return;
   }
-  if (!ok) *a.err_flag = 1;
+  if (kind == GHOST_NONE) return;
+  long long o[8];
+  if (kind == GHOST_INTERP) {
+    const long long sx = en.z & 0xffffu, pl = sx * (long long)(en.z >> 16);
+    const long long dx = (en.w & 4u) ? 1 : -1, dy = (en.w & 8u) ? sx : -sx, dz = (en.w & 16u) ? pl : -pl;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) o[q] = (long long)en.y + ((q & 1) ? dx : 0) + ((q & 2) ? dy : 0) + ((q & 4) ? dz : 0);
+  } else {
+    const int g = a.geom.g;
+    const int f[3] = {(int)(en.y & 0xffffu) - g, (int)(en.y >> 16) - g, (int)en.z - g};
+    int c0[3], c1[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) parents_of(f[d], c0[d], c1[d]);
+    if (!coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o)) return;  // reported by the plan
+  }
+  a.psi[en.x] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
+  if (FILL_PI) a.pi[en.x] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
 }
 
 }  // namespace sledge

@@ -78,7 +78,7 @@ struct LevelHost {
   int nb[3];
   // arena offsets (bytes)
   size_t off_buf[NBUF][2];
-  size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix;
+  size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix, off_ghost_list;
   // run state
   int cur = 0, old = 0;
   bool have_pair = false;
@@ -269,6 +269,13 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.off_owner = take(L.owner.size() * sizeof(int));
     L.off_ghost_prefix = take(L.ghost_prefix.size() * sizeof(int));
     L.off_avg_prefix = take(L.avg_prefix.size() * sizeof(int));
+    L.off_ghost_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
+    // the ghost list (k_ghost.cuh) keeps cell offsets in 32 bits and pitches / indices in 16
+    if (L.plane_cells >= (1LL << 32)) return fail(nullptr, SLEDGE_EINVAL, "level %d: more than 2^32 stored cells", l);
+    for (const BoxDev& b : L.boxdev)
+      if (b.sx >= 65536 || b.sy >= 65536) return fail(nullptr, SLEDGE_EINVAL, "level %d: box pitch >= 65536 cells", l);
+    for (int d = 0; d < 3; ++d)
+      if (L.n[d] + 2 * g >= 65536) return fail(nullptr, SLEDGE_EINVAL, "level %d: more than 65535 cells per axis", l);
   }
   P.scratch_bytes = max_box_cells * P.esz;
   P.off_scratch = take(P.scratch_bytes);
@@ -330,9 +337,9 @@ LevelGeom geom_of(const Plan& P, int l) {
   return gm;
 }
 
-// K2 on buffer `buf` of level l, whose data is at time `time`
+// K2 arguments for buffer `buf` of level l, whose data is at time `time`
 template <typename T>
-int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
+GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
   GhostArgs<T> a;
@@ -345,6 +352,8 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
   a.owner = tab<int>(c, L.off_owner);
   a.geom = geom_of(P, l);
   a.err_flag = tab<int>(c, P.off_err);
+  a.list = tab<GhostEntry>(c, L.off_ghost_list);
+  a.n_entries = (unsigned)L.ghost_prefix.back() * GHOST_THREADS;
   a.has_coarse = l > 0;
   a.alpha = T(0);
   if (l > 0) {
@@ -364,7 +373,14 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
     a.c_old_pi = plane_ptr<T>(c, l - 1, bo, 1);
     a.c_new_pi = plane_ptr<T>(c, l - 1, bn, 1);
   }
-  const int grid = L.ghost_prefix.back();
+  return a;
+}
+
+// K2 on buffer `buf` of level l: streams the level's ghost list (built once by plan_ghosts)
+template <typename T>
+int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
+  const GhostArgs<T> a = ghost_args<T>(c, l, buf, time);
+  const int grid = c->plan.lev[l].ghost_prefix.back();
   if (grid == 0) return SLEDGE_OK;
   {
     Timed t(c, KIND_GHOST);
@@ -372,6 +388,16 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
     else k_fill_ghosts<T, false><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
   }
   return check_launch(c, "k_fill_ghosts");
+}
+
+// create-time: resolve every ghost cell of level l into its list entry
+template <typename T>
+int plan_ghosts(sledge_ctx* c, int l) {
+  const GhostArgs<T> a = ghost_args<T>(c, l, 0, 0.0);
+  const int grid = c->plan.lev[l].ghost_prefix.back();
+  if (grid == 0) return SLEDGE_OK;
+  k_plan_ghosts<T><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+  return check_launch(c, "k_plan_ghosts");
 }
 
 template <typename T, int ORDER, int MODE>
@@ -680,6 +706,19 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     up(L.off_owner, L.owner.data(), L.owner.size() * sizeof(int));
     up(L.off_ghost_prefix, L.ghost_prefix.data(), L.ghost_prefix.size() * sizeof(int));
     up(L.off_avg_prefix, L.avg_prefix.data(), L.avg_prefix.size() * sizeof(int));
+  }
+  // ghost lists: resolved on the device from the tables just uploaded (the plan kernel of level l reads the
+  // tables of l and l-1 only); its launches do not count as hot-path launches
+  if (e == cudaSuccess) {
+    const int64_t before = c->launches;
+    for (int l = 0; l < P.p.n_levels && rc == SLEDGE_OK; ++l)
+      rc = DISPATCH(c, plan_ghosts<float>(c, l), plan_ghosts<double>(c, l));
+    c->launches = before;
+    if (rc != SLEDGE_OK) {
+      g_err = c->err;
+      delete c;
+      return rc;
+    }
   }
   // the tables above are pageable host memory: make sure the copies are done before they can go away
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
