@@ -119,6 +119,99 @@ __device__ __forceinline__ T pot_of(T lam_eta2, T a_mass, T p1, T p2) {
   return fma(lam_eta2, fma(p1, p1, fma(p2, p2, T(-1))), a_mass);
 }
 
+// One cell of one sweep: from the Laplacians lap[f][c] of the differenced fields, their centre values wc[f] and
+// the pointwise inputs pc[q], the new state(s) opsi[q], opi[q] of the mode's data-flow (see the header).
+template <typename T, int MODE>
+__device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[ModeInfo<MODE>::NF][2],
+                                        const typename PairOf<T>::type (&wc)[ModeInfo<MODE>::NF],
+                                        const typename PairOf<T>::type (&pc)[ModeInfo<MODE>::NP > 0 ? ModeInfo<MODE>::NP : 1],
+                                        typename PairOf<T>::type (&opsi)[ModeInfo<MODE>::NOUT],
+                                        typename PairOf<T>::type (&opi)[ModeInfo<MODE>::NOUT]) {
+  using P = typename PairOf<T>::type;
+  constexpr int NP = ModeInfo<MODE>::NP, NOUT = ModeInfo<MODE>::NOUT;
+  constexpr int NPA = NP > 0 ? NP : 1;
+  if (MODE == FUSED_A) {
+    // stages 1 + 2 (O4): U3 = Y + dt/2 k(U2), U2 = Y + dt/2 k(Y); U2 is never stored
+    const T hdt = T(0.5) * a.adt;
+    const T y1 = wc[0].x, y2 = wc[0].y, q1 = wc[1].x, q2 = wc[1].y;
+    const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
+    const T k1a = kpi_of(lap[0][0], y1, pot1, a.fric[0], q1);
+    const T k1b = kpi_of(lap[0][1], y2, pot1, a.fric[0], q2);
+    const T p2a = fma(hdt, k1a, q1), p2b = fma(hdt, k1b, q2);  // Pi(U2)
+    const T u2a = fma(hdt, q1, y1), u2b = fma(hdt, q2, y2);    // psi(U2)
+    const T l2a = fma(hdt, lap[1][0], lap[0][0]), l2b = fma(hdt, lap[1][1], lap[0][1]);
+    const T pot2 = pot_of(a.lam_eta2[1], a.a_mass, u2a, u2b);
+    const T k2a = kpi_of(l2a, u2a, pot2, a.fric[1], p2a);
+    const T k2b = kpi_of(l2b, u2b, pot2, a.fric[1], p2b);
+    opsi[0] = mkpair(fma(hdt, p2a, y1), fma(hdt, p2b, y2));
+    opi[0] = mkpair(fma(hdt, k2a, q1), fma(hdt, k2b, q2));
+  } else if (MODE == FUSED_B) {
+    // stages 3 + 4 and the final combination; k1 recomputed from Y (same expression, same bits as in
+    // PASS A), dt/2 k2 = Pi3 - Pi_Y
+    const T dt = a.adt, hdt = T(0.5) * a.adt, sixth = a.adt / T(6);
+    const T u3a = wc[0].x, u3b = wc[0].y, p3a = wc[1].x, p3b = wc[1].y;
+    const T y1 = wc[2].x, y2 = wc[2].y, q1 = pc[0].x, q2 = pc[0].y;
+    const T pot3 = pot_of(a.lam_eta2[1], a.a_mass, u3a, u3b);
+    const T k3a = kpi_of(lap[0][0], u3a, pot3, a.fric[1], p3a);
+    const T k3b = kpi_of(lap[0][1], u3b, pot3, a.fric[1], p3b);
+    const T u4a = fma(dt, p3a, y1), u4b = fma(dt, p3b, y2);  // psi(U4)
+    const T p4a = fma(dt, k3a, q1), p4b = fma(dt, k3b, q2);  // Pi(U4)
+    const T l4a = fma(dt, lap[1][0], lap[2][0]), l4b = fma(dt, lap[1][1], lap[2][1]);
+    const T pot4 = pot_of(a.lam_eta2[2], a.a_mass, u4a, u4b);
+    const T k4a = kpi_of(l4a, u4a, pot4, a.fric[2], p4a);
+    const T k4b = kpi_of(l4b, u4b, pot4, a.fric[2], p4b);
+    const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
+    const T k1a = kpi_of(lap[2][0], y1, pot1, a.fric[0], q1);
+    const T k1b = kpi_of(lap[2][1], y2, pot1, a.fric[0], q2);
+    const T p2a = fma(hdt, k1a, q1), p2b = fma(hdt, k1b, q2);  // Pi(U2), same bits as in PASS A
+    const T twothirds = T(2) / T(3);
+    opsi[0] = mkpair(fma(sixth, (q1 + p4a) + T(2) * (p2a + p3a), y1),
+                           fma(sixth, (q2 + p4b) + T(2) * (p2b + p3b), y2));
+    opi[0] = mkpair(fma(sixth, fma(T(2), k3a, k1a + k4a), fma(twothirds, p3a - q1, q1)),
+                          fma(sixth, fma(T(2), k3b, k1b + k4b), fma(twothirds, p3b - q2, q2)));
+  } else {
+    const T psi1 = wc[0].x, psi2 = wc[0].y;
+    const T pi1 = pc[0].x, pi2 = pc[0].y;
+    const T pot = pot_of(a.lam_eta2[0], a.a_mass, psi1, psi2);
+    const T kpsi1 = pi1, kpsi2 = pi2;
+    const T kpi1 = kpi_of(lap[0][0], psi1, pot, a.fric[0], pi1);
+    const T kpi2 = kpi_of(lap[0][1], psi2, pot, a.fric[0], pi2);
+    // pointwise inputs: in_psi(q) = pv[1 + 2q], in_pi(q) = pv[2 + 2q]
+    auto ipsi = [&](int q) -> const P& { return pc[(1 + 2 * q) < NPA ? (1 + 2 * q) : 0]; };
+    auto ipi = [&](int q) -> const P& { return pc[(2 + 2 * q) < NPA ? (2 + 2 * q) : 0]; };
+    auto axpy = [](T c, T k, T y) -> T { return fma(c, k, y); };
+    if (MODE == LEAN_S1) {  // U2 = U + adt k   (U = Y)
+      opsi[0] = mkpair(axpy(a.adt, kpsi1, psi1), axpy(a.adt, kpsi2, psi2));
+      opi[0] = mkpair(axpy(a.adt, kpi1, pi1), axpy(a.adt, kpi2, pi2));
+    } else if (MODE == LEAN_S23) {  // U' = Y + adt k   (in0 = Y)
+      opsi[0] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
+      opi[0] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
+    } else if (MODE == LEAN_S4) {  // in0 = Y, in1 = U2, in2 = U3, U = U4, adt = dt/6
+      const T third = T(1) / T(3);
+      auto comb = [&](T yv, T u2, T u3, T u4, T kk) -> T {
+        return fma(a.adt, kk, ((fma(T(2), u3, u2) + u4) - yv) * third);
+      };
+      opsi[0] = mkpair(comb(ipsi(0).x, ipsi(1).x, ipsi(2).x, psi1, kpsi1),
+                             comb(ipsi(0).y, ipsi(1).y, ipsi(2).y, psi2, kpsi2));
+      opi[0] = mkpair(comb(ipi(0).x, ipi(1).x, ipi(2).x, pi1, kpi1),
+                            comb(ipi(0).y, ipi(1).y, ipi(2).y, pi2, kpi2));
+    } else if (MODE == CLASSIC_S1) {  // out0 = U + adt k ; out1 (ACC) = U + bdt k
+      opsi[0] = mkpair(axpy(a.adt, kpsi1, psi1), axpy(a.adt, kpsi2, psi2));
+      opi[0] = mkpair(axpy(a.adt, kpi1, pi1), axpy(a.adt, kpi2, pi2));
+      opsi[NOUT - 1] = mkpair(axpy(a.bdt, kpsi1, psi1), axpy(a.bdt, kpsi2, psi2));
+      opi[NOUT - 1] = mkpair(axpy(a.bdt, kpi1, pi1), axpy(a.bdt, kpi2, pi2));
+    } else if (MODE == CLASSIC_S23) {  // in0 = Y, in1 = ACC ; out0 = Y + adt k ; out1 = ACC + bdt k
+      opsi[0] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
+      opi[0] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
+      opsi[NOUT - 1] = mkpair(axpy(a.bdt, kpsi1, ipsi(1).x), axpy(a.bdt, kpsi2, ipsi(1).y));
+      opi[NOUT - 1] = mkpair(axpy(a.bdt, kpi1, ipi(1).x), axpy(a.bdt, kpi2, ipi(1).y));
+    } else {  // CLASSIC_S4: in0 = ACC ; out0 = ACC + adt k
+      opsi[0] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
+      opi[0] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
+    }
+  }
+}
+
 template <typename T, int ORDER, int MODE, int TX, int TY, int D>
 struct PipeCfg {
   static constexpr int R = ORDER;
@@ -297,85 +390,16 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
             lap[f][c] = lap_from<T, ORDER>(comp(w[f][R].p[p]), xm, xp, ym, yp, zm, zp, a.inv_h2);
           }
         }
-        if (MODE == FUSED_A) {
-          // stages 1 + 2 (O4): U3 = Y + dt/2 k(U2), U2 = Y + dt/2 k(Y); U2 is never stored
-          const T hdt = T(0.5) * a.adt;
-          const T y1 = w[0][R].p[p].x, y2 = w[0][R].p[p].y, q1 = w[1][R].p[p].x, q2 = w[1][R].p[p].y;
-          const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
-          const T k1a = kpi_of(lap[0][0], y1, pot1, a.fric[0], q1);
-          const T k1b = kpi_of(lap[0][1], y2, pot1, a.fric[0], q2);
-          const T p2a = fma(hdt, k1a, q1), p2b = fma(hdt, k1b, q2);  // Pi(U2)
-          const T u2a = fma(hdt, q1, y1), u2b = fma(hdt, q2, y2);    // psi(U2)
-          const T l2a = fma(hdt, lap[1][0], lap[0][0]), l2b = fma(hdt, lap[1][1], lap[0][1]);
-          const T pot2 = pot_of(a.lam_eta2[1], a.a_mass, u2a, u2b);
-          const T k2a = kpi_of(l2a, u2a, pot2, a.fric[1], p2a);
-          const T k2b = kpi_of(l2b, u2b, pot2, a.fric[1], p2b);
-          o_psi[0].p[p] = mkpair(fma(hdt, p2a, y1), fma(hdt, p2b, y2));
-          o_pi[0].p[p] = mkpair(fma(hdt, k2a, q1), fma(hdt, k2b, q2));
-        } else if (MODE == FUSED_B) {
-          // stages 3 + 4 and the final combination; k1 recomputed from Y (same expression, same bits as in
-          // PASS A), dt/2 k2 = Pi3 - Pi_Y
-          const T dt = a.adt, hdt = T(0.5) * a.adt, sixth = a.adt / T(6);
-          const T u3a = w[0][R].p[p].x, u3b = w[0][R].p[p].y, p3a = w[1][R].p[p].x, p3b = w[1][R].p[p].y;
-          const T y1 = w[2][R].p[p].x, y2 = w[2][R].p[p].y, q1 = pv[0].p[p].x, q2 = pv[0].p[p].y;
-          const T pot3 = pot_of(a.lam_eta2[1], a.a_mass, u3a, u3b);
-          const T k3a = kpi_of(lap[0][0], u3a, pot3, a.fric[1], p3a);
-          const T k3b = kpi_of(lap[0][1], u3b, pot3, a.fric[1], p3b);
-          const T u4a = fma(dt, p3a, y1), u4b = fma(dt, p3b, y2);  // psi(U4)
-          const T p4a = fma(dt, k3a, q1), p4b = fma(dt, k3b, q2);  // Pi(U4)
-          const T l4a = fma(dt, lap[1][0], lap[2][0]), l4b = fma(dt, lap[1][1], lap[2][1]);
-          const T pot4 = pot_of(a.lam_eta2[2], a.a_mass, u4a, u4b);
-          const T k4a = kpi_of(l4a, u4a, pot4, a.fric[2], p4a);
-          const T k4b = kpi_of(l4b, u4b, pot4, a.fric[2], p4b);
-          const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
-          const T k1a = kpi_of(lap[2][0], y1, pot1, a.fric[0], q1);
-          const T k1b = kpi_of(lap[2][1], y2, pot1, a.fric[0], q2);
-          const T p2a = fma(hdt, k1a, q1), p2b = fma(hdt, k1b, q2);  // Pi(U2), same bits as in PASS A
-          const T twothirds = T(2) / T(3);
-          o_psi[0].p[p] = mkpair(fma(sixth, (q1 + p4a) + T(2) * (p2a + p3a), y1),
-                                 fma(sixth, (q2 + p4b) + T(2) * (p2b + p3b), y2));
-          o_pi[0].p[p] = mkpair(fma(sixth, fma(T(2), k3a, k1a + k4a), fma(twothirds, p3a - q1, q1)),
-                                fma(sixth, fma(T(2), k3b, k1b + k4b), fma(twothirds, p3b - q2, q2)));
-        } else {
-          const T psi1 = w[0][R].p[p].x, psi2 = w[0][R].p[p].y;
-          const T pi1 = pv[0].p[p].x, pi2 = pv[0].p[p].y;
-          const T pot = pot_of(a.lam_eta2[0], a.a_mass, psi1, psi2);
-          const T kpsi1 = pi1, kpsi2 = pi2;
-          const T kpi1 = kpi_of(lap[0][0], psi1, pot, a.fric[0], pi1);
-          const T kpi2 = kpi_of(lap[0][1], psi2, pot, a.fric[0], pi2);
-          // pointwise inputs: in_psi(q) = pv[1 + 2q], in_pi(q) = pv[2 + 2q]
-          auto ipsi = [&](int q) -> const P& { return pv[(1 + 2 * q) < NPA ? (1 + 2 * q) : 0].p[p]; };
-          auto ipi = [&](int q) -> const P& { return pv[(2 + 2 * q) < NPA ? (2 + 2 * q) : 0].p[p]; };
-          auto axpy = [](T c, T k, T y) -> T { return fma(c, k, y); };
-          if (MODE == LEAN_S1) {  // U2 = U + adt k   (U = Y)
-            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, psi1), axpy(a.adt, kpsi2, psi2));
-            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, pi1), axpy(a.adt, kpi2, pi2));
-          } else if (MODE == LEAN_S23) {  // U' = Y + adt k   (in0 = Y)
-            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
-            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
-          } else if (MODE == LEAN_S4) {  // in0 = Y, in1 = U2, in2 = U3, U = U4, adt = dt/6
-            const T third = T(1) / T(3);
-            auto comb = [&](T yv, T u2, T u3, T u4, T kk) -> T {
-              return fma(a.adt, kk, ((fma(T(2), u3, u2) + u4) - yv) * third);
-            };
-            o_psi[0].p[p] = mkpair(comb(ipsi(0).x, ipsi(1).x, ipsi(2).x, psi1, kpsi1),
-                                   comb(ipsi(0).y, ipsi(1).y, ipsi(2).y, psi2, kpsi2));
-            o_pi[0].p[p] = mkpair(comb(ipi(0).x, ipi(1).x, ipi(2).x, pi1, kpi1),
-                                  comb(ipi(0).y, ipi(1).y, ipi(2).y, pi2, kpi2));
-          } else if (MODE == CLASSIC_S1) {  // out0 = U + adt k ; out1 (ACC) = U + bdt k
-            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, psi1), axpy(a.adt, kpsi2, psi2));
-            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, pi1), axpy(a.adt, kpi2, pi2));
-            o_psi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpsi1, psi1), axpy(a.bdt, kpsi2, psi2));
-            o_pi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpi1, pi1), axpy(a.bdt, kpi2, pi2));
-          } else if (MODE == CLASSIC_S23) {  // in0 = Y, in1 = ACC ; out0 = Y + adt k ; out1 = ACC + bdt k
-            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
-            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
-            o_psi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpsi1, ipsi(1).x), axpy(a.bdt, kpsi2, ipsi(1).y));
-            o_pi[NOUT - 1].p[p] = mkpair(axpy(a.bdt, kpi1, ipi(1).x), axpy(a.bdt, kpi2, ipi(1).y));
-          } else {  // CLASSIC_S4: in0 = ACC ; out0 = ACC + adt k
-            o_psi[0].p[p] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
-            o_pi[0].p[p] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
-          }
+        P wc[NF], pc[NPA], opsi[NOUT], opi[NOUT];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) wc[f] = w[f][R].p[p];
+#pragma unroll
+        for (int q = 0; q < NPA; ++q) pc[q] = pv[q].p[p];
+        rk_cell<T, MODE>(a, lap, wc, pc, opsi, opi);
+#pragma unroll
+        for (int q = 0; q < NOUT; ++q) {
+          o_psi[q].p[p] = opsi[q];
+          o_pi[q].p[p] = opi[q];
         }
       }
       const long long oo = off + (long long)zz * plane;

@@ -18,6 +18,7 @@
 #include "k_avgdown.cuh"
 #include "k_ghost.cuh"
 #include "k_rk_pipe.cuh"
+#include "k_rk_plane.cuh"
 #include "k_tag.cuh"
 
 using namespace sledge;
@@ -49,17 +50,40 @@ constexpr size_t ALIGN = 256;
 #define SLEDGE_K1F_TY 8
 #endif
 #ifndef SLEDGE_K1F_SMEM
-#define SLEDGE_K1F_SMEM (56 * 1024)
+#define SLEDGE_K1F_SMEM (113 * 1024)
 #endif
 constexpr int K1_TX = 32, K1_TY = SLEDGE_K1_TY, K1_NZ = SLEDGE_K1_NZ;
 constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
 constexpr int K1F_TY = SLEDGE_K1F_TY;            // tile rows / budget of the FUSED sweeps
 constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
+// which on-chip data path a sweep uses: 1 = k_rk_plane (ghosted plane ring), 0 = k_rk_pipe (ring + centre plane)
+#ifndef SLEDGE_K1F_PLANE
+#define SLEDGE_K1F_PLANE 1
+#endif
+#ifndef SLEDGE_K1_PLANE
+#define SLEDGE_K1_PLANE 0
+#endif
+#ifndef SLEDGE_K1F_PDMAX
+#define SLEDGE_K1F_PDMAX 2
+#endif
+#ifndef SLEDGE_K1F_RY
+#define SLEDGE_K1F_RY 2
+#endif
+#ifndef SLEDGE_K1F_MINB_A
+#define SLEDGE_K1F_MINB_A 3
+#endif
+#ifndef SLEDGE_K1F_MINB_B
+#define SLEDGE_K1F_MINB_B 2
+#endif
 template <int MODE> struct K1Shape {
   static constexpr bool fused = (MODE == FUSED_A || MODE == FUSED_B);
   static constexpr int TY = fused ? K1F_TY : K1_TY;
   static constexpr size_t SMEM = fused ? K1F_SMEM : K1_SMEM;
+  static constexpr bool plane = fused ? (SLEDGE_K1F_PLANE != 0) : (SLEDGE_K1_PLANE != 0);
+  static constexpr int PDMAX = fused ? SLEDGE_K1F_PDMAX : 3;
+  static constexpr int RY = fused ? SLEDGE_K1F_RY : 1;  // rows per thread (k_rk_plane)
+  static constexpr int MINB = MODE == FUSED_A ? SLEDGE_K1F_MINB_A : (MODE == FUSED_B ? SLEDGE_K1F_MINB_B : 1);
 };
 
 thread_local std::string g_err;
@@ -403,17 +427,31 @@ int plan_ghosts(sledge_ctx* c, int l) {
 template <typename T, int ORDER, int MODE>
 cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   constexpr int TY = K1Shape<MODE>::TY;
-  constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, TY>(K1Shape<MODE>::SMEM, K1_DMAX);
-  static_assert(PipeCfg<T, ORDER, MODE, K1_TX, TY, D>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
-  using C = PipeCfg<T, ORDER, MODE, K1_TX, TY, D>;
-  auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, TY, D>;
   static bool configured = false;  // per instantiation
-  if (!configured) {
-    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    configured = true;
+  if constexpr (K1Shape<MODE>::plane) {
+    constexpr int RY = K1Shape<MODE>::RY;
+    constexpr int PD = plane_depth<T, ORDER, MODE, K1_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
+    using C = PlaneCfg<T, ORDER, MODE, K1_TX, TY, PD, RY>;
+    static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
+    auto kern = k_rk_plane<T, ORDER, MODE, K1_TX, TY, PD, RY, K1Shape<MODE>::MINB>;
+    if (!configured) {
+      const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+      if (e != cudaSuccess) return e;
+      configured = true;
+    }
+    kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(a);
+  } else {
+    constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, TY>(K1Shape<MODE>::SMEM, K1_DMAX);
+    static_assert(PipeCfg<T, ORDER, MODE, K1_TX, TY, D>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
+    using C = PipeCfg<T, ORDER, MODE, K1_TX, TY, D>;
+    auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, TY, D>;
+    if (!configured) {
+      const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+      if (e != cudaSuccess) return e;
+      configured = true;
+    }
+    kern<<<grid, K1_TX * TY, C::SMEM_BYTES, c->stream>>>(a);
   }
-  kern<<<grid, K1_TX * TY, C::SMEM_BYTES, c->stream>>>(a);
   return cudaSuccess;
 }
 template <typename T, int ORDER>
