@@ -16,21 +16,33 @@
 // and only the edges that START at a cell are ever evaluated (3 cross products per cell instead of 12).
 // A warp owns a 31 x TAG_RY patch of cells and marches along z without any block-level synchronisation: lane l
 // holds the column x0+l of TAG_RY+1 rows (the last row and lane 31 are halo: they only supply edges), the
-// plane below stays in registers, loads run one plane ahead, psi(P+x) and the packed edges of P+x come from
+// plane below stays in registers, loads run TAG_PF planes ahead, psi(P+x) and the packed edges of P+x come from
 // lane l+1 by shuffle.  Per plane and thread: Ex, Ez on TAG_RY+1 rows and Ey on TAG_RY rows (3.5 edges per cell
 // for TAG_RY = 4).  Warps step by 31 cells in x so that every lane's +x partner is in the warp.
 // Counts: per-thread counters, reduced over the warp (redux) and flushed with one atomicAdd per 32-block
 // whenever the warp leaves a 32-block in z.
 #pragma once
 #include "layout.h"
+#include "k_rk_pipe.cuh"  // cp.async helpers
 
 namespace sledge {
 
 constexpr int TAG_TX = 31;                 // cells per warp row that produce tags (lane 31 is the +x halo)
-constexpr int TAG_RY = 4;                  // rows per warp
-constexpr int TAG_WARPS = 4;               // warps per CTA, stacked in y
+#ifndef SLEDGE_TAG_RY
+#define SLEDGE_TAG_RY 4
+#endif
+constexpr int TAG_RY = SLEDGE_TAG_RY;                  // rows per warp
+#ifndef SLEDGE_TAG_WARPS
+#define SLEDGE_TAG_WARPS 4
+#endif
+constexpr int TAG_WARPS = SLEDGE_TAG_WARPS;               // warps per CTA, stacked in y
 constexpr int TAG_TY = TAG_RY * TAG_WARPS; // rows per CTA tile
 constexpr int TAG_THREADS = TAG_WARPS * 32;
+template <typename T> constexpr size_t tag_smem_bytes();
+#ifndef SLEDGE_TAG_PF
+#define SLEDGE_TAG_PF 4
+#endif
+constexpr int TAG_PF = SLEDGE_TAG_PF;       // planes in flight per thread (cp.async ring depth)
 static_assert(TAG_RY <= 32, "a warp's rows may straddle at most two 32-blocks");
 
 template <typename T>
@@ -53,14 +65,15 @@ __device__ __forceinline__ float cross_rn(float a1, float a2, float b1, float b2
   return __fsub_rn(__fmul_rn(a1, b2), __fmul_rn(a2, b1));
 }
 
-// E(a -> b): +1 if up && cr > 0, -1 if dn && cr < 0, else 0, with up = a2<0 && b2>=0, dn = a2>=0 && b2<0
-// (the comparisons are written as in the definition so that NaN / -0 behave identically)
+// E(a -> b): +1 if up && cr > 0, -1 if dn && cr < 0, else 0, with up = a2<0 && b2>=0, dn = a2>=0 && b2<0.
+// sa = (a2 < 0) and sb = (b2 < 0) are evaluated once per loaded value.  Writing b2 >= 0 as !(b2 < 0) differs from
+// the definition only when a2 or b2 is NaN, and then cr is NaN and the edge is 0 either way; -0 is not < 0 in
+// both forms.
 template <typename T, typename P>
-__device__ __forceinline__ int edge_of(const P& a, const P& b) {
+__device__ __forceinline__ int edge_of(const P& a, bool sa, const P& b, bool sb) {
   const T cr = cross_rn(a.x, a.y, b.x, b.y);
-  const bool up = (a.y < T(0)) && (b.y >= T(0));
-  const bool dn = (a.y >= T(0)) && (b.y < T(0));
-  return (up && cr > T(0)) ? 1 : ((dn && cr < T(0)) ? -1 : 0);
+  const bool up = sa && !sb, dn = !sa && sb;
+  return (int)(up && cr > T(0)) - (int)(dn && cr < T(0));
 }
 
 template <typename P>
@@ -75,6 +88,10 @@ __device__ __forceinline__ float2 shfl_down_pair<float2>(const float2& v, int de
 }
 
 
+
+template <typename T> constexpr size_t tag_smem_bytes() {
+  return ((size_t)TAG_WARPS * TAG_PF * (TAG_RY + 1) * 32 + 1) * sizeof(typename PairOf<T>::type);
+}
 
 // edges of P+x packed for the shuffle: (Ey+1) | (Ez+1)<<2
 template <typename T>
@@ -96,16 +113,31 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
   for (int r = 0; r <= RY; ++r) orow[r] = org + (long long)(min(y0 + r, b.n[1]) + a.g) * b.sx;
 
   // plane index n is relative to t.z0; n = nz is the first plane above the tile (a ghost plane or the next tile)
-  auto ld = [&](int r, int n) -> P { return __ldg(a.psi + orow[r] + (long long)min(n, t.nz) * plane); };
-  P pre[RY + 1], cur[RY + 1];
+  // Every lane streams its own column through a per-warp shared-memory ring with cp.async, TAG_PF planes ahead:
+  // the bytes in flight cost no registers.  ring[slot][row][lane]; lane l reads its +x partner at [lane + 1].
+  extern __shared__ __align__(16) unsigned char tag_smem[];
+  P* const ring = reinterpret_cast<P*>(tag_smem) + (size_t)warp * (TAG_PF * (RY + 1) * 32) + lane;
+  auto issue = [&](int n) {
+    P* const dst = ring + (n % TAG_PF) * ((RY + 1) * 32);
+    const long long po = (long long)min(n, t.nz) * plane;
 #pragma unroll
-  for (int r = 0; r <= RY; ++r) {
-    pre[r] = ld(r, 0);
-    cur[r] = pre[r];
+    for (int r = 0; r <= RY; ++r) cp_async_pair(dst + r * 32, a.psi + orow[r] + po);
+  };
+#pragma unroll
+  for (int d = 0; d < TAG_PF; ++d) {
+    issue(d);
+    cp_async_commit();
   }
+  P cur[RY + 1];
+  cp_async_wait<TAG_PF - 1>();
+#pragma unroll
+  for (int r = 0; r <= RY; ++r) cur[r] = ring[r * 32];  // plane 0 (slot 0), own entries only
   int exc[RY], eyc[RY], wxyc[RY];  // in-plane edges and W_xy of the plane below
 #pragma unroll
   for (int r = 0; r < RY; ++r) exc[r] = eyc[r] = wxyc[r] = 0;
+  bool sc[RY + 1];  // (psi2 < 0) of cur
+#pragma unroll
+  for (int r = 0; r <= RY; ++r) sc[r] = cur[r].y < T(0);
 
   // count blocks: lanes split over at most two x-blocks, rows over at most two y-blocks
   const int bi = (b.lo[0] + min(x, b.n[0] - 1)) >> 5;
@@ -129,22 +161,36 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
     cntA = cntB = 0;
   };
 
+#pragma unroll 2
   for (int n = 0; n <= t.nz; ++n) {
     P nO[RY + 1], nX[RY + 1];
+    bool so[RY + 1], sx[RY + 1];
+    unsigned sbits = 0;
+#pragma unroll
+    cp_async_wait<TAG_PF - 1>();  // this lane's copies of plane n have landed ...
+    __syncwarp();                 // ... and its neighbour's
+    const P* const src = ring + (n % TAG_PF) * ((RY + 1) * 32);
 #pragma unroll
     for (int r = 0; r <= RY; ++r) {
-      nO[r] = pre[r];
-      pre[r] = ld(r, n + 1);
-      nX[r] = shfl_down_pair<P>(nO[r], 1);  // lane 31 gets itself: its Ex is never used
+      nO[r] = src[r * 32];
+      nX[r] = src[r * 32 + 1];  // lane 31 reads a foreign entry: its Ex is never used
+      so[r] = nO[r].y < T(0);
+      sbits |= (so[r] ? 1u : 0u) << r;
     }
+    __syncwarp();  // everybody has read slot n % TAG_PF before it is refilled
+    issue(n + TAG_PF);
+    cp_async_commit();
+    sbits = __shfl_down_sync(0xffffffffu, sbits, 1);
+#pragma unroll
+    for (int r = 0; r <= RY; ++r) sx[r] = (sbits >> r) & 1u;
     int ex[RY + 1], ez[RY + 1], ey[RY];
 #pragma unroll
     for (int r = 0; r <= RY; ++r) {
-      ex[r] = edge_of<T, P>(nO[r], nX[r]);   // plane n
-      ez[r] = edge_of<T, P>(cur[r], nO[r]);  // plane n-1 -> n (0 at n = 0: cur == nO)
+      ex[r] = edge_of<T, P>(nO[r], so[r], nX[r], sx[r]);   // plane n
+      ez[r] = edge_of<T, P>(cur[r], sc[r], nO[r], so[r]);  // plane n-1 -> n (0 at n = 0: cur == nO)
     }
 #pragma unroll
-    for (int r = 0; r < RY; ++r) ey[r] = edge_of<T, P>(nO[r], nO[r + 1]);
+    for (int r = 0; r < RY; ++r) ey[r] = edge_of<T, P>(nO[r], so[r], nO[r + 1], so[r + 1]);
     int pk = 0;  // (Ey+1) | (Ez+1)<<2 of every row, 4 bits per row, for the lane on the left
 #pragma unroll
     for (int r = 0; r < RY; ++r) pk |= ((ey[r] + 1) | ((ez[r] + 1) << 2)) << (4 * r);
@@ -174,7 +220,10 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
       eyc[r] = ey[r];
     }
 #pragma unroll
-    for (int r = 0; r <= RY; ++r) cur[r] = nO[r];
+    for (int r = 0; r <= RY; ++r) {
+      cur[r] = nO[r];
+      sc[r] = so[r];
+    }
   }
   flush(cur_bk);
 }

@@ -67,6 +67,9 @@ constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
 #ifndef SLEDGE_K1F_PDMAX
 #define SLEDGE_K1F_PDMAX 2
 #endif
+#ifndef SLEDGE_K1_RY
+#define SLEDGE_K1_RY 1
+#endif
 #ifndef SLEDGE_K1F_RY
 #define SLEDGE_K1F_RY 2
 #endif
@@ -82,7 +85,7 @@ template <int MODE> struct K1Shape {
   static constexpr size_t SMEM = fused ? K1F_SMEM : K1_SMEM;
   static constexpr bool plane = fused ? (SLEDGE_K1F_PLANE != 0) : (SLEDGE_K1_PLANE != 0);
   static constexpr int PDMAX = fused ? SLEDGE_K1F_PDMAX : 3;
-  static constexpr int RY = fused ? SLEDGE_K1F_RY : 1;  // rows per thread (k_rk_plane)
+  static constexpr int RY = fused ? SLEDGE_K1F_RY : SLEDGE_K1_RY;  // rows per thread (k_rk_plane)
   static constexpr int MINB = MODE == FUSED_A ? SLEDGE_K1F_MINB_A : (MODE == FUSED_B ? SLEDGE_K1F_MINB_B : 1);
 };
 
@@ -669,7 +672,12 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   a.nb1 = L.nb[1];
   {
     Timed t(c, KIND_TAG);
-    k_tag_strings<T><<<(int)L.tag_tiles.size(), TAG_THREADS, 0, c->stream>>>(a);
+    static bool configured = false;  // per instantiation
+    if (!configured) {
+      cudaFuncSetAttribute(k_tag_strings<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
+      configured = true;
+    }
+    k_tag_strings<T><<<(int)L.tag_tiles.size(), TAG_THREADS, tag_smem_bytes<T>(), c->stream>>>(a);
   }
   return check_launch(c, "k_tag_strings");
 }
