@@ -27,6 +27,23 @@ METRIC = "Gcell-updates/s per RK stage"
 UNIT = "Gcell-updates/s"
 
 
+def ncu_traffic(workload, flow):
+    """mean dram__bytes_read.sum + dram__bytes_write.sum per K1 launch of this workload / data-flow, from the committed
+    `ncu --set full` capture (profiles/r01_traffic.csv; command in profiles/r01_c3_ncu_full_final.md); None if
+    that workload was not captured."""
+    import csv
+    try:
+        rows = [r for r in csv.DictReader(open(os.path.join(ROOT, "profiles", "r01_traffic.csv")))
+                if r["workload"] == workload and r["flow"] == flow and "k_rk_" in r["kernel"]]
+    except OSError:
+        return None
+    if not rows:
+        return None
+    return {"dram_bytes_per_launch": sum(float(r["dram_bytes_per_launch"]) for r in rows) / len(rows),
+            "algorithmic_bytes_per_launch": sum(float(r["algorithmic_bytes_per_launch"]) for r in rows) / len(rows),
+            "source": "profiles/r01_traffic.csv (ncu --set full, one capture per sweep kernel)"}
+
+
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -309,9 +326,11 @@ def run_sledge(args, cfg):
     # profile counters cover the timed K steps: n_stage launches moved cell_steps * words * esz bytes per step
     stage_bytes_total = stage_words_per_step * esz * args.steps
     achieved = stage_bytes_total / (ms_stage * 1e-3) / 1e9 if ms_stage > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_rk_pipe (K1, mean over the stage launches of a step: 2 sweeps per level-step FUSED, 4 otherwise)", "achieved": achieved,
+    tr = ncu_traffic(cfg.name, args.flow)
+    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_plane FUSED sweeps on level 0, k_rk_pipe staged sweeps elsewhere; mean over the "
+                                          "stage launches of a step: 2 sweeps per level-step FUSED, 4 otherwise)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
-                "peak_source": peak_src, "traffic": None,
+                "peak_source": peak_src, "traffic": (tr or {}).get("dram_bytes_per_launch"), "traffic_detail": tr,
                 "bytes_per_cell_step": words_per_cell_step * esz,
                 "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage}
     shares = {k: (v[1] / args.steps) for k, v in prof.items()}
