@@ -227,21 +227,15 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
   *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW);
 }
 
-// The fill itself: one thread per entry of the level's list.
+// The fill itself: GHOST_EPT entries of the level's list per thread (strided by the CTA size, so that a warp still
+// reads consecutive entries).  All entries, then all copy sources, are loaded before anything is stored: the
+// dependent chain entry -> source -> store is paid once per thread, not once per ghost cell.
+constexpr int GHOST_EPT = 4;
+
 template <typename T, bool FILL_PI>
-__global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T> a) {
-  const unsigned e = blockIdx.x * GHOST_THREADS + threadIdx.x;
-  if (e >= a.n_entries) return;
-  const uint4 en = __ldg(reinterpret_cast<const uint4*>(a.list) + e);
-  const unsigned kind = en.w & 3u;
-  if (kind == GHOST_COPY) {
-    a.psi[en.x] = a.psi[en.y];
-    if (FILL_PI) a.pi[en.x] = a.pi[en.y];
-    return;
-  }
-  if (kind == GHOST_NONE) return;
+__device__ __forceinline__ void ghost_interp_entry(const GhostArgs<T>& a, const uint4 en) {
   long long o[8];
-  if (kind == GHOST_INTERP) {
+  if ((en.w & 3u) == GHOST_INTERP) {
     const long long sx = en.z & 0xffffu, pl = sx * (long long)(en.z >> 16);
     const long long dx = (en.w & 4u) ? 1 : -1, dy = (en.w & 8u) ? sx : -sx, dz = (en.w & 16u) ? pl : -pl;
 #pragma unroll
@@ -256,6 +250,36 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
   }
   a.psi[en.x] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
   if (FILL_PI) a.pi[en.x] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
+}
+
+template <typename T, bool FILL_PI>
+__global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T> a) {
+  using P = typename PairOf<T>::type;
+  const unsigned e0 = blockIdx.x * (GHOST_THREADS * GHOST_EPT) + threadIdx.x;
+  uint4 en[GHOST_EPT];
+#pragma unroll
+  for (int j = 0; j < GHOST_EPT; ++j) {
+    const unsigned e = e0 + j * GHOST_THREADS;
+    en[j] = e < a.n_entries ? __ldg(reinterpret_cast<const uint4*>(a.list) + e) : make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
+  }
+  P v[GHOST_EPT], vp[GHOST_EPT];
+#pragma unroll
+  for (int j = 0; j < GHOST_EPT; ++j)
+    if ((en[j].w & 3u) == GHOST_COPY) {
+      v[j] = a.psi[en[j].y];
+      if (FILL_PI) vp[j] = a.pi[en[j].y];
+    }
+#pragma unroll
+  for (int j = 0; j < GHOST_EPT; ++j)
+    if ((en[j].w & 3u) == GHOST_COPY) {
+      a.psi[en[j].x] = v[j];
+      if (FILL_PI) a.pi[en[j].x] = vp[j];
+    }
+#pragma unroll
+  for (int j = 0; j < GHOST_EPT; ++j) {
+    const unsigned kind = en[j].w & 3u;
+    if (kind == GHOST_INTERP || kind == GHOST_SLOW) ghost_interp_entry<T, FILL_PI>(a, en[j]);
+  }
 }
 
 }  // namespace sledge

@@ -407,7 +407,7 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
 template <typename T>
 int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
   const GhostArgs<T> a = ghost_args<T>(c, l, buf, time);
-  const int grid = c->plan.lev[l].ghost_prefix.back();
+  const int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
   if (grid == 0) return SLEDGE_OK;
   {
     Timed t(c, KIND_GHOST);

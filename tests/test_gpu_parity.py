@@ -125,6 +125,52 @@ def test_ragged_multibox_fp64(order, g, flow):
     _compare_tags(o, s, 0)
 
 
+def _bf4_boxes():
+    # 44 x 36 x 40 domain, blocking factor 4: tile heights that are not multiples of the K1 tile (4, 12, 20, 24
+    # rows), box corners that are not multiples of 32 (a tagging warp straddles two count blocks in x)
+    return [
+        (0, (0, 0, 0), (27, 11, 39)),
+        (0, (28, 0, 0), (43, 11, 39)),
+        (0, (0, 12, 0), (43, 35, 19)),
+        (0, (0, 12, 20), (19, 35, 39)),
+        (0, (20, 12, 20), (43, 31, 39)),
+        (0, (20, 32, 20), (43, 35, 39)),
+    ]
+
+
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (2, 3)])
+@pytest.mark.parametrize("flow", ["lean", "fused"])
+def test_ragged_blocking_factor_4(order, g, flow):
+    P = _pair()
+    n0 = (44, 36, 40)
+    o, s = P.make_pair(n0, boxes=_bf4_boxes(), nghost=g, blocking_factor=4, lap_order=order, h0=0.5, lam=1.0,
+                       rk_dataflow=flow)
+    P.init_smooth(o, s, n0, seed=12)
+    eta, dt = 1.2, 0.1
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    _compare_tags(o, s, 0)
+
+
+def test_blocking_factor_2_rows_of_one_warp_straddle_two_count_blocks():
+    # box 2 starts at y = 30: the four rows of a tagging warp (30..33) fall into two 32-blocks
+    P = _pair()
+    n0 = (34, 38, 36)
+    boxes = [(0, (0, 0, 0), (33, 29, 35)), (0, (0, 30, 0), (17, 37, 35)), (0, (18, 30, 0), (33, 37, 35))]
+    o, s = P.make_pair(n0, boxes=boxes, nghost=1, blocking_factor=2, lap_order=1, h0=0.5, lam=1.0, rk_dataflow="fused")
+    P.init_smooth(o, s, n0, seed=13)
+    eta, dt = 1.0, 0.1
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    _compare_tags(o, s, 0)
+
+
 def test_eta_fixed_minkowski_variant():
     P = _pair()
     o, s = P.make_pair(16, nghost=2, lap_order=2, h0=0.25, eta_fixed=True)
