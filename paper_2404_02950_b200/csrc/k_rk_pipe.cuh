@@ -67,6 +67,8 @@ struct PipeArgs {
   P* out_psi[2];
   P* out_pi[2];
   int g, ox;
+  int wrap;        // k_rk_plane only: the level is ONE box covering the periodic domain and the kernel wraps its halo /
+                   // window addresses itself (L23), so no ghost fill is needed before the sweep
   T inv_h2;        // 1/h^2 (order 1) or 1/(12 h^2) (order 2)
   T lam_eta2[3];   // lambda * eta^2 at t, t + dt/2, t + dt (unfused: [0] = the stage's value)
   T fric[3];       // kappa / eta at the same times

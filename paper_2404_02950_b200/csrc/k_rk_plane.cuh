@@ -84,6 +84,14 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_plane(const PipeArgs<T
   const long long tile_org =
       b.base + (long long)(t.z0 + a.g) * plane + (long long)(t.y0 + a.g) * b.sx + (t.x0 + a.ox);
   const long long off = tile_org + (long long)ty * b.sx + tx * CPT;  // this thread's first cell in plane z0
+  // periodic single-box level (a.wrap): anything outside [0, n) is read at its wrapped position instead of from
+  // the ghost layers (L23).  wofs(c, n) = displacement that brings coordinate c into the box.
+  const bool wr = a.wrap != 0;
+  auto wofs = [wr](int c, int n) -> int { return !wr ? 0 : (c < 0 ? n : (c >= n ? -n : 0)); };
+  long long offl[RY];  // load address of row j (== off + j * sx unless the row / column lies past the box edge)
+#pragma unroll
+  for (int j = 0; j < RY; ++j) offl[j] = off + (long long)(j + wofs(y + j, b.n[1])) * b.sx + wofs(x, b.n[0]);
+  auto zofs = [&](int p) -> long long { return (long long)(p + wofs(t.z0 + p, b.n[2])) * plane; };
 
   // halo assignment: pair index -> (hx, hy) relative to the tile origin
   int h_goff[HPT];  // global offset relative to tile_org (within a plane)
@@ -105,7 +113,7 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_plane(const PipeArgs<T
     }
     // stay inside the box's ghosted extent (partial tiles at the high end of a box)
     ok = ok && (t.x0 + hx < b.n[0] + R) && (t.y0 + hy < b.n[1] + R);
-    h_goff[q] = hy * b.sx + hx;
+    h_goff[q] = (hy + wofs(t.y0 + hy, b.n[1])) * b.sx + hx + wofs(t.x0 + hx, b.n[0]);
     h_soff[q] = ok ? ((hy + R) * SW + (hx + XO)) : -1;
   }
   const int s_own = (ty + R) * SW + (tx * CPT + XO);  // row j of this thread: s_own + j * SW
@@ -113,12 +121,12 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_plane(const PipeArgs<T
   // copy of the ghosted plane p (relative to z0) of every differenced field into `slot`
   auto issue_plane = [&](int p, int slot) {
     P* const dst = planes + (size_t)slot * NF * PSZ;
-    const long long po = (long long)p * plane;
+    const long long po = zofs(p);
 #pragma unroll
     for (int j = 0; j < RY; ++j)
       if (loader[j]) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) cp_async_16(dst + f * PSZ + s_own + j * SW, a.sten[f] + off + po + (long long)j * b.sx);
+        for (int f = 0; f < NF; ++f) cp_async_16(dst + f * PSZ + s_own + j * SW, a.sten[f] + offl[j] + po);
       }
 #pragma unroll
     for (int q = 0; q < HPT; ++q)
@@ -160,7 +168,7 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_plane(const PipeArgs<T
     for (int j = 0; j < RY; ++j)
 #pragma unroll
       for (int m = 0; m < 2 * R; ++m)
-        if (loader[j]) w[f][j][m + 1] = ldg16_keep<T>(a.sten[f] + off + (long long)(m - R) * plane + (long long)j * b.sx);
+        if (loader[j]) w[f][j][m + 1] = ldg16_keep<T>(a.sten[f] + offl[j] + zofs(m - R));
 
   int slot_c = 0;             // slot of the centre plane zz
   int slot_t = R % S;         // slot of plane zz + R

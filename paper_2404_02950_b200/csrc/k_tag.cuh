@@ -54,6 +54,8 @@ struct TagArgs {
   uint8_t* tags;     // may be null
   uint32_t* counts;  // may be null
   int g, ox;
+  int wrap;      // the level is ONE box covering the periodic domain: +1 neighbours past the box edge are read at
+                 // their wrapped position instead of from the ghost layer (L23), no ghost fill needed
   int nb0, nb1;  // count blocks per axis (x, y)
 };
 
@@ -104,13 +106,14 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
   const int x = t.x0 + lane, y0 = t.y0 + warp * RY;
   if (y0 >= b.n[1]) return;  // whole warp leaves together; there is no block-level synchronisation
   // cells past the box edge clamp to the first ghost layer (g >= 1): valid memory, results unused
-  const int xc = min(x, b.n[0]);
+  const bool wr = a.wrap != 0;
+  const int xc = (wr && x >= b.n[0]) ? 0 : min(x, b.n[0]);
   const bool actx = lane < TAG_TX && x < b.n[0];
   const long long plane = (long long)b.sx * b.sy;
   const long long org = b.base + (long long)(t.z0 + a.g) * plane + (xc + a.ox);
   long long orow[RY + 1];
 #pragma unroll
-  for (int r = 0; r <= RY; ++r) orow[r] = org + (long long)(min(y0 + r, b.n[1]) + a.g) * b.sx;
+  for (int r = 0; r <= RY; ++r) orow[r] = org + (long long)(((wr && y0 + r >= b.n[1]) ? 0 : min(y0 + r, b.n[1])) + a.g) * b.sx;
 
   // plane index n is relative to t.z0; n = nz is the first plane above the tile (a ghost plane or the next tile)
   // Every lane streams its own column through a per-warp shared-memory ring with cp.async, TAG_PF planes ahead:
@@ -119,7 +122,8 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
   P* const ring = reinterpret_cast<P*>(tag_smem) + (size_t)warp * (TAG_PF * (RY + 1) * 32) + lane;
   auto issue = [&](int n) {
     P* const dst = ring + (n % TAG_PF) * ((RY + 1) * 32);
-    const long long po = (long long)min(n, t.nz) * plane;
+    const int pn = min(n, t.nz);
+    const long long po = (long long)((wr && t.z0 + pn >= b.n[2]) ? -t.z0 : pn) * plane;
 #pragma unroll
     for (int r = 0; r <= RY; ++r) cp_async_pair(dst + r * 32, a.psi + orow[r] + po);
   };

@@ -35,7 +35,7 @@ constexpr size_t ALIGN = 256;
 #define SLEDGE_K1_TY 16
 #endif
 #ifndef SLEDGE_K1_NZ
-#define SLEDGE_K1_NZ 64
+#define SLEDGE_K1_NZ 128
 #endif
 #ifndef SLEDGE_K1_DMAX
 #define SLEDGE_K1_DMAX 4
@@ -55,6 +55,7 @@ constexpr size_t ALIGN = 256;
 constexpr int K1_TX = 32, K1_TY = SLEDGE_K1_TY, K1_NZ = SLEDGE_K1_NZ;
 constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
+constexpr long long K1F_MIN_TILES = 3500;  // below this many CTAs the fused sweeps halve their z-chunk
 constexpr int K1F_TY = SLEDGE_K1F_TY;            // tile rows / budget of the FUSED sweeps
 constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
 // which on-chip data path a sweep uses: 1 = k_rk_plane (ghosted plane ring), 0 = k_rk_pipe (ring + centre plane)
@@ -72,6 +73,9 @@ constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
 #endif
 #ifndef SLEDGE_K1F_RY
 #define SLEDGE_K1F_RY 2
+#endif
+#ifndef SLEDGE_K1F_RY32
+#define SLEDGE_K1F_RY32 1  // fp32 sweeps move half the bytes per cell through shared memory: one row per thread is faster
 #endif
 #ifndef SLEDGE_K1F_MINB_A
 #define SLEDGE_K1F_MINB_A 3
@@ -103,6 +107,7 @@ struct LevelHost {
   long long valid_cells = 0;
   long long count_blocks = 0;
   int nb[3];
+  bool periodic_box = false;  // ONE box covering the periodic domain: K1 (plane variant) and K3 wrap by themselves
   // arena offsets (bytes)
   size_t off_buf[NBUF][2];
   size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix, off_ghost_list;
@@ -256,17 +261,25 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   const int cpt = p.dtype == SLEDGE_F64 ? 1 : 2;
   for (int l = 0; l < p.n_levels; ++l) {
     LevelHost& L = P.lev[l];
+    L.periodic_box = L.boxdev.size() == 1 && L.boxdev[0].n[0] == L.n[0] && L.boxdev[0].n[1] == L.n[1] &&
+                     L.boxdev[0].n[2] == L.n[2];
     L.ghost_prefix.assign(1, 0);
     L.avg_prefix.assign(1, 0);
+    // z-chunk of the fused sweeps: long marches amortise the pipeline prologue, but the grid must stay many waves
+    // deep (148 SMs x 2-3 CTAs); measured on C2 / C3 (profiles/r01_k1_tile_sweep.md)
+    const int txc = K1_TX * cpt;
+    long long ft_long = 0;
+    for (const BoxDev& b : L.boxdev)
+      ft_long += (long long)((b.n[0] + txc - 1) / txc) * ((b.n[1] + K1F_TY - 1) / K1F_TY) * ((b.n[2] + K1_NZ - 1) / K1_NZ);
+    const int fnz = ft_long >= K1F_MIN_TILES ? K1_NZ : K1_NZ / 2;
     for (size_t q = 0; q < L.boxdev.size(); ++q) {
       const BoxDev& b = L.boxdev[q];
-      const int txc = K1_TX * cpt;
       for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
         for (int y0 = 0; y0 < b.n[1]; y0 += K1_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
-      for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
+      for (int z0 = 0; z0 < b.n[2]; z0 += fnz)
         for (int y0 = 0; y0 < b.n[1]; y0 += K1F_TY)
-          for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
+          for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(fnz, b.n[2] - z0)});
       for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
         for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
@@ -432,7 +445,7 @@ cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   constexpr int TY = K1Shape<MODE>::TY;
   static bool configured = false;  // per instantiation
   if constexpr (K1Shape<MODE>::plane) {
-    constexpr int RY = K1Shape<MODE>::RY;
+    constexpr int RY = (K1Shape<MODE>::fused && sizeof(T) == 4) ? SLEDGE_K1F_RY32 : K1Shape<MODE>::RY;
     constexpr int PD = plane_depth<T, ORDER, MODE, K1_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
     using C = PlaneCfg<T, ORDER, MODE, K1_TX, TY, PD, RY>;
     static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
@@ -522,9 +535,12 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
   set_eta(P, a, 1, fx ? eta_const : t + 0.5 * dt);
   set_eta(P, a, 2, fx ? eta_const : t + dt);
   a.adt = (T)dt;
-  int rc;
+  // a level that is one box over the periodic domain needs no ghost fill: k_rk_plane wraps its own addresses
+  const bool wrap = L.periodic_box && (SLEDGE_K1F_PLANE != 0);
+  a.wrap = wrap ? 1 : 0;
+  int rc = SLEDGE_OK;
   if (pass == 0) {
-    rc = launch_ghosts<T>(c, l, cur, t, true);
+    if (!wrap) rc = launch_ghosts<T>(c, l, cur, t, true);
     if (rc) return rc;
     a.sten[0] = plane_ptr<T>(c, l, cur, 0);
     a.sten[1] = plane_ptr<T>(c, l, cur, 1);
@@ -532,7 +548,7 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
     a.out_pi[0] = plane_ptr<T>(c, l, cur + 1, 1);
     return launch_k1<T>(c, l, FUSED_A, a);
   }
-  rc = launch_ghosts<T>(c, l, cur + 1, t + 0.5 * dt, true);  // Y's ghosts are still valid from pass 0
+  if (!wrap) rc = launch_ghosts<T>(c, l, cur + 1, t + 0.5 * dt, true);  // Y's ghosts are still valid from pass 0
   if (rc) return rc;
   a.sten[0] = plane_ptr<T>(c, l, cur + 1, 0);
   a.sten[1] = plane_ptr<T>(c, l, cur + 1, 1);
@@ -657,7 +673,7 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   LevelHost& L = P.lev[l];
   // after a coarse step every level sits at its parent's t_new: alpha = 1, no temporal interpolation (L74)
   const double tcur = (l > 0 && P.lev[l - 1].have_pair) ? P.lev[l - 1].t_new : 0.0;
-  int rc = launch_ghosts<T>(c, l, L.cur, tcur, false);
+  int rc = L.periodic_box ? SLEDGE_OK : launch_ghosts<T>(c, l, L.cur, tcur, false);  // K3 wraps by itself there
   if (rc) return rc;
   if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)L.count_blocks, c->stream);
   TagArgs<T> a;
@@ -668,6 +684,7 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   a.counts = counts;
   a.g = P.p.nghost;
   a.ox = P.ox;
+  a.wrap = L.periodic_box ? 1 : 0;
   a.nb0 = L.nb[0];
   a.nb1 = L.nb[1];
   {
