@@ -43,16 +43,21 @@ constexpr size_t ALIGN = 256;
 #ifndef SLEDGE_K1_SMEM
 #define SLEDGE_K1_SMEM (227 * 1024)
 #endif
-// The FUSED sweeps are not HBM-bound (fp64 pipe, shared-memory bandwidth and HBM all within 2x of each other):
-// they want several small CTAs per SM so that one CTA's barrier / load phase overlaps another's arithmetic.
-// Measured on C3 (profiles/r01_k1_tile_sweep.md): 32x8 threads with a 56 KB budget (3-4 CTAs per SM).
+// The FUSED sweeps load fp64 pipe, shared-memory bandwidth and HBM to within 2x of each other: they want several
+// small CTAs per SM so that one CTA's barrier / load phase overlaps another's arithmetic.  Measured on C3
+// (profiles/r01_k1_tile_sweep.md): 32x8 tile, two rows per thread (128 threads), prefetch distance 2 (113 KB budget),
+// 3 (sweep A) / 2 (sweep B) CTAs per SM.
 #ifndef SLEDGE_K1F_TY
 #define SLEDGE_K1F_TY 8
 #endif
 #ifndef SLEDGE_K1F_SMEM
 #define SLEDGE_K1F_SMEM (113 * 1024)
 #endif
+#ifndef SLEDGE_K1F_TX
+#define SLEDGE_K1F_TX 32
+#endif
 constexpr int K1_TX = 32, K1_TY = SLEDGE_K1_TY, K1_NZ = SLEDGE_K1_NZ;
+constexpr int K1F_TX = SLEDGE_K1F_TX;  // x vectors per fused tile (k_rk_plane)
 constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
 constexpr long long K1F_MIN_TILES = 3500;  // below this many CTAs the fused sweeps halve their z-chunk
@@ -267,10 +272,10 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.avg_prefix.assign(1, 0);
     // z-chunk of the fused sweeps: long marches amortise the pipeline prologue, but the grid must stay many waves
     // deep (148 SMs x 2-3 CTAs); measured on C2 / C3 (profiles/r01_k1_tile_sweep.md)
-    const int txc = K1_TX * cpt;
+    const int txc = K1_TX * cpt, ftxc = K1F_TX * cpt;
     long long ft_long = 0;
     for (const BoxDev& b : L.boxdev)
-      ft_long += (long long)((b.n[0] + txc - 1) / txc) * ((b.n[1] + K1F_TY - 1) / K1F_TY) * ((b.n[2] + K1_NZ - 1) / K1_NZ);
+      ft_long += (long long)((b.n[0] + ftxc - 1) / ftxc) * ((b.n[1] + K1F_TY - 1) / K1F_TY) * ((b.n[2] + K1_NZ - 1) / K1_NZ);
     const int fnz = ft_long >= K1F_MIN_TILES ? K1_NZ : K1_NZ / 2;
     for (size_t q = 0; q < L.boxdev.size(); ++q) {
       const BoxDev& b = L.boxdev[q];
@@ -279,7 +284,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
           for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
       for (int z0 = 0; z0 < b.n[2]; z0 += fnz)
         for (int y0 = 0; y0 < b.n[1]; y0 += K1F_TY)
-          for (int x0 = 0; x0 < b.n[0]; x0 += txc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(fnz, b.n[2] - z0)});
+          for (int x0 = 0; x0 < b.n[0]; x0 += ftxc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(fnz, b.n[2] - z0)});
       for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
         for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
@@ -446,10 +451,10 @@ cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   static bool configured = false;  // per instantiation
   if constexpr (K1Shape<MODE>::plane) {
     constexpr int RY = (K1Shape<MODE>::fused && sizeof(T) == 4) ? SLEDGE_K1F_RY32 : K1Shape<MODE>::RY;
-    constexpr int PD = plane_depth<T, ORDER, MODE, K1_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
-    using C = PlaneCfg<T, ORDER, MODE, K1_TX, TY, PD, RY>;
+    constexpr int PD = plane_depth<T, ORDER, MODE, K1F_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
+    using C = PlaneCfg<T, ORDER, MODE, K1F_TX, TY, PD, RY>;
     static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
-    auto kern = k_rk_plane<T, ORDER, MODE, K1_TX, TY, PD, RY, K1Shape<MODE>::MINB>;
+    auto kern = k_rk_plane<T, ORDER, MODE, K1F_TX, TY, PD, RY, K1Shape<MODE>::MINB>;
     if (!configured) {
       const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
       if (e != cudaSuccess) return e;
