@@ -33,6 +33,7 @@ constexpr int GHOST_THREADS = 256;
 enum GhostKind { GHOST_COPY = 0, GHOST_INTERP = 1, GHOST_SLOW = 2, GHOST_NONE = 3 };
 // x = dst, y / z = see above, w = kind | signs << 2 (bit d of signs: c1 = c0 + 1 along axis d)
 typedef uint4 GhostEntry;
+constexpr unsigned GHOST_STAR = 32u;  // bit 5 of w
 
 template <typename T>
 struct GhostArgs {
@@ -57,6 +58,9 @@ struct GhostArgs {
   int* err_flag;  // set to 1 if a ghost cell has neither a same-level owner nor coarse data
   GhostEntry* list;  // GHOST_THREADS entries per CTA of the enumeration (written by the plan, read by the fill)
   unsigned n_entries;
+  int star_depth;  // plan: the Laplacian's radius R (L649).  Entries of ghost cells that a star stencil of that radius
+                   // can reach -- outside the box along exactly ONE axis, by at most R -- carry GHOST_STAR
+  int star_only;   // fill: move only GHOST_STAR entries (the fill before an RK sweep); 0 = every ghost cell
 };
 
 __device__ __forceinline__ long long cell_offset(const BoxDev& b, int g, int ox, int i, int j, int k) {
@@ -187,6 +191,11 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
     j = (int)jj;
     i = (int)xx < g ? (int)xx - g : nx + ((int)xx - g);
   }
+  // how far outside the box, per axis (0 = inside)
+  const int dxo = i < 0 ? -i : (i >= nx ? i - nx + 1 : 0), dyo = j < 0 ? -j : (j >= ny ? j - ny + 1 : 0);
+  const int dzo = k < 0 ? -k : (k >= nz ? k - nz + 1 : 0);
+  const int nout = (dxo > 0) + (dyo > 0) + (dzo > 0);
+  const unsigned star = (nout == 1 && dxo + dyo + dzo <= a.star_depth) ? GHOST_STAR : 0u;
   const int f0 = b.lo[0] + i, f1 = b.lo[1] + j, f2 = b.lo[2] + k;  // unwrapped level index
   const int wi = wrap1(f0, a.geom.n[0]), wj = wrap1(f1, a.geom.n[1]), wk = wrap1(f2, a.geom.n[2]);
   const unsigned dst = (unsigned)cell_offset(b, g, a.geom.ox, i, j, k);
@@ -194,7 +203,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
   if (ow >= 0) {  // same-level copy wins (R9)
     const BoxDev sb = a.boxes[ow];
     const long long src = cell_offset(sb, g, a.geom.ox, wi - sb.lo[0], wj - sb.lo[1], wk - sb.lo[2]);
-    *out = make_uint4(dst, (unsigned)src, 0u, (unsigned)GHOST_COPY);
+    *out = make_uint4(dst, (unsigned)src, 0u, (unsigned)GHOST_COPY | star);
     return;
   }
   if (!a.has_coarse) {
@@ -218,13 +227,13 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
     const BoxDev cb = a.cboxes[ow0];
     const long long o0 = cell_offset(cb, a.cgeom.g, a.cgeom.ox, w0[0] - cb.lo[0], w0[1] - cb.lo[1], w0[2] - cb.lo[2]);
     const unsigned signs = (c1[0] > c0[0] ? 1u : 0u) | (c1[1] > c0[1] ? 2u : 0u) | (c1[2] > c0[2] ? 4u : 0u);
-    *out = make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (signs << 2));
+    *out = make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (signs << 2) | star);
     return;
   }
   // parents in several coarse boxes (or across the periodic seam of a single one): resolved at fill time
   long long o[8];
   if (!coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o)) *a.err_flag = 1;
-  *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW);
+  *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW | star);
 }
 
 // The fill itself: GHOST_EPT entries of the level's list per thread (strided by the CTA size, so that a warp still
@@ -261,6 +270,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
   for (int j = 0; j < GHOST_EPT; ++j) {
     const unsigned e = e0 + j * GHOST_THREADS;
     en[j] = e < a.n_entries ? __ldg(reinterpret_cast<const uint4*>(a.list) + e) : make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
+    if (a.star_only && !(en[j].w & GHOST_STAR)) en[j].w = (unsigned)GHOST_NONE;  // a star stencil never reads this cell
   }
   P v[GHOST_EPT], vp[GHOST_EPT];
 #pragma unroll

@@ -399,6 +399,8 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.err_flag = tab<int>(c, P.off_err);
   a.list = tab<GhostEntry>(c, L.off_ghost_list);
   a.n_entries = (unsigned)L.ghost_prefix.back() * GHOST_THREADS;
+  a.star_depth = P.p.lap_order;
+  a.star_only = 0;
   a.has_coarse = l > 0;
   a.alpha = T(0);
   if (l > 0) {
@@ -423,8 +425,9 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
 
 // K2 on buffer `buf` of level l: streams the level's ghost list (built once by plan_ghosts)
 template <typename T>
-int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi) {
-  const GhostArgs<T> a = ghost_args<T>(c, l, buf, time);
+int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false) {
+  GhostArgs<T> a = ghost_args<T>(c, l, buf, time);
+  a.star_only = star_only ? 1 : 0;  // before an RK sweep only the cells its star stencil reaches are needed
   const int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
   if (grid == 0) return SLEDGE_OK;
   {
@@ -545,7 +548,7 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
   a.wrap = wrap ? 1 : 0;
   int rc = SLEDGE_OK;
   if (pass == 0) {
-    if (!wrap) rc = launch_ghosts<T>(c, l, cur, t, true);
+    if (!wrap) rc = launch_ghosts<T>(c, l, cur, t, true, true);
     if (rc) return rc;
     a.sten[0] = plane_ptr<T>(c, l, cur, 0);
     a.sten[1] = plane_ptr<T>(c, l, cur, 1);
@@ -553,7 +556,7 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
     a.out_pi[0] = plane_ptr<T>(c, l, cur + 1, 1);
     return launch_k1<T>(c, l, FUSED_A, a);
   }
-  if (!wrap) rc = launch_ghosts<T>(c, l, cur + 1, t + 0.5 * dt, true);  // Y's ghosts are still valid from pass 0
+  if (!wrap) rc = launch_ghosts<T>(c, l, cur + 1, t + 0.5 * dt, true, true);  // Y's ghosts are still valid from pass 0
   if (rc) return rc;
   a.sten[0] = plane_ptr<T>(c, l, cur + 1, 0);
   a.sten[1] = plane_ptr<T>(c, l, cur + 1, 1);
@@ -602,7 +605,7 @@ int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const)
     else if (s == 2) { ubuf = cur + 3; mode = CLASSIC_S23; in[0] = cur; in[1] = cur + 1; out[0] = cur + 2; out[1] = cur + 1; bdt = dt / 3.0; }
     else { ubuf = cur + 2; mode = CLASSIC_S4; in[0] = cur + 1; out[0] = cur + 1; }
   }
-  int rc = launch_ghosts<T>(c, l, ubuf, ts, false);
+  int rc = launch_ghosts<T>(c, l, ubuf, ts, false, true);
   if (rc) return rc;
   PipeArgs<T> a;
   memset(&a, 0, sizeof a);
