@@ -95,7 +95,11 @@ int sledge_get_ghosted(sledge_ctx* ctx, int box, int comp, void* dev_dst);
  * same level at the periodically wrapped index if one exists, else trilinear interpolation of the
  * next coarser level, itself linearly interpolated in time between its states at the start and end
  * of its last step (alpha = (time - t_old)/(t_new - t_old); the current coarse state alone if that
- * level has not stepped since its state was set). */
+ * level has not stepped since its state was set).  This explicit call fills EVERY ghost cell (psi and Pi).
+ * The fills that sledge_rk_step / sledge_rk_stage issue themselves move only the ghost cells the Laplacian's star
+ * stencil reaches (outside the box along one axis, by at most lap_order), and none at all on a level that is one
+ * box over the periodic domain (the kernels read the wrapped cell directly), so after a step the ghost contents
+ * are unspecified until this function is called. */
 int sledge_fill_ghosts(sledge_ctx* ctx, int level, double time);
 
 /* One classic-RK4 stage (integrator.type 4, L808) of `level`: ghost fill of the stage input at
