@@ -17,6 +17,7 @@
 //                    space + linear in time                                       L68-74
 //   O6 subcycling  : advance l, then l+1 twice, then synchronise                  L66-76, L88 Fig.2
 //   O7 average-down: coarse <- mean of 8 fine children                            L74, L88
+//   O9 TEE tags    : |coarse - mean of children| > eps at synchronisation         L82-111 Eq.5-6, L373-380 Eq.12
 //   O8 string tags : plaquette winding number of (psi1,psi2) around 0; rule not printed in the
 //                    paper (L349-371 gives only the bool-per-cell hook) -> DESIGN.md reading R8
 //   diagnostics    : energies used only by the pins (L678 App.B; Gradient<order> L651-658)
@@ -100,6 +101,11 @@ struct Level {
   bool have_pair = false;
   LevelState K[4];          // RK4 slopes (k of the last orc_eval_rhs in K[0])
   LevelState U;             // stage state
+  // O9: truncation-error tags of this (fine) level, written by average_down when tee_on (L82-111, Eq.5-6, Eq.12)
+  bool tee_on = false;
+  double tee_eps[2] = {0, 0};
+  uint8_t* tee_tags = nullptr;     // caller's arrays (dense per box, x fastest, boxes back to back)
+  uint32_t* tee_counts = nullptr;  // tagged cells per aligned FLAG_BLOCK^3 block of this level
 };
 
 struct Oracle {
@@ -351,12 +357,23 @@ void eval_rhs(const Oracle& o, int l, const LevelState& S, LevelState& K, double
   }
 }
 
-// ---- O7: average-down -------------------------------------------------------------------------
+// ---- O7: average-down, O9: truncation-error tags ----------------------------------------------
+// O9 (self-shadow method, L82-98; Eq.5, Eq.6/12 with f = identity): just before level lf is synchronised onto
+// lf-1, both have evolved the same region independently for 2 dt_lf.  For every coarse cell C under fine cells
+//   Delta_c(C) = | phi_c^{lf-1}(C) - (1/8) sum_children phi_c^{lf} |,   c = psi1, psi2 (the scalar components),
+// with the coarse value taken BEFORE it is overwritten, and the 8 children of C get the tag byte
+//   bit0 = Delta_psi1 > eps_psi1,  bit1 = Delta_psi2 > eps_psi2          (strict >, Eq.12).
+// counts: tagged fine cells per aligned FLAG_BLOCK^3 block of level lf.
 bool average_down(Oracle& o, int lf) {
   if (lf < 1 || lf >= o.p.n_levels) { o.err = "average_down: bad fine level"; return false; }
   Level& Lf = o.lev[lf];
   Level& Lc = o.lev[lf - 1];
   bool all_ok = true;
+  const bool tee = Lf.tee_on;
+  int nb[3];
+  for (int d = 0; d < 3; ++d) nb[d] = (Lf.n[d] + FLAG_BLOCK - 1) / FLAG_BLOCK;
+  if (tee && Lf.tee_counts) memset(Lf.tee_counts, 0, sizeof(uint32_t) * (size_t)nb[0] * nb[1] * nb[2]);
+  size_t tag_off = 0;
   for (int q = 0; q < (int)Lf.boxes.size(); ++q) {
     const BoxIn& B = o.box[Lf.boxes[q]];
     const Field& F = Lf.Y[q];
@@ -367,14 +384,33 @@ bool average_down(Oracle& o, int lf) {
           int ow = owner_of(o, lf - 1, ci, cj, ck);
           if (ow < 0) { all_ok = false; continue; }
           const BoxIn& Bc = o.box[Lc.boxes[ow]];
+          uint8_t tag = 0;
           for (int c = 0; c < NCOMP; ++c) {
             double s = 0.0;
             for (int rz = 0; rz < 2; ++rz)
               for (int ry = 0; ry < 2; ++ry)
                 for (int rx = 0; rx < 2; ++rx) s += F.at(c, i + rx, j + ry, k + rz);
-            Lc.Y[ow].at(c, ci - Bc.lo[0], cj - Bc.lo[1], ck - Bc.lo[2]) = 0.125 * s;
+            double mean = 0.125 * s;
+            double& coarse = Lc.Y[ow].at(c, ci - Bc.lo[0], cj - Bc.lo[1], ck - Bc.lo[2]);
+            if (tee && c < 2) {  // c = PSI1, PSI2
+              double delta = std::fabs(coarse - mean);
+              if (delta > Lf.tee_eps[c]) tag |= (uint8_t)(1u << c);
+            }
+            coarse = mean;
+          }
+          if (tee) {
+            for (int rz = 0; rz < 2; ++rz)
+              for (int ry = 0; ry < 2; ++ry)
+                for (int rx = 0; rx < 2; ++rx)
+                  if (Lf.tee_tags)
+                    Lf.tee_tags[tag_off + ((size_t)(k + rz) * F.n[1] + (j + ry)) * F.n[0] + (i + rx)] = tag;
+            if (tag && Lf.tee_counts) {
+              int bi = (B.lo[0] + i) / FLAG_BLOCK, bj = (B.lo[1] + j) / FLAG_BLOCK, bk = (B.lo[2] + k) / FLAG_BLOCK;
+              Lf.tee_counts[((size_t)bk * nb[1] + bj) * nb[0] + bi] += 8;
+            }
           }
         }
+    tag_off += (size_t)F.n[0] * F.n[1] * F.n[2];
   }
   if (!all_ok) o.err = "average_down: fine cell without a coarse parent";
   return all_ok;
@@ -614,6 +650,20 @@ int orc_eval_rhs(void* h, int level, double eta, int do_fill) {
 int orc_rk_step(void* h, double dt, double eta) {
   Oracle& o = *(Oracle*)h;
   return advance(o, 0, eta, dt, eta) ? 0 : -1;
+}
+
+// O9: from now on every synchronisation of `fine_level` also writes truncation-error tags (tags / counts stay owned
+// by the caller and must outlive the handle's use; tags == nullptr switches it off)
+int orc_tee_enable(void* h, int fine_level, double eps_psi1, double eps_psi2, uint8_t* tags, uint32_t* counts) {
+  Oracle& o = *(Oracle*)h;
+  if (fine_level < 1 || fine_level >= o.p.n_levels) return -1;
+  Level& L = o.lev[fine_level];
+  L.tee_on = tags != nullptr || counts != nullptr;
+  L.tee_eps[0] = eps_psi1;
+  L.tee_eps[1] = eps_psi2;
+  L.tee_tags = tags;
+  L.tee_counts = counts;
+  return 0;
 }
 
 int orc_average_down(void* h, int fine_level) { return average_down(*(Oracle*)h, fine_level) ? 0 : -1; }

@@ -421,6 +421,94 @@ def test_average_down_affine_and_mean_preserving():
 
 
 # ------------------------------------------------------------------------------------------------
+# O9: truncation-error tags at synchronisation (L82-111 Eq.5-6, L373-380 Eq.12)
+# ------------------------------------------------------------------------------------------------
+
+
+def test_tee_is_zero_when_coarse_is_the_mean_of_its_children():
+    """Exactly representable affine data whose coarse values are the children's means: Delta = 0, and Eq.12 is a
+    strict inequality, so nothing is tagged even for eps = 0; a second synchronisation sees coarse == mean too."""
+    o = two_level(h0=1.0, lam=0.0)
+    coef = (0.5, 1.0, -2.0, 0.25)
+    for c in range(4):
+        o.set_state(0, c, affine(1.0, (16, 16, 16), (0, 0, 0), coef))
+        o.set_state(1, c, affine(0.5, o.box_shape(1), (8, 16, 8), coef))
+    o.tee_enable(1, 0.0, 0.0)
+    for _ in range(2):
+        o.average_down(1)
+        tags, counts = o.tee_tags(1)
+        assert not tags[0].any() and not counts.any()
+
+
+def test_tee_tags_equal_the_prescribed_offsets_exactly():
+    """fine = 1 everywhere (mean exactly 1), coarse = 1 + delta(C) with dyadic offsets: Delta = |delta| exactly, so
+    the tags are (|delta| > eps) per component, copied to the 8 children, and the block counts are 8 x the number
+    of tagged coarse cells in the block -- all computed here independently of the oracle."""
+    o = two_level(n0=32, lo=(8, 24, 16), hi=(39, 47, 47), h0=1.0, lam=0.0)  # fine box straddles 32-blocks
+    rng = np.random.default_rng(9)
+    d = [rng.integers(-8, 9, size=(32, 32, 32)) / 64.0 for _ in range(2)]  # multiples of 1/64 in [-1/8, 1/8]
+    for c in range(2):
+        o.set_state(0, c, 1.0 + d[c])
+        o.set_state(1, c, np.ones(o.box_shape(1)))
+    eps = (3 / 64.0, 5 / 64.0)
+    o.tee_enable(1, *eps)
+    o.average_down(1)
+    tags, counts = o.tee_tags(1)
+    cov = (slice(8, 24), slice(12, 24), slice(4, 20))  # z, y, x coarse footprint of the fine box
+    want_c = ((np.abs(d[0][cov]) > eps[0]).astype(np.uint8) | ((np.abs(d[1][cov]) > eps[1]).astype(np.uint8) << 1))
+    assert want_c.any() and not want_c.all()
+    want_f = want_c.repeat(2, axis=0).repeat(2, axis=1).repeat(2, axis=2)
+    assert np.array_equal(tags[0], want_f)
+    # a value exactly at the threshold is NOT tagged (strict >)
+    at = np.abs(d[0][cov]) == eps[0]
+    assert at.any() and not (want_c[at] & 1).any()
+    want_counts = np.zeros_like(counts)
+    zz, yy, xx = np.nonzero(want_f)
+    np.add.at(want_counts, ((zz + 16) // 32, (yy + 24) // 32, (xx + 8) // 32), 1)
+    assert np.array_equal(counts, want_counts) and counts.sum() == 8 * np.count_nonzero(want_c)
+    # the synchronisation itself is unchanged: covered coarse cells now hold the children's mean
+    assert np.all(o.get_state(0, 0)[cov] == 1.0)
+
+
+def test_tee_inside_rk_step_shrinks_with_resolution():
+    """Self-shadow estimate on a smooth standing wave (lambda = 0): the largest |coarse - fine| at the sync inside
+    rk_step, found by bisecting eps on the tag output, drops by more than 4x when h and dt are halved (one step of
+    length dt ~ h times a spatial error of at least O(h^2), the trilinear ghosts at the fine boundary, L100), i.e.
+    the tags respond to convergence as L98 describes."""
+    def max_tee(n0):
+        h0 = 1.0 / n0
+        lo = (n0 // 2,) * 3                # fine indices: the fine box refines coarse cells [n0/4, 3 n0/4)
+        hi = (3 * n0 // 2 - 1,) * 3
+        def run(eps):
+            o = Oracle(n0, boxes=[(0, (0, 0, 0), (n0 - 1,) * 3), (1, lo, hi)], n_levels=2, nghost=2, blocking_factor=4,
+                       lap_order=2, h0=h0, lam=0.0)
+            for l, ib in ((0, 0), (1, 1)):
+                hl = h0 / (1 << l)
+                blo = (0, 0, 0) if l == 0 else lo
+                z, y, x = coords(o.box_shape(ib))
+                X = (x + blo[0] + 0.5) * hl
+                Yc = (y + blo[1] + 0.5) * hl
+                Z = (z + blo[2] + 0.5) * hl
+                o.set_state(ib, 0, np.cos(2 * np.pi * X) * np.cos(2 * np.pi * Yc) * np.cos(2 * np.pi * Z))
+                o.set_state(ib, 1, np.sin(2 * np.pi * X) + 0 * Yc + 0 * Z)
+            o.average_down(1)  # start from identical states: coarse = mean of its children (Eq.5 "identical states")
+            o.tee_enable(1, eps, 1e30)
+            o.rk_step(0.25 * h0, 1.0)
+            return o.tee_tags(1)[0][0].any()
+        lo_e, hi_e = 0.0, 1.0
+        assert run(lo_e) and not run(hi_e)
+        for _ in range(24):
+            mid = 0.5 * (lo_e + hi_e)
+            if run(mid):
+                lo_e = mid
+            else:
+                hi_e = mid
+        return hi_e
+    e8, e16 = max_tee(8), max_tee(16)
+    assert e8 > 0 and e16 < e8 / 4.0
+
+
+# ------------------------------------------------------------------------------------------------
 # O6: subcycling bookkeeping
 # ------------------------------------------------------------------------------------------------
 
