@@ -125,6 +125,22 @@ int sledge_tag_strings(sledge_ctx* ctx, int level, uint8_t* dev_tags, uint32_t* 
  * children, all four components, on the current states. */
 int sledge_average_down(sledge_ctx* ctx, int fine_level);
 
+/* Truncation-error (TEE) tags of the self-shadow method (L82-111 Eq.5-6, L373-380 Eq.12 with f = identity), fused
+ * into the synchronisation: from now on every average-down of `fine_level` -- the explicit call above and the ones
+ * inside sledge_rk_step -- first compares, for every coarse cell C under a fine box, the coarse level's own value
+ * with the mean of its 8 fine children, Delta_c = |phi_c^{l-1}(C) - mean_c| for the scalar components c = psi1, psi2
+ * (in the context's dtype), and gives the 8 children the tag byte (Delta_psi1 > eps_psi1) | (Delta_psi2 > eps_psi2) << 1
+ * (strict >, Eq.12); then it overwrites the coarse value as before.
+ *   dev_tags   : device, one byte per VALID cell of `fine_level`, boxes of the level back to back in input order,
+ *                x fastest (the layout of sledge_tag_strings); 2-byte aligned; may be NULL.
+ *   dev_counts : device, uint32 per aligned 32^3 block of the fine level's index space (x fastest), zeroed and
+ *                refilled at every synchronisation: tagged fine cells in the block; may be NULL.
+ * Both NULL switches the tags off.  The buffers stay owned by the caller and must stay valid while enabled.  A level
+ * synchronises once per step of its parent, so after sledge_rk_step the buffers hold the LAST synchronisation.
+ * Level 0 has no coarser partner (the paper's shadow level, L98, is not built): SLEDGE_EINVAL. */
+int sledge_tee_enable(sledge_ctx* ctx, int fine_level, double eps_psi1, double eps_psi2, uint8_t* dev_tags,
+                      uint32_t* dev_counts);
+
 /* Bookkeeping. */
 int sledge_level_cells(const sledge_ctx* ctx, int level, int64_t* valid_cells, int64_t* count_blocks);
 int64_t sledge_launch_count(const sledge_ctx* ctx); /* kernels launched by this context so far */

@@ -5,6 +5,12 @@
 // 32 x 2 consecutive fine pairs per row (coalesced) and writes 32 consecutive coarse pairs.  The coarse
 // destination is found through the coarse owner table (a fine box may lie over several coarse boxes).
 // Children are summed in the fixed order z, y, x (x fastest) starting from 0, then scaled by 1/8.
+//
+// TEE variant (Eq.5-6, L373-380 Eq.12; self-shadow method, f = identity): the same thread reads the
+// coarse value BEFORE overwriting it, Delta_c = |coarse_c - mean_c| for c = psi1, psi2, tag = (Delta_psi1 > eps1) |
+// (Delta_psi2 > eps2) << 1 in the kernel's precision, writes the byte to the 8 children (four 2-byte stores) and adds
+// 8 to the fine level's 32^3 block count when the tag is set.  No extra pass over the data: the truncation-error
+// estimate rides on the synchronisation.
 #pragma once
 #include "k_ghost.cuh"
 
@@ -27,6 +33,11 @@ struct AvgArgs {
   P* c_psi;
   P* c_pi;
   int* err_flag;
+  // TEE variant only
+  T tee_eps[2];
+  uint8_t* tee_tags;     // dense tags of the FINE level (boxes back to back, x fastest); may be null
+  uint32_t* tee_counts;  // tagged fine cells per aligned 32^3 block of the fine level; may be null
+  int nb0, nb1;          // count blocks per axis (x, y) of the fine level
 };
 
 template <typename T>
@@ -46,7 +57,7 @@ __device__ __forceinline__ typename PairOf<T>::type mean8(const typename PairOf<
   return mkpair(T(0.125) * s0, T(0.125) * s1);
 }
 
-template <typename T>
+template <typename T, bool TEE>
 __global__ void __launch_bounds__(AVG_THREADS) k_average_down(const AvgArgs<T> a) {
   int lo_b = 0, hi_b = a.nfbox;
   const int blk = blockIdx.x;
@@ -71,7 +82,27 @@ __global__ void __launch_bounds__(AVG_THREADS) k_average_down(const AvgArgs<T> a
   const long long fo = cell_offset(fb, a.fgeom.g, a.fgeom.ox, 2 * I, 2 * J, 2 * K);
   const long long co = cell_offset(cb, a.cgeom.g, a.cgeom.ox, ci - cb.lo[0], cj - cb.lo[1], ck - cb.lo[2]);
   const long long fplane = (long long)fb.sx * fb.sy;
-  a.c_psi[co] = mean8<T>(a.f_psi, fo, fb.sx, fplane);
+  const typename PairOf<T>::type m = mean8<T>(a.f_psi, fo, fb.sx, fplane);
+  if (TEE) {
+    const typename PairOf<T>::type c = a.c_psi[co];  // the coarse level's own result, before the overwrite
+    const T d1 = fabs(c.x - m.x), d2 = fabs(c.y - m.y);
+    const unsigned tag = (d1 > a.tee_eps[0] ? 1u : 0u) | (d2 > a.tee_eps[1] ? 2u : 0u);
+    if (a.tee_tags) {
+      const unsigned short two = (unsigned short)(tag | (tag << 8));
+#pragma unroll
+      for (int rz = 0; rz < 2; ++rz)
+#pragma unroll
+        for (int ry = 0; ry < 2; ++ry) {
+          const long long o = fb.tag_base + ((long long)(2 * K + rz) * fb.n[1] + (2 * J + ry)) * fb.n[0] + 2 * I;
+          *reinterpret_cast<unsigned short*>(a.tee_tags + o) = two;  // o is even: n0 and tag_base are
+        }
+    }
+    if (tag && a.tee_counts) {
+      const int bi = (fb.lo[0] + 2 * I) >> 5, bj = (fb.lo[1] + 2 * J) >> 5, bk = (fb.lo[2] + 2 * K) >> 5;
+      atomicAdd(a.tee_counts + ((long long)bk * a.nb1 + bj) * a.nb0 + bi, 8u);
+    }
+  }
+  a.c_psi[co] = m;
   a.c_pi[co] = mean8<T>(a.f_pi, fo, fb.sx, fplane);
 }
 

@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -116,6 +117,11 @@ struct LevelHost {
   // arena offsets (bytes)
   size_t off_buf[NBUF][2];
   size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix, off_ghost_list;
+  // truncation-error tags written at this (fine) level's synchronisations (sledge_tee_enable)
+  bool tee_on = false;
+  double tee_eps[2] = {0, 0};
+  uint8_t* tee_tags = nullptr;
+  uint32_t* tee_counts = nullptr;
   // run state
   int cur = 0, old = 0;
   bool have_pair = false;
@@ -650,9 +656,19 @@ int do_average_down(sledge_ctx* c, int lf) {
   a.c_pi = plane_ptr<T>(c, lf - 1, C.cur, 1);
   a.err_flag = tab<int>(c, P.off_err);
   const int grid = F.avg_prefix.back();
+  if (F.tee_on) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
+    a.tee_eps[0] = (T)F.tee_eps[0];
+    a.tee_eps[1] = (T)F.tee_eps[1];
+    a.tee_tags = F.tee_tags;
+    a.tee_counts = F.tee_counts;
+    a.nb0 = F.nb[0];
+    a.nb1 = F.nb[1];
+    if (F.tee_counts) cudaMemsetAsync(F.tee_counts, 0, sizeof(uint32_t) * (size_t)F.count_blocks, c->stream);
+  }
   {
     Timed t(c, KIND_AVG);
-    k_average_down<T><<<grid, AVG_THREADS, 0, c->stream>>>(a);
+    if (F.tee_on) k_average_down<T, true><<<grid, AVG_THREADS, 0, c->stream>>>(a);
+    else k_average_down<T, false><<<grid, AVG_THREADS, 0, c->stream>>>(a);
   }
   return check_launch(c, "k_average_down");
 }
@@ -912,6 +928,22 @@ int sledge_level_cells(const sledge_ctx* c, int level, int64_t* valid_cells, int
   if (!c || level < 0 || level >= c->plan.p.n_levels) return SLEDGE_EINVAL;
   if (valid_cells) *valid_cells = c->plan.lev[level].valid_cells;
   if (count_blocks) *count_blocks = c->plan.lev[level].count_blocks;
+  return SLEDGE_OK;
+}
+
+int sledge_tee_enable(sledge_ctx* c, int fine_level, double eps_psi1, double eps_psi2, uint8_t* dev_tags,
+                      uint32_t* dev_counts) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  if (fine_level < 1 || fine_level >= c->plan.p.n_levels)
+    return fail(c, SLEDGE_EINVAL, "tee_enable: level %d has no coarser level to compare with", fine_level);
+  if (!(eps_psi1 >= 0) || !(eps_psi2 >= 0)) return fail(c, SLEDGE_EINVAL, "tee_enable: thresholds must be >= 0");
+  if (dev_tags && ((uintptr_t)dev_tags & 1)) return fail(c, SLEDGE_EINVAL, "tee_enable: tags must be 2-byte aligned");
+  LevelHost& L = c->plan.lev[fine_level];
+  L.tee_on = dev_tags != nullptr || dev_counts != nullptr;
+  L.tee_eps[0] = eps_psi1;
+  L.tee_eps[1] = eps_psi2;
+  L.tee_tags = dev_tags;
+  L.tee_counts = dev_counts;
   return SLEDGE_OK;
 }
 

@@ -23,7 +23,7 @@ COUNT_BLOCK = 32
 SYMBOLS = [
     "sledge_arena_bytes", "sledge_create", "sledge_destroy", "sledge_set_state", "sledge_get_state",
     "sledge_set_state_host", "sledge_get_state_host", "sledge_get_ghosted", "sledge_fill_ghosts",
-    "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_level_cells",
+    "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable", "sledge_level_cells",
     "sledge_launch_count", "sledge_synchronize", "sledge_profile_enable", "sledge_profile_read",
     "sledge_last_error",
 ]
@@ -68,6 +68,7 @@ def lib():
         L.sledge_rk_step.argtypes = [vp, d, d]
         L.sledge_tag_strings.argtypes = [vp, i, vp, vp]
         L.sledge_average_down.argtypes = [vp, i]
+        L.sledge_tee_enable.argtypes = [vp, i, C.c_double, C.c_double, vp, vp]
         L.sledge_level_cells.argtypes = [vp, i, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.sledge_launch_count.argtypes = [vp]
         L.sledge_launch_count.restype = C.c_int64
@@ -241,6 +242,23 @@ class Sledge:
 
     def average_down(self, fine_level):
         self._chk(lib().sledge_average_down(self._h, fine_level), "sledge_average_down")
+
+    def tee_enable(self, fine_level, eps_psi1, eps_psi2, tags: torch.Tensor | None = None,
+                   counts: torch.Tensor | None = None):
+        """sledge_tee_enable: every later synchronisation of `fine_level` writes truncation-error tags into the
+        returned (tags uint8 [valid cells of the level], counts int32 [bz, by, bx]) tensors, which this object
+        keeps alive."""
+        ncell, _ = self.level_cells(fine_level)
+        if tags is None:
+            tags = torch.zeros(ncell, dtype=torch.uint8, device=self.device)
+        if counts is None:
+            counts = torch.zeros(self.count_shape(fine_level), dtype=torch.int32, device=self.device)
+        self._chk(lib().sledge_tee_enable(self._h, fine_level, float(eps_psi1), float(eps_psi2), tags.data_ptr(),
+                                          counts.data_ptr()), "sledge_tee_enable")
+        if not hasattr(self, "_tee"):
+            self._tee = {}
+        self._tee[fine_level] = (tags, counts)
+        return tags, counts
 
     def synchronize(self):
         self._chk(lib().sledge_synchronize(self._h), "sledge_synchronize")

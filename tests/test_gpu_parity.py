@@ -260,6 +260,78 @@ def test_average_down_matches_oracle_bitwise():
 
 # ---- AMR with subcycling ---------------------------------------------------------------------------------
 
+# ---- truncation-error tags fused into the synchronisation (S8(f) NEXT-1) ----------------------------------
+
+def _tee_compare(o, s, level):
+    ot, oc = o.tee_tags(level)
+    gt, gc = s._tee[level]
+    s.synchronize()
+    for a, b in zip(ot, s.split_tags(level, gt)):
+        assert np.array_equal(a, b.cpu().numpy())
+    assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
+    return sum(int((a != 0).sum()) for a in ot)
+
+
+def test_tee_tags_at_explicit_average_down_match_oracle_bitwise():
+    """Same input state on both sides (independent smooth fields on the two levels, so that Delta is O(1e-2) and the
+    thresholds cut through its distribution): tags, 32^3 counts and the synchronised coarse state are bit-exact."""
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=2, lap_order=2, h0=1.0)
+    P.init_smooth(o, s, n0, seed=21)
+    eps = (0.004, 0.009)
+    o.tee_enable(1, *eps)
+    s.tee_enable(1, *eps)
+    o.average_down(1)
+    s.average_down(1)
+    ntag = _tee_compare(o, s, 1)
+    ncell = sum(int(np.prod(o.box_shape(ib))) for ib in o.level_boxes(1))
+    assert 0 < ntag < ncell
+    assert P.max_err(o, s) == 0.0
+    # second synchronisation: coarse already equals the mean -> Delta = 0, nothing tagged on either side
+    o.average_down(1)
+    s.average_down(1)
+    assert _tee_compare(o, s, 1) == 0
+
+
+def test_tee_tags_inside_rk_step_three_levels():
+    """TEE enabled on levels 1 and 2 of a ring hierarchy: after a coarse step the buffers hold the tags of each
+    level's LAST synchronisation.  Free-running states agree to <= 1e-11, so the comparison is restricted to cells
+    whose Delta is not within 1e-9 of the threshold: run both sides with eps*(1 -+ 1e-6) on the oracle and require
+    oracle(eps+) <= gpu(eps) <= oracle(eps-) cell by cell."""
+    P = _pair()
+    n0 = 32
+    rings, boxes, _ = _ring_hierarchy(n0)
+    kw = dict(boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.25, lam=1.0)
+    eps = 2e-4
+    runs = []
+    for scale in (1.0 + 1e-6, 1.0 - 1e-6):
+        o, s = P.make_pair(n0, **kw)
+        for ib, (l, lo, hi) in enumerate(boxes):
+            re, im = inputs.ring_field(rings, l, lo, hi)
+            P.set_both(o, s, ib, 0, re.numpy())
+            P.set_both(o, s, ib, 1, im.numpy())
+        for l in (1, 2):
+            o.tee_enable(l, eps * scale, eps * scale)
+            s.tee_enable(l, eps, eps)
+        o.rk_step(0.0625, 2.0)
+        s.rk_step(0.0625, 2.0)
+        s.synchronize()
+        assert P.max_err(o, s) <= F64_TOL
+        runs.append((o, s))
+    (o_hi, s), (o_lo, _) = runs
+    total = 0
+    for l in (1, 2):
+        t_hi, _ = o_hi.tee_tags(l)
+        t_lo, _ = o_lo.tee_tags(l)
+        g = [b.cpu().numpy() for b in s.split_tags(l, s._tee[l][0])]
+        for a, b, c in zip(t_hi, g, t_lo):
+            assert np.all((a & ~b) == 0) and np.all((b & ~c) == 0)
+            total += int((b != 0).sum())
+    assert total > 0
+
+
 @pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
 def test_two_level_subcycled_steps(flow):
     P = _pair()
