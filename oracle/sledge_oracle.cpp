@@ -8,9 +8,10 @@
 //
 // What it computes, and the passage each part follows (PAPER.md line / section):
 //   O1 grid        : block-structured levels, ratio 2, periodic domain          L23, L39-53 Eq.1-3
-//   O2 Laplacian   : utils::Laplacian<order>, order 1 -> 7-pt, 2 -> 13-pt       L207-212, L649 App.A
+//   O2 Laplacian   : utils::Laplacian<order>, order 1 -> 7-pt, 2 -> 13-pt,
+//                    3 -> 19-pt                                                  L207-212, L649 App.A
 //                    (coefficients are not printed; they are the unique maximal-order central
-//                    stencils on 3 / 5 points per axis -- pinned by polynomial exactness)
+//                    stencils on 3 / 5 / 7 points per axis -- pinned by polynomial exactness)
 //   O3 RHS         : Eq.10-11 with friction kappa, mass term a, coupling lambda  L178-181, L214-223
 //   O4 integrator  : classic RK4 (integrator.type = 4)                           L808 Table V
 //   O5 ghost fill  : periodic wrap, same-level copy, coarse->fine trilinear in
@@ -137,7 +138,7 @@ bool build(Oracle& o, const BoxIn* b, int nbox) {
   int bf = p.blocking_factor;
   if (bf < 1 || (bf & (bf - 1))) { o.err = "blocking_factor must be a power of 2 (L39)"; return false; }
   if (p.nghost >= bf) { o.err = "nghost must be smaller than blocking_factor (L772)"; return false; }
-  if (p.lap_order < 1 || p.lap_order > 2) { o.err = "lap_order must be 1 or 2"; return false; }
+  if (p.lap_order < 1 || p.lap_order > 3) { o.err = "lap_order must be 1, 2 or 3 (L649)"; return false; }
   if (p.lap_order > p.nghost) { o.err = "lap_order must be <= nghost (L240)"; return false; }
   if (!(p.h0 > 0)) { o.err = "h0 must be positive"; return false; }
   o.lev.resize(p.n_levels);
@@ -327,7 +328,14 @@ inline double laplacian(const Field& F, int c, int i, int j, int k, int order, d
   double n2z = (F.at(c, i, j, k + 2) - u) + (F.at(c, i, j, k - 2) - u);
   double s1 = (n1x + n1y) + n1z;
   double s2 = (n2x + n2y) + n2z;
-  return (16.0 * s1 - s2) / (12.0 * (h * h));
+  if (order == 2) return (16.0 * s1 - s2) / (12.0 * (h * h));
+  // order 3, 19-point (L649): per axis [2, -27, 270, -490, 270, -27, 2] / (180 h^2), the unique 6th-order central
+  // stencil on 7 points, in the same neighbour-minus-centre form
+  double n3x = (F.at(c, i + 3, j, k) - u) + (F.at(c, i - 3, j, k) - u);
+  double n3y = (F.at(c, i, j + 3, k) - u) + (F.at(c, i, j - 3, k) - u);
+  double n3z = (F.at(c, i, j, k + 3) - u) + (F.at(c, i, j, k - 3) - u);
+  double s3 = (n3x + n3y) + n3z;
+  return ((270.0 * s1 - 27.0 * s2) + 2.0 * s3) / (180.0 * (h * h));
 }
 
 // ---- O3: right-hand side, Eq.10-11 ------------------------------------------------------------

@@ -27,11 +27,11 @@ def coords(shape):
 # ------------------------------------------------------------------------------------------------
 
 
-@pytest.mark.parametrize("order,deg", [(1, 2), (1, 3), (2, 4), (2, 5)])
+@pytest.mark.parametrize("order,deg", [(1, 2), (1, 3), (2, 4), (2, 5), (3, 6), (3, 7)])
 def test_laplacian_exact_on_polynomials(order, deg):
-    """Central 3-point (5-point) second differences are exact on cubics (quintics) per axis.  Ghosts are
-    filled analytically on a NON-periodic box, so a wrong coefficient, sign or axis shows up directly."""
-    g = 2
+    """Central 3-point (5-, 7-point) second differences are exact on cubics (quintics, septics) per axis.  Ghosts
+    are filled analytically on a NON-periodic box, so a wrong coefficient, sign or axis shows up directly."""
+    g = 3 if order == 3 else 2
     n = (8, 16, 24)  # x, y, z -- all different to catch a transposed index
     h = 0.37
     o = Oracle(n, nghost=g, blocking_factor=8, lap_order=order, h0=h, lam=0.0)
@@ -72,14 +72,31 @@ def test_laplacian_order1_not_exact_on_quartic():
     assert np.allclose(err, 2 * h ** 2, rtol=1e-9)
 
 
-@pytest.mark.parametrize("order", [1, 2])
+def test_laplacian_order2_not_exact_on_sextic():
+    """The 5-point stencil must NOT be exact on x^6: its error is -(h^4/90) u^(6) = -8 h^4, which the 7-point stencil
+    of order 3 removes (separates the two on the same data)."""
+    g, n, h = 3, (8, 8, 8), 0.5
+    zz, yy, xx = np.meshgrid(*[(np.arange(-g, s + g) + 0.5) * h for s in n], indexing="ij")
+    v = slice(g, -g)
+    exact = 30 * xx[v, v, v] ** 4
+    res = {}
+    for order in (2, 3):
+        o = Oracle(n, nghost=g, lap_order=order, h0=h, lam=0.0)
+        o.set_raw(0, 0, xx ** 6)
+        res[order] = o.eval_rhs(0, 1.0, fill=False)[0][2] - exact
+    assert np.allclose(res[2], -8 * h ** 4, rtol=1e-8)
+    assert np.abs(res[3]).max() < 1e-9
+
+
+@pytest.mark.parametrize("order", [1, 2, 3])
 def test_laplacian_symbol_on_plane_waves(order):
     """exp(i k.x) is an eigenvector of the periodic discrete Laplacian with eigenvalue
-    -(1/h^2) sum_i 4 sin^2(k_i h/2)                               (order 1)
-    -(1/h^2) sum_i [16/3 sin^2(k_i h/2) - 1/3 sin^2(k_i h)]       (order 2)."""
+    -(1/h^2) sum_i 4 sin^2(k_i h/2)                                                   (order 1)
+    -(1/h^2) sum_i [16/3 sin^2(k_i h/2) - 1/3 sin^2(k_i h)]                           (order 2)
+    -(1/h^2) sum_i [6 sin^2(k_i h/2) - 3/5 sin^2(k_i h) + 2/45 sin^2(3 k_i h/2)]      (order 3)."""
     n = (16, 24, 32)
     h = 0.8
-    o = Oracle(n, nghost=2, lap_order=order, h0=h, lam=0.0)
+    o = Oracle(n, nghost=3, lap_order=order, h0=h, lam=0.0)
     x, y, z = coords(n[::-1])
     m = (3, 2, 5)  # mode numbers per axis
     kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
@@ -89,8 +106,10 @@ def test_laplacian_symbol_on_plane_waves(order):
     k = o.eval_rhs(0, 1.0)[0]
     if order == 1:
         ev = -sum(4 * math.sin(a / 2) ** 2 for a in kh) / h ** 2
-    else:
+    elif order == 2:
         ev = -sum(16 / 3 * math.sin(a / 2) ** 2 - 1 / 3 * math.sin(a) ** 2 for a in kh) / h ** 2
+    else:
+        ev = -sum(6 * math.sin(a / 2) ** 2 - 0.6 * math.sin(a) ** 2 + 2 / 45 * math.sin(1.5 * a) ** 2 for a in kh) / h ** 2
     assert np.abs(k[2] - ev * np.cos(ph)).max() < 1e-12 * abs(ev)
     assert np.abs(k[3] - ev * np.sin(ph)).max() < 1e-12 * abs(ev)
 
@@ -137,22 +156,24 @@ def test_constant_field_equals_scalar_ode(order, eta_fixed):
         assert abs(got.flat[0] - y[c]) <= 64 * np.finfo(float).eps * max(1.0, abs(y[c]))
 
 
-@pytest.mark.parametrize("order", [1, 2])
+@pytest.mark.parametrize("order", [1, 2, 3])
 def test_linear_plane_wave_matches_rk4_amplification_matrix(order):
     """lambda = 0: a lattice plane wave evolves by R(dt A)^n exactly, A = [[0,1],[-w^2,0]],
     R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24, w^2 = lattice symbol (BASELINE.json 'discrete-dispersion plane
     wave' for the 2nd-order stencil; the 13-point symbol for order 2)."""
     n = (16, 8, 24)
     h = 0.5
-    o = Oracle(n, nghost=2, lap_order=order, h0=h, lam=0.0)
+    o = Oracle(n, nghost=3, lap_order=order, h0=h, lam=0.0)
     x, y, z = coords(n[::-1])
     m = (1, 2, 3)
     kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
     ph = kh[0] * x + kh[1] * y + kh[2] * z
     if order == 1:
         w2 = sum(4 * math.sin(a / 2) ** 2 for a in kh) / h ** 2
-    else:
+    elif order == 2:
         w2 = sum(16 / 3 * math.sin(a / 2) ** 2 - 1 / 3 * math.sin(a) ** 2 for a in kh) / h ** 2
+    else:
+        w2 = sum(6 * math.sin(a / 2) ** 2 - 0.6 * math.sin(a) ** 2 + 2 / 45 * math.sin(1.5 * a) ** 2 for a in kh) / h ** 2
     A0, B0 = 0.7, -0.4  # psi1 = A cos, Pi1 = B cos ; psi2 = 2A sin, Pi2 = -B sin
     o.set_state(0, 0, A0 * np.cos(ph))
     o.set_state(0, 2, B0 * np.cos(ph))
