@@ -57,7 +57,7 @@ typedef struct {
   int32_t nghost;          /* ghost layers per box (L68-70, L772): lap_order <= nghost < blocking_factor */
   int32_t blocking_factor; /* power of 2 (L39, L771)                                              */
   int32_t dtype;           /* SLEDGE_F32 / SLEDGE_F64: storage AND arithmetic type                */
-  int32_t lap_order;       /* paper's `order` (L649): 1 = 7-point, 2 = 13-point Laplacian         */
+  int32_t lap_order;       /* paper's `order` (L649): 1 = 7-, 2 = 13-, 3 = 19-point Laplacian      */
   int32_t eta_fixed;       /* 1 = Minkowski test variant: eta_s = eta for every stage (R3)         */
   int32_t rk_dataflow;     /* words moved per cell-step (R5): SLEDGE_RK_FUSED 20 (two stages per sweep on
                               level 0, LEAN on finer levels), SLEDGE_RK_LEAN 52, SLEDGE_RK_CLASSIC 64   */

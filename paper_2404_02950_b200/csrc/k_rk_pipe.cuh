@@ -69,7 +69,7 @@ struct PipeArgs {
   int g, ox;
   int wrap;        // k_rk_plane only: the level is ONE box covering the periodic domain and the kernel wraps its halo /
                    // window addresses itself (L23), so no ghost fill is needed before the sweep
-  T inv_h2;        // 1/h^2 (order 1) or 1/(12 h^2) (order 2)
+  T inv_h2;        // 1/h^2 (order 1), 1/(12 h^2) (order 2) or 1/(180 h^2) (order 3)
   T lam_eta2[3];   // lambda * eta^2 at t, t + dt/2, t + dt (unfused: [0] = the stage's value)
   T fric[3];       // kappa / eta at the same times
   T a_mass;
@@ -98,7 +98,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
 // Laplacian of one component from its 6 (12) neighbours.  The library is compiled with --fmad=false (the tag
 // rule needs individually rounded products); K1 is where the fp64 pipe matters, so it contracts explicitly:
 // neighbour-sum form s_r = sum_d (u(+r e_d) + u(-r e_d)), then
-//   order 1: (s1 - 6u) / h^2            order 2: (16 s1 - s2 - 90u) / (12 h^2)
+//   order 1: (s1 - 6u) / h^2      order 2: (16 s1 - s2 - 90u) / (12 h^2)      order 3: (270 s1 - 27 s2 + 2 s3 - 1470u) / (180 h^2)
 // 13 fp64 instructions for the 13-point stencil instead of 25 in difference form.  The result differs from the
 // difference form sum_d [(u+ - u) + (u- - u)] by rounding only (|err| <~ 1e-15 / h^2 on O(1) fields; R11).
 template <typename T, int ORDER>
@@ -107,7 +107,10 @@ __device__ __forceinline__ T lap_from(T u, const T* xm, const T* xp, const T* ym
   const T s1 = ((xp[0] + xm[0]) + (yp[0] + ym[0])) + (zp[0] + zm[0]);
   if (ORDER == 1) return fma(T(-6), u, s1) * inv_h2;
   const T s2 = ((xp[1] + xm[1]) + (yp[1] + ym[1])) + (zp[1] + zm[1]);
-  return fma(T(16), s1, fma(T(-90), u, -s2)) * inv_h2;
+  if (ORDER == 2) return fma(T(16), s1, fma(T(-90), u, -s2)) * inv_h2;
+  // order 3, 19-point: (270 s1 - 27 s2 + 2 s3 - 1470 u) / (180 h^2)
+  const T s3 = ((xp[2] + xm[2]) + (yp[2] + ym[2])) + (zp[2] + zm[2]);
+  return fma(T(270), s1, fma(T(-27), s2, fma(T(2), s3, T(-1470) * u))) * inv_h2;
 }
 
 // k_Pi of one component (Eq.11 generalised, R2): lap - psi * pot - fric * pi, contracted
@@ -379,7 +382,7 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
 #pragma unroll
           for (int c = 0; c < 2; ++c) {
             auto comp = [c](const P& v) -> T { return c == 0 ? v.x : v.y; };
-            T xm[2], xp[2], ym[2], yp[2], zm[2], zp[2];
+            T xm[3], xp[3], ym[3], yp[3], zm[3], zp[3];
 #pragma unroll
             for (int r = 1; r <= R; ++r) {
               xm[r - 1] = comp(s[sc - r]);

@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_plane(const PipeArgs<T
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
               auto comp = [c](const P& v) -> T { return c == 0 ? v.x : v.y; };
-              T xm[2], xp[2], ym[2], yp[2], zm[2], zp[2];
+              T xm[3], xp[3], ym[3], yp[3], zm[3], zp[3];
 #pragma unroll
               for (int r = 1; r <= R; ++r) {
                 xm[r - 1] = comp(xn[2 * (r - 1) + 0]);

@@ -181,7 +181,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   const int bf = p.blocking_factor;
   if (bf < 2 || (bf & (bf - 1))) return fail(nullptr, SLEDGE_EINVAL, "blocking_factor must be a power of 2 >= 2 (L39)");
   if (p.nghost < 1 || p.nghost >= bf) return fail(nullptr, SLEDGE_EINVAL, "need 1 <= nghost < blocking_factor (L772)");
-  if (p.lap_order < 1 || p.lap_order > 2) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be 1 (7-point) or 2 (13-point)");
+  if (p.lap_order < 1 || p.lap_order > 3) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be 1 (7-point), 2 (13-point) or 3 (19-point) (L649)");
   if (p.lap_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be <= nghost (L240)");
   if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
   if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
@@ -459,11 +459,13 @@ cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   constexpr int TY = K1Shape<MODE>::TY;
   static bool configured = false;  // per instantiation
   if constexpr (K1Shape<MODE>::plane) {
-    constexpr int RY = (K1Shape<MODE>::fused && sizeof(T) == 4) ? SLEDGE_K1F_RY32 : K1Shape<MODE>::RY;
+    // the 7-plane z-window of the 19-point stencil leaves no registers for a second row
+    constexpr int RY = ORDER == 3 ? 1 : ((K1Shape<MODE>::fused && sizeof(T) == 4) ? SLEDGE_K1F_RY32 : K1Shape<MODE>::RY);
     constexpr int PD = plane_depth<T, ORDER, MODE, K1F_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
     using C = PlaneCfg<T, ORDER, MODE, K1F_TX, TY, PD, RY>;
     static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
-    auto kern = k_rk_plane<T, ORDER, MODE, K1F_TX, TY, PD, RY, K1Shape<MODE>::MINB>;
+    constexpr int MINB = ORDER == 3 ? 1 : K1Shape<MODE>::MINB;
+    auto kern = k_rk_plane<T, ORDER, MODE, K1F_TX, TY, PD, RY, MINB>;
     if (!configured) {
       const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
       if (e != cudaSuccess) return e;
@@ -508,13 +510,14 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   a.g = P.p.nghost;
   a.ox = P.ox;
   const double h2 = L.h * L.h;
-  a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : 1.0 / (12.0 * h2));
+  a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : (P.p.lap_order == 2 ? 1.0 / (12.0 * h2) : 1.0 / (180.0 * h2)));
   a.a_mass = (T)P.p.a_mass;
   const int grid = (int)(fused ? L.ftiles.size() : L.tiles.size());
   cudaError_t e;
   {
     Timed tm(c, KIND_STAGE);
-    e = P.p.lap_order == 1 ? launch_pipe_mode<T, 1>(c, a, grid, mode) : launch_pipe_mode<T, 2>(c, a, grid, mode);
+    e = P.p.lap_order == 1 ? launch_pipe_mode<T, 1>(c, a, grid, mode)
+        : (P.p.lap_order == 2 ? launch_pipe_mode<T, 2>(c, a, grid, mode) : launch_pipe_mode<T, 3>(c, a, grid, mode));
   }
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "k_rk_pipe: %s", cudaGetErrorString(e));
   return check_launch(c, "k_rk_pipe");

@@ -108,7 +108,7 @@ def _ragged_boxes():
     ]
 
 
-@pytest.mark.parametrize("order,g", [(1, 1), (1, 3), (2, 2), (2, 3)])
+@pytest.mark.parametrize("order,g", [(1, 1), (1, 3), (2, 2), (2, 3), (3, 3), (3, 5)])
 @pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
 def test_ragged_multibox_fp64(order, g, flow):
     P = _pair()
@@ -138,7 +138,7 @@ def _bf4_boxes():
     ]
 
 
-@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (2, 3)])
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (2, 3), (3, 3)])
 @pytest.mark.parametrize("flow", ["lean", "fused"])
 def test_ragged_blocking_factor_4(order, g, flow):
     P = _pair()
@@ -181,7 +181,7 @@ def test_eta_fixed_minkowski_variant():
     assert P.max_err(o, s) <= F64_TOL
 
 
-@pytest.mark.parametrize("order,g", [(1, 1), (2, 2)])
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (3, 3)])
 def test_fp32_relative_error(order, g):
     P = _pair()
     n = 64
@@ -333,11 +333,12 @@ def test_tee_tags_inside_rk_step_three_levels():
 
 
 @pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
-def test_two_level_subcycled_steps(flow):
+@pytest.mark.parametrize("order", [2, 3])
+def test_two_level_subcycled_steps(flow, order):
     P = _pair()
     n0 = 32
     boxes = P.two_level_boxes(n0)
-    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=3, lap_order=2, h0=0.5, rk_dataflow=flow)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=3, lap_order=order, h0=0.5, rk_dataflow=flow)
     P.init_smooth(o, s, n0, seed=9, comps=(0, 1))
     eta, dt = 2.0, 0.1
     for _ in range(3):
