@@ -40,6 +40,9 @@ class _Params(C.Structure):
         ("lam", C.c_double),
         ("a_mass", C.c_double),
         ("friction", C.c_double),
+        ("ko_strength", C.c_double * 4),
+        ("ko_order", C.c_int32),
+        ("pad_", C.c_int32),
     ]
 
 
@@ -99,7 +102,7 @@ class Oracle:
     """
 
     def __init__(self, n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, lap_order=1,
-                 h0=1.0, lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False):
+                 h0=1.0, lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, ko_order=0, ko_strength=0.0):
         if np.isscalar(n0):
             n0 = (int(n0),) * 3
         if boxes is None:
@@ -120,6 +123,9 @@ class Oracle:
         p.lam = lam
         p.a_mass = a_mass
         p.friction = friction
+        ks = (ko_strength,) * 4 if np.isscalar(ko_strength) else tuple(ko_strength)
+        p.ko_strength[:] = [float(v) for v in ks]
+        p.ko_order = ko_order
         arr = (_Box * len(self.boxes))()
         for q, (l, lo, hi) in enumerate(self.boxes):
             arr[q].level = l

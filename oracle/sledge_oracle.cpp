@@ -18,6 +18,7 @@
 //                    space + linear in time                                       L68-74
 //   O6 subcycling  : advance l, then l+1 twice, then synchronise                  L66-76, L88 Fig.2
 //   O7 average-down: coarse <- mean of 8 fine children                            L74, L88
+//   O10 KO term    : Kreiss-Oliger dissipation Q_l added to every component's RHS  L141-146 Eq.7
 //   O9 TEE tags    : |coarse - mean of children| > eps at synchronisation         L82-111 Eq.5-6, L373-380 Eq.12
 //   O8 string tags : plaquette winding number of (psi1,psi2) around 0; rule not printed in the
 //                    paper (L349-371 gives only the bool-per-cell hook) -> DESIGN.md reading R8
@@ -57,6 +58,9 @@ struct Params {
   double lambda;
   double a_mass;
   double friction;
+  double ko_strength[4];  // epsilon_KO of Eq.7 per component psi1, psi2, Pi1, Pi2 (L749-750; 0 = off)
+  int32_t ko_order;       // sim.dissipation_order = ghost cells the term needs (L751): 2 or 3
+  int32_t pad_;
 };
 
 struct BoxIn {
@@ -140,6 +144,11 @@ bool build(Oracle& o, const BoxIn* b, int nbox) {
   if (p.nghost >= bf) { o.err = "nghost must be smaller than blocking_factor (L772)"; return false; }
   if (p.lap_order < 1 || p.lap_order > 3) { o.err = "lap_order must be 1, 2 or 3 (L649)"; return false; }
   if (p.lap_order > p.nghost) { o.err = "lap_order must be <= nghost (L240)"; return false; }
+  const bool ko_on = p.ko_strength[0] != 0.0 || p.ko_strength[1] != 0.0 || p.ko_strength[2] != 0.0 || p.ko_strength[3] != 0.0;
+  for (int c = 0; c < 4; ++c)
+    if (!(p.ko_strength[c] >= 0.0)) { o.err = "dissipation strength must be >= 0 (L749)"; return false; }
+  if (ko_on && (p.ko_order < 2 || p.ko_order > 3)) { o.err = "dissipation order must be 2 or 3 (L751)"; return false; }
+  if (ko_on && p.ko_order > p.nghost) { o.err = "dissipation order must be <= nghost (L751)"; return false; }
   if (!(p.h0 > 0)) { o.err = "h0 must be positive"; return false; }
   o.lev.resize(p.n_levels);
   for (int l = 0; l < p.n_levels; ++l) {
@@ -338,6 +347,31 @@ inline double laplacian(const Field& F, int c, int i, int j, int k, int order, d
   return ((270.0 * s1 - 27.0 * s2) + 2.0 * s3) / (180.0 * (h * h));
 }
 
+// ---- O10: Kreiss-Oliger dissipation, Eq.7 (L141-146, L749-751) ---------------------------------
+// sim.dissipation_order r in {2, 3} is "the number of ghost cells needed" (L751); Eq.7's p is then 2r - 1 (its
+// (p+1)-st derivative is the 2r-th one, and (-1)^((p+3)/2) = (-1)^(r+1) is real only for odd p):
+//   Q u = (-1)^(r+1) eps h^(2r-1) / 2^(2r) * sum_d d^(2r)u/dx_d^(2r),
+// with the 2r-th derivative as the (2r+1)-point central difference delta^(2r) u / h^(2r):
+//   r = 2: [1, -4, 6, -4, 1]        r = 3: [1, -6, 15, -20, 15, -6, 1]      (binomial coefficients, alternating)
+// so Q u = (-1)^(r+1) eps / (2^(2r) h) * sum_d delta_d^(2r) u.  On a plane wave its eigenvalue is
+// -(eps/h) sum_d sin^(2r)(k_d h / 2) <= 0.  It is added to the evolution of EVERY component, momenta included
+// (L146 "each scalar field component"; the listing's Scalar::Pi1, L202, and Table I "for all field components",
+// L749-750, make Pi1, Pi2 members of that set), each with its own strength (R22).
+inline double ko_term(const Field& F, int c, int i, int j, int k, int r, double eps, double h) {
+  static const double C2[5] = {1, -4, 6, -4, 1};
+  static const double C3[7] = {1, -6, 15, -20, 15, -6, 1};
+  const double* co = (r == 2) ? C2 : C3;
+  double sum = 0.0;
+  for (int d = 0; d < 3; ++d) {
+    double dd = 0.0;
+    for (int m = -r; m <= r; ++m)
+      dd += co[m + r] * F.at(c, i + (d == 0 ? m : 0), j + (d == 1 ? m : 0), k + (d == 2 ? m : 0));
+    sum += dd;
+  }
+  double sign = (r % 2 == 0) ? -1.0 : 1.0;  // (-1)^(r+1)
+  return sign * eps / (std::pow(2.0, 2 * r) * h) * sum;
+}
+
 // ---- O3: right-hand side, Eq.10-11 ------------------------------------------------------------
 //   k_psi_c = Pi_c
 //   k_Pi_c  = -(kappa/eta) Pi_c + Lap(psi_c) - lambda eta^2 psi_c (psi1^2 + psi2^2 - 1) - a psi_c
@@ -361,6 +395,8 @@ void eval_rhs(const Oracle& o, int l, const LevelState& S, LevelState& K, double
           R.at(PSI2, i, j, k) = pi2;
           R.at(PI1, i, j, k) = (lap1 - psi1 * pot) - fr * pi1;
           R.at(PI2, i, j, k) = (lap2 - psi2 * pot) - fr * pi2;
+          for (int c = 0; c < NCOMP; ++c)  // Eq.7: Q_l u_c added to the evolution of every component
+            if (p.ko_strength[c] != 0.0) R.at(c, i, j, k) += ko_term(F, c, i, j, k, p.ko_order, p.ko_strength[c], L.h);
         }
   }
 }
@@ -563,6 +599,9 @@ typedef struct {
   int32_t lap_order;
   int32_t eta_fixed;
   double h0, lambda, a_mass, friction;
+  double ko_strength[4];
+  int32_t ko_order;
+  int32_t pad_;
 } orc_params;
 
 typedef struct {

@@ -115,6 +115,137 @@ def test_laplacian_symbol_on_plane_waves(order):
 
 
 # ------------------------------------------------------------------------------------------------
+# O10 Kreiss-Oliger dissipation (Eq.7; dissipation_order r in {2,3} = ghost cells, p = 2r - 1, L751)
+# ------------------------------------------------------------------------------------------------
+
+KO_EPS = (0.013, 0.021, 0.034, 0.055)  # all different: a swapped component index shows up
+
+
+@pytest.mark.parametrize("r", [2, 3])
+def test_ko_annihilates_low_degree_and_is_exact_on_the_leading_monomial(r):
+    """Eq.7 applied to a monomial, by hand: Q x^m = 0 for m <= 2r - 1 = p, and for u = (x/h)^(2r) the (p+1)-st
+    derivative is (2r)!/h^(2r), so Q u = (-1)^((p+3)/2) eps h^p / 2^(p+1) * (2r)!/h^(2r)
+    = -1.5 eps/h (r = 2) and +11.25 eps/h (r = 3), the same for every cell.  The (2r+1)-point central difference is
+    exact on both, so sign, normalisation, power of h and the axis sum are all pinned; ghosts are analytic on a
+    non-periodic box; lambda = 0 and Laplacian<1> of the same data is subtracted analytically."""
+    g, n, h = r, (8, 16, 24), 0.37
+    o = Oracle(n, nghost=g, lap_order=1, h0=h, lam=0.0, ko_order=r, ko_strength=KO_EPS)
+    kk, jj, ii = np.meshgrid(*[np.arange(-g, s + g, dtype=np.float64) for s in n[::-1]], indexing="ij")
+    v = slice(g, -g)
+    # degree <= p per axis (plus a cross term): Q vanishes on every component
+    rng = np.random.default_rng(3)
+    co = rng.uniform(-1, 1, size=(4, 3, 2 * r))
+    lowdeg = [sum(co[c, 0, m] * (ii / 8) ** m + co[c, 1, m] * (jj / 8) ** m + co[c, 2, m] * (kk / 8) ** m
+                  for m in range(2 * r)) + 0.1 * (ii * jj * kk) / 512 for c in range(4)]
+    for c in range(4):
+        o.set_raw(0, c, lowdeg[c])
+    k = o.eval_rhs(0, eta=1.0, fill=False)[0]
+    assert np.abs(k[0] - lowdeg[2][v, v, v]).max() < 1e-12  # k_psi = Pi + 0
+    assert np.abs(k[1] - lowdeg[3][v, v, v]).max() < 1e-12
+    # leading monomials: psi1 = i^(2r), psi2 = j^(2r) + 2 k^(2r), Pi1 = k^(2r), Pi2 = -i^(2r)
+    lead = math.factorial(2 * r) / 2 ** (2 * r) / h * (-1 if r == 2 else 1)
+    assert lead == (-1.5 / h if r == 2 else 11.25 / h)
+    u = [ii ** (2 * r), jj ** (2 * r) + 2 * kk ** (2 * r), kk ** (2 * r), -(ii ** (2 * r))]
+    for c in range(4):
+        o.set_raw(0, c, u[c])
+    k = o.eval_rhs(0, eta=1.0, fill=False)[0]
+    want = [KO_EPS[0] * lead, KO_EPS[1] * 3 * lead, KO_EPS[2] * lead, -KO_EPS[3] * lead]
+    scale = float(max(n) + g) ** (2 * r)
+    assert np.abs(k[0] - (u[2][v, v, v] + want[0])).max() < 1e-13 * scale
+    assert np.abs(k[1] - (u[3][v, v, v] + want[1])).max() < 1e-13 * scale
+    # k_Pi = Lap<1> psi + Q Pi; second difference of i^(2r) along x, analytic
+    d2 = lambda t: ((t + 1) ** (2 * r) - 2 * t ** (2 * r) + (t - 1) ** (2 * r)) / h ** 2
+    lap1 = d2(ii)
+    lap2 = d2(jj) + 2 * d2(kk)
+    assert np.abs(k[2] - (lap1[v, v, v] + want[2])).max() < 1e-13 * scale / h ** 2
+    assert np.abs(k[3] - (lap2[v, v, v] + want[3])).max() < 1e-13 * scale / h ** 2
+
+
+def ko_symbol(r, eps, kh, h):
+    """Eq.7 on exp(i k.x) with the derivative as the (2r+1)-point central difference delta^(2r) = (-4 sin^2(kh/2))^r:
+    eigenvalue -(eps/h) sum_d sin^(2r)(k_d h/2), never positive: the term only damps."""
+    return -(eps / h) * sum(math.sin(a / 2) ** (2 * r) for a in kh)
+
+
+@pytest.mark.parametrize("r", [2, 3])
+def test_ko_symbol_on_plane_waves(r):
+    n, h = (16, 24, 32), 0.8
+    o = Oracle(n, nghost=3, lap_order=2, h0=h, lam=0.0, ko_order=r, ko_strength=KO_EPS)
+    x, y, z = coords(n[::-1])
+    m = (3, 2, 5)
+    kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
+    ph = kh[0] * x + kh[1] * y + kh[2] * z
+    amp = (1.0, 0.6, -0.4, 0.9)
+    wave = [np.cos(ph), np.sin(ph), np.cos(ph), np.sin(ph)]
+    for c in range(4):
+        o.set_state(0, c, amp[c] * wave[c])
+    k = o.eval_rhs(0, 1.0)[0]
+    lap = -sum(16 / 3 * math.sin(a / 2) ** 2 - 1 / 3 * math.sin(a) ** 2 for a in kh) / h ** 2
+    q = [ko_symbol(r, KO_EPS[c], kh, h) for c in range(4)]
+    for c in range(2):
+        assert np.abs(k[c] - (amp[c + 2] + q[c] * amp[c]) * wave[c]).max() < 1e-14
+        assert np.abs(k[c + 2] - (lap * amp[c] + q[c + 2] * amp[c + 2]) * wave[c]).max() < 1e-13 * abs(lap)
+    # the Nyquist checkerboard is damped at the largest rate, -3 eps/h
+    cb = (-1.0) ** (x + y + z)
+    o.set_state(0, 0, cb)
+    o.set_state(0, 2, 0 * cb)
+    k = o.eval_rhs(0, 1.0)[0]
+    assert np.abs(k[0] + 3 * KO_EPS[0] / h * cb).max() < 1e-14
+
+
+@pytest.mark.parametrize("r", [2, 3])
+def test_ko_inside_rk4_matches_the_damped_amplification_matrix(r):
+    """lambda = 0 with dissipation: a plane wave evolves by R(dt A)^n with A = [[q_psi, 1], [-w^2, q_Pi]]: the term
+    is evaluated at every stage state, on psi and Pi, with the level's h."""
+    n, h = (16, 8, 24), 0.5
+    eps = (0.2, 0.3, 0.5, 0.7)  # large on purpose: the damping is far above the 1e-13 tolerance
+    o = Oracle(n, nghost=3, lap_order=1, h0=h, lam=0.0, ko_order=r, ko_strength=eps)
+    x, y, z = coords(n[::-1])
+    m = (1, 2, 3)
+    kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
+    ph = kh[0] * x + kh[1] * y + kh[2] * z
+    w2 = sum(4 * math.sin(a / 2) ** 2 for a in kh) / h ** 2
+    A0, B0 = 0.7, -0.4
+    o.set_state(0, 0, A0 * np.cos(ph))
+    o.set_state(0, 2, B0 * np.cos(ph))
+    o.set_state(0, 1, 2 * A0 * np.sin(ph))
+    o.set_state(0, 3, -B0 * np.sin(ph))
+    dt, steps = 0.2 * h, 25
+    eta = 3.0
+    for _ in range(steps):
+        o.rk_step(dt, eta)
+        eta += dt
+    out = []
+    for c in range(2):
+        Z = dt * np.array([[ko_symbol(r, eps[c], kh, h), 1.0], [-w2, ko_symbol(r, eps[c + 2], kh, h)]])
+        R = np.eye(2) + Z + Z @ Z / 2 + Z @ Z @ Z / 6 + Z @ Z @ Z @ Z / 24
+        out.append(np.linalg.matrix_power(R, steps) @ (np.array([A0, B0]) if c == 0 else np.array([2 * A0, -B0])))
+    assert np.abs(o.get_state(0, 0) - out[0][0] * np.cos(ph)).max() < 1e-13
+    assert np.abs(o.get_state(0, 2) - out[0][1] * np.cos(ph)).max() < 1e-12
+    assert np.abs(o.get_state(0, 1) - out[1][0] * np.sin(ph)).max() < 1e-13
+    assert np.abs(o.get_state(0, 3) - out[1][1] * np.sin(ph)).max() < 1e-12
+    # and the damping is really there: without the term the same run differs by far more than the tolerance
+    o2 = Oracle(n, nghost=3, lap_order=1, h0=h, lam=0.0)
+    o2.set_state(0, 0, A0 * np.cos(ph))
+    o2.set_state(0, 2, B0 * np.cos(ph))
+    eta = 3.0
+    for _ in range(steps):
+        o2.rk_step(dt, eta)
+        eta += dt
+    assert np.abs(o2.get_state(0, 0) - o.get_state(0, 0)).max() > 1e-3
+
+
+def test_ko_validation_and_off_switch():
+    with pytest.raises(OracleError):
+        Oracle(16, nghost=2, lap_order=1, ko_order=3, ko_strength=0.01)  # needs 3 ghost cells (L751)
+    with pytest.raises(OracleError):
+        Oracle(16, nghost=3, lap_order=1, ko_order=1, ko_strength=0.01)  # order is 2 or 3 (L751)
+    with pytest.raises(OracleError):
+        Oracle(16, nghost=3, lap_order=1, ko_order=2, ko_strength=-0.01)
+    Oracle(16, nghost=1, lap_order=1, ko_order=0, ko_strength=0.0)  # strength 0 removes the term (L749)
+
+
+# ------------------------------------------------------------------------------------------------
 # O3 + O4: potential, friction, eta handling and the RK4 tableau against a textbook scalar ODE solve
 # ------------------------------------------------------------------------------------------------
 
@@ -534,17 +665,19 @@ def test_tee_inside_rk_step_shrinks_with_resolution():
 # ------------------------------------------------------------------------------------------------
 
 
-@pytest.mark.parametrize("order,g", [(1, 1), (2, 2)])
-def test_fully_covered_level1_equals_uniform_fine_run(order, g):
+@pytest.mark.parametrize("order,g,ko", [(1, 1, 0), (2, 2, 0), (1, 2, 2), (2, 3, 3)])
+def test_fully_covered_level1_equals_uniform_fine_run(order, g, ko):
     """A hierarchy whose level 1 covers 100 % of the domain never interpolates: level 1 must reproduce the
-    single-level 2N run with dt/2 bit-for-bit, and level 0 must equal its average."""
+    single-level 2N run with dt/2 bit-for-bit, and level 0 must equal its average.  With Kreiss-Oliger dissipation
+    on (ko = dissipation order) this also pins that Q_l uses the level's own spacing (Eq.7: Delta x_l)."""
+    kw = dict(ko_order=ko, ko_strength=(0.02, 0.03, 0.05, 0.07)) if ko else {}
     n0, h0, dt, eta0 = 8, 1.0, 0.25, 1.0  # binary fractions: both runs see identical stage times
     nf = 2 * n0
     psi = [inputs.grf(nf, 0.5, s).numpy() for s in (41, 42)]
     pi = [0.1 * inputs.grf(nf, 0.5, s).numpy() for s in (43, 44)]
-    ref = run_single(nf, None, psi, pi, 4, dt / 2, eta0, nghost=g, lap_order=order, h0=h0 / 2, lam=1.0)
+    ref = run_single(nf, None, psi, pi, 4, dt / 2, eta0, nghost=g, lap_order=order, h0=h0 / 2, lam=1.0, **kw)
     boxes = [(0, (0, 0, 0), (n0 - 1,) * 3), (1, (0, 0, 0), (nf - 1,) * 3)]
-    o = Oracle(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=order, h0=h0, lam=1.0)
+    o = Oracle(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=order, h0=h0, lam=1.0, **kw)
     for c, a in enumerate(psi + pi):
         o.set_state(1, c, a)
     o.average_down(1)
