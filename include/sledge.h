@@ -65,6 +65,14 @@ typedef struct {
   double lambda;           /* Eq.11 generalised (R2): k_Pi = -(friction/eta) Pi + Lap psi          */
   double a_mass;           /*        - lambda eta^2 psi (psi1^2+psi2^2-1) - a_mass psi             */
   double friction;         /* paper: 2 (Eq.11); BASELINE.json configs: 0                          */
+  double ko_strength[4];   /* Kreiss-Oliger dissipation (Eq.7): epsilon_KO >= 0 of psi1, psi2, Pi1, Pi2
+                              (sim.dissipation_strength[_$ScalarField], L749-750); all 0 = term removed.
+                              Q_l u = (-1)^(r+1) eps h_l^(2r-1) / 2^(2r) * sum_d d^(2r)u/dx_d^(2r) is added to the
+                              RHS of every component, the derivative as the (2r+1)-point central difference.
+                              With the term on, every level runs the staged LEAN / CLASSIC sweeps (FUSED needs
+                              k_psi = Pi pointwise) and the stage fills move Pi ghosts as well.          */
+  int32_t ko_order;        /* r = sim.dissipation_order in {2,3} = ghost cells the term needs (L751): r <= nghost */
+  int32_t reserved_;       /* 0 */
 } sledge_params;
 
 /* Size of the device arena needed for this hierarchy.  Host-only: validates params and boxes

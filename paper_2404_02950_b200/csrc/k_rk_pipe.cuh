@@ -75,6 +75,8 @@ struct PipeArgs {
   T a_mass;
   T adt;           // unfused: a_s * dt (S1-S3) or dt/6 (S4);  fused: dt
   T bdt;           // classic: b_s * dt for the accumulator
+  T ko_c[4];       // Kreiss-Oliger (Eq.7): (-1)^(r+1) eps_c / (2^(2r) h) for psi1, psi2, Pi1, Pi2; staged sweeps with
+                   // KO != 0 only, where sten[1] = Pi(U) takes the place of pnt[0]
 };
 
 __device__ __forceinline__ void cp_async_16(void* smem, const void* gmem) {
@@ -113,6 +115,19 @@ __device__ __forceinline__ T lap_from(T u, const T* xm, const T* xp, const T* ym
   return fma(T(270), s1, fma(T(-27), s2, fma(T(2), s3, T(-1470) * u))) * inv_h2;
 }
 
+// Kreiss-Oliger term of one component (Eq.7, dissipation order r = KO in {2, 3}, p = 2r - 1): the 2r-th
+// central differences along x, y, z in neighbour-sum form, s_m as in lap_from:
+//   r = 2: s2 - 4 s1 + 18 u        r = 3: s3 - 6 s2 + 15 s1 - 60 u        times coef = (-1)^(r+1) eps / (2^(2r) h)
+template <typename T, int KO>
+__device__ __forceinline__ T ko_from(T u, const T* xm, const T* xp, const T* ym, const T* yp, const T* zm,
+                                     const T* zp, T coef) {
+  const T s1 = ((xp[0] + xm[0]) + (yp[0] + ym[0])) + (zp[0] + zm[0]);
+  const T s2 = ((xp[1] + xm[1]) + (yp[1] + ym[1])) + (zp[1] + zm[1]);
+  if (KO == 2) return fma(T(-4), s1, fma(T(18), u, s2)) * coef;
+  const T s3 = ((xp[2] + xm[2]) + (yp[2] + ym[2])) + (zp[2] + zm[2]);
+  return fma(T(15), s1, fma(T(-6), s2, fma(T(-60), u, s3))) * coef;
+}
+
 // k_Pi of one component (Eq.11 generalised, R2): lap - psi * pot - fric * pi, contracted
 template <typename T>
 __device__ __forceinline__ T kpi_of(T lap, T psi, T pot, T fric, T pi) {
@@ -126,13 +141,16 @@ __device__ __forceinline__ T pot_of(T lam_eta2, T a_mass, T p1, T p2) {
 
 // One cell of one sweep: from the Laplacians lap[f][c] of the differenced fields, their centre values wc[f] and
 // the pointwise inputs pc[q], the new state(s) opsi[q], opi[q] of the mode's data-flow (see the header).
-template <typename T, int MODE>
+// With HASKO (staged modes only) ko[c] = Q_l u_c of Eq.7 is added to the RHS of every component.
+template <typename T, int MODE, bool HASKO = false>
 __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[ModeInfo<MODE>::NF][2],
                                         const typename PairOf<T>::type (&wc)[ModeInfo<MODE>::NF],
                                         const typename PairOf<T>::type (&pc)[ModeInfo<MODE>::NP > 0 ? ModeInfo<MODE>::NP : 1],
                                         typename PairOf<T>::type (&opsi)[ModeInfo<MODE>::NOUT],
-                                        typename PairOf<T>::type (&opi)[ModeInfo<MODE>::NOUT]) {
+                                        typename PairOf<T>::type (&opi)[ModeInfo<MODE>::NOUT],
+                                        const T* ko = nullptr) {
   using P = typename PairOf<T>::type;
+  static_assert(!HASKO || (MODE != FUSED_A && MODE != FUSED_B), "the fused sweeps rely on k_psi = Pi being pointwise");
   constexpr int NP = ModeInfo<MODE>::NP, NOUT = ModeInfo<MODE>::NOUT;
   constexpr int NPA = NP > 0 ? NP : 1;
   if (MODE == FUSED_A) {
@@ -178,9 +196,15 @@ __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[Mod
     const T psi1 = wc[0].x, psi2 = wc[0].y;
     const T pi1 = pc[0].x, pi2 = pc[0].y;
     const T pot = pot_of(a.lam_eta2[0], a.a_mass, psi1, psi2);
-    const T kpsi1 = pi1, kpsi2 = pi2;
-    const T kpi1 = kpi_of(lap[0][0], psi1, pot, a.fric[0], pi1);
-    const T kpi2 = kpi_of(lap[0][1], psi2, pot, a.fric[0], pi2);
+    T kpsi1 = pi1, kpsi2 = pi2;
+    T kpi1 = kpi_of(lap[0][0], psi1, pot, a.fric[0], pi1);
+    T kpi2 = kpi_of(lap[0][1], psi2, pot, a.fric[0], pi2);
+    if (HASKO) {
+      kpsi1 += ko[0];
+      kpsi2 += ko[1];
+      kpi1 += ko[2];
+      kpi2 += ko[3];
+    }
     // pointwise inputs: in_psi(q) = pv[1 + 2q], in_pi(q) = pv[2 + 2q]
     auto ipsi = [&](int q) -> const P& { return pc[(1 + 2 * q) < NPA ? (1 + 2 * q) : 0]; };
     auto ipi = [&](int q) -> const P& { return pc[(2 + 2 * q) < NPA ? (2 + 2 * q) : 0]; };
@@ -217,9 +241,11 @@ __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[Mod
   }
 }
 
-template <typename T, int ORDER, int MODE, int TX, int TY, int D>
+// KO = 0, or the Kreiss-Oliger dissipation order (2, 3): the window radius is the larger of the two stencils, and
+// Pi(U) becomes a second differenced field (it takes the ring slot that pnt[0] had).
+template <typename T, int ORDER, int MODE, int TX, int TY, int D, int KO = 0>
 struct PipeCfg {
-  static constexpr int R = ORDER;
+  static constexpr int R = ORDER > KO ? ORDER : KO;
   static constexpr int CPT = Vec16<T>::CPT;
   static constexpr int TXC = TX * CPT;
   static constexpr int SW = TXC + 2 * R;
@@ -227,38 +253,41 @@ struct PipeCfg {
   static constexpr int NT = TX * TY;
   static constexpr int NH = 2 * R * (TXC + TY);  // halo pairs per plane (star stencil: no corners)
   static constexpr int HPT = (NH + NT - 1) / NT;
-  static constexpr int NF = ModeInfo<MODE>::NF;
+  static constexpr int P0 = KO ? 1 : 0;  // first pointwise input that is still streamed
+  static constexpr int NF = ModeInfo<MODE>::NF + P0;
   static constexpr int NP = ModeInfo<MODE>::NP;
   static constexpr int NOUT = ModeInfo<MODE>::NOUT;
+  static constexpr int NOWN = NF + NP - P0;  // ring slots per stage and thread
   static constexpr size_t PAIR = 2 * sizeof(T);
-  static constexpr size_t OWN_BYTES = (size_t)D * (NF + NP) * NT * 16;
+  static constexpr size_t OWN_BYTES = (size_t)D * NOWN * NT * 16;
   static constexpr size_t HALO_BYTES = (size_t)D * NF * NH * PAIR;  // ring slot = NH pairs per field
   static constexpr size_t CTR_BYTES = (size_t)2 * NF * SH * SW * PAIR;
   static constexpr size_t SMEM_BYTES = OWN_BYTES + HALO_BYTES + CTR_BYTES;
 };
 
 // Deepest ring (<= dmax stages, >= 2) whose shared memory fits `budget` bytes.
-template <typename T, int ORDER, int MODE, int TX, int TY>
+template <typename T, int ORDER, int MODE, int TX, int TY, int KO = 0>
 constexpr int pipe_depth(size_t budget, int dmax) {
   int d = 2;
-  if (dmax >= 3 && PipeCfg<T, ORDER, MODE, TX, TY, 3>::SMEM_BYTES <= budget) d = 3;
-  if (dmax >= 4 && PipeCfg<T, ORDER, MODE, TX, TY, 4>::SMEM_BYTES <= budget) d = 4;
-  if (dmax >= 5 && PipeCfg<T, ORDER, MODE, TX, TY, 5>::SMEM_BYTES <= budget) d = 5;
-  if (dmax >= 6 && PipeCfg<T, ORDER, MODE, TX, TY, 6>::SMEM_BYTES <= budget) d = 6;
+  if (dmax >= 3 && PipeCfg<T, ORDER, MODE, TX, TY, 3, KO>::SMEM_BYTES <= budget) d = 3;
+  if (dmax >= 4 && PipeCfg<T, ORDER, MODE, TX, TY, 4, KO>::SMEM_BYTES <= budget) d = 4;
+  if (dmax >= 5 && PipeCfg<T, ORDER, MODE, TX, TY, 5, KO>::SMEM_BYTES <= budget) d = 5;
+  if (dmax >= 6 && PipeCfg<T, ORDER, MODE, TX, TY, 6, KO>::SMEM_BYTES <= budget) d = 6;
   return d;
 }
 
-template <typename T, int ORDER, int MODE, int TX, int TY, int D>
+template <typename T, int ORDER, int MODE, int TX, int TY, int D, int KO = 0>
 __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
   using P = typename PairOf<T>::type;
   using V = Vec16<T>;
-  using C = PipeCfg<T, ORDER, MODE, TX, TY, D>;
+  using C = PipeCfg<T, ORDER, MODE, TX, TY, D, KO>;
   constexpr int R = C::R, CPT = C::CPT, TXC = C::TXC, SW = C::SW, SH = C::SH, NT = C::NT, NH = C::NH, HPT = C::HPT;
-  constexpr int NF = C::NF, NP = C::NP, NOUT = C::NOUT;
+  constexpr int NF = C::NF, NP = C::NP, NOUT = C::NOUT, P0 = C::P0, NOWN = C::NOWN;
+  constexpr int NFM = ModeInfo<MODE>::NF;  // fields the Laplacian is taken of
   constexpr int NPA = NP > 0 ? NP : 1;
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  V* const own = reinterpret_cast<V*>(smem_raw);                             // [D][NF + NP][NT]
+  V* const own = reinterpret_cast<V*>(smem_raw);                             // [D][NOWN][NT]
   P* const halo = reinterpret_cast<P*>(smem_raw + C::OWN_BYTES);             // [D][NF][NH]
   P* const ctr = reinterpret_cast<P*>(smem_raw + C::OWN_BYTES + C::HALO_BYTES);  // [2][NF][SH * SW]
 
@@ -305,7 +334,7 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
   // differenced fields, pointwise inputs of plane z0+st, x/y halo of plane z0+st
   auto issue = [&](int st) {
     const int slot = st % D;
-    V* const o = own + (size_t)slot * (NF + NP) * NT + tid;
+    V* const o = own + (size_t)slot * NOWN * NT + tid;
     const long long po = off + (long long)st * plane;  // `off` is never advanced (see below)
     if (loader) {
 #pragma unroll
@@ -313,7 +342,7 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
     }
     if (active) {
 #pragma unroll
-      for (int q = 0; q < NP; ++q) cp_async_16(o + (NF + q) * NT, a.pnt[q] + po);
+      for (int q = P0; q < NP; ++q) cp_async_16(o + (NF + q - P0) * NT, a.pnt[q] + po);
     }
     const long long ho = tile_org + (long long)st * plane;
 #pragma unroll
@@ -342,7 +371,7 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
     const int slot = zz % D;
     P* const cb = ctr + (size_t)(zz & 1) * NF * SH * SW;
     cp_async_wait<D - 1>();  // this thread's copies of stage zz have landed (only this thread reads them)
-    const V* const o = own + (size_t)slot * (NF + NP) * NT + tid;
+    const V* const o = own + (size_t)slot * NOWN * NT + tid;
     V pv[NPA];
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
@@ -356,7 +385,8 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
     }
     if (active) {
 #pragma unroll
-      for (int q = 0; q < NP; ++q) pv[q] = o[(NF + q) * NT];
+      for (int q = P0; q < NP; ++q) pv[q] = o[(NF + q - P0) * NT];
+      if (KO) pv[0] = w[NF - 1][R];  // Pi(U) of this plane comes from its own z-window
     }
 #pragma unroll
     for (int q = 0; q < HPT; ++q)
@@ -375,7 +405,8 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
 #pragma unroll
       for (int p = 0; p < CPT; ++p) {
         const int sc = s_own + p;
-        T lap[NF][2];
+        T lap[NFM][2];
+        T ko[4] = {T(0), T(0), T(0), T(0)};
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
           const P* const s = cb + f * SH * SW;
@@ -392,15 +423,16 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
               zm[r - 1] = comp(w[f][R - r].p[p]);
               zp[r - 1] = comp(w[f][R + r].p[p]);
             }
-            lap[f][c] = lap_from<T, ORDER>(comp(w[f][R].p[p]), xm, xp, ym, yp, zm, zp, a.inv_h2);
+            if (f < NFM) lap[f < NFM ? f : 0][c] = lap_from<T, ORDER>(comp(w[f][R].p[p]), xm, xp, ym, yp, zm, zp, a.inv_h2);
+            if (KO) ko[2 * f + c] = ko_from<T, KO ? KO : 2>(comp(w[f][R].p[p]), xm, xp, ym, yp, zm, zp, a.ko_c[2 * f + c]);
           }
         }
-        P wc[NF], pc[NPA], opsi[NOUT], opi[NOUT];
+        P wc[NFM], pc[NPA], opsi[NOUT], opi[NOUT];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) wc[f] = w[f][R].p[p];
+        for (int f = 0; f < NFM; ++f) wc[f] = w[f][R].p[p];
 #pragma unroll
         for (int q = 0; q < NPA; ++q) pc[q] = pv[q].p[p];
-        rk_cell<T, MODE>(a, lap, wc, pc, opsi, opi);
+        rk_cell<T, MODE, KO != 0>(a, lap, wc, pc, opsi, opi, ko);
 #pragma unroll
         for (int q = 0; q < NOUT; ++q) {
           o_psi[q].p[p] = opsi[q];

@@ -154,6 +154,12 @@ struct sledge_ctx {
 
 namespace {
 
+// Kreiss-Oliger dissipation (Eq.7) is on when any component has a non-zero strength (L749)
+inline bool ko_on(const sledge_params& p) {
+  return p.ko_strength[0] != 0.0 || p.ko_strength[1] != 0.0 || p.ko_strength[2] != 0.0 || p.ko_strength[3] != 0.0;
+}
+inline int stencil_radius(const sledge_params& p) { return ko_on(p) && p.ko_order > p.lap_order ? p.ko_order : p.lap_order; }
+
 int fail(sledge_ctx* ctx, int code, const char* fmt, ...) {
   char buf[512];
   va_list ap;
@@ -183,6 +189,12 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   if (p.nghost < 1 || p.nghost >= bf) return fail(nullptr, SLEDGE_EINVAL, "need 1 <= nghost < blocking_factor (L772)");
   if (p.lap_order < 1 || p.lap_order > 3) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be 1 (7-point), 2 (13-point) or 3 (19-point) (L649)");
   if (p.lap_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "lap_order must be <= nghost (L240)");
+  for (int q = 0; q < 4; ++q)
+    if (!(p.ko_strength[q] >= 0.0)) return fail(nullptr, SLEDGE_EINVAL, "dissipation strength must be >= 0 (L749)");
+  if (ko_on(p)) {
+    if (p.ko_order < 2 || p.ko_order > 3) return fail(nullptr, SLEDGE_EINVAL, "dissipation order must be 2 or 3 (L751)");
+    if (p.ko_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "dissipation order must be <= nghost (L751)");
+  }
   if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
   if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
   if (!(p.h0 > 0)) return fail(nullptr, SLEDGE_EINVAL, "h0 must be positive");
@@ -405,7 +417,7 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.err_flag = tab<int>(c, P.off_err);
   a.list = tab<GhostEntry>(c, L.off_ghost_list);
   a.n_entries = (unsigned)L.ghost_prefix.back() * GHOST_THREADS;
-  a.star_depth = P.p.lap_order;
+  a.star_depth = stencil_radius(P.p);
   a.star_only = 0;
   a.has_coarse = l > 0;
   a.alpha = T(0);
@@ -454,11 +466,11 @@ int plan_ghosts(sledge_ctx* c, int l) {
   return check_launch(c, "k_plan_ghosts");
 }
 
-template <typename T, int ORDER, int MODE>
+template <typename T, int ORDER, int MODE, int KO = 0>
 cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   constexpr int TY = K1Shape<MODE>::TY;
   static bool configured = false;  // per instantiation
-  if constexpr (K1Shape<MODE>::plane) {
+  if constexpr (K1Shape<MODE>::plane && KO == 0) {
     // the 7-plane z-window of the 19-point stencil leaves no registers for a second row
     constexpr int RY = ORDER == 3 ? 1 : ((K1Shape<MODE>::fused && sizeof(T) == 4) ? SLEDGE_K1F_RY32 : K1Shape<MODE>::RY);
     constexpr int PD = plane_depth<T, ORDER, MODE, K1F_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
@@ -473,10 +485,10 @@ cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
     }
     kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(a);
   } else {
-    constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, TY>(K1Shape<MODE>::SMEM, K1_DMAX);
-    static_assert(PipeCfg<T, ORDER, MODE, K1_TX, TY, D>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
-    using C = PipeCfg<T, ORDER, MODE, K1_TX, TY, D>;
-    auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, TY, D>;
+    constexpr int D = pipe_depth<T, ORDER, MODE, K1_TX, TY, KO>(K1Shape<MODE>::SMEM, K1_DMAX);
+    static_assert(PipeCfg<T, ORDER, MODE, K1_TX, TY, D, KO>::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
+    using C = PipeCfg<T, ORDER, MODE, K1_TX, TY, D, KO>;
+    auto kern = k_rk_pipe<T, ORDER, MODE, K1_TX, TY, D, KO>;
     if (!configured) {
       const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
       if (e != cudaSuccess) return e;
@@ -486,8 +498,23 @@ cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   }
   return cudaSuccess;
 }
+// staged sweeps with the Kreiss-Oliger term (never the fused ones)
+template <typename T, int ORDER, int KO>
+cudaError_t launch_pipe_mode_ko(sledge_ctx* c, const PipeArgs<T>& a, int grid, int mode) {
+  switch (mode) {
+    case LEAN_S1: return launch_pipe_kernel<T, ORDER, LEAN_S1, KO>(c, a, grid);
+    case LEAN_S23: return launch_pipe_kernel<T, ORDER, LEAN_S23, KO>(c, a, grid);
+    case LEAN_S4: return launch_pipe_kernel<T, ORDER, LEAN_S4, KO>(c, a, grid);
+    case CLASSIC_S1: return launch_pipe_kernel<T, ORDER, CLASSIC_S1, KO>(c, a, grid);
+    case CLASSIC_S23: return launch_pipe_kernel<T, ORDER, CLASSIC_S23, KO>(c, a, grid);
+    case CLASSIC_S4: return launch_pipe_kernel<T, ORDER, CLASSIC_S4, KO>(c, a, grid);
+    default: return cudaErrorInvalidValue;
+  }
+}
 template <typename T, int ORDER>
-cudaError_t launch_pipe_mode(sledge_ctx* c, const PipeArgs<T>& a, int grid, int mode) {
+cudaError_t launch_pipe_mode(sledge_ctx* c, const PipeArgs<T>& a, int grid, int mode, int ko) {
+  if (ko == 2) return launch_pipe_mode_ko<T, ORDER, 2>(c, a, grid, mode);
+  if (ko == 3) return launch_pipe_mode_ko<T, ORDER, 3>(c, a, grid, mode);
   switch (mode) {
     case LEAN_S1: return launch_pipe_kernel<T, ORDER, LEAN_S1>(c, a, grid);
     case LEAN_S23: return launch_pipe_kernel<T, ORDER, LEAN_S23>(c, a, grid);
@@ -512,12 +539,18 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   const double h2 = L.h * L.h;
   a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : (P.p.lap_order == 2 ? 1.0 / (12.0 * h2) : 1.0 / (180.0 * h2)));
   a.a_mass = (T)P.p.a_mass;
+  const int ko = ko_on(P.p) ? P.p.ko_order : 0;
+  if (ko) {  // Eq.7: (-1)^(r+1) eps / (2^(2r) h_l); Pi(U) is differenced too and moves from pnt[0] to sten[1]
+    const double sgn = (ko % 2 == 0) ? -1.0 : 1.0;
+    for (int q = 0; q < 4; ++q) a.ko_c[q] = (T)(sgn * P.p.ko_strength[q] / ((double)(1 << (2 * ko)) * L.h));
+    a.sten[1] = a.pnt[0];
+  }
   const int grid = (int)(fused ? L.ftiles.size() : L.tiles.size());
   cudaError_t e;
   {
     Timed tm(c, KIND_STAGE);
-    e = P.p.lap_order == 1 ? launch_pipe_mode<T, 1>(c, a, grid, mode)
-        : (P.p.lap_order == 2 ? launch_pipe_mode<T, 2>(c, a, grid, mode) : launch_pipe_mode<T, 3>(c, a, grid, mode));
+    e = P.p.lap_order == 1 ? launch_pipe_mode<T, 1>(c, a, grid, mode, ko)
+        : (P.p.lap_order == 2 ? launch_pipe_mode<T, 2>(c, a, grid, mode, ko) : launch_pipe_mode<T, 3>(c, a, grid, mode, ko));
   }
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "k_rk_pipe: %s", cudaGetErrorString(e));
   return check_launch(c, "k_rk_pipe");
@@ -582,7 +615,8 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
 // Fused sweeps need every psi AND Pi ghost to be a copy of a valid cell of the same level, which holds on
 // level 0 (it covers the periodic domain, L39); finer levels take their ghosts from time-interpolated coarse
 // data at every stage time (L72) and run the LEAN stages.
-inline bool level_is_fused(const Plan& P, int l) { return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0; }
+// With Kreiss-Oliger dissipation k_psi = Pi + Q psi is no longer pointwise: every level runs the staged sweeps.
+inline bool level_is_fused(const Plan& P, int l) { return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0 && !ko_on(P.p); }
 
 // One RK4 stage of level l: ghost fill of the stage input at its time, then K1.
 // t = time at the start of the level's step, eta_const = eta used when eta_fixed.
@@ -614,7 +648,7 @@ int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const)
     else if (s == 2) { ubuf = cur + 3; mode = CLASSIC_S23; in[0] = cur; in[1] = cur + 1; out[0] = cur + 2; out[1] = cur + 1; bdt = dt / 3.0; }
     else { ubuf = cur + 2; mode = CLASSIC_S4; in[0] = cur + 1; out[0] = cur + 1; }
   }
-  int rc = launch_ghosts<T>(c, l, ubuf, ts, false, true);
+  int rc = launch_ghosts<T>(c, l, ubuf, ts, ko_on(P.p), true);  // the dissipation term differences Pi as well
   if (rc) return rc;
   PipeArgs<T> a;
   memset(&a, 0, sizeof a);

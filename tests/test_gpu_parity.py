@@ -125,6 +125,83 @@ def test_ragged_multibox_fp64(order, g, flow):
     _compare_tags(o, s, 0)
 
 
+# ---- Kreiss-Oliger dissipation (Eq.7; S8(f) NEXT-2) inside K1 ---------------------------------
+
+KO_EPS = (0.02, 0.03, 0.05, 0.07)  # per component, all different (L750)
+
+
+@pytest.mark.parametrize("order,ko,g", [(1, 2, 2), (2, 2, 3), (3, 2, 3), (1, 3, 3), (2, 3, 3), (3, 3, 5)])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
+def test_kreiss_oliger_ragged_multibox_fp64(order, ko, g, flow):
+    """Every (Laplacian order, dissipation order) pair: the z-window radius is the larger of the two, Pi is differenced
+    too; `fused` must fall back to the staged sweeps (k_psi is no longer pointwise)."""
+    P = _pair()
+    n0 = (40, 24, 72)
+    o, s = P.make_pair(n0, boxes=_ragged_boxes(), nghost=g, lap_order=order, h0=0.5, lam=0.7, a_mass=0.3,
+                       friction=2.0, rk_dataflow=flow, ko_order=ko, ko_strength=KO_EPS)
+    P.init_smooth(o, s, n0, seed=13)
+    # grid-scale noise on top, so that the dissipation term is far above the tolerance
+    rng = np.random.default_rng(5)
+    for ib, (l, lo, hi) in enumerate(s.boxes):
+        for c in range(4):
+            a = o.get_state(ib, c)
+            P.set_both(o, s, ib, c, a + 0.05 * rng.standard_normal(a.shape))
+    eta, dt = 1.5, 0.1
+    for _ in range(4):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    _compare_tags(o, s, 0)
+
+
+def test_kreiss_oliger_changes_the_result():
+    """guards the test above against a silently ignored parameter: with and without the term the GPU runs differ"""
+    P = _pair()
+    n = 32
+    out = []
+    for eps in (0.0, 0.05):
+        o, s = P.make_pair(n, nghost=3, lap_order=2, h0=0.5, ko_order=3 if eps else 0, ko_strength=eps)
+        P.init_grf(o, s, n, 0.9, (81, 82))
+        s.rk_step(0.1, 1.0)
+        out.append(s.get_state(0, 0).cpu().numpy())
+    assert np.abs(out[0] - out[1]).max() > 1e-4
+
+
+@pytest.mark.parametrize("ko", [2, 3])
+@pytest.mark.parametrize("flow", ["lean", "fused"])
+def test_kreiss_oliger_two_level_subcycled(ko, flow):
+    """Pi ghosts of the fine level come from the time-interpolated coarse state at every stage (L72), h_l per level"""
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=3, lap_order=2, h0=0.5, rk_dataflow=flow, ko_order=ko,
+                       ko_strength=KO_EPS)
+    P.init_smooth(o, s, n0, seed=9)
+    eta, dt = 2.0, 0.1
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    for l in (0, 1):
+        _compare_tags(o, s, l)
+
+
+@pytest.mark.parametrize("ko", [2, 3])
+def test_kreiss_oliger_fp32(ko):
+    P = _pair()
+    n = 64
+    o, s = P.make_pair(n, nghost=3, lap_order=2, h0=0.125, dtype="f32", ko_order=ko, ko_strength=0.05)
+    P.init_grf(o, s, n, 0.25, (71, 72))
+    eta, dt = 1.0, 0.03125
+    for _ in range(20):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, relative=True) <= F32_TOL
+
+
 def _bf4_boxes():
     # 44 x 36 x 40 domain, blocking factor 4: tile heights that are not multiples of the K1 tile (4, 12, 20, 24
     # rows), box corners that are not multiples of 32 (a tagging warp straddles two count blocks in x)
