@@ -52,6 +52,9 @@ def parse():
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="sledge", choices=["sledge", "reference"])
     ap.add_argument("--flow", default="fused", choices=["fused", "lean", "classic"])
+    ap.add_argument("--ko-order", type=int, default=0, choices=[0, 2, 3],
+                    help="Kreiss-Oliger dissipation order (Eq.7); 0 = off, as in every BASELINE.json config")
+    ap.add_argument("--ko-strength", type=float, default=0.01)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -233,6 +236,28 @@ def run_reference(args, cfg):
 
 
 # ---------------------------------------------------------------------------------------------------
+# replicas: the path does not shard; N ranks run N independent replicas
+# ---------------------------------------------------------------------------------------------------
+
+def max_over_ranks(ms, world, device):
+    """Device time of the slowest replica (the contract's max over ranks); one scalar all-reduce, outside the
+    timed region.  `device`: where the backend wants the tensor (cuda for nccl, cpu for gloo)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, cell_steps, ms):
+    """Gcell-updates/s per RK stage of the whole job: every replica advances `cell_steps` cell-steps (x 4 stages)
+    per step, the job takes as long as its slowest replica."""
+    return world * cell_steps * 4 / (ms * 1e-3) / 1e9
+
+
+# ---------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------------
 
@@ -256,8 +281,12 @@ def run_sledge(args, cfg):
 
     rings, boxes, cover = hierarchy(cfg)
     cell_steps, per_level = cells_per_step(cfg, boxes)
-    s = S.Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=cfg.nghost, blocking_factor=cfg.blocking_factor,
-                 dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=args.flow, device=dev)
+    s = S.Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=max(cfg.nghost, args.ko_order),
+                 blocking_factor=cfg.blocking_factor,
+                 dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=args.flow, device=dev,
+                 ko_order=args.ko_order, ko_strength=args.ko_strength if args.ko_order else 0.0)
+    if args.ko_order and args.flow == "fused":
+        args.flow = "lean"  # with the dissipation term k_psi is not pointwise: every level runs the staged sweeps
     for ib, c, t in initial_fields(cfg, rings, boxes, dev, s.tdtype):
         s.set_state(ib, c, t)
         del t
@@ -302,10 +331,7 @@ def run_sledge(args, cfg):
     s.profile_enable(False)
     clocks = clk.stop() if rank == 0 else None
     s.synchronize()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
 
     # ---- roofline of the dominant kernel (K1) -----------------------------------------------------
     esz = 8 if cfg.dtype == "f64" else 4
@@ -335,13 +361,14 @@ def run_sledge(args, cfg):
                 "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage}
     shares = {k: (v[1] / args.steps) for k, v in prof.items()}
 
-    value = world * cell_steps * 4 / (ms * 1e-3) / 1e9
+    value = whole_job_value(world, cell_steps, ms)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"{cfg.name}: {cfg.n0}^3 base, {cfg.n_levels} level(s), {cfg.dtype}, "
                                    f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, RK4 ({args.flow} data-flow), "
-                                   f"dt={cfg.dt}, h0={cfg.h0}, tags + 32^3 counts every step",
+                                   f"dt={cfg.dt}, h0={cfg.h0}, tags + 32^3 counts every step"
+                                   + (f", Kreiss-Oliger order {args.ko_order} eps {args.ko_strength}" if args.ko_order else ""),
                        "cells_per_level": per_level, "coverage": cover, "cell_steps_per_step": cell_steps,
                        "l2": "state buffers >> 126 MB L2 (no flush needed)" if cell_steps * esz * 4 > 4e8 else
                              "state fits in L2 (small case; not a roofline workload)",
