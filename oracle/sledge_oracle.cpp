@@ -18,6 +18,7 @@
 //                    space + linear in time                                       L68-74
 //   O6 subcycling  : advance l, then l+1 twice, then synchronise                  L66-76, L88 Fig.2
 //   O7 average-down: coarse <- mean of 8 fine children                            L74, L88
+//   O11 SSPRK3     : Shu-Osher three-stage scheme (integrator.type 3 / 10)            L808
 //   O10 KO term    : Kreiss-Oliger dissipation Q_l added to every component's RHS  L141-146 Eq.7
 //   O9 TEE tags    : |coarse - mean of children| > eps at synchronisation         L82-111 Eq.5-6, L373-380 Eq.12
 //   O8 string tags : plaquette winding number of (psi1,psi2) around 0; rule not printed in the
@@ -60,7 +61,7 @@ struct Params {
   double friction;
   double ko_strength[4];  // epsilon_KO of Eq.7 per component psi1, psi2, Pi1, Pi2 (L749-750; 0 = off)
   int32_t ko_order;       // sim.dissipation_order = ghost cells the term needs (L751): 2 or 3
-  int32_t pad_;
+  int32_t integrator;     // integrator.type (L808): 0 or 4 = RK4; 3 or 10 = SSPRK3 (10 = its low-storage form)
 };
 
 struct BoxIn {
@@ -149,6 +150,7 @@ bool build(Oracle& o, const BoxIn* b, int nbox) {
     if (!(p.ko_strength[c] >= 0.0)) { o.err = "dissipation strength must be >= 0 (L749)"; return false; }
   if (ko_on && (p.ko_order < 2 || p.ko_order > 3)) { o.err = "dissipation order must be 2 or 3 (L751)"; return false; }
   if (ko_on && p.ko_order > p.nghost) { o.err = "dissipation order must be <= nghost (L751)"; return false; }
+  if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10) { o.err = "integrator.type must be 4 (RK4) or 3 / 10 (SSPRK3) (L808)"; return false; }
   if (!(p.h0 > 0)) { o.err = "h0 must be positive"; return false; }
   o.lev.resize(p.n_levels);
   for (int l = 0; l < p.n_levels; ++l) {
@@ -463,7 +465,54 @@ bool average_down(Oracle& o, int lf) {
 // ---- O4 + O6: classic RK4 with recursive time subcycling ---------------------------------------
 //   U_1 = Y;  k_s = f(U_s, eta_s), eta_s = t + c_s dt, c = (0, 1/2, 1/2, 1)
 //   U_{s+1} = Y + a_s dt k_s, a = (1/2, 1/2, 1);  Y_new = Y + dt/6 (k_1 + 2 k_2 + 2 k_3 + k_4)
+bool advance(Oracle& o, int l, double t, double dt, double eta_const);
+
+// ---- O11: SSPRK3 (integrator.type 3 / 10, L808), the Shu-Osher form -----------------------------
+//   U1   = Y + dt f(Y, t)
+//   U2   = 3/4 Y + 1/4 (U1 + dt f(U1, t + dt))
+//   Ynew = 1/3 Y + 2/3 (U2 + dt f(U2, t + dt/2))
+// Types 3 and 10 are the same scheme ("smaller memory footprint", L808); ghosts of a stage state are filled at
+// that stage's time t + c_s dt, c = (0, 1, 1/2), as for RK4 (L72).
+bool advance_ssprk3(Oracle& o, int l, double t, double dt, double eta_const) {
+  Level& L = o.lev[l];
+  static const double cs[3] = {0.0, 1.0, 0.5};
+  static const double wy[3] = {0.0, 0.75, 1.0 / 3.0};  // convex combination of a stage: wy Y + wu (U + dt f(U))
+  static const double wu[3] = {1.0, 0.25, 2.0 / 3.0};
+  L.Yold = L.Y;
+  L.U = L.Y;
+  for (int s = 0; s < 3; ++s) {
+    double ts = t + cs[s] * dt;
+    if (!fill_ghosts(o, l, L.U, ts)) return false;
+    double eta_s = o.p.eta_fixed ? eta_const : ts;
+    eval_rhs(o, l, L.U, L.K[s], eta_s);
+#pragma omp parallel for schedule(dynamic)
+    for (int q = 0; q < (int)L.boxes.size(); ++q) {
+      Field& U = L.U[q];
+      const Field& Y = L.Y[q];
+      const Field& K = L.K[s][q];
+      for (int c = 0; c < NCOMP; ++c)
+        for (int k = 0; k < U.n[2]; ++k)
+          for (int j = 0; j < U.n[1]; ++j)
+            for (int i = 0; i < U.n[0]; ++i) {
+              double euler = U.at(c, i, j, k) + dt * K.at(c, i, j, k);  // forward-Euler step from the stage state
+              U.at(c, i, j, k) = (s == 0) ? euler : wy[s] * Y.at(c, i, j, k) + wu[s] * euler;
+            }
+    }
+  }
+  L.Y = L.U;
+  L.t_old = t;
+  L.t_new = t + dt;
+  L.have_pair = true;
+  if (l + 1 < o.p.n_levels) {
+    if (!advance(o, l + 1, t, 0.5 * dt, eta_const)) return false;
+    if (!advance(o, l + 1, t + 0.5 * dt, 0.5 * dt, eta_const)) return false;
+    if (!average_down(o, l + 1)) return false;
+  }
+  return true;
+}
+
 bool advance(Oracle& o, int l, double t, double dt, double eta_const) {
+  if (o.p.integrator == 3 || o.p.integrator == 10) return advance_ssprk3(o, l, t, dt, eta_const);
   Level& L = o.lev[l];
   static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
   static const double as[3] = {0.5, 0.5, 1.0};
@@ -601,7 +650,7 @@ typedef struct {
   double h0, lambda, a_mass, friction;
   double ko_strength[4];
   int32_t ko_order;
-  int32_t pad_;
+  int32_t integrator;
 } orc_params;
 
 typedef struct {

@@ -505,14 +505,15 @@ def test_trilinear_reproduces_affine_data_in_space():
         assert np.all(raw[g:-g, g:-g, g:-g] == 0.0)  # valid cells are never touched by a fill
 
 
-@pytest.mark.parametrize("order", [1, 2])
-def test_time_interpolation_is_linear_between_coarse_old_and_new(order):
-    """lambda = 0 and psi = b + c t (Pi = c, spatially constant) is an exact solution that RK4 reproduces
+@pytest.mark.parametrize("order,integrator", [(1, 4), (2, 4), (2, 10)])
+def test_time_interpolation_is_linear_between_coarse_old_and_new(order, integrator):
+    """lambda = 0 and psi = b + c t (Pi = c, spatially constant) is an exact solution that RK4 (and SSPRK3, whose
+    stage times are t, t + dt, t + dt/2: alpha in {0, 1/2, 1/4} and {1/2, 1, 3/4}) reproduces
     exactly; during the fine substeps the ghosts must then carry b + c t_s for alpha in {0, 1/4, 1/2, 3/4, 1}.
     The fine interior sees a ghost value consistent with its own only if alpha is right; any wrong alpha
     puts a kink at the box edge that the Laplacian turns into a non-zero k_Pi."""
     h0 = 1.0
-    o = two_level(h0=h0, lam=0.0, order=order)
+    o = two_level(h0=h0, lam=0.0, order=order, integrator=integrator)
     b, c = 0.25, 0.5
     for ib in (0, 1):
         shp = o.box_shape(ib)
@@ -665,12 +666,13 @@ def test_tee_inside_rk_step_shrinks_with_resolution():
 # ------------------------------------------------------------------------------------------------
 
 
-@pytest.mark.parametrize("order,g,ko", [(1, 1, 0), (2, 2, 0), (1, 2, 2), (2, 3, 3)])
-def test_fully_covered_level1_equals_uniform_fine_run(order, g, ko):
+@pytest.mark.parametrize("order,g,ko,integrator", [(1, 1, 0, 4), (2, 2, 0, 4), (1, 2, 2, 4), (2, 3, 3, 4), (2, 2, 0, 10)])
+def test_fully_covered_level1_equals_uniform_fine_run(order, g, ko, integrator):
     """A hierarchy whose level 1 covers 100 % of the domain never interpolates: level 1 must reproduce the
     single-level 2N run with dt/2 bit-for-bit, and level 0 must equal its average.  With Kreiss-Oliger dissipation
     on (ko = dissipation order) this also pins that Q_l uses the level's own spacing (Eq.7: Delta x_l)."""
     kw = dict(ko_order=ko, ko_strength=(0.02, 0.03, 0.05, 0.07)) if ko else {}
+    kw["integrator"] = integrator
     n0, h0, dt, eta0 = 8, 1.0, 0.25, 1.0  # binary fractions: both runs see identical stage times
     nf = 2 * n0
     psi = [inputs.grf(nf, 0.5, s).numpy() for s in (41, 42)]
@@ -959,3 +961,96 @@ def test_c1_literal_parameters_blow_up():
     assert lit[7] > 1e2 and not lit[9] < 1e100
     stab = run(0.0625, 40)
     assert max(stab) < 4.5 and max(stab[20:]) < 3.0  # the initial GRF peaks at ~4 sigma, then relaxes
+
+# ------------------------------------------------------------------------------------------------
+# O11 SSPRK3 (integrator.type 3 / 10, L808)
+# ------------------------------------------------------------------------------------------------
+
+
+def scalar_ssprk3_butcher(y, eta, dt, lam, a, kappa):
+    """SSPRK3 in BUTCHER form (the oracle is written in Shu-Osher form): c = (0, 1, 1/2), a21 = 1,
+    a31 = a32 = 1/4, b = (1/6, 1/6, 2/3), for the 4-variable ODE of a spatially constant field."""
+
+    def f(y, e):
+        p1, p2, q1, q2 = y
+        pot = lam * e * e * (p1 * p1 + p2 * p2 - 1.0) + a
+        fr = kappa / e if kappa != 0 else 0.0
+        return np.array([q1, q2, -p1 * pot - fr * q1, -p2 * pot - fr * q2])
+
+    k1 = f(y, eta)
+    k2 = f(y + dt * k1, eta + dt)
+    k3 = f(y + 0.25 * dt * (k1 + k2), eta + 0.5 * dt)
+    return y + dt * (k1 / 6.0 + k2 / 6.0 + 2.0 * k3 / 3.0)
+
+
+@pytest.mark.parametrize("integrator", [3, 10])
+def test_ssprk3_constant_field_equals_butcher_form_scalar_ode(integrator):
+    n = 8
+    lam, a, kappa = 1.3, 0.56233, 2.0
+    o = Oracle(n, nghost=2, lap_order=2, h0=0.7, lam=lam, a_mass=a, friction=kappa, integrator=integrator)
+    y = np.array([0.3, -0.8, 0.1, 0.25])
+    for c in range(4):
+        o.set_state(0, c, np.full((n, n, n), y[c]))
+    eta, dt = 1.5, 0.05
+    for _ in range(20):
+        o.rk_step(dt, eta)
+        y = scalar_ssprk3_butcher(y, eta, dt, lam, a, kappa)
+        eta += dt
+    for c in range(4):
+        got = o.get_state(0, c)
+        assert np.all(got == got.flat[0])
+        assert abs(got.flat[0] - y[c]) <= 256 * np.finfo(float).eps * max(1.0, abs(y[c]))
+    # and it is NOT RK4: the two schemes differ at O(dt^4) per step, far above that tolerance
+    o4 = Oracle(n, nghost=2, lap_order=2, h0=0.7, lam=lam, a_mass=a, friction=kappa)
+    y0 = np.array([0.3, -0.8, 0.1, 0.25])
+    for c in range(4):
+        o4.set_state(0, c, np.full((n, n, n), y0[c]))
+    eta = 1.5
+    for _ in range(20):
+        o4.rk_step(dt, eta)
+        eta += dt
+    assert abs(o4.get_state(0, 2).flat[0] - y[2]) > 1e-7
+
+
+def test_ssprk3_linear_plane_wave_matches_cubic_amplification_matrix():
+    """lambda = 0: every 3-stage third-order scheme has R(z) = 1 + z + z^2/2 + z^3/6 on linear problems."""
+    n, h = (16, 8, 24), 0.5
+    o = Oracle(n, nghost=2, lap_order=2, h0=h, lam=0.0, integrator=10)
+    x, y, z = coords(n[::-1])
+    m = (1, 2, 3)
+    kh = [2 * math.pi * m[d] / n[d] for d in range(3)]
+    ph = kh[0] * x + kh[1] * y + kh[2] * z
+    w2 = sum(16 / 3 * math.sin(a / 2) ** 2 - 1 / 3 * math.sin(a) ** 2 for a in kh) / h ** 2
+    A0, B0 = 0.7, -0.4
+    o.set_state(0, 0, A0 * np.cos(ph))
+    o.set_state(0, 2, B0 * np.cos(ph))
+    o.set_state(0, 1, 2 * A0 * np.sin(ph))
+    o.set_state(0, 3, -B0 * np.sin(ph))
+    dt, steps = 0.2 * h, 25
+    Z = dt * np.array([[0.0, 1.0], [-w2, 0.0]])
+    R = np.eye(2) + Z + Z @ Z / 2 + Z @ Z @ Z / 6
+    Rn = np.linalg.matrix_power(R, steps)
+    eta = 3.0
+    for _ in range(steps):
+        o.rk_step(dt, eta)
+        eta += dt
+    a1, b1 = Rn @ np.array([A0, B0])
+    a2, b2 = Rn @ np.array([2 * A0, -B0])
+    assert np.abs(o.get_state(0, 0) - a1 * np.cos(ph)).max() < 1e-13
+    assert np.abs(o.get_state(0, 2) - b1 * np.cos(ph)).max() < 1e-12
+    assert np.abs(o.get_state(0, 1) - a2 * np.sin(ph)).max() < 1e-13
+    assert np.abs(o.get_state(0, 3) - b2 * np.sin(ph)).max() < 1e-12
+
+
+def test_ssprk3_is_third_order_on_the_nonlinear_problem():
+    """error against a fine-dt RK4 run of the same semi-discrete system drops by ~8 when dt is halved"""
+    n, T = 16, 0.4
+    psi = [inputs.grf(n, 0.5, s).numpy() for s in (61, 62)]
+    pi = [0.1 * inputs.grf(n, 0.5, s).numpy() for s in (63, 64)]
+    kw = dict(nghost=2, lap_order=2, h0=0.5, lam=1.0)
+    ref = run_single(n, None, psi, pi, 128, T / 128, 1.0, **kw)
+    err = []
+    for steps in (8, 16, 32):
+        got = run_single(n, None, psi, pi, steps, T / steps, 1.0, integrator=10, **kw)
+        err.append(np.abs(got - ref).max())
+    assert 6.5 < err[0] / err[1] < 9.5 and 6.5 < err[1] / err[2] < 9.5, err
