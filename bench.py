@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--ko-order", type=int, default=0, choices=[0, 2, 3],
                     help="Kreiss-Oliger dissipation order (Eq.7); 0 = off, as in every BASELINE.json config")
     ap.add_argument("--ko-strength", type=float, default=0.01)
+    ap.add_argument("--integrator", type=int, default=4, choices=[4, 3, 10],
+                    help="integrator.type (L808): 4 = RK4 (every BASELINE.json config), 3 / 10 = SSPRK3")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -251,10 +253,10 @@ def max_over_ranks(ms, world, device):
     return float(t.item())
 
 
-def whole_job_value(world, cell_steps, ms):
+def whole_job_value(world, cell_steps, ms, stages=4):
     """Gcell-updates/s per RK stage of the whole job: every replica advances `cell_steps` cell-steps (x 4 stages)
     per step, the job takes as long as its slowest replica."""
-    return world * cell_steps * 4 / (ms * 1e-3) / 1e9
+    return world * cell_steps * stages / (ms * 1e-3) / 1e9
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -284,7 +286,11 @@ def run_sledge(args, cfg):
     s = S.Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=max(cfg.nghost, args.ko_order),
                  blocking_factor=cfg.blocking_factor,
                  dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=args.flow, device=dev,
-                 ko_order=args.ko_order, ko_strength=args.ko_strength if args.ko_order else 0.0)
+                 ko_order=args.ko_order, ko_strength=args.ko_strength if args.ko_order else 0.0,
+                 integrator=args.integrator)
+    ssp = args.integrator in (3, 10)
+    if ssp:
+        args.flow = "ssprk3"  # three staged sweeps, 8 + 12 + 12 words per cell-step
     if args.ko_order and args.flow == "fused":
         args.flow = "lean"  # with the dissipation term k_psi is not pointwise: every level runs the staged sweeps
     for ib, c, t in initial_fields(cfg, rings, boxes, dev, s.tdtype):
@@ -337,7 +343,7 @@ def run_sledge(args, cfg):
     esz = 8 if cfg.dtype == "f64" else 4
     # algorithmic words (reals read + written) per cell-step of the data-flow that runs:
     # FUSED 20 on level 0 (finer levels run LEAN), LEAN 52, CLASSIC 64
-    flow_words = {"fused": 20, "lean": 52, "classic": 64}
+    flow_words = {"fused": 20, "lean": 52, "classic": 64, "ssprk3": 32}
     stage_words_per_step = sum(n * (1 << l) * (flow_words[args.flow] if (l == 0 or args.flow != "fused") else 52)
                                for l, n in enumerate(per_level))
     words_per_cell_step = stage_words_per_step / cell_steps
@@ -361,19 +367,19 @@ def run_sledge(args, cfg):
                 "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage}
     shares = {k: (v[1] / args.steps) for k, v in prof.items()}
 
-    value = whole_job_value(world, cell_steps, ms)
+    value = whole_job_value(world, cell_steps, ms, stages=3 if ssp else 4)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"{cfg.name}: {cfg.n0}^3 base, {cfg.n_levels} level(s), {cfg.dtype}, "
-                                   f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, RK4 ({args.flow} data-flow), "
+                                   f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, {'SSPRK3' if ssp else 'RK4'} ({args.flow} data-flow), "
                                    f"dt={cfg.dt}, h0={cfg.h0}, tags + 32^3 counts every step"
                                    + (f", Kreiss-Oliger order {args.ko_order} eps {args.ko_strength}" if args.ko_order else ""),
                        "cells_per_level": per_level, "coverage": cover, "cell_steps_per_step": cell_steps,
                        "l2": "state buffers >> 126 MB L2 (no flush needed)" if cell_steps * esz * 4 > 4e8 else
                              "state fits in L2 (small case; not a roofline workload)",
                        "multi_gpu": "replicas only"},
-            "gcell_steps_per_s": value / 4,
+            "gcell_steps_per_s": value / (3 if ssp else 4),
             "kernel_ms_per_step": shares, "roofline": roofline, "gpu_launches": launches, "clocks": clocks}
 
     # ---- e2e: same step through the C ABI with HOST buffers -----------------------------------------

@@ -72,7 +72,8 @@ typedef struct {
                               With the term on, every level runs the staged LEAN / CLASSIC sweeps (FUSED needs
                               k_psi = Pi pointwise) and the stage fills move Pi ghosts as well.          */
   int32_t ko_order;        /* r = sim.dissipation_order in {2,3} = ghost cells the term needs (L751): r <= nghost */
-  int32_t reserved_;       /* 0 */
+  int32_t integrator;      /* integrator.type (L808): 0 or 4 = classic RK4; 3 or 10 = SSPRK3 (Shu-Osher form,
+                              three state buffers, 32 words per cell-step; rk_dataflow is ignored)      */
 } sledge_params;
 
 /* Size of the device arena needed for this hierarchy.  Host-only: validates params and boxes
@@ -113,7 +114,9 @@ int sledge_fill_ghosts(sledge_ctx* ctx, int level, double time);
 /* One classic-RK4 stage (integrator.type 4, L808) of `level`: ghost fill of the stage input at
  * eta + c_s dt, then the fused Laplacian + potential + stage-update kernel (Eq.10-11).  stage =
  * 0,1,2,3 in order; `eta` is the time at the START of the step for all four calls.  Stage 3 makes
- * the new state current.  Test / timing hook; sledge_rk_step is built from it. */
+ * the new state current.  With integrator 3 / 10 (SSPRK3) stages 0,1,2 are the scheme's three stages
+ * (c = 0, 1, 1/2), stage 2 makes the new state current and stage 3 is a no-op.
+ * Test / timing hook; sledge_rk_step is built from it. */
 int sledge_rk_stage(sledge_ctx* ctx, int level, int stage, double dt, double eta);
 
 /* ONE coarse step eta -> eta + dt of the whole hierarchy (L64-76, L88 Fig.2): level l takes 2^l steps

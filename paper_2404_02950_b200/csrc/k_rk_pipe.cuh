@@ -40,7 +40,8 @@ enum StageMode {
   CLASSIC_S23 = 4,
   CLASSIC_S4 = 5,
   FUSED_A = 6,
-  FUSED_B = 7
+  FUSED_B = 7,
+  SSP_S23 = 8  // SSPRK3 (integrator.type 3 / 10, L808) stages 2 and 3: out = wy Y + wu (U + dt k(U)); stage 1 = LEAN_S1
 };
 
 template <int MODE> struct ModeInfo;
@@ -51,6 +52,7 @@ template <> struct ModeInfo<LEAN_S4> { static constexpr int NF = 1, NP = 7, NOUT
 template <> struct ModeInfo<CLASSIC_S1> { static constexpr int NF = 1, NP = 1, NOUT = 2; };
 template <> struct ModeInfo<CLASSIC_S23> { static constexpr int NF = 1, NP = 5, NOUT = 2; };
 template <> struct ModeInfo<CLASSIC_S4> { static constexpr int NF = 1, NP = 3, NOUT = 1; };
+template <> struct ModeInfo<SSP_S23> { static constexpr int NF = 1, NP = 3, NOUT = 1; };
 template <> struct ModeInfo<FUSED_A> { static constexpr int NF = 2, NP = 0, NOUT = 1; };
 template <> struct ModeInfo<FUSED_B> { static constexpr int NF = 3, NP = 1, NOUT = 1; };
 
@@ -75,6 +77,7 @@ struct PipeArgs {
   T a_mass;
   T adt;           // unfused: a_s * dt (S1-S3) or dt/6 (S4);  fused: dt
   T bdt;           // classic: b_s * dt for the accumulator
+  T wy, wu;        // SSP_S23: weights of Y and of the forward-Euler step from U (3/4, 1/4 and 1/3, 2/3)
   T ko_c[4];       // Kreiss-Oliger (Eq.7): (-1)^(r+1) eps_c / (2^(2r) h) for psi1, psi2, Pi1, Pi2; staged sweeps with
                    // KO != 0 only, where sten[1] = Pi(U) takes the place of pnt[0]
 };
@@ -215,6 +218,9 @@ __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[Mod
     } else if (MODE == LEAN_S23) {  // U' = Y + adt k   (in0 = Y)
       opsi[0] = mkpair(axpy(a.adt, kpsi1, ipsi(0).x), axpy(a.adt, kpsi2, ipsi(0).y));
       opi[0] = mkpair(axpy(a.adt, kpi1, ipi(0).x), axpy(a.adt, kpi2, ipi(0).y));
+    } else if (MODE == SSP_S23) {  // in0 = Y: out = wy Y + wu (U + adt k), adt = dt
+      opsi[0] = mkpair(fma(a.wy, ipsi(0).x, a.wu * axpy(a.adt, kpsi1, psi1)), fma(a.wy, ipsi(0).y, a.wu * axpy(a.adt, kpsi2, psi2)));
+      opi[0] = mkpair(fma(a.wy, ipi(0).x, a.wu * axpy(a.adt, kpi1, pi1)), fma(a.wy, ipi(0).y, a.wu * axpy(a.adt, kpi2, pi2)));
     } else if (MODE == LEAN_S4) {  // in0 = Y, in1 = U2, in2 = U3, U = U4, adt = dt/6
       const T third = T(1) / T(3);
       auto comb = [&](T yv, T u2, T u3, T u4, T kk) -> T {

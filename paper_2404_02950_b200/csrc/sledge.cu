@@ -195,6 +195,8 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     if (p.ko_order < 2 || p.ko_order > 3) return fail(nullptr, SLEDGE_EINVAL, "dissipation order must be 2 or 3 (L751)");
     if (p.ko_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "dissipation order must be <= nghost (L751)");
   }
+  if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10)
+    return fail(nullptr, SLEDGE_EINVAL, "integrator must be 4 (RK4) or 3 / 10 (SSPRK3) (L808)");
   if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
   if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
   if (!(p.h0 > 0)) return fail(nullptr, SLEDGE_EINVAL, "h0 must be positive");
@@ -508,6 +510,7 @@ cudaError_t launch_pipe_mode_ko(sledge_ctx* c, const PipeArgs<T>& a, int grid, i
     case CLASSIC_S1: return launch_pipe_kernel<T, ORDER, CLASSIC_S1, KO>(c, a, grid);
     case CLASSIC_S23: return launch_pipe_kernel<T, ORDER, CLASSIC_S23, KO>(c, a, grid);
     case CLASSIC_S4: return launch_pipe_kernel<T, ORDER, CLASSIC_S4, KO>(c, a, grid);
+    case SSP_S23: return launch_pipe_kernel<T, ORDER, SSP_S23, KO>(c, a, grid);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -522,6 +525,7 @@ cudaError_t launch_pipe_mode(sledge_ctx* c, const PipeArgs<T>& a, int grid, int 
     case CLASSIC_S1: return launch_pipe_kernel<T, ORDER, CLASSIC_S1>(c, a, grid);
     case CLASSIC_S23: return launch_pipe_kernel<T, ORDER, CLASSIC_S23>(c, a, grid);
     case CLASSIC_S4: return launch_pipe_kernel<T, ORDER, CLASSIC_S4>(c, a, grid);
+    case SSP_S23: return launch_pipe_kernel<T, ORDER, SSP_S23>(c, a, grid);
     case FUSED_A: return launch_pipe_kernel<T, ORDER, FUSED_A>(c, a, grid);
     default: return launch_pipe_kernel<T, ORDER, FUSED_B>(c, a, grid);
   }
@@ -616,7 +620,46 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
 // level 0 (it covers the periodic domain, L39); finer levels take their ghosts from time-interpolated coarse
 // data at every stage time (L72) and run the LEAN stages.
 // With Kreiss-Oliger dissipation k_psi = Pi + Q psi is no longer pointwise: every level runs the staged sweeps.
-inline bool level_is_fused(const Plan& P, int l) { return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0 && !ko_on(P.p); }
+inline bool is_ssprk3(const sledge_params& p) { return p.integrator == 3 || p.integrator == 10; }
+inline bool level_is_fused(const Plan& P, int l) {
+  return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0 && !ko_on(P.p) && !is_ssprk3(P.p);
+}
+
+// One SSPRK3 stage (integrator.type 3 / 10, L808; Shu-Osher form) of level l, s = 0, 1, 2:
+//   U1 = Y + dt f(Y, t);  U2 = 3/4 Y + 1/4 (U1 + dt f(U1, t + dt));  Ynew = 1/3 Y + 2/3 (U2 + dt f(U2, t + dt/2))
+// Buffers: cur = Y, cur+1 = U1 (then Ynew), cur+2 = U2: three buffers ("smaller memory footprint", type 10);
+// 8 + 12 + 12 = 32 words per cell-step.
+template <typename T>
+int do_stage_ssp(sledge_ctx* c, int l, int s, double t, double dt, double eta_const) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  static const double cs[3] = {0.0, 1.0, 0.5};
+  static const double wy[3] = {0.0, 0.75, 1.0 / 3.0}, wu[3] = {1.0, 0.25, 2.0 / 3.0};
+  const double ts = t + cs[s] * dt;
+  const int cur = L.cur;
+  const int ubuf = s == 0 ? cur : (s == 1 ? cur + 1 : cur + 2);
+  const int obuf = s == 1 ? cur + 2 : cur + 1;
+  int rc = launch_ghosts<T>(c, l, ubuf, ts, ko_on(P.p), true);
+  if (rc) return rc;
+  PipeArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.sten[0] = plane_ptr<T>(c, l, ubuf, 0);
+  a.pnt[0] = plane_ptr<T>(c, l, ubuf, 1);
+  if (s > 0) {
+    a.pnt[1] = plane_ptr<T>(c, l, cur, 0);
+    a.pnt[2] = plane_ptr<T>(c, l, cur, 1);
+  }
+  a.out_psi[0] = plane_ptr<T>(c, l, obuf, 0);
+  a.out_pi[0] = plane_ptr<T>(c, l, obuf, 1);
+  set_eta(P, a, 0, P.p.eta_fixed ? eta_const : ts);
+  a.adt = (T)dt;
+  a.wy = (T)wy[s];
+  a.wu = (T)wu[s];
+  rc = launch_k1<T>(c, l, s == 0 ? LEAN_S1 : SSP_S23, a);
+  if (rc) return rc;
+  if (s == 2) finish_step(L, cur + 1, t, dt);
+  return SLEDGE_OK;
+}
 
 // One RK4 stage of level l: ghost fill of the stage input at its time, then K1.
 // t = time at the start of the level's step, eta_const = eta used when eta_fixed.
@@ -624,6 +667,7 @@ template <typename T>
 int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
+  if (is_ssprk3(P.p)) return s < 3 ? do_stage_ssp<T>(c, l, s, t, dt, eta_const) : SLEDGE_OK;
   if (level_is_fused(P, l)) {  // stage calls 1 and 3 run the two sweeps, 0 and 2 are no-ops
     if (s == 1) return do_fused_pass<T>(c, l, 0, t, dt, eta_const);
     if (s == 3) return do_fused_pass<T>(c, l, 1, t, dt, eta_const);

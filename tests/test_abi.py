@@ -62,9 +62,11 @@ def test_validation_rules_from_the_paper():
         dict(ok, h0=0.0),
         dict(ok, ko_order=3, ko_strength=0.01),    # dissipation order = ghost cells needed (L751): 3 > nghost
         dict(ok, ko_order=1, ko_strength=0.01),    # order is 2 or 3 (L751)
+        dict(ok, integrator=21),                   # RKN tableaux are not printed in the paper: not built
         dict(ok, ko_order=2, ko_strength=(0.0, -0.1, 0.0, 0.0)),  # strength in R+ (L749)
     ]
     S.sledge_arena_bytes(32, **dict(ok, ko_order=2, ko_strength=(0.0, 0.0, 0.02, 0.0)))
+    S.sledge_arena_bytes(32, **dict(ok, integrator=10))
     S.sledge_arena_bytes(32, **dict(ok, ko_order=7, ko_strength=0.0))  # strength 0 removes the term, order unused
     for kw in bad:
         with pytest.raises(S.SledgeError):

@@ -202,6 +202,70 @@ def test_kreiss_oliger_fp32(ko):
     assert P.max_err(o, s, relative=True) <= F32_TOL
 
 
+# ---- SSPRK3 (integrator.type 3 / 10, L808; S8(f) NEXT-2) ------------------------------------------------
+
+
+@pytest.mark.parametrize("order,g,ko", [(1, 1, 0), (2, 2, 0), (3, 3, 0), (2, 3, 3), (1, 2, 2)])
+@pytest.mark.parametrize("integrator", [3, 10])
+def test_ssprk3_ragged_multibox_fp64(order, g, ko, integrator):
+    P = _pair()
+    n0 = (40, 24, 72)
+    o, s = P.make_pair(n0, boxes=_ragged_boxes(), nghost=g, lap_order=order, h0=0.5, lam=0.7, a_mass=0.3,
+                       friction=2.0, rk_dataflow="fused", integrator=integrator, ko_order=ko,
+                       ko_strength=KO_EPS if ko else 0.0)
+    P.init_smooth(o, s, n0, seed=17)
+    eta, dt = 1.5, 0.1
+    for _ in range(4):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    _compare_tags(o, s, 0)
+
+
+def test_ssprk3_is_not_rk4_on_the_gpu():
+    P = _pair()
+    n = 32
+    out = []
+    for integ in (4, 10):
+        o, s = P.make_pair(n, nghost=2, lap_order=2, h0=0.5, integrator=integ)
+        P.init_grf(o, s, n, 0.5, (81, 82))
+        for q in range(3):
+            s.rk_step(0.1, 1.0 + 0.1 * q)
+        out.append(s.get_state(0, 0).cpu().numpy())
+    assert np.abs(out[0] - out[1]).max() > 1e-7
+
+
+def test_ssprk3_three_level_subcycled():
+    """stage times t, t + dt, t + dt/2 in the coarse->fine ghost interpolation (L72), average-down"""
+    P = _pair()
+    n0 = 32
+    _, boxes, _ = _ring_hierarchy(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5, integrator=10)
+    P.init_smooth(o, s, n0, seed=23)
+    eta, dt = 2.0, 0.1
+    for _ in range(2):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    for l in range(3):
+        _compare_tags(o, s, l)
+
+
+def test_ssprk3_fp32():
+    P = _pair()
+    n = 64
+    o, s = P.make_pair(n, nghost=2, lap_order=2, h0=0.125, dtype="f32", integrator=10)
+    P.init_grf(o, s, n, 0.25, (71, 72))
+    eta, dt = 1.0, 0.03125
+    for _ in range(20):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, relative=True) <= F32_TOL
+
+
 def _bf4_boxes():
     # 44 x 36 x 40 domain, blocking factor 4: tile heights that are not multiples of the K1 tile (4, 12, 20, 24
     # rows), box corners that are not multiples of 32 (a tagging warp straddles two count blocks in x)
