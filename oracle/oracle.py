@@ -72,7 +72,7 @@ def lib():
         L.orc_eval_rhs.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int]
         L.orc_rk_step.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.orc_average_down.argtypes = [C.c_void_p, C.c_int]
-        L.orc_tee_enable.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
+        L.orc_tee_enable.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         L.orc_tag_strings.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_plaquette_winding.argtypes = [dp, dp, dp, dp]
         L.orc_energy.argtypes = [C.c_void_p, C.c_double, dp]
@@ -200,7 +200,7 @@ class Oracle:
     def average_down(self, fine_level):
         self._chk(lib().orc_average_down(self._h, fine_level))
 
-    def tee_enable(self, fine_level, eps_psi1, eps_psi2):
+    def tee_enable(self, fine_level, eps_psi1, eps_psi2, eps_pi1=np.inf, eps_pi2=np.inf):
         """O9: every later synchronisation of `fine_level` (average_down, also inside rk_step) writes truncation-error
         tags; read them with tee_tags(fine_level)."""
         ibs = self.level_boxes(fine_level)
@@ -210,7 +210,8 @@ class Oracle:
         tags = np.zeros(n, dtype=np.uint8)
         counts = np.zeros(self.count_shape(fine_level), dtype=np.uint32)
         self._tee[fine_level] = (tags, counts)
-        self._chk(lib().orc_tee_enable(self._h, fine_level, eps_psi1, eps_psi2, tags.ctypes.data, counts.ctypes.data))
+        eps = (C.c_double * 4)(eps_psi1, eps_psi2, eps_pi1, eps_pi2)
+        self._chk(lib().orc_tee_enable(self._h, fine_level, eps, tags.ctypes.data, counts.ctypes.data))
 
     def tee_tags(self, fine_level):
         """(list of uint8 tag arrays [z,y,x], one per box of the level; uint32 counts [bz,by,bx]) of the last sync."""

@@ -109,7 +109,7 @@ struct Level {
   LevelState U;             // stage state
   // O9: truncation-error tags of this (fine) level, written by average_down when tee_on (L82-111, Eq.5-6, Eq.12)
   bool tee_on = false;
-  double tee_eps[2] = {0, 0};
+  double tee_eps[4] = {0, 0, 0, 0};  // threshold per component psi1, psi2, Pi1, Pi2 (te_crit_$ScalarField, L781-782)
   uint8_t* tee_tags = nullptr;     // caller's arrays (dense per box, x fastest, boxes back to back)
   uint32_t* tee_counts = nullptr;  // tagged cells per aligned FLAG_BLOCK^3 block of this level
 };
@@ -438,7 +438,7 @@ bool average_down(Oracle& o, int lf) {
                 for (int rx = 0; rx < 2; ++rx) s += F.at(c, i + rx, j + ry, k + rz);
             double mean = 0.125 * s;
             double& coarse = Lc.Y[ow].at(c, ci - Bc.lo[0], cj - Bc.lo[1], ck - Bc.lo[2]);
-            if (tee && c < 2) {  // c = PSI1, PSI2
+            if (tee) {  // every component has its own threshold; DBL_MAX (the default) never tags
               double delta = std::fabs(coarse - mean);
               if (delta > Lf.tee_eps[c]) tag |= (uint8_t)(1u << c);
             }
@@ -750,13 +750,12 @@ int orc_rk_step(void* h, double dt, double eta) {
 
 // O9: from now on every synchronisation of `fine_level` also writes truncation-error tags (tags / counts stay owned
 // by the caller and must outlive the handle's use; tags == nullptr switches it off)
-int orc_tee_enable(void* h, int fine_level, double eps_psi1, double eps_psi2, uint8_t* tags, uint32_t* counts) {
+int orc_tee_enable(void* h, int fine_level, const double* eps4, uint8_t* tags, uint32_t* counts) {
   Oracle& o = *(Oracle*)h;
   if (fine_level < 1 || fine_level >= o.p.n_levels) return -1;
   Level& L = o.lev[fine_level];
   L.tee_on = tags != nullptr || counts != nullptr;
-  L.tee_eps[0] = eps_psi1;
-  L.tee_eps[1] = eps_psi2;
+  for (int c = 0; c < NCOMP; ++c) L.tee_eps[c] = eps4[c];
   L.tee_tags = tags;
   L.tee_counts = counts;
   return 0;

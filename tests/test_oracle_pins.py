@@ -599,16 +599,20 @@ def test_tee_tags_equal_the_prescribed_offsets_exactly():
     of tagged coarse cells in the block -- all computed here independently of the oracle."""
     o = two_level(n0=32, lo=(8, 24, 16), hi=(39, 47, 47), h0=1.0, lam=0.0)  # fine box straddles 32-blocks
     rng = np.random.default_rng(9)
-    d = [rng.integers(-8, 9, size=(32, 32, 32)) / 64.0 for _ in range(2)]  # multiples of 1/64 in [-1/8, 1/8]
-    for c in range(2):
+    d = [rng.integers(-8, 9, size=(32, 32, 32)) / 64.0 for _ in range(4)]  # multiples of 1/64 in [-1/8, 1/8]
+    for c in range(4):
         o.set_state(0, c, 1.0 + d[c])
         o.set_state(1, c, np.ones(o.box_shape(1)))
-    eps = (3 / 64.0, 5 / 64.0)
+    # one threshold per component, momenta included (te_crit_$ScalarField, L781-782; Scalar::Pi1, L202)
+    eps = (3 / 64.0, 5 / 64.0, 6 / 64.0, 2 / 64.0)
     o.tee_enable(1, *eps)
     o.average_down(1)
     tags, counts = o.tee_tags(1)
     cov = (slice(8, 24), slice(12, 24), slice(4, 20))  # z, y, x coarse footprint of the fine box
-    want_c = ((np.abs(d[0][cov]) > eps[0]).astype(np.uint8) | ((np.abs(d[1][cov]) > eps[1]).astype(np.uint8) << 1))
+    want_c = np.zeros(d[0][cov].shape, dtype=np.uint8)
+    for c in range(4):
+        want_c |= (np.abs(d[c][cov]) > eps[c]).astype(np.uint8) << c
+    assert all(((want_c >> c) & 1).any() and not ((want_c >> c) & 1).all() for c in range(4))
     assert want_c.any() and not want_c.all()
     want_f = want_c.repeat(2, axis=0).repeat(2, axis=1).repeat(2, axis=2)
     assert np.array_equal(tags[0], want_f)
@@ -621,6 +625,13 @@ def test_tee_tags_equal_the_prescribed_offsets_exactly():
     assert np.array_equal(counts, want_counts) and counts.sum() == 8 * np.count_nonzero(want_c)
     # the synchronisation itself is unchanged: covered coarse cells now hold the children's mean
     assert np.all(o.get_state(0, 0)[cov] == 1.0)
+    # the default threshold (DBL_MAX, L781) switches a component off: psi-only thresholds give bits 0, 1 only
+    for c in range(4):
+        o.set_state(0, c, 1.0 + d[c])
+    o.tee_enable(1, eps[0], eps[1])
+    o.average_down(1)
+    tags2, _ = o.tee_tags(1)
+    assert np.array_equal(tags2[0], want_f & 3)
 
 
 def test_tee_inside_rk_step_shrinks_with_resolution():
