@@ -432,7 +432,8 @@ def e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags):
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / args.e2e_steps
-    return {"value": world * cell_steps * 4 / (ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms,
+    return {"value": whole_job_value(world, cell_steps, ms, stages=3 if args.integrator in (3, 10) else 4),
+            "unit": UNIT, "ms_per_step": ms,
             "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "steps": args.e2e_steps,
             "what": "sledge_set_state_host x4/box + sledge_rk_step + sledge_tag_strings + sledge_get_state_host x4/box + counts"}
 

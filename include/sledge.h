@@ -139,9 +139,11 @@ int sledge_average_down(sledge_ctx* ctx, int fine_level);
 /* Truncation-error (TEE) tags of the self-shadow method (L82-111 Eq.5-6, L373-380 Eq.12 with f = identity), fused
  * into the synchronisation: from now on every average-down of `fine_level` -- the explicit call above and the ones
  * inside sledge_rk_step -- first compares, for every coarse cell C under a fine box, the coarse level's own value
- * with the mean of its 8 fine children, Delta_c = |phi_c^{l-1}(C) - mean_c| for the scalar components c = psi1, psi2
- * (in the context's dtype), and gives the 8 children the tag byte (Delta_psi1 > eps_psi1) | (Delta_psi2 > eps_psi2) << 1
- * (strict >, Eq.12); then it overwrites the coarse value as before.
+ * with the mean of its 8 fine children, Delta_c = |phi_c^{l-1}(C) - mean_c| for every component c = psi1, psi2, Pi1,
+ * Pi2 (in the context's dtype), and gives the 8 children the tag byte  sum_c (Delta_c > eps4[c]) << c  (strict >,
+ * Eq.12); then it overwrites the coarse value as before.
+ *   eps4       : HOST, four thresholds >= 0 (amr.te_crit_$ScalarField, L781-782; the momenta are members of the
+ *                Scalar set, L202); DBL_MAX or +inf -- the paper's default -- leaves a component untagged.
  *   dev_tags   : device, one byte per VALID cell of `fine_level`, boxes of the level back to back in input order,
  *                x fastest (the layout of sledge_tag_strings); 2-byte aligned; may be NULL.
  *   dev_counts : device, uint32 per aligned 32^3 block of the fine level's index space (x fastest), zeroed and
@@ -149,7 +151,7 @@ int sledge_average_down(sledge_ctx* ctx, int fine_level);
  * Both NULL switches the tags off.  The buffers stay owned by the caller and must stay valid while enabled.  A level
  * synchronises once per step of its parent, so after sledge_rk_step the buffers hold the LAST synchronisation.
  * Level 0 has no coarser partner (the paper's shadow level, L98, is not built): SLEDGE_EINVAL. */
-int sledge_tee_enable(sledge_ctx* ctx, int fine_level, double eps_psi1, double eps_psi2, uint8_t* dev_tags,
+int sledge_tee_enable(sledge_ctx* ctx, int fine_level, const double* eps4, uint8_t* dev_tags,
                       uint32_t* dev_counts);
 
 /* Bookkeeping. */

@@ -34,7 +34,7 @@ struct AvgArgs {
   P* c_pi;
   int* err_flag;
   // TEE variant only
-  T tee_eps[2];
+  T tee_eps[4];          // threshold per component psi1, psi2, Pi1, Pi2 (L781-782); +inf = never tags
   uint8_t* tee_tags;     // dense tags of the FINE level (boxes back to back, x fastest); may be null
   uint32_t* tee_counts;  // tagged fine cells per aligned 32^3 block of the fine level; may be null
   int nb0, nb1;          // count blocks per axis (x, y) of the fine level
@@ -83,10 +83,13 @@ __global__ void __launch_bounds__(AVG_THREADS) k_average_down(const AvgArgs<T> a
   const long long co = cell_offset(cb, a.cgeom.g, a.cgeom.ox, ci - cb.lo[0], cj - cb.lo[1], ck - cb.lo[2]);
   const long long fplane = (long long)fb.sx * fb.sy;
   const typename PairOf<T>::type m = mean8<T>(a.f_psi, fo, fb.sx, fplane);
+  const typename PairOf<T>::type mp = mean8<T>(a.f_pi, fo, fb.sx, fplane);
   if (TEE) {
     const typename PairOf<T>::type c = a.c_psi[co];  // the coarse level's own result, before the overwrite
-    const T d1 = fabs(c.x - m.x), d2 = fabs(c.y - m.y);
-    const unsigned tag = (d1 > a.tee_eps[0] ? 1u : 0u) | (d2 > a.tee_eps[1] ? 2u : 0u);
+    const typename PairOf<T>::type cp = a.c_pi[co];
+    const T d1 = fabs(c.x - m.x), d2 = fabs(c.y - m.y), d3 = fabs(cp.x - mp.x), d4 = fabs(cp.y - mp.y);
+    const unsigned tag = (d1 > a.tee_eps[0] ? 1u : 0u) | (d2 > a.tee_eps[1] ? 2u : 0u) |
+                         (d3 > a.tee_eps[2] ? 4u : 0u) | (d4 > a.tee_eps[3] ? 8u : 0u);
     if (a.tee_tags) {
       const unsigned short two = (unsigned short)(tag | (tag << 8));
 #pragma unroll
@@ -103,7 +106,7 @@ __global__ void __launch_bounds__(AVG_THREADS) k_average_down(const AvgArgs<T> a
     }
   }
   a.c_psi[co] = m;
-  a.c_pi[co] = mean8<T>(a.f_pi, fo, fb.sx, fplane);
+  a.c_pi[co] = mp;
 }
 
 // ---- dense <-> padded copies (one component of one box) -------------------------------------------

@@ -119,7 +119,7 @@ struct LevelHost {
   size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix, off_ghost_list;
   // truncation-error tags written at this (fine) level's synchronisations (sledge_tee_enable)
   bool tee_on = false;
-  double tee_eps[2] = {0, 0};
+  double tee_eps[4] = {0, 0, 0, 0};
   uint8_t* tee_tags = nullptr;
   uint32_t* tee_counts = nullptr;
   // run state
@@ -738,8 +738,7 @@ int do_average_down(sledge_ctx* c, int lf) {
   a.err_flag = tab<int>(c, P.off_err);
   const int grid = F.avg_prefix.back();
   if (F.tee_on) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
-    a.tee_eps[0] = (T)F.tee_eps[0];
-    a.tee_eps[1] = (T)F.tee_eps[1];
+    for (int q = 0; q < 4; ++q) a.tee_eps[q] = (T)F.tee_eps[q];
     a.tee_tags = F.tee_tags;
     a.tee_counts = F.tee_counts;
     a.nb0 = F.nb[0];
@@ -1012,17 +1011,17 @@ int sledge_level_cells(const sledge_ctx* c, int level, int64_t* valid_cells, int
   return SLEDGE_OK;
 }
 
-int sledge_tee_enable(sledge_ctx* c, int fine_level, double eps_psi1, double eps_psi2, uint8_t* dev_tags,
-                      uint32_t* dev_counts) {
+int sledge_tee_enable(sledge_ctx* c, int fine_level, const double* eps4, uint8_t* dev_tags, uint32_t* dev_counts) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
   if (fine_level < 1 || fine_level >= c->plan.p.n_levels)
     return fail(c, SLEDGE_EINVAL, "tee_enable: level %d has no coarser level to compare with", fine_level);
-  if (!(eps_psi1 >= 0) || !(eps_psi2 >= 0)) return fail(c, SLEDGE_EINVAL, "tee_enable: thresholds must be >= 0");
+  if (!eps4) return fail(c, SLEDGE_EINVAL, "tee_enable: null thresholds");
+  for (int q = 0; q < 4; ++q)
+    if (!(eps4[q] >= 0)) return fail(c, SLEDGE_EINVAL, "tee_enable: thresholds must be >= 0");
   if (dev_tags && ((uintptr_t)dev_tags & 1)) return fail(c, SLEDGE_EINVAL, "tee_enable: tags must be 2-byte aligned");
   LevelHost& L = c->plan.lev[fine_level];
   L.tee_on = dev_tags != nullptr || dev_counts != nullptr;
-  L.tee_eps[0] = eps_psi1;
-  L.tee_eps[1] = eps_psi2;
+  for (int q = 0; q < 4; ++q) L.tee_eps[q] = eps4[q];
   L.tee_tags = dev_tags;
   L.tee_counts = dev_counts;
   return SLEDGE_OK;

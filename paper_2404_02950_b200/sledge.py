@@ -69,7 +69,7 @@ def lib():
         L.sledge_rk_step.argtypes = [vp, d, d]
         L.sledge_tag_strings.argtypes = [vp, i, vp, vp]
         L.sledge_average_down.argtypes = [vp, i]
-        L.sledge_tee_enable.argtypes = [vp, i, C.c_double, C.c_double, vp, vp]
+        L.sledge_tee_enable.argtypes = [vp, i, C.POINTER(C.c_double), vp, vp]
         L.sledge_level_cells.argtypes = [vp, i, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.sledge_launch_count.argtypes = [vp]
         L.sledge_launch_count.restype = C.c_int64
@@ -251,8 +251,8 @@ class Sledge:
     def average_down(self, fine_level):
         self._chk(lib().sledge_average_down(self._h, fine_level), "sledge_average_down")
 
-    def tee_enable(self, fine_level, eps_psi1, eps_psi2, tags: torch.Tensor | None = None,
-                   counts: torch.Tensor | None = None):
+    def tee_enable(self, fine_level, eps_psi1, eps_psi2, eps_pi1=float("inf"), eps_pi2=float("inf"),
+                   tags: torch.Tensor | None = None, counts: torch.Tensor | None = None):
         """sledge_tee_enable: every later synchronisation of `fine_level` writes truncation-error tags into the
         returned (tags uint8 [valid cells of the level], counts int32 [bz, by, bx]) tensors, which this object
         keeps alive."""
@@ -261,8 +261,9 @@ class Sledge:
             tags = torch.zeros(ncell, dtype=torch.uint8, device=self.device)
         if counts is None:
             counts = torch.zeros(self.count_shape(fine_level), dtype=torch.int32, device=self.device)
-        self._chk(lib().sledge_tee_enable(self._h, fine_level, float(eps_psi1), float(eps_psi2), tags.data_ptr(),
-                                          counts.data_ptr()), "sledge_tee_enable")
+        eps = (C.c_double * 4)(float(eps_psi1), float(eps_psi2), float(eps_pi1), float(eps_pi2))
+        self._chk(lib().sledge_tee_enable(self._h, fine_level, eps, tags.data_ptr(), counts.data_ptr()),
+                  "sledge_tee_enable")
         if not hasattr(self, "_tee"):
             self._tee = {}
         self._tee[fine_level] = (tags, counts)

@@ -421,12 +421,14 @@ def test_tee_tags_at_explicit_average_down_match_oracle_bitwise():
     boxes = P.two_level_boxes(n0)
     o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=2, lap_order=2, h0=1.0)
     P.init_smooth(o, s, n0, seed=21)
-    eps = (0.004, 0.009)
+    eps = (0.004, 0.009, 0.006, 0.012)  # psi1, psi2, Pi1, Pi2 (L781-782)
     o.tee_enable(1, *eps)
     s.tee_enable(1, *eps)
     o.average_down(1)
     s.average_down(1)
     ntag = _tee_compare(o, s, 1)
+    bits = np.concatenate([t.ravel() for t in o.tee_tags(1)[0]])
+    assert all(0 < int(((bits >> c) & 1).sum()) < bits.size for c in range(4))  # every component's bit is exercised
     ncell = sum(int(np.prod(o.box_shape(ib))) for ib in o.level_boxes(1))
     assert 0 < ntag < ncell
     assert P.max_err(o, s) == 0.0
@@ -454,8 +456,8 @@ def test_tee_tags_inside_rk_step_three_levels():
             P.set_both(o, s, ib, 0, re.numpy())
             P.set_both(o, s, ib, 1, im.numpy())
         for l in (1, 2):
-            o.tee_enable(l, eps * scale, eps * scale)
-            s.tee_enable(l, eps, eps)
+            o.tee_enable(l, eps * scale, eps * scale, 4 * eps * scale, 4 * eps * scale)
+            s.tee_enable(l, eps, eps, 4 * eps, 4 * eps)
         o.rk_step(0.0625, 2.0)
         s.rk_step(0.0625, 2.0)
         s.synchronize()
