@@ -43,6 +43,8 @@ class _Params(C.Structure):
         ("ko_strength", C.c_double * 4),
         ("ko_order", C.c_int32),
         ("integrator", C.c_int32),
+        ("interp", C.c_int32),
+        ("pad_", C.c_int32),
     ]
 
 
@@ -103,7 +105,7 @@ class Oracle:
 
     def __init__(self, n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, lap_order=1,
                  h0=1.0, lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, ko_order=0, ko_strength=0.0,
-                 integrator=4):
+                 integrator=4, interp=0):
         if np.isscalar(n0):
             n0 = (int(n0),) * 3
         if boxes is None:
@@ -128,6 +130,7 @@ class Oracle:
         p.ko_strength[:] = [float(v) for v in ks]
         p.ko_order = ko_order
         p.integrator = integrator
+        p.interp = interp
         arr = (_Box * len(self.boxes))()
         for q, (l, lo, hi) in enumerate(self.boxes):
             arr[q].level = l

@@ -18,6 +18,7 @@
 //                    space + linear in time                                       L68-74
 //   O6 subcycling  : advance l, then l+1 twice, then synchronise                  L66-76, L88 Fig.2
 //   O7 average-down: coarse <- mean of 8 fine children                            L74, L88
+//   O12 quartic    : quartic polynomial conservative coarse->fine interpolation      L70, L780
 //   O11 SSPRK3     : Shu-Osher three-stage scheme (integrator.type 3 / 10)            L808
 //   O10 KO term    : Kreiss-Oliger dissipation Q_l added to every component's RHS  L141-146 Eq.7
 //   O9 TEE tags    : |coarse - mean of children| > eps at synchronisation         L82-111 Eq.5-6, L373-380 Eq.12
@@ -62,6 +63,9 @@ struct Params {
   double ko_strength[4];  // epsilon_KO of Eq.7 per component psi1, psi2, Pi1, Pi2 (L749-750; 0 = off)
   int32_t ko_order;       // sim.dissipation_order = ghost cells the term needs (L751): 2 or 3
   int32_t integrator;     // integrator.type (L808): 0 or 4 = RK4; 3 or 10 = SSPRK3 (10 = its low-storage form)
+  int32_t interp;         // coarse->fine ghost interpolation: 0 = cell-centred trilinear (BASELINE.json config 5),
+                          // 4 = quartic polynomial conservative (amr.interpolation_type 4, the paper's default)
+  int32_t pad_;
 };
 
 struct BoxIn {
@@ -151,6 +155,7 @@ bool build(Oracle& o, const BoxIn* b, int nbox) {
   if (ko_on && (p.ko_order < 2 || p.ko_order > 3)) { o.err = "dissipation order must be 2 or 3 (L751)"; return false; }
   if (ko_on && p.ko_order > p.nghost) { o.err = "dissipation order must be <= nghost (L751)"; return false; }
   if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10) { o.err = "integrator.type must be 4 (RK4) or 3 / 10 (SSPRK3) (L808)"; return false; }
+  if (p.interp != 0 && p.interp != 4) { o.err = "interp must be 0 (trilinear) or 4 (quartic conservative, L780)"; return false; }
   if (!(p.h0 > 0)) { o.err = "h0 must be positive"; return false; }
   o.lev.resize(p.n_levels);
   for (int l = 0; l < p.n_levels; ++l) {
@@ -292,6 +297,31 @@ bool fill_ghosts(Oracle& o, int l, LevelState& S, double time) {
             c0[d] = floordiv2(f[d]);
             int r = f[d] - 2 * c0[d];
             c1[d] = (r == 0) ? c0[d] - 1 : c0[d] + 1;
+          }
+          if (o.p.interp == 4) {
+            // O12, L70 "fourth-order spatial interpolation", L780 type 4 "quartic polynomial conservative": per axis
+            // the quartic whose averages over the coarse cells c0-2 .. c0+2 equal their values, averaged over the
+            // fine cell (the left or right half of c0):
+            //   r = 0: c0 + (-3 c[-2] + 22 c[-1] - 22 c[+1] + 3 c[+2]) / 128      r = 1: the mirror image
+            // (the two children average to c0: conservative); tensor product over the three axes.
+            static const double WQ[2][5] = {{-3.0 / 128, 22.0 / 128, 1.0, -22.0 / 128, 3.0 / 128},
+                                            {3.0 / 128, -22.0 / 128, 1.0, 22.0 / 128, -3.0 / 128}};
+            int r[3];
+            for (int d = 0; d < 3; ++d) r[d] = f[d] - 2 * c0[d];
+            for (int c = 0; c < NCOMP; ++c) {
+              double sum = 0.0;
+              for (int mz = -2; mz <= 2; ++mz)
+                for (int my = -2; my <= 2; ++my)
+                  for (int mx = -2; mx <= 2; ++mx) {
+                    double vo = value(o, l - 1, *Cold, c, c0[0] + mx, c0[1] + my, c0[2] + mz, &ok);
+                    double vn = value(o, l - 1, *Cnew, c, c0[0] + mx, c0[1] + my, c0[2] + mz, &ok);
+                    double cv = (1.0 - alpha) * vo + alpha * vn;
+                    double wt = (WQ[r[2]][mz + 2] * WQ[r[1]][my + 2]) * WQ[r[0]][mx + 2];
+                    sum += wt * cv;
+                  }
+              F.at(c, i, j, k) = sum;
+            }
+            continue;
           }
           const double w[2] = {0.75, 0.25};
           for (int c = 0; c < NCOMP; ++c) {
@@ -651,6 +681,8 @@ typedef struct {
   double ko_strength[4];
   int32_t ko_order;
   int32_t integrator;
+  int32_t interp;
+  int32_t pad_;
 } orc_params;
 
 typedef struct {

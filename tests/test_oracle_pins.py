@@ -1065,3 +1065,111 @@ def test_ssprk3_is_third_order_on_the_nonlinear_problem():
         got = run_single(n, None, psi, pi, steps, T / steps, 1.0, integrator=10, **kw)
         err.append(np.abs(got - ref).max())
     assert 6.5 < err[0] / err[1] < 9.5 and 6.5 < err[1] / err[2] < 9.5, err
+
+
+# ------------------------------------------------------------------------------------------------
+# O12 quartic polynomial conservative coarse->fine interpolation (amr.interpolation_type 4, L70, L780)
+# ------------------------------------------------------------------------------------------------
+
+
+def _cell_avg_monomial(p, lo, hi):
+    """exact average of x^p over [lo, hi] (arrays allowed)"""
+    return (hi ** (p + 1) - lo ** (p + 1)) / ((p + 1) * (hi - lo))
+
+
+def _poly_cell_averages(level_h, shape, lo, coefs, g=0):
+    """cell averages of sum_t a_t x^px y^py z^pz over the cells of an index range (z, y, x array)"""
+    ax = []
+    for l, s in zip(lo[::-1], shape):  # z, y, x
+        idx = np.arange(l - g, l + s + g, dtype=np.float64)
+        ax.append((idx * level_h, (idx + 1) * level_h))
+    out = 0.0
+    for a, (px, py, pz) in coefs:
+        Z = _cell_avg_monomial(pz, *ax[0])[:, None, None]
+        Y = _cell_avg_monomial(py, *ax[1])[None, :, None]
+        X = _cell_avg_monomial(px, *ax[2])[None, None, :]
+        out = out + a * Z * Y * X
+    return out
+
+
+def test_quartic_interpolation_reproduces_cell_averages_of_quartic_polynomials():
+    """The defining property (L780 "quartic polynomial conservative"): if the coarse values are the cell averages of a
+    polynomial of degree <= 4 per axis, every interpolated fine ghost cell is that polynomial's average over the fine
+    cell.  Distinct powers per axis catch a swapped axis or a mirrored left/right child; degree 5 is NOT reproduced."""
+    h0 = 1.0 / 16  # coordinates in [0, 1): keeps the monomials O(1)
+    o = two_level(h0=h0, lam=0.0, interp=4)
+    coefs = [(0.7, (4, 0, 0)), (-1.1, (0, 4, 0)), (0.9, (0, 0, 4)), (1.3, (3, 2, 1)), (-0.8, (1, 4, 2)), (0.5, (2, 1, 4)),
+             (2.0, (4, 4, 4)), (0.25, (0, 0, 0)), (-0.6, (1, 0, 3))]
+    o.set_state(0, 0, _poly_cell_averages(h0, (16, 16, 16), (0, 0, 0), coefs))
+    o.fill_ghosts(1, 0.0)
+    raw = o.get_raw(1, 0)
+    want = _poly_cell_averages(h0 / 2, o.box_shape(1), (8, 16, 8), coefs, g=3)
+    ghost = np.ones(raw.shape, dtype=bool)
+    ghost[3:-3, 3:-3, 3:-3] = False
+    assert np.abs(raw - want)[ghost].max() < 2e-15
+    # a quintic is not reproduced (the scheme is exactly quartic), and trilinear does not reproduce the quartic
+    o.set_state(0, 0, _poly_cell_averages(h0, (16, 16, 16), (0, 0, 0), [(1.0, (5, 0, 0))]))
+    o.fill_ghosts(1, 0.0)
+    want5 = _poly_cell_averages(h0 / 2, o.box_shape(1), (8, 16, 8), [(1.0, (5, 0, 0))], g=3)
+    assert 1e-9 < np.abs(o.get_raw(1, 0) - want5)[ghost].max() < 1e-5
+    o1 = two_level(h0=h0, lam=0.0)
+    o1.set_state(0, 0, _poly_cell_averages(h0, (16, 16, 16), (0, 0, 0), coefs))
+    o1.fill_ghosts(1, 0.0)
+    assert np.abs(o1.get_raw(1, 0) - want)[ghost].max() > 1e-4
+
+
+def test_quartic_interpolation_is_conservative_and_matches_a_numerical_polynomial_fit():
+    rng = np.random.default_rng(12)
+    g = 2  # two ghost layers = one whole coarse cell per face: every coarse cell in the shell has all 8 children there
+    o = two_level(g=g, h0=1.0, lam=0.0, interp=4)
+    coarse = [rng.normal(size=(16, 16, 16)) for _ in range(4)]
+    for c in range(4):
+        o.set_state(0, c, coarse[c])
+    o.fill_ghosts(1, 0.0)
+    lo = (8, 16, 8)  # fine lo (x, y, z); raw index (kz, jy, ix) <-> fine index lo - g + index
+    for c in range(4):
+        raw = o.get_raw(1, c)
+        nz, ny, nx = raw.shape
+        blocks = raw.reshape(nz // 2, 2, ny // 2, 2, nx // 2, 2).mean(axis=(1, 3, 5))
+        cz0, cy0, cx0 = (lo[2] - g) // 2, (lo[1] - g) // 2, (lo[0] - g) // 2
+        par = coarse[c][cz0:cz0 + nz // 2, cy0:cy0 + ny // 2, cx0:cx0 + nx // 2]
+        shell = np.ones(par.shape, dtype=bool)
+        shell[1:-1, 1:-1, 1:-1] = False
+        assert np.abs(blocks - par)[shell].max() < 4e-15  # conservative: the 8 children average to their parent
+    # data varying along ONE axis: the ghost value is the fine-cell average of the quartic fitted, numerically, to
+    # the five coarse cell averages around the parent (no weights typed in)
+    for axis in range(3):  # 0 = x
+        prof = rng.normal(size=16)
+        shape = [1, 1, 1]
+        shape[2 - axis] = 16
+        o.set_state(0, 0, np.broadcast_to(prof.reshape(shape), (16, 16, 16)).copy())
+        o.fill_ghosts(1, 0.0)
+        raw = o.get_raw(1, 0)
+        for fidx in (lo[axis] - 2, lo[axis] - 1):  # the two low-side ghost layers along this axis
+            c0, r = fidx // 2, fidx % 2
+            edges = np.arange(-2.5, 3.0, 1.0)
+            A = np.array([[_cell_avg_monomial(p, edges[m], edges[m + 1]) for p in range(5)] for m in range(5)])
+            coef = np.linalg.solve(A, prof[c0 - 2:c0 + 3])
+            a, b = (-0.5, 0.0) if r == 0 else (0.0, 0.5)
+            want = sum(coef[p] * _cell_avg_monomial(p, a, b) for p in range(5))
+            sl = [slice(g, g + 1)] * 3
+            sl[2 - axis] = slice(fidx - (lo[axis] - g), fidx - (lo[axis] - g) + 1)
+            assert abs(raw[tuple(sl)].item() - want) < 1e-13
+
+
+def test_quartic_interpolation_in_time_and_validation():
+    """same linear-in-time rule as the trilinear fill (L72): psi = b + c t stays exact through two coarse steps"""
+    o = two_level(h0=1.0, lam=0.0, order=2, interp=4)
+    b, c = 0.25, 0.5
+    for ib in (0, 1):
+        shp = o.box_shape(ib)
+        o.set_state(ib, 0, np.full(shp, b))
+        o.set_state(ib, 2, np.full(shp, c))
+    t, dt = 2.0, 0.5
+    for _ in range(2):
+        o.rk_step(dt, t)
+        t += dt
+    for ib in (0, 1):
+        assert np.abs(o.get_state(ib, 0) - (b + c * (t - 2.0))).max() < 1e-14
+    with pytest.raises(OracleError):
+        Oracle(16, interp=2)  # only trilinear (0) and quartic conservative (4) are built
