@@ -45,6 +45,8 @@ enum { SLEDGE_F32 = 0, SLEDGE_F64 = 1 };
 enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1, SLEDGE_RK_FUSED = 2 };
 
 /* Inclusive cell range lo..hi of one box in the index space of `level`; axis order x, y, z. */
+enum { SLEDGE_INTERP_TRILINEAR = 0, SLEDGE_INTERP_QUARTIC = 4 };
+
 typedef struct {
   int32_t level;
   int32_t lo[3];
@@ -74,6 +76,13 @@ typedef struct {
   int32_t ko_order;        /* r = sim.dissipation_order in {2,3} = ghost cells the term needs (L751): r <= nghost */
   int32_t integrator;      /* integrator.type (L808): 0 or 4 = classic RK4; 3 or 10 = SSPRK3 (Shu-Osher form,
                               three state buffers, 32 words per cell-step; rk_dataflow is ignored)      */
+  int32_t interp;          /* coarse->fine ghost interpolation (L70-72): SLEDGE_INTERP_TRILINEAR = cell-centred
+                              trilinear, weights 3/4, 1/4 per axis (BASELINE.json config 5); SLEDGE_INTERP_QUARTIC =
+                              amr.interpolation_type 4, the paper's default (L780): per axis the quartic matching the
+                              averages of the coarse cells c0-2..c0+2, averaged over the fine cell,
+                              c0 -+ (3 c[-2] - 22 c[-1] + 22 c[+1] - 3 c[+2])/128, tensor product; both linear in time.
+                              Quartic needs ceil(nghost/2) + 2 <= blocking_factor/2 on a multi-level hierarchy. */
+  int32_t reserved_;       /* 0 */
 } sledge_params;
 
 /* Size of the device arena needed for this hierarchy.  Host-only: validates params and boxes

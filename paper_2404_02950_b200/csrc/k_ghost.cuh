@@ -61,6 +61,10 @@ struct GhostArgs {
   int star_depth;  // plan: the Laplacian's radius R (L649).  Entries of ghost cells that a star stencil of that radius
                    // can reach -- outside the box along exactly ONE axis, by at most R -- carry GHOST_STAR
   int star_only;   // fill: move only GHOST_STAR entries (the fill before an RK sweep); 0 = every ghost cell
+  int quartic;     // coarse->fine interpolation: 0 = trilinear (2^3 parents), 1 = quartic conservative (5^3 parents
+                   // c0-2 .. c0+2 per axis; amr.interpolation_type 4, L70, L780).  Same entry formats: an INTERP entry
+                   // then means "all 5^3 parents in one coarse box", y = offset of the (c0,c0,c0) cell, and the sign
+                   // bits are r = f - 2 c0 per axis
 };
 
 __device__ __forceinline__ long long cell_offset(const BoxDev& b, int g, int ox, int i, int j, int k) {
@@ -212,6 +216,35 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
     return;
   }
   const int f[3] = {f0, f1, f2};
+  if (a.quartic) {
+    int c0[3], wl[3], wh[3];
+    bool unit = true;
+    unsigned rbits = 0u;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      c0[d] = floordiv2(f[d]);
+      rbits |= (unsigned)(f[d] - 2 * c0[d]) << d;
+      wl[d] = wrap1(c0[d] - 2, a.cgeom.n[d]);
+      wh[d] = wrap1(c0[d] + 2, a.cgeom.n[d]);
+      unit = unit && (wh[d] - wl[d] == 4);  // no periodic seam inside the 5-cell window
+    }
+    const int owl = owner_lookup(a.cowner, a.cgeom, wl[0], wl[1], wl[2]);
+    const int owh = owner_lookup(a.cowner, a.cgeom, wh[0], wh[1], wh[2]);
+    if (unit && owl >= 0 && owl == owh) {  // a box is convex: the whole window lies in it
+      const BoxDev cb = a.cboxes[owl];
+      const long long o0 = cell_offset(cb, a.cgeom.g, a.cgeom.ox, wl[0] + 2 - cb.lo[0], wl[1] + 2 - cb.lo[1], wl[2] + 2 - cb.lo[2]);
+      *out = make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (rbits << 2) | star);
+      return;
+    }
+    for (int mz = -2; mz <= 2; ++mz)
+      for (int my = -2; my <= 2; ++my)
+        for (int mx = -2; mx <= 2; ++mx)
+          if (owner_lookup(a.cowner, a.cgeom, wrap1(c0[0] + mx, a.cgeom.n[0]), wrap1(c0[1] + my, a.cgeom.n[1]),
+                           wrap1(c0[2] + mz, a.cgeom.n[2])) < 0)
+            *a.err_flag = 1;
+    *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW | star);
+    return;
+  }
   int c0[3], c1[3], w0[3], w1[3];
   bool unit = true;
 #pragma unroll
@@ -261,7 +294,90 @@ __device__ __forceinline__ void ghost_interp_entry(const GhostArgs<T>& a, const 
   if (FILL_PI) a.pi[en.x] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
 }
 
+// Quartic polynomial conservative interpolation (amr.interpolation_type 4, L70, L780): per axis the quartic whose
+// averages over the coarse cells c0-2 .. c0+2 are their values, averaged over the fine cell f = 2 c0 + r:
+//   r = 0: c0 + (-3 c[-2] + 22 c[-1] - 22 c[+1] + 3 c[+2]) / 128,   r = 1: the mirror image
+// tensor product over the axes, each coarse value linear in time between the coarse old and new states (L72).
+// Summed mz, my, mx (x fastest) from 0 with individually rounded operations.
+template <typename T>
+__device__ __forceinline__ T quartic_weight(int m, int r) {  // m = 0..4 <-> offset m - 2
+  const T b = (m == 2) ? T(1) : ((m == 0 || m == 4) ? T(3.0 / 128) : T(22.0 / 128));
+  const bool neg = (m == 0 || m == 3) != (r != 0);  // r = 0: -, +, 1, -, +
+  return (m != 2 && neg) ? -b : b;
+}
+
 template <typename T, bool FILL_PI>
+__device__ __forceinline__ void ghost_quartic_entry(const GhostArgs<T>& a, const uint4 en) {
+  using P = typename PairOf<T>::type;
+  const bool fast = (en.w & 3u) == GHOST_INTERP;
+  int r[3], c0[3] = {0, 0, 0};
+  long long base = 0, sx = 0, pl = 0;
+  if (fast) {
+    sx = en.z & 0xffffu;
+    pl = sx * (long long)(en.z >> 16);
+    base = (long long)en.y;
+    r[0] = (en.w >> 2) & 1;
+    r[1] = (en.w >> 3) & 1;
+    r[2] = (en.w >> 4) & 1;
+  } else {
+    const int g = a.geom.g;
+    const int f[3] = {(int)(en.y & 0xffffu) - g, (int)(en.y >> 16) - g, (int)en.z - g};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      c0[d] = floordiv2(f[d]);
+      r[d] = f[d] - 2 * c0[d];
+    }
+  }
+  const T oma = T(1) - a.alpha;
+  T s0 = T(0), s1 = T(0), t0 = T(0), t1 = T(0);
+#pragma unroll 1
+  for (int mz = 0; mz < 5; ++mz) {
+    const T wz = quartic_weight<T>(mz, r[2]);
+#pragma unroll 1
+    for (int my = 0; my < 5; ++my) {
+      const T wzy = wz * quartic_weight<T>(my, r[1]);
+      long long o[5];
+      if (fast) {
+#pragma unroll
+        for (int mx = 0; mx < 5; ++mx) o[mx] = base + (mz - 2) * pl + (my - 2) * sx + (mx - 2);
+      } else {
+        const int cj = wrap1(c0[1] + my - 2, a.cgeom.n[1]), ck = wrap1(c0[2] + mz - 2, a.cgeom.n[2]);
+#pragma unroll
+        for (int mx = 0; mx < 5; ++mx) {
+          const int ci = wrap1(c0[0] + mx - 2, a.cgeom.n[0]);
+          const int ow = owner_lookup(a.cowner, a.cgeom, ci, cj, ck);
+          if (ow < 0) return;  // reported by the plan
+          const BoxDev cb = a.cboxes[ow];
+          o[mx] = cell_offset(cb, a.cgeom.g, a.cgeom.ox, ci - cb.lo[0], cj - cb.lo[1], ck - cb.lo[2]);
+        }
+      }
+      P vo[5], vn[5], po[5], pn[5];
+#pragma unroll
+      for (int mx = 0; mx < 5; ++mx) {
+        vo[mx] = a.c_old_psi[o[mx]];
+        vn[mx] = a.c_new_psi[o[mx]];
+        if (FILL_PI) {
+          po[mx] = a.c_old_pi[o[mx]];
+          pn[mx] = a.c_new_pi[o[mx]];
+        }
+      }
+#pragma unroll
+      for (int mx = 0; mx < 5; ++mx) {
+        const T wt = wzy * quartic_weight<T>(mx, r[0]);
+        s0 += wt * (oma * vo[mx].x + a.alpha * vn[mx].x);
+        s1 += wt * (oma * vo[mx].y + a.alpha * vn[mx].y);
+        if (FILL_PI) {
+          t0 += wt * (oma * po[mx].x + a.alpha * pn[mx].x);
+          t1 += wt * (oma * po[mx].y + a.alpha * pn[mx].y);
+        }
+      }
+    }
+  }
+  a.psi[en.x] = mkpair(s0, s1);
+  if (FILL_PI) a.pi[en.x] = mkpair(t0, t1);
+}
+
+template <typename T, bool FILL_PI, bool QUARTIC = false>
 __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T> a) {
   using P = typename PairOf<T>::type;
   const unsigned e0 = blockIdx.x * (GHOST_THREADS * GHOST_EPT) + threadIdx.x;
@@ -288,7 +404,10 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_ghosts(const GhostArgs<T
 #pragma unroll
   for (int j = 0; j < GHOST_EPT; ++j) {
     const unsigned kind = en[j].w & 3u;
-    if (kind == GHOST_INTERP || kind == GHOST_SLOW) ghost_interp_entry<T, FILL_PI>(a, en[j]);
+    if (kind == GHOST_INTERP || kind == GHOST_SLOW) {
+      if (QUARTIC) ghost_quartic_entry<T, FILL_PI>(a, en[j]);
+      else ghost_interp_entry<T, FILL_PI>(a, en[j]);
+    }
   }
 }
 

@@ -197,6 +197,12 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   }
   if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10)
     return fail(nullptr, SLEDGE_EINVAL, "integrator must be 4 (RK4) or 3 / 10 (SSPRK3) (L808)");
+  if (p.interp != SLEDGE_INTERP_TRILINEAR && p.interp != SLEDGE_INTERP_QUARTIC)
+    return fail(nullptr, SLEDGE_EINVAL, "interp must be SLEDGE_INTERP_TRILINEAR (0) or SLEDGE_INTERP_QUARTIC (4) (L780)");
+  // the 5-cell window around the parent of the outermost ghost cell must stay inside the nesting gap of one
+  // blocking factor (L70: "we may not be able to set ghost cells ... because the domain might not extend far enough")
+  if (p.interp == SLEDGE_INTERP_QUARTIC && p.n_levels > 1 && (p.nghost + 1) / 2 + 2 > p.blocking_factor / 2)
+    return fail(nullptr, SLEDGE_EINVAL, "quartic interpolation: ceil(nghost/2) + 2 coarse cells exceed the nesting gap of blocking_factor/2 (L70)");
   if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
   if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
   if (!(p.h0 > 0)) return fail(nullptr, SLEDGE_EINVAL, "h0 must be positive");
@@ -421,6 +427,7 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.n_entries = (unsigned)L.ghost_prefix.back() * GHOST_THREADS;
   a.star_depth = stencil_radius(P.p);
   a.star_only = 0;
+  a.quartic = P.p.interp == SLEDGE_INTERP_QUARTIC ? 1 : 0;
   a.has_coarse = l > 0;
   a.alpha = T(0);
   if (l > 0) {
@@ -452,8 +459,13 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
   if (grid == 0) return SLEDGE_OK;
   {
     Timed t(c, KIND_GHOST);
-    if (fill_pi) k_fill_ghosts<T, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
-    else k_fill_ghosts<T, false><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+    if (a.quartic && l > 0) {
+      if (fill_pi) k_fill_ghosts<T, true, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+      else k_fill_ghosts<T, false, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+    } else {
+      if (fill_pi) k_fill_ghosts<T, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+      else k_fill_ghosts<T, false><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+    }
   }
   return check_launch(c, "k_fill_ghosts");
 }

@@ -43,6 +43,7 @@ class sledge_params(C.Structure):
         ("dtype", C.c_int32), ("lap_order", C.c_int32), ("eta_fixed", C.c_int32), ("rk_dataflow", C.c_int32),
         ("h0", C.c_double), ("lam", C.c_double), ("a_mass", C.c_double), ("friction", C.c_double),
         ("ko_strength", C.c_double * 4), ("ko_order", C.c_int32), ("integrator", C.c_int32),
+        ("interp", C.c_int32), ("reserved_", C.c_int32),
     ]
 
 
@@ -83,7 +84,7 @@ def lib():
 
 
 def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0, lam, a_mass, friction, eta_fixed,
-             rk_dataflow, ko_order=0, ko_strength=0.0, integrator=4):
+             rk_dataflow, ko_order=0, ko_strength=0.0, integrator=4, interp=0):
     if isinstance(n0, int):
         n0 = (n0,) * 3
     if boxes is None:
@@ -102,6 +103,7 @@ def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0,
     p.ko_strength[:] = [float(v) for v in ks]
     p.ko_order = ko_order
     p.integrator = integrator
+    p.interp = interp
     arr = (sledge_box * len(boxes))()
     for q, (l, lo, hi) in enumerate(boxes):
         arr[q].level = int(l)
@@ -112,10 +114,10 @@ def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0,
 
 def sledge_arena_bytes(n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, dtype="f64", lap_order=1, h0=1.0,
                        lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, rk_dataflow="lean", ko_order=0,
-                       ko_strength=0.0, integrator=4) -> int:
+                       ko_strength=0.0, integrator=4, interp=0) -> int:
     """Host-only: validates the parameters and the box list and returns the arena size (needs no GPU)."""
     p, arr, boxes, _ = _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0, lam, a_mass,
-                                friction, eta_fixed, rk_dataflow, ko_order, ko_strength, integrator)
+                                friction, eta_fixed, rk_dataflow, ko_order, ko_strength, integrator, interp)
     out = C.c_size_t(0)
     rc = lib().sledge_arena_bytes(C.byref(p), arr, len(boxes), C.byref(out))
     if rc != 0:
@@ -132,14 +134,14 @@ class Sledge:
 
     def __init__(self, n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, dtype="f64", lap_order=1, h0=1.0,
                  lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, rk_dataflow="lean", ko_order=0, ko_strength=0.0,
-                 integrator=4, device="cuda:0"):
+                 integrator=4, interp=0, device="cuda:0"):
         self._h = None
         L = lib()
         if not torch.cuda.is_available():
             raise SledgeError("no CUDA device: the sledge path has no CPU fallback")
         p, arr, self.boxes, self.n0 = _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0, lam,
                                                a_mass, friction, eta_fixed, rk_dataflow, ko_order, ko_strength,
-                                               integrator)
+                                               integrator, interp)
         self.n_levels, self.nghost, self.dtype = n_levels, nghost, dtype
         self.tdtype = torch.float64 if dtype == "f64" else torch.float32
         self.device = torch.device(device)

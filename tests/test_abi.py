@@ -62,11 +62,16 @@ def test_validation_rules_from_the_paper():
         dict(ok, h0=0.0),
         dict(ok, ko_order=3, ko_strength=0.01),    # dissipation order = ghost cells needed (L751): 3 > nghost
         dict(ok, ko_order=1, ko_strength=0.01),    # order is 2 or 3 (L751)
+        dict(ok, interp=2),                        # only trilinear (0) and quartic conservative (4, L780)
+        dict(ok, n_levels=2, nghost=5, lap_order=2, interp=4,  # ceil(5/2) + 2 > 8/2: window leaves the nesting gap (L70)
+             boxes=[(0, (0, 0, 0), (31, 31, 31)), (1, (16, 16, 16), (47, 47, 47))]),
         dict(ok, integrator=21),                   # RKN tableaux are not printed in the paper: not built
         dict(ok, ko_order=2, ko_strength=(0.0, -0.1, 0.0, 0.0)),  # strength in R+ (L749)
     ]
     S.sledge_arena_bytes(32, **dict(ok, ko_order=2, ko_strength=(0.0, 0.0, 0.02, 0.0)))
     S.sledge_arena_bytes(32, **dict(ok, integrator=10))
+    S.sledge_arena_bytes(32, **dict(ok, n_levels=2, nghost=3, interp=4,
+                                    boxes=[(0, (0, 0, 0), (31, 31, 31)), (1, (16, 16, 16), (47, 47, 47))]))
     S.sledge_arena_bytes(32, **dict(ok, ko_order=7, ko_strength=0.0))  # strength 0 removes the term, order unused
     for kw in bad:
         with pytest.raises(S.SledgeError):

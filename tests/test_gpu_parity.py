@@ -380,6 +380,97 @@ def test_ghost_fill_time_interpolation():
     s.synchronize()
 
 
+# ---- quartic polynomial conservative coarse->fine interpolation (amr.interpolation_type 4, L780; S8(f) NEXT-3) -----
+
+
+@pytest.mark.parametrize("g", [1, 2, 3])
+def test_quartic_ghost_fill_two_levels_matches_oracle_bitwise(g):
+    """5^3 parents per ghost cell, fast entries (window inside one coarse box) and the periodic / multi-box slow path;
+    same summation order and individually rounded operations on both sides -> identical bits"""
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=g, lap_order=1, h0=1.0, interp=4)
+    P.init_smooth(o, s, n0, seed=3)
+    for l in (0, 1):
+        o.fill_ghosts(l, 0.0)
+        s.fill_ghosts(l, 0.0)
+    s.synchronize()
+    for ib in range(len(boxes)):
+        for c in range(4):
+            a = o.get_raw(ib, c)
+            b = s.get_ghosted(ib, c).cpu().numpy()
+            assert np.array_equal(a, b), (ib, c)
+
+
+def test_quartic_differs_from_trilinear_on_the_gpu():
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    out = []
+    for interp in (0, 4):
+        o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=2, lap_order=1, h0=1.0, interp=interp)
+        P.init_smooth(o, s, n0, seed=3)
+        s.fill_ghosts(1, 0.0)
+        out.append(s.get_ghosted(1, 0).cpu().numpy())
+    assert np.abs(out[0] - out[1]).max() > 1e-4
+
+
+def test_quartic_ghost_fill_multibox_coarse_level_and_time_interpolation():
+    """coarse level cut into 8^3 boxes: every 5-cell window straddles boxes (slow entries only); then alpha in (0, 1)"""
+    P = _pair()
+    n0 = 32
+    boxes = [(0, lo, hi) for _, lo, hi in inputs.split_level0(n0, 8)] + P.two_level_boxes(n0)[1:]
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=3, lap_order=2, h0=0.5, interp=4)
+    P.init_smooth(o, s, n0, seed=4)
+    o.rk_step(0.1, 1.0)
+    s.rk_step(0.1, 1.0)
+    for time in (1.0, 1.025, 1.05, 1.1):
+        o.fill_ghosts(1, time)
+        s.fill_ghosts(1, time)
+        for ib in s.level_boxes(1):
+            for c in range(4):
+                a = o.get_raw(ib, c)
+                b = s.get_ghosted(ib, c).cpu().numpy()
+                assert np.abs(a - b).max() <= F64_TOL, (time, ib, c)
+    s.synchronize()
+
+
+@pytest.mark.parametrize("flow,integrator", [("fused", 4), ("lean", 4), ("lean", 10)])
+def test_quartic_three_level_subcycled(flow, integrator):
+    P = _pair()
+    n0 = 32
+    rings, boxes, _ = _ring_hierarchy(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.25, rk_dataflow=flow,
+                       integrator=integrator, interp=4)
+    for ib, (l, lo, hi) in enumerate(boxes):
+        re, im = inputs.ring_field(rings, l, lo, hi)
+        P.set_both(o, s, ib, 0, re.numpy())
+        P.set_both(o, s, ib, 1, im.numpy())
+    eta, dt = 2.0, 0.0625
+    for _ in range(2):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    for l in range(3):
+        _compare_tags(o, s, l)
+
+
+def test_quartic_fp32_two_level():
+    P = _pair()
+    n0 = 32
+    boxes = P.two_level_boxes(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=2, nghost=3, lap_order=2, h0=0.5, dtype="f32", interp=4)
+    P.init_smooth(o, s, n0, seed=9, comps=(0, 1))
+    eta, dt = 2.0, 0.1
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, relative=True) <= F32_TOL
+
+
 # ---- average-down ------------------------------------------------------------------------------------
 
 def test_average_down_matches_oracle_bitwise():
