@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--ko-order", type=int, default=0, choices=[0, 2, 3],
                     help="Kreiss-Oliger dissipation order (Eq.7); 0 = off, as in every BASELINE.json config")
     ap.add_argument("--ko-strength", type=float, default=0.01)
+    ap.add_argument("--interp", type=int, default=0, choices=[0, 4],
+                    help="coarse->fine ghost interpolation: 0 = trilinear (BASELINE.json config 5), 4 = quartic (L780)")
     ap.add_argument("--integrator", type=int, default=4, choices=[4, 3, 10],
                     help="integrator.type (L808): 4 = RK4 (every BASELINE.json config), 3 / 10 = SSPRK3")
     ap.add_argument("--no-e2e", action="store_true")
@@ -287,7 +289,7 @@ def run_sledge(args, cfg):
                  blocking_factor=cfg.blocking_factor,
                  dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=args.flow, device=dev,
                  ko_order=args.ko_order, ko_strength=args.ko_strength if args.ko_order else 0.0,
-                 integrator=args.integrator)
+                 integrator=args.integrator, interp=args.interp)
     ssp = args.integrator in (3, 10)
     if ssp:
         args.flow = "ssprk3"  # three staged sweeps, 8 + 12 + 12 words per cell-step
@@ -374,7 +376,8 @@ def run_sledge(args, cfg):
             "config": {"workload": f"{cfg.name}: {cfg.n0}^3 base, {cfg.n_levels} level(s), {cfg.dtype}, "
                                    f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, {'SSPRK3' if ssp else 'RK4'} ({args.flow} data-flow), "
                                    f"dt={cfg.dt}, h0={cfg.h0}, tags + 32^3 counts every step"
-                                   + (f", Kreiss-Oliger order {args.ko_order} eps {args.ko_strength}" if args.ko_order else ""),
+                                   + (f", Kreiss-Oliger order {args.ko_order} eps {args.ko_strength}" if args.ko_order else "")
+                                   + (", quartic conservative coarse->fine interpolation" if args.interp == 4 and cfg.n_levels > 1 else ""),
                        "cells_per_level": per_level, "coverage": cover, "cell_steps_per_step": cell_steps,
                        "l2": "state buffers >> 126 MB L2 (no flush needed)" if cell_steps * esz * 4 > 4e8 else
                              "state fits in L2 (small case; not a roofline workload)",

@@ -109,6 +109,8 @@ struct LevelHost {
   std::vector<int> owner;
   std::vector<TileDev> tiles, ftiles, tag_tiles;  // K1 staged / K1 fused / K3
   std::vector<int> ghost_prefix, avg_prefix;
+  std::vector<int> qp_prefix;  // quartic interpolation by coarse parent (k_fill_qparents): CTAs before box b
+  size_t off_qp_prefix = 0, off_qp_list = 0;
   long long plane_cells = 0;  // pairs per plane (all boxes, ghosts and padding included)
   long long valid_cells = 0;
   long long count_blocks = 0;
@@ -122,6 +124,9 @@ struct LevelHost {
   double tee_eps[4] = {0, 0, 0, 0};
   uint8_t* tee_tags = nullptr;
   uint32_t* tee_counts = nullptr;
+  // quartic interpolation reads coarse windows through the coarse boxes' ghost cells: true while the whole ghost
+  // shell of buffer b (psi and Pi) holds same-level copies of the buffer's current valid data
+  bool shell_ok[NBUF] = {false, false, false, false};
   // run state
   int cur = 0, old = 0;
   bool have_pair = false;
@@ -158,6 +163,9 @@ namespace {
 inline bool ko_on(const sledge_params& p) {
   return p.ko_strength[0] != 0.0 || p.ko_strength[1] != 0.0 || p.ko_strength[2] != 0.0 || p.ko_strength[3] != 0.0;
 }
+// quartic coarse->fine interpolation evaluated per coarse parent through the coarse boxes' ghost cells (needs two
+// coarse ghost layers); with one ghost layer the per-cell entries of k_fill_ghosts<.., QUARTIC> are used
+inline bool quartic_by_parent(const sledge_params& p) { return p.interp == SLEDGE_INTERP_QUARTIC && p.nghost >= 2; }
 inline int stencil_radius(const sledge_params& p) { return ko_on(p) && p.ko_order > p.lap_order ? p.ko_order : p.lap_order; }
 
 int fail(sledge_ctx* ctx, int code, const char* fmt, ...) {
@@ -296,6 +304,8 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
                      L.boxdev[0].n[2] == L.n[2];
     L.ghost_prefix.assign(1, 0);
     L.avg_prefix.assign(1, 0);
+    L.qp_prefix.assign(1, 0);
+    const bool qparents = quartic_by_parent(p) && l > 0;
     // z-chunk of the fused sweeps: long marches amortise the pipeline prologue, but the grid must stay many waves
     // deep (148 SMs x 2-3 CTAs); measured on C2 / C3 (profiles/r01_k1_tile_sweep.md)
     const int txc = K1_TX * cpt, ftxc = K1F_TX * cpt;
@@ -319,6 +329,11 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       L.ghost_prefix.push_back(L.ghost_prefix.back() + (int)((nghost + GHOST_THREADS - 1) / GHOST_THREADS));
       const long long ncoarse = (long long)(b.n[0] / 2) * (b.n[1] / 2) * (b.n[2] / 2);
       L.avg_prefix.push_back(L.avg_prefix.back() + (int)((ncoarse + AVG_THREADS - 1) / AVG_THREADS));
+      if (qparents) {  // parents of the ghost shell: the shell of thickness ceil(g/2) around the coarse footprint
+        const long long t = (g + 1) / 2, cx = b.n[0] / 2, cy = b.n[1] / 2, cz = b.n[2] / 2;
+        const long long npar = (cx + 2 * t) * (cy + 2 * t) * 2 * t + (cx + 2 * t) * 2 * t * cz + 2 * t * cy * cz;
+        L.qp_prefix.push_back(L.qp_prefix.back() + (int)((npar + GHOST_THREADS - 1) / GHOST_THREADS));
+      }
     }
   }
   // arena layout
@@ -341,6 +356,8 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.off_ghost_prefix = take(L.ghost_prefix.size() * sizeof(int));
     L.off_avg_prefix = take(L.avg_prefix.size() * sizeof(int));
     L.off_ghost_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
+    L.off_qp_prefix = take(L.qp_prefix.size() * sizeof(int));
+    L.off_qp_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
     // the ghost list (k_ghost.cuh) keeps cell offsets in 32 bits and pitches / indices in 16
     if (L.plane_cells >= (1LL << 32)) return fail(nullptr, SLEDGE_EINVAL, "level %d: more than 2^32 stored cells", l);
     for (const BoxDev& b : L.boxdev)
@@ -427,7 +444,11 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.n_entries = (unsigned)L.ghost_prefix.back() * GHOST_THREADS;
   a.star_depth = stencil_radius(P.p);
   a.star_only = 0;
-  a.quartic = P.p.interp == SLEDGE_INTERP_QUARTIC ? 1 : 0;
+  a.quartic = P.p.interp == SLEDGE_INTERP_QUARTIC ? (quartic_by_parent(P.p) ? 2 : 1) : 0;
+  a.copy_only = 0;
+  a.qblk_prefix = tab<int>(c, L.off_qp_prefix);
+  a.qlist = tab<uint4>(c, L.off_qp_list);
+  a.n_qentries = (unsigned)L.qp_prefix.back() * GHOST_THREADS;
   a.has_coarse = l > 0;
   a.alpha = T(0);
   if (l > 0) {
@@ -451,15 +472,38 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
 }
 
 // K2 on buffer `buf` of level l: streams the level's ghost list (built once by plan_ghosts)
+// Whole ghost shell of buffer `buf` of level l <- same-level / periodic copies (psi and Pi), no interpolation.
+template <typename T>
+int fill_shell_copies(sledge_ctx* c, int l, int buf) {
+  LevelHost& L = c->plan.lev[l];
+  if (L.shell_ok[buf & 3]) return SLEDGE_OK;
+  GhostArgs<T> a = ghost_args<T>(c, l, buf, 0.0);
+  a.copy_only = 1;
+  const int grid = (L.ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
+  if (grid > 0) {
+    Timed t(c, KIND_GHOST);
+    k_fill_ghosts<T, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+  }
+  L.shell_ok[buf & 3] = true;
+  return check_launch(c, "k_fill_ghosts (coarse shell)");
+}
+
 template <typename T>
 int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false) {
   GhostArgs<T> a = ghost_args<T>(c, l, buf, time);
+  if (a.quartic == 2 && l > 0) {  // the coarse windows are read through the coarse boxes' ghost cells
+    LevelHost& C = c->plan.lev[l - 1];
+    const bool pair = C.have_pair && C.t_new != C.t_old;
+    int rc = fill_shell_copies<T>(c, l - 1, C.cur);
+    if (rc == SLEDGE_OK && pair) rc = fill_shell_copies<T>(c, l - 1, C.old);
+    if (rc) return rc;
+  }
   a.star_only = star_only ? 1 : 0;  // before an RK sweep only the cells its star stencil reaches are needed
   const int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
   if (grid == 0) return SLEDGE_OK;
   {
     Timed t(c, KIND_GHOST);
-    if (a.quartic && l > 0) {
+    if (a.quartic == 1 && l > 0) {
       if (fill_pi) k_fill_ghosts<T, true, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
       else k_fill_ghosts<T, false, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
     } else {
@@ -467,7 +511,16 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
       else k_fill_ghosts<T, false><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
     }
   }
-  return check_launch(c, "k_fill_ghosts");
+  int rc = check_launch(c, "k_fill_ghosts");
+  if (rc) return rc;
+  const int qgrid = c->plan.lev[l].qp_prefix.back();
+  if (a.quartic == 2 && l > 0 && qgrid > 0) {  // the interpolated cells, one thread per coarse parent
+    Timed t(c, KIND_GHOST);
+    if (fill_pi) k_fill_qparents<T, true><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+    else k_fill_qparents<T, false><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+    rc = check_launch(c, "k_fill_qparents");
+  }
+  return rc;
 }
 
 // create-time: resolve every ghost cell of level l into its list entry
@@ -477,7 +530,13 @@ int plan_ghosts(sledge_ctx* c, int l) {
   const int grid = c->plan.lev[l].ghost_prefix.back();
   if (grid == 0) return SLEDGE_OK;
   k_plan_ghosts<T><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
-  return check_launch(c, "k_plan_ghosts");
+  int rc = check_launch(c, "k_plan_ghosts");
+  const int qgrid = c->plan.lev[l].qp_prefix.back();
+  if (rc == SLEDGE_OK && qgrid > 0) {
+    k_plan_qparents<T><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+    rc = check_launch(c, "k_plan_qparents");
+  }
+  return rc;
 }
 
 template <typename T, int ORDER, int MODE, int KO = 0>
@@ -555,6 +614,7 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   const double h2 = L.h * L.h;
   a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : (P.p.lap_order == 2 ? 1.0 / (12.0 * h2) : 1.0 / (180.0 * h2)));
   a.a_mass = (T)P.p.a_mass;
+  for (int b = 0; b < NBUF; ++b) L.shell_ok[b] = false;  // a sweep rewrites valid cells of this level's buffers
   const int ko = ko_on(P.p) ? P.p.ko_order : 0;
   if (ko) {  // Eq.7: (-1)^(r+1) eps / (2^(2r) h_l); Pi(U) is differenced too and moves from pnt[0] to sten[1]
     const double sgn = (ko % 2 == 0) ? -1.0 : 1.0;
@@ -749,6 +809,7 @@ int do_average_down(sledge_ctx* c, int lf) {
   a.c_pi = plane_ptr<T>(c, lf - 1, C.cur, 1);
   a.err_flag = tab<int>(c, P.off_err);
   const int grid = F.avg_prefix.back();
+  C.shell_ok[C.cur & 3] = false;  // covered coarse cells change: ghost copies of them are stale
   if (F.tee_on) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
     for (int q = 0; q < 4; ++q) a.tee_eps[q] = (T)F.tee_eps[q];
     a.tee_tags = F.tee_tags;
@@ -825,6 +886,7 @@ int do_copy_comp(sledge_ctx* c, int ib, int comp, void* dense, bool to_state, bo
   const long long total = (long long)(b.n[0] + 2 * e) * (b.n[1] + 2 * e) * (b.n[2] + 2 * e);
   const int grid = (int)std::min<long long>((total + 255) / 256, 148 * 32);
   auto* pl = plane_ptr<T>(c, l, L.cur, comp >> 1);
+  if (to_state) L.shell_ok[L.cur & 3] = false;
   ++c->launches;
   if (to_state) k_copy_comp<T, true><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
   else k_copy_comp<T, false><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
@@ -885,6 +947,7 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     up(L.off_owner, L.owner.data(), L.owner.size() * sizeof(int));
     up(L.off_ghost_prefix, L.ghost_prefix.data(), L.ghost_prefix.size() * sizeof(int));
     up(L.off_avg_prefix, L.avg_prefix.data(), L.avg_prefix.size() * sizeof(int));
+    up(L.off_qp_prefix, L.qp_prefix.data(), L.qp_prefix.size() * sizeof(int));
   }
   // ghost lists: resolved on the device from the tables just uploaded (the plan kernel of level l reads the
   // tables of l and l-1 only); its launches do not count as hot-path launches

@@ -385,8 +385,9 @@ def test_ghost_fill_time_interpolation():
 
 @pytest.mark.parametrize("g", [1, 2, 3])
 def test_quartic_ghost_fill_two_levels_matches_oracle_bitwise(g):
-    """5^3 parents per ghost cell, fast entries (window inside one coarse box) and the periodic / multi-box slow path;
-    same summation order and individually rounded operations on both sides -> identical bits"""
+    """5^3 parents per ghost cell.  g = 1: fast entries (window inside one coarse box) and the periodic / multi-box slow
+    path; g >= 2: windows read through the coarse boxes' ghost cells.  Same summation order and individually rounded
+    operations on both sides -> identical bits"""
     P = _pair()
     n0 = 32
     boxes = P.two_level_boxes(n0)
