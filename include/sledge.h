@@ -105,8 +105,9 @@ int sledge_get_state(sledge_ctx* ctx, int box, int comp, void* dev_dst);
  * (cudaMemcpyAsync on the context stream; truly asynchronous only for pinned memory). */
 int sledge_set_state_host(sledge_ctx* ctx, int box, int comp, const void* host_src);
 int sledge_get_state_host(sledge_ctx* ctx, int box, int comp, void* host_dst);
-/* One component of one box INCLUDING ghosts: (nx+2g)*(ny+2g)*(nz+2g) reals, x fastest.  Only psi1,
- * psi2 ghosts are ever filled (Pi is never differenced, R10). */
+/* One component of one box INCLUDING ghosts: (nx+2g)*(ny+2g)*(nz+2g) reals, x fastest.  Ghost values are those of
+ * the last fill that touched them: sledge_fill_ghosts fills every ghost cell of all four components; the fills
+ * inside a step move psi only unless Pi is differenced (FUSED sweeps, Kreiss-Oliger term), R10. */
 int sledge_get_ghosted(sledge_ctx* ctx, int box, int comp, void* dev_dst);
 
 /* Ghost fill of the CURRENT state of `level` (L68-74): every psi ghost cell <- the valid cell of the
@@ -116,7 +117,9 @@ int sledge_get_ghosted(sledge_ctx* ctx, int box, int comp, void* dev_dst);
  * level has not stepped since its state was set).  This explicit call fills EVERY ghost cell (psi and Pi).
  * The fills that sledge_rk_step / sledge_rk_stage issue themselves move only the ghost cells the Laplacian's star
  * stencil reaches (outside the box along one axis, by at most lap_order), and none at all on a level that is one
- * box over the periodic domain (the kernels read the wrapped cell directly), so after a step the ghost contents
+ * box over the periodic domain (the kernels read the wrapped cell directly); with quartic interpolation and
+ * nghost >= 2 a fill of level l > 0 first refreshes, where stale, the whole ghost shell of level l-1's old and new
+ * states with same-level copies (the 5^3 windows are read through them).  So after a step the ghost contents
  * are unspecified until this function is called. */
 int sledge_fill_ghosts(sledge_ctx* ctx, int level, double time);
 
