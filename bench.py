@@ -60,6 +60,7 @@ def parse():
     ap.add_argument("--integrator", type=int, default=4, choices=[4, 3, 10],
                     help="integrator.type (L808): 4 = RK4 (every BASELINE.json config), 3 / 10 = SSPRK3")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="skip the C1 CUDA-graph replay leg")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     return ap.parse_args()
@@ -390,12 +391,97 @@ def run_sledge(args, cfg):
         line["e2e"] = e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags=(tags, counts))
     del s
     torch.cuda.empty_cache()
+    if rank == 0 and not args.no_graph and args.integrator == 4 and not args.ko_order:
+        from paper_2404_02950_b200 import inputs as _inputs
+        line["c1_graph_replay"] = graph_leg(_inputs.CONFIGS["C1"], dev, "fused")
     if rank == 0 and not args.no_cpu:
         line["cpu_baseline"], _, _ = time_oracle(cfg)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------------
+# C1 under CUDA Graph replay (the 32^3 case is launch-bound)
+# ---------------------------------------------------------------------------------------------------
+
+def capture_run(s, ic, tags, counts, steps, dt, eta0):
+    """Capture `restore the initial state + steps x (sledge_rk_step + sledge_tag_strings)` of a single-level context
+    into ONE CUDA graph on the context's stream.  Every library call is an asynchronous launch on that stream (no
+    allocation, no host synchronisation), eta enters as kernel arguments, so the whole run replays with one launch.
+    The context must have run the same sequence once eagerly (first launches set kernel attributes)."""
+    import torch
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s.stream):
+        for c, t in enumerate(ic):
+            s.set_state(0, c, t)
+        eta = eta0
+        for _ in range(steps):
+            s.rk_step(dt, eta)
+            eta += dt
+            s.tag_strings(0, tags, counts)
+    return g
+
+
+def graph_leg(cfg, dev, flow, replays=20, dt=None):
+    """The C1 run (10 steps of 32^3) eagerly and as one CUDA graph replay: ms per step of both."""
+    import torch
+    from paper_2404_02950_b200 import inputs
+    from paper_2404_02950_b200 import sledge as S
+    dt = cfg.dt if dt is None else dt
+    side = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(side):  # the context adopts torch's current stream: capture needs a non-default one
+        s = S.Sledge(cfg.n0, nghost=cfg.nghost, dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam,
+                     rk_dataflow=flow, device=dev)
+        ic = [inputs.grf(cfg.n0, cfg.grf_f, seed, device=dev, dtype=s.tdtype).contiguous() for seed in cfg.seeds]
+        ic += [torch.zeros_like(ic[0]), torch.zeros_like(ic[0])]
+        tags = torch.empty(s.level_cells(0)[0], dtype=torch.uint8, device=dev)
+        counts = torch.empty(s.count_shape(0), dtype=torch.int32, device=dev)
+
+        def eager():
+            for c, t in enumerate(ic):
+                s.set_state(0, c, t)
+            eta = cfg.eta0
+            for _ in range(cfg.steps):
+                s.rk_step(dt, eta)
+                eta += dt
+                s.tag_strings(0, tags, counts)
+
+        eager()
+        side.synchronize()
+        l0 = s.launch_count()
+        eager()
+        per_run = s.launch_count() - l0
+        ref = [s.get_state(0, c).clone() for c in range(4)]
+        ref_tags = tags.clone()
+        g = capture_run(s, ic, tags, counts, cfg.steps, dt, cfg.eta0)
+
+        def timed(fn):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(3):
+                fn()
+            side.synchronize()
+            e0.record(side)
+            for _ in range(replays):
+                fn()
+            e1.record(side)
+            side.synchronize()
+            return e0.elapsed_time(e1) / (replays * cfg.steps)
+
+        ms_eager = timed(eager)
+        ms_graph = timed(g.replay)
+        got = [s.get_state(0, c) for c in range(4)]
+        side.synchronize()
+        same = all(torch.equal(a.view(torch.int64), b.view(torch.int64)) for a, b in zip(ref, got)) and \
+            torch.equal(ref_tags, tags)
+        s.close()
+    cells = cfg.n0 ** 3
+    return {"workload": f"{cfg.name}: {cfg.n0}^3 {cfg.dtype}, {cfg.steps} steps + tags, {flow} data-flow; the graph also "
+                        "restores the initial state (4 copy kernels)",
+            "launches_per_run": per_run, "ms_per_step_eager": ms_eager, "ms_per_step_graph": ms_graph,
+            "value_eager": cells * 4 / (ms_eager * 1e-3) / 1e9, "value_graph": cells * 4 / (ms_graph * 1e-3) / 1e9,
+            "unit": UNIT, "replay_equals_eager_bitwise": bool(same)}
 
 
 def e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags):

@@ -686,3 +686,16 @@ def test_create_rejects_bad_arena():
     buf = torch.empty(1024, dtype=torch.uint8, device="cuda")
     rc = S.lib().sledge_create(C.byref(h), C.byref(p), arr, 1, buf.data_ptr(), 1024, None)
     assert rc == -2 and b"arena" in S.lib().sledge_last_error(None)
+
+
+def test_c1_run_as_one_cuda_graph_replays_bit_for_bit():
+    """C1 additionally under CUDA Graph replay.  The stabilised C1 run (dt = 0.0625) captured into one
+    graph (restore + 10 x (rk_step + tag_strings)) reproduces the eager run bit for bit, fields and tags."""
+    import bench
+    cfg = inputs.CONFIGS["C1"]
+    for flow in ("fused", "lean"):
+        r = bench.graph_leg(cfg, "cuda:0", flow, replays=3, dt=0.0625)
+        assert r["replay_equals_eager_bitwise"], flow
+        assert r["launches_per_run"] >= 4 + 3 * cfg.steps
+        assert r["ms_per_step_graph"] > 0
+
