@@ -544,14 +544,18 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs
           q0 = oma * po[mx].x + a.alpha * pn[mx].x;
           q1 = oma * po[mx].y + a.alpha * pn[mx].y;
         }
+        // the weights of the 8 children differ by exact sign flips only (the r = 1 table is the mirror image:
+        // w(m, 1) = -w(m, 0) for m != 2), and rounding is symmetric: one product per value, then +- per child
+        const T w0 = (quartic_weight<T>(mz, 0) * quartic_weight<T>(my, 0)) * quartic_weight<T>(mx, 0);
+        const T t0 = w0 * c0, t1 = w0 * c1, u0 = w0 * q0, u1 = w0 * q1;
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
-          const T wt = (quartic_weight<T>(mz, c >> 2) * quartic_weight<T>(my, (c >> 1) & 1)) * quartic_weight<T>(mx, c & 1);
-          s[c][0] += wt * c0;
-          s[c][1] += wt * c1;
+          const bool neg = (((c >> 2) & 1) && mz != 2) != ((((c >> 1) & 1) && my != 2) != ((c & 1) && mx != 2));
+          s[c][0] += neg ? -t0 : t0;
+          s[c][1] += neg ? -t1 : t1;
           if (FILL_PI) {
-            p[c][0] += wt * q0;
-            p[c][1] += wt * q1;
+            p[c][0] += neg ? -u0 : u0;
+            p[c][1] += neg ? -u1 : u1;
           }
         }
       }

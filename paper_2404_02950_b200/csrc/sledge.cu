@@ -126,7 +126,7 @@ struct LevelHost {
   uint32_t* tee_counts = nullptr;
   // quartic interpolation reads coarse windows through the coarse boxes' ghost cells: true while the whole ghost
   // shell of buffer b (psi and Pi) holds same-level copies of the buffer's current valid data
-  bool shell_ok[NBUF] = {false, false, false, false};
+  int shell_ok[NBUF] = {0, 0, 0, 0};  // 0 = stale, 1 = psi shell valid, 2 = psi and Pi
   // run state
   int cur = 0, old = 0;
   bool have_pair = false;
@@ -474,17 +474,19 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
 // K2 on buffer `buf` of level l: streams the level's ghost list (built once by plan_ghosts)
 // Whole ghost shell of buffer `buf` of level l <- same-level / periodic copies (psi and Pi), no interpolation.
 template <typename T>
-int fill_shell_copies(sledge_ctx* c, int l, int buf) {
+int fill_shell_copies(sledge_ctx* c, int l, int buf, bool with_pi) {
   LevelHost& L = c->plan.lev[l];
-  if (L.shell_ok[buf & 3]) return SLEDGE_OK;
+  const int need = with_pi ? 2 : 1;
+  if (L.shell_ok[buf & 3] >= need) return SLEDGE_OK;
   GhostArgs<T> a = ghost_args<T>(c, l, buf, 0.0);
   a.copy_only = 1;
   const int grid = (L.ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
   if (grid > 0) {
     Timed t(c, KIND_GHOST);
-    k_fill_ghosts<T, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+    if (with_pi) k_fill_ghosts<T, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
+    else k_fill_ghosts<T, false><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
   }
-  L.shell_ok[buf & 3] = true;
+  L.shell_ok[buf & 3] = need;
   return check_launch(c, "k_fill_ghosts (coarse shell)");
 }
 
@@ -494,8 +496,8 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
   if (a.quartic == 2 && l > 0) {  // the coarse windows are read through the coarse boxes' ghost cells
     LevelHost& C = c->plan.lev[l - 1];
     const bool pair = C.have_pair && C.t_new != C.t_old;
-    int rc = fill_shell_copies<T>(c, l - 1, C.cur);
-    if (rc == SLEDGE_OK && pair) rc = fill_shell_copies<T>(c, l - 1, C.old);
+    int rc = fill_shell_copies<T>(c, l - 1, C.cur, fill_pi);
+    if (rc == SLEDGE_OK && pair) rc = fill_shell_copies<T>(c, l - 1, C.old, fill_pi);
     if (rc) return rc;
   }
   a.star_only = star_only ? 1 : 0;  // before an RK sweep only the cells its star stencil reaches are needed
@@ -614,7 +616,7 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   const double h2 = L.h * L.h;
   a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : (P.p.lap_order == 2 ? 1.0 / (12.0 * h2) : 1.0 / (180.0 * h2)));
   a.a_mass = (T)P.p.a_mass;
-  for (int b = 0; b < NBUF; ++b) L.shell_ok[b] = false;  // a sweep rewrites valid cells of this level's buffers
+  for (int b = 0; b < NBUF; ++b) L.shell_ok[b] = 0;  // a sweep rewrites valid cells of this level's buffers
   const int ko = ko_on(P.p) ? P.p.ko_order : 0;
   if (ko) {  // Eq.7: (-1)^(r+1) eps / (2^(2r) h_l); Pi(U) is differenced too and moves from pnt[0] to sten[1]
     const double sgn = (ko % 2 == 0) ? -1.0 : 1.0;
@@ -809,7 +811,7 @@ int do_average_down(sledge_ctx* c, int lf) {
   a.c_pi = plane_ptr<T>(c, lf - 1, C.cur, 1);
   a.err_flag = tab<int>(c, P.off_err);
   const int grid = F.avg_prefix.back();
-  C.shell_ok[C.cur & 3] = false;  // covered coarse cells change: ghost copies of them are stale
+  C.shell_ok[C.cur & 3] = 0;  // covered coarse cells change: ghost copies of them are stale
   if (F.tee_on) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
     for (int q = 0; q < 4; ++q) a.tee_eps[q] = (T)F.tee_eps[q];
     a.tee_tags = F.tee_tags;
@@ -886,7 +888,7 @@ int do_copy_comp(sledge_ctx* c, int ib, int comp, void* dense, bool to_state, bo
   const long long total = (long long)(b.n[0] + 2 * e) * (b.n[1] + 2 * e) * (b.n[2] + 2 * e);
   const int grid = (int)std::min<long long>((total + 255) / 256, 148 * 32);
   auto* pl = plane_ptr<T>(c, l, L.cur, comp >> 1);
-  if (to_state) L.shell_ok[L.cur & 3] = false;
+  if (to_state) L.shell_ok[L.cur & 3] = 0;
   ++c->launches;
   if (to_state) k_copy_comp<T, true><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
   else k_copy_comp<T, false><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
