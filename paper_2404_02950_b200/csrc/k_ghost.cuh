@@ -54,6 +54,9 @@ struct GhostArgs {
   const P* c_old_pi;
   const P* c_new_pi;
   T alpha;
+  int single;      // alpha is exactly 0 or 1 (or the coarse level has one state only): c_old == c_new point at the one
+                   // buffer that counts; k_fill_qparents then skips the blend (1-alpha) old + alpha new, which would
+                   // return it unchanged, together with the second load (the per-cell paths blend as usual: same bits)
   int has_coarse;
   int* err_flag;  // set to 1 if a ghost cell has neither a same-level owner nor coarse data
   GhostEntry* list;  // GHOST_THREADS entries per CTA of the enumeration (written by the plan, read by the fill)
@@ -505,7 +508,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_qparents(const GhostArgs
   out[1] = make_uint4(mask | (smask << 8), 0u, 0u, 0u);
 }
 
-template <typename T, bool FILL_PI>
+template <typename T, bool FILL_PI, bool SINGLE>
 __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs<T> a) {
   using P = typename PairOf<T>::type;
   const unsigned e = blockIdx.x * GHOST_THREADS + threadIdx.x;
@@ -530,19 +533,20 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs
 #pragma unroll
       for (int mx = 0; mx < 5; ++mx) {
         vo[mx] = a.c_old_psi[row + mx];
-        vn[mx] = a.c_new_psi[row + mx];
+        if (!SINGLE) vn[mx] = a.c_new_psi[row + mx];
         if (FILL_PI) {
           po[mx] = a.c_old_pi[row + mx];
-          pn[mx] = a.c_new_pi[row + mx];
+          if (!SINGLE) pn[mx] = a.c_new_pi[row + mx];
         }
       }
 #pragma unroll
       for (int mx = 0; mx < 5; ++mx) {
-        const T c0 = oma * vo[mx].x + a.alpha * vn[mx].x, c1 = oma * vo[mx].y + a.alpha * vn[mx].y;
+        const T c0 = SINGLE ? vo[mx].x : oma * vo[mx].x + a.alpha * vn[mx].x;
+        const T c1 = SINGLE ? vo[mx].y : oma * vo[mx].y + a.alpha * vn[mx].y;
         T q0 = T(0), q1 = T(0);
         if (FILL_PI) {
-          q0 = oma * po[mx].x + a.alpha * pn[mx].x;
-          q1 = oma * po[mx].y + a.alpha * pn[mx].y;
+          q0 = SINGLE ? po[mx].x : oma * po[mx].x + a.alpha * pn[mx].x;
+          q1 = SINGLE ? po[mx].y : oma * po[mx].y + a.alpha * pn[mx].y;
         }
         // the weights of the 8 children differ by exact sign flips only (the r = 1 table is the mirror image:
         // w(m, 1) = -w(m, 0) for m != 2), and rounding is symmetric: one product per value, then +- per child

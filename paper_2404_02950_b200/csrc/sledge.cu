@@ -463,6 +463,10 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
       bo = C.old;
     }
     a.alpha = (T)alpha;
+    // alpha exactly 0 or 1 (first / last stage of a fine step pair, the fill before tagging) or a coarse level
+    // with one state only: the blend returns one of the two buffers unchanged, so only that one is read
+    if (bo == bn || alpha == 0.0) { bn = bo; a.single = 1; }
+    else if (alpha == 1.0) { bo = bn; a.single = 1; }
     a.c_old_psi = plane_ptr<T>(c, l - 1, bo, 0);
     a.c_new_psi = plane_ptr<T>(c, l - 1, bn, 0);
     a.c_old_pi = plane_ptr<T>(c, l - 1, bo, 1);
@@ -518,8 +522,13 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
   const int qgrid = c->plan.lev[l].qp_prefix.back();
   if (a.quartic == 2 && l > 0 && qgrid > 0) {  // the interpolated cells, one thread per coarse parent
     Timed t(c, KIND_GHOST);
-    if (fill_pi) k_fill_qparents<T, true><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
-    else k_fill_qparents<T, false><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+    if (a.single) {
+      if (fill_pi) k_fill_qparents<T, true, true><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+      else k_fill_qparents<T, false, true><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+    } else {
+      if (fill_pi) k_fill_qparents<T, true, false><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+      else k_fill_qparents<T, false, false><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+    }
     rc = check_launch(c, "k_fill_qparents");
   }
   return rc;
