@@ -76,6 +76,8 @@ struct GhostArgs {
   const int* qblk_prefix;  // nbox + 1 entries, CTAs of the parent enumeration before box b
   uint4* qlist;            // 2 x uint4 per slot
   unsigned n_qentries;
+  uint4* qstar_list;       // plan: the parents with star children, packed (order = order of arrival); the fills before
+  unsigned* qstar_count;   //       an RK sweep run over this list only, with every lane busy
 };
 
 __device__ __forceinline__ long long cell_offset(const BoxDev& b, int g, int ox, int i, int j, int k) {
@@ -504,8 +506,15 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_qparents(const GhostArgs
   const BoxDev cb = a.cboxes[owc];
   const long long o0 = cell_offset(cb, a.cgeom.g, a.cgeom.ox, wc[0] - cb.lo[0], wc[1] - cb.lo[1], wc[2] - cb.lo[2]);
   const long long d0 = cell_offset(b, g, a.geom.ox, 2 * I, 2 * J, 2 * K);
-  out[0] = make_uint4((unsigned)d0, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)b.sx | ((unsigned)b.sy << 16));
-  out[1] = make_uint4(mask | (smask << 8), 0u, 0u, 0u);
+  const uint4 ea = make_uint4((unsigned)d0, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)b.sx | ((unsigned)b.sy << 16));
+  const uint4 eb = make_uint4(mask | (smask << 8), 0u, 0u, 0u);
+  out[0] = ea;
+  out[1] = eb;
+  if (smask) {
+    const unsigned idx = atomicAdd(a.qstar_count, 1u);
+    a.qstar_list[2 * (size_t)idx] = ea;
+    a.qstar_list[2 * (size_t)idx + 1] = eb;
+  }
 }
 
 template <typename T, bool FILL_PI, bool SINGLE>

@@ -110,7 +110,8 @@ struct LevelHost {
   std::vector<TileDev> tiles, ftiles, tag_tiles;  // K1 staged / K1 fused / K3
   std::vector<int> ghost_prefix, avg_prefix;
   std::vector<int> qp_prefix;  // quartic interpolation by coarse parent (k_fill_qparents): CTAs before box b
-  size_t off_qp_prefix = 0, off_qp_list = 0;
+  size_t off_qp_prefix = 0, off_qp_list = 0, off_qs_list = 0, off_qs_count = 0;
+  unsigned n_star_parents = 0;  // read back from the device after the plan
   long long plane_cells = 0;  // pairs per plane (all boxes, ghosts and padding included)
   long long valid_cells = 0;
   long long count_blocks = 0;
@@ -358,6 +359,8 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.off_ghost_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
     L.off_qp_prefix = take(L.qp_prefix.size() * sizeof(int));
     L.off_qp_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
+    L.off_qs_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
+    L.off_qs_count = take(sizeof(unsigned));
     // the ghost list (k_ghost.cuh) keeps cell offsets in 32 bits and pitches / indices in 16
     if (L.plane_cells >= (1LL << 32)) return fail(nullptr, SLEDGE_EINVAL, "level %d: more than 2^32 stored cells", l);
     for (const BoxDev& b : L.boxdev)
@@ -449,6 +452,8 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.qblk_prefix = tab<int>(c, L.off_qp_prefix);
   a.qlist = tab<uint4>(c, L.off_qp_list);
   a.n_qentries = (unsigned)L.qp_prefix.back() * GHOST_THREADS;
+  a.qstar_list = tab<uint4>(c, L.off_qs_list);
+  a.qstar_count = tab<unsigned>(c, L.off_qs_count);
   a.has_coarse = l > 0;
   a.alpha = T(0);
   if (l > 0) {
@@ -519,7 +524,12 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
   }
   int rc = check_launch(c, "k_fill_ghosts");
   if (rc) return rc;
-  const int qgrid = c->plan.lev[l].qp_prefix.back();
+  int qgrid = c->plan.lev[l].qp_prefix.back();
+  if (a.quartic == 2 && l > 0 && qgrid > 0 && star_only) {  // only the parents with star children, packed
+    a.qlist = a.qstar_list;
+    a.n_qentries = c->plan.lev[l].n_star_parents;
+    qgrid = (int)((a.n_qentries + GHOST_THREADS - 1) / GHOST_THREADS);
+  }
   if (a.quartic == 2 && l > 0 && qgrid > 0) {  // the interpolated cells, one thread per coarse parent
     Timed t(c, KIND_GHOST);
     if (a.single) {
@@ -975,6 +985,9 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   }
   // the tables above are pageable host memory: make sure the copies are done before they can go away
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  for (int l = 1; l < P.p.n_levels && e == cudaSuccess; ++l)
+    if (P.lev[l].qp_prefix.back() > 0)
+      e = cudaMemcpy(&P.lev[l].n_star_parents, c->arena + P.lev[l].off_qs_count, sizeof(unsigned), cudaMemcpyDeviceToHost);
   if (e != cudaSuccess) {
     rc = fail(nullptr, SLEDGE_ECUDA, "sledge_create: %s", cudaGetErrorString(e));
     delete c;
