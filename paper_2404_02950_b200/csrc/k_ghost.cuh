@@ -76,6 +76,8 @@ struct GhostArgs {
   const int* qblk_prefix;  // nbox + 1 entries, CTAs of the parent enumeration before box b
   uint4* qlist;            // 2 x uint4 per slot
   unsigned n_qentries;
+  GhostEntry* star_list;   // plan: the GHOST_STAR entries of `list`, packed; n_star of them (read back by the host)
+  unsigned* star_count;
   uint4* qstar_list;       // plan: the parents with star children, packed (order = order of arrival); the fills before
   unsigned* qstar_count;   //       an RK sweep run over this list only, with every lane busy
 };
@@ -168,6 +170,12 @@ __device__ __forceinline__ void parents_of(int f, int& c0, int& c1) {
 template <typename T>
 __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T> a) {
   GhostEntry* const out = a.list + (size_t)blockIdx.x * GHOST_THREADS + threadIdx.x;
+  // every entry goes to its slot of the full list; those a star stencil reaches are also appended to the packed
+  // star list (order of arrival), which is what the fills before an RK sweep stream
+  auto emit = [&](const uint4 e) {
+    *out = e;
+    if ((e.w & GHOST_STAR) && (e.w & 3u) != GHOST_NONE) a.star_list[atomicAdd(a.star_count, 1u)] = e;
+  };
   // blockIdx.x -> box
   int lo_b = 0, hi_b = a.nbox;
   const int blk = blockIdx.x;
@@ -186,7 +194,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
   const unsigned nC = g2 * (unsigned)ny * (unsigned)nz;  // x slabs
   const unsigned q = (unsigned)(blk - a.blk_prefix[lo_b]) * GHOST_THREADS + threadIdx.x;
   if (q >= nA + nB + nC) {
-    *out = make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
+    emit(make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE));
     return;
   }
   int i, j, k;
@@ -220,12 +228,12 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
   if (ow >= 0) {  // same-level copy wins (R9)
     const BoxDev sb = a.boxes[ow];
     const long long src = cell_offset(sb, g, a.geom.ox, wi - sb.lo[0], wj - sb.lo[1], wk - sb.lo[2]);
-    *out = make_uint4(dst, (unsigned)src, 0u, (unsigned)GHOST_COPY | star);
+    emit(make_uint4(dst, (unsigned)src, 0u, (unsigned)GHOST_COPY | star));
     return;
   }
   if (!a.has_coarse) {
     *a.err_flag = 1;
-    *out = make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
+    emit(make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE));
     return;
   }
   const int f[3] = {f0, f1, f2};
@@ -242,7 +250,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
       unit = unit && (wh[d] - wl[d] == 4);  // no periodic seam inside the 5-cell window
     }
     if (a.quartic == 2) {  // interpolated by coarse parent (k_fill_qparents), not by this list
-      *out = make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE);
+      emit(make_uint4(0u, 0u, 0u, (unsigned)GHOST_NONE));
       return;
     }
     const int owl = owner_lookup(a.cowner, a.cgeom, wl[0], wl[1], wl[2]);
@@ -250,7 +258,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
     if (unit && owl >= 0 && owl == owh) {  // a box is convex: the whole window lies in it
       const BoxDev cb = a.cboxes[owl];
       const long long o0 = cell_offset(cb, a.cgeom.g, a.cgeom.ox, wl[0] + 2 - cb.lo[0], wl[1] + 2 - cb.lo[1], wl[2] + 2 - cb.lo[2]);
-      *out = make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (rbits << 2) | star);
+      emit(make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (rbits << 2) | star));
       return;
     }
     for (int mz = -2; mz <= 2; ++mz)
@@ -259,7 +267,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
           if (owner_lookup(a.cowner, a.cgeom, wrap1(c0[0] + mx, a.cgeom.n[0]), wrap1(c0[1] + my, a.cgeom.n[1]),
                            wrap1(c0[2] + mz, a.cgeom.n[2])) < 0)
             *a.err_flag = 1;
-    *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW | star);
+    emit(make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW | star));
     return;
   }
   int c0[3], c1[3], w0[3], w1[3];
@@ -277,13 +285,13 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_plan_ghosts(const GhostArgs<T
     const BoxDev cb = a.cboxes[ow0];
     const long long o0 = cell_offset(cb, a.cgeom.g, a.cgeom.ox, w0[0] - cb.lo[0], w0[1] - cb.lo[1], w0[2] - cb.lo[2]);
     const unsigned signs = (c1[0] > c0[0] ? 1u : 0u) | (c1[1] > c0[1] ? 2u : 0u) | (c1[2] > c0[2] ? 4u : 0u);
-    *out = make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (signs << 2) | star);
+    emit(make_uint4(dst, (unsigned)o0, (unsigned)cb.sx | ((unsigned)cb.sy << 16), (unsigned)GHOST_INTERP | (signs << 2) | star));
     return;
   }
   // parents in several coarse boxes (or across the periodic seam of a single one): resolved at fill time
   long long o[8];
   if (!coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o)) *a.err_flag = 1;
-  *out = make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW | star);
+  emit(make_uint4(dst, (unsigned)(f0 + g) | ((unsigned)(f1 + g) << 16), (unsigned)(f2 + g), (unsigned)GHOST_SLOW | star));
 }
 
 // The fill itself: GHOST_EPT entries of the level's list per thread (strided by the CTA size, so that a warp still

@@ -112,6 +112,8 @@ struct LevelHost {
   std::vector<int> qp_prefix;  // quartic interpolation by coarse parent (k_fill_qparents): CTAs before box b
   size_t off_qp_prefix = 0, off_qp_list = 0, off_qs_list = 0, off_qs_count = 0;
   unsigned n_star_parents = 0;  // read back from the device after the plan
+  size_t off_star_list = 0, off_star_count = 0;
+  unsigned n_star = 0;          // GHOST_STAR entries of the ghost list, packed (read back after the plan)
   long long plane_cells = 0;  // pairs per plane (all boxes, ghosts and padding included)
   long long valid_cells = 0;
   long long count_blocks = 0;
@@ -357,6 +359,8 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.off_ghost_prefix = take(L.ghost_prefix.size() * sizeof(int));
     L.off_avg_prefix = take(L.avg_prefix.size() * sizeof(int));
     L.off_ghost_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
+    L.off_star_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
+    L.off_star_count = take(sizeof(unsigned));
     L.off_qp_prefix = take(L.qp_prefix.size() * sizeof(int));
     L.off_qp_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
     L.off_qs_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
@@ -452,6 +456,8 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.qblk_prefix = tab<int>(c, L.off_qp_prefix);
   a.qlist = tab<uint4>(c, L.off_qp_list);
   a.n_qentries = (unsigned)L.qp_prefix.back() * GHOST_THREADS;
+  a.star_list = tab<GhostEntry>(c, L.off_star_list);
+  a.star_count = tab<unsigned>(c, L.off_star_count);
   a.qstar_list = tab<uint4>(c, L.off_qs_list);
   a.qstar_count = tab<unsigned>(c, L.off_qs_count);
   a.has_coarse = l > 0;
@@ -509,10 +515,15 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     if (rc == SLEDGE_OK && pair) rc = fill_shell_copies<T>(c, l - 1, C.old, fill_pi);
     if (rc) return rc;
   }
-  a.star_only = star_only ? 1 : 0;  // before an RK sweep only the cells its star stencil reaches are needed
-  const int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
-  if (grid == 0) return SLEDGE_OK;
-  {
+  int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
+  if (star_only) {  // before an RK sweep only the cells its star stencil reaches are needed: the packed list
+    a.star_only = 1;
+    a.list = a.star_list;
+    a.n_entries = c->plan.lev[l].n_star;
+    grid = (int)((a.n_entries + GHOST_THREADS * GHOST_EPT - 1) / (GHOST_THREADS * GHOST_EPT));
+  }
+  if (grid == 0 && !(a.quartic == 2 && l > 0)) return SLEDGE_OK;
+  if (grid > 0) {
     Timed t(c, KIND_GHOST);
     if (a.quartic == 1 && l > 0) {
       if (fill_pi) k_fill_ghosts<T, true, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
@@ -985,6 +996,8 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   }
   // the tables above are pageable host memory: make sure the copies are done before they can go away
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  for (int l = 0; l < P.p.n_levels && e == cudaSuccess; ++l)
+    e = cudaMemcpy(&P.lev[l].n_star, c->arena + P.lev[l].off_star_count, sizeof(unsigned), cudaMemcpyDeviceToHost);
   for (int l = 1; l < P.p.n_levels && e == cudaSuccess; ++l)
     if (P.lev[l].qp_prefix.back() > 0)
       e = cudaMemcpy(&P.lev[l].n_star_parents, c->arena + P.lev[l].off_qs_count, sizeof(unsigned), cudaMemcpyDeviceToHost);
