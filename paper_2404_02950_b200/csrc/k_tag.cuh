@@ -67,15 +67,21 @@ __device__ __forceinline__ float cross_rn(float a1, float a2, float b1, float b2
   return __fsub_rn(__fmul_rn(a1, b2), __fmul_rn(a2, b1));
 }
 
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+
 // E(a -> b): +1 if up && cr > 0, -1 if dn && cr < 0, else 0, with up = a2<0 && b2>=0, dn = a2>=0 && b2<0.
 // sa = (a2 < 0) and sb = (b2 < 0) are evaluated once per loaded value.  Writing b2 >= 0 as !(b2 < 0) differs from
 // the definition only when a2 or b2 is NaN, and then cr is NaN and the edge is 0 either way; -0 is not < 0 in
 // both forms.
+// cr = RN(p - q) with p = RN(a1 b2), q = RN(a2 b1): the rounded difference of two floating-point numbers has the sign
+// of the exact difference (gradual underflow keeps a non-zero difference non-zero; inf - inf and NaN give NaN, for
+// which both orderings are false as well), so cr > 0 <=> p > q and cr < 0 <=> p < q: the subtraction is not needed.
 template <typename T, typename P>
 __device__ __forceinline__ int edge_of(const P& a, bool sa, const P& b, bool sb) {
-  const T cr = cross_rn(a.x, a.y, b.x, b.y);
+  const T p = mul_rn(a.x, b.y), q = mul_rn(a.y, b.x);
   const bool up = sa && !sb, dn = !sa && sb;
-  return (int)(up && cr > T(0)) - (int)(dn && cr < T(0));
+  return (int)(up && p > q) - (int)(dn && p < q);
 }
 
 template <typename P>
