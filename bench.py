@@ -200,6 +200,16 @@ def oracle_step(o, cfg, eta, levels):
         o.tag_strings(l)
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def time_oracle(cfg, budget_s=12.0, steps=None, warmup=1):
     from oracle import oracle as orc
     o, cells, desc, levels = oracle_sample(cfg)
@@ -217,8 +227,18 @@ def time_oracle(cfg, budget_s=12.0, steps=None, warmup=1):
         oracle_step(o, cfg, eta, levels)
         eta += cfg.dt
     dt = (time.perf_counter() - t0) / n
-    return {"value": cells * 4 / dt / 1e9, "unit": UNIT, "cores": orc.omp_threads(), "kind": "oracle",
-            "sample": f"{desc}; {n} steps of rk_step + tag_strings, {dt * 1e3:.1f} ms/step"}, dt, n
+    cores = orc.omp_threads()
+    # the same sample on ONE host thread (single-thread and all-core numbers), two steps
+    orc.set_threads(1)
+    t0 = time.perf_counter()
+    for _ in range(2):
+        oracle_step(o, cfg, eta, levels)
+        eta += cfg.dt
+    dt1 = (time.perf_counter() - t0) / 2
+    orc.set_threads(cores)
+    return {"value": cells * 4 / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{desc}; {n} steps of rk_step + tag_strings, {dt * 1e3:.1f} ms/step",
+            "single_thread_value": cells * 4 / dt1 / 1e9, "cpu_model": cpu_model()}, dt, n
 
 
 # ---------------------------------------------------------------------------------------------------

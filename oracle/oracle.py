@@ -79,12 +79,18 @@ def lib():
         L.orc_plaquette_winding.argtypes = [dp, dp, dp, dp]
         L.orc_energy.argtypes = [C.c_void_p, C.c_double, dp]
         L.orc_omp_threads.restype = C.c_int
+        L.orc_set_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
 
 
 def omp_threads() -> int:
     return int(lib().orc_omp_threads())
+
+
+def set_threads(n: int) -> None:
+    """OpenMP threads for the oracle's loops over boxes (timing only; results do not depend on it)."""
+    lib().orc_set_threads(int(n))
 
 
 def plaquette_winding(A, B, Cc, D) -> int:

@@ -842,6 +842,15 @@ int orc_energy(void* h, double eta, double* out) {
   return 0;
 }
 
+// test / timing infrastructure: number of OpenMP threads the loops over boxes may use (1 = serial)
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+  if (n >= 1) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
 int orc_omp_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();
