@@ -80,3 +80,55 @@ def test_c4_1024cubed_fp32_7pt_20_steps_all_cells_and_tags():
     if free < 90e9:
         pytest.skip("needs ~80 GB of free HBM")
     _run_tiled("C4", 64, "fused", check_tags=True)
+
+
+# ---- C5 at full size: a property that holds at any size ------------------------------------------------------------
+
+@pytest.mark.parametrize("interp", [0, 4])
+def test_c5_full_hierarchy_reproduces_an_affine_linear_in_time_solution(interp):
+    """The oracle cannot step the 2,067-box C5 hierarchy in seconds, but with lambda = 0 the field
+    psi_c = a_c . x + b_c + v_c t, Pi_c = v_c solves Eq.10-11 exactly, and every piece of the path reproduces it exactly
+    (up to rounding): the central Laplacians vanish on affine data, RK4 is exact for a solution linear in time, trilinear
+    and quartic interpolation reproduce affine data, linear-in-time ghosts are exact, the mean of 8 children of an affine
+    field is its value at the parent's centre.  Any wrong ghost source, parent, time weight or box offset anywhere in
+    the full hierarchy shows up as a non-zero Laplacian.  The periodic wrap breaks the affine field at the domain
+    faces; that disturbance travels at most lap_order cells per stage, so cells further than 12 coarse cells from a face
+    must hold the exact solution after one coarse step, in the launch configuration bench.py times."""
+    import bench
+    from paper_2404_02950_b200.sledge import Sledge
+    cfg = inputs.CONFIGS["C5"]
+    rings, boxes, cover = bench.hierarchy(cfg)
+    s = Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=cfg.nghost, blocking_factor=cfg.blocking_factor,
+               dtype="f64", lap_order=cfg.lap_order, h0=cfg.h0, lam=0.0, rk_dataflow="fused", interp=interp)
+    A = torch.tensor([[0.01, 0.02, -0.015], [-0.02, 0.005, 0.01]], dtype=torch.float64, device="cuda")  # per comp: x, y, z
+    B = (0.3, -0.8)
+    V = (0.1, 0.25)
+
+    def coords(l, lo, hi):
+        h = cfg.h0 / (1 << l)
+        ax = [(torch.arange(lo[d], hi[d] + 1, dtype=torch.float64, device="cuda") + 0.5) * h for d in range(3)]
+        return ax[0][None, None, :], ax[1][None, :, None], ax[2][:, None, None]
+
+    for ib, (l, lo, hi) in enumerate(boxes):
+        X, Y, Z = coords(l, lo, hi)
+        for c in range(2):
+            s.set_state(ib, c, (A[c, 0] * X + A[c, 1] * Y + A[c, 2] * Z + B[c]).contiguous())
+            s.set_state(ib, c + 2, torch.full(s.box_shape(ib), V[c], dtype=torch.float64, device="cuda"))
+    s.rk_step(cfg.dt, cfg.eta0)
+    s.synchronize()
+    L = cfg.n0 * cfg.h0
+    margin = 12 * cfg.h0
+    worst, checked = 0.0, 0
+    for ib, (l, lo, hi) in enumerate(boxes):
+        X, Y, Z = coords(l, lo, hi)
+        inner = ((X > margin) & (X < L - margin)) & ((Y > margin) & (Y < L - margin)) & ((Z > margin) & (Z < L - margin))
+        if not bool(inner.any()):
+            continue
+        for c in range(2):
+            want = A[c, 0] * X + A[c, 1] * Y + A[c, 2] * Z + (B[c] + V[c] * cfg.dt)
+            worst = max(worst, float(((s.get_state(ib, c) - want).abs() * inner).max()))
+            worst = max(worst, float(((s.get_state(ib, c + 2) - V[c]).abs() * inner).max()))
+        checked += int(inner.sum())
+    assert checked > 0.5 * sum(int(np.prod(s.box_shape(ib))) for ib in range(len(boxes)))
+    assert worst <= F64_TOL, worst
+    s.close()
