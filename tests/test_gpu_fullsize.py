@@ -84,8 +84,9 @@ def test_c4_1024cubed_fp32_7pt_20_steps_all_cells_and_tags():
 
 # ---- C5 at full size: a property that holds at any size ------------------------------------------------------------
 
-@pytest.mark.parametrize("interp", [0, 4])
-def test_c5_full_hierarchy_reproduces_an_affine_linear_in_time_solution(interp):
+@pytest.mark.parametrize("interp,extra", [(0, {}), (4, {}),
+                                          (4, dict(integrator=10, ko_order=3, ko_strength=(0.02, 0.03, 0.05, 0.07)))])
+def test_c5_full_hierarchy_reproduces_an_affine_linear_in_time_solution(interp, extra):
     """The oracle cannot step the 2,067-box C5 hierarchy in seconds, but with lambda = 0 the field
     psi_c = a_c . x + b_c + v_c t, Pi_c = v_c solves Eq.10-11 exactly, and every piece of the path reproduces it exactly
     (up to rounding): the central Laplacians vanish on affine data, RK4 is exact for a solution linear in time, trilinear
@@ -93,13 +94,14 @@ def test_c5_full_hierarchy_reproduces_an_affine_linear_in_time_solution(interp):
     field is its value at the parent's centre.  Any wrong ghost source, parent, time weight or box offset anywhere in
     the full hierarchy shows up as a non-zero Laplacian.  The periodic wrap breaks the affine field at the domain
     faces; that disturbance travels at most lap_order cells per stage, so cells further than 12 coarse cells from a face
-    must hold the exact solution after one coarse step, in the launch configuration bench.py times."""
+    must hold the exact solution after one coarse step, in the launch configuration bench.py times.  The third variant
+    runs SSPRK3 with the order-3 Kreiss-Oliger term, which vanishes on affine data as well (at most 3 cells per stage)."""
     import bench
     from paper_2404_02950_b200.sledge import Sledge
     cfg = inputs.CONFIGS["C5"]
     rings, boxes, cover = bench.hierarchy(cfg)
     s = Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=cfg.nghost, blocking_factor=cfg.blocking_factor,
-               dtype="f64", lap_order=cfg.lap_order, h0=cfg.h0, lam=0.0, rk_dataflow="fused", interp=interp)
+               dtype="f64", lap_order=cfg.lap_order, h0=cfg.h0, lam=0.0, rk_dataflow="fused", interp=interp, **extra)
     A = torch.tensor([[0.01, 0.02, -0.015], [-0.02, 0.005, 0.01]], dtype=torch.float64, device="cuda")  # per comp: x, y, z
     B = (0.3, -0.8)
     V = (0.1, 0.25)
