@@ -65,6 +65,8 @@ struct PipeArgs {
   const BoxDev* boxes;
   const TileDev* tiles;
   const P* sten[3];
+  const void* tmap[3];  // k_rk_tma only: per differenced field, the tensor maps (CUtensorMap, one per box of the level) of
+                         // the buffer plane sten[f] points at
   const P* pnt[7];
   P* out_psi[2];
   P* out_pi[2];

@@ -14,11 +14,26 @@
 //   W_yz(P) = Ey(P) + Ez(P+y) - Ey(P+z) - Ez(P)
 //   W_zx(P) = Ez(P) + Ex(P+z) - Ez(P+x) - Ex(P)
 // and only the edges that START at a cell are ever evaluated (3 cross products per cell instead of 12).
-// A warp owns a 31 x TAG_RY patch of cells and marches along z without any block-level synchronisation: lane l
-// holds the column x0+l of TAG_RY+1 rows (the last row and lane 31 are halo: they only supply edges), the
-// plane below stays in registers, loads run TAG_PF planes ahead, psi(P+x) and the packed edges of P+x come from
-// lane l+1 by shuffle.  Per plane and thread: Ex, Ez on TAG_RY+1 rows and Ey on TAG_RY rows (3.5 edges per cell
-// for TAG_RY = 4).  Warps step by 31 cells in x so that every lane's +x partner is in the warp.
+//
+// One comparison per edge.  With s(v) = (v2 < 0), an edge contributes only if s(a) != s(b), and then
+//   up (s(a), !s(b)):  p > q  with p = RN(a1 b2) = RN(a1 |b2|) =: P,  q = RN(a2 b1) = -RN(|a2| b1) =: -Q
+//   dn (!s(a), s(b)):  p < q  with p = -P, q = Q
+// (rounding to nearest is symmetric in sign, so the identities hold bit for bit, zeros, infinities and NaNs
+// included: a comparison with NaN is false on both sides, +0 and -0 compare equal on both sides), i.e. in both
+// cases the edge counts iff P > -Q, and its sign is +1 if s(a), else -1.  The comparison "cr > 0" of the
+// definition equals "p > q" because the rounded difference of two floating-point numbers has the sign of the
+// exact difference (gradual underflow).
+//
+// Bit-sliced windings.  A warp owns a 31 x TAG_RY patch of cells (lane 31 and a (TAG_RY+1)-th row are halo: they
+// only supply edges) and marches along z with no block-level synchronisation.  A lane keeps, per plane, ONE word
+// per quantity with a 3-bit field per row (bit 3r = row r): S = s(psi), G = the comparison results of its x / y / z
+// edges.  Edges that count: N = G & (S ^ S_partner), split by sign into N & S_a and N & ~S_a; the four signed
+// terms of a winding are added as 3-bit integers for all rows at once (two 3-input adds), positive and negative
+// terms separately, and W != 0 <=> the two sums differ.  The three winding masks interleave into the tag bits:
+// (m_xy | m_yz << 1 | m_zx << 2) >> 3r & 7 is the tag byte of row r.  The masks of P+x come from lane + 1 by
+// shuffle.  ~40 instructions per cell instead of ~130 with per-cell integer arithmetic.
+// Loads: every lane streams its column through a per-warp cp.async ring, TAG_PF planes ahead (bytes in flight cost
+// no registers); psi(P+x) is read from the neighbouring lane's ring entry.
 // Counts: per-thread counters, reduced over the warp (redux) and flushed with one atomicAdd per 32-block
 // whenever the warp leaves a 32-block in z.
 #pragma once
@@ -29,7 +44,7 @@ namespace sledge {
 
 constexpr int TAG_TX = 31;                 // cells per warp row that produce tags (lane 31 is the +x halo)
 #ifndef SLEDGE_TAG_RY
-#define SLEDGE_TAG_RY 4
+#define SLEDGE_TAG_RY 8
 #endif
 constexpr int TAG_RY = SLEDGE_TAG_RY;                  // rows per warp
 #ifndef SLEDGE_TAG_WARPS
@@ -40,10 +55,10 @@ constexpr int TAG_TY = TAG_RY * TAG_WARPS; // rows per CTA tile
 constexpr int TAG_THREADS = TAG_WARPS * 32;
 template <typename T> constexpr size_t tag_smem_bytes();
 #ifndef SLEDGE_TAG_PF
-#define SLEDGE_TAG_PF 4
+#define SLEDGE_TAG_PF 3
 #endif
 constexpr int TAG_PF = SLEDGE_TAG_PF;       // planes in flight per thread (cp.async ring depth)
-static_assert(TAG_RY <= 32, "a warp's rows may straddle at most two 32-blocks");
+static_assert(TAG_RY <= 9, "3-bit fields of TAG_RY + 1 rows must fit a 32-bit word with the << 2 of the tag interleave");
 
 template <typename T>
 struct TagArgs {
@@ -59,49 +74,32 @@ struct TagArgs {
   int nb0, nb1;  // count blocks per axis (x, y)
 };
 
-// individually rounded a1*b2 - a2*b1 (R8: no FMA)
-__device__ __forceinline__ double cross_rn(double a1, double a2, double b1, double b2) {
-  return __dsub_rn(__dmul_rn(a1, b2), __dmul_rn(a2, b1));
-}
-__device__ __forceinline__ float cross_rn(float a1, float a2, float b1, float b2) {
-  return __fsub_rn(__fmul_rn(a1, b2), __fmul_rn(a2, b1));
-}
-
 __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
 __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
 
-// E(a -> b): +1 if up && cr > 0, -1 if dn && cr < 0, else 0, with up = a2<0 && b2>=0, dn = a2>=0 && b2<0.
-// sa = (a2 < 0) and sb = (b2 < 0) are evaluated once per loaded value.  Writing b2 >= 0 as !(b2 < 0) differs from
-// the definition only when a2 or b2 is NaN, and then cr is NaN and the edge is 0 either way; -0 is not < 0 in
-// both forms.
-// cr = RN(p - q) with p = RN(a1 b2), q = RN(a2 b1): the rounded difference of two floating-point numbers has the sign
-// of the exact difference (gradual underflow keeps a non-zero difference non-zero; inf - inf and NaN give NaN, for
-// which both orderings are false as well), so cr > 0 <=> p > q and cr < 0 <=> p < q: the subtraction is not needed.
+// the comparison of edge a -> b (see the header): P > -Q with P = RN(a1 |b2|), Q = RN(|a2| b1)
 template <typename T, typename P>
-__device__ __forceinline__ int edge_of(const P& a, bool sa, const P& b, bool sb) {
-  const T p = mul_rn(a.x, b.y), q = mul_rn(a.y, b.x);
-  const bool up = sa && !sb, dn = !sa && sb;
-  return (int)(up && p > q) - (int)(dn && p < q);
+__device__ __forceinline__ bool edge_cmp(const P& a, const P& b) {
+  return mul_rn(a.x, fabs(b.y)) > -mul_rn(fabs(a.y), b.x);
 }
-
-template <typename P>
-__device__ __forceinline__ P shfl_down_pair(const P& v, int delta);
-template <>
-__device__ __forceinline__ double2 shfl_down_pair<double2>(const double2& v, int delta) {
-  return make_double2(__shfl_down_sync(0xffffffffu, v.x, delta), __shfl_down_sync(0xffffffffu, v.y, delta));
-}
-template <>
-__device__ __forceinline__ float2 shfl_down_pair<float2>(const float2& v, int delta) {
-  return make_float2(__shfl_down_sync(0xffffffffu, v.x, delta), __shfl_down_sync(0xffffffffu, v.y, delta));
-}
-
-
 
 template <typename T> constexpr size_t tag_smem_bytes() {
   return ((size_t)TAG_WARPS * TAG_PF * (TAG_RY + 1) * 32 + 1) * sizeof(typename PairOf<T>::type);
 }
 
-// edges of P+x packed for the shuffle: (Ey+1) | (Ez+1)<<2
+// one 3-bit field per row: bit 3r
+__host__ __device__ constexpr unsigned tag_rowbits(int rows) {
+  unsigned m = 0;
+  for (int r = 0; r < rows; ++r) m |= 1u << (3 * r);
+  return m;
+}
+// field-wise "a != b" of two words of 3-bit integers -> bit 3r
+__device__ __forceinline__ unsigned tag_differs(unsigned a, unsigned b) {
+  const unsigned v = a ^ b;
+  constexpr unsigned ROWS = tag_rowbits(TAG_RY);
+  return (v | (v >> 1) | (v >> 2)) & ROWS;
+}
+
 template <typename T>
 __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a) {
   using P = typename PairOf<T>::type;
@@ -117,42 +115,46 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
   const bool actx = lane < TAG_TX && x < b.n[0];
   const long long plane = (long long)b.sx * b.sy;
   const long long org = b.base + (long long)(t.z0 + a.g) * plane + (xc + a.ox);
-  long long orow[RY + 1];
+  const char* prow[RY + 1];  // this lane's cell of row r in plane t.z0
 #pragma unroll
-  for (int r = 0; r <= RY; ++r) orow[r] = org + (long long)(((wr && y0 + r >= b.n[1]) ? 0 : min(y0 + r, b.n[1])) + a.g) * b.sx;
+  for (int r = 0; r <= RY; ++r)
+    prow[r] = reinterpret_cast<const char*>(
+        a.psi + org + (long long)(((wr && y0 + r >= b.n[1]) ? 0 : min(y0 + r, b.n[1])) + a.g) * b.sx);
 
-  // plane index n is relative to t.z0; n = nz is the first plane above the tile (a ghost plane or the next tile)
-  // Every lane streams its own column through a per-warp shared-memory ring with cp.async, TAG_PF planes ahead:
-  // the bytes in flight cost no registers.  ring[slot][row][lane]; lane l reads its +x partner at [lane + 1].
+  // plane index n is relative to t.z0; n = nz is the first plane above the tile (a ghost plane, the next tile, or
+  // plane 0 of the periodic box); planes past it are never used and re-read plane nz.
+  // ring[slot][row][lane]; lane l reads its +x partner at [lane + 1].
   extern __shared__ __align__(16) unsigned char tag_smem[];
-  P* const ring = reinterpret_cast<P*>(tag_smem) + (size_t)warp * (TAG_PF * (RY + 1) * 32) + lane;
-  auto issue = [&](int n) {
-    P* const dst = ring + (n % TAG_PF) * ((RY + 1) * 32);
-    const int pn = min(n, t.nz);
-    const long long po = (long long)((wr && t.z0 + pn >= b.n[2]) ? -t.z0 : pn) * plane;
+  constexpr int SLOT = (RY + 1) * 32;  // pairs per ring slot
+  P* const ring = reinterpret_cast<P*>(tag_smem) + (size_t)warp * (TAG_PF * SLOT) + lane;
+  const long long plane_bytes = plane * (long long)sizeof(P);
+  const long long top_bytes = (wr && t.z0 + t.nz >= b.n[2]) ? -(long long)t.z0 * plane_bytes : (long long)t.nz * plane_bytes;
+  long long po = 0;  // byte offset of the next plane to issue
+  int pn = 0;        // its index
+  auto issue = [&](P* dst) {
 #pragma unroll
-    for (int r = 0; r <= RY; ++r) cp_async_pair(dst + r * 32, a.psi + orow[r] + po);
+    for (int r = 0; r <= RY; ++r) cp_async_pair(dst + r * 32, reinterpret_cast<const P*>(prow[r] + po));
+    ++pn;
+    po = pn < t.nz ? po + plane_bytes : top_bytes;
   };
 #pragma unroll
   for (int d = 0; d < TAG_PF; ++d) {
-    issue(d);
+    issue(ring + d * SLOT);
     cp_async_commit();
   }
-  P cur[RY + 1];
-  cp_async_wait<TAG_PF - 1>();
-#pragma unroll
-  for (int r = 0; r <= RY; ++r) cur[r] = ring[r * 32];  // plane 0 (slot 0), own entries only
-  int exc[RY], eyc[RY], wxyc[RY];  // in-plane edges and W_xy of the plane below
-#pragma unroll
-  for (int r = 0; r < RY; ++r) exc[r] = eyc[r] = wxyc[r] = 0;
-  bool sc[RY + 1];  // (psi2 < 0) of cur
-#pragma unroll
-  for (int r = 0; r <= RY; ++r) sc[r] = cur[r].y < T(0);
 
-  // count blocks: lanes split over at most two x-blocks, rows over at most two y-blocks
+  // rows of this warp that exist and produce tags, as 3-bit fields; rows in the first of the (at most two) y count blocks
+  const int nrows = min(RY, b.n[1] - y0);
+  const int bj0 = (b.lo[1] + y0) >> 5;
+  unsigned act = 0, rowsA = 0;
+#pragma unroll
+  for (int r = 0; r < RY; ++r) {
+    if (actx && r < nrows) act |= 1u << (3 * r);
+    if (((b.lo[1] + y0 + r) >> 5) == bj0) rowsA |= 1u << (3 * r);
+  }
+  // count blocks: lanes split over at most two x-blocks
   const int bi = (b.lo[0] + min(x, b.n[0] - 1)) >> 5;
   const int bi0 = __shfl_sync(0xffffffffu, bi, 0);
-  const int bj0 = (b.lo[1] + y0) >> 5;
   int cntA = 0, cntB = 0;  // this thread's tagged cells in y-block bj0 / bj0 + 1
   int cur_bk = (b.lo[2] + t.z0) >> 5;
   auto flush = [&](int bk) {
@@ -170,70 +172,81 @@ __global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a)
     }
     cntA = cntB = 0;
   };
+  uint8_t* tagp = a.tags ? a.tags + b.tag_base + ((long long)(t.z0 - 1) * b.n[1] + y0) * b.n[0] + x : nullptr;
+  const long long tag_plane = (long long)b.n[1] * b.n[0];
+
+  // state carried from plane n-1: its values, sign word, signed in-plane edges (x, y) and W_xy mask
+  P cur[RY + 1];
+#pragma unroll
+  for (int r = 0; r <= RY; ++r) cur[r] = mkpair(T(0), T(0));
+  unsigned Sp = 0, Spx = 0, XPp = 0, XNp = 0, YPp = 0, YNp = 0, mxy_p = 0;
+  int slot = 0;
 
 #pragma unroll 2
   for (int n = 0; n <= t.nz; ++n) {
     P nO[RY + 1], nX[RY + 1];
-    bool so[RY + 1], sx[RY + 1];
-    unsigned sbits = 0;
-#pragma unroll
     cp_async_wait<TAG_PF - 1>();  // this lane's copies of plane n have landed ...
     __syncwarp();                 // ... and its neighbour's
-    const P* const src = ring + (n % TAG_PF) * ((RY + 1) * 32);
+    P* const src = ring + slot * SLOT;
 #pragma unroll
     for (int r = 0; r <= RY; ++r) {
       nO[r] = src[r * 32];
-      nX[r] = src[r * 32 + 1];  // lane 31 reads a foreign entry: its Ex is never used
-      so[r] = nO[r].y < T(0);
-      sbits |= (so[r] ? 1u : 0u) << r;
+      nX[r] = src[r * 32 + 1];  // lane 31 reads a foreign entry: its results are never used
     }
     __syncwarp();  // everybody has read slot n % TAG_PF before it is refilled
-    issue(n + TAG_PF);
+    issue(src);  // plane n + TAG_PF goes into the slot just drained
     cp_async_commit();
-    sbits = __shfl_down_sync(0xffffffffu, sbits, 1);
-#pragma unroll
-    for (int r = 0; r <= RY; ++r) sx[r] = (sbits >> r) & 1u;
-    int ex[RY + 1], ez[RY + 1], ey[RY];
+    slot = slot + 1 == TAG_PF ? 0 : slot + 1;
+
+    unsigned S = 0, Gx = 0, Gy = 0, Gz = 0;
 #pragma unroll
     for (int r = 0; r <= RY; ++r) {
-      ex[r] = edge_of<T, P>(nO[r], so[r], nX[r], sx[r]);   // plane n
-      ez[r] = edge_of<T, P>(cur[r], sc[r], nO[r], so[r]);  // plane n-1 -> n (0 at n = 0: cur == nO)
+      if (nO[r].y < T(0)) S |= 1u << (3 * r);
+      if (edge_cmp<T, P>(nO[r], nX[r])) Gx |= 1u << (3 * r);   // plane n
+      if (edge_cmp<T, P>(cur[r], nO[r])) Gz |= 1u << (3 * r);  // plane n-1 -> n
     }
 #pragma unroll
-    for (int r = 0; r < RY; ++r) ey[r] = edge_of<T, P>(nO[r], so[r], nO[r + 1], so[r + 1]);
-    int pk = 0;  // (Ey+1) | (Ez+1)<<2 of every row, 4 bits per row, for the lane on the left
-#pragma unroll
-    for (int r = 0; r < RY; ++r) pk |= ((ey[r] + 1) | ((ez[r] + 1) << 2)) << (4 * r);
-    const int nb = __shfl_down_sync(0xffffffffu, pk, 1);
+    for (int r = 0; r < RY; ++r)
+      if (edge_cmp<T, P>(nO[r], nO[r + 1])) Gy |= 1u << (3 * r);
+    const unsigned Sx = __shfl_down_sync(0xffffffffu, S, 1);
+    const unsigned X = Gx & (S ^ Sx), Y = Gy & (S ^ (S >> 3)), Z = Gz & (Sp ^ S);  // edges that count
+    const unsigned XP = X & S, XN = X & ~S, YP = Y & S, YN = Y & ~S, ZP = Z & Sp, ZN = Z & ~Sp;
+    // Y and Z of the lane on the right (P + x): one shuffle, signs from Sx (plane n) and Spx (plane n - 1)
+    const unsigned YZx = __shfl_down_sync(0xffffffffu, Y | (Z << 1), 1);
+    constexpr unsigned ROWS = tag_rowbits(RY);
+    const unsigned Yx = YZx & ROWS, Zx = (YZx >> 1) & ROWS;
+    const unsigned YPx = Yx & Sx, YNx = Yx & ~Sx, ZPx = Zx & Spx, ZNx = Zx & ~Spx;
+    // W_xy of plane n (tagged one iteration later, with the plane's other two windings)
+    const unsigned mxy = tag_differs(XP + YPx + ((XN >> 3) + YN), XN + YNx + ((XP >> 3) + YP));
     const int z = t.z0 + n - 1;
     const int bk = (b.lo[2] + z) >> 5;
-    if (n > 0 && bk != cur_bk) {
-      flush(cur_bk);
-      cur_bk = bk;
-    }
-#pragma unroll
-    for (int r = 0; r < RY; ++r) {
-      const int eyx = ((nb >> (4 * r)) & 3) - 1, ezx = ((nb >> (4 * r + 2)) & 3) - 1;  // Ey(P+x), Ez(P+x)
-      const int wxyn = ex[r] + eyx - ex[r + 1] - ey[r];
-      if (n > 0) {
-        const int wyz = eyc[r] + ez[r + 1] - ey[r] - ez[r];
-        const int wzx = ez[r] + ex[r] - ezx - exc[r];
-        const uint8_t tag = (uint8_t)((wxyc[r] != 0 ? 1 : 0) | (wyz != 0 ? 2 : 0) | (wzx != 0 ? 4 : 0));
-        const int y = y0 + r;
-        const bool act = actx && y < b.n[1];
-        if (a.tags && act) a.tags[b.tag_base + ((long long)z * b.n[1] + y) * b.n[0] + x] = tag;
-        const int hit = (act && tag != 0) ? 1 : 0;
-        if (((b.lo[1] + y) >> 5) == bj0) cntA += hit; else cntB += hit;
+    if (n > 0) {
+      if (bk != cur_bk) {
+        flush(cur_bk);
+        cur_bk = bk;
       }
-      wxyc[r] = wxyn;
-      exc[r] = ex[r];
-      eyc[r] = ey[r];
-    }
+      const unsigned myz = tag_differs(YPp + (ZP >> 3) + (YN + ZN), YNp + (ZN >> 3) + (YP + ZP));
+      const unsigned mzx = tag_differs(ZP + XP + (ZNx + XNp), ZN + XN + (ZPx + XPp));
+      const unsigned c3 = mxy_p | (myz << 1) | (mzx << 2);  // field r = tag byte of row r
+      if (a.tags) {
 #pragma unroll
-    for (int r = 0; r <= RY; ++r) {
-      cur[r] = nO[r];
-      sc[r] = so[r];
+        for (int r = 0; r < RY; ++r)
+          if ((act >> (3 * r)) & 1u) tagp[(long long)r * b.n[0]] = (uint8_t)((c3 >> (3 * r)) & 7u);
+      }
+      const unsigned any = (mxy_p | myz | mzx) & act;
+      cntA += __popc(any & rowsA);
+      cntB += __popc(any & ~rowsA);
     }
+    tagp += tag_plane;
+    mxy_p = mxy;
+    Sp = S;
+    Spx = Sx;
+    XPp = XP;
+    XNp = XN;
+    YPp = YP;
+    YNp = YN;
+#pragma unroll
+    for (int r = 0; r <= RY; ++r) cur[r] = nO[r];
   }
   flush(cur_bk);
 }

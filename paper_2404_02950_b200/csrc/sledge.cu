@@ -12,6 +12,7 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -20,6 +21,7 @@
 #include "k_ghost.cuh"
 #include "k_rk_pipe.cuh"
 #include "k_rk_plane.cuh"
+#include "k_rk_tma.cuh"
 #include "k_tag.cuh"
 
 using namespace sledge;
@@ -61,7 +63,8 @@ constexpr int K1_TX = 32, K1_TY = SLEDGE_K1_TY, K1_NZ = SLEDGE_K1_NZ;
 constexpr int K1F_TX = SLEDGE_K1F_TX;  // x vectors per fused tile (k_rk_plane)
 constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
-constexpr long long K1F_MIN_TILES = 3500;  // below this many CTAs the fused sweeps halve their z-chunk
+constexpr long long K1F_MIN_TILES = 3500;
+constexpr long long TAG_MIN_TILES = 148 * 4 * 6;  // below this many CTAs the tag pass halves its z-chunk (down to 32 planes)  // below this many CTAs the fused sweeps halve their z-chunk
 constexpr int K1F_TY = SLEDGE_K1F_TY;            // tile rows / budget of the FUSED sweeps
 constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
 // which on-chip data path a sweep uses: 1 = k_rk_plane (ghosted plane ring), 0 = k_rk_pipe (ring + centre plane)
@@ -99,6 +102,15 @@ template <int MODE> struct K1Shape {
   static constexpr int MINB = MODE == FUSED_A ? SLEDGE_K1F_MINB_A : (MODE == FUSED_B ? SLEDGE_K1F_MINB_B : 1);
 };
 
+// rows per thread of the FUSED sweeps (k_rk_plane / k_rk_tma); the tensor maps' box shape follows from it
+template <typename T, int ORDER> struct FusedTile {
+  // the 7-plane z-window of the 19-point stencil leaves no registers for a second row
+  static constexpr int RY = ORDER == 3 ? 1 : (sizeof(T) == 4 ? SLEDGE_K1F_RY32 : SLEDGE_K1F_RY);
+};
+#ifndef SLEDGE_K1F_TMA_PDMAX
+#define SLEDGE_K1F_TMA_PDMAX 2
+#endif
+
 thread_local std::string g_err;
 
 struct LevelHost {
@@ -113,6 +125,12 @@ struct LevelHost {
   size_t off_qp_prefix = 0, off_qp_list = 0, off_qs_list = 0, off_qs_count = 0;
   unsigned n_star_parents = 0;  // read back from the device after the plan
   size_t off_star_list = 0, off_star_count = 0;
+  size_t off_tmaps = 0;        // k_rk_tma: CUtensorMap[NBUF * 2][nbox] of the level's state planes (fused levels only)
+  bool has_tmaps = false;
+  std::vector<CUtensorMap> tmaps_host;
+  // periodic one-box level under the TMA sweeps: star ghost cells (psi and Pi) of buffer b are periodic images of
+  // the buffer's current valid data (the sweep that wrote the buffer stored them, or a K2 fill since)
+  bool star_ok[4] = {false, false, false, false};
   unsigned n_star = 0;          // GHOST_STAR entries of the ghost list, packed (read back after the plan)
   long long plane_cells = 0;  // pairs per plane (all boxes, ghosts and padding included)
   long long valid_cells = 0;
@@ -156,6 +174,7 @@ struct sledge_ctx {
   std::string err;
   int64_t launches = 0;
   bool profiling = false;
+  bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
   size_t ev_used[4] = {0, 0, 0, 0};
 };
@@ -316,6 +335,14 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     for (const BoxDev& b : L.boxdev)
       ft_long += (long long)((b.n[0] + ftxc - 1) / ftxc) * ((b.n[1] + K1F_TY - 1) / K1F_TY) * ((b.n[2] + K1_NZ - 1) / K1_NZ);
     const int fnz = ft_long >= K1F_MIN_TILES ? K1_NZ : K1_NZ / 2;
+    // z-chunk of the tag pass (K3): a tile costs one extra plane, but the grid should be several waves of 148 SMs x 4 CTAs
+    int tnz = K1_NZ;
+    for (; tnz > 32; tnz /= 2) {
+      long long nt = 0;
+      for (const BoxDev& b : L.boxdev)
+        nt += (long long)((b.n[0] + TAG_TX - 1) / TAG_TX) * ((b.n[1] + TAG_TY - 1) / TAG_TY) * ((b.n[2] + tnz - 1) / tnz);
+      if (nt >= TAG_MIN_TILES) break;
+    }
     for (size_t q = 0; q < L.boxdev.size(); ++q) {
       const BoxDev& b = L.boxdev[q];
       for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
@@ -324,9 +351,9 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       for (int z0 = 0; z0 < b.n[2]; z0 += fnz)
         for (int y0 = 0; y0 < b.n[1]; y0 += K1F_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += ftxc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(fnz, b.n[2] - z0)});
-      for (int z0 = 0; z0 < b.n[2]; z0 += K1_NZ)
+      for (int z0 = 0; z0 < b.n[2]; z0 += tnz)
         for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
-          for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(K1_NZ, b.n[2] - z0)});
+          for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(tnz, b.n[2] - z0)});
       const long long Gx = b.n[0] + 2 * g, Gy = b.n[1] + 2 * g;
       const long long nghost = Gx * Gy * 2 * g + Gx * 2 * g * b.n[2] + 2LL * g * b.n[1] * b.n[2];
       L.ghost_prefix.push_back(L.ghost_prefix.back() + (int)((nghost + GHOST_THREADS - 1) / GHOST_THREADS));
@@ -361,6 +388,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.off_ghost_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
     L.off_star_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
     L.off_star_count = take(sizeof(unsigned));
+    L.off_tmaps = take(L.boxdev.size() * NBUF * 2 * sizeof(CUtensorMap));
     L.off_qp_prefix = take(L.qp_prefix.size() * sizeof(int));
     L.off_qp_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
     L.off_qs_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
@@ -571,13 +599,73 @@ int plan_ghosts(sledge_ctx* c, int l) {
   return rc;
 }
 
+// Tensor maps of the FUSED level's state planes for k_rk_tma: per box and buffer plane a 3-D tensor
+// (2 sx reals, sy rows, nz + 2g planes) with the sweep's tile box (2 SW reals, SH rows, 1 plane); out-of-bounds
+// elements (high end of a partial tile) are zero-filled.  cuTensorMapEncodeTiled is a host-only driver entry point,
+// fetched at run time so that the library keeps loading on machines without a driver.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int make_tensor_maps(sledge_ctx* c, int l) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return fail(c, SLEDGE_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  }
+  const EncodeTiledFn encode = (EncodeTiledFn)fn;
+  const int R = P.p.lap_order, g = P.p.nghost;
+  const int cpt = P.p.dtype == SLEDGE_F64 ? 1 : 2;
+  const int xo = (R + cpt - 1) / cpt * cpt;
+  const cuuint32_t sw = (cuuint32_t)(K1F_TX * cpt + 2 * xo), sh = (cuuint32_t)(K1F_TY + 2 * R);
+  const size_t nb = L.boxdev.size();
+  L.tmaps_host.assign(nb * NBUF * 2, CUtensorMap());
+  for (int buf = 0; buf < NBUF; ++buf)
+    for (int which = 0; which < 2; ++which)
+      for (size_t q = 0; q < nb; ++q) {
+        const BoxDev& b = L.boxdev[q];
+        void* base = c->arena + L.off_buf[buf][which] + (size_t)b.base * 2 * P.esz;
+        const cuuint64_t dims[3] = {(cuuint64_t)2 * b.sx, (cuuint64_t)b.sy, (cuuint64_t)(b.n[2] + 2 * g)};
+        const cuuint64_t strides[2] = {(cuuint64_t)b.sx * 2 * P.esz, (cuuint64_t)b.sx * b.sy * 2 * P.esz};
+        const cuuint32_t box[3] = {2 * sw, sh, 1};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        const CUresult r = encode(&L.tmaps_host[(size_t)(buf * 2 + which) * nb + q],
+                                  P.p.dtype == SLEDGE_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
+                                  base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(c, SLEDGE_ECUDA, "cuTensorMapEncodeTiled failed (%d) for box %zu of level %d", (int)r, q, l);
+      }
+  L.has_tmaps = true;
+  return SLEDGE_OK;
+}
+
 template <typename T, int ORDER, int MODE, int KO = 0>
 cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   constexpr int TY = K1Shape<MODE>::TY;
   static bool configured = false;  // per instantiation
+  if constexpr (K1Shape<MODE>::fused && KO == 0) {
+    if (a.tmap[0]) {  // TMA-staged plane ring (k_rk_tma.cuh); the maps exist on fused levels unless SLEDGE_K1_TMA=0
+      constexpr int RY = FusedTile<T, ORDER>::RY;
+      constexpr int PD = tma_depth<T, ORDER, MODE, K1F_TX, TY, RY>(K1Shape<MODE>::SMEM, SLEDGE_K1F_TMA_PDMAX);
+      using C = TmaCfg<T, ORDER, MODE, K1F_TX, TY, PD, RY>;
+      static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
+      constexpr int MINB = ORDER == 3 ? 1 : K1Shape<MODE>::MINB;
+      auto kern = k_rk_tma<T, ORDER, MODE, K1F_TX, TY, PD, RY, MINB>;
+      static bool configured_tma = false;
+      if (!configured_tma) {
+        const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        configured_tma = true;
+      }
+      kern<<<grid, C::NT, C::SMEM_BYTES, c->stream>>>(a);
+      return cudaSuccess;
+    }
+  }
   if constexpr (K1Shape<MODE>::plane && KO == 0) {
-    // the 7-plane z-window of the 19-point stencil leaves no registers for a second row
-    constexpr int RY = ORDER == 3 ? 1 : ((K1Shape<MODE>::fused && sizeof(T) == 4) ? SLEDGE_K1F_RY32 : K1Shape<MODE>::RY);
+    constexpr int RY = K1Shape<MODE>::fused ? FusedTile<T, ORDER>::RY : (ORDER == 3 ? 1 : K1Shape<MODE>::RY);
     constexpr int PD = plane_depth<T, ORDER, MODE, K1F_TX, TY, RY>(K1Shape<MODE>::SMEM, K1Shape<MODE>::PDMAX);
     using C = PlaneCfg<T, ORDER, MODE, K1F_TX, TY, PD, RY>;
     static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
@@ -647,6 +735,8 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : (P.p.lap_order == 2 ? 1.0 / (12.0 * h2) : 1.0 / (180.0 * h2)));
   a.a_mass = (T)P.p.a_mass;
   for (int b = 0; b < NBUF; ++b) L.shell_ok[b] = 0;  // a sweep rewrites valid cells of this level's buffers
+  if (!fused)
+    for (int b = 0; b < NBUF; ++b) L.star_ok[b] = false;
   const int ko = ko_on(P.p) ? P.p.ko_order : 0;
   if (ko) {  // Eq.7: (-1)^(r+1) eps / (2^(2r) h_l); Pi(U) is differenced too and moves from pnt[0] to sten[1]
     const double sgn = (ko % 2 == 0) ? -1.0 : 1.0;
@@ -693,29 +783,50 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
   set_eta(P, a, 1, fx ? eta_const : t + 0.5 * dt);
   set_eta(P, a, 2, fx ? eta_const : t + dt);
   a.adt = (T)dt;
-  // a level that is one box over the periodic domain needs no ghost fill: k_rk_plane wraps its own addresses
-  const bool wrap = L.periodic_box && (SLEDGE_K1F_PLANE != 0);
+  // A level that is one box over the periodic domain needs no ghost fill before a sweep: k_rk_plane wraps its own
+  // addresses; k_rk_tma (no wrap in a tensor map) stores the periodic images of its results into the star ghost
+  // cells of its output instead, so only a state that no such sweep wrote (set_state, average-down) is filled here.
+  const bool tma = c->use_tma && L.has_tmaps;
+  const int R = P.p.lap_order;
+  const bool wrap = L.periodic_box && (tma ? (L.n[0] >= 2 * R && L.n[1] >= 2 * R && L.n[2] >= 2 * R) : (SLEDGE_K1F_PLANE != 0));
   a.wrap = wrap ? 1 : 0;
+  auto tmaps = [&](int buf, int which) -> const void* {
+    return tma ? (const void*)(tab<CUtensorMap>(c, L.off_tmaps) + (size_t)((buf & 3) * 2 + which) * L.boxdev.size()) : nullptr;
+  };
+  auto ensure_ghosts = [&](int buf, double time) -> int {
+    if (!wrap) return launch_ghosts<T>(c, l, buf, time, true, true);
+    if (!tma || L.star_ok[buf & 3]) return SLEDGE_OK;
+    L.star_ok[buf & 3] = true;
+    return launch_ghosts<T>(c, l, buf, time, true, true);
+  };
   int rc = SLEDGE_OK;
   if (pass == 0) {
-    if (!wrap) rc = launch_ghosts<T>(c, l, cur, t, true, true);
+    rc = ensure_ghosts(cur, t);
     if (rc) return rc;
     a.sten[0] = plane_ptr<T>(c, l, cur, 0);
     a.sten[1] = plane_ptr<T>(c, l, cur, 1);
+    a.tmap[0] = tmaps(cur, 0);
+    a.tmap[1] = tmaps(cur, 1);
     a.out_psi[0] = plane_ptr<T>(c, l, cur + 1, 0);
     a.out_pi[0] = plane_ptr<T>(c, l, cur + 1, 1);
-    return launch_k1<T>(c, l, FUSED_A, a);
+    rc = launch_k1<T>(c, l, FUSED_A, a);
+    L.star_ok[(cur + 1) & 3] = tma && wrap;
+    return rc;
   }
-  if (!wrap) rc = launch_ghosts<T>(c, l, cur + 1, t + 0.5 * dt, true, true);  // Y's ghosts are still valid from pass 0
+  rc = ensure_ghosts(cur + 1, t + 0.5 * dt);  // Y's ghosts are still valid from pass 0
   if (rc) return rc;
   a.sten[0] = plane_ptr<T>(c, l, cur + 1, 0);
   a.sten[1] = plane_ptr<T>(c, l, cur + 1, 1);
   a.sten[2] = plane_ptr<T>(c, l, cur, 0);
+  a.tmap[0] = tmaps(cur + 1, 0);
+  a.tmap[1] = tmaps(cur + 1, 1);
+  a.tmap[2] = tmaps(cur, 0);
   a.pnt[0] = plane_ptr<T>(c, l, cur, 1);
   a.out_psi[0] = plane_ptr<T>(c, l, cur + 2, 0);
   a.out_pi[0] = plane_ptr<T>(c, l, cur + 2, 1);
   rc = launch_k1<T>(c, l, FUSED_B, a);
   if (rc) return rc;
+  L.star_ok[(cur + 2) & 3] = tma && wrap;
   finish_step(L, cur + 2, t, dt);
   return SLEDGE_OK;
 }
@@ -842,6 +953,7 @@ int do_average_down(sledge_ctx* c, int lf) {
   a.err_flag = tab<int>(c, P.off_err);
   const int grid = F.avg_prefix.back();
   C.shell_ok[C.cur & 3] = 0;  // covered coarse cells change: ghost copies of them are stale
+  C.star_ok[C.cur & 3] = false;
   if (F.tee_on) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
     for (int q = 0; q < 4; ++q) a.tee_eps[q] = (T)F.tee_eps[q];
     a.tee_tags = F.tee_tags;
@@ -919,6 +1031,7 @@ int do_copy_comp(sledge_ctx* c, int ib, int comp, void* dense, bool to_state, bo
   const int grid = (int)std::min<long long>((total + 255) / 256, 148 * 32);
   auto* pl = plane_ptr<T>(c, l, L.cur, comp >> 1);
   if (to_state) L.shell_ok[L.cur & 3] = 0;
+  if (to_state) L.star_ok[L.cur & 3] = false;
   ++c->launches;
   if (to_state) k_copy_comp<T, true><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
   else k_copy_comp<T, false><<<grid, 256, 0, c->stream>>>(b, P.p.nghost, P.ox, e, comp, pl, (T*)dense);
@@ -971,7 +1084,18 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   auto up = [&](size_t off, const void* src, size_t bytes) {
     if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(c->arena + off, src, bytes, cudaMemcpyHostToDevice, c->stream);
   };
+  {
+    const char* ev = getenv("SLEDGE_K1_TMA");
+    c->use_tma = ev && ev[0] == '1';  // opt-in until validated on the GPU
+  }
+  for (int l = 0; l < P.p.n_levels && c->use_tma; ++l)
+    if (level_is_fused(P, l) && (rc = make_tensor_maps(c, l)) != SLEDGE_OK) {
+      g_err = c->err;
+      delete c;
+      return rc;
+    }
   for (LevelHost& L : P.lev) {
+    up(L.off_tmaps, L.tmaps_host.data(), L.tmaps_host.size() * sizeof(CUtensorMap));
     up(L.off_boxes, L.boxdev.data(), L.boxdev.size() * sizeof(BoxDev));
     up(L.off_tiles, L.tiles.data(), L.tiles.size() * sizeof(TileDev));
     up(L.off_ftiles, L.ftiles.data(), L.ftiles.size() * sizeof(TileDev));
