@@ -62,6 +62,9 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="skip the C1 CUDA-graph replay leg")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the short runs of the other BASELINE.json workloads (key other_workloads) and the C5 graph leg")
+    ap.add_argument("--other-steps", type=int, default=4)
     ap.add_argument("--e2e-steps", type=int, default=2)
     return ap.parse_args()
 
@@ -286,24 +289,12 @@ def whole_job_value(world, cell_steps, ms, stages=4):
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------------
 
-def run_sledge(args, cfg):
+def measure(args, cfg, dev, world, rank, local, steps, warmup):
+    """Build the workload `cfg` on `dev`, run `warmup` + `steps` steps and return (bench line, context, tags, counts,
+    boxes, cell_steps).  A step = sledge_rk_step + sledge_tag_strings on every level."""
     import torch
     import torch.distributed as dist
-    from paper_2404_02950_b200 import build as sbuild
     from paper_2404_02950_b200 import sledge as S
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the sledge path has no CPU fallback)")
-    torch.cuda.set_device(local)
-    dev = f"cuda:{local}"
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
-    if not os.path.exists(S.LIB_PATH):
-        sbuild.build()
-
     rings, boxes, cover = hierarchy(cfg)
     cell_steps, per_level = cells_per_step(cfg, boxes)
     s = S.Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=max(cfg.nghost, args.ko_order),
@@ -337,7 +328,7 @@ def run_sledge(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     s.synchronize()
     # ---- timed region: K steps, CUDA events on the launching stream, clocks sampled meanwhile ----
@@ -349,11 +340,11 @@ def run_sledge(args, cfg):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record()
     barrier()
-    ms = e0.elapsed_time(e1) / args.steps
+    ms = e0.elapsed_time(e1) / steps
     launches = s.launch_count() - l0
     prof = {k: s.profile_read(kind) for k, kind in
             (("stage", S.KIND_STAGE), ("ghost", S.KIND_GHOST), ("tag", S.KIND_TAG), ("avg", S.KIND_AVG))}
@@ -379,20 +370,28 @@ def run_sledge(args, cfg):
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     # profile counters cover the timed K steps: n_stage launches moved cell_steps * words * esz bytes per step
-    stage_bytes_total = stage_words_per_step * esz * args.steps
+    stage_bytes_total = stage_words_per_step * esz * steps
+    # K1 launches the timed steps must have produced (2 sweeps per level-step FUSED on level 0, one per stage
+    # otherwise); the library keeps at most 4096 event pairs per kind, so scale the bytes to the launches it timed
+    sweeps = [(2 if (l == 0 and args.flow == "fused") else (3 if ssp else 4)) * (1 << l) for l in range(cfg.n_levels)]
+    expected_stage = steps * sum(sweeps)
+    timed_all = n_stage == expected_stage
+    if not timed_all and expected_stage > 0:
+        stage_bytes_total *= n_stage / expected_stage
     achieved = stage_bytes_total / (ms_stage * 1e-3) / 1e9 if ms_stage > 0 else 0.0
     tr = ncu_traffic(cfg.name, args.flow)
-    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_plane FUSED sweeps on level 0, k_rk_pipe staged sweeps elsewhere; mean over the "
+    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_tma FUSED sweeps on level 0, k_rk_pipe staged sweeps elsewhere; mean over the "
                                           "stage launches of a step: 2 sweeps per level-step FUSED, 4 otherwise)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "peak_source": peak_src, "traffic": (tr or {}).get("dram_bytes_per_launch"), "traffic_detail": tr,
                 "bytes_per_cell_step": words_per_cell_step * esz,
-                "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage}
-    shares = {k: (v[1] / args.steps) for k, v in prof.items()}
+                "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage, "launches_expected": expected_stage,
+                "all_launches_timed": timed_all}
+    shares = {k: (v[1] / steps) for k, v in prof.items()}
 
     value = whole_job_value(world, cell_steps, ms, stages=3 if ssp else 4)
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"{cfg.name}: {cfg.n0}^3 base, {cfg.n_levels} level(s), {cfg.dtype}, "
                                    f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, {'SSPRK3' if ssp else 'RK4'} ({args.flow} data-flow), "
@@ -406,14 +405,42 @@ def run_sledge(args, cfg):
             "gcell_steps_per_s": value / (3 if ssp else 4),
             "kernel_ms_per_step": shares, "roofline": roofline, "gpu_launches": launches, "clocks": clocks}
 
+    return line, s, tags, counts, boxes, cell_steps
+
+
+def run_sledge(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2404_02950_b200 import build as sbuild
+    from paper_2404_02950_b200 import sledge as S
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the sledge path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    if not os.path.exists(S.LIB_PATH):
+        sbuild.build()
+
+    line, s, tags, counts, boxes, cell_steps = measure(args, cfg, dev, world, rank, local, args.steps, args.warmup)
+
     # ---- e2e: same step through the C ABI with HOST buffers -----------------------------------------
     if not args.no_e2e:
         line["e2e"] = e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags=(tags, counts))
     del s
     torch.cuda.empty_cache()
+    default_run = args.integrator == 4 and not args.ko_order and args.flow == "fused" and args.interp == 0
     if rank == 0 and not args.no_graph and args.integrator == 4 and not args.ko_order:
         from paper_2404_02950_b200 import inputs as _inputs
         line["c1_graph_replay"] = graph_leg(_inputs.CONFIGS["C1"], dev, "fused")
+        if default_run and not args.no_others:
+            line["c5_graph_replay"] = graph_step_leg(_inputs.CONFIGS["C5"], dev, "fused")
+    if rank == 0 and default_run and not args.no_others:
+        line["other_workloads"] = other_workloads(args, cfg, dev)
     if rank == 0 and not args.no_cpu:
         line["cpu_baseline"], _, _ = time_oracle(cfg)
     if rank == 0:
@@ -501,6 +528,104 @@ def graph_leg(cfg, dev, flow, replays=20, dt=None):
                         "restores the initial state (4 copy kernels)",
             "launches_per_run": per_run, "ms_per_step_eager": ms_eager, "ms_per_step_graph": ms_graph,
             "value_eager": cells * 4 / (ms_eager * 1e-3) / 1e9, "value_graph": cells * 4 / (ms_graph * 1e-3) / 1e9,
+            "unit": UNIT, "replay_equals_eager_bitwise": bool(same)}
+
+
+def other_workloads(args, main_cfg, dev):
+    """Short runs (resident state, same timed-region rules, `--other-steps` steps after 3 warm-up steps) of the other
+    BASELINE.json workloads that fit one GPU, so that the bench record carries them: value, ms per step, per-kernel
+    time, K1 roofline fraction, clocks.  The headline line and its config stay those of the main workload."""
+    import copy
+    import torch
+    from paper_2404_02950_b200 import inputs
+    out = {}
+    for name in ("C2", "C4", "C5"):
+        if name == main_cfg.name:
+            continue
+        a = copy.copy(args)
+        a.flow = "fused"
+        try:
+            line, s, tags, counts, _, _ = measure(a, inputs.CONFIGS[name], dev, 1, 0, 0, args.other_steps, 3)
+        except Exception as e:  # e.g. out of memory on a smaller part: reported, not fatal for the headline
+            out[name] = {"error": str(e)[:200]}
+            continue
+        out[name] = {"workload": line["config"]["workload"], "value": line["value"], "unit": UNIT, "dtype": line["dtype"],
+                     "ms_per_step": line["ms_per_step"], "steps": line["steps"],
+                     "kernel_ms_per_step": line["kernel_ms_per_step"], "k1_frac": line["roofline"]["frac"],
+                     "k1_achieved_gbs": line["roofline"]["achieved"], "gpu_launches": line["gpu_launches"],
+                     "clocks": line["clocks"]}
+        s.close()
+        del s, tags, counts
+        torch.cuda.empty_cache()
+    return out
+
+
+def graph_step_leg(cfg, dev, flow, steps=5):
+    """ONE coarse step of `cfg` (sledge_rk_step: subcycled stages, ghost fills, average-downs; then sledge_tag_strings
+    on every level) eagerly and as one CUDA graph replay: ms per coarse step of both, and
+    whether the replayed step equals the eager one bit for bit.  The graph is captured from a freshly set state, so a
+    replay recomputes that same step (the step never writes the buffer it starts from)."""
+    import torch
+    from paper_2404_02950_b200 import sledge as S
+    rings, boxes, _ = hierarchy(cfg)
+    side = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(side):
+        s = S.Sledge(cfg.n0, boxes=boxes, n_levels=cfg.n_levels, nghost=cfg.nghost, blocking_factor=cfg.blocking_factor,
+                     dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=flow, device=dev)
+        ic = {(ib, c): t for ib, c, t in initial_fields(cfg, rings, boxes, dev, s.tdtype)}
+        zero = {}
+        tags = [torch.empty(s.level_cells(l)[0], dtype=torch.uint8, device=dev) for l in range(cfg.n_levels)]
+        counts = [torch.empty(s.count_shape(l), dtype=torch.int32, device=dev) for l in range(cfg.n_levels)]
+
+        def restore():
+            for ib in range(len(boxes)):
+                for c in range(4):
+                    t = ic.get((ib, c))
+                    if t is None:
+                        t = zero.setdefault(tuple(s.box_shape(ib)), torch.zeros(s.box_shape(ib), dtype=s.tdtype, device=dev))
+                    s.set_state(ib, c, t)
+
+        def step(eta):
+            s.rk_step(cfg.dt, eta)
+            for l in range(cfg.n_levels):
+                s.tag_strings(l, tags[l], counts[l])
+
+        def timed(fn):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            fn()
+            side.synchronize()
+            e0.record(side)
+            for _ in range(steps):
+                fn()
+            e1.record(side)
+            side.synchronize()
+            return e0.elapsed_time(e1) / steps
+
+        restore()
+        l0 = s.launch_count()
+        step(cfg.eta0)
+        per_step = s.launch_count() - l0
+        ms_eager = timed(lambda: step(cfg.eta0))
+        restore()
+        step(cfg.eta0)
+        ref = [s.get_state(ib, c).clone() for ib in range(len(boxes)) for c in range(4)]
+        ref_tags = [t.clone() for t in tags]
+        restore()
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            step(cfg.eta0)
+        g.replay()
+        got = [s.get_state(ib, c) for ib in range(len(boxes)) for c in range(4)]
+        side.synchronize()
+        same = all(torch.equal(a.view(torch.int64), b.view(torch.int64)) for a, b in zip(ref, got)) and \
+            all(torch.equal(a, b) for a, b in zip(ref_tags, tags))
+        ms_graph = timed(g.replay)
+        s.close()
+    cell_steps, _ = cells_per_step(cfg, boxes)
+    return {"workload": f"{cfg.name}: one coarse step of the {len(boxes)}-box hierarchy + tags on {cfg.n_levels} levels, {flow} data-flow",
+            "launches_per_step": per_step, "ms_per_step_eager": ms_eager, "ms_per_step_graph": ms_graph,
+            "value_eager": cell_steps * 4 / (ms_eager * 1e-3) / 1e9, "value_graph": cell_steps * 4 / (ms_graph * 1e-3) / 1e9,
             "unit": UNIT, "replay_equals_eager_bitwise": bool(same)}
 
 

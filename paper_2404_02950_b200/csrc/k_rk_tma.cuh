@@ -21,7 +21,9 @@
 // Pipeline per CTA (z-march, ring of S = R + 1 + PD planes per field, as in k_rk_plane): iteration zz waits for
 // the mbarrier of plane zz + R, passes ONE __syncthreads (which retires plane zz - 1), thread 0 re-arms that
 // slot's mbarrier and issues the TMA of plane zz + R + PD into it.  Pointwise inputs keep their per-thread
-// cp.async ring.
+// cp.async ring.  (A variant without the block-wide barrier -- an "empty" mbarrier per slot on which every warp
+// arrives after its shared-memory reads, so that the warps of a CTA drift apart -- was measured 2.5 % SLOWER on
+// C3 and is not kept: profiles/r02_k1_variants.md.)
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only)
 
@@ -36,18 +38,25 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes)
                : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, unsigned parity) {
+  unsigned ok;
   asm volatile(
       "{\n\t"
       ".reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t"
-      "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
-      "r"(parity)
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}"
+      : "=r"(ok)
+      : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity)
       : "memory");
+  return ok != 0;
+}
+// try_wait suspends the thread for a hardware time slice per attempt; a load that never completes (a bad tensor
+// map) becomes a trap -- reported as SLEDGE_ECUDA by the next call -- instead of a hung GPU
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  unsigned spins = 0;
+  while (!mbar_try_wait(bar, parity))
+    if (++spins > (1u << 22)) __trap();
 }
 // one tile box: coordinates (c0 = first real, c1 = row, c2 = plane) in the box's stored array
 __device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {

@@ -1086,7 +1086,7 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   };
   {
     const char* ev = getenv("SLEDGE_K1_TMA");
-    c->use_tma = ev && ev[0] == '1';  // opt-in until validated on the GPU
+    c->use_tma = !(ev && ev[0] == '0');
   }
   for (int l = 0; l < P.p.n_levels && c->use_tma; ++l)
     if (level_is_fused(P, l) && (rc = make_tensor_maps(c, l)) != SLEDGE_OK) {
