@@ -18,6 +18,8 @@ _LIB = os.path.join(_HERE, "libsledge_oracle.so")
 
 FLAG_BLOCK = 32
 COMPS = ("psi1", "psi2", "pi1", "pi2")
+GW_COMPS = tuple(f"u_{ij}" for ij in ("xx", "yy", "zz", "xy", "xz", "yz")) + \
+    tuple(f"du_{ij}" for ij in ("xx", "yy", "zz", "xy", "xz", "yz"))  # components 4..15 (L436)
 
 
 def build(force: bool = False) -> str:
@@ -44,7 +46,15 @@ class _Params(C.Structure):
         ("ko_order", C.c_int32),
         ("integrator", C.c_int32),
         ("interp", C.c_int32),
+        ("gw", C.c_int32),
+        ("gw_coupling", C.c_double),
+        ("gw_friction", C.c_double),
+        ("rkn_stages", C.c_int32),
         ("pad_", C.c_int32),
+        ("rkn_c", C.c_double * 6),
+        ("rkn_b", C.c_double * 6),
+        ("rkn_bbar", C.c_double * 6),
+        ("rkn_a", C.c_double * 21),
     ]
 
 
@@ -74,6 +84,7 @@ def lib():
         L.orc_eval_rhs.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int]
         L.orc_rk_step.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.orc_average_down.argtypes = [C.c_void_p, C.c_int]
+        L.orc_shadow_tee.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         L.orc_tee_enable.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         L.orc_tag_strings.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_plaquette_winding.argtypes = [dp, dp, dp, dp]
@@ -111,7 +122,10 @@ class Oracle:
 
     def __init__(self, n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, lap_order=1,
                  h0=1.0, lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, ko_order=0, ko_strength=0.0,
-                 integrator=4, interp=0):
+                 integrator=4, interp=0, gw=False, gw_coupling=0.0, gw_friction=0.0, rkn=None):
+        """rkn: for integrator 20, the user's Runge-Kutta-Nystrom tableau as a dict with `nodes` (c), `weights_b`,
+        `weights_bar_b` (length s) and `tableau` (flattened lower triangle INCLUDING the diagonal, s(s+1)/2 values),
+        the four arrays of Table V (L812-815)."""
         if np.isscalar(n0):
             n0 = (int(n0),) * 3
         if boxes is None:
@@ -137,6 +151,18 @@ class Oracle:
         p.ko_order = ko_order
         p.integrator = integrator
         p.interp = interp
+        p.gw = 1 if gw else 0
+        p.gw_coupling = gw_coupling
+        p.gw_friction = gw_friction
+        self.ncomp = 16 if gw else 4
+        if rkn is not None:
+            st = len(rkn["nodes"])
+            assert len(rkn["weights_b"]) == st and len(rkn["weights_bar_b"]) == st and len(rkn["tableau"]) == st * (st + 1) // 2
+            p.rkn_stages = st
+            p.rkn_c[:st] = [float(v) for v in rkn["nodes"]]
+            p.rkn_b[:st] = [float(v) for v in rkn["weights_b"]]
+            p.rkn_bbar[:st] = [float(v) for v in rkn["weights_bar_b"]]
+            p.rkn_a[:st * (st + 1) // 2] = [float(v) for v in rkn["tableau"]]
         arr = (_Box * len(self.boxes))()
         for q, (l, lo, hi) in enumerate(self.boxes):
             arr[q].level = l
@@ -191,13 +217,14 @@ class Oracle:
         self._chk(lib().orc_fill_ghosts(self._h, level, time))
 
     def eval_rhs(self, level, eta, fill=True):
-        """k = f(Y, eta); returns [k_psi1, k_psi2, k_pi1, k_pi2] for each box of the level (valid cells)."""
+        """k = f(Y, eta); returns [k_psi1, k_psi2, k_pi1, k_pi2 (, k_u_xx .. k_du_yz)] for each box of the level
+        (valid cells)."""
         self._chk(lib().orc_eval_rhs(self._h, level, eta, 1 if fill else 0))
         g = self.nghost
         out = []
         for ib in self.level_boxes(level):
             ks = []
-            for c in range(4):
+            for c in range(self.ncomp):
                 r = self.get_raw(ib, c, which=1)
                 ks.append(r[g:-g, g:-g, g:-g].copy())
             out.append(ks)
@@ -221,6 +248,21 @@ class Oracle:
         self._tee[fine_level] = (tags, counts)
         eps = (C.c_double * 4)(eps_psi1, eps_psi2, eps_pi1, eps_pi2)
         self._chk(lib().orc_tee_enable(self._h, fine_level, eps, tags.ctypes.data, counts.ctypes.data))
+
+    def shadow_tee(self, dt, eta, eps_psi1, eps_psi2, eps_pi1=np.inf, eps_pi2=np.inf):
+        """O15 (L98): level-0 truncation-error tags against the shadow level.  Advances the hierarchy by TWO coarse
+        steps of dt; returns (list of uint8 tag arrays [z,y,x], one per level-0 box; uint32 counts [bz,by,bx])."""
+        ibs = self.level_boxes(0)
+        sizes = [int(np.prod(self.box_shape(ib))) for ib in ibs]
+        tags = np.zeros(sum(sizes), dtype=np.uint8)
+        counts = np.zeros(self.count_shape(0), dtype=np.uint32)
+        eps = (C.c_double * 4)(eps_psi1, eps_psi2, eps_pi1, eps_pi2)
+        self._chk(lib().orc_shadow_tee(self._h, dt, eta, eps, tags.ctypes.data, counts.ctypes.data))
+        out, off = [], 0
+        for ib, s in zip(ibs, sizes):
+            out.append(tags[off:off + s].reshape(self.box_shape(ib)).copy())
+            off += s
+        return out, counts
 
     def tee_tags(self, fine_level):
         """(list of uint8 tag arrays [z,y,x], one per box of the level; uint32 counts [bz,by,bx]) of the last sync."""

@@ -22,6 +22,11 @@
 //   O11 SSPRK3     : Shu-Osher three-stage scheme (integrator.type 3 / 10)            L808
 //   O10 KO term    : Kreiss-Oliger dissipation Q_l added to every component's RHS  L141-146 Eq.7
 //   O9 TEE tags    : |coarse - mean of children| > eps at synchronisation         L82-111 Eq.5-6, L373-380 Eq.12
+//   O13 GW fields  : auxiliary fields u_ij, du_ij (6 + 6 components) of Eq.16, sourced by
+//                    sum_c d_i psi_c d_j psi_c with Gradient<order>                L400-436 Eq.16
+//   O14 RKN        : user-defined Runge-Kutta-Nystrom tableau (integrator.type 20)   L808-815 Table V
+//   O15 shadow     : level-0 truncation-error tags against a coarsened copy of level 0
+//                    evolved for one step of 2 dt                                    L98
 //   O8 string tags : plaquette winding number of (psi1,psi2) around 0; rule not printed in the
 //                    paper (L349-371 gives only the bool-per-cell hook) -> DESIGN.md reading R8
 //   diagnostics    : energies used only by the pins (L678 App.B; Gradient<order> L651-658)
@@ -47,6 +52,10 @@ namespace {
 
 constexpr int NCOMP = 4;  // psi1, psi2, pi1, pi2  (L189-190)
 constexpr int PSI1 = 0, PSI2 = 1, PI1 = 2, PI2 = 3;
+// with sim.gravitational_waves (L404, L436): Gw::u_xx, yy, zz, xy, xz, yz = 4..9, Gw::du_xx .. du_yz = 10..15
+constexpr int NCOMP_GW = 16, GW_U = 4, GW_DU = 10;
+constexpr int GW_I[6] = {0, 1, 2, 0, 0, 1}, GW_J[6] = {0, 1, 2, 1, 2, 2};  // xx, yy, zz, xy, xz, yz (L436)
+constexpr int RKN_MAX = 6;
 constexpr int FLAG_BLOCK = 32;  // box-flag reduction granularity (BASELINE.json config 3)
 
 struct Params {
@@ -65,7 +74,15 @@ struct Params {
   int32_t integrator;     // integrator.type (L808): 0 or 4 = RK4; 3 or 10 = SSPRK3 (10 = its low-storage form)
   int32_t interp;         // coarse->fine ghost interpolation: 0 = cell-centred trilinear (BASELINE.json config 5),
                           // 4 = quartic polynomial conservative (amr.interpolation_type 4, the paper's default)
+  int32_t gw;             // sim.gravitational_waves (L404): 1 = evolve the 12 auxiliary components as well
+  double gw_coupling;     // Eq.16's 16 pi G (times whatever the project's units absorb), multiplies T_ij
+  double gw_friction;     // Eq.16's 3H written like Eq.11's 2/eta: the friction term is (gw_friction / eta) du_ij
+  int32_t rkn_stages;     // integrator.type 20: number of stages s of the user's RKN tableau, 1..RKN_MAX
   int32_t pad_;
+  double rkn_c[RKN_MAX];     // rkn.nodes (L814)
+  double rkn_b[RKN_MAX];     // rkn.weights_b (L812)
+  double rkn_bbar[RKN_MAX];  // rkn.weights_bar_b (L813)
+  double rkn_a[RKN_MAX * (RKN_MAX + 1) / 2];  // rkn.tableau (L815): rows of the lower triangle incl. the diagonal
 };
 
 struct BoxIn {
@@ -79,14 +96,16 @@ struct Field {
   int n[3] = {0, 0, 0};
   int g = 0;
   int s[3] = {0, 0, 0};
+  int nc = NCOMP;
   std::vector<double> v;
-  void init(const int nn[3], int gg) {
+  void init(const int nn[3], int gg, int ncomp = NCOMP) {
     g = gg;
+    nc = ncomp;
     for (int d = 0; d < 3; ++d) {
       n[d] = nn[d];
       s[d] = nn[d] + 2 * gg;
     }
-    v.assign((size_t)NCOMP * s[0] * s[1] * s[2], 0.0);
+    v.assign((size_t)nc * s[0] * s[1] * s[2], 0.0);
   }
   // i,j,k relative to the box's low corner; ghosts are -g..-1 and n..n+g-1.
   inline double& at(int c, int i, int j, int k) {
@@ -110,6 +129,7 @@ struct Level {
   double t_old = 0, t_new = 0;
   bool have_pair = false;
   LevelState K[4];          // RK4 slopes (k of the last orc_eval_rhs in K[0])
+  std::vector<LevelState> KN;  // O14: f_j of the RKN stages (allocated on first use)
   LevelState U;             // stage state
   // O9: truncation-error tags of this (fine) level, written by average_down when tee_on (L82-111, Eq.5-6, Eq.12)
   bool tee_on = false;
@@ -154,7 +174,15 @@ bool build(Oracle& o, const BoxIn* b, int nbox) {
     if (!(p.ko_strength[c] >= 0.0)) { o.err = "dissipation strength must be >= 0 (L749)"; return false; }
   if (ko_on && (p.ko_order < 2 || p.ko_order > 3)) { o.err = "dissipation order must be 2 or 3 (L751)"; return false; }
   if (ko_on && p.ko_order > p.nghost) { o.err = "dissipation order must be <= nghost (L751)"; return false; }
-  if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10) { o.err = "integrator.type must be 4 (RK4) or 3 / 10 (SSPRK3) (L808)"; return false; }
+  if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10 && p.integrator != 20) { o.err = "integrator.type must be 4 (RK4), 3 / 10 (SSPRK3) or 20 (user RKN tableau) (L808)"; return false; }
+  if (p.integrator == 20) {  // O14: an explicit Nystrom scheme integrates psi'' = f(psi, eta): no first-derivative terms
+    if (p.rkn_stages < 1 || p.rkn_stages > RKN_MAX) { o.err = "rkn: 1..6 stages"; return false; }
+    if (p.friction != 0.0 || ko_on) { o.err = "rkn: the scheme needs psi'' = f(psi): friction and dissipation must be 0"; return false; }
+    if (p.gw) { o.err = "rkn: gravitational-wave fields are not integrated by the RKN scheme"; return false; }
+    for (int i = 0; i < p.rkn_stages; ++i)
+      if (p.rkn_a[i * (i + 1) / 2 + i] != 0.0) { o.err = "rkn.tableau: only explicit schemes (zero diagonal) (L815)"; return false; }
+  }
+  if (p.gw != 0 && p.gw != 1) { o.err = "gw must be 0 or 1 (L404)"; return false; }
   if (p.interp != 0 && p.interp != 4) { o.err = "interp must be 0 (trilinear) or 4 (quartic conservative, L780)"; return false; }
   if (!(p.h0 > 0)) { o.err = "h0 must be positive"; return false; }
   o.lev.resize(p.n_levels);
@@ -226,7 +254,7 @@ bool build(Oracle& o, const BoxIn* b, int nbox) {
       for (size_t q = 0; q < L.boxes.size(); ++q) {
         const BoxIn& B = o.box[L.boxes[q]];
         int nn[3] = {B.hi[0] - B.lo[0] + 1, B.hi[1] - B.lo[1] + 1, B.hi[2] - B.lo[2] + 1};
-        S[q].init(nn, p.nghost);
+        S[q].init(nn, p.nghost, p.gw ? NCOMP_GW : NCOMP);
       }
     };
     alloc(L.Y); alloc(L.Yold); alloc(L.U);
@@ -286,7 +314,7 @@ bool fill_ghosts(Oracle& o, int l, LevelState& S, double time) {
           int ow = owner_of(o, l, wi, wj, wk);
           if (ow >= 0) {
             const BoxIn& Bo = o.box[L.boxes[ow]];
-            for (int c = 0; c < NCOMP; ++c)
+            for (int c = 0; c < F.nc; ++c)
               F.at(c, i, j, k) = S[ow].at(c, wi - Bo.lo[0], wj - Bo.lo[1], wk - Bo.lo[2]);
             continue;
           }
@@ -308,7 +336,7 @@ bool fill_ghosts(Oracle& o, int l, LevelState& S, double time) {
                                             {3.0 / 128, -22.0 / 128, 1.0, 22.0 / 128, -3.0 / 128}};
             int r[3];
             for (int d = 0; d < 3; ++d) r[d] = f[d] - 2 * c0[d];
-            for (int c = 0; c < NCOMP; ++c) {
+            for (int c = 0; c < F.nc; ++c) {
               double sum = 0.0;
               for (int mz = -2; mz <= 2; ++mz)
                 for (int my = -2; my <= 2; ++my)
@@ -324,7 +352,7 @@ bool fill_ghosts(Oracle& o, int l, LevelState& S, double time) {
             continue;
           }
           const double w[2] = {0.75, 0.25};
-          for (int c = 0; c < NCOMP; ++c) {
+          for (int c = 0; c < F.nc; ++c) {
             double sum = 0.0;
             for (int dz = 0; dz < 2; ++dz)
               for (int dy = 0; dy < 2; ++dy)
@@ -404,6 +432,22 @@ inline double ko_term(const Field& F, int c, int i, int j, int k, int r, double 
   return sign * eps / (std::pow(2.0, 2 * r) * h) * sum;
 }
 
+// ---- Gradient<order> (L651-658) ------------------------------------------------------------------
+// "three-point, five-point, and seven-point stencil" for order 1, 2, 3; coefficients not printed: the unique
+// maximal-order central first-difference stencils,
+//   order 1: (u(+1) - u(-1)) / (2h)
+//   order 2: (8 (u(+1) - u(-1)) - (u(+2) - u(-2))) / (12h)
+//   order 3: (45 (u(+1) - u(-1)) - 9 (u(+2) - u(-2)) + (u(+3) - u(-3))) / (60h)
+// (pinned by polynomial exactness up to degree 2 / 4 / 6 and the plane-wave symbols).
+inline double gradient(const Field& F, int c, int i, int j, int k, int d, int order, double h) {
+  int e[3] = {0, 0, 0};
+  e[d] = 1;
+  auto u = [&](int m) { return F.at(c, i + m * e[0], j + m * e[1], k + m * e[2]); };
+  if (order == 1) return (u(1) - u(-1)) / (2.0 * h);
+  if (order == 2) return (8.0 * (u(1) - u(-1)) - (u(2) - u(-2))) / (12.0 * h);
+  return ((45.0 * (u(1) - u(-1)) - 9.0 * (u(2) - u(-2))) + (u(3) - u(-3))) / (60.0 * h);
+}
+
 // ---- O3: right-hand side, Eq.10-11 ------------------------------------------------------------
 //   k_psi_c = Pi_c
 //   k_Pi_c  = -(kappa/eta) Pi_c + Lap(psi_c) - lambda eta^2 psi_c (psi1^2 + psi2^2 - 1) - a psi_c
@@ -429,6 +473,25 @@ void eval_rhs(const Oracle& o, int l, const LevelState& S, LevelState& K, double
           R.at(PI2, i, j, k) = (lap2 - psi2 * pot) - fr * pi2;
           for (int c = 0; c < NCOMP; ++c)  // Eq.7: Q_l u_c added to the evolution of every component
             if (p.ko_strength[c] != 0.0) R.at(c, i, j, k) += ko_term(F, c, i, j, k, p.ko_order, p.ko_strength[c], L.h);
+          if (p.gw) {
+            // O13, Eq.16 (L400-436) in the conformal-time form of Eq.9-11 (R25): for the six auxiliary
+            // components ij = xx, yy, zz, xy, xz, yz
+            //   k_u_ij  = du_ij
+            //   k_du_ij = -(kappa_u / eta) du_ij + Lap(u_ij) + c_gw T_ij,   T_ij = sum_c d_i psi_c d_j psi_c
+            // with Laplacian<order> and Gradient<order> of the same order (L649-658); the trace part of the scalar
+            // stress tensor (delta_ij L) drops out under the TT projection of Eq.13-15 and is not added.
+            double gr[2][3];
+            for (int c = 0; c < 2; ++c)
+              for (int d = 0; d < 3; ++d) gr[c][d] = gradient(F, c, i, j, k, d, p.lap_order, L.h);
+            double fru = (p.gw_friction != 0.0) ? p.gw_friction / eta : 0.0;
+            for (int m = 0; m < 6; ++m) {
+              double T = gr[0][GW_I[m]] * gr[0][GW_J[m]] + gr[1][GW_I[m]] * gr[1][GW_J[m]];
+              double lapu = laplacian(F, GW_U + m, i, j, k, p.lap_order, L.h);
+              double du = F.at(GW_DU + m, i, j, k);
+              R.at(GW_U + m, i, j, k) = du;
+              R.at(GW_DU + m, i, j, k) = (lapu + p.gw_coupling * T) - fru * du;
+            }
+          }
         }
   }
 }
@@ -436,9 +499,9 @@ void eval_rhs(const Oracle& o, int l, const LevelState& S, LevelState& K, double
 // ---- O7: average-down, O9: truncation-error tags ----------------------------------------------
 // O9 (self-shadow method, L82-98; Eq.5, Eq.6/12 with f = identity): just before level lf is synchronised onto
 // lf-1, both have evolved the same region independently for 2 dt_lf.  For every coarse cell C under fine cells
-//   Delta_c(C) = | phi_c^{lf-1}(C) - (1/8) sum_children phi_c^{lf} |,   c = psi1, psi2 (the scalar components),
+//   Delta_c(C) = | phi_c^{lf-1}(C) - (1/8) sum_children phi_c^{lf} |,   c = psi1, psi2, Pi1, Pi2 (R21),
 // with the coarse value taken BEFORE it is overwritten, and the 8 children of C get the tag byte
-//   bit0 = Delta_psi1 > eps_psi1,  bit1 = Delta_psi2 > eps_psi2          (strict >, Eq.12).
+//   bit c = Delta_c > eps_c, one threshold per component            (strict >, Eq.12).
 // counts: tagged fine cells per aligned FLAG_BLOCK^3 block of level lf.
 bool average_down(Oracle& o, int lf) {
   if (lf < 1 || lf >= o.p.n_levels) { o.err = "average_down: bad fine level"; return false; }
@@ -461,14 +524,14 @@ bool average_down(Oracle& o, int lf) {
           if (ow < 0) { all_ok = false; continue; }
           const BoxIn& Bc = o.box[Lc.boxes[ow]];
           uint8_t tag = 0;
-          for (int c = 0; c < NCOMP; ++c) {
+          for (int c = 0; c < F.nc; ++c) {
             double s = 0.0;
             for (int rz = 0; rz < 2; ++rz)
               for (int ry = 0; ry < 2; ++ry)
                 for (int rx = 0; rx < 2; ++rx) s += F.at(c, i + rx, j + ry, k + rz);
             double mean = 0.125 * s;
             double& coarse = Lc.Y[ow].at(c, ci - Bc.lo[0], cj - Bc.lo[1], ck - Bc.lo[2]);
-            if (tee) {  // every component has its own threshold; DBL_MAX (the default) never tags
+            if (tee && c < NCOMP) {  // every scalar component has its own threshold; DBL_MAX (the default) never tags
               double delta = std::fabs(coarse - mean);
               if (delta > Lf.tee_eps[c]) tag |= (uint8_t)(1u << c);
             }
@@ -520,7 +583,7 @@ bool advance_ssprk3(Oracle& o, int l, double t, double dt, double eta_const) {
       Field& U = L.U[q];
       const Field& Y = L.Y[q];
       const Field& K = L.K[s][q];
-      for (int c = 0; c < NCOMP; ++c)
+      for (int c = 0; c < U.nc; ++c)
         for (int k = 0; k < U.n[2]; ++k)
           for (int j = 0; j < U.n[1]; ++j)
             for (int i = 0; i < U.n[0]; ++i) {
@@ -541,8 +604,75 @@ bool advance_ssprk3(Oracle& o, int l, double t, double dt, double eta_const) {
   return true;
 }
 
+// ---- O14: user-defined Runge-Kutta-Nystrom scheme (integrator.type 20, L808-815) ------------------
+// For psi'' = f(psi, eta) (Eq.9-11 without the friction term: f = Lap psi - psi (lambda eta^2 (|psi|^2 - 1) + a)),
+// with the user's nodes c, weights b, bar-b and strictly lower-triangular tableau a (R26), s stages:
+//   Psi_i   = psi + c_i dt Pi + dt^2 sum_{j<i} a_ij f_j,      f_i = f(Psi_i, t + c_i dt)
+//   psi_new = psi + dt Pi + dt^2 sum_i bbar_i f_i,            Pi_new = Pi + dt sum_i b_i f_i
+// Ghosts of a stage field are filled at its time t + c_i dt like those of any stage state (L72).  Sums run over
+// j (i) ascending, starting from 0.
+bool advance_rkn(Oracle& o, int l, double t, double dt, double eta_const) {
+  Level& L = o.lev[l];
+  const Params& p = o.p;
+  const int s = p.rkn_stages;
+  if ((int)L.KN.size() < s) {
+    L.KN.resize(s);
+    for (int i = 0; i < s; ++i) L.KN[i] = L.K[0];
+  }
+  L.Yold = L.Y;
+  for (int i = 0; i < s; ++i) {
+    const double* arow = p.rkn_a + i * (i + 1) / 2;
+#pragma omp parallel for schedule(dynamic)
+    for (int q = 0; q < (int)L.boxes.size(); ++q) {
+      Field& U = L.U[q];
+      const Field& Y = L.Y[q];
+      for (int c = 0; c < 2; ++c)
+        for (int k = 0; k < U.n[2]; ++k)
+          for (int j = 0; j < U.n[1]; ++j)
+            for (int ii = 0; ii < U.n[0]; ++ii) {
+              double acc = 0.0;
+              for (int m = 0; m < i; ++m) acc += arow[m] * L.KN[m][q].at(PI1 + c, ii, j, k);
+              U.at(c, ii, j, k) = (Y.at(c, ii, j, k) + (p.rkn_c[i] * dt) * Y.at(PI1 + c, ii, j, k)) + (dt * dt) * acc;
+              U.at(PI1 + c, ii, j, k) = Y.at(PI1 + c, ii, j, k);
+            }
+    }
+    double ts = t + p.rkn_c[i] * dt;
+    if (!fill_ghosts(o, l, L.U, ts)) return false;
+    double eta_s = p.eta_fixed ? eta_const : ts;
+    eval_rhs(o, l, L.U, L.KN[i], eta_s);  // friction = 0, no dissipation: its Pi components are f_i
+  }
+#pragma omp parallel for schedule(dynamic)
+  for (int q = 0; q < (int)L.boxes.size(); ++q) {
+    Field& Y = L.Y[q];
+    for (int c = 0; c < 2; ++c)
+      for (int k = 0; k < Y.n[2]; ++k)
+        for (int j = 0; j < Y.n[1]; ++j)
+          for (int i = 0; i < Y.n[0]; ++i) {
+            double sb = 0.0, sbb = 0.0;
+            for (int m = 0; m < s; ++m) {
+              double f = L.KN[m][q].at(PI1 + c, i, j, k);
+              sb += p.rkn_b[m] * f;
+              sbb += p.rkn_bbar[m] * f;
+            }
+            double y = Y.at(c, i, j, k), yp = Y.at(PI1 + c, i, j, k);
+            Y.at(c, i, j, k) = (y + dt * yp) + (dt * dt) * sbb;
+            Y.at(PI1 + c, i, j, k) = yp + dt * sb;
+          }
+  }
+  L.t_old = t;
+  L.t_new = t + dt;
+  L.have_pair = true;
+  if (l + 1 < o.p.n_levels) {
+    if (!advance(o, l + 1, t, 0.5 * dt, eta_const)) return false;
+    if (!advance(o, l + 1, t + 0.5 * dt, 0.5 * dt, eta_const)) return false;
+    if (!average_down(o, l + 1)) return false;
+  }
+  return true;
+}
+
 bool advance(Oracle& o, int l, double t, double dt, double eta_const) {
   if (o.p.integrator == 3 || o.p.integrator == 10) return advance_ssprk3(o, l, t, dt, eta_const);
+  if (o.p.integrator == 20) return advance_rkn(o, l, t, dt, eta_const);
   Level& L = o.lev[l];
   static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
   static const double as[3] = {0.5, 0.5, 1.0};
@@ -560,7 +690,7 @@ bool advance(Oracle& o, int l, double t, double dt, double eta_const) {
         Field& U = L.U[q];
         const Field& Y = L.Y[q];
         const Field& K = L.K[s][q];
-        for (int c = 0; c < NCOMP; ++c)
+        for (int c = 0; c < U.nc; ++c)
           for (int k = 0; k < U.n[2]; ++k)
             for (int j = 0; j < U.n[1]; ++j)
               for (int i = 0; i < U.n[0]; ++i) U.at(c, i, j, k) = Y.at(c, i, j, k) + adt * K.at(c, i, j, k);
@@ -570,7 +700,7 @@ bool advance(Oracle& o, int l, double t, double dt, double eta_const) {
 #pragma omp parallel for schedule(dynamic)
   for (int q = 0; q < (int)L.boxes.size(); ++q) {
     Field& Y = L.Y[q];
-    for (int c = 0; c < NCOMP; ++c)
+    for (int c = 0; c < Y.nc; ++c)
       for (int k = 0; k < Y.n[2]; ++k)
         for (int j = 0; j < Y.n[1]; ++j)
           for (int i = 0; i < Y.n[0]; ++i) {
@@ -653,16 +783,6 @@ bool tag_strings(Oracle& o, int l, uint8_t* tags, uint32_t* counts) {
   return true;
 }
 
-// ---- diagnostics used by the pins (single-level, level 0) ---------------------------------------
-// Gradient<order> (L651-658): 3-point [ -1, 0, 1 ]/(2h), 5-point [1,-8,0,8,-1]/(12h).
-inline double gradient(const Field& F, int c, int i, int j, int k, int d, int order, double h) {
-  int e[3] = {0, 0, 0};
-  e[d] = 1;
-  auto u = [&](int m) { return F.at(c, i + m * e[0], j + m * e[1], k + m * e[2]); };
-  if (order == 1) return (u(1) - u(-1)) / (2.0 * h);
-  return (8.0 * (u(1) - u(-1)) - (u(2) - u(-2))) / (12.0 * h);
-}
-
 }  // namespace
 
 // =================================================================================================
@@ -682,7 +802,11 @@ typedef struct {
   int32_t ko_order;
   int32_t integrator;
   int32_t interp;
+  int32_t gw;
+  double gw_coupling, gw_friction;
+  int32_t rkn_stages;
   int32_t pad_;
+  double rkn_c[6], rkn_b[6], rkn_bbar[6], rkn_a[21];
 } orc_params;
 
 typedef struct {
@@ -718,7 +842,7 @@ int orc_num_boxes(void* h, int level) { return (int)((Oracle*)h)->lev[level].box
 // src/dst: dense valid region of global box `ib`, x fastest.
 int orc_set_state(void* h, int ib, int comp, const double* src) {
   Oracle& o = *(Oracle*)h;
-  if (ib < 0 || ib >= (int)o.box.size() || comp < 0 || comp >= NCOMP) return -1;
+  if (ib < 0 || ib >= (int)o.box.size() || comp < 0 || comp >= (o.p.gw ? NCOMP_GW : NCOMP)) return -1;
   Field& F = o.lev[o.box[ib].level].Y[o.box_local[ib]];
   size_t q = 0;
   for (int k = 0; k < F.n[2]; ++k)
@@ -728,7 +852,7 @@ int orc_set_state(void* h, int ib, int comp, const double* src) {
 }
 int orc_get_state(void* h, int ib, int comp, double* dst) {
   Oracle& o = *(Oracle*)h;
-  if (ib < 0 || ib >= (int)o.box.size() || comp < 0 || comp >= NCOMP) return -1;
+  if (ib < 0 || ib >= (int)o.box.size() || comp < 0 || comp >= (o.p.gw ? NCOMP_GW : NCOMP)) return -1;
   const Field& F = o.lev[o.box[ib].level].Y[o.box_local[ib]];
   size_t q = 0;
   for (int k = 0; k < F.n[2]; ++k)
@@ -794,6 +918,77 @@ int orc_tee_enable(void* h, int fine_level, const double* eps4, uint8_t* tags, u
 }
 
 int orc_average_down(void* h, int fine_level) { return average_down(*(Oracle*)h, fine_level) ? 0 : -1; }
+
+// O15, the shadow level (L98; R27): level 0 has no coarser partner, so "shortly before cell tagging" a
+// coarsened copy of it is made -- shadow cell C <- mean of its 8 level-0 children, spacing 2 h_0, ONE box over the
+// same periodic domain -- and evolved for a single step of 2 dt while the hierarchy takes two coarse steps of dt; then
+//   Delta_c(C) = | shadow_c(C) - (1/8) sum_children phi_c^0 |,  c = psi1, psi2, Pi1, Pi2
+// tags the 8 children with bit c iff Delta_c > eps_c (strict, as O9), and the shadow level is discarded.
+// tags: one byte per valid level-0 cell, boxes back to back in input order, x fastest; counts: tagged cells per
+// aligned 32^3 block of level 0.  The hierarchy ends at eta + 2 dt.
+int orc_shadow_tee(void* h, double dt, double eta, const double* eps4, uint8_t* tags, uint32_t* counts) {
+  Oracle& o = *(Oracle*)h;
+  const Params& p = o.p;
+  Oracle sh;
+  sh.p = p;
+  sh.p.n_levels = 1;
+  sh.p.h0 = 2.0 * p.h0;
+  int bf = p.blocking_factor;
+  for (int d = 0; d < 3; ++d) {
+    if (p.n0[d] % 2) { o.err = "shadow level: n0 must be even"; return -1; }
+    sh.p.n0[d] = p.n0[d] / 2;
+    while (bf > 1 && sh.p.n0[d] % bf) bf /= 2;
+  }
+  sh.p.blocking_factor = bf;
+  BoxIn sb;
+  sb.level = 0;
+  for (int d = 0; d < 3; ++d) { sb.lo[d] = 0; sb.hi[d] = sh.p.n0[d] - 1; }
+  if (!build(sh, &sb, 1)) { o.err = "shadow level: " + sh.err; return -1; }
+  Level& L0 = o.lev[0];
+  Field& S = sh.lev[0].Y[0];
+  auto child = [&](int c, int i, int j, int k) {  // valid level-0 value at level index (i, j, k)
+    int ow = owner_of(o, 0, i, j, k);
+    const BoxIn& B = o.box[L0.boxes[ow]];
+    return L0.Y[ow].at(c, i - B.lo[0], j - B.lo[1], k - B.lo[2]);
+  };
+  auto mean8 = [&](int c, int I, int J, int K) {
+    double s = 0.0;
+    for (int rz = 0; rz < 2; ++rz)
+      for (int ry = 0; ry < 2; ++ry)
+        for (int rx = 0; rx < 2; ++rx) s += child(c, 2 * I + rx, 2 * J + ry, 2 * K + rz);
+    return 0.125 * s;
+  };
+  for (int c = 0; c < S.nc; ++c)
+    for (int K = 0; K < S.n[2]; ++K)
+      for (int J = 0; J < S.n[1]; ++J)
+        for (int I = 0; I < S.n[0]; ++I) S.at(c, I, J, K) = mean8(c, I, J, K);
+  if (!advance(sh, 0, eta, 2.0 * dt, eta)) { o.err = "shadow level: " + sh.err; return -1; }
+  if (!advance(o, 0, eta, dt, eta)) return -1;
+  if (!advance(o, 0, eta + dt, dt, eta + dt)) return -1;
+  int nb[3];
+  for (int d = 0; d < 3; ++d) nb[d] = (L0.n[d] + FLAG_BLOCK - 1) / FLAG_BLOCK;
+  if (counts) memset(counts, 0, sizeof(uint32_t) * (size_t)nb[0] * nb[1] * nb[2]);
+  std::vector<size_t> tag_off(L0.boxes.size(), 0);
+  for (size_t q = 1; q < L0.boxes.size(); ++q)
+    tag_off[q] = tag_off[q - 1] + (size_t)L0.Y[q - 1].n[0] * L0.Y[q - 1].n[1] * L0.Y[q - 1].n[2];
+  for (int K = 0; K < S.n[2]; ++K)
+    for (int J = 0; J < S.n[1]; ++J)
+      for (int I = 0; I < S.n[0]; ++I) {
+        uint8_t tag = 0;
+        for (int c = 0; c < NCOMP; ++c)
+          if (std::fabs(S.at(c, I, J, K) - mean8(c, I, J, K)) > eps4[c]) tag |= (uint8_t)(1u << c);
+        int ow = owner_of(o, 0, 2 * I, 2 * J, 2 * K);
+        const BoxIn& B = o.box[L0.boxes[ow]];
+        const Field& F = L0.Y[ow];
+        for (int rz = 0; rz < 2; ++rz)
+          for (int ry = 0; ry < 2; ++ry)
+            for (int rx = 0; rx < 2; ++rx)
+              if (tags)
+                tags[tag_off[ow] + ((size_t)(2 * K + rz - B.lo[2]) * F.n[1] + (2 * J + ry - B.lo[1])) * F.n[0] + (2 * I + rx - B.lo[0])] = tag;
+        if (tag && counts) counts[((size_t)(2 * K / FLAG_BLOCK) * nb[1] + 2 * J / FLAG_BLOCK) * nb[0] + 2 * I / FLAG_BLOCK] += 8;
+      }
+  return 0;
+}
 
 int orc_tag_strings(void* h, int level, uint8_t* tags, uint32_t* counts) {
   Oracle& o = *(Oracle*)h;
