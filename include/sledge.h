@@ -46,6 +46,7 @@ enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1, SLEDGE_RK_FUSED = 2 };
 
 /* Inclusive cell range lo..hi of one box in the index space of `level`; axis order x, y, z. */
 enum { SLEDGE_INTERP_TRILINEAR = 0, SLEDGE_INTERP_QUARTIC = 4 };
+enum { SLEDGE_NCOMP = 4, SLEDGE_NCOMP_GW = 16, SLEDGE_RKN_MAX_STAGES = 5 };
 
 typedef struct {
   int32_t level;
@@ -75,14 +76,36 @@ typedef struct {
                               k_psi = Pi pointwise) and the stage fills move Pi ghosts as well.          */
   int32_t ko_order;        /* r = sim.dissipation_order in {2,3} = ghost cells the term needs (L751): r <= nghost */
   int32_t integrator;      /* integrator.type (L808): 0 or 4 = classic RK4; 3 or 10 = SSPRK3 (Shu-Osher form,
-                              three state buffers, 32 words per cell-step; rk_dataflow is ignored)      */
+                              three state buffers, 32 words per cell-step; rk_dataflow is ignored); 20 = the user's
+                              Runge-Kutta-Nystrom tableau below (rk_dataflow is ignored)                  */
   int32_t interp;          /* coarse->fine ghost interpolation (L70-72): SLEDGE_INTERP_TRILINEAR = cell-centred
                               trilinear, weights 3/4, 1/4 per axis (BASELINE.json config 5); SLEDGE_INTERP_QUARTIC =
                               amr.interpolation_type 4, the paper's default (L780): per axis the quartic matching the
                               averages of the coarse cells c0-2..c0+2, averaged over the fine cell,
                               c0 -+ (3 c[-2] - 22 c[-1] + 22 c[+1] - 3 c[+2])/128, tensor product; both linear in time.
                               Quartic needs ceil(nghost/2) + 2 <= blocking_factor/2 on a multi-level hierarchy. */
-  int32_t reserved_;       /* 0 */
+  int32_t shadow_level;    /* 1 = reserve room in the arena for the shadow level of level 0 (L98): a coarsened copy of
+                              level 0 (spacing 2 h0, one periodic box) that sledge_shadow_tee evolves; n0 must be even */
+  int32_t gw;              /* sim.gravitational_waves (L404): 1 = every cell also carries the auxiliary fields of Eq.16,
+                              components 4..9 = Gw::u_xx, u_yy, u_zz, u_xy, u_xz, u_yz and 10..15 = Gw::du_xx .. du_yz
+                              (L436), evolved with (R25, conformal-time form of Eq.16 like Eq.9-11)
+                                k_u_ij = du_ij,  k_du_ij = -(gw_friction/eta) du_ij + Lap u_ij + gw_coupling T_ij,
+                                T_ij = sum_c d_i psi_c d_j psi_c,  Laplacian<lap_order> and Gradient<lap_order> (L649-658).
+                              Classic RK4 only; the scalar sector then runs the staged LEAN / CLASSIC sweeps (the
+                              source needs psi of every stage state), the auxiliary fields the LEAN data-flow;
+                              trilinear coarse->fine interpolation only.                                        */
+  int32_t rkn_stages;      /* integrator 20: stages s of the tableau, 1..5                                     */
+  double gw_coupling;      /* Eq.16's 16 pi G in the project's units                                           */
+  double gw_friction;      /* Eq.16's 3H written like Eq.11's 2/eta: friction term (gw_friction / eta) du_ij    */
+  /* integrator.type 20 (L808-815 Table V; R26): explicit Runge-Kutta-Nystrom scheme for
+   * psi'' = f(psi, eta) = Lap psi - psi (lambda eta^2 (|psi|^2 - 1) + a_mass); friction and ko_strength must be 0:
+   *   Psi_i = psi + c_i dt Pi + dt^2 sum_{j<i} a_ij f_j,  f_i = f(Psi_i, eta + c_i dt)
+   *   psi' = psi + dt Pi + dt^2 sum_i barb_i f_i,          Pi' = Pi + dt sum_i b_i f_i                        */
+  double rkn_nodes[6];         /* rkn.nodes c (L814); entries past rkn_stages are ignored                      */
+  double rkn_weights_b[6];     /* rkn.weights_b (L812)                                                          */
+  double rkn_weights_bar_b[6]; /* rkn.weights_bar_b (L813)                                                      */
+  double rkn_tableau[21];      /* rkn.tableau (L815): flattened lower triangle INCLUDING the diagonal, row i =
+                                  a_i0 .. a_ii; the diagonal must be 0 (explicit schemes only)                  */
 } sledge_params;
 
 /* Size of the device arena needed for this hierarchy.  Host-only: validates params and boxes
@@ -96,7 +119,7 @@ int sledge_create(sledge_ctx** ctx, const sledge_params* params, const sledge_bo
                   void* dev_arena, size_t arena_bytes, void* cuda_stream);
 int sledge_destroy(sledge_ctx* ctx);
 
-/* Copy one component of one box between a dense device array of its valid region (x fastest,
+/* Copy one component (0..3, or 0..15 with gw) of one box between a dense device array of its valid region (x fastest,
  * nx*ny*nz reals of the context's dtype) and the current state.  Setting a state invalidates the
  * level's (old,new) pair used for temporal ghost interpolation. */
 int sledge_set_state(sledge_ctx* ctx, int box, int comp, const void* dev_src);
@@ -162,9 +185,21 @@ int sledge_average_down(sledge_ctx* ctx, int fine_level);
  *                refilled at every synchronisation: tagged fine cells in the block; may be NULL.
  * Both NULL switches the tags off.  The buffers stay owned by the caller and must stay valid while enabled.  A level
  * synchronises once per step of its parent, so after sledge_rk_step the buffers hold the LAST synchronisation.
- * Level 0 has no coarser partner (the paper's shadow level, L98, is not built): SLEDGE_EINVAL. */
+ * Level 0 has no coarser partner: SLEDGE_EINVAL here; its tags come from sledge_shadow_tee below. */
 int sledge_tee_enable(sledge_ctx* ctx, int fine_level, const double* eps4, uint8_t* dev_tags,
                       uint32_t* dev_counts);
+
+/* Truncation-error tags of LEVEL 0 through the shadow level (L98: "we do indeed introduce such a coarsened version of the
+ * coarse level ... only evolved for a single time step Delta t_s = 2 Delta t_{l=0}"; R27).  Needs
+ * shadow_level = 1 at create.  The call (1) fills the shadow level with the mean of the 8 level-0 children of each of
+ * its cells (K4 run into the shadow box), (2) advances the shadow level by ONE step of 2 dt from eta (same equation,
+ * spacing 2 h0, periodic) and the hierarchy by TWO coarse steps of dt (as two sledge_rk_step calls at eta and eta + dt),
+ * (3) compares, for every shadow cell C, Delta_c = |shadow_c(C) - mean of its 8 level-0 children| with eps4[c] and gives
+ * the 8 children the tag byte sum_c (Delta_c > eps4[c]) << c (the K4 TEE kernel of sledge_tee_enable, coarse side =
+ * the shadow box).  dev_tags: one byte per valid level-0 cell, boxes back to back in input order, x fastest, 2-byte
+ * aligned; dev_counts: uint32 per aligned 32^3 block of level 0, zeroed by the call; either may be NULL.  Afterwards the
+ * hierarchy is at eta + 2 dt and the shadow level's contents are dead (it is rebuilt by the next call). */
+int sledge_shadow_tee(sledge_ctx* ctx, double dt, double eta, const double* eps4, uint8_t* dev_tags, uint32_t* dev_counts);
 
 /* Bookkeeping. */
 int sledge_level_cells(const sledge_ctx* ctx, int level, int64_t* valid_cells, int64_t* count_blocks);

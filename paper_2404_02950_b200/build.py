@@ -16,7 +16,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsledge.so")
 SOURCES = ["sledge.cu"]
-DEPS = ["sledge.cu", "layout.h", "k_rk_pipe.cuh", "k_rk_plane.cuh", "k_ghost.cuh", "k_tag.cuh", "k_avgdown.cuh",
+DEPS = ["sledge.cu", "layout.h", "k_rk_pipe.cuh", "k_rk_plane.cuh", "k_rk_tma.cuh", "k_gw.cuh", "k_ghost.cuh", "k_tag.cuh",
+        "k_avgdown.cuh",
         os.path.join("..", "..", "include", "sledge.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--fmad=false",
               "-shared", "-Xcompiler", "-fPIC"]

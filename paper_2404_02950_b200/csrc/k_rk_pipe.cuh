@@ -41,7 +41,10 @@ enum StageMode {
   CLASSIC_S4 = 5,
   FUSED_A = 6,
   FUSED_B = 7,
-  SSP_S23 = 8  // SSPRK3 (integrator.type 3 / 10, L808) stages 2 and 3: out = wy Y + wu (U + dt k(U)); stage 1 = LEAN_S1
+  SSP_S23 = 8,  // SSPRK3 (integrator.type 3 / 10, L808) stages 2 and 3: out = wy Y + wu (U + dt k(U)); stage 1 = LEAN_S1
+  RKN_ST = 9    // one stage of a user-defined Runge-Kutta-Nystrom scheme (integrator.type 20, L808-815): f = f(Psi_i), and
+                // two linear combinations of psi_n, Pi_n, f_1 .. f_4 and f (the stage's f and the next stage field, or
+                // the new psi and Pi)
 };
 
 template <int MODE> struct ModeInfo;
@@ -53,6 +56,7 @@ template <> struct ModeInfo<CLASSIC_S1> { static constexpr int NF = 1, NP = 1, N
 template <> struct ModeInfo<CLASSIC_S23> { static constexpr int NF = 1, NP = 5, NOUT = 2; };
 template <> struct ModeInfo<CLASSIC_S4> { static constexpr int NF = 1, NP = 3, NOUT = 1; };
 template <> struct ModeInfo<SSP_S23> { static constexpr int NF = 1, NP = 3, NOUT = 1; };
+template <> struct ModeInfo<RKN_ST> { static constexpr int NF = 1, NP = 6, NOUT = 1; };
 template <> struct ModeInfo<FUSED_A> { static constexpr int NF = 2, NP = 0, NOUT = 1; };
 template <> struct ModeInfo<FUSED_B> { static constexpr int NF = 3, NP = 1, NOUT = 1; };
 
@@ -80,6 +84,8 @@ struct PipeArgs {
   T adt;           // unfused: a_s * dt (S1-S3) or dt/6 (S4);  fused: dt
   T bdt;           // classic: b_s * dt for the accumulator
   T wy, wu;        // SSP_S23: weights of Y and of the forward-Euler step from U (3/4, 1/4 and 1/3, 2/3)
+  T rkn_w[2][7];   // RKN_ST: sten[0] = Psi_i; pnt[0] = psi_n, pnt[1] = Pi_n, pnt[2..5] = f_1 .. f_4 (null = absent);
+                   // out_psi[0] = sum_q rkn_w[0][q] in_q + rkn_w[0][6] f,  out_pi[0] = the same with rkn_w[1]
   T ko_c[4];       // Kreiss-Oliger (Eq.7): (-1)^(r+1) eps_c / (2^(2r) h) for psi1, psi2, Pi1, Pi2; staged sweeps with
                    // KO != 0 only, where sten[1] = Pi(U) takes the place of pnt[0]
 };
@@ -197,6 +203,26 @@ __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[Mod
                            fma(sixth, (q2 + p4b) + T(2) * (p2b + p3b), y2));
     opi[0] = mkpair(fma(sixth, fma(T(2), k3a, k1a + k4a), fma(twothirds, p3a - q1, q1)),
                           fma(sixth, fma(T(2), k3b, k1b + k4b), fma(twothirds, p3b - q2, q2)));
+  } else if (MODE == RKN_ST) {
+    // f = Lap Psi - Psi (lambda eta_s^2 (|Psi|^2 - 1) + a): no first-derivative term in a Nystrom scheme
+    const T p1 = wc[0].x, p2 = wc[0].y;
+    const T pot = pot_of(a.lam_eta2[0], a.a_mass, p1, p2);
+    const T f1 = fma(-p1, pot, lap[0][0]), f2 = fma(-p2, pot, lap[0][1]);
+    T o[2][2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      T s1 = a.rkn_w[r][6] * f1, s2 = a.rkn_w[r][6] * f2;
+#pragma unroll
+      for (int q = NPA - 1; q >= 0; --q)
+        if (a.pnt[q]) {
+          s1 = fma(a.rkn_w[r][q], pc[q].x, s1);
+          s2 = fma(a.rkn_w[r][q], pc[q].y, s2);
+        }
+      o[r][0] = s1;
+      o[r][1] = s2;
+    }
+    opsi[0] = mkpair(o[0][0], o[0][1]);
+    opi[0] = mkpair(o[1][0], o[1][1]);
   } else {
     const T psi1 = wc[0].x, psi2 = wc[0].y;
     const T pi1 = pc[0].x, pi2 = pc[0].y;
@@ -350,7 +376,8 @@ __global__ void __launch_bounds__(TX* TY) k_rk_pipe(const PipeArgs<T> a) {
     }
     if (active) {
 #pragma unroll
-      for (int q = P0; q < NP; ++q) cp_async_16(o + (NF + q - P0) * NT, a.pnt[q] + po);
+      for (int q = P0; q < NP; ++q)
+        if (MODE != RKN_ST || a.pnt[q]) cp_async_16(o + (NF + q - P0) * NT, a.pnt[q] + po);
     }
     const long long ho = tile_org + (long long)st * plane;
 #pragma unroll

@@ -19,6 +19,7 @@
 
 #include "k_avgdown.cuh"
 #include "k_ghost.cuh"
+#include "k_gw.cuh"
 #include "k_rk_pipe.cuh"
 #include "k_rk_plane.cuh"
 #include "k_rk_tma.cuh"
@@ -64,6 +65,7 @@ constexpr int K1F_TX = SLEDGE_K1F_TX;  // x vectors per fused tile (k_rk_plane)
 constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that fits K1_SMEM, at most this
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
 constexpr long long K1F_MIN_TILES = 3500;
+static_assert(GW_TY == SLEDGE_K1F_TY && GW_TX == SLEDGE_K1F_TX, "k_gw_stage runs over the fused-sweep tiles");
 constexpr long long TAG_MIN_TILES = 148 * 4 * 6;  // below this many CTAs the tag pass halves its z-chunk (down to 32 planes)  // below this many CTAs the fused sweeps halve their z-chunk
 constexpr int K1F_TY = SLEDGE_K1F_TY;            // tile rows / budget of the FUSED sweeps
 constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
@@ -139,6 +141,7 @@ struct LevelHost {
   bool periodic_box = false;  // ONE box covering the periodic domain: K1 (plane variant) and K3 wrap by themselves
   // arena offsets (bytes)
   size_t off_buf[NBUF][2];
+  size_t off_gw[NBUF][6] = {};  // gw: pair planes (u_xx,u_yy) (u_zz,u_xy) (u_xz,u_yz) (du_xx,du_yy) (du_zz,du_xy) (du_xz,du_yz)
   size_t off_boxes, off_tiles, off_ftiles, off_tag_tiles, off_owner, off_ghost_prefix, off_avg_prefix, off_ghost_list;
   // truncation-error tags written at this (fine) level's synchronisations (sledge_tee_enable)
   bool tee_on = false;
@@ -163,6 +166,10 @@ struct Plan {
   int cpa = 8;       // cells (pairs) per 128 bytes
   int ox = 8;        // x offset of the first valid cell inside a row
   size_t off_scratch = 0, scratch_bytes = 0, off_err = 0, total = 0;
+  // shadow level of level 0 (L98): a nested one-box context inside the same arena
+  size_t off_shadow = 0, shadow_bytes = 0;
+  sledge_params shadow_p;
+  sledge_box shadow_box;
 };
 
 }  // namespace
@@ -175,6 +182,7 @@ struct sledge_ctx {
   int64_t launches = 0;
   bool profiling = false;
   bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
+  sledge_ctx* shadow = nullptr;  // the shadow level's context (shadow_level = 1)
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
   size_t ev_used[4] = {0, 0, 0, 0};
 };
@@ -188,6 +196,7 @@ inline bool ko_on(const sledge_params& p) {
 // quartic coarse->fine interpolation evaluated per coarse parent through the coarse boxes' ghost cells (needs two
 // coarse ghost layers); with one ghost layer the per-cell entries of k_fill_ghosts<.., QUARTIC> are used
 inline bool quartic_by_parent(const sledge_params& p) { return p.interp == SLEDGE_INTERP_QUARTIC && p.nghost >= 2; }
+inline bool is_rkn(const sledge_params& p) { return p.integrator == 20; }
 inline int stencil_radius(const sledge_params& p) { return ko_on(p) && p.ko_order > p.lap_order ? p.ko_order : p.lap_order; }
 
 int fail(sledge_ctx* ctx, int code, const char* fmt, ...) {
@@ -225,8 +234,25 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     if (p.ko_order < 2 || p.ko_order > 3) return fail(nullptr, SLEDGE_EINVAL, "dissipation order must be 2 or 3 (L751)");
     if (p.ko_order > p.nghost) return fail(nullptr, SLEDGE_EINVAL, "dissipation order must be <= nghost (L751)");
   }
-  if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10)
-    return fail(nullptr, SLEDGE_EINVAL, "integrator must be 4 (RK4) or 3 / 10 (SSPRK3) (L808)");
+  if (p.integrator != 0 && p.integrator != 4 && p.integrator != 3 && p.integrator != 10 && p.integrator != 20)
+    return fail(nullptr, SLEDGE_EINVAL, "integrator must be 4 (RK4), 3 / 10 (SSPRK3) or 20 (user RKN tableau) (L808)");
+  if (p.integrator == 20) {  // explicit Nystrom scheme for psi'' = f(psi, eta) (L808-815)
+    if (p.rkn_stages < 1 || p.rkn_stages > SLEDGE_RKN_MAX_STAGES)
+      return fail(nullptr, SLEDGE_EINVAL, "rkn_stages must be 1..5 (L812-815)");
+    if (p.friction != 0.0 || ko_on(p))
+      return fail(nullptr, SLEDGE_EINVAL, "integrator 20 integrates psi'' = f(psi): friction and ko_strength must be 0");
+    if (p.gw) return fail(nullptr, SLEDGE_EINVAL, "integrator 20 does not evolve the gravitational-wave fields");
+    if (p.rkn_nodes[0] != 0.0) return fail(nullptr, SLEDGE_EINVAL, "rkn_nodes[0] must be 0 (the first stage is the state itself)");
+    for (int i = 0; i < p.rkn_stages; ++i)
+      if (p.rkn_tableau[i * (i + 1) / 2 + i] != 0.0)
+        return fail(nullptr, SLEDGE_EINVAL, "rkn_tableau: only explicit schemes, the diagonal must be 0 (L815)");
+  }
+  if (p.gw != 0 && p.gw != 1) return fail(nullptr, SLEDGE_EINVAL, "gw must be 0 or 1 (L404)");
+  if (p.gw && (p.integrator == 3 || p.integrator == 10))
+    return fail(nullptr, SLEDGE_EINVAL, "gw: the auxiliary fields are integrated with classic RK4 (integrator 4) only");
+  if (p.gw && p.interp != SLEDGE_INTERP_TRILINEAR)
+    return fail(nullptr, SLEDGE_EINVAL, "gw: trilinear coarse->fine interpolation only");
+  if (p.shadow_level != 0 && p.shadow_level != 1) return fail(nullptr, SLEDGE_EINVAL, "shadow_level must be 0 or 1 (L98)");
   if (p.interp != SLEDGE_INTERP_TRILINEAR && p.interp != SLEDGE_INTERP_QUARTIC)
     return fail(nullptr, SLEDGE_EINVAL, "interp must be SLEDGE_INTERP_TRILINEAR (0) or SLEDGE_INTERP_QUARTIC (4) (L780)");
   // the 5-cell window around the parent of the outermost ghost cell must stay inside the nesting gap of one
@@ -378,6 +404,9 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     const size_t plane_bytes = (size_t)L.plane_cells * 2 * P.esz;
     for (int b = 0; b < NBUF; ++b)
       for (int c = 0; c < 2; ++c) L.off_buf[b][c] = take(plane_bytes);
+    if (p.gw)
+      for (int b = 0; b < NBUF; ++b)
+        for (int c = 0; c < 6; ++c) L.off_gw[b][c] = take(plane_bytes);
     L.off_boxes = take(L.boxdev.size() * sizeof(BoxDev));
     L.off_tiles = take(L.tiles.size() * sizeof(TileDev));
     L.off_ftiles = take(L.ftiles.size() * sizeof(TileDev));
@@ -403,6 +432,32 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   P.scratch_bytes = max_box_cells * P.esz;
   P.off_scratch = take(P.scratch_bytes);
   P.off_err = take(sizeof(int));
+  if (p.shadow_level) {  // L98: level 0 coarsened by 2, ONE box over the same periodic domain
+    sledge_params sp = p;
+    sp.n_levels = 1;
+    sp.shadow_level = 0;
+    sp.h0 = 2.0 * p.h0;
+    int sbf = bf;
+    for (int d = 0; d < 3; ++d) {
+      if (p.n0[d] % 2) return fail(nullptr, SLEDGE_EINVAL, "shadow_level: n0 must be even (L98)");
+      sp.n0[d] = p.n0[d] / 2;
+      while (sbf > 1 && sp.n0[d] % sbf) sbf /= 2;
+    }
+    sp.blocking_factor = sbf;
+    sledge_box sb;
+    sb.level = 0;
+    for (int d = 0; d < 3; ++d) {
+      sb.lo[d] = 0;
+      sb.hi[d] = sp.n0[d] - 1;
+    }
+    Plan PS;
+    const int rc = make_plan(PS, &sp, &sb, 1);
+    if (rc) return fail(nullptr, rc, "shadow_level: the coarsened level 0 is not a valid grid (%s)", g_err.c_str());
+    P.shadow_p = sp;
+    P.shadow_box = sb;
+    P.shadow_bytes = PS.total;
+    P.off_shadow = take(PS.total);
+  }
   P.total = off;
   return SLEDGE_OK;
 }
@@ -442,8 +497,11 @@ int check_launch(sledge_ctx* c, const char* what) {
   return SLEDGE_OK;
 }
 
+// which: 0 = (psi1,psi2), 1 = (Pi1,Pi2); with gw 2..4 = the u pair planes, 5..7 = the du pair planes (component c of
+// the state lives in plane c / 2, lane c % 2)
 template <typename T> typename PairOf<T>::type* plane_ptr(sledge_ctx* c, int l, int buf, int which) {
-  return reinterpret_cast<typename PairOf<T>::type*>(c->arena + c->plan.lev[l].off_buf[buf & 3][which]);
+  const LevelHost& L = c->plan.lev[l];
+  return reinterpret_cast<typename PairOf<T>::type*>(c->arena + (which < 2 ? L.off_buf[buf & 3][which] : L.off_gw[buf & 3][which - 2]));
 }
 template <typename U> U* tab(sledge_ctx* c, size_t off) { return reinterpret_cast<U*>(c->arena + off); }
 
@@ -462,7 +520,7 @@ LevelGeom geom_of(const Plan& P, int l) {
 
 // K2 arguments for buffer `buf` of level l, whose data is at time `time`
 template <typename T>
-GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
+GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, int wb = 1) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
   GhostArgs<T> a;
@@ -470,8 +528,8 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
   a.boxes = tab<BoxDev>(c, L.off_boxes);
   a.blk_prefix = tab<int>(c, L.off_ghost_prefix);
   a.nbox = (int)L.boxdev.size();
-  a.psi = plane_ptr<T>(c, l, buf, 0);
-  a.pi = plane_ptr<T>(c, l, buf, 1);
+  a.psi = plane_ptr<T>(c, l, buf, wa);  // the kernels call their two planes psi and pi; any pair of planes will do
+  a.pi = plane_ptr<T>(c, l, buf, wb);
   a.owner = tab<int>(c, L.off_owner);
   a.geom = geom_of(P, l);
   a.err_flag = tab<int>(c, P.off_err);
@@ -506,10 +564,10 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time) {
     // with one state only: the blend returns one of the two buffers unchanged, so only that one is read
     if (bo == bn || alpha == 0.0) { bn = bo; a.single = 1; }
     else if (alpha == 1.0) { bo = bn; a.single = 1; }
-    a.c_old_psi = plane_ptr<T>(c, l - 1, bo, 0);
-    a.c_new_psi = plane_ptr<T>(c, l - 1, bn, 0);
-    a.c_old_pi = plane_ptr<T>(c, l - 1, bo, 1);
-    a.c_new_pi = plane_ptr<T>(c, l - 1, bn, 1);
+    a.c_old_psi = plane_ptr<T>(c, l - 1, bo, wa);
+    a.c_new_psi = plane_ptr<T>(c, l - 1, bn, wa);
+    a.c_old_pi = plane_ptr<T>(c, l - 1, bo, wb);
+    a.c_new_pi = plane_ptr<T>(c, l - 1, bn, wb);
   }
   return a;
 }
@@ -534,8 +592,8 @@ int fill_shell_copies(sledge_ctx* c, int l, int buf, bool with_pi) {
 }
 
 template <typename T>
-int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false) {
-  GhostArgs<T> a = ghost_args<T>(c, l, buf, time);
+int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false, int wa = 0, int wb = 1) {
+  GhostArgs<T> a = ghost_args<T>(c, l, buf, time, wa, wb);
   if (a.quartic == 2 && l > 0) {  // the coarse windows are read through the coarse boxes' ghost cells
     LevelHost& C = c->plan.lev[l - 1];
     const bool pair = C.have_pair && C.t_new != C.t_old;
@@ -717,6 +775,7 @@ cudaError_t launch_pipe_mode(sledge_ctx* c, const PipeArgs<T>& a, int grid, int 
     case CLASSIC_S23: return launch_pipe_kernel<T, ORDER, CLASSIC_S23>(c, a, grid);
     case CLASSIC_S4: return launch_pipe_kernel<T, ORDER, CLASSIC_S4>(c, a, grid);
     case SSP_S23: return launch_pipe_kernel<T, ORDER, SSP_S23>(c, a, grid);
+    case RKN_ST: return launch_pipe_kernel<T, ORDER, RKN_ST>(c, a, grid);
     case FUSED_A: return launch_pipe_kernel<T, ORDER, FUSED_A>(c, a, grid);
     default: return launch_pipe_kernel<T, ORDER, FUSED_B>(c, a, grid);
   }
@@ -837,7 +896,7 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
 // With Kreiss-Oliger dissipation k_psi = Pi + Q psi is no longer pointwise: every level runs the staged sweeps.
 inline bool is_ssprk3(const sledge_params& p) { return p.integrator == 3 || p.integrator == 10; }
 inline bool level_is_fused(const Plan& P, int l) {
-  return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0 && !ko_on(P.p) && !is_ssprk3(P.p);
+  return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0 && !ko_on(P.p) && !is_ssprk3(P.p) && !is_rkn(P.p) && !P.p.gw;
 }
 
 // One SSPRK3 stage (integrator.type 3 / 10, L808; Shu-Osher form) of level l, s = 0, 1, 2:
@@ -876,6 +935,114 @@ int do_stage_ssp(sledge_ctx* c, int l, int s, double t, double dt, double eta_co
   return SLEDGE_OK;
 }
 
+// Stage s of the gravitational-wave auxiliary fields (Eq.16; R25) in the LEAN data-flow of the
+// scalar sector: U = stage input (buffer ubuf, whose psi ghosts the scalar stage has just filled), Y = cur,
+// U2 = cur+1 (then the new state), U3 = cur+2, U4 = cur+3.
+template <typename T>
+int do_stage_gw(sledge_ctx* c, int l, int s, int ubuf, int cur, double ts, double dt, double eta_s) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  // ghosts of the three u pair planes of the stage input, at the stage time (L72)
+  int rc = launch_ghosts<T>(c, l, ubuf, ts, true, true, 2, 3);
+  if (rc == SLEDGE_OK) rc = launch_ghosts<T>(c, l, ubuf, ts, false, true, 4, 4);
+  if (rc) return rc;
+  GwArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.boxes = tab<BoxDev>(c, L.off_boxes);
+  a.tiles = tab<TileDev>(c, L.off_ftiles);
+  a.g = P.p.nghost;
+  a.ox = P.ox;
+  a.psi = plane_ptr<T>(c, l, ubuf, 0);
+  for (int q = 0; q < 3; ++q) {
+    a.u[q] = plane_ptr<T>(c, l, ubuf, 2 + q);
+    a.du[q] = plane_ptr<T>(c, l, ubuf, 5 + q);
+  }
+  const int in[3] = {cur, cur + 1, cur + 2};
+  const int nin = s == 0 ? 0 : (s == 3 ? 3 : 1);
+  for (int m = 0; m < nin; ++m)
+    for (int q = 0; q < 6; ++q) a.in[m][q] = plane_ptr<T>(c, l, in[m], 2 + q);
+  const int obuf = s == 3 ? cur + 1 : cur + 1 + s;
+  for (int q = 0; q < 6; ++q) a.out[q] = plane_ptr<T>(c, l, obuf, 2 + q);
+  const double h = L.h, h2 = h * h;
+  a.inv_h2 = (T)(P.p.lap_order == 1 ? 1.0 / h2 : (P.p.lap_order == 2 ? 1.0 / (12.0 * h2) : 1.0 / (180.0 * h2)));
+  a.inv_h = (T)(P.p.lap_order == 1 ? 1.0 / (2.0 * h) : (P.p.lap_order == 2 ? 1.0 / (12.0 * h) : 1.0 / (60.0 * h)));
+  a.coupling = (T)P.p.gw_coupling;
+  a.fric = (T)(P.p.gw_friction != 0.0 ? P.p.gw_friction / eta_s : 0.0);
+  static const double as[4] = {0.5, 0.5, 1.0, 1.0 / 6.0};
+  a.adt = (T)(as[s] * dt);
+  const int grid = (int)L.ftiles.size();
+  {
+    Timed tm(c, KIND_STAGE);
+    const int mode = s == 0 ? LEAN_S1 : (s == 3 ? LEAN_S4 : LEAN_S23);
+    rc = P.p.lap_order == 1 ? launch_gw<T, 1>(c->stream, a, grid, mode)
+         : (P.p.lap_order == 2 ? launch_gw<T, 2>(c->stream, a, grid, mode) : launch_gw<T, 3>(c->stream, a, grid, mode));
+  }
+  if (rc) return fail(c, SLEDGE_ECUDA, "k_gw_stage: bad mode");
+  return check_launch(c, "k_gw_stage");
+}
+
+// Stage i of the user-defined Runge-Kutta-Nystrom scheme (integrator.type 20, L808-815; R26).
+// Planes: cur = (psi_n, Pi_n); the stage fields Psi_1, Psi_2, ... alternate between (cur+1).psi and (cur+2).psi;
+// f_0 .. f_3 are kept in (cur+1).Pi, (cur+2).Pi, (cur+3).psi, (cur+3).Pi, ordered so that the plane the new Pi
+// overwrites in place (pointwise) is paired with the plane the new psi goes to: the new state is buffer
+// X = cur+1 if the number of stages is odd, else cur+2.
+template <typename T>
+int do_stage_rkn(sledge_ctx* c, int l, int i, double t, double dt, double eta_const) {
+  Plan& P = c->plan;
+  LevelHost& L = P.lev[l];
+  const sledge_params& p = P.p;
+  const int s = p.rkn_stages, cur = L.cur;
+  const bool last = i == s - 1;
+  using PP = typename PairOf<T>::type;
+  auto ping = [&](int k) -> int { return cur + 1 + (k & 1); };  // buffer whose psi plane holds Psi_{k+1}
+  PP* const fpl[4] = {plane_ptr<T>(c, l, cur + 1, 1), plane_ptr<T>(c, l, cur + 2, 1), plane_ptr<T>(c, l, cur + 3, 0),
+                      plane_ptr<T>(c, l, cur + 3, 1)};
+  // f_j lives in fpl[slot(j)]: the in-place target X.Pi must hold a stored f only if one is stored there
+  const int X = ping(s - 1);  // buffer of the new state
+  auto slot = [&](int j) -> int {  // keep X.Pi for the LAST stored f so that every earlier one is read before the overwrite
+    const int xs = (X == cur + 1) ? 0 : 1, other = 1 - xs;
+    const int order[4] = {other, 2, 3, xs};
+    return order[j];
+  };
+  const double ts = t + p.rkn_nodes[i] * dt;
+  const int ubuf = i == 0 ? cur : ping(i - 1);
+  int rc = launch_ghosts<T>(c, l, ubuf, ts, false, true);
+  if (rc) return rc;
+  PipeArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.sten[0] = plane_ptr<T>(c, l, ubuf, 0);
+  a.pnt[0] = plane_ptr<T>(c, l, cur, 0);
+  a.pnt[1] = plane_ptr<T>(c, l, cur, 1);
+  for (int j = 0; j < i; ++j) a.pnt[2 + j] = fpl[slot(j)];
+  set_eta(P, a, 0, p.eta_fixed ? eta_const : ts);
+  const double* arow = p.rkn_tableau + (i + 1) * (i + 2) / 2;  // row of the NEXT stage
+  if (!last) {  // out 0 = f_i, out 1 = Psi_{i+1} = psi_n + c_{i+1} dt Pi_n + dt^2 sum_{j<=i} a_{i+1,j} f_j
+    a.rkn_w[0][6] = (T)1;
+    a.rkn_w[1][0] = (T)1;
+    a.rkn_w[1][1] = (T)(p.rkn_nodes[i + 1] * dt);
+    for (int j = 0; j < i; ++j) a.rkn_w[1][2 + j] = (T)(dt * dt * arow[j]);
+    a.rkn_w[1][6] = (T)(dt * dt * arow[i]);
+    a.out_psi[0] = fpl[slot(i)];
+    a.out_pi[0] = plane_ptr<T>(c, l, ping(i), 0);
+  } else {  // out 0 = psi_new, out 1 = Pi_new
+    a.rkn_w[0][0] = (T)1;
+    a.rkn_w[0][1] = (T)dt;
+    a.rkn_w[1][1] = (T)1;
+    for (int j = 0; j < i; ++j) {
+      a.rkn_w[0][2 + j] = (T)(dt * dt * p.rkn_weights_bar_b[j]);
+      a.rkn_w[1][2 + j] = (T)(dt * p.rkn_weights_b[j]);
+    }
+    a.rkn_w[0][6] = (T)(dt * dt * p.rkn_weights_bar_b[i]);
+    a.rkn_w[1][6] = (T)(dt * p.rkn_weights_b[i]);
+    a.out_psi[0] = plane_ptr<T>(c, l, X, 0);
+    a.out_pi[0] = plane_ptr<T>(c, l, X, 1);
+  }
+  rc = launch_k1<T>(c, l, RKN_ST, a);
+  if (rc) return rc;
+  if (last) finish_step(L, X, t, dt);
+  return SLEDGE_OK;
+}
+
 // One RK4 stage of level l: ghost fill of the stage input at its time, then K1.
 // t = time at the start of the level's step, eta_const = eta used when eta_fixed.
 template <typename T>
@@ -883,6 +1050,8 @@ int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const)
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
   if (is_ssprk3(P.p)) return s < 3 ? do_stage_ssp<T>(c, l, s, t, dt, eta_const) : SLEDGE_OK;
+  if (is_rkn(P.p)) return s < P.p.rkn_stages ? do_stage_rkn<T>(c, l, s, t, dt, eta_const) : SLEDGE_OK;
+  if (s > 3) return SLEDGE_OK;
   if (level_is_fused(P, l)) {  // stage calls 1 and 3 run the two sweeps, 0 and 2 are no-ops
     if (s == 1) return do_fused_pass<T>(c, l, 0, t, dt, eta_const);
     if (s == 3) return do_fused_pass<T>(c, l, 1, t, dt, eta_const);
@@ -893,7 +1062,7 @@ int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const)
   const double ts = t + cs[s] * dt;
   const double eta_s = P.p.eta_fixed ? eta_const : ts;
   const int cur = L.cur;
-  const bool lean = P.p.rk_dataflow != SLEDGE_RK_CLASSIC;
+  const bool lean = P.p.rk_dataflow != SLEDGE_RK_CLASSIC || P.p.gw;  // with gw both sectors share the LEAN buffer roles
   int ubuf, mode, in[3] = {-1, -1, -1}, out[2] = {-1, -1};
   double adt = (s < 3) ? as[s] * dt : dt / 6.0, bdt = 0.0;
   if (lean) {  // buffers: cur = Y, cur+1 = U2 (then Ynew), cur+2 = U3, cur+3 = U4
@@ -928,52 +1097,69 @@ int do_stage(sledge_ctx* c, int l, int s, double t, double dt, double eta_const)
   a.bdt = (T)bdt;
   rc = launch_k1<T>(c, l, mode, a);
   if (rc) return rc;
+  if (P.p.gw) {  // the auxiliary fields of Eq.16 take the same stage (LEAN data-flow, same buffers)
+    rc = do_stage_gw<T>(c, l, s, ubuf, cur, ts, dt, eta_s);
+    if (rc) return rc;
+  }
   if (s == 3) finish_step(L, cur + 1, t, dt);
   return SLEDGE_OK;
 }
 
+// K4 between level lf of context fc (fine) and level lc of context cc (coarse; the same context for an ordinary
+// synchronisation, the shadow context for L98), on the plane pair (wa, wb) of the current states.  With tee the
+// truncation-error comparison rides on it (scalar planes only).
 template <typename T>
-int do_average_down(sledge_ctx* c, int lf) {
-  Plan& P = c->plan;
-  LevelHost& F = P.lev[lf];
-  LevelHost& C = P.lev[lf - 1];
+int avg_between(sledge_ctx* fc, int lf, sledge_ctx* cc, int lc, int wa, int wb, bool tee, const double* eps,
+                uint8_t* tags, uint32_t* counts) {
+  LevelHost& F = fc->plan.lev[lf];
+  LevelHost& C = cc->plan.lev[lc];
   AvgArgs<T> a;
   memset(&a, 0, sizeof a);
-  a.fboxes = tab<BoxDev>(c, F.off_boxes);
-  a.blk_prefix = tab<int>(c, F.off_avg_prefix);
+  a.fboxes = tab<BoxDev>(fc, F.off_boxes);
+  a.blk_prefix = tab<int>(fc, F.off_avg_prefix);
   a.nfbox = (int)F.boxdev.size();
-  a.f_psi = plane_ptr<T>(c, lf, F.cur, 0);
-  a.f_pi = plane_ptr<T>(c, lf, F.cur, 1);
-  a.fgeom = geom_of(P, lf);
-  a.cboxes = tab<BoxDev>(c, C.off_boxes);
-  a.cowner = tab<int>(c, C.off_owner);
-  a.cgeom = geom_of(P, lf - 1);
-  a.c_psi = plane_ptr<T>(c, lf - 1, C.cur, 0);
-  a.c_pi = plane_ptr<T>(c, lf - 1, C.cur, 1);
-  a.err_flag = tab<int>(c, P.off_err);
+  a.f_psi = plane_ptr<T>(fc, lf, F.cur, wa);
+  a.f_pi = plane_ptr<T>(fc, lf, F.cur, wb);
+  a.fgeom = geom_of(fc->plan, lf);
+  a.cboxes = tab<BoxDev>(cc, C.off_boxes);
+  a.cowner = tab<int>(cc, C.off_owner);
+  a.cgeom = geom_of(cc->plan, lc);
+  a.c_psi = plane_ptr<T>(cc, lc, C.cur, wa);
+  a.c_pi = plane_ptr<T>(cc, lc, C.cur, wb);
+  a.err_flag = tab<int>(fc, fc->plan.off_err);
   const int grid = F.avg_prefix.back();
   C.shell_ok[C.cur & 3] = 0;  // covered coarse cells change: ghost copies of them are stale
   C.star_ok[C.cur & 3] = false;
-  if (F.tee_on) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
-    for (int q = 0; q < 4; ++q) a.tee_eps[q] = (T)F.tee_eps[q];
-    a.tee_tags = F.tee_tags;
-    a.tee_counts = F.tee_counts;
+  if (tee) {  // truncation-error tags ride on the synchronisation (L98: "just before synchronization")
+    for (int q = 0; q < 4; ++q) a.tee_eps[q] = (T)eps[q];
+    a.tee_tags = tags;
+    a.tee_counts = counts;
     a.nb0 = F.nb[0];
     a.nb1 = F.nb[1];
-    if (F.tee_counts) cudaMemsetAsync(F.tee_counts, 0, sizeof(uint32_t) * (size_t)F.count_blocks, c->stream);
+    if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)F.count_blocks, fc->stream);
   }
   {
-    Timed t(c, KIND_AVG);
-    if (F.tee_on) k_average_down<T, true><<<grid, AVG_THREADS, 0, c->stream>>>(a);
-    else k_average_down<T, false><<<grid, AVG_THREADS, 0, c->stream>>>(a);
+    Timed t(fc, KIND_AVG);
+    if (tee) k_average_down<T, true><<<grid, AVG_THREADS, 0, fc->stream>>>(a);
+    else k_average_down<T, false><<<grid, AVG_THREADS, 0, fc->stream>>>(a);
   }
-  return check_launch(c, "k_average_down");
+  return check_launch(fc, "k_average_down");
+}
+
+template <typename T>
+int do_average_down(sledge_ctx* c, int lf) {
+  LevelHost& F = c->plan.lev[lf];
+  int rc = avg_between<T>(c, lf, c, lf - 1, 0, 1, F.tee_on, F.tee_eps, F.tee_tags, F.tee_counts);
+  if (c->plan.p.gw)  // the auxiliary fields synchronise like every other component (L74)
+    for (int w = 2; w < 8 && rc == SLEDGE_OK; w += 2) rc = avg_between<T>(c, lf, c, lf - 1, w, w + 1, false, nullptr, nullptr, nullptr);
+  return rc;
 }
 
 // O6 / L66-76, Fig.2: level l one step, then level l+1 two half steps, then synchronise.
 template <typename T>
 int advance(sledge_ctx* c, int l, double t, double dt, double eta_const) {
-  for (int s = 0; s < 4; ++s) {
+  const int nst = is_rkn(c->plan.p) ? c->plan.p.rkn_stages : 4;
+  for (int s = 0; s < nst; ++s) {
     const int rc = do_stage<T>(c, l, s, t, dt, eta_const);
     if (rc) return rc;
   }
@@ -1130,12 +1316,20 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     delete c;
     return rc;
   }
+  if (P.p.shadow_level) {  // the shadow level of level 0 (L98) is a one-box context of its own inside the arena
+    rc = sledge_create(&c->shadow, &P.shadow_p, &P.shadow_box, 1, c->arena + P.off_shadow, P.shadow_bytes, cuda_stream);
+    if (rc != SLEDGE_OK) {
+      sledge_destroy(c);
+      return rc;
+    }
+  }
   *out = c;
   return SLEDGE_OK;
 }
 
 int sledge_destroy(sledge_ctx* c) {
   if (!c) return SLEDGE_OK;
+  if (c->shadow) sledge_destroy(c->shadow);
   cudaStreamSynchronize(c->stream);
   for (auto& v : c->ev)
     for (auto& pr : v) {
@@ -1149,7 +1343,8 @@ int sledge_destroy(sledge_ctx* c) {
 static int check_box_comp(sledge_ctx* c, int box, int comp, const void* ptr) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
   if (box < 0 || box >= (int)c->plan.box.size()) return fail(c, SLEDGE_EINVAL, "box index %d out of range", box);
-  if (comp < 0 || comp > 3) return fail(c, SLEDGE_EINVAL, "component %d out of range (0..3)", comp);
+  const int ncomp = c->plan.p.gw ? SLEDGE_NCOMP_GW : SLEDGE_NCOMP;
+  if (comp < 0 || comp >= ncomp) return fail(c, SLEDGE_EINVAL, "component %d out of range (0..%d)", comp, ncomp - 1);
   if (!ptr) return fail(c, SLEDGE_EINVAL, "null data pointer");
   return SLEDGE_OK;
 }
@@ -1211,13 +1406,18 @@ int sledge_fill_ghosts(sledge_ctx* c, int level, double time) {
   int rc = check_level(c, level);
   if (rc) return rc;
   const int cur = c->plan.lev[level].cur;
-  return DISPATCH(c, launch_ghosts<float>(c, level, cur, time, true), launch_ghosts<double>(c, level, cur, time, true));
+  rc = DISPATCH(c, launch_ghosts<float>(c, level, cur, time, true), launch_ghosts<double>(c, level, cur, time, true));
+  if (c->plan.p.gw)
+    for (int w = 2; w < 8 && rc == SLEDGE_OK; w += 2)
+      rc = DISPATCH(c, launch_ghosts<float>(c, level, cur, time, true, false, w, w + 1),
+                    launch_ghosts<double>(c, level, cur, time, true, false, w, w + 1));
+  return rc;
 }
 
 int sledge_rk_stage(sledge_ctx* c, int level, int stage, double dt, double eta) {
   int rc = check_level(c, level);
   if (rc) return rc;
-  if (stage < 0 || stage > 3) return fail(c, SLEDGE_EINVAL, "stage must be 0..3");
+  if (stage < 0 || stage > 4) return fail(c, SLEDGE_EINVAL, "stage must be 0..3 (0..4 for a five-stage RKN tableau)");
   return DISPATCH(c, do_stage<float>(c, level, stage, eta, dt, eta), do_stage<double>(c, level, stage, eta, dt, eta));
 }
 
@@ -1261,6 +1461,36 @@ int sledge_tee_enable(sledge_ctx* c, int fine_level, const double* eps4, uint8_t
   L.tee_tags = dev_tags;
   L.tee_counts = dev_counts;
   return SLEDGE_OK;
+}
+
+int sledge_shadow_tee(sledge_ctx* c, double dt, double eta, const double* eps4, uint8_t* dev_tags, uint32_t* dev_counts) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  if (!c->shadow) return fail(c, SLEDGE_ESTATE, "shadow_tee: the context was created without shadow_level = 1 (L98)");
+  if (!(dt > 0)) return fail(c, SLEDGE_EINVAL, "dt must be positive");
+  if (!eps4) return fail(c, SLEDGE_EINVAL, "shadow_tee: null thresholds");
+  for (int q = 0; q < 4; ++q)
+    if (!(eps4[q] >= 0)) return fail(c, SLEDGE_EINVAL, "shadow_tee: thresholds must be >= 0");
+  if (dev_tags && ((uintptr_t)dev_tags & 1)) return fail(c, SLEDGE_EINVAL, "shadow_tee: tags must be 2-byte aligned");
+  sledge_ctx* sh = c->shadow;
+  const bool gw = c->plan.p.gw != 0;
+  // (1) shadow <- mean of the 8 level-0 children (every component)
+  sh->plan.lev[0].have_pair = false;
+  int rc = SLEDGE_OK;
+  for (int w = 0; w < (gw ? 8 : 2) && rc == SLEDGE_OK; w += 2)
+    rc = DISPATCH(c, avg_between<float>(c, 0, sh, 0, w, w + 1, false, nullptr, nullptr, nullptr),
+                  avg_between<double>(c, 0, sh, 0, w, w + 1, false, nullptr, nullptr, nullptr));
+  // (2) one step of 2 dt on the shadow level, two coarse steps of dt on the hierarchy
+  if (rc == SLEDGE_OK) rc = sledge_rk_step(sh, 2.0 * dt, eta);
+  if (rc != SLEDGE_OK && sh->err.size()) c->err = "shadow level: " + sh->err;
+  if (rc == SLEDGE_OK) rc = sledge_rk_step(c, dt, eta);
+  if (rc == SLEDGE_OK) rc = sledge_rk_step(c, dt, eta + dt);
+  // (3) compare and tag (the K4 TEE kernel with the shadow box on the coarse side)
+  if (rc == SLEDGE_OK)
+    rc = DISPATCH(c, avg_between<float>(c, 0, sh, 0, 0, 1, true, eps4, dev_tags, dev_counts),
+                  avg_between<double>(c, 0, sh, 0, 0, 1, true, eps4, dev_tags, dev_counts));
+  c->launches += sh->launches;
+  sh->launches = 0;
+  return rc;
 }
 
 int64_t sledge_launch_count(const sledge_ctx* c) { return c ? c->launches : 0; }

@@ -23,7 +23,8 @@ COUNT_BLOCK = 32
 SYMBOLS = [
     "sledge_arena_bytes", "sledge_create", "sledge_destroy", "sledge_set_state", "sledge_get_state",
     "sledge_set_state_host", "sledge_get_state_host", "sledge_get_ghosted", "sledge_fill_ghosts",
-    "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable", "sledge_level_cells",
+    "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable",
+    "sledge_shadow_tee", "sledge_level_cells",
     "sledge_launch_count", "sledge_synchronize", "sledge_profile_enable", "sledge_profile_read",
     "sledge_last_error",
 ]
@@ -43,7 +44,10 @@ class sledge_params(C.Structure):
         ("dtype", C.c_int32), ("lap_order", C.c_int32), ("eta_fixed", C.c_int32), ("rk_dataflow", C.c_int32),
         ("h0", C.c_double), ("lam", C.c_double), ("a_mass", C.c_double), ("friction", C.c_double),
         ("ko_strength", C.c_double * 4), ("ko_order", C.c_int32), ("integrator", C.c_int32),
-        ("interp", C.c_int32), ("reserved_", C.c_int32),
+        ("interp", C.c_int32), ("shadow_level", C.c_int32), ("gw", C.c_int32), ("rkn_stages", C.c_int32),
+        ("gw_coupling", C.c_double), ("gw_friction", C.c_double),
+        ("rkn_nodes", C.c_double * 6), ("rkn_weights_b", C.c_double * 6), ("rkn_weights_bar_b", C.c_double * 6),
+        ("rkn_tableau", C.c_double * 21),
     ]
 
 
@@ -71,6 +75,7 @@ def lib():
         L.sledge_tag_strings.argtypes = [vp, i, vp, vp]
         L.sledge_average_down.argtypes = [vp, i]
         L.sledge_tee_enable.argtypes = [vp, i, C.POINTER(C.c_double), vp, vp]
+        L.sledge_shadow_tee.argtypes = [vp, d, d, C.POINTER(C.c_double), vp, vp]
         L.sledge_level_cells.argtypes = [vp, i, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.sledge_launch_count.argtypes = [vp]
         L.sledge_launch_count.restype = C.c_int64
@@ -84,7 +89,8 @@ def lib():
 
 
 def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0, lam, a_mass, friction, eta_fixed,
-             rk_dataflow, ko_order=0, ko_strength=0.0, integrator=4, interp=0):
+             rk_dataflow, ko_order=0, ko_strength=0.0, integrator=4, interp=0, shadow_level=False, gw=False,
+             gw_coupling=0.0, gw_friction=0.0, rkn=None):
     if isinstance(n0, int):
         n0 = (n0,) * 3
     if boxes is None:
@@ -104,6 +110,16 @@ def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0,
     p.ko_order = ko_order
     p.integrator = integrator
     p.interp = interp
+    p.shadow_level = 1 if shadow_level else 0
+    p.gw = 1 if gw else 0
+    p.gw_coupling, p.gw_friction = float(gw_coupling), float(gw_friction)
+    if rkn is not None:  # the four arrays of Table V (L812-815), passed through unchanged
+        st = len(rkn["nodes"])
+        p.rkn_stages = st
+        p.rkn_nodes[:st] = [float(v) for v in rkn["nodes"]]
+        p.rkn_weights_b[:st] = [float(v) for v in rkn["weights_b"]]
+        p.rkn_weights_bar_b[:st] = [float(v) for v in rkn["weights_bar_b"]]
+        p.rkn_tableau[:len(rkn["tableau"])] = [float(v) for v in rkn["tableau"]]
     arr = (sledge_box * len(boxes))()
     for q, (l, lo, hi) in enumerate(boxes):
         arr[q].level = int(l)
@@ -114,10 +130,12 @@ def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0,
 
 def sledge_arena_bytes(n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, dtype="f64", lap_order=1, h0=1.0,
                        lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, rk_dataflow="lean", ko_order=0,
-                       ko_strength=0.0, integrator=4, interp=0) -> int:
+                       ko_strength=0.0, integrator=4, interp=0, shadow_level=False, gw=False, gw_coupling=0.0,
+                       gw_friction=0.0, rkn=None) -> int:
     """Host-only: validates the parameters and the box list and returns the arena size (needs no GPU)."""
     p, arr, boxes, _ = _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0, lam, a_mass,
-                                friction, eta_fixed, rk_dataflow, ko_order, ko_strength, integrator, interp)
+                                friction, eta_fixed, rk_dataflow, ko_order, ko_strength, integrator, interp,
+                                shadow_level, gw, gw_coupling, gw_friction, rkn)
     out = C.c_size_t(0)
     rc = lib().sledge_arena_bytes(C.byref(p), arr, len(boxes), C.byref(out))
     if rc != 0:
@@ -134,15 +152,17 @@ class Sledge:
 
     def __init__(self, n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, dtype="f64", lap_order=1, h0=1.0,
                  lam=1.0, a_mass=0.0, friction=0.0, eta_fixed=False, rk_dataflow="lean", ko_order=0, ko_strength=0.0,
-                 integrator=4, interp=0, device="cuda:0"):
+                 integrator=4, interp=0, shadow_level=False, gw=False, gw_coupling=0.0, gw_friction=0.0, rkn=None,
+                 device="cuda:0"):
         self._h = None
         L = lib()
         if not torch.cuda.is_available():
             raise SledgeError("no CUDA device: the sledge path has no CPU fallback")
         p, arr, self.boxes, self.n0 = _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0, lam,
                                                a_mass, friction, eta_fixed, rk_dataflow, ko_order, ko_strength,
-                                               integrator, interp)
+                                               integrator, interp, shadow_level, gw, gw_coupling, gw_friction, rkn)
         self.n_levels, self.nghost, self.dtype = n_levels, nghost, dtype
+        self.ncomp = 16 if gw else 4
         self.tdtype = torch.float64 if dtype == "f64" else torch.float32
         self.device = torch.device(device)
         nbytes = C.c_size_t(0)
@@ -269,6 +289,20 @@ class Sledge:
         if not hasattr(self, "_tee"):
             self._tee = {}
         self._tee[fine_level] = (tags, counts)
+        return tags, counts
+
+    def shadow_tee(self, dt, eta, eps_psi1, eps_psi2, eps_pi1=float("inf"), eps_pi2=float("inf"),
+                   tags: torch.Tensor | None = None, counts: torch.Tensor | None = None):
+        """sledge_shadow_tee: level-0 truncation-error tags through the shadow level (L98); advances the hierarchy by
+        two coarse steps of dt.  Returns (tags uint8 [valid level-0 cells], counts int32 [bz, by, bx])."""
+        ncell, _ = self.level_cells(0)
+        if tags is None:
+            tags = torch.zeros(ncell, dtype=torch.uint8, device=self.device)
+        if counts is None:
+            counts = torch.zeros(self.count_shape(0), dtype=torch.int32, device=self.device)
+        eps = (C.c_double * 4)(float(eps_psi1), float(eps_psi2), float(eps_pi1), float(eps_pi2))
+        self._chk(lib().sledge_shadow_tee(self._h, float(dt), float(eta), eps, tags.data_ptr(), counts.data_ptr()),
+                  "sledge_shadow_tee")
         return tags, counts
 
     def synchronize(self):

@@ -10,14 +10,16 @@ from paper_2404_02950_b200.sledge import Sledge
 
 def make_pair(n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, lap_order=1, h0=1.0, lam=1.0, a_mass=0.0,
               friction=0.0, eta_fixed=False, dtype="f64", rk_dataflow="lean", ko_order=0, ko_strength=0.0,
-              integrator=4, interp=0):
+              integrator=4, interp=0, gw=False, gw_coupling=0.0, gw_friction=0.0, rkn=None, shadow_level=False):
     o = Oracle(n0, boxes=boxes, n_levels=n_levels, nghost=nghost, blocking_factor=blocking_factor,
                lap_order=lap_order, h0=h0, lam=lam, a_mass=a_mass, friction=friction, eta_fixed=eta_fixed,
-               ko_order=ko_order, ko_strength=ko_strength, integrator=integrator, interp=interp)
+               ko_order=ko_order, ko_strength=ko_strength, integrator=integrator, interp=interp, gw=gw,
+               gw_coupling=gw_coupling, gw_friction=gw_friction, rkn=rkn)
     s = Sledge(n0, boxes=boxes, n_levels=n_levels, nghost=nghost, blocking_factor=blocking_factor, dtype=dtype,
                lap_order=lap_order, h0=h0, lam=lam, a_mass=a_mass, friction=friction, eta_fixed=eta_fixed,
                rk_dataflow=rk_dataflow, ko_order=ko_order, ko_strength=ko_strength, integrator=integrator,
-               interp=interp)
+               interp=interp, gw=gw, gw_coupling=gw_coupling, gw_friction=gw_friction, rkn=rkn,
+               shadow_level=shadow_level)
     return o, s
 
 

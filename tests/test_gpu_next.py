@@ -1,0 +1,208 @@
+"""GPU parity of the rows added in round 2: gravitational-wave auxiliary fields (NEXT-4), the
+user-defined Runge-Kutta-Nystrom integrator (NEXT-2) and the level-0 shadow level (NEXT-1), each against the CPU oracle
+on the same seeded inputs.  Bars as everywhere: fp64 <= 1e-11 absolute, fp32 <= 2e-5 relative, tags bit-exact where
+the decision is not within rounding of the threshold."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2404_02950_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+F64_TOL = 1e-11
+F32_TOL = 2e-5
+
+RKN4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_b=[1 / 6, 1 / 3, 0.0],
+            tableau=[0.0, 1 / 8, 0.0, 0.0, 0.5, 0.0])
+RK4_AS_RKN = dict(nodes=[0.0, 0.5, 0.5, 1.0], weights_b=[1 / 6, 1 / 3, 1 / 3, 1 / 6], weights_bar_b=[1 / 6, 1 / 6, 1 / 6, 0.0],
+                  tableau=[0.0, 0.0, 0.0, 0.25, 0.0, 0.0, 0.0, 0.5, 0.0, 0.0])
+# a five-stage tableau with every entry non-zero (consistency is irrelevant here: both sides must compute the same thing)
+RKN5_DENSE = dict(nodes=[0.0, 0.2, 0.5, 0.7, 1.0], weights_b=[0.1, 0.3, 0.2, 0.3, 0.1], weights_bar_b=[0.1, 0.15, 0.1, 0.1, 0.05],
+                  tableau=[0.0, 0.02, 0.0, 0.05, 0.075, 0.0, 0.06, 0.085, 0.1, 0.0, 0.1, 0.12, 0.14, 0.14, 0.0])
+
+
+def _pair():
+    import _pair as P
+    return P
+
+
+def _ring_hierarchy(n0=32, box=16, n_levels=3):
+    """the three-level hierarchy of test_gpu_parity.py: boxes of 16^3 around two seeded vortex rings"""
+    rings = inputs.make_rings(n0, 2, 5.0, 9.0, 1.5, seed=77)
+    boxes, _ = inputs.amr_boxes_for_rings(rings, n_levels=n_levels, box=box, r1=3.0, r2=1.0, blocking_factor=8)
+    return boxes
+
+
+def _ragged_boxes():
+    """40 x 24 x 72 periodic level 0 in boxes of different shapes: partial K1 tiles in x and y, several boxes in z."""
+    return [(0, (0, 0, 0), (23, 23, 39)), (0, (24, 0, 0), (39, 23, 39)), (0, (0, 0, 40), (39, 7, 71)),
+            (0, (0, 8, 40), (39, 23, 71))]
+
+
+# ---- NEXT-4: gravitational-wave auxiliary fields (Eq.16) ------------------------------------------------
+
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (2, 3), (3, 3)])
+def test_gw_ragged_multibox_fp64(order, g):
+    P = _pair()
+    n0 = (40, 24, 72)
+    o, s = P.make_pair(n0, boxes=_ragged_boxes(), nghost=g, blocking_factor=8, lap_order=order, h0=0.5, lam=0.7,
+                       a_mass=0.3, friction=2.0, gw=True, gw_coupling=0.8, gw_friction=3.0)
+    P.init_smooth(o, s, n0, 5, comps=range(16), amp=0.5)
+    eta, dt = 1.5, 0.05
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    s.synchronize()
+    assert P.max_err(o, s, comps=range(16)) <= F64_TOL
+    # the auxiliary fields must actually have been sourced
+    assert max(float(np.abs(o.get_state(0, c)).max()) for c in range(4, 10)) > 1e-3
+
+
+def test_gw_classic_dataflow_and_fp32():
+    P = _pair()
+    n0 = (40, 24, 72)
+    o, s = P.make_pair(n0, boxes=_ragged_boxes(), nghost=2, lap_order=2, h0=0.5, lam=1.0, gw=True, gw_coupling=1.0,
+                       rk_dataflow="classic")
+    P.init_smooth(o, s, n0, 6, comps=range(16), amp=0.5)
+    o32, s32 = P.make_pair(n0, boxes=_ragged_boxes(), nghost=2, lap_order=2, h0=0.5, lam=1.0, gw=True, gw_coupling=1.0,
+                           dtype="f32", rk_dataflow="fused")  # fused is not applicable with gw: staged sweeps run
+    P.init_smooth(o32, s32, n0, 6, comps=range(16), amp=0.5)
+    eta, dt = 1.0, 0.05
+    for _ in range(3):
+        for a in (o, s, o32, s32):
+            a.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, comps=range(16)) <= F64_TOL
+    assert P.max_err(o32, s32, comps=range(16), relative=True) <= F32_TOL
+
+
+def test_gw_three_levels_subcycled_with_average_down():
+    """16 components through the whole AMR path: per-stage ghost fills (same-level + trilinear coarse->fine, linear
+    in time), subcycling and average-down."""
+    P = _pair()
+    n0 = 32
+    boxes = _ring_hierarchy(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=2, lap_order=2, h0=0.5, lam=1.0, gw=True, gw_coupling=0.5,
+                       gw_friction=1.0)
+    P.init_smooth(o, s, n0, 7, comps=range(16), amp=0.5)
+    for l in (2, 1):
+        o.average_down(l)
+        s.average_down(l)
+    eta, dt = 1.0, 0.1
+    for _ in range(2):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, comps=range(16)) <= F64_TOL
+    # ghosts of the auxiliary fields after an explicit fill
+    o.fill_ghosts(1, eta)
+    s.fill_ghosts(1, eta)
+    for ib in s.level_boxes(1):
+        for c in (4, 9, 15):
+            a = o.get_raw(ib, c)
+            b = s.get_ghosted(ib, c).cpu().numpy()
+            assert np.abs(a - b).max() <= F64_TOL
+
+
+# ---- NEXT-2: user-defined Runge-Kutta-Nystrom tableau (integrator.type 20) ------------------------------
+
+@pytest.mark.parametrize("tab", [RKN4, RK4_AS_RKN, RKN5_DENSE], ids=["nystrom4", "rk4-as-rkn", "dense5"])
+@pytest.mark.parametrize("order,g", [(1, 1), (2, 2), (3, 3)])
+def test_rkn_ragged_multibox_fp64(tab, order, g):
+    P = _pair()
+    n0 = (40, 24, 72)
+    o, s = P.make_pair(n0, boxes=_ragged_boxes(), nghost=g, lap_order=order, h0=0.5, lam=0.7, a_mass=0.3,
+                       integrator=20, rkn=tab)
+    P.init_smooth(o, s, n0, 8, amp=0.5)
+    eta, dt = 1.5, 0.05
+    for _ in range(4):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+
+
+@pytest.mark.parametrize("interp", [0, 4])
+def test_rkn_three_levels_subcycled_and_fp32(interp):
+    P = _pair()
+    n0 = 32
+    boxes = _ring_hierarchy(n0)
+    kw = dict(boxes=boxes, n_levels=3, nghost=2, lap_order=2, h0=0.5, lam=1.0, integrator=20, rkn=RKN4, interp=interp)
+    o, s = P.make_pair(n0, **kw)
+    o32, s32 = P.make_pair(n0, dtype="f32", **kw)
+    for a, b in ((o, s), (o32, s32)):
+        P.init_smooth(a, b, n0, 9, amp=0.5)
+        for l in (2, 1):
+            a.average_down(l)
+            b.average_down(l)
+    eta, dt = 1.0, 0.1
+    for _ in range(3):
+        for a in (o, s, o32, s32):
+            a.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    assert P.max_err(o32, s32, relative=True) <= F32_TOL
+
+
+# ---- NEXT-1: the shadow level of level 0 (L98) ------------------------------------------------------------
+
+@pytest.mark.parametrize("flow,nlev", [("fused", 1), ("lean", 1), ("fused", 2)])
+def test_shadow_level_tags_of_level0(flow, nlev):
+    """sledge_shadow_tee against the oracle: same final state (two coarse steps), and the same level-0 tags wherever
+    the oracle's decision does not change when its thresholds move by 1e-6 relative (the two sides' Delta differ by
+    rounding, 1e-13, against thresholds of 1e-4 .. 1e-2)."""
+    P = _pair()
+    n0 = 32
+    boxes = inputs.split_level0(n0, 16) if nlev == 1 else P.two_level_boxes(n0, 8)
+    kw = dict(boxes=boxes, n_levels=nlev, nghost=2, lap_order=2, h0=0.5, lam=1.0)
+    eta, dt = 1.0, 0.1
+
+    def fresh():
+        o, s = P.make_pair(n0, rk_dataflow=flow, shadow_level=True, **kw)
+        P.init_smooth(o, s, n0, 3, amp=0.6)
+        if nlev == 2:
+            o.average_down(1)
+            s.average_down(1)
+        return o, s
+
+    # thresholds at the median of the level-0 Delta of each component: found by bisection on the oracle
+    eps = []
+    for c in range(4):
+        lo, hi = 0.0, 1.0
+        for _ in range(16):
+            mid = 0.5 * (lo + hi)
+            o, _ = fresh()
+            e = [np.inf] * 4
+            e[c] = mid
+            t, _ = o.shadow_tee(dt, eta, *e)
+            frac = np.mean([float((a != 0).mean()) for a in t])
+            if frac > 0.5:
+                lo = mid
+            else:
+                hi = mid
+        eps.append(hi)
+    assert all(1e-9 < e < 1.0 for e in eps), eps
+    o, s = fresh()
+    ot, oc = o.shadow_tee(dt, eta, *eps)
+    gt, gc = s.shadow_tee(dt, eta, *eps)
+    s.synchronize()
+    assert P.max_err(o, s) <= F64_TOL
+    lo_t = fresh()[0].shadow_tee(dt, eta, *[e * (1 - 1e-6) for e in eps])[0]
+    hi_t = fresh()[0].shadow_tee(dt, eta, *[e * (1 + 1e-6) for e in eps])[0]
+    gts = s.split_tags(0, gt)
+    n_sure = n_all = n_tagged = 0
+    for a, b, l_, h_ in zip(ot, gts, lo_t, hi_t):
+        sure = l_ == h_
+        n_sure += int(sure.sum())
+        n_all += sure.size
+        n_tagged += int((a != 0).sum())
+        assert np.array_equal(a[sure], b.cpu().numpy()[sure])
+    assert n_sure > 0.999 * n_all and 0.2 * n_all < n_tagged < n_all
+    # counts: equal up to the cells that are not sure (8 per parent)
+    assert np.abs(oc.astype(np.int64) - gc.cpu().numpy().astype(np.int64)).sum() <= 8 * (n_all - n_sure)
+    # a context without the shadow level refuses
+    _, s2 = P.make_pair(n0, **kw)
+    with pytest.raises(Exception):
+        s2.shadow_tee(dt, eta, 1.0, 1.0)
