@@ -25,6 +25,9 @@ sys.path.insert(0, ROOT)
 
 METRIC = "Gcell-updates/s per RK stage"
 UNIT = "Gcell-updates/s"
+# Nystrom's classical three-stage fourth-order scheme as rkn.nodes / weights_b / weights_bar_b / tableau (L812-815)
+RKN4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_b=[1 / 6, 1 / 3, 0.0],
+            tableau=[0.0, 1 / 8, 0.0, 0.0, 0.5, 0.0])
 
 
 def ncu_traffic(workload, flow):
@@ -57,8 +60,11 @@ def parse():
     ap.add_argument("--ko-strength", type=float, default=0.01)
     ap.add_argument("--interp", type=int, default=0, choices=[0, 4],
                     help="coarse->fine ghost interpolation: 0 = trilinear (BASELINE.json config 5), 4 = quartic (L780)")
-    ap.add_argument("--integrator", type=int, default=4, choices=[4, 3, 10],
-                    help="integrator.type (L808): 4 = RK4 (every BASELINE.json config), 3 / 10 = SSPRK3")
+    ap.add_argument("--integrator", type=int, default=4, choices=[4, 3, 10, 20],
+                    help="integrator.type (L808): 4 = RK4 (every BASELINE.json config), 3 / 10 = SSPRK3, 20 = user RKN "
+                         "tableau (here: Nystrom's classical three-stage fourth-order scheme)")
+    ap.add_argument("--gw", action="store_true",
+                    help="also evolve the 12 gravitational-wave auxiliary components of Eq.16 (sim.gravitational_waves)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="skip the C1 CUDA-graph replay leg")
     ap.add_argument("--no-cpu", action="store_true")
@@ -301,10 +307,16 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
                  blocking_factor=cfg.blocking_factor,
                  dtype=cfg.dtype, lap_order=cfg.lap_order, h0=cfg.h0, lam=cfg.lam, rk_dataflow=args.flow, device=dev,
                  ko_order=args.ko_order, ko_strength=args.ko_strength if args.ko_order else 0.0,
-                 integrator=args.integrator, interp=args.interp)
+                 integrator=args.integrator, interp=args.interp, gw=args.gw, gw_coupling=1.0 if args.gw else 0.0,
+                 rkn=RKN4 if args.integrator == 20 else None)
     ssp = args.integrator in (3, 10)
+    rkn_st = len(RKN4["nodes"]) if args.integrator == 20 else 0
     if ssp:
         args.flow = "ssprk3"  # three staged sweeps, 8 + 12 + 12 words per cell-step
+    if rkn_st:
+        args.flow = "rkn"     # stage i: Psi_i (psi_n itself for i = 0), psi_n, Pi_n, f_0..f_{i-1} in; 4 words out
+    if args.gw and args.flow == "fused":
+        args.flow = "lean"    # the source needs psi of every stage state: staged sweeps, plus the auxiliary fields' own
     if args.ko_order and args.flow == "fused":
         args.flow = "lean"  # with the dissipation term k_psi is not pointwise: every level runs the staged sweeps
     for ib, c, t in initial_fields(cfg, rings, boxes, dev, s.tdtype):
@@ -357,8 +369,11 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
     esz = 8 if cfg.dtype == "f64" else 4
     # algorithmic words (reals read + written) per cell-step of the data-flow that runs:
     # FUSED 20 on level 0 (finer levels run LEAN), LEAN 52, CLASSIC 64
-    flow_words = {"fused": 20, "lean": 52, "classic": 64, "ssprk3": 32}
-    stage_words_per_step = sum(n * (1 << l) * (flow_words[args.flow] if (l == 0 or args.flow != "fused") else 52)
+    flow_words = {"fused": 20, "lean": 52, "classic": 64, "ssprk3": 32,
+                  "rkn": sum((2 if i else 0) + 4 + 2 * i + 4 for i in range(max(rkn_st, 1)))}
+    # gravitational-wave sector (LEAN): psi + U (u, du) in, 12 out, plus Y in stages 2-3 and Y, U2, U3 in stage 4
+    gw_words = (14 + 12) + 2 * (26 + 12) + (50 + 12) if args.gw else 0
+    stage_words_per_step = sum(n * (1 << l) * ((flow_words[args.flow] if (l == 0 or args.flow != "fused") else 52) + gw_words)
                                for l, n in enumerate(per_level))
     words_per_cell_step = stage_words_per_step / cell_steps
     n_stage, ms_stage = prof["stage"]
@@ -373,7 +388,8 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
     stage_bytes_total = stage_words_per_step * esz * steps
     # K1 launches the timed steps must have produced (2 sweeps per level-step FUSED on level 0, one per stage
     # otherwise); the library keeps at most 4096 event pairs per kind, so scale the bytes to the launches it timed
-    sweeps = [(2 if (l == 0 and args.flow == "fused") else (3 if ssp else 4)) * (1 << l) for l in range(cfg.n_levels)]
+    sweeps = [((2 if (l == 0 and args.flow == "fused") else (3 if ssp else (rkn_st if rkn_st else 4))) + (4 if args.gw else 0))
+              * (1 << l) for l in range(cfg.n_levels)]
     expected_stage = steps * sum(sweeps)
     timed_all = n_stage == expected_stage
     if not timed_all and expected_stage > 0:
@@ -389,20 +405,22 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
                 "all_launches_timed": timed_all}
     shares = {k: (v[1] / steps) for k, v in prof.items()}
 
-    value = whole_job_value(world, cell_steps, ms, stages=3 if ssp else 4)
+    nstage = 3 if ssp else (rkn_st if rkn_st else 4)
+    value = whole_job_value(world, cell_steps, ms, stages=nstage)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
             "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"{cfg.name}: {cfg.n0}^3 base, {cfg.n_levels} level(s), {cfg.dtype}, "
-                                   f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, {'SSPRK3' if ssp else 'RK4'} ({args.flow} data-flow), "
+                                   f"{'13' if cfg.lap_order == 2 else '7'}-point Laplacian, {'SSPRK3' if ssp else ('RKN4 (integrator 20)' if rkn_st else 'RK4')} ({args.flow} data-flow), "
                                    f"dt={cfg.dt}, h0={cfg.h0}, tags + 32^3 counts every step"
                                    + (f", Kreiss-Oliger order {args.ko_order} eps {args.ko_strength}" if args.ko_order else "")
+                                   + (", with the 12 gravitational-wave auxiliary components (Eq.16)" if args.gw else "")
                                    + (", quartic conservative coarse->fine interpolation" if args.interp == 4 and cfg.n_levels > 1 else ""),
                        "cells_per_level": per_level, "coverage": cover, "cell_steps_per_step": cell_steps,
                        "l2": "state buffers >> 126 MB L2 (no flush needed)" if cell_steps * esz * 4 > 4e8 else
                              "state fits in L2 (small case; not a roofline workload)",
                        "multi_gpu": "replicas only"},
-            "gcell_steps_per_s": value / (3 if ssp else 4),
+            "gcell_steps_per_s": value / nstage,
             "kernel_ms_per_step": shares, "roofline": roofline, "gpu_launches": launches, "clocks": clocks}
 
     return line, s, tags, counts, boxes, cell_steps
@@ -433,7 +451,7 @@ def run_sledge(args, cfg):
         line["e2e"] = e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags=(tags, counts))
     del s
     torch.cuda.empty_cache()
-    default_run = args.integrator == 4 and not args.ko_order and args.flow == "fused" and args.interp == 0
+    default_run = args.integrator == 4 and not args.ko_order and args.flow == "fused" and args.interp == 0 and not args.gw
     if rank == 0 and not args.no_graph and args.integrator == 4 and not args.ko_order:
         from paper_2404_02950_b200 import inputs as _inputs
         line["c1_graph_replay"] = graph_leg(_inputs.CONFIGS["C1"], dev, "fused")
@@ -666,7 +684,7 @@ def e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags):
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / args.e2e_steps
-    return {"value": whole_job_value(world, cell_steps, ms, stages=3 if args.integrator in (3, 10) else 4),
+    return {"value": whole_job_value(world, cell_steps, ms, stages={3: 3, 10: 3, 20: len(RKN4["nodes"])}.get(args.integrator, 4)),
             "unit": UNIT, "ms_per_step": ms,
             "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "steps": args.e2e_steps,
             "what": "sledge_set_state_host x4/box + sledge_rk_step + sledge_tag_strings + sledge_get_state_host x4/box + counts"}

@@ -80,6 +80,10 @@ struct GhostArgs {
   unsigned* star_count;
   uint4* qstar_list;       // plan: the parents with star children, packed (order = order of arrival); the fills before
   unsigned* qstar_count;   //       an RK sweep run over this list only, with every lane busy
+  // star patches (k_fill_patches): the fills before an RK sweep as rectangular regions, 2 x uint4 per patch
+  const uint4* patches;
+  unsigned n_patches;
+  int patch_smem_pairs;    // shared-memory pairs per warp and plane (largest coarse region of an interpolation patch)
 };
 
 __device__ __forceinline__ long long cell_offset(const BoxDev& b, int g, int ox, int i, int j, int k) {
@@ -589,6 +593,121 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs
       a.psi[dst] = mkpair(s[c][0], s[c][1]);
       if (FILL_PI) a.pi[dst] = mkpair(p[c][0], p[c][1]);
     }
+}
+
+// ---- star patches: the fill before an RK sweep, by rectangular region ---------------------------------------------
+// The cells a star stencil of radius R reaches outside a box are six slabs R cells thick.  Cut along the blocking
+// factor (the granularity of box ownership, L39), every piece -- a patch of R x bf x bf, bf x R x bf or bf x bf x R
+// cells -- takes all its data from ONE place, resolved on the host at create time (sledge.cu: plan_patches):
+//   COPY    a box of the same level (periodic wrap included): dst / src corner offsets and the two boxes' pitches;
+//           16 bytes read + 16 written per cell and plane, no per-cell list entry (2 + 2 words)
+//   INTERP  coarse->fine with every parent of the patch in ONE coarse box: the warp stages the coarse region
+//           ((bf/2 + 2)^2 x (R/2 + 2) cells or less) in shared memory, blended in time ONCE per coarse cell
+//           (c = (1-alpha) old + alpha new, L72), and every fine cell takes its 8 corners from there: ~1.7 coarse
+//           loads per fine cell instead of 16, same arithmetic in the same order as interp_coarse (bit-identical)
+//   SLOW    parents in several coarse boxes or across the periodic seam: per cell, as ghost_interp_entry
+// One warp per patch.  Entry (2 x uint4):
+//   A = {dst, src | coarse region base, dst sx | sy << 16, src sx | sy << 16}
+//   B = {ex | ey << 8 | ez << 16 | kind << 24, cex | cey << 8 | cez << 16 | parity << 24, (f0+g) | (f1+g) << 16, f2+g}
+// parity bit d = (first fine index along d) mod 2; (f0,f1,f2) = unwrapped level index of the first cell.
+enum PatchKind { PATCH_COPY = 0, PATCH_INTERP = 1, PATCH_SLOW = 2 };
+constexpr int PATCH_WARPS = 4;
+
+template <typename T, bool FILL_PI>
+__global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostArgs<T> a) {
+  using P = typename PairOf<T>::type;
+  extern __shared__ __align__(16) unsigned char patch_smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned ip = blockIdx.x * PATCH_WARPS + warp;
+  if (ip >= a.n_patches) return;
+  const uint4 A = __ldg(a.patches + 2 * (size_t)ip), B = __ldg(a.patches + 2 * (size_t)ip + 1);
+  const int ex = B.x & 0xff, ey = (B.x >> 8) & 0xff, ez = (B.x >> 16) & 0xff, kind = B.x >> 24;
+  const int dsx = A.z & 0xffff, dpl = dsx * (int)(A.z >> 16);
+  const int ncell = ex * ey * ez;
+  if (kind == PATCH_COPY) {
+    const int ssx = A.w & 0xffff, spl = ssx * (int)(A.w >> 16);
+    for (int q = lane; q < ncell; q += 32) {
+      const int i = q % ex, j = (q / ex) % ey, k = q / (ex * ey);
+      const unsigned so = A.y + (unsigned)(k * spl + j * ssx + i), d = A.x + (unsigned)(k * dpl + j * dsx + i);
+      const P v = a.psi[so];
+      P vp;
+      if (FILL_PI) vp = a.pi[so];
+      a.psi[d] = v;
+      if (FILL_PI) a.pi[d] = vp;
+    }
+    return;
+  }
+  if (kind == PATCH_INTERP) {
+    const int cex = B.y & 0xff, cey = (B.y >> 8) & 0xff, cez = (B.y >> 16) & 0xff, par = B.y >> 24;
+    const int csx = A.w & 0xffff, cpl = csx * (int)(A.w >> 16);
+    P* const cs = reinterpret_cast<P*>(patch_smem) + (size_t)warp * a.patch_smem_pairs * (FILL_PI ? 2 : 1);
+    P* const cp = cs + a.patch_smem_pairs;
+    const int ncoarse = cex * cey * cez;
+    const T oma = T(1) - a.alpha;
+    for (int q = lane; q < ncoarse; q += 32) {
+      const int i = q % cex, j = (q / cex) % cey, k = q / (cex * cey);
+      const long long o = (long long)A.y + (k * cpl + j * csx + i);
+      const P vo = a.c_old_psi[o];
+      if (a.single) {
+        cs[q] = vo;
+        if (FILL_PI) cp[q] = a.c_old_pi[o];
+      } else {
+        const P vn = a.c_new_psi[o];
+        cs[q] = mkpair(oma * vo.x + a.alpha * vn.x, oma * vo.y + a.alpha * vn.y);
+        if (FILL_PI) {
+          const P po = a.c_old_pi[o], pn = a.c_new_pi[o];
+          cp[q] = mkpair(oma * po.x + a.alpha * pn.x, oma * po.y + a.alpha * pn.y);
+        }
+      }
+    }
+    __syncwarp();
+    const T w[2] = {T(0.75), T(0.25)};
+    for (int q = lane; q < ncell; q += 32) {
+      const int i = q % ex, j = (q / ex) % ey, k = q / (ex * ey);
+      // parents of fine index f = 2m + par + i relative to the region's first coarse cell (which is the lowest parent
+      // of the patch's first cell: m - 1 if par = 0, else m): c0 = m + ((par + i) >> 1); the second parent is
+      // c0 - 1 (even fine index) or c0 + 1 (odd)
+      const int px = par & 1, py = (par >> 1) & 1, pz = (par >> 2) & 1;
+      const int x0 = ((px + i) >> 1) + 1 - px, y0 = ((py + j) >> 1) + 1 - py, z0 = ((pz + k) >> 1) + 1 - pz;
+      const int x1 = ((px + i) & 1) ? x0 + 1 : x0 - 1, y1 = ((py + j) & 1) ? y0 + 1 : y0 - 1, z1 = ((pz + k) & 1) ? z0 + 1 : z0 - 1;
+      T s0 = T(0), s1 = T(0), t0 = T(0), t1 = T(0);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        const int o = (((c & 4) ? z1 : z0) * cey + ((c & 2) ? y1 : y0)) * cex + ((c & 1) ? x1 : x0);
+        const T wt = (w[(c >> 2) & 1] * w[(c >> 1) & 1]) * w[c & 1];
+        const P cv = cs[o];
+        s0 += wt * cv.x;
+        s1 += wt * cv.y;
+        if (FILL_PI) {
+          const P pv = cp[o];
+          t0 += wt * pv.x;
+          t1 += wt * pv.y;
+        }
+      }
+      const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
+      a.psi[d] = mkpair(s0, s1);
+      if (FILL_PI) a.pi[d] = mkpair(t0, t1);
+    }
+    return;
+  }
+  // PATCH_SLOW: parents looked up per cell
+  const int g = a.geom.g;
+  const int f0 = (int)(B.z & 0xffffu) - g, f1 = (int)(B.z >> 16) - g, f2 = (int)B.w - g;
+  for (int q = lane; q < ncell; q += 32) {
+    const int i = q % ex, j = (q / ex) % ey, k = q / (ex * ey);
+    const int f[3] = {f0 + i, f1 + j, f2 + k};
+    int c0[3], c1[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) parents_of(f[d], c0[d], c1[d]);
+    long long o[8];
+    if (!coarse_offsets(a.cboxes, a.cowner, a.cgeom, c0, c1, o)) {
+      *a.err_flag = 1;
+      continue;
+    }
+    const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
+    a.psi[d] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
+    if (FILL_PI) a.pi[d] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
+  }
 }
 
 }  // namespace sledge

@@ -51,11 +51,15 @@ def test_arena_bytes_matches_hand_count_single_box():
     assert n32 >= 8 * 64 * 34 * 34 * 8
 
 
+RKN4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_b=[1 / 6, 1 / 3, 0.0],
+            tableau=[0.0, 1 / 8, 0.0, 0.0, 0.5, 0.0])
+
+
 def test_validation_rules_from_the_paper():
     ok = dict(n_levels=1, nghost=2, blocking_factor=8, lap_order=2)
     S.sledge_arena_bytes(32, **ok)
     bad = [
-        dict(ok, lap_order=3),                     # only 7- and 13-point stencils
+        dict(ok, lap_order=3),                     # the 19-point stencil needs 3 ghost layers: lap_order <= nghost (L240)
         dict(ok, nghost=1),                        # lap_order <= nghost (L240)
         dict(ok, nghost=8),                        # nghost < blocking_factor (L772)
         dict(ok, blocking_factor=12),              # power of 2 (L39)
@@ -65,11 +69,27 @@ def test_validation_rules_from_the_paper():
         dict(ok, interp=2),                        # only trilinear (0) and quartic conservative (4, L780)
         dict(ok, n_levels=2, nghost=5, lap_order=2, interp=4,  # ceil(5/2) + 2 > 8/2: window leaves the nesting gap (L70)
              boxes=[(0, (0, 0, 0), (31, 31, 31)), (1, (16, 16, 16), (47, 47, 47))]),
-        dict(ok, integrator=21),                   # RKN tableaux are not printed in the paper: not built
+        dict(ok, integrator=21),                   # the RKN4 / RKN5 tableaux (types 21, 22) are not printed in the paper: unavailable
+        dict(ok, integrator=20),                   # type 20 needs the user's tableau (L812-815)
+        dict(ok, integrator=20, rkn=RKN4, friction=2.0),         # a Nystrom scheme integrates psi'' = f(psi) only
+        dict(ok, integrator=20, rkn=RKN4, ko_order=2, ko_strength=0.01),
+        dict(ok, integrator=20, rkn=dict(RKN4, tableau=[0.0, 1 / 8, 0.1, 0.0, 0.5, 0.0])),  # implicit diagonal entry (L815)
+        dict(ok, integrator=20, rkn=dict(RKN4, nodes=[0.1, 0.5, 1.0])),                      # first stage = the state
+        dict(ok, integrator=20, rkn=RKN4, gw=True),
+        dict(ok, gw=True, integrator=10),          # auxiliary fields: classic RK4 only
+        dict(ok, gw=True, interp=4, n_levels=2, nghost=3,
+             boxes=[(0, (0, 0, 0), (31, 31, 31)), (1, (16, 16, 16), (47, 47, 47))]),
         dict(ok, ko_order=2, ko_strength=(0.0, -0.1, 0.0, 0.0)),  # strength in R+ (L749)
     ]
     S.sledge_arena_bytes(32, **dict(ok, ko_order=2, ko_strength=(0.0, 0.0, 0.02, 0.0)))
     S.sledge_arena_bytes(32, **dict(ok, integrator=10))
+    S.sledge_arena_bytes(32, **dict(ok, integrator=20, rkn=RKN4))
+    # the auxiliary fields add six pair planes per state buffer: 4x the state
+    assert S.sledge_arena_bytes(32, **dict(ok, gw=True)) > 3.5 * S.sledge_arena_bytes(32, **ok)
+    # shadow level (L98): level 0 coarsened by 2 in one box; n0 must be even and the coarsened grid valid
+    assert S.sledge_arena_bytes(32, **dict(ok, shadow_level=True)) > S.sledge_arena_bytes(32, **ok)
+    with pytest.raises(S.SledgeError, match="shadow"):
+        S.sledge_arena_bytes(8, **dict(ok, shadow_level=True, nghost=4))  # 4^3 cells cannot carry 4 ghost layers (L772)
     S.sledge_arena_bytes(32, **dict(ok, n_levels=2, nghost=3, interp=4,
                                     boxes=[(0, (0, 0, 0), (31, 31, 31)), (1, (16, 16, 16), (47, 47, 47))]))
     S.sledge_arena_bytes(32, **dict(ok, ko_order=7, ko_strength=0.0))  # strength 0 removes the term, order unused
