@@ -626,14 +626,27 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostAr
   const int ncell = ex * ey * ez;
   if (kind == PATCH_COPY) {
     const int ssx = A.w & 0xffff, spl = ssx * (int)(A.w >> 16);
-    for (int q = lane; q < ncell; q += 32) {
-      const int i = q % ex, j = (q / ex) % ey, k = q / (ex * ey);
-      const unsigned so = A.y + (unsigned)(k * spl + j * ssx + i), d = A.x + (unsigned)(k * dpl + j * dsx + i);
-      const P v = a.psi[so];
-      P vp;
-      if (FILL_PI) vp = a.pi[so];
-      a.psi[d] = v;
-      if (FILL_PI) a.pi[d] = vp;
+    // four cells per lane and pass, every load issued before the first store
+    for (int q0 = lane; q0 < ncell; q0 += 128) {
+      P v[4], vp[4];
+      unsigned d[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int q = q0 + 32 * u;
+        if (q < ncell) {
+          const int i = q % ex, j = (q / ex) % ey, k = q / (ex * ey);
+          const unsigned so = A.y + (unsigned)(k * spl + j * ssx + i);
+          d[u] = A.x + (unsigned)(k * dpl + j * dsx + i);
+          v[u] = a.psi[so];
+          if (FILL_PI) vp[u] = a.pi[so];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (q0 + 32 * u < ncell) {
+          a.psi[d[u]] = v[u];
+          if (FILL_PI) a.pi[d[u]] = vp[u];
+        }
     }
     return;
   }
@@ -644,19 +657,33 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostAr
     P* const cp = cs + a.patch_smem_pairs;
     const int ncoarse = cex * cey * cez;
     const T oma = T(1) - a.alpha;
-    for (int q = lane; q < ncoarse; q += 32) {
-      const int i = q % cex, j = (q / cex) % cey, k = q / (cex * cey);
-      const long long o = (long long)A.y + (k * cpl + j * csx + i);
-      const P vo = a.c_old_psi[o];
-      if (a.single) {
-        cs[q] = vo;
-        if (FILL_PI) cp[q] = a.c_old_pi[o];
-      } else {
-        const P vn = a.c_new_psi[o];
-        cs[q] = mkpair(oma * vo.x + a.alpha * vn.x, oma * vo.y + a.alpha * vn.y);
-        if (FILL_PI) {
-          const P po = a.c_old_pi[o], pn = a.c_new_pi[o];
-          cp[q] = mkpair(oma * po.x + a.alpha * pn.x, oma * po.y + a.alpha * pn.y);
+    for (int q0 = lane; q0 < ncoarse; q0 += 128) {  // four coarse cells per lane and pass, loads first
+      P vo[4], vn[4], po[4], pn[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int q = q0 + 32 * u;
+        if (q < ncoarse) {
+          const int i = q % cex, j = (q / cex) % cey, k = q / (cex * cey);
+          const long long o = (long long)A.y + (k * cpl + j * csx + i);
+          vo[u] = a.c_old_psi[o];
+          if (!a.single) vn[u] = a.c_new_psi[o];
+          if (FILL_PI) {
+            po[u] = a.c_old_pi[o];
+            if (!a.single) pn[u] = a.c_new_pi[o];
+          }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int q = q0 + 32 * u;
+        if (q < ncoarse) {
+          if (a.single) {
+            cs[q] = vo[u];
+            if (FILL_PI) cp[q] = po[u];
+          } else {
+            cs[q] = mkpair(oma * vo[u].x + a.alpha * vn[u].x, oma * vo[u].y + a.alpha * vn[u].y);
+            if (FILL_PI) cp[q] = mkpair(oma * po[u].x + a.alpha * pn[u].x, oma * po[u].y + a.alpha * pn[u].y);
+          }
         }
       }
     }

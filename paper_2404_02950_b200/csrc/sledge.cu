@@ -127,6 +127,9 @@ struct LevelHost {
   size_t off_qp_prefix = 0, off_qp_list = 0, off_qs_list = 0, off_qs_count = 0;
   unsigned n_star_parents = 0;  // read back from the device after the plan
   size_t off_star_list = 0, off_star_count = 0;
+  std::vector<uint4> patches, tag_patches;  // star patches / tag patches (k_fill_patches), 2 x uint4 each
+  size_t off_patches = 0, off_tag_patches = 0;
+  int patch_smem_pairs = 0;    // largest coarse region of an interpolation patch (pairs)
   size_t off_tmaps = 0;        // k_rk_tma: CUtensorMap[NBUF * 2][nbox] of the level's state planes (fused levels only)
   bool has_tmaps = false;
   std::vector<CUtensorMap> tmaps_host;
@@ -182,6 +185,7 @@ struct sledge_ctx {
   int64_t launches = 0;
   bool profiling = false;
   bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
+  bool use_patches = true;  // fills before an RK sweep by region (SLEDGE_K2_PATCHES=0 selects the packed per-cell list)
   sledge_ctx* shadow = nullptr;  // the shadow level's context (shadow_level = 1)
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
   size_t ev_used[4] = {0, 0, 0, 0};
@@ -216,6 +220,110 @@ inline int ilog2(int v) {
   return s;
 }
 inline int fdiv2(int i) { return i >> 1; }
+
+// Star patches of level l (k_ghost.cuh "star patches"): the six slabs of thickness R = stencil radius around every
+// box, cut along the blocking factor; each piece is a same-level copy (periodic wrap included), an interpolation
+// whose parents all lie in one coarse box, or a slow patch (parents in several coarse boxes / across the seam).
+void plan_patches(Plan& P, int l, bool tagset) {
+  LevelHost& L = P.lev[l];
+  const sledge_params& p = P.p;
+  const int bf = p.blocking_factor, bfs = ilog2(bf), g = p.nghost, R = stencil_radius(p);
+  auto wrapi = [](int i, int n) { int r = i % n; return r < 0 ? r + n : r; };
+  auto owner_at = [&](const LevelHost& V, int i, int j, int k) {  // wrapped cell index -> local box or -1
+    return V.owner[((size_t)(k >> bfs) * V.no[1] + (j >> bfs)) * V.no[0] + (i >> bfs)];
+  };
+  auto cell_off = [&](const BoxDev& b, int i, int j, int k) {  // box-relative cell -> offset in the level plane
+    return b.base + ((long long)(k + g) * b.sy + (j + g)) * b.sx + (i + P.ox);
+  };
+  std::vector<uint4>& out = tagset ? L.tag_patches : L.patches;
+  out.clear();
+  if (!tagset) L.patch_smem_pairs = 0;
+  for (size_t q = 0; q < L.boxdev.size(); ++q) {
+    const BoxDev& b = L.boxdev[q];
+    // slabs: star set = six faces of thickness R; tag set (the +1 neighbours the plaquettes of K3 need) = the cells
+    // with every coordinate in [0, n] and at least one equal to n: x = n (y, z up to n), y = n (x < n, z up to n),
+    // z = n (x, y < n); the extra row / column at n is cut off as pieces one cell wide
+    struct Slab { int lo[3], ext[3]; };
+    std::vector<Slab> slabs;
+    if (!tagset) {
+      for (int d = 0; d < 3; ++d)
+        for (int side = 0; side < 2; ++side) {
+          Slab sl = {{0, 0, 0}, {b.n[0], b.n[1], b.n[2]}};
+          sl.lo[d] = side ? b.n[d] : -R;
+          sl.ext[d] = R;
+          slabs.push_back(sl);
+        }
+    } else {
+      for (int m = 1; m < 8; ++m) {  // bit d of m: coordinate d equals n (one cell), else runs over [0, n)
+        Slab sl;
+        for (int d = 0; d < 3; ++d) {
+          sl.lo[d] = ((m >> d) & 1) ? b.n[d] : 0;
+          sl.ext[d] = ((m >> d) & 1) ? 1 : b.n[d];
+        }
+        slabs.push_back(sl);
+      }
+    }
+    for (const Slab& sl : slabs) {
+        int lo[3], ext[3], step[3];
+        for (int d = 0; d < 3; ++d) {
+          lo[d] = sl.lo[d];
+          ext[d] = sl.ext[d];
+          step[d] = std::min(bf, sl.ext[d]);  // outside the box a slab is thinner than a blocking cell: one piece
+        }
+        for (int k0 = lo[2]; k0 < lo[2] + ext[2]; k0 += step[2])
+          for (int j0 = lo[1]; j0 < lo[1] + ext[1]; j0 += step[1])
+            for (int i0 = lo[0]; i0 < lo[0] + ext[0]; i0 += step[0]) {
+              const int e[3] = {step[0], step[1], step[2]};
+              const int c[3] = {i0, j0, k0};                                      // box-relative first cell
+              const int f[3] = {b.lo[0] + i0, b.lo[1] + j0, b.lo[2] + k0};          // unwrapped level index
+              const int w[3] = {wrapi(f[0], L.n[0]), wrapi(f[1], L.n[1]), wrapi(f[2], L.n[2])};
+              uint4 A = make_uint4((unsigned)cell_off(b, c[0], c[1], c[2]), 0u, (unsigned)b.sx | ((unsigned)b.sy << 16), 0u);
+              uint4 B = make_uint4((unsigned)e[0] | ((unsigned)e[1] << 8) | ((unsigned)e[2] << 16), 0u,
+                                   (unsigned)(f[0] + g) | ((unsigned)(f[1] + g) << 16), (unsigned)(f[2] + g));
+              // a patch never straddles a blocking-factor cell along the two in-face axes, and along the face normal
+              // it is R < bf cells starting or ending on a box face: one owner cell, no periodic seam inside
+              const int ow = owner_at(L, w[0], w[1], w[2]);
+              if (ow >= 0) {
+                const BoxDev& sb = L.boxdev[ow];
+                A.y = (unsigned)cell_off(sb, w[0] - sb.lo[0], w[1] - sb.lo[1], w[2] - sb.lo[2]);
+                A.w = (unsigned)sb.sx | ((unsigned)sb.sy << 16);
+                B.x |= (unsigned)PATCH_COPY << 24;
+              } else if (l == 0) {
+                continue;  // cannot happen: level 0 covers the domain (checked)
+              } else {
+                const LevelHost& C = P.lev[l - 1];
+                int cmin[3], cmax[3], par = 0;
+                bool one = true;
+                for (int a2 = 0; a2 < 3; ++a2) {
+                  const int fl = f[a2] + e[a2] - 1;
+                  const int m0 = fdiv2(f[a2]), m1 = fdiv2(fl);
+                  const int p0 = f[a2] - 2 * m0, p1 = fl - 2 * m1;
+                  cmin[a2] = p0 ? m0 : m0 - 1;
+                  cmax[a2] = p1 ? m1 + 1 : m1;
+                  par |= p0 << a2;
+                }
+                const int wl[3] = {wrapi(cmin[0], C.n[0]), wrapi(cmin[1], C.n[1]), wrapi(cmin[2], C.n[2])};
+                const int wh[3] = {wrapi(cmax[0], C.n[0]), wrapi(cmax[1], C.n[1]), wrapi(cmax[2], C.n[2])};
+                for (int a2 = 0; a2 < 3; ++a2) one = one && (wh[a2] - wl[a2] == cmax[a2] - cmin[a2]);  // no seam inside
+                const int owl = owner_at(C, wl[0], wl[1], wl[2]), owh = owner_at(C, wh[0], wh[1], wh[2]);
+                const int ce[3] = {cmax[0] - cmin[0] + 1, cmax[1] - cmin[1] + 1, cmax[2] - cmin[2] + 1};
+                if (one && owl >= 0 && owl == owh && ce[0] < 256 && ce[1] < 256 && ce[2] < 256) {  // a box is convex
+                  const BoxDev& cb = C.boxdev[owl];
+                  A.y = (unsigned)cell_off(cb, wl[0] - cb.lo[0], wl[1] - cb.lo[1], wl[2] - cb.lo[2]);
+                  A.w = (unsigned)cb.sx | ((unsigned)cb.sy << 16);
+                  B.x |= (unsigned)PATCH_INTERP << 24;
+                  B.y = (unsigned)ce[0] | ((unsigned)ce[1] << 8) | ((unsigned)ce[2] << 16) | ((unsigned)par << 24);
+                  L.patch_smem_pairs = std::max(L.patch_smem_pairs, ce[0] * ce[1] * ce[2]);  // shared by both sets
+                } else {
+                  B.x |= (unsigned)PATCH_SLOW << 24;
+                }
+              }
+              out.push_back(A);
+              out.push_back(B);
+            }
+    }
+  }
+}
 
 // ---- validation + layout (host only; shared by sledge_arena_bytes and sledge_create) --------------
 int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbox) {
@@ -392,6 +500,11 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       }
     }
   }
+  for (int l = 0; l < p.n_levels; ++l)
+    if (bf <= 128) {  // patch extents are kept in 8 bits
+      plan_patches(P, l, false);
+      plan_patches(P, l, true);
+    }
   // arena layout
   size_t off = 0;
   auto take = [&](size_t bytes) {
@@ -418,6 +531,8 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     L.off_star_list = take((size_t)L.ghost_prefix.back() * GHOST_THREADS * sizeof(GhostEntry));
     L.off_star_count = take(sizeof(unsigned));
     L.off_tmaps = take(L.boxdev.size() * NBUF * 2 * sizeof(CUtensorMap));
+    L.off_patches = take(L.patches.size() * sizeof(uint4));
+    L.off_tag_patches = take(L.tag_patches.size() * sizeof(uint4));
     L.off_qp_prefix = take(L.qp_prefix.size() * sizeof(int));
     L.off_qp_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
     L.off_qs_list = take((size_t)L.qp_prefix.back() * GHOST_THREADS * 2 * sizeof(uint4));
@@ -546,6 +661,9 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, 
   a.star_count = tab<unsigned>(c, L.off_star_count);
   a.qstar_list = tab<uint4>(c, L.off_qs_list);
   a.qstar_count = tab<unsigned>(c, L.off_qs_count);
+  a.patches = tab<uint4>(c, L.off_patches);
+  a.n_patches = (unsigned)(L.patches.size() / 2);
+  a.patch_smem_pairs = L.patch_smem_pairs;
   a.has_coarse = l > 0;
   a.alpha = T(0);
   if (l > 0) {
@@ -592,14 +710,37 @@ int fill_shell_copies(sledge_ctx* c, int l, int buf, bool with_pi) {
 }
 
 template <typename T>
-int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false, int wa = 0, int wb = 1) {
+int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false, int wa = 0, int wb = 1,
+                  bool tag_only = false) {
   GhostArgs<T> a = ghost_args<T>(c, l, buf, time, wa, wb);
+  if (tag_only && a.quartic == 0 && c->use_patches && !c->plan.lev[l].tag_patches.empty()) {
+    // the fill before K3: only the +1 neighbours of the plaquettes (every coordinate in [0, n], one of them = n)
+    a.patches = tab<uint4>(c, c->plan.lev[l].off_tag_patches);
+    a.n_patches = (unsigned)(c->plan.lev[l].tag_patches.size() / 2);
+    star_only = true;
+  }
   if (a.quartic == 2 && l > 0) {  // the coarse windows are read through the coarse boxes' ghost cells
     LevelHost& C = c->plan.lev[l - 1];
     const bool pair = C.have_pair && C.t_new != C.t_old;
     int rc = fill_shell_copies<T>(c, l - 1, C.cur, fill_pi);
     if (rc == SLEDGE_OK && pair) rc = fill_shell_copies<T>(c, l - 1, C.old, fill_pi);
     if (rc) return rc;
+  }
+  if (star_only && a.quartic == 0 && a.n_patches > 0 && c->use_patches) {  // by rectangular region (k_fill_patches)
+    const int pgrid = (int)((a.n_patches + PATCH_WARPS - 1) / PATCH_WARPS);
+    const size_t smem = (size_t)PATCH_WARPS * a.patch_smem_pairs * (fill_pi ? 2 : 1) * sizeof(typename PairOf<T>::type);
+    if (smem > 48 * 1024) {
+      static bool configured[2] = {false, false};  // per instantiation
+      if (!configured[fill_pi]) {
+        if (fill_pi) cudaFuncSetAttribute(k_fill_patches<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        else cudaFuncSetAttribute(k_fill_patches<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        configured[fill_pi] = true;
+      }
+    }
+    Timed t(c, KIND_GHOST);
+    if (fill_pi) k_fill_patches<T, true><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
+    else k_fill_patches<T, false><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
+    return check_launch(c, "k_fill_patches");
   }
   int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
   if (star_only) {  // before an RK sweep only the cells its star stencil reaches are needed: the packed list
@@ -1180,7 +1321,7 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   LevelHost& L = P.lev[l];
   // after a coarse step every level sits at its parent's t_new: alpha = 1, no temporal interpolation (L74)
   const double tcur = (l > 0 && P.lev[l - 1].have_pair) ? P.lev[l - 1].t_new : 0.0;
-  int rc = L.periodic_box ? SLEDGE_OK : launch_ghosts<T>(c, l, L.cur, tcur, false);  // K3 wraps by itself there
+  int rc = L.periodic_box ? SLEDGE_OK : launch_ghosts<T>(c, l, L.cur, tcur, false, false, 0, 1, true);  // K3 wraps by itself there
   if (rc) return rc;
   if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)L.count_blocks, c->stream);
   TagArgs<T> a;
@@ -1273,6 +1414,8 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   {
     const char* ev = getenv("SLEDGE_K1_TMA");
     c->use_tma = !(ev && ev[0] == '0');
+    const char* ep = getenv("SLEDGE_K2_PATCHES");
+    c->use_patches = !(ep && ep[0] == '0');
   }
   for (int l = 0; l < P.p.n_levels && c->use_tma; ++l)
     if (level_is_fused(P, l) && (rc = make_tensor_maps(c, l)) != SLEDGE_OK) {
@@ -1282,6 +1425,8 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     }
   for (LevelHost& L : P.lev) {
     up(L.off_tmaps, L.tmaps_host.data(), L.tmaps_host.size() * sizeof(CUtensorMap));
+    up(L.off_patches, L.patches.data(), L.patches.size() * sizeof(uint4));
+    up(L.off_tag_patches, L.tag_patches.data(), L.tag_patches.size() * sizeof(uint4));
     up(L.off_boxes, L.boxdev.data(), L.boxdev.size() * sizeof(BoxDev));
     up(L.off_tiles, L.tiles.data(), L.tiles.size() * sizeof(TileDev));
     up(L.off_ftiles, L.ftiles.data(), L.ftiles.size() * sizeof(TileDev));
