@@ -187,6 +187,7 @@ struct sledge_ctx {
   bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
   bool use_patches = true;  // fills before an RK sweep by region (SLEDGE_K2_PATCHES=0 selects the packed per-cell list)
   sledge_ctx* shadow = nullptr;  // the shadow level's context (shadow_level = 1)
+  int device = 0;  // the device the arena lives on: every entry point runs with it current (DeviceGuard)
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
   size_t ev_used[4] = {0, 0, 0, 0};
 };
@@ -212,6 +213,25 @@ int fail(sledge_ctx* ctx, int code, const char* fmt, ...) {
   if (ctx) ctx->err = buf; else g_err = buf;
   return code;
 }
+
+// Kernel attributes (opt-in shared-memory size) are per device: one flag per device and kernel instantiation.
+constexpr int MAX_DEVICES = 64;
+struct PerDevice {
+  bool done[MAX_DEVICES] = {};
+  bool& operator[](int d) { return done[d >= 0 && d < MAX_DEVICES ? d : 0]; }
+};
+// Makes the context's device current for the duration of an entry point and restores the caller's.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    else cudaGetLastError();
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int ilog2(int v) {
@@ -730,11 +750,12 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     const int pgrid = (int)((a.n_patches + PATCH_WARPS - 1) / PATCH_WARPS);
     const size_t smem = (size_t)PATCH_WARPS * a.patch_smem_pairs * (fill_pi ? 2 : 1) * sizeof(typename PairOf<T>::type);
     if (smem > 48 * 1024) {
-      static bool configured[2] = {false, false};  // per instantiation
-      if (!configured[fill_pi]) {
+      static PerDevice configured2[2];  // per instantiation and device
+      bool& cfg = configured2[fill_pi][c->device];
+      if (!cfg) {
         if (fill_pi) cudaFuncSetAttribute(k_fill_patches<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         else cudaFuncSetAttribute(k_fill_patches<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured[fill_pi] = true;
+        cfg = true;
       }
     }
     Timed t(c, KIND_GHOST);
@@ -844,7 +865,8 @@ int make_tensor_maps(sledge_ctx* c, int l) {
 template <typename T, int ORDER, int MODE, int KO = 0>
 cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
   constexpr int TY = K1Shape<MODE>::TY;
-  static bool configured = false;  // per instantiation
+  static PerDevice configured_dev;  // per instantiation and device
+  bool& configured = configured_dev[c->device];
   if constexpr (K1Shape<MODE>::fused && KO == 0) {
     if (a.tmap[0]) {  // TMA-staged plane ring (k_rk_tma.cuh); the maps exist on fused levels unless SLEDGE_K1_TMA=0
       constexpr int RY = FusedTile<T, ORDER>::RY;
@@ -853,7 +875,8 @@ cudaError_t launch_pipe_kernel(sledge_ctx* c, const PipeArgs<T>& a, int grid) {
       static_assert(C::SMEM_BYTES <= 227 * 1024, "K1 tile does not fit shared memory");
       constexpr int MINB = ORDER == 3 ? 1 : K1Shape<MODE>::MINB;
       auto kern = k_rk_tma<T, ORDER, MODE, K1F_TX, TY, PD, RY, MINB>;
-      static bool configured_tma = false;
+      static PerDevice configured_tma_dev;
+      bool& configured_tma = configured_tma_dev[c->device];
       if (!configured_tma) {
         const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
@@ -1337,7 +1360,8 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   a.nb1 = L.nb[1];
   {
     Timed t(c, KIND_TAG);
-    static bool configured = false;  // per instantiation
+    static PerDevice configured_dev;  // per instantiation and device
+    bool& configured = configured_dev[c->device];
     if (!configured) {
       cudaFuncSetAttribute(k_tag_strings<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
       configured = true;
@@ -1407,6 +1431,15 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   }
   c->arena = (char*)dev_arena;
   c->stream = (cudaStream_t)cuda_stream;
+  {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, dev_arena) == cudaSuccess && at.type == cudaMemoryTypeDevice) c->device = at.device;
+    else {
+      cudaGetLastError();
+      cudaGetDevice(&c->device);
+    }
+  }
+  DeviceGuard guard(c->device);
   cudaError_t e = cudaMemsetAsync(c->arena, 0, P.total, c->stream);
   auto up = [&](size_t off, const void* src, size_t bytes) {
     if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(c->arena + off, src, bytes, cudaMemcpyHostToDevice, c->stream);
@@ -1456,8 +1489,15 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   for (int l = 1; l < P.p.n_levels && e == cudaSuccess; ++l)
     if (P.lev[l].qp_prefix.back() > 0)
       e = cudaMemcpy(&P.lev[l].n_star_parents, c->arena + P.lev[l].off_qs_count, sizeof(unsigned), cudaMemcpyDeviceToHost);
+  int plan_flag = 0;  // a plan kernel met a ghost or coarse cell that no box provides
+  if (e == cudaSuccess) e = cudaMemcpy(&plan_flag, c->arena + P.off_err, sizeof(int), cudaMemcpyDeviceToHost);
   if (e != cudaSuccess) {
     rc = fail(nullptr, SLEDGE_ECUDA, "sledge_create: %s", cudaGetErrorString(e));
+    delete c;
+    return rc;
+  }
+  if (plan_flag) {
+    rc = fail(nullptr, SLEDGE_ESTATE, "sledge_create: a ghost cell has neither a same-level owner nor coarse data (nesting)");
     delete c;
     return rc;
   }
@@ -1474,6 +1514,7 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
 
 int sledge_destroy(sledge_ctx* c) {
   if (!c) return SLEDGE_OK;
+  DeviceGuard guard(c->device);
   if (c->shadow) sledge_destroy(c->shadow);
   cudaStreamSynchronize(c->stream);
   for (auto& v : c->ev)
@@ -1497,6 +1538,7 @@ static int check_box_comp(sledge_ctx* c, int box, int comp, const void* ptr) {
 int sledge_set_state(sledge_ctx* c, int box, int comp, const void* dev_src) {
   int rc = check_box_comp(c, box, comp, dev_src);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   c->plan.lev[c->plan.box[box].level].have_pair = false;
   return DISPATCH(c, do_copy_comp<float>(c, box, comp, (void*)dev_src, true, false),
                   do_copy_comp<double>(c, box, comp, (void*)dev_src, true, false));
@@ -1505,6 +1547,7 @@ int sledge_set_state(sledge_ctx* c, int box, int comp, const void* dev_src) {
 int sledge_get_state(sledge_ctx* c, int box, int comp, void* dev_dst) {
   int rc = check_box_comp(c, box, comp, dev_dst);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   return DISPATCH(c, do_copy_comp<float>(c, box, comp, dev_dst, false, false),
                   do_copy_comp<double>(c, box, comp, dev_dst, false, false));
 }
@@ -1512,6 +1555,7 @@ int sledge_get_state(sledge_ctx* c, int box, int comp, void* dev_dst) {
 int sledge_get_ghosted(sledge_ctx* c, int box, int comp, void* dev_dst) {
   int rc = check_box_comp(c, box, comp, dev_dst);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   return DISPATCH(c, do_copy_comp<float>(c, box, comp, dev_dst, false, true),
                   do_copy_comp<double>(c, box, comp, dev_dst, false, true));
 }
@@ -1524,6 +1568,7 @@ static size_t box_valid_bytes(sledge_ctx* c, int box) {
 int sledge_set_state_host(sledge_ctx* c, int box, int comp, const void* host_src) {
   int rc = check_box_comp(c, box, comp, host_src);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   void* scratch = c->arena + c->plan.off_scratch;
   const cudaError_t e = cudaMemcpyAsync(scratch, host_src, box_valid_bytes(c, box), cudaMemcpyHostToDevice, c->stream);
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "set_state_host: %s", cudaGetErrorString(e));
@@ -1533,6 +1578,7 @@ int sledge_set_state_host(sledge_ctx* c, int box, int comp, const void* host_src
 int sledge_get_state_host(sledge_ctx* c, int box, int comp, void* host_dst) {
   int rc = check_box_comp(c, box, comp, host_dst);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   void* scratch = c->arena + c->plan.off_scratch;
   rc = sledge_get_state(c, box, comp, scratch);
   if (rc) return rc;
@@ -1550,6 +1596,7 @@ static int check_level(sledge_ctx* c, int level) {
 int sledge_fill_ghosts(sledge_ctx* c, int level, double time) {
   int rc = check_level(c, level);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   const int cur = c->plan.lev[level].cur;
   rc = DISPATCH(c, launch_ghosts<float>(c, level, cur, time, true), launch_ghosts<double>(c, level, cur, time, true));
   if (c->plan.p.gw)
@@ -1562,12 +1609,14 @@ int sledge_fill_ghosts(sledge_ctx* c, int level, double time) {
 int sledge_rk_stage(sledge_ctx* c, int level, int stage, double dt, double eta) {
   int rc = check_level(c, level);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   if (stage < 0 || stage > 4) return fail(c, SLEDGE_EINVAL, "stage must be 0..3 (0..4 for a five-stage RKN tableau)");
   return DISPATCH(c, do_stage<float>(c, level, stage, eta, dt, eta), do_stage<double>(c, level, stage, eta, dt, eta));
 }
 
 int sledge_rk_step(sledge_ctx* c, double dt, double eta) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  DeviceGuard guard(c->device);
   if (!(dt > 0)) return fail(c, SLEDGE_EINVAL, "dt must be positive");
   return DISPATCH(c, advance<float>(c, 0, eta, dt, eta), advance<double>(c, 0, eta, dt, eta));
 }
@@ -1575,12 +1624,14 @@ int sledge_rk_step(sledge_ctx* c, double dt, double eta) {
 int sledge_tag_strings(sledge_ctx* c, int level, uint8_t* dev_tags, uint32_t* dev_counts) {
   int rc = check_level(c, level);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   return DISPATCH(c, do_tag<float>(c, level, dev_tags, dev_counts), do_tag<double>(c, level, dev_tags, dev_counts));
 }
 
 int sledge_average_down(sledge_ctx* c, int fine_level) {
   int rc = check_level(c, fine_level);
   if (rc) return rc;
+  DeviceGuard guard(c->device);
   if (fine_level < 1) return fail(c, SLEDGE_EINVAL, "average_down needs fine_level >= 1");
   return DISPATCH(c, do_average_down<float>(c, fine_level), do_average_down<double>(c, fine_level));
 }
@@ -1610,6 +1661,7 @@ int sledge_tee_enable(sledge_ctx* c, int fine_level, const double* eps4, uint8_t
 
 int sledge_shadow_tee(sledge_ctx* c, double dt, double eta, const double* eps4, uint8_t* dev_tags, uint32_t* dev_counts) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  DeviceGuard guard(c->device);
   if (!c->shadow) return fail(c, SLEDGE_ESTATE, "shadow_tee: the context was created without shadow_level = 1 (L98)");
   if (!(dt > 0)) return fail(c, SLEDGE_EINVAL, "dt must be positive");
   if (!eps4) return fail(c, SLEDGE_EINVAL, "shadow_tee: null thresholds");
@@ -1642,11 +1694,15 @@ int64_t sledge_launch_count(const sledge_ctx* c) { return c ? c->launches : 0; }
 
 int sledge_synchronize(sledge_ctx* c) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  DeviceGuard guard(c->device);
   cudaError_t e = cudaStreamSynchronize(c->stream);
   int flag = 0;
   if (e == cudaSuccess) e = cudaMemcpy(&flag, c->arena + c->plan.off_err, sizeof(int), cudaMemcpyDeviceToHost);
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "synchronize: %s", cudaGetErrorString(e));
-  if (flag) return fail(c, SLEDGE_ESTATE, "a kernel found a cell with neither a same-level owner nor coarse data (nesting)");
+  if (flag) {  // reported once: cleared so that later calls report later faults only
+    cudaMemset(c->arena + c->plan.off_err, 0, sizeof(int));
+    return fail(c, SLEDGE_ESTATE, "a kernel found a cell with neither a same-level owner nor coarse data (nesting)");
+  }
   return SLEDGE_OK;
 }
 
@@ -1659,6 +1715,7 @@ int sledge_profile_enable(sledge_ctx* c, int on) {
 
 int sledge_profile_read(sledge_ctx* c, int kind, int64_t* launches, double* total_ms) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  DeviceGuard guard(c->device);
   if (kind < 0 || kind > 3) return fail(c, SLEDGE_EINVAL, "kind must be 0..3");
   const cudaError_t e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "profile_read: %s", cudaGetErrorString(e));
