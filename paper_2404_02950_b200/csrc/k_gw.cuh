@@ -10,10 +10,12 @@
 // Storage: six pair planes per state buffer, (u_xx,u_yy) (u_zz,u_xy) (u_xz,u_yz) and the same for du, each laid out
 // exactly like the (psi1,psi2) plane, so that K2 and K4 serve them unchanged.
 //
-// Mapping: a CTA owns a 32 x GW_TY column tile of one box and marches along z; a thread keeps the 2R+1 z-window of
-// its cell of the four differenced planes (psi and the three u planes) in registers and reads the x/y neighbours of
-// the centre plane through the read-only L1 path (the tile's rows are 512-byte runs that the CTA's own threads
-// have just pulled in).  Words per cell-stage: 2 (psi) + 12 (U) + 12 per pointwise input state + 12 written.
+// Mapping: a CTA owns a 32 x GW_TY column tile of one box and ONE of the three pair planes (blockIdx.y) and marches
+// along z; a thread keeps the 2R+1 z-window of its cell of the two differenced planes (psi and its u plane) in
+// registers and reads the x/y neighbours of the centre plane through the read-only L1 path (the tile's rows are
+// 512-byte runs that the CTA's own threads have just pulled in).  psi is read by all three CTAs of a tile (through
+// L2).  Words per cell-stage: 2 (psi) + 12 (U) + 12 per pointwise input state + 12 written.
+// (One CTA for all three planes needs four z-windows: 255 registers, one CTA per SM, 39 % of the HBM roofline.)
 // This is the straightforward version of the sweep: no shared-memory staging yet.
 #pragma once
 #include "k_rk_pipe.cuh"
@@ -49,13 +51,14 @@ __device__ __forceinline__ T grad_from(const T* m, const T* p, T inv_h) {
 }
 
 template <typename T, int ORDER, int MODE>
-__global__ void __launch_bounds__(GW_TX* GW_TY) k_gw_stage(const GwArgs<T> a) {
+__global__ void __launch_bounds__(GW_TX* GW_TY, 2) k_gw_stage(const GwArgs<T> a) {
   using P = typename PairOf<T>::type;
   constexpr int R = ORDER;
   constexpr int CPT = Vec16<T>::CPT;  // the tiles are 32 * CPT cells wide: CPT passes over x
   constexpr int NIN = MODE == LEAN_S1 ? 0 : (MODE == LEAN_S4 ? 3 : 1);
   const TileDev t = a.tiles[blockIdx.x];
   const BoxDev b = a.boxes[t.box];
+  const int q = blockIdx.y;  // which u / du pair plane: 0 = (xx,yy), 1 = (zz,xy), 2 = (xz,yz)
   const int tx = threadIdx.x % GW_TX, ty = threadIdx.x / GW_TX;
   const int y = t.y0 + ty;
   if (y >= b.n[1]) return;
@@ -64,25 +67,25 @@ __global__ void __launch_bounds__(GW_TX* GW_TY) k_gw_stage(const GwArgs<T> a) {
     const int x = t.x0 + px * GW_TX + tx;
     if (x >= b.n[0]) continue;
     const long long off = b.base + (long long)(t.z0 + a.g) * plane + (long long)(y + a.g) * b.sx + (x + a.ox);
-    // z-windows of the four differenced planes: w[0] = psi, w[1..3] = u planes; w[f][m] = plane z + m - R
-    const P* const src[4] = {a.psi, a.u[0], a.u[1], a.u[2]};
-    P w[4][2 * R + 1];
+    // z-windows of the two differenced planes: w[0] = psi, w[1] = this CTA's u pair plane; w[f][m] = plane z + m - R
+    const P* const src[2] = {a.psi, a.u[q]};
+    P w[2][2 * R + 1];
 #pragma unroll
-    for (int f = 0; f < 4; ++f)
+    for (int f = 0; f < 2; ++f)
 #pragma unroll
       for (int m = 0; m < 2 * R; ++m) w[f][m + 1] = __ldg(src[f] + off + (long long)(m - R) * plane);
     for (int zz = 0; zz < t.nz; ++zz) {
       const long long o = off + (long long)zz * plane;
 #pragma unroll
-      for (int f = 0; f < 4; ++f) {
+      for (int f = 0; f < 2; ++f) {
 #pragma unroll
         for (int m = 0; m < 2 * R; ++m) w[f][m] = w[f][m + 1];
         w[f][2 * R] = __ldg(src[f] + o + (long long)R * plane);
       }
       // x / y neighbours of the centre plane
-      P xm[4][R], xp[4][R], ym[4][R], yp[4][R];
+      P xm[2][R], xp[2][R], ym[2][R], yp[2][R];
 #pragma unroll
-      for (int f = 0; f < 4; ++f)
+      for (int f = 0; f < 2; ++f)
 #pragma unroll
         for (int r = 1; r <= R; ++r) {
           xm[f][r - 1] = __ldg(src[f] + o - r);
@@ -106,9 +109,7 @@ __global__ void __launch_bounds__(GW_TX* GW_TY) k_gw_stage(const GwArgs<T> a) {
         for (int r = 0; r < R; ++r) { m[r] = comp(w[0][R - 1 - r]); p[r] = comp(w[0][R + 1 + r]); }
         gr[c][2] = grad_from<T, ORDER>(m, p, a.inv_h);
       }
-      const int GI[6] = {0, 1, 2, 0, 0, 1}, GJ[6] = {0, 1, 2, 1, 2, 2};  // xx, yy, zz, xy, xz, yz (L436)
-#pragma unroll
-      for (int q = 0; q < 3; ++q) {  // pair plane q holds components 2q, 2q + 1
+      {  // pair plane q holds components 2q, 2q + 1
         const P dv = __ldg(a.du[q] + o);
         T ku[2], kdu[2], uc[2], duc[2];
 #pragma unroll
@@ -118,17 +119,20 @@ __global__ void __launch_bounds__(GW_TX* GW_TY) k_gw_stage(const GwArgs<T> a) {
           T xm_[3], xp_[3], ym_[3], yp_[3], zm_[3], zp_[3];
 #pragma unroll
           for (int r = 0; r < R; ++r) {
-            xm_[r] = comp(xm[1 + q][r]);
-            xp_[r] = comp(xp[1 + q][r]);
-            ym_[r] = comp(ym[1 + q][r]);
-            yp_[r] = comp(yp[1 + q][r]);
-            zm_[r] = comp(w[1 + q][R - 1 - r]);
-            zp_[r] = comp(w[1 + q][R + 1 + r]);
+            xm_[r] = comp(xm[1][r]);
+            xp_[r] = comp(xp[1][r]);
+            ym_[r] = comp(ym[1][r]);
+            yp_[r] = comp(yp[1][r]);
+            zm_[r] = comp(w[1][R - 1 - r]);
+            zp_[r] = comp(w[1][R + 1 + r]);
           }
-          uc[c] = comp(w[1 + q][R]);
+          uc[c] = comp(w[1][R]);
           duc[c] = comp(dv);
           const T lap = lap_from<T, ORDER>(uc[c], xm_, xp_, ym_, yp_, zm_, zp_, a.inv_h2);
-          const T Tij = gr[0][GI[mc]] * gr[0][GJ[mc]] + gr[1][GI[mc]] * gr[1][GJ[mc]];
+          // (i, j) of component mc in the order xx, yy, zz, xy, xz, yz (L436), one hex digit each
+          const int gi = (0x100210 >> (4 * mc)) & 3, gj = (0x221210 >> (4 * mc)) & 3;
+          auto pick = [](const T* v, int d) -> T { return d == 0 ? v[0] : (d == 1 ? v[1] : v[2]); };
+          const T Tij = pick(gr[0], gi) * pick(gr[0], gj) + pick(gr[1], gi) * pick(gr[1], gj);
           ku[c] = duc[c];
           kdu[c] = (lap + a.coupling * Tij) - a.fric * duc[c];
         }
@@ -162,9 +166,10 @@ __global__ void __launch_bounds__(GW_TX* GW_TY) k_gw_stage(const GwArgs<T> a) {
 template <typename T, int ORDER>
 int launch_gw(cudaStream_t stream, const GwArgs<T>& a, int grid, int mode) {
   const int nt = GW_TX * GW_TY;
-  if (mode == LEAN_S1) k_gw_stage<T, ORDER, LEAN_S1><<<grid, nt, 0, stream>>>(a);
-  else if (mode == LEAN_S23) k_gw_stage<T, ORDER, LEAN_S23><<<grid, nt, 0, stream>>>(a);
-  else if (mode == LEAN_S4) k_gw_stage<T, ORDER, LEAN_S4><<<grid, nt, 0, stream>>>(a);
+  const dim3 g3(grid, 3);  // y: the three pair planes
+  if (mode == LEAN_S1) k_gw_stage<T, ORDER, LEAN_S1><<<g3, nt, 0, stream>>>(a);
+  else if (mode == LEAN_S23) k_gw_stage<T, ORDER, LEAN_S23><<<g3, nt, 0, stream>>>(a);
+  else if (mode == LEAN_S4) k_gw_stage<T, ORDER, LEAN_S4><<<g3, nt, 0, stream>>>(a);
   else return 1;
   return 0;
 }
