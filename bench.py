@@ -32,11 +32,12 @@ RKN4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_
 
 def ncu_traffic(workload, flow):
     """mean dram__bytes_read.sum + dram__bytes_write.sum per K1 launch of this workload / data-flow, from the committed
-    `ncu --set full` capture (profiles/r01_traffic.csv; command in profiles/r01_c3_ncu_full_final.md); None if
-    that workload was not captured."""
+    `ncu --set full` captures (profiles/r02_traffic.csv; commands in profiles/r02_k1_variants.md and
+    profiles/r02_ncu_full.md); a constant read from that file, NOT a measurement of this run; None if that workload
+    was not captured."""
     import csv
     try:
-        rows = [r for r in csv.DictReader(open(os.path.join(ROOT, "profiles", "r01_traffic.csv")))
+        rows = [r for r in csv.DictReader(open(os.path.join(ROOT, "profiles", "r02_traffic.csv")))
                 if r["workload"] == workload and r["flow"] == flow and "k_rk_" in r["kernel"]]
     except OSError:
         return None
@@ -44,7 +45,7 @@ def ncu_traffic(workload, flow):
         return None
     return {"dram_bytes_per_launch": sum(float(r["dram_bytes_per_launch"]) for r in rows) / len(rows),
             "algorithmic_bytes_per_launch": sum(float(r["algorithmic_bytes_per_launch"]) for r in rows) / len(rows),
-            "source": "profiles/r01_traffic.csv (ncu --set full, one capture per sweep kernel)"}
+            "source": "profiles/r02_traffic.csv (ncu --set full, one capture per sweep kernel; constant, not measured in this run)"}
 
 
 def parse():
@@ -246,6 +247,8 @@ def time_oracle(cfg, budget_s=12.0, steps=None, warmup=1):
     dt1 = (time.perf_counter() - t0) / 2
     orc.set_threads(cores)
     return {"value": cells * 4 / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "note": "the unoptimised correctness oracle (g++ -O2, no -march, one loop nest per definition) on a sample: "
+                    "a reported baseline of the checker, not a tuned CPU implementation",
             "sample": f"{desc}; {n} steps of rk_step + tag_strings, {dt * 1e3:.1f} ms/step",
             "single_thread_value": cells * 4 / dt1 / 1e9, "cpu_model": cpu_model()}, dt, n
 
