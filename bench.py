@@ -372,12 +372,10 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
     esz = 8 if cfg.dtype == "f64" else 4
     # algorithmic words (reals read + written) per cell-step of the data-flow that runs:
     # FUSED 20 on level 0 (finer levels run LEAN), LEAN 52, CLASSIC 64
-    flow_words = {"fused": 20, "lean": 52, "classic": 64, "ssprk3": 32,
-                  "rkn": sum((2 if i else 0) + 4 + 2 * i + 4 for i in range(max(rkn_st, 1)))}
-    # gravitational-wave sector (LEAN): psi + U (u, du) in, 12 out, plus Y in stages 2-3 and Y, U2, U3 in stage 4
-    gw_words = (14 + 12) + 2 * (26 + 12) + (50 + 12) if args.gw else 0
-    stage_words_per_step = sum(n * (1 << l) * ((flow_words[args.flow] if (l == 0 or args.flow != "fused") else 52) + gw_words)
-                               for l, n in enumerate(per_level))
+    # algorithmic words (reals read + written) per cell-step and K1 launches per level-step of the data-flow each
+    # level runs, as the library reports them (sledge_level_dataflow)
+    flows = [s.level_dataflow(l) for l in range(cfg.n_levels)]
+    stage_words_per_step = sum(n * (1 << l) * flows[l][1] for l, n in enumerate(per_level))
     words_per_cell_step = stage_words_per_step / cell_steps
     n_stage, ms_stage = prof["stage"]
     peaks = {}
@@ -391,20 +389,20 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
     stage_bytes_total = stage_words_per_step * esz * steps
     # K1 launches the timed steps must have produced (2 sweeps per level-step FUSED on level 0, one per stage
     # otherwise); the library keeps at most 4096 event pairs per kind, so scale the bytes to the launches it timed
-    sweeps = [((2 if (l == 0 and args.flow == "fused") else (3 if ssp else (rkn_st if rkn_st else 4))) + (4 if args.gw else 0))
-              * (1 << l) for l in range(cfg.n_levels)]
+    sweeps = [flows[l][0] * (1 << l) for l in range(cfg.n_levels)]
     expected_stage = steps * sum(sweeps)
     timed_all = n_stage == expected_stage
     if not timed_all and expected_stage > 0:
         stage_bytes_total *= n_stage / expected_stage
     achieved = stage_bytes_total / (ms_stage * 1e-3) / 1e9 if ms_stage > 0 else 0.0
     tr = ncu_traffic(cfg.name, args.flow)
-    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_tma FUSED sweeps on level 0, k_rk_pipe staged sweeps elsewhere; mean over the "
+    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_tma FUSED sweeps on level 0 and, under trilinear interpolation, on the finer levels; k_rk_pipe staged sweeps otherwise; mean over the "
                                           "stage launches of a step: 2 sweeps per level-step FUSED, 4 otherwise)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "peak_source": peak_src, "traffic": (tr or {}).get("dram_bytes_per_launch"), "traffic_detail": tr,
                 "bytes_per_cell_step": words_per_cell_step * esz,
                 "avg_launch_ms": ms_stage / max(n_stage, 1), "launches": n_stage, "launches_expected": expected_stage,
+                "k1_launches_and_words_per_level": flows,
                 "all_launches_timed": timed_all}
     shares = {k: (v[1] / steps) for k, v in prof.items()}
 

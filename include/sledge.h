@@ -204,6 +204,11 @@ int sledge_shadow_tee(sledge_ctx* ctx, double dt, double eta, const double* eps4
 /* Bookkeeping. */
 int sledge_level_cells(const sledge_ctx* ctx, int level, int64_t* valid_cells, int64_t* count_blocks);
 int64_t sledge_launch_count(const sledge_ctx* ctx); /* kernels launched by this context so far */
+/* The data-flow `level` runs: K1 launches per step of that level (the auxiliary-field stages of
+ * gw included) and algorithmic words (reals read + written) per cell-step of those launches: FUSED 2 / 20 (level 0, and
+ * finer levels unless quartic interpolation runs per cell, nghost = 1), LEAN 4 / 52, CLASSIC 4 / 64, SSPRK3 3 / 32, RKN s / sum over the
+ * stages, plus 4 / 164 with gw.  bench.py's roofline numerator. */
+int sledge_level_dataflow(const sledge_ctx* ctx, int level, int* k1_launches_per_step, int* words_per_cell_step);
 
 /* Wait for everything enqueued so far and report deferred errors: SLEDGE_ECUDA for a kernel fault,
  * SLEDGE_ESTATE if a kernel met a ghost or coarse cell that no box provides (cannot happen for box

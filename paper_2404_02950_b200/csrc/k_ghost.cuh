@@ -83,6 +83,14 @@ struct GhostArgs {
   // star patches (k_fill_patches): the fills before an RK sweep as rectangular regions, 2 x uint4 per patch
   const uint4* patches;
   unsigned n_patches;
+  // "velocity" ghosts of the second plane (k_fill_patches, interpolated cells only; FUSED sweeps on a fine level): the
+  // sweep forms the NEXT stage's psi at a ghost cell as psi_g + tau Pi_g, and that must be the coarse state
+  // interpolated at the later time t_b (L72), so Pi_g <- (I_psi(alpha_b) - I_psi(alpha_a)) * vel_scale with
+  // I_psi(alpha) the space-time interpolation of the coarse PSI planes and vel_scale = 1 / (t_b - t_a)
+  int vel;
+  T alpha_a, alpha_b, vel_scale;
+  T vel_c;  // k_fill_qparents: the same velocity ghost written as I[(psi_new - psi_old)] / (t_new - t_old) of the coarse
+            // level (I is linear, so it equals (I_psi(alpha_b) - I_psi(alpha_a)) / (t_b - t_a) up to rounding)
   int patch_smem_pairs;    // shared-memory pairs per warp and plane (largest coarse region of an interpolation patch)
 };
 
@@ -555,7 +563,7 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs
       for (int mx = 0; mx < 5; ++mx) {
         vo[mx] = a.c_old_psi[row + mx];
         if (!SINGLE) vn[mx] = a.c_new_psi[row + mx];
-        if (FILL_PI) {
+        if (FILL_PI && !a.vel) {
           po[mx] = a.c_old_pi[row + mx];
           if (!SINGLE) pn[mx] = a.c_new_pi[row + mx];
         }
@@ -566,8 +574,13 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs
         const T c1 = SINGLE ? vo[mx].y : oma * vo[mx].y + a.alpha * vn[mx].y;
         T q0 = T(0), q1 = T(0);
         if (FILL_PI) {
-          q0 = SINGLE ? po[mx].x : oma * po[mx].x + a.alpha * pn[mx].x;
-          q1 = SINGLE ? po[mx].y : oma * po[mx].y + a.alpha * pn[mx].y;
+          if (a.vel) {  // velocity ghosts (host: never SINGLE)
+            q0 = SINGLE ? T(0) : (vn[mx].x - vo[mx].x) * a.vel_c;
+            q1 = SINGLE ? T(0) : (vn[mx].y - vo[mx].y) * a.vel_c;
+          } else {
+            q0 = SINGLE ? po[mx].x : oma * po[mx].x + a.alpha * pn[mx].x;
+            q1 = SINGLE ? po[mx].y : oma * po[mx].y + a.alpha * pn[mx].y;
+          }
         }
         // the weights of the 8 children differ by exact sign flips only (the r = 1 table is the mirror image:
         // w(m, 1) = -w(m, 0) for m != 2), and rounding is symmetric: one product per value, then +- per child
@@ -624,6 +637,7 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostAr
   const int ex = B.x & 0xff, ey = (B.x >> 8) & 0xff, ez = (B.x >> 16) & 0xff, kind = B.x >> 24;
   const int dsx = A.z & 0xffff, dpl = dsx * (int)(A.z >> 16);
   const int ncell = ex * ey * ez;
+  if (a.copy_only && kind != PATCH_COPY) return;  // quartic interpolation: k_fill_qparents does the rest
   if (kind == PATCH_COPY) {
     const int ssx = A.w & 0xffff, spl = ssx * (int)(A.w >> 16);
     // four cells per lane and pass, every load issued before the first store
@@ -657,6 +671,30 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostAr
     P* const cp = cs + a.patch_smem_pairs;
     const int ncoarse = cex * cey * cez;
     const T oma = T(1) - a.alpha;
+    const bool vel = FILL_PI && a.vel != 0;  // cs = coarse psi OLD, cp = coarse psi NEW, blended per use
+    if (vel) {
+      for (int q0 = lane; q0 < ncoarse; q0 += 128) {
+        P vo[4], vn[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int q = q0 + 32 * u;
+          if (q < ncoarse) {
+            const int i = q % cex, j = (q / cex) % cey, k = q / (cex * cey);
+            const long long o = (long long)A.y + (k * cpl + j * csx + i);
+            vo[u] = a.c_old_psi[o];
+            vn[u] = a.c_new_psi[o];
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int q = q0 + 32 * u;
+          if (q < ncoarse) {
+            cs[q] = vo[u];
+            cp[q] = vn[u];
+          }
+        }
+      }
+    } else
     for (int q0 = lane; q0 < ncoarse; q0 += 128) {  // four coarse cells per lane and pass, loads first
       P vo[4], vn[4], po[4], pn[4];
 #pragma unroll
@@ -698,6 +736,26 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostAr
       const int x0 = ((px + i) >> 1) + 1 - px, y0 = ((py + j) >> 1) + 1 - py, z0 = ((pz + k) >> 1) + 1 - pz;
       const int x1 = ((px + i) & 1) ? x0 + 1 : x0 - 1, y1 = ((py + j) & 1) ? y0 + 1 : y0 - 1, z1 = ((pz + k) & 1) ? z0 + 1 : z0 - 1;
       T s0 = T(0), s1 = T(0), t0 = T(0), t1 = T(0);
+      if (vel) {  // psi at alpha; Pi <- (psi at alpha_b - psi at alpha_a) * vel_scale, each as interp_coarse would give it
+        const T al[3] = {a.alpha, a.alpha_a, a.alpha_b};
+        T r[3][2] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          const int o = (((c & 4) ? z1 : z0) * cey + ((c & 2) ? y1 : y0)) * cex + ((c & 1) ? x1 : x0);
+          const T wt = (w[(c >> 2) & 1] * w[(c >> 1) & 1]) * w[c & 1];
+          const P vo = cs[o], vn = cp[o];
+#pragma unroll
+          for (int m = 0; m < 3; ++m) {
+            const T om = T(1) - al[m];
+            r[m][0] += wt * (om * vo.x + al[m] * vn.x);
+            r[m][1] += wt * (om * vo.y + al[m] * vn.y);
+          }
+        }
+        const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
+        a.psi[d] = mkpair(r[0][0], r[0][1]);
+        a.pi[d] = mkpair((r[2][0] - r[1][0]) * a.vel_scale, (r[2][1] - r[1][1]) * a.vel_scale);
+        continue;
+      }
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         const int o = (((c & 4) ? z1 : z0) * cey + ((c & 2) ? y1 : y0)) * cex + ((c & 1) ? x1 : x0);
@@ -733,7 +791,15 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostAr
     }
     const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
     a.psi[d] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
-    if (FILL_PI) a.pi[d] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
+    if (FILL_PI) {
+      if (a.vel) {
+        const P pa = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha_a, o);
+        const P pb = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha_b, o);
+        a.pi[d] = mkpair((pb.x - pa.x) * a.vel_scale, (pb.y - pa.y) * a.vel_scale);
+      } else {
+        a.pi[d] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
+      }
+    }
   }
 }
 

@@ -169,6 +169,7 @@ struct Plan {
   int cpa = 8;       // cells (pairs) per 128 bytes
   int ox = 8;        // x offset of the first valid cell inside a row
   size_t off_scratch = 0, scratch_bytes = 0, off_err = 0, total = 0;
+  bool fine_fused = false;  // FUSED sweeps on levels > 0 too (needs the patch fills' velocity ghosts; set at create)
   // shadow level of level 0 (L98): a nested one-box context inside the same arena
   size_t off_shadow = 0, shadow_bytes = 0;
   sledge_params shadow_p;
@@ -654,8 +655,13 @@ LevelGeom geom_of(const Plan& P, int l) {
 }
 
 // K2 arguments for buffer `buf` of level l, whose data is at time `time`
+struct VelFill {  // velocity ghosts of the second plane between the times ta and tb (FUSED sweeps on a fine level)
+  bool on = false;
+  double ta = 0, tb = 0;
+};
+
 template <typename T>
-GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, int wb = 1) {
+GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, int wb = 1, VelFill vf = VelFill()) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
   GhostArgs<T> a;
@@ -702,6 +708,17 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, 
     // with one state only: the blend returns one of the two buffers unchanged, so only that one is read
     if (bo == bn || alpha == 0.0) { bn = bo; a.single = 1; }
     else if (alpha == 1.0) { bo = bn; a.single = 1; }
+    if (vf.on) {  // both coarse states are needed whatever alpha is
+      const bool pair = C.have_pair && C.t_new != C.t_old;
+      bo = pair ? C.old : C.cur;
+      bn = C.cur;
+      a.single = 0;
+      a.vel = 1;
+      a.alpha_a = (T)(pair ? (vf.ta - C.t_old) / (C.t_new - C.t_old) : 0.0);
+      a.alpha_b = (T)(pair ? (vf.tb - C.t_old) / (C.t_new - C.t_old) : 0.0);
+      a.vel_scale = (T)(1.0 / (vf.tb - vf.ta));
+      a.vel_c = (T)(pair ? 1.0 / (C.t_new - C.t_old) : 0.0);
+    }
     a.c_old_psi = plane_ptr<T>(c, l - 1, bo, wa);
     a.c_new_psi = plane_ptr<T>(c, l - 1, bn, wa);
     a.c_old_pi = plane_ptr<T>(c, l - 1, bo, wb);
@@ -731,14 +748,17 @@ int fill_shell_copies(sledge_ctx* c, int l, int buf, bool with_pi) {
 
 template <typename T>
 int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool star_only = false, int wa = 0, int wb = 1,
-                  bool tag_only = false) {
-  GhostArgs<T> a = ghost_args<T>(c, l, buf, time, wa, wb);
-  if (tag_only && a.quartic == 0 && c->use_patches && !c->plan.lev[l].tag_patches.empty()) {
-    // the fill before K3: only the +1 neighbours of the plaquettes (every coordinate in [0, n], one of them = n)
+                  bool tag_only = false, VelFill vf = VelFill()) {
+  GhostArgs<T> a = ghost_args<T>(c, l, buf, time, wa, wb, vf);
+  // fills before a sweep (star_only) or before K3 (tag_only) go by rectangular patch; with quartic interpolation by
+  // coarse parent the patches move the copies only and k_fill_qparents the interpolated cells
+  const bool patchable = c->use_patches && (a.quartic == 0 || a.quartic == 2);
+  const bool tagp = tag_only && patchable && !c->plan.lev[l].tag_patches.empty();
+  if (tagp) {  // only the +1 neighbours of the plaquettes (every coordinate in [0, n], one of them = n)
     a.patches = tab<uint4>(c, c->plan.lev[l].off_tag_patches);
     a.n_patches = (unsigned)(c->plan.lev[l].tag_patches.size() / 2);
-    star_only = true;
   }
+  const bool by_patch = patchable && a.n_patches > 0 && (star_only || tagp);
   if (a.quartic == 2 && l > 0) {  // the coarse windows are read through the coarse boxes' ghost cells
     LevelHost& C = c->plan.lev[l - 1];
     const bool pair = C.have_pair && C.t_new != C.t_old;
@@ -746,7 +766,8 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     if (rc == SLEDGE_OK && pair) rc = fill_shell_copies<T>(c, l - 1, C.old, fill_pi);
     if (rc) return rc;
   }
-  if (star_only && a.quartic == 0 && a.n_patches > 0 && c->use_patches) {  // by rectangular region (k_fill_patches)
+  if (by_patch) {  // by rectangular region (k_fill_patches)
+    if (a.quartic == 2) a.copy_only = 1;
     const int pgrid = (int)((a.n_patches + PATCH_WARPS - 1) / PATCH_WARPS);
     const size_t smem = (size_t)PATCH_WARPS * a.patch_smem_pairs * (fill_pi ? 2 : 1) * sizeof(typename PairOf<T>::type);
     if (smem > 48 * 1024) {
@@ -761,7 +782,9 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     Timed t(c, KIND_GHOST);
     if (fill_pi) k_fill_patches<T, true><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
     else k_fill_patches<T, false><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
-    return check_launch(c, "k_fill_patches");
+    const int prc = check_launch(c, "k_fill_patches");
+    if (prc || a.quartic == 0) return prc;
+    a.copy_only = 0;
   }
   int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
   if (star_only) {  // before an RK sweep only the cells its star stencil reaches are needed: the packed list
@@ -771,7 +794,7 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     grid = (int)((a.n_entries + GHOST_THREADS * GHOST_EPT - 1) / (GHOST_THREADS * GHOST_EPT));
   }
   if (grid == 0 && !(a.quartic == 2 && l > 0)) return SLEDGE_OK;
-  if (grid > 0) {
+  if (grid > 0 && !by_patch) {  // (with by_patch the copies are done and only the parents kernel below is left)
     Timed t(c, KIND_GHOST);
     if (a.quartic == 1 && l > 0) {
       if (fill_pi) k_fill_ghosts<T, true, true><<<grid, GHOST_THREADS, 0, c->stream>>>(a);
@@ -1017,6 +1040,13 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
     return tma ? (const void*)(tab<CUtensorMap>(c, L.off_tmaps) + (size_t)((buf & 3) * 2 + which) * L.boxdev.size()) : nullptr;
   };
   auto ensure_ghosts = [&](int buf, double time) -> int {
+    if (l > 0) {  // fine level: Pi ghosts of interpolated cells carry the psi of the sweep's later stage (t + dt/2 or t + dt)
+      VelFill vf;
+      vf.on = true;
+      vf.ta = t;
+      vf.tb = pass == 0 ? t + 0.5 * dt : t + dt;
+      return launch_ghosts<T>(c, l, buf, time, true, true, 0, 1, false, vf);
+    }
     if (!wrap) return launch_ghosts<T>(c, l, buf, time, true, true);
     if (!tma || L.star_ok[buf & 3]) return SLEDGE_OK;
     L.star_ok[buf & 3] = true;
@@ -1060,7 +1090,11 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
 // With Kreiss-Oliger dissipation k_psi = Pi + Q psi is no longer pointwise: every level runs the staged sweeps.
 inline bool is_ssprk3(const sledge_params& p) { return p.integrator == 3 || p.integrator == 10; }
 inline bool level_is_fused(const Plan& P, int l) {
-  return P.p.rk_dataflow == SLEDGE_RK_FUSED && l == 0 && !ko_on(P.p) && !is_ssprk3(P.p) && !is_rkn(P.p) && !P.p.gw;
+  // level 0: its ghosts are copies of valid cells.  Finer levels: the ghosts a sweep forms for the NEXT stage must be
+  // the coarse state interpolated at that stage's time (L72), which the patch fills provide as "velocity" ghosts of
+  // Pi (k_ghost.cuh: k_fill_patches for trilinear, k_fill_qparents for quartic interpolation by coarse parent)
+  const bool lev_ok = l == 0 || (P.fine_fused && (P.p.interp == SLEDGE_INTERP_TRILINEAR || quartic_by_parent(P.p)) && !P.lev[l].patches.empty());
+  return P.p.rk_dataflow == SLEDGE_RK_FUSED && lev_ok && !ko_on(P.p) && !is_ssprk3(P.p) && !is_rkn(P.p) && !P.p.gw;
 }
 
 // One SSPRK3 stage (integrator.type 3 / 10, L808; Shu-Osher form) of level l, s = 0, 1, 2:
@@ -1449,6 +1483,8 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     c->use_tma = !(ev && ev[0] == '0');
     const char* ep = getenv("SLEDGE_K2_PATCHES");
     c->use_patches = !(ep && ep[0] == '0');
+    const char* ef = getenv("SLEDGE_FINE_FUSED");
+    P.fine_fused = c->use_patches && c->use_tma && !(ef && ef[0] == '0');
   }
   for (int l = 0; l < P.p.n_levels && c->use_tma; ++l)
     if (level_is_fused(P, l) && (rc = make_tensor_maps(c, l)) != SLEDGE_OK) {
@@ -1691,6 +1727,30 @@ int sledge_shadow_tee(sledge_ctx* c, double dt, double eta, const double* eps4, 
 }
 
 int64_t sledge_launch_count(const sledge_ctx* c) { return c ? c->launches : 0; }
+
+int sledge_level_dataflow(const sledge_ctx* c, int level, int* k1_launches_per_step, int* words_per_cell_step) {
+  if (!c || level < 0 || level >= c->plan.p.n_levels) return SLEDGE_EINVAL;
+  const Plan& P = c->plan;
+  int n = 4, w = P.p.rk_dataflow == SLEDGE_RK_CLASSIC && !P.p.gw ? 64 : 52;
+  if (is_ssprk3(P.p)) {
+    n = 3;
+    w = 32;
+  } else if (is_rkn(P.p)) {  // stage i: Psi_i (psi_n itself for i = 0), psi_n, Pi_n, f_0..f_{i-1} in; two planes out
+    n = P.p.rkn_stages;
+    w = 0;
+    for (int i = 0; i < n; ++i) w += (i ? 2 : 0) + 4 + 2 * i + 4;
+  } else if (level_is_fused(P, level)) {
+    n = 2;
+    w = 20;
+  }
+  if (P.p.gw) {  // psi + U (u, du) in, 12 out, plus Y in stages 2-3 and Y, U2, U3 in stage 4
+    n += 4;
+    w += (14 + 12) + 2 * (26 + 12) + (50 + 12);
+  }
+  if (k1_launches_per_step) *k1_launches_per_step = n;
+  if (words_per_cell_step) *words_per_cell_step = w;
+  return SLEDGE_OK;
+}
 
 int sledge_synchronize(sledge_ctx* c) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");

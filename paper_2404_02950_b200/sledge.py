@@ -24,7 +24,7 @@ SYMBOLS = [
     "sledge_arena_bytes", "sledge_create", "sledge_destroy", "sledge_set_state", "sledge_get_state",
     "sledge_set_state_host", "sledge_get_state_host", "sledge_get_ghosted", "sledge_fill_ghosts",
     "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable",
-    "sledge_shadow_tee", "sledge_level_cells",
+    "sledge_shadow_tee", "sledge_level_cells", "sledge_level_dataflow",
     "sledge_launch_count", "sledge_synchronize", "sledge_profile_enable", "sledge_profile_read",
     "sledge_last_error",
 ]
@@ -77,6 +77,7 @@ def lib():
         L.sledge_tee_enable.argtypes = [vp, i, C.POINTER(C.c_double), vp, vp]
         L.sledge_shadow_tee.argtypes = [vp, d, d, C.POINTER(C.c_double), vp, vp]
         L.sledge_level_cells.argtypes = [vp, i, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.sledge_level_dataflow.argtypes = [vp, i, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.sledge_launch_count.argtypes = [vp]
         L.sledge_launch_count.restype = C.c_int64
         L.sledge_synchronize.argtypes = [vp]
@@ -211,6 +212,12 @@ class Sledge:
         v, b = C.c_int64(0), C.c_int64(0)
         self._chk(lib().sledge_level_cells(self._h, level, C.byref(v), C.byref(b)), "sledge_level_cells")
         return int(v.value), int(b.value)
+
+    def level_dataflow(self, level):
+        """(K1 launches per step of the level, algorithmic words per cell-step of those launches)"""
+        n, w = C.c_int(0), C.c_int(0)
+        self._chk(lib().sledge_level_dataflow(self._h, level, C.byref(n), C.byref(w)), "sledge_level_dataflow")
+        return int(n.value), int(w.value)
 
     def count_shape(self, level):
         return tuple((self.n0[d] * (1 << level) + COUNT_BLOCK - 1) // COUNT_BLOCK for d in (2, 1, 0))
