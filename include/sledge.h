@@ -62,8 +62,9 @@ typedef struct {
   int32_t dtype;           /* SLEDGE_F32 / SLEDGE_F64: storage AND arithmetic type                */
   int32_t lap_order;       /* paper's `order` (L649): 1 = 7-, 2 = 13-, 3 = 19-point Laplacian      */
   int32_t eta_fixed;       /* 1 = Minkowski test variant: eta_s = eta for every stage (R3)         */
-  int32_t rk_dataflow;     /* words moved per cell-step (R5): SLEDGE_RK_FUSED 20 (two stages per sweep on
-                              level 0, LEAN on finer levels), SLEDGE_RK_LEAN 52, SLEDGE_RK_CLASSIC 64   */
+  int32_t rk_dataflow;     /* words moved per cell-step (R5): SLEDGE_RK_FUSED 20 (two stages per sweep, on every
+                              level; a level falls back to LEAN only with quartic interpolation and nghost = 1),
+                              SLEDGE_RK_LEAN 52, SLEDGE_RK_CLASSIC 64; sledge_level_dataflow tells what runs  */
   double h0;               /* level-0 spacing, Eq.1                                               */
   double lambda;           /* Eq.11 generalised (R2): k_Pi = -(friction/eta) Pi + Lap psi          */
   double a_mass;           /*        - lambda eta^2 psi (psi1^2+psi2^2-1) - a_mass psi             */
@@ -130,7 +131,10 @@ int sledge_set_state_host(sledge_ctx* ctx, int box, int comp, const void* host_s
 int sledge_get_state_host(sledge_ctx* ctx, int box, int comp, void* host_dst);
 /* One component of one box INCLUDING ghosts: (nx+2g)*(ny+2g)*(nz+2g) reals, x fastest.  Ghost values are those of
  * the last fill that touched them: sledge_fill_ghosts fills every ghost cell of all four components; the fills
- * inside a step move psi only unless Pi is differenced (FUSED sweeps, Kreiss-Oliger term), R10. */
+ * inside a step move psi only unless Pi is differenced (FUSED sweeps, Kreiss-Oliger term), R10; before a FUSED sweep
+ * of a level > 0 the Pi ghost cells that are interpolated from the coarse level do NOT hold Pi but the finite
+ * difference in time of the interpolated coarse psi between the sweep's two stage times (what the sweep needs to form
+ * the later stage's psi there, L72), so after a step only sledge_fill_ghosts makes the ghost contents meaningful. */
 int sledge_get_ghosted(sledge_ctx* ctx, int box, int comp, void* dev_dst);
 
 /* Ghost fill of the CURRENT state of `level` (L68-74): every psi ghost cell <- the valid cell of the

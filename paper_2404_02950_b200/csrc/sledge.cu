@@ -864,6 +864,14 @@ int make_tensor_maps(sledge_ctx* c, int l) {
   const int cpt = P.p.dtype == SLEDGE_F64 ? 1 : 2;
   const int xo = (R + cpt - 1) / cpt * cpt;
   const cuuint32_t sw = (cuuint32_t)(K1F_TX * cpt + 2 * xo), sh = (cuuint32_t)(K1F_TY + 2 * R);
+  // L2 promotion of the tile loads: 64 bytes (measured: C5's 32^3 boxes 6.15 -> 5.70 ms of K1 per coarse step against
+  // 128 bytes, C3 unchanged); SLEDGE_TMA_L2PROMO = 0 / 128 / 256 selects another size
+  CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
+  if (const char* ev = getenv("SLEDGE_TMA_L2PROMO")) {
+    const int v = atoi(ev);
+    promo = v == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : (v == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+            : (v == 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B));
+  }
   const size_t nb = L.boxdev.size();
   L.tmaps_host.assign(nb * NBUF * 2, CUtensorMap());
   for (int buf = 0; buf < NBUF; ++buf)
@@ -878,7 +886,7 @@ int make_tensor_maps(sledge_ctx* c, int l) {
         const CUresult r = encode(&L.tmaps_host[(size_t)(buf * 2 + which) * nb + q],
                                   P.p.dtype == SLEDGE_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
                                   base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                  promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(c, SLEDGE_ECUDA, "cuTensorMapEncodeTiled failed (%d) for box %zu of level %d", (int)r, q, l);
       }
   L.has_tmaps = true;

@@ -206,3 +206,50 @@ def test_shadow_level_tags_of_level0(flow, nlev):
     _, s2 = P.make_pair(n0, **kw)
     with pytest.raises(Exception):
         s2.shadow_tee(dt, eta, 1.0, 1.0)
+
+
+# ---- bookkeeping: which data-flow a level runs ---------------------------------------------------------------
+
+def test_level_dataflow_reports_launches_and_words():
+    from paper_2404_02950_b200.sledge import Sledge
+    n0 = 32
+    boxes = _ring_hierarchy(n0)
+    kw = dict(boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5)
+    s = Sledge(n0, rk_dataflow="fused", **kw)
+    assert [s.level_dataflow(l) for l in range(3)] == [(2, 20)] * 3      # FUSED on every level (velocity ghosts)
+    s = Sledge(n0, rk_dataflow="fused", interp=4, **kw)
+    assert [s.level_dataflow(l) for l in range(3)] == [(2, 20)] * 3      # quartic by coarse parent
+    s = Sledge(n0, rk_dataflow="lean", **kw)
+    assert s.level_dataflow(1) == (4, 52)
+    s = Sledge(n0, rk_dataflow="classic", **kw)
+    assert s.level_dataflow(2) == (4, 64)
+    s = Sledge(n0, rk_dataflow="fused", integrator=10, **kw)
+    assert s.level_dataflow(0) == (3, 32)
+    s = Sledge(n0, rk_dataflow="fused", integrator=20, rkn=RKN4, **kw)
+    assert s.level_dataflow(0) == (3, 8 + 12 + 14)
+    s = Sledge(n0, rk_dataflow="fused", gw=True, **kw)
+    assert s.level_dataflow(1) == (8, 52 + 164)
+    s = Sledge(n0, rk_dataflow="fused", ko_order=2, ko_strength=0.01, **kw)
+    assert s.level_dataflow(0) == (4, 52)
+
+
+def test_fused_on_fine_levels_matches_the_oracle_with_moving_coarse_data():
+    """The velocity ghosts (K2) must make the two-stage sweeps of a fine level see the coarse state at t + dt/2 and
+    t + dt: a hierarchy with large coarse time derivatives (Pi of order 1), five coarse steps, friction and mass on."""
+    P = _pair()
+    n0 = 32
+    boxes = _ring_hierarchy(n0)
+    for interp in (0, 4):
+        o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5, lam=0.7, a_mass=0.3,
+                           friction=2.0, rk_dataflow="fused", interp=interp)
+        assert s.level_dataflow(2) == (2, 20)
+        P.init_smooth(o, s, n0, 13, amp=0.8)
+        for l in (2, 1):
+            o.average_down(l)
+            s.average_down(l)
+        eta, dt = 1.5, 0.1
+        for _ in range(5):
+            o.rk_step(dt, eta)
+            s.rk_step(dt, eta)
+            eta += dt
+        assert P.max_err(o, s) <= F64_TOL
