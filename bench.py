@@ -72,7 +72,7 @@ def parse():
     ap.add_argument("--no-others", action="store_true",
                     help="skip the short runs of the other BASELINE.json workloads (key other_workloads) and the C5 graph leg")
     ap.add_argument("--other-steps", type=int, default=4)
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=4)
     return ap.parse_args()
 
 
@@ -682,6 +682,7 @@ def e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags):
     e0.record()
     for _ in range(args.e2e_steps):
         one()
+    s.host_copies_join()  # the context stream waits for the last downloads: e1 includes them
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / args.e2e_steps

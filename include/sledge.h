@@ -125,10 +125,17 @@ int sledge_destroy(sledge_ctx* ctx);
  * level's (old,new) pair used for temporal ghost interpolation. */
 int sledge_set_state(sledge_ctx* ctx, int box, int comp, const void* dev_src);
 int sledge_get_state(sledge_ctx* ctx, int box, int comp, void* dev_dst);
-/* Same with HOST buffers: the library stages through a device scratch inside the arena
- * (cudaMemcpyAsync on the context stream; truly asynchronous only for pinned memory). */
+/* Same with HOST buffers (pinned memory for truly asynchronous copies).  The library stages through slots inside
+ * the arena, two per direction, and runs the host<->device copies on two streams of its own, ordered against the
+ * context stream with events: the upload of component c+1 overlaps the repacking kernel of c, downloads drain while
+ * the context stream goes on, and the downloads of one step overlap the uploads of the next (PCIe is full duplex).
+ * Ordering seen by the caller is that of the context stream: a set is complete for every later call on the context;
+ * a get has delivered its data after sledge_synchronize, or once work enqueued after sledge_host_copies_join runs. */
 int sledge_set_state_host(sledge_ctx* ctx, int box, int comp, const void* host_src);
 int sledge_get_state_host(sledge_ctx* ctx, int box, int comp, void* host_dst);
+/* Make the context stream wait for every host copy enqueued so far (e.g. before recording an event that should
+ * include the downloads). */
+int sledge_host_copies_join(sledge_ctx* ctx);
 /* One component of one box INCLUDING ghosts: (nx+2g)*(ny+2g)*(nz+2g) reals, x fastest.  Ghost values are those of
  * the last fill that touched them: sledge_fill_ghosts fills every ghost cell of all four components; the fills
  * inside a step move psi only unless Pi is differenced (FUSED sweeps, Kreiss-Oliger term), R10; before a FUSED sweep

@@ -188,6 +188,13 @@ struct sledge_ctx {
   bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
   bool use_patches = true;  // fills before an RK sweep by region (SLEDGE_K2_PATCHES=0 selects the packed per-cell list)
   sledge_ctx* shadow = nullptr;  // the shadow level's context (shadow_level = 1)
+  // host-buffer copies (sledge_set_state_host / get_state_host) run on two streams of their own, double-buffered through
+  // the staging slots, so that uploads, repacking kernels and downloads overlap (PCIe is full duplex)
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+  cudaEvent_t ev_in_ready[2] = {nullptr, nullptr}, ev_in_free[2] = {nullptr, nullptr};
+  cudaEvent_t ev_out_ready[2] = {nullptr, nullptr}, ev_out_free[2] = {nullptr, nullptr};
+  bool in_used[2] = {false, false}, out_used[2] = {false, false};
+  unsigned n_in = 0, n_out = 0;
   int device = 0;  // the device the arena lives on: every entry point runs with it current (DeviceGuard)
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
   size_t ev_used[4] = {0, 0, 0, 0};
@@ -566,7 +573,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       if (L.n[d] + 2 * g >= 65536) return fail(nullptr, SLEDGE_EINVAL, "level %d: more than 65535 cells per axis", l);
   }
   P.scratch_bytes = max_box_cells * P.esz;
-  P.off_scratch = take(P.scratch_bytes);
+  P.off_scratch = take(P.scratch_bytes * 4);  // host copies: two staging slots per direction (in 0, 1; out 2, 3)
   P.off_err = take(sizeof(int));
   if (p.shadow_level) {  // L98: level 0 coarsened by 2, ONE box over the same periodic domain
     sledge_params sp = p;
@@ -1561,6 +1568,18 @@ int sledge_destroy(sledge_ctx* c) {
   DeviceGuard guard(c->device);
   if (c->shadow) sledge_destroy(c->shadow);
   cudaStreamSynchronize(c->stream);
+  if (c->s_h2d) {
+    cudaStreamSynchronize(c->s_h2d);
+    cudaStreamSynchronize(c->s_d2h);
+    for (int k = 0; k < 2; ++k) {
+      cudaEventDestroy(c->ev_in_ready[k]);
+      cudaEventDestroy(c->ev_in_free[k]);
+      cudaEventDestroy(c->ev_out_ready[k]);
+      cudaEventDestroy(c->ev_out_free[k]);
+    }
+    cudaStreamDestroy(c->s_h2d);
+    cudaStreamDestroy(c->s_d2h);
+  }
   for (auto& v : c->ev)
     for (auto& pr : v) {
       cudaEventDestroy(pr.first);
@@ -1609,25 +1628,71 @@ static size_t box_valid_bytes(sledge_ctx* c, int box) {
   return (size_t)(B.hi[0] - B.lo[0] + 1) * (B.hi[1] - B.lo[1] + 1) * (B.hi[2] - B.lo[2] + 1) * c->plan.esz;
 }
 
+static int host_streams(sledge_ctx* c) {
+  if (c->s_h2d) return SLEDGE_OK;
+  cudaError_t e = cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking);
+  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+    e = cudaEventCreateWithFlags(&c->ev_in_ready[k], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_in_free[k], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_out_ready[k], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_out_free[k], cudaEventDisableTiming);
+  }
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "host copy streams: %s", cudaGetErrorString(e));
+  return SLEDGE_OK;
+}
+
 int sledge_set_state_host(sledge_ctx* c, int box, int comp, const void* host_src) {
   int rc = check_box_comp(c, box, comp, host_src);
   if (rc) return rc;
   DeviceGuard guard(c->device);
-  void* scratch = c->arena + c->plan.off_scratch;
-  const cudaError_t e = cudaMemcpyAsync(scratch, host_src, box_valid_bytes(c, box), cudaMemcpyHostToDevice, c->stream);
+  if ((rc = host_streams(c)) != SLEDGE_OK) return rc;
+  const int k = (int)(c->n_in++ & 1u);
+  void* slot = c->arena + c->plan.off_scratch + (size_t)k * c->plan.scratch_bytes;
+  cudaError_t e = cudaSuccess;
+  if (c->in_used[k]) e = cudaStreamWaitEvent(c->s_h2d, c->ev_in_free[k], 0);  // the slot's last repack has read it
+  if (e == cudaSuccess) e = cudaMemcpyAsync(slot, host_src, box_valid_bytes(c, box), cudaMemcpyHostToDevice, c->s_h2d);
+  if (e == cudaSuccess) e = cudaEventRecord(c->ev_in_ready[k], c->s_h2d);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(c->stream, c->ev_in_ready[k], 0);
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "set_state_host: %s", cudaGetErrorString(e));
-  return sledge_set_state(c, box, comp, scratch);
+  rc = sledge_set_state(c, box, comp, slot);
+  if (rc) return rc;
+  c->in_used[k] = true;
+  e = cudaEventRecord(c->ev_in_free[k], c->stream);
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "set_state_host: %s", cudaGetErrorString(e));
+  return SLEDGE_OK;
 }
 
 int sledge_get_state_host(sledge_ctx* c, int box, int comp, void* host_dst) {
   int rc = check_box_comp(c, box, comp, host_dst);
   if (rc) return rc;
   DeviceGuard guard(c->device);
-  void* scratch = c->arena + c->plan.off_scratch;
-  rc = sledge_get_state(c, box, comp, scratch);
-  if (rc) return rc;
-  const cudaError_t e = cudaMemcpyAsync(host_dst, scratch, box_valid_bytes(c, box), cudaMemcpyDeviceToHost, c->stream);
+  if ((rc = host_streams(c)) != SLEDGE_OK) return rc;
+  const int k = (int)(c->n_out++ & 1u);
+  void* slot = c->arena + c->plan.off_scratch + (size_t)(2 + k) * c->plan.scratch_bytes;
+  cudaError_t e = cudaSuccess;
+  if (c->out_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_out_free[k], 0);  // the slot's last download is done
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "get_state_host: %s", cudaGetErrorString(e));
+  rc = sledge_get_state(c, box, comp, slot);
+  if (rc) return rc;
+  e = cudaEventRecord(c->ev_out_ready[k], c->stream);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(c->s_d2h, c->ev_out_ready[k], 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(host_dst, slot, box_valid_bytes(c, box), cudaMemcpyDeviceToHost, c->s_d2h);
+  if (e == cudaSuccess) e = cudaEventRecord(c->ev_out_free[k], c->s_d2h);
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "get_state_host: %s", cudaGetErrorString(e));
+  c->out_used[k] = true;
+  return SLEDGE_OK;
+}
+
+int sledge_host_copies_join(sledge_ctx* c) {
+  if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
+  DeviceGuard guard(c->device);
+  cudaError_t e = cudaSuccess;
+  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+    if (c->out_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_out_free[k], 0);
+    if (e == cudaSuccess && c->in_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_in_free[k], 0);
+  }
+  if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "host_copies_join: %s", cudaGetErrorString(e));
   return SLEDGE_OK;
 }
 
@@ -1764,6 +1829,8 @@ int sledge_synchronize(sledge_ctx* c) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
   DeviceGuard guard(c->device);
   cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e == cudaSuccess && c->s_d2h) e = cudaStreamSynchronize(c->s_d2h);
+  if (e == cudaSuccess && c->s_h2d) e = cudaStreamSynchronize(c->s_h2d);
   int flag = 0;
   if (e == cudaSuccess) e = cudaMemcpy(&flag, c->arena + c->plan.off_err, sizeof(int), cudaMemcpyDeviceToHost);
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "synchronize: %s", cudaGetErrorString(e));

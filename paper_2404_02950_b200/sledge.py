@@ -22,7 +22,7 @@ COUNT_BLOCK = 32
 
 SYMBOLS = [
     "sledge_arena_bytes", "sledge_create", "sledge_destroy", "sledge_set_state", "sledge_get_state",
-    "sledge_set_state_host", "sledge_get_state_host", "sledge_get_ghosted", "sledge_fill_ghosts",
+    "sledge_set_state_host", "sledge_get_state_host", "sledge_host_copies_join", "sledge_get_ghosted", "sledge_fill_ghosts",
     "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable",
     "sledge_shadow_tee", "sledge_level_cells", "sledge_level_dataflow",
     "sledge_launch_count", "sledge_synchronize", "sledge_profile_enable", "sledge_profile_read",
@@ -69,6 +69,7 @@ def lib():
         for name in ("sledge_set_state", "sledge_get_state", "sledge_set_state_host", "sledge_get_state_host",
                      "sledge_get_ghosted"):
             getattr(L, name).argtypes = [vp, i, i, vp]
+        L.sledge_host_copies_join.argtypes = [vp]
         L.sledge_fill_ghosts.argtypes = [vp, i, d]
         L.sledge_rk_stage.argtypes = [vp, i, i, d, d]
         L.sledge_rk_step.argtypes = [vp, d, d]
@@ -241,6 +242,9 @@ class Sledge:
         assert tuple(out.shape) == self.box_shape(ib)
         self._chk(lib().sledge_get_state_host(self._h, ib, comp, out.data_ptr()), "sledge_get_state_host")
         return out
+
+    def host_copies_join(self):
+        self._chk(lib().sledge_host_copies_join(self._h), "sledge_host_copies_join")
 
     def get_ghosted(self, ib, comp) -> torch.Tensor:
         out = torch.empty(self.box_shape(ib, ghosts=True), dtype=self.tdtype, device=self.device)

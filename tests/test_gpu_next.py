@@ -253,3 +253,55 @@ def test_fused_on_fine_levels_matches_the_oracle_with_moving_coarse_data():
             s.rk_step(dt, eta)
             eta += dt
         assert P.max_err(o, s) <= F64_TOL
+
+
+def test_fused_on_fine_levels_fp32():
+    P = _pair()
+    n0 = 32
+    boxes = _ring_hierarchy(n0)
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5, lam=1.0, rk_dataflow="fused", dtype="f32")
+    assert s.level_dataflow(1) == (2, 20)
+    P.init_smooth(o, s, n0, 14, amp=0.8)
+    for l in (2, 1):
+        o.average_down(l)
+        s.average_down(l)
+    eta, dt = 1.5, 0.1
+    for _ in range(4):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s, relative=True) <= F32_TOL
+
+
+def test_host_buffer_copies_are_pipelined_but_ordered():
+    """sledge_set_state_host / sledge_get_state_host run on the library's own copy streams through two staging slots
+    per direction: many back-to-back copies of different boxes and components, a step in between, and a second round
+    that overwrites the first must behave exactly like the device-buffer calls."""
+    from paper_2404_02950_b200.sledge import Sledge
+    n0 = (40, 24, 72)
+    boxes = _ragged_boxes()
+    kw = dict(boxes=boxes, nghost=2, lap_order=2, h0=0.5, lam=1.0, rk_dataflow="fused")
+    a, b = Sledge(n0, **kw), Sledge(n0, **kw)
+    rng = np.random.default_rng(5)
+    for rnd in range(2):
+        host = {}
+        for ib in range(len(boxes)):
+            for c in range(4):
+                t = torch.from_numpy(rng.normal(size=a.box_shape(ib)) * (0.5 if c < 2 else 0.1)).pin_memory()
+                host[(ib, c)] = t
+                a.set_state_host(ib, c, t)
+                b.set_state(ib, c, t.cuda())
+        a.rk_step(0.05, 1.0)
+        b.rk_step(0.05, 1.0)
+        outs = {k: torch.empty_like(v).pin_memory() for k, v in host.items()}
+        for (ib, c), o in outs.items():
+            a.get_state_host(ib, c, o)
+        a.synchronize()
+        for (ib, c), o in outs.items():
+            assert torch.equal(o, b.get_state(ib, c).cpu()), (rnd, ib, c)
+    # join: work enqueued on the context stream afterwards sees the downloads done
+    o2 = torch.empty(a.box_shape(0), dtype=torch.float64).pin_memory()
+    a.get_state_host(0, 0, o2)
+    a.host_copies_join()
+    torch.cuda.current_stream().synchronize()
+    assert torch.equal(o2, b.get_state(0, 0).cpu())
