@@ -22,7 +22,10 @@
 
 namespace sledge {
 
-constexpr int GW_TX = 32, GW_TY = 8;
+#ifndef SLEDGE_GW_TY
+#define SLEDGE_GW_TY 8
+#endif
+constexpr int GW_TX = 32, GW_TY = SLEDGE_GW_TY;  // = the fused-sweep tile (sledge.cu asserts it)
 
 template <typename T>
 struct GwArgs {
