@@ -27,9 +27,22 @@
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only)
 
+#include <utility>
+
 #include "k_rk_plane.cuh"
 
 namespace sledge {
+
+// f(integral_constant<int, 0>) ... f(integral_constant<int, N-1>): a loop whose index is a compile-time constant in
+// the body (the register z-windows rotate through their slots instead of being shifted)
+template <class F, int... I>
+__device__ __forceinline__ void static_for_impl(F&& f, std::integer_sequence<int, I...>) {
+  (f(std::integral_constant<int, I>{}), ...);
+}
+template <int N, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+  static_for_impl(f, std::make_integer_sequence<int, N>{});
+}
 
 __device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
@@ -158,14 +171,17 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
     cp_async_commit();
   }
   // lower 2R planes of the z-windows straight into registers
-  V w[NF][RY][2 * R + 1];  // w[f][j][m] = field f, row j, plane z + m - R
+  // The window ROTATES: in the iteration with zz % W == u the value of plane z + m - R sits in w[f][j][(m + u) % W]
+  // (W = 2R + 1), so that nothing is moved from one iteration to the next; the z loop is unrolled W times for it.
+  constexpr int W = 2 * R + 1;
+  V w[NF][RY][W];
 #pragma unroll
   for (int f = 0; f < NF; ++f)
 #pragma unroll
     for (int j = 0; j < RY; ++j)
 #pragma unroll
       for (int m = 0; m < 2 * R; ++m)
-        if (active[j]) w[f][j][m + 1] = ldg16_keep<T>(a.sten[f] + off + (long long)j * b.sx + (long long)(m - R) * plane);
+        if (active[j]) w[f][j][m] = ldg16_keep<T>(a.sten[f] + off + (long long)j * b.sx + (long long)(m - R) * plane);
 #pragma unroll
   for (int p = 0; p < R; ++p) mbar_wait(full + p, 0);
 
@@ -188,7 +204,8 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
   int slot_t = R % S;         // slot of plane zz + R
   int slot_n = (R + PD) % S;  // slot of plane zz + R + PD
   unsigned par_t = 0;         // parity of the phase that completes plane zz + R in slot_t
-  for (int zz = 0; zz < t.nz; ++zz) {
+  auto step = [&](const int zz, auto uc) {
+    constexpr int u = decltype(uc)::value;  // zz % W
     mbar_wait(full + slot_t, par_t);  // plane zz + R has landed
     cp_async_wait<PD - 1>();          // this thread's pointwise inputs of plane zz
     __syncthreads();                  // plane zz-1 is retired
@@ -199,9 +216,7 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
     for (int f = 0; f < NF; ++f)
 #pragma unroll
       for (int j = 0; j < RY; ++j) {
-#pragma unroll
-        for (int m = 0; m < 2 * R; ++m) w[f][j][m] = w[f][j][m + 1];
-        w[f][j][2 * R] = *reinterpret_cast<const V*>(tb + f * PSZ + s_own + j * SW);
+        w[f][j][(2 * R + u) % W] = *reinterpret_cast<const V*>(tb + f * PSZ + s_own + j * SW);
       }
     if (NP > 0) {
       const V* const o = pring + (size_t)(zz % PD) * NP * RY * NT + tid;
@@ -229,7 +244,7 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
           P col[RY + 2 * R];
 #pragma unroll
           for (int i = 0; i < RY + 2 * R; ++i) {
-            if (i >= R && i < R + RY) col[i] = w[f][i - R][R].p[p];
+            if (i >= R && i < R + RY) col[i] = w[f][i - R][(R + u) % W].p[p];
             else col[i] = s[(i - R) * SW];
           }
 #pragma unroll
@@ -250,10 +265,10 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
                 xp[r - 1] = comp(xn[2 * (r - 1) + 1]);
                 ym[r - 1] = comp(col[j + R - r]);
                 yp[r - 1] = comp(col[j + R + r]);
-                zm[r - 1] = comp(w[f][j][R - r].p[p]);
-                zp[r - 1] = comp(w[f][j][R + r].p[p]);
+                zm[r - 1] = comp(w[f][j][(R - r + u) % W].p[p]);
+                zp[r - 1] = comp(w[f][j][(R + r + u) % W].p[p]);
               }
-              lap[j][f][c] = lap_from<T, ORDER>(comp(w[f][j][R].p[p]), xm, xp, ym, yp, zm, zp, a.inv_h2);
+              lap[j][f][c] = lap_from<T, ORDER>(comp(w[f][j][(R + u) % W].p[p]), xm, xp, ym, yp, zm, zp, a.inv_h2);
             }
           }
         }
@@ -261,7 +276,7 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
         for (int j = 0; j < RY; ++j) {
           P wc[NF], pc[NPA], opsi[NOUT], opi[NOUT];
 #pragma unroll
-          for (int f = 0; f < NF; ++f) wc[f] = w[f][j][R].p[p];
+          for (int f = 0; f < NF; ++f) wc[f] = w[f][j][(R + u) % W].p[p];
 #pragma unroll
           for (int q = 0; q < NPA; ++q) pc[q] = pv[j][q].p[p];
           rk_cell<T, MODE>(a, lap[j], wc, pc, opsi, opi);
@@ -322,7 +337,11 @@ __global__ void __launch_bounds__(TX* TY / RY, MINB) k_rk_tma(const PipeArgs<T> 
       ++slot_t;
     }
     slot_n = slot_n + 1 == S ? 0 : slot_n + 1;
-  }
+  };
+  for (int zz0 = 0; zz0 < t.nz; zz0 += W)
+    static_for<W>([&](auto uc) {
+      if (zz0 + decltype(uc)::value < t.nz) step(zz0 + decltype(uc)::value, uc);  // uniform over the CTA
+    });
 }
 
 }  // namespace sledge
