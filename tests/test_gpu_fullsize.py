@@ -305,3 +305,46 @@ def test_c3_real_untiled_initial_data_two_steps():
         pytest.skip(f"the oracle needs ~{need:.0f} GB of host RAM for 512^3 in 64^3 boxes; {_host_ram_free_gb():.0f} GB free")
     cfg = inputs.CONFIGS["C3"]
     _untiled(cfg.n0, 64, "fused", 2, cfg.grf_f, cfg.seeds, cfg)
+
+
+# ---- round-2 rows at bench size: the workloads bench.py --gw / --integrator 20 time --------------------------------
+
+def _tiled_extra(n_full, period, steps, **kw):
+    """C2-sized periodic box, period-`period` seeded data (every component), GPU against the tiled oracle run."""
+    from oracle.oracle import Oracle
+    from paper_2404_02950_b200.sledge import Sledge
+    cfg = inputs.CONFIGS["C2"]
+    reps = n_full // period
+    okw = dict(nghost=2, lap_order=2, h0=cfg.h0, lam=cfg.lam)
+    o = Oracle(period, **okw, **kw)
+    s = Sledge(n_full, rk_dataflow="fused", **okw, **kw)
+    ncomp = 16 if kw.get("gw") else 4
+    for c in range(ncomp):
+        amp = 1.0 if c < 2 else 0.1
+        small = amp * inputs.grf(period, 0.2, 7000 + c).to(torch.float64)
+        o.set_state(0, c, small.numpy())
+        s.set_state(0, c, inputs.tile_periodic(small.cuda(), reps).contiguous())
+    eta = cfg.eta0
+    for _ in range(steps):
+        o.rk_step(cfg.dt, eta)
+        s.rk_step(cfg.dt, eta)
+        eta += cfg.dt
+    s.synchronize()
+    worst = 0.0
+    for c in range(ncomp):
+        ref = torch.from_numpy(o.get_state(0, c)).cuda()
+        got = s.get_state(0, c)
+        worst = max(worst, float((got.view(reps, period, reps, period, reps, period) - ref[None, :, None, :, None, :]).abs().max()))
+        del got, ref
+    s.close()
+    return worst
+
+
+def test_gw_256cubed_all_16_components():
+    assert _tiled_extra(256, 64, 5, gw=True, gw_coupling=1.0, gw_friction=2.0) <= F64_TOL
+
+
+def test_rkn_256cubed_nystrom4():
+    rkn4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_b=[1 / 6, 1 / 3, 0.0],
+                tableau=[0.0, 1 / 8, 0.0, 0.0, 0.5, 0.0])
+    assert _tiled_extra(256, 64, 20, integrator=20, rkn=rkn4) <= F64_TOL
