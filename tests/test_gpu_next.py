@@ -305,3 +305,63 @@ def test_host_buffer_copies_are_pipelined_but_ordered():
     a.host_copies_join()
     torch.cuda.current_stream().synchronize()
     assert torch.equal(o2, b.get_state(0, 0).cpu())
+
+
+# ---- patches and velocity ghosts on other shapes: small blocking factors, non-cubic domains ------------------------
+
+@pytest.mark.parametrize("bf,g,order", [(4, 2, 2), (4, 3, 3), (2, 1, 1), (8, 3, 2)])
+@pytest.mark.parametrize("interp", [0, 4])
+def test_fused_multilevel_small_blocking_factors_and_noncubic_domain(bf, g, order, interp):
+    """Level 1 made of boxes of different shapes on a 24 x 16 x 32 periodic domain, level 2 inside it; the fills before
+    the sweeps go by patch (bf x bf x R pieces), the sweeps are FUSED on every level where the library allows it."""
+    P = _pair()
+    if interp == 4 and (g + 1) // 2 + 2 > bf // 2:
+        pytest.skip("quartic window leaves the nesting gap for this blocking factor (L70)")
+    n0 = (24, 16, 32)
+    m = max(bf, 4)  # fine boxes are multiples of 2 bf so that level 2 can nest with a gap of one blocking factor
+    boxes = [(0, (0, 0, 0), (n0[0] - 1, n0[1] - 1, n0[2] - 1))]
+    # level 1 (index space 48 x 32 x 64): an L of three boxes around the middle, wrapping around the periodic z seam
+    boxes += [(1, (8, 8, 56), (8 + 4 * m - 1, 8 + 2 * m - 1, 63)), (1, (8, 8, 0), (8 + 4 * m - 1, 8 + 2 * m - 1, 2 * m - 1)),
+              (1, (8, 8 + 2 * m, 0), (8 + 2 * m - 1, 8 + 4 * m - 1 if 8 + 4 * m <= 32 else 31, 2 * m - 1))]
+    boxes = [b for b in boxes if all(b[2][d] < (n0[d] << b[0]) for d in range(3))]
+    nlev = 2
+    if bf <= 4:  # level 2 (index space 96 x 64 x 128) inside the first level-1 boxes, gap >= bf fine cells
+        boxes.append((2, (24, 20, 4), (24 + 2 * bf - 1, 20 + 2 * bf - 1, 4 + 2 * bf - 1)))
+        nlev = 3
+    from paper_2404_02950_b200 import sledge as S
+    try:
+        S.sledge_arena_bytes(n0, boxes=boxes, n_levels=nlev, nghost=g, blocking_factor=bf, lap_order=order, interp=interp)
+    except S.SledgeError as e:
+        pytest.skip(f"hierarchy not valid for this case: {e}")
+    o, s = P.make_pair(n0, boxes=boxes, n_levels=nlev, nghost=g, blocking_factor=bf, lap_order=order, h0=0.5, lam=0.8,
+                       a_mass=0.2, rk_dataflow="fused", interp=interp)
+    P.init_smooth(o, s, n0, 21, amp=0.7)
+    for l in range(nlev - 1, 0, -1):
+        o.average_down(l)
+        s.average_down(l)
+    eta, dt = 1.2, 0.08
+    for _ in range(3):
+        o.rk_step(dt, eta)
+        s.rk_step(dt, eta)
+        eta += dt
+    assert P.max_err(o, s) <= F64_TOL
+    for l in range(nlev):
+        P.upload_oracle_state(o, s) if l == 0 else None
+        ot, oc = o.tag_strings(l)
+        gt, gc = s.tag_strings(l)
+        s.synchronize()
+        for a, b in zip(ot, s.split_tags(l, gt)):
+            assert np.array_equal(a, b.cpu().numpy())
+        assert np.array_equal(oc.astype(np.int64), gc.cpu().numpy().astype(np.int64))
+
+
+def test_shadow_level_with_auxiliary_fields():
+    P = _pair()
+    n0 = 32
+    boxes = inputs.split_level0(n0, 16)
+    o, s = P.make_pair(n0, boxes=boxes, nghost=2, lap_order=2, h0=0.5, lam=1.0, gw=True, gw_coupling=0.7, shadow_level=True)
+    P.init_smooth(o, s, n0, 4, comps=range(16), amp=0.5)
+    o.shadow_tee(0.1, 1.0, 1e-3, 1e-3)
+    s.shadow_tee(0.1, 1.0, 1e-3, 1e-3)
+    s.synchronize()
+    assert P.max_err(o, s, comps=range(16)) <= F64_TOL
