@@ -629,8 +629,11 @@ enum PatchKind { PATCH_COPY = 0, PATCH_INTERP = 1, PATCH_SLOW = 2 };
 #endif
 constexpr int PATCH_WARPS = SLEDGE_PATCH_WARPS;
 
+#ifndef SLEDGE_PATCH_MINB
+#define SLEDGE_PATCH_MINB 5  // measured on C5: 5 CTAs of 4 warps per SM (102 registers) beats 4 (124) and 6 (85, spills)
+#endif
 template <typename T, bool FILL_PI>
-__global__ void __launch_bounds__(PATCH_WARPS * 32) k_fill_patches(const GhostArgs<T> a) {
+__global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_patches(const GhostArgs<T> a) {
   using P = typename PairOf<T>::type;
   extern __shared__ __align__(16) unsigned char patch_smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
