@@ -100,8 +100,11 @@ __device__ __forceinline__ unsigned tag_differs(unsigned a, unsigned b) {
   return (v | (v >> 1) | (v >> 2)) & ROWS;
 }
 
+#ifndef SLEDGE_TAG_MINB
+#define SLEDGE_TAG_MINB 1
+#endif
 template <typename T>
-__global__ void __launch_bounds__(TAG_THREADS) k_tag_strings(const TagArgs<T> a) {
+__global__ void __launch_bounds__(TAG_THREADS, SLEDGE_TAG_MINB) k_tag_strings(const TagArgs<T> a) {
   using P = typename PairOf<T>::type;
   constexpr int RY = TAG_RY;
   const TileDev t = a.tiles[blockIdx.x];
