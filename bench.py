@@ -418,6 +418,8 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
                                    + (", with the 12 gravitational-wave auxiliary components (Eq.16)" if args.gw else "")
                                    + (", quartic conservative coarse->fine interpolation" if args.interp == 4 and cfg.n_levels > 1 else ""),
                        "cells_per_level": per_level, "coverage": cover, "cell_steps_per_step": cell_steps,
+                       "boxes_per_level": [len(s.level_boxes(l)) for l in range(cfg.n_levels)],
+                       "storage_boxes_per_level": [s.level_storage(l)[0] for l in range(cfg.n_levels)],
                        "l2": "state buffers >> 126 MB L2 (no flush needed)" if cell_steps * esz * 4 > 4e8 else
                              "state fits in L2 (small case; not a roofline workload)",
                        "multi_gpu": "replicas only"},

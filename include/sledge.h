@@ -215,6 +215,13 @@ int sledge_shadow_tee(sledge_ctx* ctx, double dt, double eta, const double* eps4
 /* Bookkeeping. */
 int sledge_level_cells(const sledge_ctx* ctx, int level, int64_t* valid_cells, int64_t* count_blocks);
 int64_t sledge_launch_count(const sledge_ctx* ctx); /* kernels launched by this context so far */
+/* Storage layout of `level` ("storage boxes"): the boxes given to sledge_create are coalesced
+ * into larger rectangles wherever two of them share a whole face, so that no ghost cells lie between them; every entry
+ * point still addresses the caller's boxes (box index, tag layout, dense copies).  storage_boxes: rectangles the level
+ * is stored in (= the caller's box count of that level when nothing could be merged, or with SLEDGE_COALESCE=0 in the
+ * environment at create); stored_cells: cells per plane of one state buffer, ghost layers and row padding included.
+ * Either pointer may be NULL.  SLEDGE_EINVAL for a bad level. */
+int sledge_level_storage(const sledge_ctx* ctx, int level, int* storage_boxes, int64_t* stored_cells);
 /* The data-flow `level` runs: K1 launches per step of that level (the auxiliary-field stages of
  * gw included) and algorithmic words (reals read + written) per cell-step of those launches: FUSED 2 / 20 (level 0, and
  * finer levels unless quartic interpolation runs per cell, nghost = 1), LEAN 4 / 52, CLASSIC 4 / 64, SSPRK3 3 / 32, RKN s / sum over the

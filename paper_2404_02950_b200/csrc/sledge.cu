@@ -119,7 +119,9 @@ struct LevelHost {
   int n[3], no[3];
   double h;
   std::vector<int> boxes;  // global box ids in input order
-  std::vector<BoxDev> boxdev;
+  std::vector<BoxDev> boxdev;   // STORAGE boxes: the caller's boxes coalesced into larger rectangles (K1, K2, K4 coarse side)
+  std::vector<BoxDev> viewdev;  // the caller's boxes in input order, as windows into their storage box (K3, K4 fine side, copies)
+  size_t off_views = 0;
   std::vector<int> owner;
   std::vector<TileDev> tiles, ftiles, tag_tiles;  // K1 staged / K1 fused / K3
   std::vector<int> ghost_prefix, avg_prefix;
@@ -441,17 +443,14 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
           if (ow != -1) return fail(nullptr, SLEDGE_EINVAL, "box %d overlaps box %d of level %d", ib, L.boxes[ow], B.level);
           ow = li;
         }
-    // row: [0, ox) left pad + ghosts, [ox, ox+n) valid, then >= g ghosts, pitch a multiple of 128 bytes
-    bd.sx = (P.ox + bd.n[0] + g + P.cpa - 1) / P.cpa * P.cpa;
-    bd.sy = bd.n[1] + 2 * g;
-    bd.base = L.plane_cells;
+    bd.sx = bd.sy = 0;  // pitches and base follow from the storage box (below)
+    bd.base = 0;
     bd.tag_base = L.valid_cells;
-    L.plane_cells += (long long)bd.sx * bd.sy * (bd.n[2] + 2 * g);
     L.valid_cells += (long long)bd.n[0] * bd.n[1] * bd.n[2];
     max_box_cells = std::max(max_box_cells, (size_t)(bd.n[0] + 2 * g) * (bd.n[1] + 2 * g) * (bd.n[2] + 2 * g));
     P.box_local[ib] = li;
     L.boxes.push_back(ib);
-    L.boxdev.push_back(bd);
+    L.viewdev.push_back(bd);
   }
   for (size_t q = 0; q < P.lev[0].owner.size(); ++q)
     if (P.lev[0].owner[q] < 0) return fail(nullptr, SLEDGE_EINVAL, "level 0 must cover the whole domain (L39)");
@@ -461,7 +460,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     const LevelHost& C = P.lev[l - 1];
     if (L.boxes.empty()) return fail(nullptr, SLEDGE_EINVAL, "level %d has no boxes", l);
     for (size_t q = 0; q < L.boxes.size(); ++q) {
-      const BoxDev& b = L.boxdev[q];
+      const BoxDev& b = L.viewdev[q];
       // coarse cells touched by the grown box; owner granularity is bf coarse cells
       int clo[3], chi[3];
       for (int d = 0; d < 3; ++d) {
@@ -478,6 +477,83 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
               return fail(nullptr, SLEDGE_EINVAL, "box %d violates proper nesting: gap to the level-%d boundary < blocking factor (L70, L137)",
                           L.boxes[q], l - 1);
           }
+    }
+  }
+  // Storage boxes.  Two boxes of a level that share a whole face need no ghost cells between them: the caller's boxes
+  // (the granularity the paper's load balancer hands to MPI ranks, L39) are coalesced, greedily along x, then z, then
+  // y, into larger rectangles that K1 sweeps and K2 fills as ONE box; every caller's box stays addressable as a view
+  // (same pitches, shifted base).  Results do not depend on it: a ghost copy holds the bits of the cell it mirrors.
+  // SLEDGE_COALESCE=0 in the environment keeps one storage box per caller's box (diagnostics).
+  {
+    const char* env = getenv("SLEDGE_COALESCE");
+    const bool coalesce = !(env && env[0] == '0');
+    int order[3] = {0, 2, 1};  // x, z, y (measured on C5); SLEDGE_COALESCE=zyx (any permutation of xyz) changes it (diagnostics)
+    if (env && strlen(env) == 3) {
+      int seen = 0, o[3];
+      for (int d = 0; d < 3; ++d) {
+        o[d] = env[d] - 'x';
+        if (o[d] >= 0 && o[d] < 3) seen |= 1 << o[d];
+      }
+      if (seen == 7)
+        for (int d = 0; d < 3; ++d) order[d] = o[d];
+    }
+    for (int l = 0; l < p.n_levels; ++l) {
+      LevelHost& L = P.lev[l];
+      struct R3 { int lo[3], hi[3]; };  // inclusive
+      std::vector<R3> rs;
+      for (const BoxDev& v : L.viewdev) rs.push_back(R3{{v.lo[0], v.lo[1], v.lo[2]}, {v.lo[0] + v.n[0] - 1, v.lo[1] + v.n[1] - 1, v.lo[2] + v.n[2] - 1}});
+      for (bool merged = coalesce; merged;) {  // until a pass over the three axes merges nothing
+        merged = false;
+        for (int dd = 0; dd < 3; ++dd) {
+          const int d = order[dd], o1 = (d + 1) % 3, o2 = (d + 2) % 3;
+          std::sort(rs.begin(), rs.end(), [&](const R3& a, const R3& b) {
+            if (a.lo[o1] != b.lo[o1]) return a.lo[o1] < b.lo[o1];
+            if (a.lo[o2] != b.lo[o2]) return a.lo[o2] < b.lo[o2];
+            if (a.hi[o1] != b.hi[o1]) return a.hi[o1] < b.hi[o1];
+            if (a.hi[o2] != b.hi[o2]) return a.hi[o2] < b.hi[o2];
+            return a.lo[d] < b.lo[d];
+          });
+          std::vector<R3> out;
+          for (const R3& r : rs) {
+            if (!out.empty()) {
+              R3& q = out.back();
+              // pitches are kept in 16 bits, patch and tile tables in ints: stop well below
+              if (q.lo[o1] == r.lo[o1] && q.hi[o1] == r.hi[o1] && q.lo[o2] == r.lo[o2] && q.hi[o2] == r.hi[o2] &&
+                  q.hi[d] + 1 == r.lo[d] && r.hi[d] - q.lo[d] + 1 <= 16384) {
+                q.hi[d] = r.hi[d];
+                merged = true;
+                continue;
+              }
+            }
+            out.push_back(r);
+          }
+          rs.swap(out);
+        }
+      }
+      for (size_t q = 0; q < rs.size(); ++q) {
+        const R3& r = rs[q];
+        BoxDev bd;
+        for (int d = 0; d < 3; ++d) {
+          bd.lo[d] = r.lo[d];
+          bd.n[d] = r.hi[d] - r.lo[d] + 1;
+        }
+        // row: [0, ox) left pad + ghosts, [ox, ox+n) valid, then >= g ghosts, pitch a multiple of 128 bytes
+        bd.sx = (P.ox + bd.n[0] + g + P.cpa - 1) / P.cpa * P.cpa;
+        bd.sy = bd.n[1] + 2 * g;
+        bd.base = L.plane_cells;
+        bd.tag_base = 0;  // tags are laid out by the caller's boxes (views)
+        L.plane_cells += (long long)bd.sx * bd.sy * (bd.n[2] + 2 * g);
+        for (int k = r.lo[2] >> bfs; k <= r.hi[2] >> bfs; ++k)
+          for (int j = r.lo[1] >> bfs; j <= r.hi[1] >> bfs; ++j)
+            for (int i = r.lo[0] >> bfs; i <= r.hi[0] >> bfs; ++i) L.owner[((size_t)k * L.no[1] + j) * L.no[0] + i] = (int)q;
+        L.boxdev.push_back(bd);
+      }
+      for (BoxDev& v : L.viewdev) {
+        const BoxDev& sb = L.boxdev[L.owner[((size_t)(v.lo[2] >> bfs) * L.no[1] + (v.lo[1] >> bfs)) * L.no[0] + (v.lo[0] >> bfs)]];
+        v.sx = sb.sx;
+        v.sy = sb.sy;
+        v.base = sb.base + ((long long)(v.lo[2] - sb.lo[2]) * sb.sy + (v.lo[1] - sb.lo[1])) * sb.sx + (v.lo[0] - sb.lo[0]);
+      }
     }
   }
   // work tables
@@ -501,7 +577,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     int tnz = K1_NZ;
     for (; tnz > 32; tnz /= 2) {
       long long nt = 0;
-      for (const BoxDev& b : L.boxdev)
+      for (const BoxDev& b : L.viewdev)
         nt += (long long)((b.n[0] + TAG_TX - 1) / TAG_TX) * ((b.n[1] + TAG_TY - 1) / TAG_TY) * ((b.n[2] + tnz - 1) / tnz);
       if (nt >= TAG_MIN_TILES) break;
     }
@@ -513,19 +589,22 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       for (int z0 = 0; z0 < b.n[2]; z0 += fnz)
         for (int y0 = 0; y0 < b.n[1]; y0 += K1F_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += ftxc) L.ftiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(fnz, b.n[2] - z0)});
-      for (int z0 = 0; z0 < b.n[2]; z0 += tnz)
-        for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
-          for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(tnz, b.n[2] - z0)});
       const long long Gx = b.n[0] + 2 * g, Gy = b.n[1] + 2 * g;
       const long long nghost = Gx * Gy * 2 * g + Gx * 2 * g * b.n[2] + 2LL * g * b.n[1] * b.n[2];
       L.ghost_prefix.push_back(L.ghost_prefix.back() + (int)((nghost + GHOST_THREADS - 1) / GHOST_THREADS));
-      const long long ncoarse = (long long)(b.n[0] / 2) * (b.n[1] / 2) * (b.n[2] / 2);
-      L.avg_prefix.push_back(L.avg_prefix.back() + (int)((ncoarse + AVG_THREADS - 1) / AVG_THREADS));
       if (qparents) {  // parents of the ghost shell: the shell of thickness ceil(g/2) around the coarse footprint
         const long long t = (g + 1) / 2, cx = b.n[0] / 2, cy = b.n[1] / 2, cz = b.n[2] / 2;
         const long long npar = (cx + 2 * t) * (cy + 2 * t) * 2 * t + (cx + 2 * t) * 2 * t * cz + 2 * t * cy * cz;
         L.qp_prefix.push_back(L.qp_prefix.back() + (int)((npar + GHOST_THREADS - 1) / GHOST_THREADS));
       }
+    }
+    for (size_t q = 0; q < L.viewdev.size(); ++q) {  // K3 and the fine side of K4 keep the caller's box order (tag layout)
+      const BoxDev& b = L.viewdev[q];
+      for (int z0 = 0; z0 < b.n[2]; z0 += tnz)
+        for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
+          for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(tnz, b.n[2] - z0)});
+      const long long ncoarse = (long long)(b.n[0] / 2) * (b.n[1] / 2) * (b.n[2] / 2);
+      L.avg_prefix.push_back(L.avg_prefix.back() + (int)((ncoarse + AVG_THREADS - 1) / AVG_THREADS));
     }
   }
   for (int l = 0; l < p.n_levels; ++l)
@@ -549,6 +628,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       for (int b = 0; b < NBUF; ++b)
         for (int c = 0; c < 6; ++c) L.off_gw[b][c] = take(plane_bytes);
     L.off_boxes = take(L.boxdev.size() * sizeof(BoxDev));
+    L.off_views = take(L.viewdev.size() * sizeof(BoxDev));
     L.off_tiles = take(L.tiles.size() * sizeof(TileDev));
     L.off_ftiles = take(L.ftiles.size() * sizeof(TileDev));
     L.off_tag_tiles = take(L.tag_tiles.size() * sizeof(TileDev));
@@ -1328,9 +1408,9 @@ int avg_between(sledge_ctx* fc, int lf, sledge_ctx* cc, int lc, int wa, int wb, 
   LevelHost& C = cc->plan.lev[lc];
   AvgArgs<T> a;
   memset(&a, 0, sizeof a);
-  a.fboxes = tab<BoxDev>(fc, F.off_boxes);
+  a.fboxes = tab<BoxDev>(fc, F.off_views);
   a.blk_prefix = tab<int>(fc, F.off_avg_prefix);
-  a.nfbox = (int)F.boxdev.size();
+  a.nfbox = (int)F.viewdev.size();
   a.f_psi = plane_ptr<T>(fc, lf, F.cur, wa);
   a.f_pi = plane_ptr<T>(fc, lf, F.cur, wb);
   a.fgeom = geom_of(fc->plan, lf);
@@ -1393,18 +1473,20 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   LevelHost& L = P.lev[l];
   // after a coarse step every level sits at its parent's t_new: alpha = 1, no temporal interpolation (L74)
   const double tcur = (l > 0 && P.lev[l - 1].have_pair) ? P.lev[l - 1].t_new : 0.0;
-  int rc = L.periodic_box ? SLEDGE_OK : launch_ghosts<T>(c, l, L.cur, tcur, false, false, 0, 1, true);  // K3 wraps by itself there
+  // K3 runs over the caller's boxes (views): it wraps by itself only where the ONE box of the level is the caller's too
+  const bool k3_wraps = L.periodic_box && L.viewdev.size() == 1;
+  int rc = k3_wraps ? SLEDGE_OK : launch_ghosts<T>(c, l, L.cur, tcur, false, false, 0, 1, true);
   if (rc) return rc;
   if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)L.count_blocks, c->stream);
   TagArgs<T> a;
-  a.boxes = tab<BoxDev>(c, L.off_boxes);
+  a.boxes = tab<BoxDev>(c, L.off_views);
   a.tiles = tab<TileDev>(c, L.off_tag_tiles);
   a.psi = plane_ptr<T>(c, l, L.cur, 0);
   a.tags = tags;
   a.counts = counts;
   a.g = P.p.nghost;
   a.ox = P.ox;
-  a.wrap = L.periodic_box ? 1 : 0;
+  a.wrap = k3_wraps ? 1 : 0;
   a.nb0 = L.nb[0];
   a.nb1 = L.nb[1];
   {
@@ -1425,7 +1507,7 @@ int do_copy_comp(sledge_ctx* c, int ib, int comp, void* dense, bool to_state, bo
   Plan& P = c->plan;
   const int l = P.box[ib].level;
   LevelHost& L = P.lev[l];
-  const BoxDev& b = L.boxdev[P.box_local[ib]];
+  const BoxDev& b = L.viewdev[P.box_local[ib]];
   const int e = with_ghosts ? P.p.nghost : 0;
   const long long total = (long long)(b.n[0] + 2 * e) * (b.n[1] + 2 * e) * (b.n[2] + 2 * e);
   const int grid = (int)std::min<long long>((total + 255) / 256, 148 * 32);
@@ -1512,6 +1594,7 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     up(L.off_patches, L.patches.data(), L.patches.size() * sizeof(uint4));
     up(L.off_tag_patches, L.tag_patches.data(), L.tag_patches.size() * sizeof(uint4));
     up(L.off_boxes, L.boxdev.data(), L.boxdev.size() * sizeof(BoxDev));
+    up(L.off_views, L.viewdev.data(), L.viewdev.size() * sizeof(BoxDev));
     up(L.off_tiles, L.tiles.data(), L.tiles.size() * sizeof(TileDev));
     up(L.off_ftiles, L.ftiles.data(), L.ftiles.size() * sizeof(TileDev));
     up(L.off_tag_tiles, L.tag_tiles.data(), L.tag_tiles.size() * sizeof(TileDev));
@@ -1749,6 +1832,13 @@ int sledge_level_cells(const sledge_ctx* c, int level, int64_t* valid_cells, int
   if (!c || level < 0 || level >= c->plan.p.n_levels) return SLEDGE_EINVAL;
   if (valid_cells) *valid_cells = c->plan.lev[level].valid_cells;
   if (count_blocks) *count_blocks = c->plan.lev[level].count_blocks;
+  return SLEDGE_OK;
+}
+
+int sledge_level_storage(const sledge_ctx* c, int level, int* storage_boxes, int64_t* stored_cells) {
+  if (!c || level < 0 || level >= c->plan.p.n_levels) return SLEDGE_EINVAL;
+  if (storage_boxes) *storage_boxes = (int)c->plan.lev[level].boxdev.size();
+  if (stored_cells) *stored_cells = c->plan.lev[level].plane_cells;
   return SLEDGE_OK;
 }
 

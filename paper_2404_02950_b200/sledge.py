@@ -24,7 +24,7 @@ SYMBOLS = [
     "sledge_arena_bytes", "sledge_create", "sledge_destroy", "sledge_set_state", "sledge_get_state",
     "sledge_set_state_host", "sledge_get_state_host", "sledge_host_copies_join", "sledge_get_ghosted", "sledge_fill_ghosts",
     "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable",
-    "sledge_shadow_tee", "sledge_level_cells", "sledge_level_dataflow",
+    "sledge_shadow_tee", "sledge_level_cells", "sledge_level_storage", "sledge_level_dataflow",
     "sledge_launch_count", "sledge_synchronize", "sledge_profile_enable", "sledge_profile_read",
     "sledge_last_error",
 ]
@@ -78,6 +78,7 @@ def lib():
         L.sledge_tee_enable.argtypes = [vp, i, C.POINTER(C.c_double), vp, vp]
         L.sledge_shadow_tee.argtypes = [vp, d, d, C.POINTER(C.c_double), vp, vp]
         L.sledge_level_cells.argtypes = [vp, i, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.sledge_level_storage.argtypes = [vp, i, C.POINTER(C.c_int), C.POINTER(C.c_int64)]
         L.sledge_level_dataflow.argtypes = [vp, i, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.sledge_launch_count.argtypes = [vp]
         L.sledge_launch_count.restype = C.c_int64
@@ -213,6 +214,12 @@ class Sledge:
         v, b = C.c_int64(0), C.c_int64(0)
         self._chk(lib().sledge_level_cells(self._h, level, C.byref(v), C.byref(b)), "sledge_level_cells")
         return int(v.value), int(b.value)
+
+    def level_storage(self, level):
+        """(storage boxes the level's caller boxes were coalesced into, stored cells per plane of one state buffer)"""
+        n, w = C.c_int(0), C.c_int64(0)
+        self._chk(lib().sledge_level_storage(self._h, level, C.byref(n), C.byref(w)), "sledge_level_storage")
+        return int(n.value), int(w.value)
 
     def level_dataflow(self, level):
         """(K1 launches per step of the level, algorithmic words per cell-step of those launches)"""

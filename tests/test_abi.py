@@ -52,6 +52,25 @@ def test_arena_bytes_matches_hand_count_single_box():
     assert n32 >= 8 * 64 * 34 * 34 * 8
 
 
+def test_coalescing_removes_the_ghost_cells_between_boxes(monkeypatch):
+    """Storage boxes (include/sledge.h, sledge_level_storage): 8 boxes of 16^3 covering a 32^3 level are stored as one
+    32^3 rectangle -- the arena is that of the one-box layout (plus descriptor tables), and smaller than with
+    SLEDGE_COALESCE=0 (8 x (16 + 2g)^3 against (32 + 2g)^3 stored cells per plane)."""
+    split = inputs.split_level0(32, 16)
+    kw = dict(nghost=2, blocking_factor=8, lap_order=2)
+    monkeypatch.delenv("SLEDGE_COALESCE", raising=False)
+    one = S.sledge_arena_bytes(32, **kw)
+    merged = S.sledge_arena_bytes(32, boxes=split, **kw)
+    monkeypatch.setenv("SLEDGE_COALESCE", "0")
+    apart = S.sledge_arena_bytes(32, boxes=split, **kw)
+    # staging slots are sized by the largest caller's box: smaller for the split list
+    assert merged <= one + 64 * 1024
+    plane_one = 48 * 36 * 36 * 16          # 8 + 32 + 8 pairs per row
+    plane_apart = 8 * 32 * 20 * 20 * 16    # 8 + 16 + 8 pairs per row
+    assert apart - merged >= 8 * (plane_apart - plane_one) - 64 * 1024
+    assert apart > merged
+
+
 RKN4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_b=[1 / 6, 1 / 3, 0.0],
             tableau=[0.0, 1 / 8, 0.0, 0.0, 0.5, 0.0])
 

@@ -366,3 +366,67 @@ def test_shadow_level_with_auxiliary_fields():
     s.shadow_tee(0.1, 1.0, 1e-3, 1e-3)
     s.synchronize()
     assert P.max_err(o, s, comps=range(16)) <= F64_TOL
+
+
+# ---- storage boxes: the caller's boxes coalesced into larger rectangles --------------------------------------
+
+def _run_hierarchy(monkeypatch, coalesce, dtype, flow, interp, ragged):
+    """three coarse steps + tags + truncation-error tags on a multi-box hierarchy; returns everything a caller can see"""
+    from paper_2404_02950_b200.sledge import Sledge
+    P = _pair()
+    if coalesce is None:
+        monkeypatch.delenv("SLEDGE_COALESCE", raising=False)
+    else:
+        monkeypatch.setenv("SLEDGE_COALESCE", coalesce)
+    if ragged:
+        n0, boxes, nl = (40, 24, 72), _ragged_boxes(), 1
+    else:
+        n0, boxes, nl = 32, _ring_hierarchy(32), 3
+    s = Sledge(n0, boxes=boxes, n_levels=nl, nghost=3, lap_order=2, h0=0.5, lam=0.7, a_mass=0.3, friction=2.0,
+               rk_dataflow=flow, interp=interp, dtype=dtype)
+    n03 = (n0,) * 3 if isinstance(n0, int) else n0
+    for ib, (lvl, lo, hi) in enumerate(boxes):
+        for c in range(4):
+            f = P.smooth_field((lo, hi), lvl, n03, 31 + c, amp=0.8)
+            s.set_state(ib, c, torch.from_numpy(np.ascontiguousarray(f)).to(s.tdtype).cuda().contiguous())
+    for l in range(nl - 1, 0, -1):
+        s.average_down(l)
+    out = {"storage": [s.level_storage(l) for l in range(nl)]}
+    tee = None
+    if nl > 1:
+        tee = s.tee_enable(1, 1e-4, 1e-4, 1e-3, 1e-3)
+    eta, dt = 1.5, 0.1
+    for _ in range(3):
+        s.rk_step(dt, eta)
+        eta += dt
+    out["state"] = [s.get_state(ib, c).cpu() for ib in range(len(boxes)) for c in range(4)]
+    out["tags"] = [tuple(t.cpu() for t in s.tag_strings(l)) for l in range(nl)]
+    if tee is not None:
+        s.synchronize()
+        out["tee"] = tuple(t.cpu() for t in tee)
+    s.fill_ghosts(nl - 1, eta)
+    out["ghosted"] = [s.get_ghosted(ib, c).cpu() for ib in s.level_boxes(nl - 1) for c in (0, 3)]
+    return out
+
+
+@pytest.mark.parametrize("dtype,flow,interp,ragged", [("f64", "fused", 0, False), ("f64", "lean", 4, False),
+                                                      ("f32", "fused", 4, False), ("f64", "fused", 0, True),
+                                                      ("f32", "classic", 0, True)])
+def test_coalesced_storage_gives_the_same_bits(monkeypatch, dtype, flow, interp, ragged):
+    """Merging boxes that share a face removes ghost cells, never changes a result: states, string tags + counts,
+    truncation-error tags and ghosted copies are bit-identical with SLEDGE_COALESCE=0, the default order and zyx."""
+    ref = _run_hierarchy(monkeypatch, "0", dtype, flow, interp, ragged)
+    nbox = [len([b for b in (_ragged_boxes() if ragged else _ring_hierarchy(32)) if b[0] == l]) for l in range(len(ref["storage"]))]
+    assert [n for n, _ in ref["storage"]] == nbox
+    for mode in (None, "zyx"):
+        got = _run_hierarchy(monkeypatch, mode, dtype, flow, interp, ragged)
+        assert got["storage"][0][0] == 1          # level 0 covers the domain: one rectangle (the ragged list too)
+        assert all(g[0] <= r[0] and g[1] <= r[1] for g, r in zip(got["storage"], ref["storage"]))
+        for key in ("state", "ghosted"):
+            for a, b in zip(ref[key], got[key]):
+                assert torch.equal(a, b), key
+        for (ta, ca), (tb, cb) in zip(ref["tags"], got["tags"]):
+            assert torch.equal(ta, tb) and torch.equal(ca, cb)
+        if "tee" in ref:
+            for a, b in zip(ref["tee"], got["tee"]):
+                assert torch.equal(a, b)
