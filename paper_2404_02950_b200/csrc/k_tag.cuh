@@ -72,6 +72,12 @@ struct TagArgs {
   int wrap;      // the level is ONE box covering the periodic domain: +1 neighbours past the box edge are read at
                  // their wrapped position instead of from the ghost layer (L23), no ghost fill needed
   int nb0, nb1;  // count blocks per axis (x, y)
+  // Tiles over STORAGE boxes (several caller's boxes coalesced, sledge.cu "storage boxes"): the tag bytes keep the
+  // caller's layout, found per blocking-factor cell (the granularity of box ownership, >= TAG_RY here) in this table:
+  // {x, y} = offset of the cell's first tag byte (low, high word), z = n0 and w = n1 of the caller's box it lies in.
+  // Null: `boxes` are the caller's boxes themselves.
+  const int4* tag_cells;
+  int bfs, no0, no1;  // log2(blocking factor), owner grid extent (x, y)
 };
 
 __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
@@ -176,7 +182,18 @@ __global__ void __launch_bounds__(TAG_THREADS, SLEDGE_TAG_MINB) k_tag_strings(co
     cntA = cntB = 0;
   };
   uint8_t* tagp = a.tags ? a.tags + b.tag_base + ((long long)(t.z0 - 1) * b.n[1] + y0) * b.n[0] + x : nullptr;
-  const long long tag_plane = (long long)b.n[1] * b.n[0];
+  long long tag_plane = (long long)b.n[1] * b.n[0];
+  int tag_row = b.n[0];
+  // lookup mode: this lane's column of blocking-factor cells (x and y cell fixed, z varies), next entry prefetched
+  const bool lookup = a.tag_cells != nullptr && a.tags != nullptr;
+  const int bfm = (1 << a.bfs) - 1;
+  const int gx = b.lo[0] + min(x, b.n[0] - 1), gy = b.lo[1] + y0;
+  const int4* cellp = nullptr;
+  int4 nextc = make_int4(0, 0, 0, 0);
+  if (lookup) {
+    cellp = a.tag_cells + ((long long)((b.lo[2] + t.z0) >> a.bfs) * a.no1 + (gy >> a.bfs)) * a.no0 + (gx >> a.bfs);
+    nextc = __ldg(cellp);
+  }
 
   // state carried from plane n-1: its values, sign word, signed in-plane edges (x, y) and W_xy mask
   P cur[RY + 1];
@@ -231,10 +248,19 @@ __global__ void __launch_bounds__(TAG_THREADS, SLEDGE_TAG_MINB) k_tag_strings(co
       const unsigned myz = tag_differs(YPp + (ZP >> 3) + (YN + ZN), YNp + (ZN >> 3) + (YP + ZP));
       const unsigned mzx = tag_differs(ZP + XP + (ZNx + XNp), ZN + XN + (ZPx + XPp));
       const unsigned c3 = mxy_p | (myz << 1) | (mzx << 2);  // field r = tag byte of row r
+      if (lookup && (n == 1 || ((b.lo[2] + z) & bfm) == 0)) {  // entering a blocking-factor cell: its caller's box
+        const int4 c = nextc;
+        tag_row = c.z;
+        tag_plane = (long long)c.z * c.w;
+        tagp = a.tags + (((long long)(unsigned)c.y << 32) | (unsigned)c.x) +
+               ((long long)((b.lo[2] + z) & bfm) * c.w + (gy & bfm)) * c.z + (gx & bfm);
+        cellp += (long long)a.no1 * a.no0;
+        if (z + (bfm - ((b.lo[2] + z) & bfm)) + 1 < t.z0 + t.nz) nextc = __ldg(cellp);  // next cell of this tile, used planes later
+      }
       if (a.tags) {
 #pragma unroll
         for (int r = 0; r < RY; ++r)
-          if ((act >> (3 * r)) & 1u) tagp[(long long)r * b.n[0]] = (uint8_t)((c3 >> (3 * r)) & 7u);
+          if ((act >> (3 * r)) & 1u) tagp[(long long)r * tag_row] = (uint8_t)((c3 >> (3 * r)) & 7u);
       }
       const unsigned any = (mxy_p | myz | mzx) & act;
       cntA += __popc(any & rowsA);

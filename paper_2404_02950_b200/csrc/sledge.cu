@@ -125,6 +125,10 @@ struct LevelHost {
   std::vector<int> owner;
   std::vector<TileDev> tiles, ftiles, tag_tiles;  // K1 staged / K1 fused / K3
   std::vector<int> ghost_prefix, avg_prefix;
+  // K3 over storage boxes: per blocking-factor cell the tag offset of its first cell and n0, n1 of the caller's box
+  // (k_tag.cuh tag_cells); empty when the tag tiles run over the caller's boxes themselves
+  std::vector<int4> tag_cells;
+  size_t off_tag_cells = 0;
   std::vector<int> qp_prefix;  // quartic interpolation by coarse parent (k_fill_qparents): CTAs before box b
   size_t off_qp_prefix = 0, off_qp_list = 0, off_qs_list = 0, off_qs_count = 0;
   unsigned n_star_parents = 0;  // read back from the device after the plan
@@ -577,7 +581,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     int tnz = K1_NZ;
     for (; tnz > 32; tnz /= 2) {
       long long nt = 0;
-      for (const BoxDev& b : L.viewdev)
+      for (const BoxDev& b : (L.viewdev.size() != L.boxdev.size() && bf >= TAG_RY) ? L.boxdev : L.viewdev)
         nt += (long long)((b.n[0] + TAG_TX - 1) / TAG_TX) * ((b.n[1] + TAG_TY - 1) / TAG_TY) * ((b.n[2] + tnz - 1) / tnz);
       if (nt >= TAG_MIN_TILES) break;
     }
@@ -598,11 +602,28 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
         L.qp_prefix.push_back(L.qp_prefix.back() + (int)((npar + GHOST_THREADS - 1) / GHOST_THREADS));
       }
     }
-    for (size_t q = 0; q < L.viewdev.size(); ++q) {  // K3 and the fine side of K4 keep the caller's box order (tag layout)
-      const BoxDev& b = L.viewdev[q];
+    // K3 runs over the storage boxes too where it can find the caller's tag layout per blocking-factor cell (a warp's
+    // TAG_RY rows must lie in one such cell); otherwise over the caller's boxes
+    const bool tag_lookup = L.viewdev.size() != L.boxdev.size() && bf >= TAG_RY;
+    if (tag_lookup) {
+      L.tag_cells.assign(L.owner.size(), make_int4(0, 0, 0, 0));
+      for (const BoxDev& v : L.viewdev)
+        for (int k = v.lo[2] >> bfs; k <= (v.lo[2] + v.n[2] - 1) >> bfs; ++k)
+          for (int j = v.lo[1] >> bfs; j <= (v.lo[1] + v.n[1] - 1) >> bfs; ++j)
+            for (int i = v.lo[0] >> bfs; i <= (v.lo[0] + v.n[0] - 1) >> bfs; ++i) {
+              const long long o = v.tag_base + ((long long)((k << bfs) - v.lo[2]) * v.n[1] + ((j << bfs) - v.lo[1])) * v.n[0] + ((i << bfs) - v.lo[0]);
+              L.tag_cells[((size_t)k * L.no[1] + j) * L.no[0] + i] = make_int4((int)(unsigned)(o & 0xffffffffll), (int)(o >> 32), v.n[0], v.n[1]);
+            }
+    }
+    const std::vector<BoxDev>& tagboxes = tag_lookup ? L.boxdev : L.viewdev;
+    for (size_t q = 0; q < tagboxes.size(); ++q) {
+      const BoxDev& b = tagboxes[q];
       for (int z0 = 0; z0 < b.n[2]; z0 += tnz)
         for (int y0 = 0; y0 < b.n[1]; y0 += TAG_TY)
           for (int x0 = 0; x0 < b.n[0]; x0 += TAG_TX) L.tag_tiles.push_back(TileDev{(int)q, x0, y0, z0, std::min(tnz, b.n[2] - z0)});
+    }
+    for (size_t q = 0; q < L.viewdev.size(); ++q) {  // the fine side of K4 keeps the caller's box order (tag layout)
+      const BoxDev& b = L.viewdev[q];
       const long long ncoarse = (long long)(b.n[0] / 2) * (b.n[1] / 2) * (b.n[2] / 2);
       L.avg_prefix.push_back(L.avg_prefix.back() + (int)((ncoarse + AVG_THREADS - 1) / AVG_THREADS));
     }
@@ -629,6 +650,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
         for (int c = 0; c < 6; ++c) L.off_gw[b][c] = take(plane_bytes);
     L.off_boxes = take(L.boxdev.size() * sizeof(BoxDev));
     L.off_views = take(L.viewdev.size() * sizeof(BoxDev));
+    L.off_tag_cells = take(L.tag_cells.size() * sizeof(int4));
     L.off_tiles = take(L.tiles.size() * sizeof(TileDev));
     L.off_ftiles = take(L.ftiles.size() * sizeof(TileDev));
     L.off_tag_tiles = take(L.tag_tiles.size() * sizeof(TileDev));
@@ -1473,13 +1495,19 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
   LevelHost& L = P.lev[l];
   // after a coarse step every level sits at its parent's t_new: alpha = 1, no temporal interpolation (L74)
   const double tcur = (l > 0 && P.lev[l - 1].have_pair) ? P.lev[l - 1].t_new : 0.0;
-  // K3 runs over the caller's boxes (views): it wraps by itself only where the ONE box of the level is the caller's too
-  const bool k3_wraps = L.periodic_box && L.viewdev.size() == 1;
+  // K3 wraps by itself where its tiles run over ONE box covering the periodic domain (the caller's, or the storage box
+  // with the tag layout looked up per blocking-factor cell)
+  const bool tag_lookup = !L.tag_cells.empty();
+  const bool k3_wraps = L.periodic_box && (L.viewdev.size() == 1 || tag_lookup);
   int rc = k3_wraps ? SLEDGE_OK : launch_ghosts<T>(c, l, L.cur, tcur, false, false, 0, 1, true);
   if (rc) return rc;
   if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)L.count_blocks, c->stream);
   TagArgs<T> a;
-  a.boxes = tab<BoxDev>(c, L.off_views);
+  a.boxes = tab<BoxDev>(c, tag_lookup ? L.off_boxes : L.off_views);
+  a.tag_cells = tag_lookup ? tab<int4>(c, L.off_tag_cells) : nullptr;
+  a.bfs = ilog2(P.p.blocking_factor);
+  a.no0 = L.no[0];
+  a.no1 = L.no[1];
   a.tiles = tab<TileDev>(c, L.off_tag_tiles);
   a.psi = plane_ptr<T>(c, l, L.cur, 0);
   a.tags = tags;
@@ -1595,6 +1623,7 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
     up(L.off_tag_patches, L.tag_patches.data(), L.tag_patches.size() * sizeof(uint4));
     up(L.off_boxes, L.boxdev.data(), L.boxdev.size() * sizeof(BoxDev));
     up(L.off_views, L.viewdev.data(), L.viewdev.size() * sizeof(BoxDev));
+    up(L.off_tag_cells, L.tag_cells.data(), L.tag_cells.size() * sizeof(int4));
     up(L.off_tiles, L.tiles.data(), L.tiles.size() * sizeof(TileDev));
     up(L.off_ftiles, L.ftiles.data(), L.ftiles.size() * sizeof(TileDev));
     up(L.off_tag_tiles, L.tag_tiles.data(), L.tag_tiles.size() * sizeof(TileDev));
