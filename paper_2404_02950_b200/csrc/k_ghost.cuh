@@ -83,14 +83,13 @@ struct GhostArgs {
   // star patches (k_fill_patches): the fills before an RK sweep as rectangular regions, 2 x uint4 per patch
   const uint4* patches;
   unsigned n_patches;
-  // "velocity" ghosts of the second plane (k_fill_patches, interpolated cells only; FUSED sweeps on a fine level): the
-  // sweep forms the NEXT stage's psi at a ghost cell as psi_g + tau Pi_g, and that must be the coarse state
-  // interpolated at the later time t_b (L72), so Pi_g <- (I_psi(alpha_b) - I_psi(alpha_a)) * vel_scale with
-  // I_psi(alpha) the space-time interpolation of the coarse PSI planes and vel_scale = 1 / (t_b - t_a)
+  // "velocity" ghosts of the second plane (k_fill_patches and k_fill_qparents, interpolated cells only; FUSED sweeps on a
+  // fine level): the sweep forms the NEXT stage's psi at a ghost cell as psi_g + tau Pi_g, and that must be the coarse
+  // state interpolated at the later stage time (L72).  The space-time interpolant I_psi(t) is linear in t between the
+  // coarse old and new states, so its time derivative is I[psi_new - psi_old] / (t_new - t_old) whatever the two stage
+  // times are: Pi_g <- I[psi_new - psi_old] * vel_c (0 while the coarse level holds one state only).
   int vel;
-  T alpha_a, alpha_b, vel_scale;
-  T vel_c;  // k_fill_qparents: the same velocity ghost written as I[(psi_new - psi_old)] / (t_new - t_old) of the coarse
-            // level (I is linear, so it equals (I_psi(alpha_b) - I_psi(alpha_a)) / (t_b - t_a) up to rounding)
+  T vel_c;  // 1 / (t_new - t_old) of the coarse level
   int patch_smem_pairs;    // shared-memory pairs per warp and plane (largest coarse region of an interpolation patch)
 };
 
@@ -167,6 +166,30 @@ __device__ __forceinline__ typename PairOf<T>::type interp_coarse(const typename
     const T wt = (w[(q >> 2) & 1] * w[(q >> 1) & 1]) * w[q & 1];
     s0 += wt * cv0;
     s1 += wt * cv1;
+  }
+  return mkpair(s0, s1);
+}
+
+// the same trilinear combination of the coarse DIFFERENCE new - old (velocity ghosts: I is linear, so
+// I[psi_new - psi_old] / (t_new - t_old) is the time derivative of the space-time interpolant)
+template <typename T>
+__device__ __forceinline__ typename PairOf<T>::type interp_coarse_diff(const typename PairOf<T>::type* c_old,
+                                                                       const typename PairOf<T>::type* c_new,
+                                                                       const long long o[8]) {
+  using P = typename PairOf<T>::type;
+  const T w[2] = {T(0.75), T(0.25)};
+  T s0 = T(0), s1 = T(0);
+  P vo[8], vn[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    vo[q] = c_old[o[q]];
+    vn[q] = c_new[o[q]];
+  }
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const T wt = (w[(q >> 2) & 1] * w[(q >> 1) & 1]) * w[q & 1];
+    s0 += wt * (vn[q].x - vo[q].x);
+    s1 += wt * (vn[q].y - vo[q].y);
   }
   return mkpair(s0, s1);
 }
@@ -677,7 +700,7 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
     P* const cp = cs + a.patch_smem_pairs;
     const int ncoarse = cex * cey * cez;
     const T oma = T(1) - a.alpha;
-    const bool vel = FILL_PI && a.vel != 0;  // cs = coarse psi OLD, cp = coarse psi NEW, blended per use
+    const bool vel = FILL_PI && a.vel != 0;  // cs = coarse psi blended at alpha, cp = coarse psi NEW - OLD
     if (vel) {
       for (int q0 = lane; q0 < ncoarse; q0 += 128) {
         P vo[4], vn[4];
@@ -695,8 +718,8 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
         for (int u = 0; u < 4; ++u) {
           const int q = q0 + 32 * u;
           if (q < ncoarse) {
-            cs[q] = vo[u];
-            cp[q] = vn[u];
+            cs[q] = mkpair(oma * vo[u].x + a.alpha * vn[u].x, oma * vo[u].y + a.alpha * vn[u].y);
+            cp[q] = mkpair(vn[u].x - vo[u].x, vn[u].y - vo[u].y);
           }
         }
       }
@@ -742,26 +765,6 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
       const int x0 = ((px + i) >> 1) + 1 - px, y0 = ((py + j) >> 1) + 1 - py, z0 = ((pz + k) >> 1) + 1 - pz;
       const int x1 = ((px + i) & 1) ? x0 + 1 : x0 - 1, y1 = ((py + j) & 1) ? y0 + 1 : y0 - 1, z1 = ((pz + k) & 1) ? z0 + 1 : z0 - 1;
       T s0 = T(0), s1 = T(0), t0 = T(0), t1 = T(0);
-      if (vel) {  // psi at alpha; Pi <- (psi at alpha_b - psi at alpha_a) * vel_scale, each as interp_coarse would give it
-        const T al[3] = {a.alpha, a.alpha_a, a.alpha_b};
-        T r[3][2] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          const int o = (((c & 4) ? z1 : z0) * cey + ((c & 2) ? y1 : y0)) * cex + ((c & 1) ? x1 : x0);
-          const T wt = (w[(c >> 2) & 1] * w[(c >> 1) & 1]) * w[c & 1];
-          const P vo = cs[o], vn = cp[o];
-#pragma unroll
-          for (int m = 0; m < 3; ++m) {
-            const T om = T(1) - al[m];
-            r[m][0] += wt * (om * vo.x + al[m] * vn.x);
-            r[m][1] += wt * (om * vo.y + al[m] * vn.y);
-          }
-        }
-        const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
-        a.psi[d] = mkpair(r[0][0], r[0][1]);
-        a.pi[d] = mkpair((r[2][0] - r[1][0]) * a.vel_scale, (r[2][1] - r[1][1]) * a.vel_scale);
-        continue;
-      }
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         const int o = (((c & 4) ? z1 : z0) * cey + ((c & 2) ? y1 : y0)) * cex + ((c & 1) ? x1 : x0);
@@ -777,7 +780,8 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
       }
       const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
       a.psi[d] = mkpair(s0, s1);
-      if (FILL_PI) a.pi[d] = mkpair(t0, t1);
+      // velocity ghosts: Pi <- I[psi_new - psi_old] / (t_new - t_old) (0 while the coarse level has one state only)
+      if (FILL_PI) a.pi[d] = vel ? mkpair(t0 * a.vel_c, t1 * a.vel_c) : mkpair(t0, t1);
     }
     return;
   }
@@ -799,9 +803,8 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
     a.psi[d] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
     if (FILL_PI) {
       if (a.vel) {
-        const P pa = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha_a, o);
-        const P pb = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha_b, o);
-        a.pi[d] = mkpair((pb.x - pa.x) * a.vel_scale, (pb.y - pa.y) * a.vel_scale);
+        const P dv = interp_coarse_diff<T>(a.c_old_psi, a.c_new_psi, o);
+        a.pi[d] = mkpair(dv.x * a.vel_c, dv.y * a.vel_c);
       } else {
         a.pi[d] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
       }

@@ -823,9 +823,6 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, 
       bn = C.cur;
       a.single = 0;
       a.vel = 1;
-      a.alpha_a = (T)(pair ? (vf.ta - C.t_old) / (C.t_new - C.t_old) : 0.0);
-      a.alpha_b = (T)(pair ? (vf.tb - C.t_old) / (C.t_new - C.t_old) : 0.0);
-      a.vel_scale = (T)(1.0 / (vf.tb - vf.ta));
       a.vel_c = (T)(pair ? 1.0 / (C.t_new - C.t_old) : 0.0);
     }
     a.c_old_psi = plane_ptr<T>(c, l - 1, bo, wa);
