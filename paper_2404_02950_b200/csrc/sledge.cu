@@ -506,7 +506,12 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       struct R3 { int lo[3], hi[3]; };  // inclusive
       std::vector<R3> rs;
       for (const BoxDev& v : L.viewdev) rs.push_back(R3{{v.lo[0], v.lo[1], v.lo[2]}, {v.lo[0] + v.n[0] - 1, v.lo[1] + v.n[1] - 1, v.lo[2] + v.n[2] - 1}});
-      for (bool merged = coalesce; merged;) {  // until a pass over the three axes merges nothing
+      // a level that covers the whole domain (level 0 always does, L39) is ONE rectangle whatever the greedy merge
+      // below would make of an arbitrary partition
+      bool covered = coalesce;
+      for (size_t q = 0; covered && q < L.owner.size(); ++q) covered = L.owner[q] >= 0;
+      if (covered) rs.assign(1, R3{{0, 0, 0}, {L.n[0] - 1, L.n[1] - 1, L.n[2] - 1}});
+      for (bool merged = coalesce && !covered; merged;) {  // until a pass over the three axes merges nothing
         merged = false;
         for (int dd = 0; dd < 3; ++dd) {
           const int d = order[dd], o1 = (d + 1) % 3, o2 = (d + 2) % 3;

@@ -247,3 +247,85 @@ def split_level0(n0: int, box: int):
             for x in range(0, n0, box):
                 out.append((0, (x, y, z), (x + box - 1, y + box - 1, z + box - 1)))
     return out
+
+
+# ---------------------------------------------------------------------------------------------
+# seeded random hierarchies (tests): boxes of mixed sizes on every level, properly nested
+# ---------------------------------------------------------------------------------------------
+
+
+def _random_partition(rng, lo, hi, unit, min_units=1, p_stop=0.3):
+    """Recursive bisection of the index range [lo, hi) (x, y, z; multiples of `unit`) into rectangles whose sides are
+    multiples of `unit`: at every node either stop (probability p_stop) or cut a random axis at a random multiple."""
+    ext = [(hi[d] - lo[d]) // unit for d in range(3)]
+    axes = [d for d in range(3) if ext[d] >= 2 * min_units]
+    if not axes or rng.random() < p_stop:
+        return [(tuple(lo), tuple(hi))]
+    d = int(rng.choice(axes))
+    cut = lo[d] + unit * int(rng.integers(min_units, ext[d] - min_units + 1))
+    hi1 = list(hi)
+    hi1[d] = cut
+    lo2 = list(lo)
+    lo2[d] = cut
+    return (_random_partition(rng, list(lo), hi1, unit, min_units, p_stop)
+            + _random_partition(rng, lo2, list(hi), unit, min_units, p_stop))
+
+
+def random_hierarchy(n0, n_levels: int, blocking_factor: int, seed: int, fill: float = 0.35):
+    """Box list (level, lo, hi) of a random, valid hierarchy on the periodic domain n0 (int or (nx, ny, nz)):
+    level 0 = a random partition of the whole domain; level l > 0 = a random set of blocking-factor cells (probability
+    `fill`, grown so that it is not empty) cut down to proper nesting -- every cell of it, grown by one blocking factor,
+    lies on level l-1 -- and then cut into rectangles by random bisection of its bounding boxes.
+    Boxes of a level are disjoint; many share faces (the storage-box coalescing of the library) and many do not."""
+    rng = np.random.default_rng(seed)
+    n0 = (n0,) * 3 if isinstance(n0, int) else tuple(n0)
+    bf = blocking_factor
+    boxes = [(0, lo, tuple(h - 1 for h in hi)) for lo, hi in _random_partition(rng, [0, 0, 0], list(n0), bf, 1, 0.25)]
+    prev = np.ones(tuple(n0[d] // bf for d in (2, 1, 0)), dtype=bool)  # [z, y, x] blocking cells of level l-1 that exist
+    for l in range(1, n_levels):
+        shape = tuple(2 * s for s in prev.shape)
+        # fine blocking cells whose parent region grown by one fine blocking factor (= half a coarse blocking cell:
+        # the parent cell and, on the side the child sits, its neighbour) is covered by level l-1
+        ok = np.ones(shape, dtype=bool)
+        up = np.repeat(np.repeat(np.repeat(prev, 2, 0), 2, 1), 2, 2)
+        ok &= up
+        for ax in range(3):
+            for sh in (-1, 1):
+                ok &= np.roll(up, sh, axis=ax)  # the neighbour fine cells' parents cover the grown region
+        # corners: a grown box also touches the diagonal neighbours
+        for dz in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dx in (-1, 0, 1):
+                    ok &= np.roll(up, (dz, dy, dx), axis=(0, 1, 2))
+        want = rng.random(shape) < fill
+        # smooth the random set a little so that boxes larger than one cell appear
+        want |= np.roll(want, 1, axis=int(rng.integers(0, 3)))
+        mask = want & ok
+        if not mask.any():
+            idx = np.argwhere(ok)
+            if len(idx) == 0:
+                break
+            z, y, x = idx[int(rng.integers(0, len(idx)))]
+            mask[z, y, x] = True
+        # cut the mask into rectangles: random bisection of the domain, keep leaves that are fully inside the mask,
+        # recurse to single cells otherwise
+        def emit(lo, hi):
+            sub = mask[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]]
+            if not sub.any():
+                return []
+            if sub.all() and rng.random() < 0.7:
+                return [(l, tuple(bf * v for v in lo), tuple(bf * v - 1 for v in hi))]
+            ext = [hi[d] - lo[d] for d in range(3)]
+            axes = [d for d in range(3) if ext[d] >= 2]
+            if not axes:
+                return [(l, tuple(bf * v for v in lo), tuple(bf * v - 1 for v in hi))]
+            d = int(rng.choice(axes))
+            cut = lo[d] + int(rng.integers(1, ext[d]))
+            hi1 = list(hi)
+            hi1[d] = cut
+            lo2 = list(lo)
+            lo2[d] = cut
+            return emit(list(lo), hi1) + emit(lo2, list(hi))
+        boxes += emit([0, 0, 0], [shape[2], shape[1], shape[0]])
+        prev = mask
+    return boxes
