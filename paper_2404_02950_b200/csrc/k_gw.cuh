@@ -16,7 +16,7 @@
 // 512-byte runs that the CTA's own threads have just pulled in).  psi is read by all three CTAs of a tile (through
 // L2).  Words per cell-stage: 2 (psi) + 12 (U) + 12 per pointwise input state + 12 written.
 // (One CTA for all three planes needs four z-windows: 255 registers, one CTA per SM, 39 % of the HBM roofline.)
-// This is the straightforward version of the sweep: no shared-memory staging yet.
+// No shared-memory staging; the loads that miss L1 (window tops, du, Y of stages 2-3) are issued one plane ahead.
 #pragma once
 #include "k_rk_pipe.cuh"
 
@@ -53,8 +53,11 @@ __device__ __forceinline__ T grad_from(const T* m, const T* p, T inv_h) {
   return ((T(45) * (p[0] - m[0]) - T(9) * (p[1] - m[1])) + (p[2] - m[2])) * inv_h;
 }
 
+#ifndef SLEDGE_GW_MINB
+#define SLEDGE_GW_MINB 2
+#endif
 template <typename T, int ORDER, int MODE>
-__global__ void __launch_bounds__(GW_TX* GW_TY, 2) k_gw_stage(const GwArgs<T> a) {
+__global__ void __launch_bounds__(GW_TX* GW_TY, (sizeof(T) == 8 && ORDER == 3) ? 1 : SLEDGE_GW_MINB) k_gw_stage(const GwArgs<T> a) {
   using P = typename PairOf<T>::type;
   constexpr int R = ORDER;
   constexpr int CPT = Vec16<T>::CPT;  // the tiles are 32 * CPT cells wide: CPT passes over x
@@ -77,13 +80,44 @@ __global__ void __launch_bounds__(GW_TX* GW_TY, 2) k_gw_stage(const GwArgs<T> a)
     for (int f = 0; f < 2; ++f)
 #pragma unroll
       for (int m = 0; m < 2 * R; ++m) w[f][m + 1] = __ldg(src[f] + off + (long long)(m - R) * plane);
+    // the loads that come from HBM (top of the two z-windows, du, the pointwise stage inputs) are issued one plane
+    // ahead: a warp that needs them in the same iteration waits a full memory latency per plane
+    P nxt[2], dv_n, yu_n = mkpair(T(0), T(0)), yd_n = mkpair(T(0), T(0));
+#pragma unroll
+    for (int f = 0; f < 2; ++f) nxt[f] = __ldg(src[f] + off + (long long)R * plane);
+    dv_n = __ldg(a.du[q] + off);
+    if (MODE == LEAN_S23) {
+      yu_n = __ldg(a.in[0][q] + off);
+      yd_n = __ldg(a.in[0][3 + q] + off);
+    }
     for (int zz = 0; zz < t.nz; ++zz) {
       const long long o = off + (long long)zz * plane;
+      const bool more = zz + 1 < t.nz;
 #pragma unroll
       for (int f = 0; f < 2; ++f) {
 #pragma unroll
         for (int m = 0; m < 2 * R; ++m) w[f][m] = w[f][m + 1];
-        w[f][2 * R] = __ldg(src[f] + o + (long long)R * plane);
+        w[f][2 * R] = nxt[f];
+        if (more) nxt[f] = __ldg(src[f] + o + (long long)(R + 1) * plane);
+      }
+      const P dv = dv_n;
+      const P yu = yu_n, yd = yd_n;
+      P yv[NIN > 0 ? NIN : 1][2];
+      // S4 inputs: not prefetched (measured: no gain, spills with the 13-point windows); plain loads, because in[1]
+      // (U2) is the plane this stage overwrites in place
+      if (MODE == LEAN_S4) {
+#pragma unroll
+        for (int m = 0; m < NIN; ++m) {
+          yv[m][0] = a.in[m][q][o];
+          yv[m][1] = a.in[m][3 + q][o];
+        }
+      }
+      if (more) {
+        dv_n = __ldg(a.du[q] + o + plane);
+        if (MODE == LEAN_S23) {
+          yu_n = __ldg(a.in[0][q] + o + plane);
+          yd_n = __ldg(a.in[0][3 + q] + o + plane);
+        }
       }
       // x / y neighbours of the centre plane
       P xm[2][R], xp[2][R], ym[2][R], yp[2][R];
@@ -113,7 +147,6 @@ __global__ void __launch_bounds__(GW_TX* GW_TY, 2) k_gw_stage(const GwArgs<T> a)
         gr[c][2] = grad_from<T, ORDER>(m, p, a.inv_h);
       }
       {  // pair plane q holds components 2q, 2q + 1
-        const P dv = __ldg(a.du[q] + o);
         T ku[2], kdu[2], uc[2], duc[2];
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
@@ -144,17 +177,10 @@ __global__ void __launch_bounds__(GW_TX* GW_TY, 2) k_gw_stage(const GwArgs<T> a)
           ou = mkpair(fma(a.adt, ku[0], uc[0]), fma(a.adt, ku[1], uc[1]));
           odu = mkpair(fma(a.adt, kdu[0], duc[0]), fma(a.adt, kdu[1], duc[1]));
         } else if (MODE == LEAN_S23) {
-          const P yu = __ldg(a.in[0][q] + o), yd = __ldg(a.in[0][3 + q] + o);
           ou = mkpair(fma(a.adt, ku[0], yu.x), fma(a.adt, ku[1], yu.y));
           odu = mkpair(fma(a.adt, kdu[0], yd.x), fma(a.adt, kdu[1], yd.y));
         } else {  // LEAN_S4: (U2 + 2 U3 + U4 - Y)/3 + dt/6 k
           const T third = T(1) / T(3);
-          P yv[NIN > 0 ? NIN : 1][2];
-#pragma unroll
-          for (int m = 0; m < NIN; ++m) {
-            yv[m][0] = a.in[m][q][o];  // plain loads: in[1] (U2) is the plane this stage overwrites in place
-            yv[m][1] = a.in[m][3 + q][o];
-          }
           auto comb = [&](T y0, T u2, T u3, T u4, T kk) -> T { return fma(a.adt, kk, ((fma(T(2), u3, u2) + u4) - y0) * third); };
           ou = mkpair(comb(yv[0][0].x, yv[1][0].x, yv[2][0].x, uc[0], ku[0]), comb(yv[0][0].y, yv[1][0].y, yv[2][0].y, uc[1], ku[1]));
           odu = mkpair(comb(yv[0][1].x, yv[1][1].x, yv[2][1].x, duc[0], kdu[0]), comb(yv[0][1].y, yv[1][1].y, yv[2][1].y, duc[1], kdu[1]));
