@@ -178,6 +178,30 @@ int sledge_rk_step(sledge_ctx* ctx, double dt, double eta);
  * ceil(n/32) per axis) = number of tagged cells in it; zeroed by the call.  Either may be NULL. */
 int sledge_tag_strings(sledge_ctx* ctx, int level, uint8_t* dev_tags, uint32_t* dev_counts);
 
+/* String tagging with NO allocation anywhere: no context, no arena.  For callers that cannot call cudaMalloc (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  Tags ONE periodic box given as two dense
+ * device arrays -- the same rule, kernel (k_tag_strings) and output layout as sledge_tag_strings on a one-box level 0.
+ *   dev_psi1, dev_psi2 : device, nx*ny*nz reals each of `dtype` (SLEDGE_F32 / SLEDGE_F64), x fastest; read only.
+ *   n                  : HOST, {nx, ny, nz}, each >= 2; the box is periodic in all three directions (L23).
+ *   dev_tags           : device, one byte per cell, x fastest (bit0/1/2 as above); may be NULL.
+ *   dev_counts         : device, uint32 per aligned 32^3 block (x fastest, ceil(n/32) per axis); zeroed by the call;
+ *                        may be NULL.
+ *   cuda_stream        : a cudaStream_t (0 = legacy default stream); the call enqueues on it and returns.
+ * Scratch: the kernel reads pair-interleaved, 128-byte-aligned rows, so the call first packs
+ * the two arrays into that layout -- together with its box / tile tables -- inside a file-scope
+ * `static __device__` array of SLEDGE_STATIC_SCRATCH_BYTES (8 MiB; every GPU that loads the library holds it until the
+ * process exits).  A box whose packed size exceeds it is rejected with SLEDGE_EINVAL and a text that names the limit
+ * (fits: 72^3 in fp64, 88^3 in fp32; bytes = 256 + 20 per tile, rounded up to 256, + 2 * sizeof(real) * pitch *
+ * (ny + 2) * (nz + 2) with pitch = nx + 9 (fp64) / nx + 17 (fp32) cells rounded up to 128 bytes).  The call runs on the device that owns dev_psi1 and
+ * calls no cudaMalloc, cudaFree or allocating library routine, and copies nothing from host memory.
+ * Every call shares the one array per device, which keeps the previous call's contents (everything a call reads it
+ * has written itself first): calls whose kernels may overlap on the GPU (different streams, no ordering between
+ * them) RACE -- order them on one stream or with events.  Errors: SLEDGE_EINVAL (null / non-device pointer, bad n,
+ * dtype, too large), SLEDGE_ECUDA; text by sledge_last_error(NULL). */
+#define SLEDGE_STATIC_SCRATCH_BYTES (8u << 20)
+int sledge_tag_strings_static(const void* dev_psi1, const void* dev_psi2, const int* n, int dtype, uint8_t* dev_tags,
+                              uint32_t* dev_counts, void* cuda_stream);
+
 /* Level synchronisation (L74): every cell of level fine_level-1 covered by fine_level <- mean of its 8
  * children, all four components, on the current states. */
 int sledge_average_down(sledge_ctx* ctx, int fine_level);

@@ -1553,6 +1553,125 @@ int do_copy_comp(sledge_ctx* c, int ib, int comp, void* dense, bool to_state, bo
 }  // namespace
 
 // =================================================================================================
+// sledge_tag_strings_static: K3 on one periodic box with NO allocation (include/sledge.h)
+// =================================================================================================
+namespace {
+
+// The scratch of the no-allocation entry point: the box / tile tables and the packed pair plane k_tag_strings reads.
+// In HOST code this name is only a stand-in for the symbol, not a device address: static_scratch_ptr() asks the
+// runtime for the address once per device (with that device current) and the kernels are given that pointer.
+static __device__ __align__(256) unsigned char g_static_scratch[SLEDGE_STATIC_SCRATCH_BYTES];
+
+struct StaticLayout {  // byte offsets inside g_static_scratch
+  size_t off_box = 0, off_tiles = 256, off_plane = 0, total = 0;
+  int sx = 0, sy = 0, ox = 0, tnz = 0, ntx = 0, nty = 0, ntz = 0;
+  long long plane_cells = 0;
+};
+
+// same row layout as a context with nghost = 1 (make_plan), same z-chunk rule for the tag tiles
+StaticLayout static_layout(const int n[3], int esz) {
+  StaticLayout S;
+  const int g = 1, cpa = 128 / (2 * esz);
+  S.ox = (g + cpa - 1) / cpa * cpa;
+  S.sx = (S.ox + n[0] + g + cpa - 1) / cpa * cpa;
+  S.sy = n[1] + 2 * g;
+  S.plane_cells = (long long)S.sx * S.sy * (n[2] + 2 * g);
+  S.ntx = (n[0] + TAG_TX - 1) / TAG_TX;
+  S.nty = (n[1] + TAG_TY - 1) / TAG_TY;
+  int tnz = K1_NZ;
+  for (; tnz > 32; tnz /= 2)
+    if ((long long)S.ntx * S.nty * ((n[2] + tnz - 1) / tnz) >= TAG_MIN_TILES) break;
+  S.tnz = tnz;
+  S.ntz = (n[2] + tnz - 1) / tnz;
+  S.off_plane = align_up(S.off_tiles + (size_t)S.ntx * S.nty * S.ntz * sizeof(TileDev), ALIGN);
+  S.total = S.off_plane + (size_t)S.plane_cells * 2 * esz;
+  return S;
+}
+
+// Writes everything the tag kernel will read: the BoxDev, the tile table and the valid cells of the pair plane
+// (the periodic one-box tag pass reads no ghost cell, k_tag.cuh `wrap`).  Nothing is left over from an earlier call.
+template <typename T>
+__global__ void k_static_pack(unsigned char* scratch, const StaticLayout S, const int n0, const int n1, const int n2,
+                              const T* __restrict__ psi1, const T* __restrict__ psi2) {
+  using P = typename PairOf<T>::type;
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nth = (long long)gridDim.x * blockDim.x;
+  BoxDev b;
+  b.base = 0;
+  b.n[0] = n0; b.n[1] = n1; b.n[2] = n2;
+  b.lo[0] = b.lo[1] = b.lo[2] = 0;
+  b.sx = S.sx;
+  b.sy = S.sy;
+  b.tag_base = 0;
+  if (tid == 0) *reinterpret_cast<BoxDev*>(scratch + S.off_box) = b;
+  TileDev* const tiles = reinterpret_cast<TileDev*>(scratch + S.off_tiles);
+  const int ntiles = S.ntx * S.nty * S.ntz;
+  for (long long q = tid; q < ntiles; q += nth) {
+    const int ix = (int)(q % S.ntx), iy = (int)((q / S.ntx) % S.nty), iz = (int)(q / ((long long)S.ntx * S.nty));
+    tiles[q] = TileDev{0, ix * TAG_TX, iy * TAG_TY, iz * S.tnz, min(S.tnz, n2 - iz * S.tnz)};
+  }
+  P* const plane = reinterpret_cast<P*>(scratch + S.off_plane);
+  const long long total = (long long)n0 * n1 * n2;
+  for (long long q = tid; q < total; q += nth) {
+    const int i = (int)(q % n0), j = (int)((q / n0) % n1), k = (int)(q / ((long long)n0 * n1));
+    plane[cell_offset(b, 1, S.ox, i, j, k)] = mkpair(psi1[q], psi2[q]);
+  }
+}
+
+// device address of g_static_scratch on `dev` (which must be current): asked for once per device
+int static_scratch_ptr(int dev, unsigned char** out) {
+  static unsigned char* ptr[MAX_DEVICES] = {};
+  if (dev < 0 || dev >= MAX_DEVICES) return fail(nullptr, SLEDGE_EINVAL, "device index %d out of range", dev);
+  if (!ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p)
+      return fail(nullptr, SLEDGE_ECUDA, "cudaGetSymbolAddress(static scratch) on device %d: %s", dev, cudaGetErrorString(e));
+    ptr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = ptr[dev];
+  return SLEDGE_OK;
+}
+
+template <typename T>
+int do_tag_static(int dev, const void* psi1, const void* psi2, const int n[3], uint8_t* tags, uint32_t* counts,
+                  cudaStream_t stream) {
+  const StaticLayout S = static_layout(n, (int)sizeof(T));
+  unsigned char* scratch = nullptr;
+  int rc = static_scratch_ptr(dev, &scratch);
+  if (rc) return rc;
+  const long long cells = (long long)n[0] * n[1] * n[2];
+  const int pgrid = (int)std::min<long long>((cells + 255) / 256, 148 * 16);
+  k_static_pack<T><<<pgrid, 256, 0, stream>>>(scratch, S, n[0], n[1], n[2], static_cast<const T*>(psi1), static_cast<const T*>(psi2));
+  const int nb[3] = {(n[0] + COUNT_BLOCK - 1) / COUNT_BLOCK, (n[1] + COUNT_BLOCK - 1) / COUNT_BLOCK, (n[2] + COUNT_BLOCK - 1) / COUNT_BLOCK};
+  if (counts) cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)nb[0] * nb[1] * nb[2], stream);
+  TagArgs<T> a;
+  memset(&a, 0, sizeof a);
+  a.boxes = reinterpret_cast<const BoxDev*>(scratch + S.off_box);
+  a.tiles = reinterpret_cast<const TileDev*>(scratch + S.off_tiles);
+  a.psi = reinterpret_cast<const typename PairOf<T>::type*>(scratch + S.off_plane);
+  a.tags = tags;
+  a.counts = counts;
+  a.g = 1;
+  a.ox = S.ox;
+  a.wrap = 1;  // one box over the periodic domain: +1 neighbours are read at their wrapped position (L23)
+  a.nb0 = nb[0];
+  a.nb1 = nb[1];
+  a.tag_cells = nullptr;
+  static PerDevice configured_dev;  // per instantiation and device (its own flag: the context path keeps its own)
+  bool& configured = configured_dev[dev];
+  if (!configured) {
+    cudaFuncSetAttribute(k_tag_strings<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
+    configured = true;
+  }
+  k_tag_strings<T><<<S.ntx * S.nty * S.ntz, TAG_THREADS, tag_smem_bytes<T>(), stream>>>(a);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, SLEDGE_ECUDA, "sledge_tag_strings_static: %s", cudaGetErrorString(e));
+  return SLEDGE_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
 // C ABI (include/sledge.h)
 // =================================================================================================
 #define DISPATCH(ctx, call_f32, call_f64) ((ctx)->plan.p.dtype == SLEDGE_F64 ? (call_f64) : (call_f32))
@@ -1849,6 +1968,30 @@ int sledge_tag_strings(sledge_ctx* c, int level, uint8_t* dev_tags, uint32_t* de
   if (rc) return rc;
   DeviceGuard guard(c->device);
   return DISPATCH(c, do_tag<float>(c, level, dev_tags, dev_counts), do_tag<double>(c, level, dev_tags, dev_counts));
+}
+
+int sledge_tag_strings_static(const void* dev_psi1, const void* dev_psi2, const int* n, int dtype, uint8_t* dev_tags,
+                              uint32_t* dev_counts, void* cuda_stream) {
+  if (!dev_psi1 || !dev_psi2 || !n) return fail(nullptr, SLEDGE_EINVAL, "sledge_tag_strings_static: null input");
+  if (dtype != SLEDGE_F32 && dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
+  for (int d = 0; d < 3; ++d)
+    if (n[d] < 2 || n[d] > 32768) return fail(nullptr, SLEDGE_EINVAL, "sledge_tag_strings_static: n[%d] = %d, need 2..32768", d, n[d]);
+  const int esz = dtype == SLEDGE_F64 ? 8 : 4;
+  const StaticLayout S = static_layout(n, esz);
+  if (S.total > (size_t)SLEDGE_STATIC_SCRATCH_BYTES)
+    return fail(nullptr, SLEDGE_EINVAL,
+                "sledge_tag_strings_static: a %d x %d x %d %s box needs %zu bytes of scratch, the static array holds %u "
+                "(SLEDGE_STATIC_SCRATCH_BYTES; fits 72^3 in fp64, 88^3 in fp32): use a context (sledge_create + sledge_tag_strings)",
+                n[0], n[1], n[2], esz == 8 ? "fp64" : "fp32", S.total, (unsigned)SLEDGE_STATIC_SCRATCH_BYTES);
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, dev_psi1) != cudaSuccess || (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)) {
+    cudaGetLastError();
+    return fail(nullptr, SLEDGE_EINVAL, "sledge_tag_strings_static: dev_psi1 is not a device pointer");
+  }
+  DeviceGuard guard(at.device);
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  return esz == 8 ? do_tag_static<double>(at.device, dev_psi1, dev_psi2, n, dev_tags, dev_counts, stream)
+                  : do_tag_static<float>(at.device, dev_psi1, dev_psi2, n, dev_tags, dev_counts, stream);
 }
 
 int sledge_average_down(sledge_ctx* c, int fine_level) {

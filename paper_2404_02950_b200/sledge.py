@@ -24,7 +24,7 @@ SYMBOLS = [
     "sledge_arena_bytes", "sledge_create", "sledge_destroy", "sledge_set_state", "sledge_get_state",
     "sledge_set_state_host", "sledge_get_state_host", "sledge_host_copies_join", "sledge_get_ghosted", "sledge_fill_ghosts",
     "sledge_rk_stage", "sledge_rk_step", "sledge_tag_strings", "sledge_average_down", "sledge_tee_enable",
-    "sledge_shadow_tee", "sledge_level_cells", "sledge_level_storage", "sledge_level_dataflow",
+    "sledge_shadow_tee", "sledge_level_cells", "sledge_level_storage", "sledge_level_dataflow", "sledge_tag_strings_static",
     "sledge_launch_count", "sledge_synchronize", "sledge_profile_enable", "sledge_profile_read",
     "sledge_last_error",
 ]
@@ -74,6 +74,7 @@ def lib():
         L.sledge_rk_stage.argtypes = [vp, i, i, d, d]
         L.sledge_rk_step.argtypes = [vp, d, d]
         L.sledge_tag_strings.argtypes = [vp, i, vp, vp]
+        L.sledge_tag_strings_static.argtypes = [vp, vp, C.POINTER(C.c_int), i, vp, vp, vp]
         L.sledge_average_down.argtypes = [vp, i]
         L.sledge_tee_enable.argtypes = [vp, i, C.POINTER(C.c_double), vp, vp]
         L.sledge_shadow_tee.argtypes = [vp, d, d, C.POINTER(C.c_double), vp, vp]
@@ -144,6 +145,41 @@ def sledge_arena_bytes(n0, boxes=None, n_levels=1, nghost=1, blocking_factor=8, 
     if rc != 0:
         raise SledgeError(f"sledge_arena_bytes: {rc}: {lib().sledge_last_error(None).decode()}")
     return int(out.value)
+
+
+STATIC_SCRATCH_BYTES = 8 << 20  # SLEDGE_STATIC_SCRATCH_BYTES of include/sledge.h
+
+
+def tag_strings_static(psi1: torch.Tensor, psi2: torch.Tensor, tags: torch.Tensor | None = None,
+                       counts: torch.Tensor | None = None, stream=None):
+    """sledge_tag_strings_static: string tags of ONE periodic box given as two dense CUDA tensors [z, y, x] (fp32 or
+    fp64), with no context and no arena -- the library allocates nothing (its scratch is a static device array of
+    8 MiB: up to 72^3 in fp64, 88^3 in fp32).  Pass `tags` (uint8 [z, y, x]) and `counts` (int32 [bz, by, bx], 32^3
+    blocks) to keep this call free of allocations too; tensors created here are the binding's, not the library's.
+    Calls that may overlap on the GPU share the scratch array and race: keep them on one stream."""
+    if psi1.shape != psi2.shape or psi1.dim() != 3 or psi1.dtype != psi2.dtype or not psi1.is_cuda or not psi2.is_cuda:
+        raise SledgeError("tag_strings_static: psi1, psi2 must be CUDA tensors [z, y, x] of the same shape and dtype")
+    if not (psi1.is_contiguous() and psi2.is_contiguous()):
+        raise SledgeError("tag_strings_static: dense contiguous tensors expected")
+    if psi1.dtype not in (torch.float32, torch.float64):
+        raise SledgeError("tag_strings_static: fp32 or fp64 only")
+    nz, ny, nx = (int(v) for v in psi1.shape)
+    nb = tuple((v + COUNT_BLOCK - 1) // COUNT_BLOCK for v in (nz, ny, nx))
+    if tags is None:
+        tags = torch.empty((nz, ny, nx), dtype=torch.uint8, device=psi1.device)
+    if counts is None:
+        counts = torch.empty(nb, dtype=torch.int32, device=psi1.device)
+    if tags.numel() != nz * ny * nx or tags.dtype != torch.uint8 or counts.numel() != nb[0] * nb[1] * nb[2] \
+            or counts.dtype != torch.int32 or not tags.is_contiguous() or not counts.is_contiguous():
+        raise SledgeError("tag_strings_static: tags must be uint8 [z, y, x], counts int32 [ceil(n/32)] per axis")
+    n = (C.c_int * 3)(nx, ny, nz)
+    st = torch.cuda.current_stream(psi1.device) if stream is None else stream
+    rc = lib().sledge_tag_strings_static(psi1.data_ptr(), psi2.data_ptr(), n,
+                                         SLEDGE_F64 if psi1.dtype == torch.float64 else SLEDGE_F32,
+                                         tags.data_ptr(), counts.data_ptr(), st.cuda_stream)
+    if rc != 0:
+        raise SledgeError(f"sledge_tag_strings_static: {rc}: {lib().sledge_last_error(None).decode()}")
+    return tags, counts
 
 
 class Sledge:
