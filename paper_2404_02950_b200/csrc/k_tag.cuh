@@ -107,10 +107,15 @@ __device__ __forceinline__ unsigned tag_differs(unsigned a, unsigned b) {
 }
 
 #ifndef SLEDGE_TAG_MINB
-#define SLEDGE_TAG_MINB 1
+#define SLEDGE_TAG_MINB 3  // <= 168 registers: three CTAs of four warps per SM (fp64 needs 182 without the cap; no spills with it)
 #endif
-template <typename T>
-__global__ void __launch_bounds__(TAG_THREADS, SLEDGE_TAG_MINB) k_tag_strings(const TagArgs<T> a) {
+#ifndef SLEDGE_TAG_MINB_LOOKUP
+#define SLEDGE_TAG_MINB_LOOKUP SLEDGE_TAG_MINB
+#endif
+// LOOKUP: tiles over storage boxes, tag addresses through a.tag_cells (its own instantiation: the extra registers must
+// not cost the plain pass its third CTA per SM)
+template <typename T, bool LOOKUP = false>
+__global__ void __launch_bounds__(TAG_THREADS, LOOKUP ? SLEDGE_TAG_MINB_LOOKUP : SLEDGE_TAG_MINB) k_tag_strings(const TagArgs<T> a) {
   using P = typename PairOf<T>::type;
   constexpr int RY = TAG_RY;
   const TileDev t = a.tiles[blockIdx.x];
@@ -185,7 +190,7 @@ __global__ void __launch_bounds__(TAG_THREADS, SLEDGE_TAG_MINB) k_tag_strings(co
   long long tag_plane = (long long)b.n[1] * b.n[0];
   int tag_row = b.n[0];
   // lookup mode: this lane's column of blocking-factor cells (x and y cell fixed, z varies), next entry prefetched
-  const bool lookup = a.tag_cells != nullptr && a.tags != nullptr;
+  const bool lookup = LOOKUP && a.tags != nullptr;
   const int bfm = (1 << a.bfs) - 1;
   const int gx = b.lo[0] + min(x, b.n[0] - 1), gy = b.lo[1] + y0;
   const int4* cellp = nullptr;

@@ -66,7 +66,11 @@ constexpr int K1_DMAX = SLEDGE_K1_DMAX;          // cp.async ring: deepest that 
 constexpr size_t K1_SMEM = SLEDGE_K1_SMEM;       // shared-memory budget per CTA (227 KB = sm_100a opt-in limit)
 constexpr long long K1F_MIN_TILES = 3500;
 static_assert(GW_TY == SLEDGE_K1F_TY && GW_TX == SLEDGE_K1F_TX, "k_gw_stage runs over the fused-sweep tiles");
-constexpr long long TAG_MIN_TILES = 148 * 4 * 6;  // below this many CTAs the tag pass halves its z-chunk (down to 32 planes)  // below this many CTAs the fused sweeps halve their z-chunk
+#ifndef SLEDGE_TAG_MIN_NZ
+#define SLEDGE_TAG_MIN_NZ 16
+#endif
+constexpr int TAG_MIN_NZ = SLEDGE_TAG_MIN_NZ;  // shortest z-chunk of a tag tile
+constexpr long long TAG_MIN_TILES = 148 * 4 * 6;  // below this many CTAs the tag pass halves its z-chunk (down to TAG_MIN_NZ planes)  // below this many CTAs the fused sweeps halve their z-chunk
 constexpr int K1F_TY = SLEDGE_K1F_TY;            // tile rows / budget of the FUSED sweeps
 constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
 // which on-chip data path a sweep uses: 1 = k_rk_plane (ghosted plane ring), 0 = k_rk_pipe (ring + centre plane)
@@ -584,7 +588,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
     const int fnz = ft_long >= K1F_MIN_TILES ? K1_NZ : K1_NZ / 2;
     // z-chunk of the tag pass (K3): a tile costs one extra plane, but the grid should be several waves of 148 SMs x 4 CTAs
     int tnz = K1_NZ;
-    for (; tnz > 32; tnz /= 2) {
+    for (; tnz > TAG_MIN_NZ; tnz /= 2) {
       long long nt = 0;
       for (const BoxDev& b : (L.viewdev.size() != L.boxdev.size() && bf >= TAG_RY) ? L.boxdev : L.viewdev)
         nt += (long long)((b.n[0] + TAG_TX - 1) / TAG_TX) * ((b.n[1] + TAG_TY - 1) / TAG_TY) * ((b.n[2] + tnz - 1) / tnz);
@@ -1524,10 +1528,12 @@ int do_tag(sledge_ctx* c, int l, uint8_t* tags, uint32_t* counts) {
     static PerDevice configured_dev;  // per instantiation and device
     bool& configured = configured_dev[c->device];
     if (!configured) {
-      cudaFuncSetAttribute(k_tag_strings<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
+      cudaFuncSetAttribute(k_tag_strings<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
+      cudaFuncSetAttribute(k_tag_strings<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
       configured = true;
     }
-    k_tag_strings<T><<<(int)L.tag_tiles.size(), TAG_THREADS, tag_smem_bytes<T>(), c->stream>>>(a);
+    if (tag_lookup) k_tag_strings<T, true><<<(int)L.tag_tiles.size(), TAG_THREADS, tag_smem_bytes<T>(), c->stream>>>(a);
+    else k_tag_strings<T, false><<<(int)L.tag_tiles.size(), TAG_THREADS, tag_smem_bytes<T>(), c->stream>>>(a);
   }
   return check_launch(c, "k_tag_strings");
 }
@@ -1579,7 +1585,7 @@ StaticLayout static_layout(const int n[3], int esz) {
   S.ntx = (n[0] + TAG_TX - 1) / TAG_TX;
   S.nty = (n[1] + TAG_TY - 1) / TAG_TY;
   int tnz = K1_NZ;
-  for (; tnz > 32; tnz /= 2)
+  for (; tnz > TAG_MIN_NZ; tnz /= 2)
     if ((long long)S.ntx * S.nty * ((n[2] + tnz - 1) / tnz) >= TAG_MIN_TILES) break;
   S.tnz = tnz;
   S.ntz = (n[2] + tnz - 1) / tnz;
@@ -1660,10 +1666,10 @@ int do_tag_static(int dev, const void* psi1, const void* psi2, const int n[3], u
   static PerDevice configured_dev;  // per instantiation and device (its own flag: the context path keeps its own)
   bool& configured = configured_dev[dev];
   if (!configured) {
-    cudaFuncSetAttribute(k_tag_strings<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
+    cudaFuncSetAttribute(k_tag_strings<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tag_smem_bytes<T>());
     configured = true;
   }
-  k_tag_strings<T><<<S.ntx * S.nty * S.ntz, TAG_THREADS, tag_smem_bytes<T>(), stream>>>(a);
+  k_tag_strings<T, false><<<S.ntx * S.nty * S.ntz, TAG_THREADS, tag_smem_bytes<T>(), stream>>>(a);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(nullptr, SLEDGE_ECUDA, "sledge_tag_strings_static: %s", cudaGetErrorString(e));
   return SLEDGE_OK;
