@@ -72,7 +72,8 @@ def parse():
     ap.add_argument("--no-others", action="store_true",
                     help="skip the short runs of the other BASELINE.json workloads (key other_workloads) and the C5 graph leg")
     ap.add_argument("--other-steps", type=int, default=4)
-    ap.add_argument("--e2e-steps", type=int, default=4)
+    ap.add_argument("--e2e-steps", type=int, default=0,
+                    help="steps of the end-to-end leg (host buffers); 0 = as many as --steps, at least 4 and at most 20")
     return ap.parse_args()
 
 
@@ -691,11 +692,16 @@ def e2e_leg(args, cfg, s, boxes, cell_steps, world, step_tags):
     return {"value": whole_job_value(world, cell_steps, ms, stages={3: 3, 10: 3, 20: len(RKN4["nodes"])}.get(args.integrator, 4)),
             "unit": UNIT, "ms_per_step": ms,
             "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "steps": args.e2e_steps,
-            "what": "sledge_set_state_host x4/box + sledge_rk_step + sledge_tag_strings + sledge_get_state_host x4/box + counts"}
+            "what": "sledge_set_state_host x4/box + sledge_rk_step + sledge_tag_strings + sledge_get_state_host x4/box + counts",
+            "note": "every step uploads and downloads the whole state; the library's two copy streams let the downloads of "
+                    "step k overlap the uploads of step k+1 (PCIe is full duplex), so the first upload and the last download "
+                    "are the only unoverlapped ones and ms_per_step falls towards the one-direction copy time as steps grows"}
 
 
 def main():
     args = parse()
+    if args.e2e_steps <= 0:
+        args.e2e_steps = min(max(args.steps, 4), 20)
     from paper_2404_02950_b200 import inputs
     cfg = inputs.CONFIGS[args.workload]
     if args.impl == "reference":
