@@ -126,7 +126,7 @@ int sledge_destroy(sledge_ctx* ctx);
 int sledge_set_state(sledge_ctx* ctx, int box, int comp, const void* dev_src);
 int sledge_get_state(sledge_ctx* ctx, int box, int comp, void* dev_dst);
 /* Same with HOST buffers (pinned memory for truly asynchronous copies).  The library stages through slots inside
- * the arena, two per direction, and runs the host<->device copies on two streams of its own, ordered against the
+ * the arena (two for uploads, four for downloads) and runs the host<->device copies on two streams of its own, ordered against the
  * context stream with events: the upload of component c+1 overlaps the repacking kernel of c, downloads drain while
  * the context stream goes on, and the downloads of one step overlap the uploads of the next (PCIe is full duplex).
  * Ordering seen by the caller is that of the context stream: a set is complete for every later call on the context;

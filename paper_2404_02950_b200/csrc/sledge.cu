@@ -188,6 +188,8 @@ struct Plan {
 
 }  // namespace
 
+constexpr int N_IN_SLOTS = 2, N_OUT_SLOTS = 4;  // staging slots of the host-buffer copies (one box component each)
+
 struct sledge_ctx {
   Plan plan;
   char* arena = nullptr;
@@ -201,9 +203,11 @@ struct sledge_ctx {
   // host-buffer copies (sledge_set_state_host / get_state_host) run on two streams of their own, double-buffered through
   // the staging slots, so that uploads, repacking kernels and downloads overlap (PCIe is full duplex)
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
-  cudaEvent_t ev_in_ready[2] = {nullptr, nullptr}, ev_in_free[2] = {nullptr, nullptr};
-  cudaEvent_t ev_out_ready[2] = {nullptr, nullptr}, ev_out_free[2] = {nullptr, nullptr};
-  bool in_used[2] = {false, false}, out_used[2] = {false, false};
+  // two upload slots; four download slots, so that the repacking kernels of a whole state's downloads never wait on
+  // the context stream (ahead of the next step's uploads) for a PCIe copy to drain a slot
+  cudaEvent_t ev_in_ready[N_IN_SLOTS] = {}, ev_in_free[N_IN_SLOTS] = {};
+  cudaEvent_t ev_out_ready[N_OUT_SLOTS] = {}, ev_out_free[N_OUT_SLOTS] = {};
+  bool in_used[N_IN_SLOTS] = {}, out_used[N_OUT_SLOTS] = {};
   unsigned n_in = 0, n_out = 0;
   int device = 0;  // the device the arena lives on: every entry point runs with it current (DeviceGuard)
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[4];
@@ -685,7 +689,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
       if (L.n[d] + 2 * g >= 65536) return fail(nullptr, SLEDGE_EINVAL, "level %d: more than 65535 cells per axis", l);
   }
   P.scratch_bytes = max_box_cells * P.esz;
-  P.off_scratch = take(P.scratch_bytes * 4);  // host copies: two staging slots per direction (in 0, 1; out 2, 3)
+  P.off_scratch = take(P.scratch_bytes * 6);  // host copies: staging slots in 0, 1; out 2 .. 5 (N_IN_SLOTS, N_OUT_SLOTS)
   P.off_err = take(sizeof(int));
   if (p.shadow_level) {  // L98: level 0 coarsened by 2, ONE box over the same periodic domain
     sledge_params sp = p;
@@ -1811,9 +1815,11 @@ int sledge_destroy(sledge_ctx* c) {
   if (c->s_h2d) {
     cudaStreamSynchronize(c->s_h2d);
     cudaStreamSynchronize(c->s_d2h);
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < N_IN_SLOTS; ++k) {
       cudaEventDestroy(c->ev_in_ready[k]);
       cudaEventDestroy(c->ev_in_free[k]);
+    }
+    for (int k = 0; k < N_OUT_SLOTS; ++k) {
       cudaEventDestroy(c->ev_out_ready[k]);
       cudaEventDestroy(c->ev_out_free[k]);
     }
@@ -1872,10 +1878,12 @@ static int host_streams(sledge_ctx* c) {
   if (c->s_h2d) return SLEDGE_OK;
   cudaError_t e = cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking);
   if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking);
-  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+  for (int k = 0; k < N_IN_SLOTS && e == cudaSuccess; ++k) {
     e = cudaEventCreateWithFlags(&c->ev_in_ready[k], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_in_free[k], cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_out_ready[k], cudaEventDisableTiming);
+  }
+  for (int k = 0; k < N_OUT_SLOTS && e == cudaSuccess; ++k) {
+    e = cudaEventCreateWithFlags(&c->ev_out_ready[k], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_out_free[k], cudaEventDisableTiming);
   }
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "host copy streams: %s", cudaGetErrorString(e));
@@ -1887,7 +1895,7 @@ int sledge_set_state_host(sledge_ctx* c, int box, int comp, const void* host_src
   if (rc) return rc;
   DeviceGuard guard(c->device);
   if ((rc = host_streams(c)) != SLEDGE_OK) return rc;
-  const int k = (int)(c->n_in++ & 1u);
+  const int k = (int)(c->n_in++ % (unsigned)N_IN_SLOTS);
   void* slot = c->arena + c->plan.off_scratch + (size_t)k * c->plan.scratch_bytes;
   cudaError_t e = cudaSuccess;
   if (c->in_used[k]) e = cudaStreamWaitEvent(c->s_h2d, c->ev_in_free[k], 0);  // the slot's last repack has read it
@@ -1908,8 +1916,8 @@ int sledge_get_state_host(sledge_ctx* c, int box, int comp, void* host_dst) {
   if (rc) return rc;
   DeviceGuard guard(c->device);
   if ((rc = host_streams(c)) != SLEDGE_OK) return rc;
-  const int k = (int)(c->n_out++ & 1u);
-  void* slot = c->arena + c->plan.off_scratch + (size_t)(2 + k) * c->plan.scratch_bytes;
+  const int k = (int)(c->n_out++ % (unsigned)N_OUT_SLOTS);
+  void* slot = c->arena + c->plan.off_scratch + (size_t)(N_IN_SLOTS + k) * c->plan.scratch_bytes;
   cudaError_t e = cudaSuccess;
   if (c->out_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_out_free[k], 0);  // the slot's last download is done
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "get_state_host: %s", cudaGetErrorString(e));
@@ -1928,10 +1936,10 @@ int sledge_host_copies_join(sledge_ctx* c) {
   if (!c) return fail(nullptr, SLEDGE_EINVAL, "null context");
   DeviceGuard guard(c->device);
   cudaError_t e = cudaSuccess;
-  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+  for (int k = 0; k < N_OUT_SLOTS && e == cudaSuccess; ++k)
     if (c->out_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_out_free[k], 0);
-    if (e == cudaSuccess && c->in_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_in_free[k], 0);
-  }
+  for (int k = 0; k < N_IN_SLOTS && e == cudaSuccess; ++k)
+    if (c->in_used[k]) e = cudaStreamWaitEvent(c->stream, c->ev_in_free[k], 0);
   if (e != cudaSuccess) return fail(c, SLEDGE_ECUDA, "host_copies_join: %s", cudaGetErrorString(e));
   return SLEDGE_OK;
 }
