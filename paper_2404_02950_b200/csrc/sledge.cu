@@ -930,16 +930,17 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
   if (a.quartic == 2 && l > 0 && qgrid > 0 && star_only) {  // only the parents with star children, packed
     a.qlist = a.qstar_list;
     a.n_qentries = c->plan.lev[l].n_star_parents;
-    qgrid = (int)((a.n_qentries + GHOST_THREADS - 1) / GHOST_THREADS);
   }
   if (a.quartic == 2 && l > 0 && qgrid > 0) {  // the interpolated cells, one thread per coarse parent
+    qgrid = (int)((a.n_qentries + QP_THREADS - 1) / QP_THREADS);
     Timed t(c, KIND_GHOST);
     if (a.single) {
-      if (fill_pi) k_fill_qparents<T, true, true><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
-      else k_fill_qparents<T, false, true><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+      if (fill_pi) k_fill_qparents<T, true, true><<<qgrid, QP_THREADS, 0, c->stream>>>(a);
+      else k_fill_qparents<T, false, true><<<qgrid, QP_THREADS, 0, c->stream>>>(a);
     } else {
-      if (fill_pi) k_fill_qparents<T, true, false><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
-      else k_fill_qparents<T, false, false><<<qgrid, GHOST_THREADS, 0, c->stream>>>(a);
+      if (fill_pi && a.vel) k_fill_qparents<T, true, false, true><<<qgrid, QP_THREADS, 0, c->stream>>>(a);
+      else if (fill_pi) k_fill_qparents<T, true, false><<<qgrid, QP_THREADS, 0, c->stream>>>(a);
+      else k_fill_qparents<T, false, false><<<qgrid, QP_THREADS, 0, c->stream>>>(a);
     }
     rc = check_launch(c, "k_fill_qparents");
   }

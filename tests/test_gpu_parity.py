@@ -385,9 +385,11 @@ def test_ghost_fill_time_interpolation():
 
 @pytest.mark.parametrize("g", [1, 2, 3])
 def test_quartic_ghost_fill_two_levels_matches_oracle_bitwise(g):
-    """5^3 parents per ghost cell.  g = 1: fast entries (window inside one coarse box) and the periodic / multi-box slow
-    path; g >= 2: windows read through the coarse boxes' ghost cells.  Same summation order and individually rounded
-    operations on both sides -> identical bits"""
+    """5^3 parents per ghost cell.  g = 1: per-cell entries (fast: window inside one coarse box; slow: periodic /
+    multi-box), same summation order and individually rounded operations on both sides -> identical bits.  g >= 2: by
+    coarse parent through the coarse boxes' ghost cells, evaluated separably (x, y, z passes): equal
+    to the oracle's direct triple sum up to rounding order -> a few ulp of values of order 1, far inside the 1e-11 bar
+    of BASELINE.json's north_star."""
     P = _pair()
     n0 = 32
     boxes = P.two_level_boxes(n0)
@@ -401,7 +403,10 @@ def test_quartic_ghost_fill_two_levels_matches_oracle_bitwise(g):
         for c in range(4):
             a = o.get_raw(ib, c)
             b = s.get_ghosted(ib, c).cpu().numpy()
-            assert np.array_equal(a, b), (ib, c)
+            if g == 1:
+                assert np.array_equal(a, b), (ib, c)
+            else:
+                assert np.abs(a - b).max() <= 1e-14 * max(1.0, float(np.abs(a).max())), (ib, c)
 
 
 def test_quartic_differs_from_trilinear_on_the_gpu():
