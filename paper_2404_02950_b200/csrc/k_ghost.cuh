@@ -88,7 +88,8 @@ struct GhostArgs {
   // state interpolated at the later stage time (L72).  The space-time interpolant I_psi(t) is linear in t between the
   // coarse old and new states, so its time derivative is I[psi_new - psi_old] / (t_new - t_old) whatever the two stage
   // times are: Pi_g <- I[psi_new - psi_old] * vel_c (0 while the coarse level holds one state only).
-  int vel;
+  int vel;  // 1: velocity ghosts; 2: the second plane holds W = psi_Y + psi(U4) (FUSED_A2 / FUSED_B2 sweeps, fill before
+            // sweep B): W_g = I_psi(t) + I_psi(t + dt) = 2 I_psi(t + dt/2) = twice the first plane's ghost value
   T vel_c;  // 1 / (t_new - t_old) of the coarse level
   int patch_smem_pairs;    // shared-memory pairs per warp and plane (largest coarse region of an interpolation patch)
 };
@@ -627,9 +628,9 @@ __global__ void __launch_bounds__(QP_THREADS, SLEDGE_QP_MINB) k_fill_qparents(co
         v[mx][0] = SINGLE ? vo[mx].x : oma * vo[mx].x + a.alpha * vn[mx].x;
         v[mx][1] = SINGLE ? vo[mx].y : oma * vo[mx].y + a.alpha * vn[mx].y;
         if (FILL_PI) {
-          if (VEL) {  // velocity ghosts (host: never SINGLE)
-            v[mx][NQ - 2] = SINGLE ? T(0) : (vn[mx].x - vo[mx].x) * a.vel_c;
-            v[mx][NQ - 1] = SINGLE ? T(0) : (vn[mx].y - vo[mx].y) * a.vel_c;
+          if (VEL) {  // velocity ghosts, or W = twice the first plane (host: never SINGLE)
+            v[mx][NQ - 2] = SINGLE ? T(0) : (a.vel == 2 ? T(2) * v[mx][0] : (vn[mx].x - vo[mx].x) * a.vel_c);
+            v[mx][NQ - 1] = SINGLE ? T(0) : (a.vel == 2 ? T(2) * v[mx][1] : (vn[mx].y - vo[mx].y) * a.vel_c);
           } else {
             v[mx][NQ - 2] = SINGLE ? po[mx].x : oma * po[mx].x + a.alpha * pn[mx].x;
             v[mx][NQ - 1] = SINGLE ? po[mx].y : oma * po[mx].y + a.alpha * pn[mx].y;
@@ -828,7 +829,7 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
       const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
       a.psi[d] = mkpair(s0, s1);
       // velocity ghosts: Pi <- I[psi_new - psi_old] / (t_new - t_old) (0 while the coarse level has one state only)
-      if (FILL_PI) a.pi[d] = vel ? mkpair(t0 * a.vel_c, t1 * a.vel_c) : mkpair(t0, t1);
+      if (FILL_PI) a.pi[d] = vel ? (a.vel == 2 ? mkpair(T(2) * s0, T(2) * s1) : mkpair(t0 * a.vel_c, t1 * a.vel_c)) : mkpair(t0, t1);
     }
     return;
   }
@@ -849,7 +850,10 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
     const unsigned d = A.x + (unsigned)(k * dpl + j * dsx + i);
     a.psi[d] = interp_coarse<T>(a.c_old_psi, a.c_new_psi, a.alpha, o);
     if (FILL_PI) {
-      if (a.vel) {
+      if (a.vel == 2) {
+        const P pv = a.psi[d];  // just written by this thread
+        a.pi[d] = mkpair(T(2) * pv.x, T(2) * pv.y);
+      } else if (a.vel) {
         const P dv = interp_coarse_diff<T>(a.c_old_psi, a.c_new_psi, o);
         a.pi[d] = mkpair(dv.x * a.vel_c, dv.y * a.vel_c);
       } else {

@@ -42,6 +42,8 @@ enum StageMode {
   FUSED_A = 6,
   FUSED_B = 7,
   SSP_S23 = 8,  // SSPRK3 (integrator.type 3 / 10, L808) stages 2 and 3: out = wy Y + wu (U + dt k(U)); stage 1 = LEAN_S1
+  FUSED_A2 = 10,  // fp64 FUSED sweeps, "W" form (see rk_cell): sweep A stores W = 2 psi_Y + dt Pi_3 in place of Pi_3,
+  FUSED_B2 = 11,  // so that sweep B differences two fields (psi_3, W) instead of three (psi_3, Pi_3, psi_Y)
   RKN_ST = 9    // one stage of a user-defined Runge-Kutta-Nystrom scheme (integrator.type 20, L808-815): f = f(Psi_i), and
                 // two linear combinations of psi_n, Pi_n, f_1 .. f_4 and f (the stage's f and the next stage field, or
                 // the new psi and Pi)
@@ -59,10 +61,13 @@ template <> struct ModeInfo<SSP_S23> { static constexpr int NF = 1, NP = 3, NOUT
 template <> struct ModeInfo<RKN_ST> { static constexpr int NF = 1, NP = 6, NOUT = 1; };
 template <> struct ModeInfo<FUSED_A> { static constexpr int NF = 2, NP = 0, NOUT = 1; };
 template <> struct ModeInfo<FUSED_B> { static constexpr int NF = 3, NP = 1, NOUT = 1; };
+template <> struct ModeInfo<FUSED_A2> { static constexpr int NF = 2, NP = 0, NOUT = 1; };
+template <> struct ModeInfo<FUSED_B2> { static constexpr int NF = 2, NP = 2, NOUT = 1; };
 
 // Field roles.  Unfused modes: sten[0] = psi(U); pnt[0] = Pi(U); pnt[1+2q], pnt[2+2q] = psi, Pi of input q
 // (LEAN: q0 = Y, q1 = U2, q2 = U3; CLASSIC: q0 = Y (S23) or ACC (S4), q1 = ACC).
 // FUSED_A: sten = {psi_Y, Pi_Y}.  FUSED_B: sten = {psi_3, Pi_3, psi_Y}, pnt[0] = Pi_Y.
+// FUSED_A2: as FUSED_A, second output plane = W.  FUSED_B2: sten = {psi_3, W}, pnt = {psi_Y, Pi_Y}, wu = 1 / dt.
 template <typename T>
 struct PipeArgs {
   using P = typename PairOf<T>::type;
@@ -161,10 +166,11 @@ __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[Mod
                                         typename PairOf<T>::type (&opi)[ModeInfo<MODE>::NOUT],
                                         const T* ko = nullptr) {
   using P = typename PairOf<T>::type;
-  static_assert(!HASKO || (MODE != FUSED_A && MODE != FUSED_B), "the fused sweeps rely on k_psi = Pi being pointwise");
+  static_assert(!HASKO || (MODE != FUSED_A && MODE != FUSED_B && MODE != FUSED_A2 && MODE != FUSED_B2),
+                "the fused sweeps rely on k_psi = Pi being pointwise");
   constexpr int NP = ModeInfo<MODE>::NP, NOUT = ModeInfo<MODE>::NOUT;
   constexpr int NPA = NP > 0 ? NP : 1;
-  if (MODE == FUSED_A) {
+  if (MODE == FUSED_A || MODE == FUSED_A2) {
     // stages 1 + 2 (O4): U3 = Y + dt/2 k(U2), U2 = Y + dt/2 k(Y); U2 is never stored
     const T hdt = T(0.5) * a.adt;
     const T y1 = wc[0].x, y2 = wc[0].y, q1 = wc[1].x, q2 = wc[1].y;
@@ -178,7 +184,32 @@ __device__ __forceinline__ void rk_cell(const PipeArgs<T>& a, const T (&lap)[Mod
     const T k2a = kpi_of(l2a, u2a, pot2, a.fric[1], p2a);
     const T k2b = kpi_of(l2b, u2b, pot2, a.fric[1], p2b);
     opsi[0] = mkpair(fma(hdt, p2a, y1), fma(hdt, p2b, y2));
-    opi[0] = mkpair(fma(hdt, k2a, q1), fma(hdt, k2b, q2));
+    const T p3a = fma(hdt, k2a, q1), p3b = fma(hdt, k2b, q2);  // Pi(U3)
+    if (MODE == FUSED_A) opi[0] = mkpair(p3a, p3b);
+    else opi[0] = mkpair(fma(a.adt, p3a, T(2) * y1), fma(a.adt, p3b, T(2) * y2));  // W = psi_Y + psi(U4)
+  } else if (MODE == FUSED_B2) {
+    // Stages 3 + 4 and the final combination from psi_3, W = 2 psi_Y + dt Pi_3 (differenced) and Y (pointwise):
+    //   psi(U4) = psi_Y + dt Pi_3 = W - psi_Y,   Pi_3 = (W - 2 psi_Y) / dt  (cancellation: eps |W| / dt absolute, which
+    //   enters Ynew with factors <= 2/3: rounding level in fp64; the reason this form is not used in fp32),
+    //   k1_Pi + k4_Pi = Lap(psi_Y) + Lap(psi(U4)) + pointwise terms = Lap(W) + ...: Lap psi_Y alone is never needed,
+    //   dt/6 2 k2 = 2/3 (U3 - Y) for both components (U3 = Y + dt/2 k2).
+    const T dt = a.adt, sixth = a.adt / T(6), inv_dt = a.wu, twothirds = T(2) / T(3);
+    const T u3a = wc[0].x, u3b = wc[0].y, wa = wc[1].x, wb = wc[1].y;
+    const T y1 = pc[0].x, y2 = pc[0].y, q1 = pc[NPA > 1 ? 1 : 0].x, q2 = pc[NPA > 1 ? 1 : 0].y;
+    const T p3a = (wa - T(2) * y1) * inv_dt, p3b = (wb - T(2) * y2) * inv_dt;  // Pi(U3)
+    const T u4a = wa - y1, u4b = wb - y2;                                      // psi(U4)
+    const T pot3 = pot_of(a.lam_eta2[1], a.a_mass, u3a, u3b);
+    const T k3a = kpi_of(lap[0][0], u3a, pot3, a.fric[1], p3a);
+    const T k3b = kpi_of(lap[0][1], u3b, pot3, a.fric[1], p3b);
+    const T p4a = fma(dt, k3a, q1), p4b = fma(dt, k3b, q2);  // Pi(U4)
+    const T pot4 = pot_of(a.lam_eta2[2], a.a_mass, u4a, u4b);
+    const T pot1 = pot_of(a.lam_eta2[0], a.a_mass, y1, y2);
+    const T k14a = fma(-a.fric[2], p4a, fma(-u4a, pot4, kpi_of(lap[1][0], y1, pot1, a.fric[0], q1)));  // k1 + k4
+    const T k14b = fma(-a.fric[2], p4b, fma(-u4b, pot4, kpi_of(lap[1][1], y2, pot1, a.fric[0], q2)));
+    opsi[0] = mkpair(fma(sixth, (q1 + p4a) + T(2) * p3a, fma(twothirds, u3a - y1, y1)),
+                     fma(sixth, (q2 + p4b) + T(2) * p3b, fma(twothirds, u3b - y2, y2)));
+    opi[0] = mkpair(fma(sixth, fma(T(2), k3a, k14a), fma(twothirds, p3a - q1, q1)),
+                    fma(sixth, fma(T(2), k3b, k14b), fma(twothirds, p3b - q2, q2)));
   } else if (MODE == FUSED_B) {
     // stages 3 + 4 and the final combination; k1 recomputed from Y (same expression, same bits as in
     // PASS A), dt/2 k2 = Pi3 - Pi_Y

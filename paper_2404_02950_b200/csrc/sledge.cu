@@ -98,14 +98,17 @@ constexpr size_t K1F_SMEM = SLEDGE_K1F_SMEM;
 #ifndef SLEDGE_K1F_MINB_B
 #define SLEDGE_K1F_MINB_B 2
 #endif
+#ifndef SLEDGE_K1F_MINB_B2
+#define SLEDGE_K1F_MINB_B2 2
+#endif
 template <int MODE> struct K1Shape {
-  static constexpr bool fused = (MODE == FUSED_A || MODE == FUSED_B);
+  static constexpr bool fused = (MODE == FUSED_A || MODE == FUSED_B || MODE == FUSED_A2 || MODE == FUSED_B2);
   static constexpr int TY = fused ? K1F_TY : K1_TY;
   static constexpr size_t SMEM = fused ? K1F_SMEM : K1_SMEM;
   static constexpr bool plane = fused ? (SLEDGE_K1F_PLANE != 0) : (SLEDGE_K1_PLANE != 0);
   static constexpr int PDMAX = fused ? SLEDGE_K1F_PDMAX : 3;
   static constexpr int RY = fused ? SLEDGE_K1F_RY : SLEDGE_K1_RY;  // rows per thread (k_rk_plane)
-  static constexpr int MINB = MODE == FUSED_A ? SLEDGE_K1F_MINB_A : (MODE == FUSED_B ? SLEDGE_K1F_MINB_B : 1);
+  static constexpr int MINB = (MODE == FUSED_A || MODE == FUSED_A2) ? SLEDGE_K1F_MINB_A : (MODE == FUSED_B ? SLEDGE_K1F_MINB_B : (MODE == FUSED_B2 ? SLEDGE_K1F_MINB_B2 : 1));
 };
 
 // rows per thread of the FUSED sweeps (k_rk_plane / k_rk_tma); the tensor maps' box shape follows from it
@@ -198,6 +201,7 @@ struct sledge_ctx {
   int64_t launches = 0;
   bool profiling = false;
   bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
+  bool fused_w = true;  // fp64 FUSED sweeps in the W form (SLEDGE_FUSED_W=0 selects the three-field sweep B)
   bool use_patches = true;  // fills before an RK sweep by region (SLEDGE_K2_PATCHES=0 selects the packed per-cell list)
   sledge_ctx* shadow = nullptr;  // the shadow level's context (shadow_level = 1)
   // host-buffer copies (sledge_set_state_host / get_state_host) run on two streams of their own, double-buffered through
@@ -780,6 +784,7 @@ LevelGeom geom_of(const Plan& P, int l) {
 // K2 arguments for buffer `buf` of level l, whose data is at time `time`
 struct VelFill {  // velocity ghosts of the second plane between the times ta and tb (FUSED sweeps on a fine level)
   bool on = false;
+  bool w = false;  // the second plane holds W (FUSED_B2): ghost = twice the first plane's
   double ta = 0, tb = 0;
 };
 
@@ -836,7 +841,7 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, 
       bo = pair ? C.old : C.cur;
       bn = C.cur;
       a.single = 0;
-      a.vel = 1;
+      a.vel = vf.w ? 2 : 1;
       a.vel_c = (T)(pair ? 1.0 / (C.t_new - C.t_old) : 0.0);
     }
     a.c_old_psi = plane_ptr<T>(c, l - 1, bo, wa);
@@ -1093,6 +1098,12 @@ cudaError_t launch_pipe_mode(sledge_ctx* c, const PipeArgs<T>& a, int grid, int 
     case SSP_S23: return launch_pipe_kernel<T, ORDER, SSP_S23>(c, a, grid);
     case RKN_ST: return launch_pipe_kernel<T, ORDER, RKN_ST>(c, a, grid);
     case FUSED_A: return launch_pipe_kernel<T, ORDER, FUSED_A>(c, a, grid);
+    case FUSED_A2:
+      if constexpr (sizeof(T) == 8) return launch_pipe_kernel<T, ORDER, FUSED_A2>(c, a, grid);
+      return cudaErrorInvalidValue;
+    case FUSED_B2:
+      if constexpr (sizeof(T) == 8) return launch_pipe_kernel<T, ORDER, FUSED_B2>(c, a, grid);
+      return cudaErrorInvalidValue;
     default: return launch_pipe_kernel<T, ORDER, FUSED_B>(c, a, grid);
   }
 }
@@ -1102,7 +1113,7 @@ int launch_k1(sledge_ctx* c, int l, int mode, PipeArgs<T>& a) {
   Plan& P = c->plan;
   LevelHost& L = P.lev[l];
   a.boxes = tab<BoxDev>(c, L.off_boxes);
-  const bool fused = (mode == FUSED_A || mode == FUSED_B);
+  const bool fused = (mode == FUSED_A || mode == FUSED_B || mode == FUSED_A2 || mode == FUSED_B2);
   a.tiles = tab<TileDev>(c, fused ? L.off_ftiles : L.off_tiles);
   a.g = P.p.nghost;
   a.ox = P.ox;
@@ -1162,6 +1173,8 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
   // addresses; k_rk_tma (no wrap in a tensor map) stores the periodic images of its results into the star ghost
   // cells of its output instead, so only a state that no such sweep wrote (set_state, average-down) is filled here.
   const bool tma = c->use_tma && L.has_tmaps;
+  // fp64: the "W" form of the two sweeps (k_rk_pipe.cuh FUSED_A2 / FUSED_B2): sweep B differences two fields, not three
+  const bool use_w = sizeof(T) == 8 && c->fused_w;
   const int R = P.p.lap_order;
   const bool wrap = L.periodic_box && (tma ? (L.n[0] >= 2 * R && L.n[1] >= 2 * R && L.n[2] >= 2 * R) : (SLEDGE_K1F_PLANE != 0));
   a.wrap = wrap ? 1 : 0;
@@ -1174,6 +1187,7 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
       vf.on = true;
       vf.ta = t;
       vf.tb = pass == 0 ? t + 0.5 * dt : t + dt;
+      vf.w = use_w && pass == 1;
       return launch_ghosts<T>(c, l, buf, time, true, true, 0, 1, false, vf);
     }
     if (!wrap) return launch_ghosts<T>(c, l, buf, time, true, true);
@@ -1191,22 +1205,28 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
     a.tmap[1] = tmaps(cur, 1);
     a.out_psi[0] = plane_ptr<T>(c, l, cur + 1, 0);
     a.out_pi[0] = plane_ptr<T>(c, l, cur + 1, 1);
-    rc = launch_k1<T>(c, l, FUSED_A, a);
+    rc = launch_k1<T>(c, l, use_w ? FUSED_A2 : FUSED_A, a);
     L.star_ok[(cur + 1) & 3] = tma && wrap;
     return rc;
   }
   rc = ensure_ghosts(cur + 1, t + 0.5 * dt);  // Y's ghosts are still valid from pass 0
   if (rc) return rc;
   a.sten[0] = plane_ptr<T>(c, l, cur + 1, 0);
-  a.sten[1] = plane_ptr<T>(c, l, cur + 1, 1);
-  a.sten[2] = plane_ptr<T>(c, l, cur, 0);
+  a.sten[1] = plane_ptr<T>(c, l, cur + 1, 1);  // Pi_3, or W
   a.tmap[0] = tmaps(cur + 1, 0);
   a.tmap[1] = tmaps(cur + 1, 1);
-  a.tmap[2] = tmaps(cur, 0);
-  a.pnt[0] = plane_ptr<T>(c, l, cur, 1);
+  if (use_w) {
+    a.pnt[0] = plane_ptr<T>(c, l, cur, 0);
+    a.pnt[1] = plane_ptr<T>(c, l, cur, 1);
+    a.wu = (T)(1.0 / dt);
+  } else {
+    a.sten[2] = plane_ptr<T>(c, l, cur, 0);
+    a.tmap[2] = tmaps(cur, 0);
+    a.pnt[0] = plane_ptr<T>(c, l, cur, 1);
+  }
   a.out_psi[0] = plane_ptr<T>(c, l, cur + 2, 0);
   a.out_pi[0] = plane_ptr<T>(c, l, cur + 2, 1);
-  rc = launch_k1<T>(c, l, FUSED_B, a);
+  rc = launch_k1<T>(c, l, use_w ? FUSED_B2 : FUSED_B, a);
   if (rc) return rc;
   L.star_ok[(cur + 2) & 3] = tma && wrap;
   finish_step(L, cur + 2, t, dt);
@@ -1739,6 +1759,8 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   {
     const char* ev = getenv("SLEDGE_K1_TMA");
     c->use_tma = !(ev && ev[0] == '0');
+    const char* ew = getenv("SLEDGE_FUSED_W");
+    c->fused_w = !(ew && ew[0] == '0');
     const char* ep = getenv("SLEDGE_K2_PATCHES");
     c->use_patches = !(ep && ep[0] == '0');
     const char* ef = getenv("SLEDGE_FINE_FUSED");
