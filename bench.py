@@ -397,7 +397,7 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
         stage_bytes_total *= n_stage / expected_stage
     achieved = stage_bytes_total / (ms_stage * 1e-3) / 1e9 if ms_stage > 0 else 0.0
     tr = ncu_traffic(cfg.name, args.flow)
-    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_tma FUSED sweeps on level 0 and, under trilinear interpolation, on the finer levels; k_rk_pipe staged sweeps otherwise; mean over the "
+    roofline = {"bound": "hbm", "kernel": "K1 (k_rk_tma FUSED sweeps -- fp64: the W form FUSED_A2 / FUSED_B2, DESIGN.md section 5 -- on every level that can run them; k_rk_pipe staged sweeps otherwise; mean over the "
                                           "stage launches of a step: 2 sweeps per level-step FUSED, 4 otherwise)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "peak_source": peak_src, "traffic": (tr or {}).get("dram_bytes_per_launch"), "traffic_detail": tr,
