@@ -55,7 +55,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="sledge", choices=["sledge", "reference"])
-    ap.add_argument("--flow", default="fused", choices=["fused", "lean", "classic"])
+    ap.add_argument("--flow", default="fused", choices=["fused", "fused3", "lean", "classic"])
     ap.add_argument("--ko-order", type=int, default=0, choices=[0, 2, 3],
                     help="Kreiss-Oliger dissipation order (Eq.7); 0 = off, as in every BASELINE.json config")
     ap.add_argument("--ko-strength", type=float, default=0.01)
@@ -319,9 +319,9 @@ def measure(args, cfg, dev, world, rank, local, steps, warmup):
         args.flow = "ssprk3"  # three staged sweeps, 8 + 12 + 12 words per cell-step
     if rkn_st:
         args.flow = "rkn"     # stage i: Psi_i (psi_n itself for i = 0), psi_n, Pi_n, f_0..f_{i-1} in; 4 words out
-    if args.gw and args.flow == "fused":
+    if args.gw and args.flow in ("fused", "fused3"):
         args.flow = "lean"    # the source needs psi of every stage state: staged sweeps, plus the auxiliary fields' own
-    if args.ko_order and args.flow == "fused":
+    if args.ko_order and args.flow in ("fused", "fused3"):
         args.flow = "lean"  # with the dissipation term k_psi is not pointwise: every level runs the staged sweeps
     for ib, c, t in initial_fields(cfg, rings, boxes, dev, s.tdtype):
         s.set_state(ib, c, t)

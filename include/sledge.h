@@ -42,7 +42,7 @@ typedef enum {
 } sledge_status;
 
 enum { SLEDGE_F32 = 0, SLEDGE_F64 = 1 };
-enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1, SLEDGE_RK_FUSED = 2 };
+enum { SLEDGE_RK_LEAN = 0, SLEDGE_RK_CLASSIC = 1, SLEDGE_RK_FUSED = 2, SLEDGE_RK_FUSED3 = 3 };
 
 /* Inclusive cell range lo..hi of one box in the index space of `level`; axis order x, y, z. */
 enum { SLEDGE_INTERP_TRILINEAR = 0, SLEDGE_INTERP_QUARTIC = 4 };
@@ -64,7 +64,12 @@ typedef struct {
   int32_t eta_fixed;       /* 1 = Minkowski test variant: eta_s = eta for every stage (R3)         */
   int32_t rk_dataflow;     /* words moved per cell-step (R5): SLEDGE_RK_FUSED 20 (two stages per sweep, on every
                               level; a level falls back to LEAN only with quartic interpolation and nghost = 1),
-                              SLEDGE_RK_LEAN 52, SLEDGE_RK_CLASSIC 64; sledge_level_dataflow tells what runs  */
+                              SLEDGE_RK_LEAN 52, SLEDGE_RK_CLASSIC 64; sledge_level_dataflow tells what runs.
+                              In fp64 SLEDGE_RK_FUSED runs the "W form": the second sweep
+                              recovers Pi of the third stage as (W - 2 psi) / dt, an absolute error of about
+                              2^-53 * 2 |psi| / dt per step (1e-14 for dt = 0.025): SLEDGE_RK_FUSED3 is the same
+                              two-sweep flow without that term (three differenced fields in the second sweep,
+                              ~7 % slower), for very small dt; fp32 always runs it                            */
   double h0;               /* level-0 spacing, Eq.1                                               */
   double lambda;           /* Eq.11 generalised (R2): k_Pi = -(friction/eta) Pi + Lap psi          */
   double a_mass;           /*        - lambda eta^2 psi (psi1^2+psi2^2-1) - a_mass psi             */

@@ -414,7 +414,7 @@ int make_plan(Plan& P, const sledge_params* pp, const sledge_box* boxes, int nbo
   if (p.interp == SLEDGE_INTERP_QUARTIC && p.n_levels > 1 && (p.nghost + 1) / 2 + 2 > p.blocking_factor / 2)
     return fail(nullptr, SLEDGE_EINVAL, "quartic interpolation: ceil(nghost/2) + 2 coarse cells exceed the nesting gap of blocking_factor/2 (L70)");
   if (p.dtype != SLEDGE_F32 && p.dtype != SLEDGE_F64) return fail(nullptr, SLEDGE_EINVAL, "dtype must be SLEDGE_F32 or SLEDGE_F64");
-  if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
+  if (p.rk_dataflow < SLEDGE_RK_LEAN || p.rk_dataflow > SLEDGE_RK_FUSED3) return fail(nullptr, SLEDGE_EINVAL, "bad rk_dataflow");
   if (!(p.h0 > 0)) return fail(nullptr, SLEDGE_EINVAL, "h0 must be positive");
   for (int d = 0; d < 3; ++d) {
     if (p.n0[d] <= 0 || p.n0[d] % bf) return fail(nullptr, SLEDGE_EINVAL, "n0 must be a positive multiple of blocking_factor (L39)");
@@ -1174,7 +1174,7 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
   // cells of its output instead, so only a state that no such sweep wrote (set_state, average-down) is filled here.
   const bool tma = c->use_tma && L.has_tmaps;
   // fp64: the "W" form of the two sweeps (k_rk_pipe.cuh FUSED_A2 / FUSED_B2): sweep B differences two fields, not three
-  const bool use_w = sizeof(T) == 8 && c->fused_w;
+  const bool use_w = sizeof(T) == 8 && c->fused_w && P.p.rk_dataflow == SLEDGE_RK_FUSED;
   const int R = P.p.lap_order;
   const bool wrap = L.periodic_box && (tma ? (L.n[0] >= 2 * R && L.n[1] >= 2 * R && L.n[2] >= 2 * R) : (SLEDGE_K1F_PLANE != 0));
   a.wrap = wrap ? 1 : 0;
@@ -1243,7 +1243,7 @@ inline bool level_is_fused(const Plan& P, int l) {
   // the coarse state interpolated at that stage's time (L72), which the patch fills provide as "velocity" ghosts of
   // Pi (k_ghost.cuh: k_fill_patches for trilinear, k_fill_qparents for quartic interpolation by coarse parent)
   const bool lev_ok = l == 0 || (P.fine_fused && (P.p.interp == SLEDGE_INTERP_TRILINEAR || quartic_by_parent(P.p)) && !P.lev[l].patches.empty());
-  return P.p.rk_dataflow == SLEDGE_RK_FUSED && lev_ok && !ko_on(P.p) && !is_ssprk3(P.p) && !is_rkn(P.p) && !P.p.gw;
+  return (P.p.rk_dataflow == SLEDGE_RK_FUSED || P.p.rk_dataflow == SLEDGE_RK_FUSED3) && lev_ok && !ko_on(P.p) && !is_ssprk3(P.p) && !is_rkn(P.p) && !P.p.gw;
 }
 
 // One SSPRK3 stage (integrator.type 3 / 10, L808; Shu-Osher form) of level l, s = 0, 1, 2:

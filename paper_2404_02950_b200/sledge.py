@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsledge.so")
 
 SLEDGE_F32, SLEDGE_F64 = 0, 1
-SLEDGE_RK_LEAN, SLEDGE_RK_CLASSIC, SLEDGE_RK_FUSED = 0, 1, 2
+SLEDGE_RK_LEAN, SLEDGE_RK_CLASSIC, SLEDGE_RK_FUSED, SLEDGE_RK_FUSED3 = 0, 1, 2, 3
 KIND_STAGE, KIND_GHOST, KIND_TAG, KIND_AVG = 0, 1, 2, 3
 COUNT_BLOCK = 32
 
@@ -107,7 +107,8 @@ def _marshal(n0, boxes, n_levels, nghost, blocking_factor, dtype, lap_order, h0,
     p.dtype = {"f32": SLEDGE_F32, "f64": SLEDGE_F64}[dtype]
     p.lap_order = lap_order
     p.eta_fixed = 1 if eta_fixed else 0
-    p.rk_dataflow = {"lean": SLEDGE_RK_LEAN, "classic": SLEDGE_RK_CLASSIC, "fused": SLEDGE_RK_FUSED}[rk_dataflow]
+    p.rk_dataflow = {"lean": SLEDGE_RK_LEAN, "classic": SLEDGE_RK_CLASSIC, "fused": SLEDGE_RK_FUSED,
+                     "fused3": SLEDGE_RK_FUSED3}[rk_dataflow]
     p.h0, p.lam, p.a_mass, p.friction = h0, lam, a_mass, friction
     ks = (ko_strength,) * 4 if isinstance(ko_strength, (int, float)) else tuple(ko_strength)
     p.ko_strength[:] = [float(v) for v in ks]

@@ -88,7 +88,7 @@ def test_c1_literal_32cubed_10_steps_with_tags(flow):
     _c1_run(flow, dt=inputs.CONFIGS["C1"].dt, steps=10, literal=True)
 
 
-@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused", "fused3"])
 def test_c1s_stabilised_32cubed_eta_1_to_3p5_with_tags(flow):
     eta = _c1_run(flow, dt=0.0625, steps=40, literal=False)
     assert eta == pytest.approx(3.5)
@@ -109,7 +109,7 @@ def _ragged_boxes():
 
 
 @pytest.mark.parametrize("order,g", [(1, 1), (1, 3), (2, 2), (2, 3), (3, 3), (3, 5)])
-@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused", "fused3"])
 def test_ragged_multibox_fp64(order, g, flow):
     P = _pair()
     n0 = (40, 24, 72)
@@ -572,7 +572,7 @@ def test_tee_tags_inside_rk_step_three_levels():
     assert total > 0
 
 
-@pytest.mark.parametrize("flow", ["lean", "classic", "fused"])
+@pytest.mark.parametrize("flow", ["lean", "classic", "fused", "fused3"])
 @pytest.mark.parametrize("order", [2, 3])
 def test_two_level_subcycled_steps(flow, order):
     P = _pair()
