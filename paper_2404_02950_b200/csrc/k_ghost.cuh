@@ -91,6 +91,14 @@ struct GhostArgs {
   int vel;  // 1: velocity ghosts; 2: the second plane holds W = psi_Y + psi(U4) (FUSED_A2 / FUSED_B2 sweeps, fill before
             // sweep B): W_g = I_psi(t) + I_psi(t + dt) = 2 I_psi(t + dt/2) = twice the first plane's ghost value
   T vel_c;  // 1 / (t_new - t_old) of the coarse level
+  // k_fill_patches, vel mode before sweep A: the interpolated ghosts of the NEXT sweep's input buffer (U3) are written
+  // in the same pass -- they depend on coarse data only, and the interpolant is linear in time:
+  // psi2_g = psi_g + half_dt * Pi_g (= I_psi(t + dt/2)); pi2_g = Pi_g (velocity), or 2 psi2_g in the W form (w2 != 0).
+  // The fill before sweep B then moves the same-level copies only (copy_only).  Null: off.
+  P* psi2;
+  P* pi2;
+  T half_dt;
+  int w2;
   int patch_smem_pairs;    // shared-memory pairs per warp and plane (largest coarse region of an interpolation patch)
 };
 
@@ -830,6 +838,12 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
       a.psi[d] = mkpair(s0, s1);
       // velocity ghosts: Pi <- I[psi_new - psi_old] / (t_new - t_old) (0 while the coarse level has one state only)
       if (FILL_PI) a.pi[d] = vel ? (a.vel == 2 ? mkpair(T(2) * s0, T(2) * s1) : mkpair(t0 * a.vel_c, t1 * a.vel_c)) : mkpair(t0, t1);
+      if (FILL_PI && vel && a.psi2) {  // the ghosts of U3 as well (see GhostArgs::psi2)
+        const T v0 = t0 * a.vel_c, v1 = t1 * a.vel_c;
+        const T h0 = fma(a.half_dt, v0, s0), h1 = fma(a.half_dt, v1, s1);
+        a.psi2[d] = mkpair(h0, h1);
+        a.pi2[d] = a.w2 ? mkpair(T(2) * h0, T(2) * h1) : mkpair(v0, v1);
+      }
     }
     return;
   }
@@ -855,7 +869,14 @@ __global__ void __launch_bounds__(PATCH_WARPS * 32, SLEDGE_PATCH_MINB) k_fill_pa
         a.pi[d] = mkpair(T(2) * pv.x, T(2) * pv.y);
       } else if (a.vel) {
         const P dv = interp_coarse_diff<T>(a.c_old_psi, a.c_new_psi, o);
-        a.pi[d] = mkpair(dv.x * a.vel_c, dv.y * a.vel_c);
+        const T v0 = dv.x * a.vel_c, v1 = dv.y * a.vel_c;
+        a.pi[d] = mkpair(v0, v1);
+        if (a.psi2) {
+          const P pv = a.psi[d];  // just written by this thread
+          const T h0 = fma(a.half_dt, v0, pv.x), h1 = fma(a.half_dt, v1, pv.y);
+          a.psi2[d] = mkpair(h0, h1);
+          a.pi2[d] = a.w2 ? mkpair(T(2) * h0, T(2) * h1) : mkpair(v0, v1);
+        }
       } else {
         a.pi[d] = interp_coarse<T>(a.c_old_pi, a.c_new_pi, a.alpha, o);
       }

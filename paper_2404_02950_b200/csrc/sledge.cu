@@ -142,6 +142,7 @@ struct LevelHost {
   size_t off_star_list = 0, off_star_count = 0;
   std::vector<uint4> patches, tag_patches;  // star patches / tag patches (k_fill_patches), 2 x uint4 each
   size_t off_patches = 0, off_tag_patches = 0;
+  unsigned n_copy_patches = 0;  // the star patch list is sorted: same-level copies first (a copies-only fill launches just those)
   int patch_smem_pairs = 0;    // largest coarse region of an interpolation patch (pairs)
   size_t off_tmaps = 0;        // k_rk_tma: CUtensorMap[NBUF * 2][nbox] of the level's state planes (fused levels only)
   bool has_tmaps = false;
@@ -201,6 +202,7 @@ struct sledge_ctx {
   int64_t launches = 0;
   bool profiling = false;
   bool use_tma = true;  // FUSED sweeps through k_rk_tma (SLEDGE_K1_TMA=0 in the environment selects k_rk_plane)
+  bool fill_once = true;  // fine FUSED levels, trilinear: interpolated ghosts of both sweeps in one fill (SLEDGE_FILL_ONCE=0: two)
   bool fused_w = true;  // fp64 FUSED sweeps in the W form (SLEDGE_FUSED_W=0 selects the three-field sweep B)
   bool use_patches = true;  // fills before an RK sweep by region (SLEDGE_K2_PATCHES=0 selects the packed per-cell list)
   sledge_ctx* shadow = nullptr;  // the shadow level's context (shadow_level = 1)
@@ -367,6 +369,17 @@ void plan_patches(Plan& P, int l, bool tagset) {
               out.push_back(A);
               out.push_back(B);
             }
+    }
+  }
+  if (!tagset) {  // same-level copies first
+    struct Pair { uint4 A, B; };
+    std::vector<Pair> ps(out.size() / 2);
+    for (size_t q = 0; q < ps.size(); ++q) ps[q] = Pair{out[2 * q], out[2 * q + 1]};
+    const auto mid = std::stable_partition(ps.begin(), ps.end(), [](const Pair& e) { return (e.B.x >> 24) == (unsigned)PATCH_COPY; });
+    L.n_copy_patches = (unsigned)(mid - ps.begin());
+    for (size_t q = 0; q < ps.size(); ++q) {
+      out[2 * q] = ps[q].A;
+      out[2 * q + 1] = ps[q].B;
     }
   }
 }
@@ -785,6 +798,10 @@ LevelGeom geom_of(const Plan& P, int l) {
 struct VelFill {  // velocity ghosts of the second plane between the times ta and tb (FUSED sweeps on a fine level)
   bool on = false;
   bool w = false;  // the second plane holds W (FUSED_B2): ghost = twice the first plane's
+  int buf2 = -1;   // before sweep A: also write the interpolated ghosts of this buffer (U3), see GhostArgs::psi2
+  bool w2 = false;
+  double half_dt = 0;
+  bool copies_only = false;  // before sweep B: the interpolated ghosts are there already
   double ta = 0, tb = 0;
 };
 
@@ -842,6 +859,12 @@ GhostArgs<T> ghost_args(sledge_ctx* c, int l, int buf, double time, int wa = 0, 
       bn = C.cur;
       a.single = 0;
       a.vel = vf.w ? 2 : 1;
+      if (vf.buf2 >= 0) {
+        a.psi2 = plane_ptr<T>(c, l, vf.buf2, wa);
+        a.pi2 = plane_ptr<T>(c, l, vf.buf2, wb);
+        a.half_dt = (T)vf.half_dt;
+        a.w2 = vf.w2 ? 1 : 0;
+      }
       a.vel_c = (T)(pair ? 1.0 / (C.t_new - C.t_old) : 0.0);
     }
     a.c_old_psi = plane_ptr<T>(c, l - 1, bo, wa);
@@ -892,23 +915,28 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     if (rc) return rc;
   }
   if (by_patch) {  // by rectangular region (k_fill_patches)
-    if (a.quartic == 2) a.copy_only = 1;
-    const int pgrid = (int)((a.n_patches + PATCH_WARPS - 1) / PATCH_WARPS);
-    const size_t smem = (size_t)PATCH_WARPS * a.patch_smem_pairs * (fill_pi ? 2 : 1) * sizeof(typename PairOf<T>::type);
-    if (smem > 48 * 1024) {
-      static PerDevice configured2[2];  // per instantiation and device
-      bool& cfg = configured2[fill_pi][c->device];
-      if (!cfg) {
-        if (fill_pi) cudaFuncSetAttribute(k_fill_patches<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        else cudaFuncSetAttribute(k_fill_patches<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cfg = true;
+    if (a.quartic == 2 || vf.copies_only) a.copy_only = 1;
+    if (a.copy_only && !tagp) a.n_patches = c->plan.lev[l].n_copy_patches;  // sorted: the copies come first
+    if (a.n_patches > 0) {
+      const int pgrid = (int)((a.n_patches + PATCH_WARPS - 1) / PATCH_WARPS);
+      // the shared-memory region stages the coarse cells of an interpolation patch: none in a copies-only launch
+      const size_t smem = a.copy_only ? 0 : (size_t)PATCH_WARPS * a.patch_smem_pairs * (fill_pi ? 2 : 1) * sizeof(typename PairOf<T>::type);
+      if (smem > 48 * 1024) {
+        static PerDevice configured2[2];  // per instantiation and device
+        bool& cfg = configured2[fill_pi][c->device];
+        if (!cfg) {
+          if (fill_pi) cudaFuncSetAttribute(k_fill_patches<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+          else cudaFuncSetAttribute(k_fill_patches<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+          cfg = true;
+        }
       }
+      Timed t(c, KIND_GHOST);
+      if (fill_pi) k_fill_patches<T, true><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
+      else k_fill_patches<T, false><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
+      const int prc = check_launch(c, "k_fill_patches");
+      if (prc) return prc;
     }
-    Timed t(c, KIND_GHOST);
-    if (fill_pi) k_fill_patches<T, true><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
-    else k_fill_patches<T, false><<<pgrid, PATCH_WARPS * 32, smem, c->stream>>>(a);
-    const int prc = check_launch(c, "k_fill_patches");
-    if (prc || a.quartic == 0) return prc;
+    if (a.quartic == 0) return SLEDGE_OK;
     a.copy_only = 0;
   }
   int grid = (c->plan.lev[l].ghost_prefix.back() + GHOST_EPT - 1) / GHOST_EPT;
@@ -1188,6 +1216,17 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
       vf.ta = t;
       vf.tb = pass == 0 ? t + 0.5 * dt : t + dt;
       vf.w = use_w && pass == 1;
+      // trilinear interpolation: the fill before sweep A writes the interpolated ghosts of U3 too (they depend on the
+      // coarse level only), the fill before sweep B moves the same-level copies only
+      if (P.p.interp == SLEDGE_INTERP_TRILINEAR && c->fill_once) {
+        if (pass == 0) {
+          vf.buf2 = cur + 1;
+          vf.w2 = use_w;
+          vf.half_dt = 0.5 * dt;
+        } else {
+          vf.copies_only = true;
+        }
+      }
       return launch_ghosts<T>(c, l, buf, time, true, true, 0, 1, false, vf);
     }
     if (!wrap) return launch_ghosts<T>(c, l, buf, time, true, true);
@@ -1759,6 +1798,8 @@ int sledge_create(sledge_ctx** out, const sledge_params* params, const sledge_bo
   {
     const char* ev = getenv("SLEDGE_K1_TMA");
     c->use_tma = !(ev && ev[0] == '0');
+    const char* eo = getenv("SLEDGE_FILL_ONCE");
+    c->fill_once = !(eo && eo[0] == '0');
     const char* ew = getenv("SLEDGE_FUSED_W");
     c->fused_w = !(ew && ew[0] == '0');
     const char* ep = getenv("SLEDGE_K2_PATCHES");
