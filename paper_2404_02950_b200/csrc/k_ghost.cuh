@@ -684,6 +684,11 @@ __global__ void __launch_bounds__(QP_THREADS, SLEDGE_QP_MINB) k_fill_qparents(co
       const unsigned dst = ea.x + (unsigned)(c >> 2) * fpl + (unsigned)((c >> 1) & 1) * fsx + (unsigned)(c & 1);
       a.psi[dst] = mkpair(s[c][0], s[c][1]);
       if (FILL_PI) a.pi[dst] = mkpair(p[c][0], p[c][1]);
+      if (VEL && a.psi2 && a.vel == 1) {  // the ghosts of the next sweep's input buffer as well (GhostArgs::psi2)
+        const T h0 = fma(a.half_dt, p[c][0], s[c][0]), h1 = fma(a.half_dt, p[c][1], s[c][1]);
+        a.psi2[dst] = mkpair(h0, h1);
+        a.pi2[dst] = a.w2 ? mkpair(T(2) * h0, T(2) * h1) : mkpair(p[c][0], p[c][1]);
+      }
     }
 }
 

@@ -907,7 +907,7 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     a.n_patches = (unsigned)(c->plan.lev[l].tag_patches.size() / 2);
   }
   const bool by_patch = patchable && a.n_patches > 0 && (star_only || tagp);
-  if (a.quartic == 2 && l > 0) {  // the coarse windows are read through the coarse boxes' ghost cells
+  if (a.quartic == 2 && l > 0 && !vf.copies_only) {  // the coarse windows are read through the coarse boxes' ghost cells
     LevelHost& C = c->plan.lev[l - 1];
     const bool pair = C.have_pair && C.t_new != C.t_old;
     int rc = fill_shell_copies<T>(c, l - 1, C.cur, fill_pi);
@@ -964,7 +964,7 @@ int launch_ghosts(sledge_ctx* c, int l, int buf, double time, bool fill_pi, bool
     a.qlist = a.qstar_list;
     a.n_qentries = c->plan.lev[l].n_star_parents;
   }
-  if (a.quartic == 2 && l > 0 && qgrid > 0) {  // the interpolated cells, one thread per coarse parent
+  if (a.quartic == 2 && l > 0 && qgrid > 0 && !vf.copies_only) {  // the interpolated cells, one thread per coarse parent
     qgrid = (int)((a.n_qentries + QP_THREADS - 1) / QP_THREADS);
     Timed t(c, KIND_GHOST);
     if (a.single) {
@@ -1216,9 +1216,9 @@ int do_fused_pass(sledge_ctx* c, int l, int pass, double t, double dt, double et
       vf.ta = t;
       vf.tb = pass == 0 ? t + 0.5 * dt : t + dt;
       vf.w = use_w && pass == 1;
-      // trilinear interpolation: the fill before sweep A writes the interpolated ghosts of U3 too (they depend on the
-      // coarse level only), the fill before sweep B moves the same-level copies only
-      if (P.p.interp == SLEDGE_INTERP_TRILINEAR && c->fill_once) {
+      // the fill before sweep A writes the interpolated ghosts of U3 too (they depend on the coarse level only), the
+      // fill before sweep B moves the same-level copies only
+      if ((P.p.interp == SLEDGE_INTERP_TRILINEAR || quartic_by_parent(P.p)) && c->fill_once) {
         if (pass == 0) {
           vf.buf2 = cur + 1;
           vf.w2 = use_w;
