@@ -71,6 +71,34 @@ def test_coalescing_removes_the_ghost_cells_between_boxes(monkeypatch):
     assert apart > merged
 
 
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_random_hierarchies_validate_and_coalescing_never_costs_memory(monkeypatch, seed):
+    """host logic only (no GPU): the seeded random hierarchies of the GPU parity tests pass the library's validation
+    (alignment, disjointness, level 0 covering the domain, proper nesting: L39, L70, L137) with and without the
+    storage-box coalescing, in any merge order, and merged storage never needs more arena than separate boxes"""
+    for n0, bf, nl, g in (((32, 24, 40), 8, 3, 3), ((16, 16, 16), 4, 3, 2), ((16, 24, 16), 2, 2, 1)):
+        boxes = inputs.random_hierarchy(n0, nl, bf, 100 * seed + bf + nl)
+        kw = dict(boxes=boxes, n_levels=nl, nghost=g, blocking_factor=bf, lap_order=min(g, 2))
+        sizes = {}
+        for mode in ("0", None, "zyx", "yxz"):
+            if mode is None:
+                monkeypatch.delenv("SLEDGE_COALESCE", raising=False)
+            else:
+                monkeypatch.setenv("SLEDGE_COALESCE", mode)
+            sizes[mode] = S.sledge_arena_bytes(n0, **kw)
+        assert all(sizes[m] <= sizes["0"] for m in (None, "zyx", "yxz")), sizes
+        # a box list that violates nesting is still rejected when boxes are merged: drop a level-1 box under a level-2 one
+        if nl == 3:
+            monkeypatch.delenv("SLEDGE_COALESCE", raising=False)
+            l2 = [b for b in boxes if b[0] == 2]
+            if l2:
+                lo = tuple(v // 2 for v in l2[0][1])
+                bad = [b for b in boxes if not (b[0] == 1 and all(b[1][d] <= lo[d] <= b[2][d] for d in range(3)))]
+                if len(bad) < len(boxes):
+                    with pytest.raises(S.SledgeError):
+                        S.sledge_arena_bytes(n0, **dict(kw, boxes=bad))
+
+
 RKN4 = dict(nodes=[0.0, 0.5, 1.0], weights_b=[1 / 6, 4 / 6, 1 / 6], weights_bar_b=[1 / 6, 1 / 3, 0.0],
             tableau=[0.0, 1 / 8, 0.0, 0.0, 0.5, 0.0])
 
